@@ -1,0 +1,272 @@
+"""Pins for oracle/nn_oracle.py (CPU only).  Every check here compares the oracle
+with something the paper or the mathematics fixes independently of it:
+exact piecewise-linear enumeration, sampled/vertex soundness (Thm 2/3,
+PAPER.md:L196-214), the closed-form box maximum of an affine map,
+validity of each scalar relaxation on a dense grid, and central differences."""
+import itertools
+
+import numpy as np
+import pytest
+
+from oracle import nn_oracle as O
+
+
+def _net(rng, dims, scale=1.0):
+    Ws = [rng.standard_normal((dims[i + 1], dims[i])) * scale * np.sqrt(2.0 / (dims[i] + dims[i + 1]))
+          for i in range(len(dims) - 1)]
+    bs = [rng.uniform(-0.1, 0.1, dims[i + 1]) for i in range(len(dims) - 1)]
+    return Ws, bs
+
+
+def _true_r(Ws, bs, act, a0, X):
+    zs, p, J = O.nominal(Ws, bs, act, a0)
+    return np.array([O.mlp_eval(Ws, bs, act, x) - p - J @ (x - a0) for x in X])
+
+
+def _vertices(a0, sig):
+    return np.array([a0 + sig * np.array(s) for s in itertools.product((-1.0, 1.0), repeat=len(a0))])
+
+
+# ---------------------------------------------------------------- relaxations
+@pytest.mark.parametrize("seed", range(3))
+def test_tanh_relaxation_valid_and_touching(seed):
+    rng = np.random.default_rng(seed)
+    for _ in range(200):
+        l = rng.uniform(-3, 3)
+        u = l + rng.uniform(1e-3, 4)
+        kU, bU, kL, bL, aux = O.relax_tanh_scalar(l, u)
+        z = np.linspace(l, u, 2001)
+        up = kU * z + bU - np.tanh(z)
+        lo = np.tanh(z) - (kL * z + bL)
+        assert up.min() >= -1e-12 and lo.min() >= -1e-12, (l, u, aux)
+        # each line touches the curve somewhere on [l,u] (it is a tangent or a chord)
+        assert up.min() <= 1e-6 and lo.min() <= 1e-6, (l, u, aux)
+
+
+def test_relu_relaxation_cases():
+    assert O.relax_relu_scalar(-2.0, -1.0)[:4] == (0.0, 0.0, 0.0, 0.0)
+    assert O.relax_relu_scalar(0.5, 1.0)[:4] == (1.0, 0.0, 1.0, 0.0)
+    kU, bU, kL, bL, _ = O.relax_relu_scalar(-1.0, 3.0)
+    assert np.isclose(kU, 0.75) and np.isclose(bU, 0.75) and kL == 1.0 and bL == 0.0
+    assert O.relax_relu_scalar(-3.0, 1.0)[2] == 0.0
+    assert O.relax_relu_scalar(-1.0, 1.0)[2] == 0.0          # tie -> 0
+    for l, u in [(-1.0, 3.0), (-3.0, 1.0), (-1.0, 1.0)]:
+        kU, bU, kL, bL, _ = O.relax_relu_scalar(l, u)
+        z = np.linspace(l, u, 1001)
+        assert (kU * z + bU - np.maximum(z, 0) >= -1e-15).all()
+        assert (np.maximum(z, 0) - kL * z - bL >= -1e-15).all()
+
+
+# ---------------------------------------------------------------- zero cases
+def test_stable_relu_network_gives_zero_bound():
+    # large positive/negative biases => every neuron stable on the box => p is affine
+    rng = np.random.default_rng(1)
+    Ws, bs = _net(rng, [5, 8, 8, 3])
+    bs[0] = np.where(rng.random(8) < 0.5, 50.0, -50.0)
+    bs[1] = np.where(rng.random(8) < 0.5, 50.0, -50.0)
+    a0 = rng.standard_normal(5)
+    sig = rng.uniform(0.1, 0.5, 5)
+    out = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig)
+    assert np.abs(out["r_lo"]).max() < 1e-12 and np.abs(out["r_hi"]).max() < 1e-12
+
+
+@pytest.mark.parametrize("act", [O.ACT_RELU, O.ACT_TANH])
+def test_zero_radius_gives_zero_bound(act):
+    rng = np.random.default_rng(2)
+    Ws, bs = _net(rng, [4, 9, 7, 3])
+    a0 = rng.standard_normal(4)
+    out = O.crown_forward(Ws, bs, act, a0, np.zeros(4))
+    assert np.abs(out["r_lo"]).max() < 1e-12 and np.abs(out["r_hi"]).max() < 1e-12
+
+
+def test_tanh_bound_shrinks_quadratically():
+    rng = np.random.default_rng(3)
+    Ws, bs = _net(rng, [4, 9, 7, 3])
+    a0 = rng.standard_normal(4)
+    sig = rng.uniform(0.5, 1.0, 4)
+    w1 = O.crown_forward(Ws, bs, O.ACT_TANH, a0, 1e-3 * sig)
+    w2 = O.crown_forward(Ws, bs, O.ACT_TANH, a0, 2e-3 * sig)
+    ratio = (w2["r_hi"] - w2["r_lo"]) / (w1["r_hi"] - w1["r_lo"])
+    assert np.all(np.abs(ratio - 4.0) < 0.05), ratio
+
+
+# ---------------------------------------------------------------- exact enumeration
+def _exact_range_1hidden_relu(Ws, bs, a0, sig):
+    """r is piecewise linear: its extrema over the box are attained at vertices of
+    the arrangement {neuron hyperplanes} u {box faces}.  Enumerate them all."""
+    d = len(a0)
+    W1, b1 = Ws[0], bs[0]
+    planes = [(W1[k], -b1[k]) for k in range(W1.shape[0])]
+    for i in range(d):
+        e = np.zeros(d)
+        e[i] = 1.0
+        planes.append((e, a0[i] - sig[i]))
+        planes.append((e, a0[i] + sig[i]))
+    pts = []
+    for combo in itertools.combinations(range(len(planes)), d):
+        A = np.array([planes[c][0] for c in combo])
+        rhs = np.array([planes[c][1] for c in combo])
+        if abs(np.linalg.det(A)) < 1e-12:
+            continue
+        x = np.linalg.solve(A, rhs)
+        if np.all(np.abs(x - a0) <= sig + 1e-12):
+            pts.append(np.clip(x, a0 - sig, a0 + sig))
+    R = _true_r(Ws, bs, O.ACT_RELU, a0, np.array(pts))
+    return R.min(0), R.max(0)
+
+
+@pytest.mark.parametrize("d,H,seed", [(1, 4, 0), (2, 5, 1), (3, 5, 2), (4, 4, 3)])
+def test_encloses_exact_range_1hidden_relu(d, H, seed):
+    rng = np.random.default_rng(100 + seed)
+    Ws, bs = _net(rng, [d, H, 3], scale=2.0)
+    a0 = rng.standard_normal(d) * 0.3
+    sig = rng.uniform(0.2, 0.6, d)
+    lo, hi = _exact_range_1hidden_relu(Ws, bs, a0, sig)
+    out = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig)
+    assert np.all(out["r_lo"] <= lo + 1e-12) and np.all(out["r_hi"] >= hi - 1e-12)
+    # not vacuous: within a small factor of the exact width on these tiny nets
+    assert np.all((out["r_hi"] - out["r_lo"]) <= 6.0 * (hi - lo) + 1e-9)
+
+
+def test_exact_when_single_unstable_neuron_1d():
+    # 1-D input, one unstable neuron with output weight w: the chord touches the
+    # ReLU at both interval ends, so the side that uses the chord is exact.
+    W1 = np.array([[1.0], [1.0]])
+    b1 = np.array([0.2, 5.0])              # neuron 0 unstable on [-1,1], neuron 1 stable-on
+    for w in (+1.5, -0.7):
+        Ws = [W1, np.array([[w, 0.3]])]
+        bs = [b1, np.array([0.1])]
+        a0, sig = np.array([0.1]), np.array([1.0])
+        lo, hi = _exact_range_1hidden_relu(Ws, bs, a0, sig)
+        out = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig)
+        if w > 0:
+            assert np.isclose(out["r_hi"][0], hi[0], atol=1e-12)
+            assert out["r_lo"][0] <= lo[0] + 1e-12
+        else:
+            assert np.isclose(out["r_lo"][0], lo[0], atol=1e-12)
+            assert out["r_hi"][0] >= hi[0] - 1e-12
+
+
+# ---------------------------------------------------------------- soundness
+@pytest.mark.parametrize("act,dims,seed", [(O.ACT_RELU, [6, 12, 12, 12, 4], 0), (O.ACT_TANH, [6, 12, 12, 12, 4], 1),
+                                           (O.ACT_TANH, [5, 16, 16, 16, 16, 3], 2), (O.ACT_RELU, [8, 10, 10, 5], 3)])
+def test_soundness_samples_vertices_hidden(act, dims, seed):
+    rng = np.random.default_rng(200 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    a0 = rng.standard_normal(dims[0])
+    sig = rng.uniform(0.05, 0.3, dims[0])
+    out = O.crown_forward(Ws, bs, act, a0, sig)
+    X = np.concatenate([a0 + sig * rng.uniform(-1, 1, (100000 // 4, dims[0])), _vertices(a0, sig)])
+    R = _true_r(Ws, bs, act, a0, X)
+    assert np.all(R.min(0) >= out["r_lo"] - 1e-12) and np.all(R.max(0) <= out["r_hi"] + 1e-12)
+    for x in X[::97]:
+        for z, l, u in zip(O.mlp_hidden(Ws, bs, act, x), out["ls"], out["us"]):
+            assert np.all(z >= l - 1e-12) and np.all(z <= u + 1e-12)
+    # Thm 2 itself: W_lo a + b_lo <= p(a) <= W_up a + b_up
+    for x in X[::53]:
+        p = O.mlp_eval(Ws, bs, act, x)
+        assert np.all(out["W_lo"] @ x + out["b_lo"] <= p + 1e-12)
+        assert np.all(out["W_up"] @ x + out["b_up"] >= p - 1e-12)
+
+
+def test_concretisation_is_box_max_of_eq20():
+    # (21): r_hi_i = max over the box of the affine r_up(a) of (20); brute force on vertices
+    rng = np.random.default_rng(5)
+    Ws, bs = _net(rng, [5, 9, 9, 4], scale=1.5)
+    a0 = rng.standard_normal(5)
+    sig = rng.uniform(0.05, 0.3, 5)
+    out = O.crown_forward(Ws, bs, O.ACT_TANH, a0, sig)
+    V = _vertices(a0, sig)
+    J, p = out["J"], out["p"]
+    up = np.array([(out["W_up"] - J) @ v + J @ a0 - p + out["b_up"] for v in V]).max(0)
+    lo = np.array([(out["W_lo"] - J) @ v + J @ a0 - p + out["b_lo"] for v in V]).min(0)
+    assert np.allclose(up, out["r_hi"], rtol=0, atol=1e-12)
+    assert np.allclose(lo, out["r_lo"], rtol=0, atol=1e-12)
+
+
+def test_jacobian_matches_finite_differences():
+    rng = np.random.default_rng(6)
+    Ws, bs = _net(rng, [5, 9, 9, 4])
+    a0 = rng.standard_normal(5)
+    _, _, J = O.nominal(Ws, bs, O.ACT_TANH, a0)
+    h = 1e-6
+    Jfd = np.array([(O.mlp_eval(Ws, bs, O.ACT_TANH, a0 + h * e) - O.mlp_eval(Ws, bs, O.ACT_TANH, a0 - h * e)) / (2 * h)
+                    for e in np.eye(5)]).T
+    assert np.allclose(J, Jfd, atol=1e-8)
+
+
+def test_given_jacobian_is_used():
+    # Thm 3 holds for any J: with J' = J + E the bound must enclose r computed with J'
+    rng = np.random.default_rng(7)
+    Ws, bs = _net(rng, [4, 8, 8, 3])
+    a0 = rng.standard_normal(4)
+    sig = rng.uniform(0.05, 0.2, 4)
+    _, p, J = O.nominal(Ws, bs, O.ACT_TANH, a0)
+    J2 = J + 0.1 * rng.standard_normal(J.shape)
+    out = O.crown_forward(Ws, bs, O.ACT_TANH, a0, sig, J_given=J2)
+    X = np.concatenate([a0 + sig * rng.uniform(-1, 1, (5000, 4)), _vertices(a0, sig)])
+    R = np.array([O.mlp_eval(Ws, bs, O.ACT_TANH, x) - p - J2 @ (x - a0) for x in X])
+    assert np.all(R.min(0) >= out["r_lo"] - 1e-12) and np.all(R.max(0) <= out["r_hi"] + 1e-12)
+
+
+# ---------------------------------------------------------------- VJP
+def _fd_grad(Ws, bs, act, a0, sig, g_lo, g_hi, h=1e-6):
+    def F(a, s):
+        f = O.crown_forward(Ws, bs, act, a, s)
+        return g_hi @ f["r_hi"] + g_lo @ f["r_lo"]
+    N = len(a0)
+    gn, gr, ok_n, ok_r = np.zeros(N), np.zeros(N), np.ones(N, bool), np.ones(N, bool)
+    F0 = F(a0, sig)
+    for i in range(N):
+        e = np.zeros(N)
+        e[i] = h * max(1.0, abs(a0[i]))
+        fp, fm = F(a0 + e, sig), F(a0 - e, sig)
+        gn[i] = (fp - fm) / (2 * e[i])
+        ok_n[i] = abs((fp - F0) - (F0 - fm)) <= 1e-3 * abs(fp - fm) + 1e-12      # kink filter
+        e[i] = h * max(1.0, abs(sig[i]))
+        fp, fm = F(a0, sig + e), F(a0, sig - e)
+        gr[i] = (fp - fm) / (2 * e[i])
+        ok_r[i] = abs((fp - F0) - (F0 - fm)) <= 1e-3 * abs(fp - fm) + 1e-12
+    return gn, gr, ok_n, ok_r
+
+
+@pytest.mark.parametrize("act,dims,seed", [(O.ACT_RELU, [6, 10, 10, 10, 4], 0), (O.ACT_TANH, [6, 10, 10, 10, 4], 1),
+                                           (O.ACT_TANH, [3, 7, 5, 2], 2), (O.ACT_TANH, [5, 8, 8, 8, 8, 3], 3),
+                                           (O.ACT_RELU, [4, 9, 9, 3], 4)])
+def test_vjp_matches_central_differences(act, dims, seed):
+    rng = np.random.default_rng(300 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    a0 = rng.standard_normal(dims[0])
+    sig = rng.uniform(0.05, 0.3, dims[0])
+    g_lo, g_hi = rng.standard_normal(dims[-1]), rng.standard_normal(dims[-1])
+    gn, gr = O.crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi)
+    fn, fr, ok_n, ok_r = _fd_grad(Ws, bs, act, a0, sig, g_lo, g_hi)
+    assert ok_n.sum() + ok_r.sum() >= dims[0]            # most points are not at a kink
+    scale = max(np.abs(fn).max(), np.abs(fr).max())
+    assert np.all(np.abs(gn - fn)[ok_n] <= 1e-6 * scale + 1e-5 * np.abs(fn)[ok_n])
+    assert np.all(np.abs(gr - fr)[ok_r] <= 1e-6 * scale + 1e-5 * np.abs(fr)[ok_r])
+
+
+def test_vjp_random_directions_config3_shape():
+    # config-3 architecture (24 -> 128x3 -> 20, ReLU); directional derivatives
+    from paper_2607_01203_b200 import workloads as wl
+    w = wl.make_config(3, B=1, T=2)
+    Ws = [W.astype(np.float64) for W in w.mlp.W]
+    bs = [b.astype(np.float64) for b in w.mlp.b]
+    rng = np.random.default_rng(9)
+    a0, sig = w.nom[0, 0].astype(np.float64), w.rad[0, 0].astype(np.float64)
+    g_lo, g_hi = w.g_lo[0, 0].astype(np.float64), w.g_hi[0, 0].astype(np.float64)
+    gn, gr = O.crown_vjp(Ws, bs, O.ACT_RELU, a0, sig, g_lo, g_hi)
+
+    def F(a, s):
+        f = O.crown_forward(Ws, bs, O.ACT_RELU, a, s)
+        return g_hi @ f["r_hi"] + g_lo @ f["r_lo"]
+    h, good = 1e-7, 0
+    for _ in range(32):
+        dn, dr = rng.standard_normal(24), rng.standard_normal(24)
+        F0, fp, fm = F(a0, sig), F(a0 + h * dn, sig + h * dr), F(a0 - h * dn, sig - h * dr)
+        if abs((fp - F0) - (F0 - fm)) > 1e-3 * abs(fp - fm):
+            continue                                     # crossed a ReLU switch
+        good += 1
+        assert np.isclose((fp - fm) / (2 * h), gn @ dn + gr @ dr, rtol=1e-5, atol=1e-7)
+    assert good >= 16
