@@ -1,0 +1,170 @@
+/* leb.h -- C ABI of the B200-native linearization-error-bound (LEB) library.
+ *
+ * What the library computes (arxiv/paper_2607_01203, "GPUSLS-LEO"; citations are
+ * PAPER.md line numbers): for every trajectory b, timestep t (a "tile") and state
+ * dimension i, a sound enclosure [r_lo, r_hi] of the linearization remainder
+ *
+ *     r_i(a) = f_i(a) - f_i(a~) - J(a~)(a - a~),   a = [x; u] in the tube box A_t     (10) L133
+ *
+ * where A_t = [a~ - sigma, a~ + sigma] is the centred tube box ((25a) L272 with mu = 0),
+ *   - for analytic dynamics by the path-based interval-Hessian bound, Thm 1 eq. (15);
+ *   - for MLP dynamics by CROWN affine relaxations (Thm 2, eq. (18)) followed by the
+ *     local Jacobian correction and box concretisation of Thm 3, eq. (19)-(21) L204-220;
+ * the vector-Jacobian product of those bounds with respect to the nominal point a~ and the
+ * radii sigma (differentiability, Sec. IV-D; consumed by J_err (35) L358-362); and the
+ * fold of the per-dimension bounds into the non-zero-centred disturbance zonotope
+ * (c_bar, R_bar), Sec. IV-C, eq. (25b,c) L274-281, diagonal padding L347.
+ *
+ * Conventions (all entry points):
+ *   - extern "C", no exceptions cross the boundary, every call returns a leb_status.
+ *   - Data pointers are DEVICE pointers owned by the caller unless the call is given
+ *     LEB_FLAG_HOST_IO, in which case they are HOST pointers (pinned memory recommended) and the
+ *     library stages them through its own device buffers (H2D before, D2H after, same stream).
+ *     The library never frees caller memory and keeps no caller pointer after the call returns
+ *     (leb_set_mlp copies and re-packs the weights into memory the context owns).
+ *   - Calls are asynchronous on the caller's stream (`stream` is a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  Argument / shape errors are reported
+ *     synchronously; CUDA launch errors surface as LEB_ERR_CUDA.
+ *   - All arrays are FP32, row-major.  Trajectory arrays are [B, T, ld] with the row stride
+ *     `ld_in` (>= N = n + m) or `ld_out` (>= n) given in floats; tile (b, t) is row b*T + t.
+ *     Augmented-state order is a = [x; u] (state first, L131); this fixes the path order of (15).
+ *   - A tile whose inputs are outside the method's domain (NaN/Inf input, sigma < 0, or an
+ *     analytic box on which cos(theta) contains 0, so 1/cos is unbounded) gets r_lo = -inf,
+ *     r_hi = +inf for all its dimensions and raises the context's domain flag, readable after
+ *     synchronising the stream with leb_domain_flag().  A finite bound is never silently wrong.
+ *   - There is no CPU fallback: every numerical step runs in the library's sm_100a kernels.
+ */
+#ifndef LEB_H_
+#define LEB_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct leb_ctx leb_ctx; /* opaque: packed weights, workspace, staging buffers, flags */
+
+typedef enum {
+    LEB_OK = 0,
+    LEB_ERR_ARG = 1,         /* NULL pointer, negative size, unknown enum value */
+    LEB_ERR_SHAPE = 2,       /* ld too small, model/shape mismatch */
+    LEB_ERR_ALIGN = 3,       /* pointer not 4-byte aligned */
+    LEB_ERR_DOMAIN = 4,      /* reported by leb_domain_flag(): some tile hit a domain error */
+    LEB_ERR_UNSUPPORTED = 5, /* mu != NULL (non-centred boxes: SURVEY 8(f).1), unknown model */
+    LEB_ERR_CUDA = 6,
+    LEB_ERR_NOMEM = 7,
+    LEB_ERR_STATE = 8        /* model not set before the call that needs it */
+} leb_status;
+
+typedef enum { LEB_MODEL_UNICYCLE = 1, LEB_MODEL_QUAD12 = 2, LEB_MODEL_QUADCHAIN = 3 } leb_model_id;
+typedef enum { LEB_INTEG_EULER = 1, LEB_INTEG_RK4 = 2 } leb_integ;
+typedef enum { LEB_ACT_RELU = 1, LEB_ACT_TANH = 2 } leb_act;
+
+/* Analytic dynamics.
+ *   UNICYCLE : a = (px, py, th, v, om); f = (px + dt v cos th, py + dt v sin th, th + dt om).
+ *   QUAD12   : xi = (p[3], (phi, theta, psi), v[3], (p, q, r)) -- state order of L538 --,
+ *              nu = (T, tau[3]); ZYX rigid-body vector field (eq. (38), de-garbled).
+ *   QUADCHAIN: n_units copies of QUAD12, x = (xi_1..xi_U), u = (nu_1..nu_U) ((39) L540-543),
+ *              neighbours joined per axis by the spring k1 d + k3 d^3 (BASELINE config 4).
+ * integ = EULER: f = x + dt g(x,u) (the paper's choice, L505); RK4: classical 4 stages, u held. */
+typedef struct {
+    int model_id; /* leb_model_id */
+    int integ;    /* leb_integ (UNICYCLE is always Euler) */
+    int n_units;  /* QUADCHAIN: number of quadrotors (config 4: 14); otherwise 1 */
+    float dt, mass, g, Jx, Jy, Jz, k1, k3;
+} leb_analytic_model;
+
+/* MLP dynamics f(x,u) = x + g(x,u) if residual else g(x,u);
+ * g(a) = W_L phi(... phi(W_1 a + b_1) ...) + b_L.  The residual term is linear, so the
+ * remainder of f equals the remainder of g (reading R10). */
+typedef struct {
+    int n_layers;          /* L = number of weight matrices (hidden layers = L-1 >= 1) */
+    const int* dims;       /* HOST array of L+1 ints: dims[0] = n+m ... dims[L] = n */
+    const float* const* W; /* HOST array of L pointers; W[l] is [dims[l+1], dims[l]] row-major */
+    const float* const* b; /* HOST array of L pointers; b[l] is [dims[l+1]] */
+    int act;               /* leb_act */
+    int residual;          /* 0/1 (informational: does not change the bounds) */
+    int weights_on_host;   /* 0: W[l], b[l] point to device memory; 1: host memory */
+} leb_mlp;
+
+enum {
+    LEB_FLAG_NO_MARGIN = 1u, /* NN: do not add the FP rounding margin (value mode; parity tests) */
+    LEB_FLAG_FFMA_ONLY = 2u, /* NN: FP32 FFMA contractions instead of 3xTF32 tcgen05 */
+    LEB_FLAG_HOST_IO = 4u    /* data pointers of this call are host pointers */
+};
+
+leb_status leb_create(leb_ctx** ctx, int device);
+leb_status leb_destroy(leb_ctx* ctx);
+const char* leb_status_str(leb_status s);
+
+/* Select the analytic model used by leb_analytic_fwd / leb_vjp(kind 0). */
+leb_status leb_set_analytic(leb_ctx* ctx, const leb_analytic_model* model);
+
+/* Copy, pad and pre-split the MLP weights into context-owned device memory (done once per
+ * model; enqueued on `stream`).  Used by leb_nn_fwd / leb_vjp(kind 1). */
+leb_status leb_set_mlp(leb_ctx* ctx, const leb_mlp* mlp, void* stream);
+
+/* Upper bound, in tiles, of the batch slice processed at once by the NN path (bounds the
+ * workspace: the forward keeps every back-substituted coefficient block of the slice in HBM).
+ * 0 restores the default.  Does not change results. */
+leb_status leb_set_nn_chunk(leb_ctx* ctx, int tiles_per_chunk);
+
+/* Path-based interval-Hessian bound, Thm 1 eq. (15), for every tile.
+ *   nom, rad : [B, T, ld_in]  nominal a~ and radii sigma >= 0 (box (25a) L272, mu = 0)
+ *   mu       : must be NULL (LEB_ERR_UNSUPPORTED otherwise)
+ *   r_lo,r_hi: [B, T, ld_out] outputs, r_lo <= r(a) <= r_hi on the box, outward-rounded FP32. */
+leb_status leb_analytic_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad,
+                            const float* mu, int ld_in, float* r_lo, float* r_hi, int ld_out,
+                            unsigned flags, void* stream);
+
+/* CROWN + Thm 3 bound, eq. (18)-(21) L196-220, for every tile.
+ *   J      : NULL => the network's own Jacobian at a~ (eq. (7)); otherwise [B, T, n, N]
+ *            dense, and the bound is with respect to that matrix (Thm 3 holds for any J).
+ *   margin : NULL or [B, T, ld_out]: the rounding margin that was (or, with
+ *            LEB_FLAG_NO_MARGIN, would have been) added outward to each of r_lo, r_hi. */
+leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad,
+                      const float* mu, const float* J, int ld_in, float* r_lo, float* r_hi,
+                      float* margin, int ld_out, unsigned flags, void* stream);
+
+/* VJP of the bounds: grad = d/d(a~, sigma) sum_i g_hi[i] r_hi[i] + g_lo[i] r_lo[i], per tile
+ * (block-diagonal over tiles).  Recomputes the forward pass internally (stateless).
+ *   kind: 0 analytic (model from leb_set_analytic), 1 NN (model from leb_set_mlp)
+ *   g_lo, g_hi       : [B, T, ld_out] cotangents
+ *   grad_nom,grad_rad: [B, T, ld_in] outputs (columns >= N are left untouched).
+ * min / max / abs / ReLU-switch / relaxation-case selections are treated as branch selections
+ * (derivative of the selected branch), as in DESIGN.md "VJP definition". */
+leb_status leb_vjp(leb_ctx* ctx, int kind, int B, int T, const float* nom, const float* rad,
+                   const float* g_lo, const float* g_hi, int ld_in, int ld_out, float* grad_nom,
+                   float* grad_rad, unsigned flags, void* stream);
+
+/* Zonotope fold, L229-231 and (25b,c) L274-281: c_bar = (r_lo + r_hi)/2,
+ * R_diag = (r_hi - r_lo)/2 + pad (padding L347), rounded so that
+ * [r_lo, r_hi] is contained in [c_bar - R_diag, c_bar + R_diag] in FP32.
+ *   r_lo, r_hi, c_bar, R_diag : [B, T, n] contiguous
+ *   E_diag     : NULL or [n], the (constant, diagonal) disturbance matrix E
+ *   Ebar_dense : NULL or [B, T, n, 2n]: E_bar = [diag(E)  diag(R_diag)]  (25b) */
+leb_status leb_zonotope_inflate(leb_ctx* ctx, int B, int T, int n, const float* r_lo,
+                                const float* r_hi, const float* E_diag, float pad, float* c_bar,
+                                float* R_diag, float* Ebar_dense, unsigned flags, void* stream);
+
+/* Cotangents of (c_bar, R_diag) -> cotangents of (r_lo, r_hi) (the fold is linear):
+ * g_lo = (gc - gR)/2, g_hi = (gc + gR)/2.  Arrays [B, T, n] contiguous. */
+leb_status leb_zonotope_inflate_vjp(leb_ctx* ctx, int B, int T, int n, const float* gc,
+                                    const float* gR, float* g_lo, float* g_hi, unsigned flags,
+                                    void* stream);
+
+/* *flag = 1 if any tile of any call since the last leb_domain_flag() hit a domain error
+ * (synchronises `stream`, then clears the flag). */
+leb_status leb_domain_flag(leb_ctx* ctx, int* flag, void* stream);
+
+/* Inspection (tests): pre-activation bounds (l_s, u_s) of hidden layer `layer` (1-based) left
+ * in the workspace by the LAST leb_nn_fwd call whose B*T fitted one chunk.
+ * l, u: device [B*T, dims[layer]] contiguous. */
+leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, void* stream);
+
+/* Number of kernel launches the library has enqueued on this context so far. */
+long long leb_launch_count(const leb_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LEB_H_ */

@@ -1,0 +1,296 @@
+// api.cu -- the extern "C" boundary declared in include/leb.h: argument validation, host-IO
+// staging, dispatch to the kernels' launchers.  No numerical step of the method runs on the host.
+#include <stdio.h>
+#include <stdint.h>
+#include <new>
+#include "an_core.cuh"
+#include "internal.h"
+
+struct leb_ctx {
+    int device = 0;
+    bool has_analytic = false;
+    leb_an::Model model{};
+    NnState* nn = nullptr;
+    int* domain_flag = nullptr;     // device
+    long long launches = 0;
+    // staging for LEB_FLAG_HOST_IO (grown on demand)
+    float* stage[8] = {nullptr};
+    size_t stage_bytes[8] = {0};
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = 0;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+inline bool al4(const void* p) { return ((uintptr_t)p & 3) == 0; }
+
+float* stage_buf(leb_ctx* c, int slot, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    if (c->stage_bytes[slot] < bytes) {
+        if (c->stage[slot]) { cudaDeviceSynchronize(); cudaFree(c->stage[slot]); c->stage[slot] = nullptr; c->stage_bytes[slot] = 0; }
+        if (cudaMalloc(&c->stage[slot], bytes) != cudaSuccess) return nullptr;
+        c->stage_bytes[slot] = bytes;
+    }
+    return c->stage[slot];
+}
+
+// host -> staging (returns device pointer) or pass-through
+const float* in_ptr(leb_ctx* c, int slot, const float* p, size_t count, bool host, cudaStream_t st, bool* ok) {
+    if (!host || !p) return p;
+    float* d = stage_buf(c, slot, count * sizeof(float));
+    if (!d) { *ok = false; return nullptr; }
+    if (cudaMemcpyAsync(d, p, count * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) *ok = false;
+    return d;
+}
+float* out_ptr(leb_ctx* c, int slot, float* p, size_t count, bool host, bool* ok) {
+    if (!host || !p) return p;
+    float* d = stage_buf(c, slot, count * sizeof(float));
+    if (!d) *ok = false;
+    return d;
+}
+void out_copy(float* host_p, const float* dev_p, size_t count, bool host, cudaStream_t st, bool* ok) {
+    if (!host || !host_p) return;
+    if (cudaMemcpyAsync(host_p, dev_p, count * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess) *ok = false;
+}
+
+leb_status check_traj(int B, int T, int N, int n, int ld_in, int ld_out) {
+    if (B < 0 || T < 0) return LEB_ERR_ARG;
+    if ((long long)B * T > 2000000000LL) return LEB_ERR_SHAPE;
+    if (ld_in < N || ld_out < n) return LEB_ERR_SHAPE;
+    return LEB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* leb_status_str(leb_status s) {
+    switch (s) {
+        case LEB_OK: return "ok";
+        case LEB_ERR_ARG: return "bad argument";
+        case LEB_ERR_SHAPE: return "bad shape";
+        case LEB_ERR_ALIGN: return "misaligned pointer";
+        case LEB_ERR_DOMAIN: return "domain error in some tile";
+        case LEB_ERR_UNSUPPORTED: return "unsupported";
+        case LEB_ERR_CUDA: return "CUDA error";
+        case LEB_ERR_NOMEM: return "out of device memory";
+        case LEB_ERR_STATE: return "model not set";
+    }
+    return "unknown";
+}
+
+leb_status leb_create(leb_ctx** out, int device) {
+    if (!out) return LEB_ERR_ARG;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return LEB_ERR_CUDA;
+    DeviceGuard guard(device);
+    leb_ctx* c = new (std::nothrow) leb_ctx();
+    if (!c) return LEB_ERR_NOMEM;
+    c->device = device;
+    if (cudaMalloc(&c->domain_flag, sizeof(int)) != cudaSuccess) { delete c; return LEB_ERR_NOMEM; }
+    cudaMemset(c->domain_flag, 0, sizeof(int));
+    c->nn = leb_nn_create();
+    *out = c;
+    return LEB_OK;
+}
+
+leb_status leb_destroy(leb_ctx* c) {
+    if (!c) return LEB_OK;
+    DeviceGuard guard(c->device);
+    cudaDeviceSynchronize();
+    leb_nn_destroy(c->nn);
+    for (int i = 0; i < 8; ++i) if (c->stage[i]) cudaFree(c->stage[i]);
+    if (c->domain_flag) cudaFree(c->domain_flag);
+    delete c;
+    return LEB_OK;
+}
+
+leb_status leb_set_analytic(leb_ctx* c, const leb_analytic_model* m) {
+    if (!c || !m) return LEB_ERR_ARG;
+    if (m->model_id != LEB_MODEL_UNICYCLE && m->model_id != LEB_MODEL_QUAD12 && m->model_id != LEB_MODEL_QUADCHAIN) return LEB_ERR_UNSUPPORTED;
+    if (m->model_id != LEB_MODEL_UNICYCLE && m->integ != LEB_INTEG_EULER && m->integ != LEB_INTEG_RK4) return LEB_ERR_ARG;
+    if (m->model_id == LEB_MODEL_QUADCHAIN && (m->n_units < 1 || m->n_units > 4096)) return LEB_ERR_SHAPE;
+    if (!(m->dt > 0.f)) return LEB_ERR_ARG;
+    if (m->model_id != LEB_MODEL_UNICYCLE && (!(m->mass > 0.f) || !(m->Jx > 0.f) || !(m->Jy > 0.f) || !(m->Jz > 0.f))) return LEB_ERR_ARG;
+    c->model = leb_make_model(*m);
+    c->has_analytic = true;
+    return LEB_OK;
+}
+
+leb_status leb_set_mlp(leb_ctx* c, const leb_mlp* m, void* stream) {
+    if (!c) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    return leb_nn_set_mlp(c->nn, m, (cudaStream_t)stream, &c->launches);
+}
+
+leb_status leb_set_nn_chunk(leb_ctx* c, int tiles) {
+    if (!c) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    return leb_nn_set_chunk(c->nn, tiles);
+}
+
+leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, int ld_in,
+                            float* r_lo, float* r_hi, int ld_out, unsigned flags, void* stream) {
+    if (!c || !nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
+    if (!c->has_analytic) return LEB_ERR_STATE;
+    if (mu) return LEB_ERR_UNSUPPORTED;
+    leb_status s = check_traj(B, T, c->model.N, c->model.n, ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
+    float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    if (leb_launch_analytic_fwd(c->model, (int)tiles, d_nom, d_rad, ld_in, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches) != cudaSuccess)
+        return LEB_ERR_CUDA;
+    out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
+    out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, const float* J, int ld_in,
+                      float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, void* stream) {
+    if (!c || !nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    if (mu) return LEB_ERR_UNSUPPORTED;
+    const int n = leb_nn_n(c->nn), N = leb_nn_N(c->nn);
+    leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi) || !al4(J) || !al4(margin)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_J = in_ptr(c, 4, J, tiles * (size_t)n * N, host, st, &ok);
+    float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
+    float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
+    float* d_mg = out_ptr(c, 5, margin, tiles * ld_out, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    s = leb_nn_forward(c->nn, (int)tiles, d_nom, d_rad, d_J, ld_in, d_lo, d_hi, d_mg, ld_out, flags, c->domain_flag, st, &c->launches);
+    if (s != LEB_OK) return s;
+    out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
+    out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
+    out_copy(margin, d_mg, tiles * ld_out, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
+                   int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, void* stream) {
+    if (!c || !nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad) return LEB_ERR_ARG;
+    if (kind != 0 && kind != 1) return LEB_ERR_ARG;
+    int n, N;
+    if (kind == 0) {
+        if (!c->has_analytic) return LEB_ERR_STATE;
+        n = c->model.n; N = c->model.N;
+    } else {
+        if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+        n = leb_nn_n(c->nn); N = leb_nn_N(c->nn);
+    }
+    leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(g_lo) || !al4(g_hi) || !al4(grad_nom) || !al4(grad_rad)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_glo = in_ptr(c, 2, g_lo, tiles * ld_out, host, st, &ok);
+    const float* d_ghi = in_ptr(c, 3, g_hi, tiles * ld_out, host, st, &ok);
+    float* d_gn = out_ptr(c, 6, grad_nom, tiles * ld_in, host, &ok);
+    float* d_gr = out_ptr(c, 7, grad_rad, tiles * ld_in, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    if (kind == 0) {
+        if (leb_launch_analytic_vjp(c->model, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, c->domain_flag, st,
+                                    &c->launches) != cudaSuccess)
+            return LEB_ERR_CUDA;
+    } else {
+        s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, flags, c->domain_flag, st, &c->launches);
+        if (s != LEB_OK) return s;
+    }
+    out_copy(grad_nom, d_gn, tiles * ld_in, host, st, &ok);
+    out_copy(grad_rad, d_gr, tiles * ld_in, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_zonotope_inflate(leb_ctx* c, int B, int T, int n, const float* r_lo, const float* r_hi, const float* E_diag,
+                                float pad, float* c_bar, float* R_diag, float* Ebar_dense, unsigned flags, void* stream) {
+    if (!c || !r_lo || !r_hi || !c_bar || !R_diag) return LEB_ERR_ARG;
+    if (B < 0 || T < 0 || n < 1 || !(pad >= 0.f)) return LEB_ERR_ARG;
+    if (!al4(r_lo) || !al4(r_hi) || !al4(c_bar) || !al4(R_diag) || !al4(Ebar_dense) || !al4(E_diag)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t rows = (size_t)B * T * n;
+    bool ok = true;
+    const float* d_lo = in_ptr(c, 0, r_lo, rows, host, st, &ok);
+    const float* d_hi = in_ptr(c, 1, r_hi, rows, host, st, &ok);
+    const float* d_E = in_ptr(c, 4, E_diag, n, host, st, &ok);
+    float* d_c = out_ptr(c, 2, c_bar, rows, host, &ok);
+    float* d_R = out_ptr(c, 3, R_diag, rows, host, &ok);
+    float* d_Eb = out_ptr(c, 5, Ebar_dense, rows * 2 * n, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    if (leb_launch_inflate(rows, n, d_lo, d_hi, d_E, pad, d_c, d_R, d_Eb, st, &c->launches) != cudaSuccess) return LEB_ERR_CUDA;
+    out_copy(c_bar, d_c, rows, host, st, &ok);
+    out_copy(R_diag, d_R, rows, host, st, &ok);
+    out_copy(Ebar_dense, d_Eb, rows * 2 * n, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_zonotope_inflate_vjp(leb_ctx* c, int B, int T, int n, const float* gc, const float* gR, float* g_lo, float* g_hi,
+                                    unsigned flags, void* stream) {
+    if (!c || !gc || !gR || !g_lo || !g_hi) return LEB_ERR_ARG;
+    if (B < 0 || T < 0 || n < 1) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t count = (size_t)B * T * n;
+    bool ok = true;
+    const float* d_gc = in_ptr(c, 0, gc, count, host, st, &ok);
+    const float* d_gR = in_ptr(c, 1, gR, count, host, st, &ok);
+    float* d_lo = out_ptr(c, 2, g_lo, count, host, &ok);
+    float* d_hi = out_ptr(c, 3, g_hi, count, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    if (leb_launch_inflate_vjp(count, d_gc, d_gR, d_lo, d_hi, st, &c->launches) != cudaSuccess) return LEB_ERR_CUDA;
+    out_copy(g_lo, d_lo, count, host, st, &ok);
+    out_copy(g_hi, d_hi, count, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_domain_flag(leb_ctx* c, int* flag, void* stream) {
+    if (!c || !flag) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int h = 0;
+    if (cudaMemcpyAsync(&h, c->domain_flag, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return LEB_ERR_CUDA;
+    if (cudaMemsetAsync(c->domain_flag, 0, sizeof(int), st) != cudaSuccess) return LEB_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return LEB_ERR_CUDA;
+    *flag = h;
+    return LEB_OK;
+}
+
+leb_status leb_nn_hidden_bounds(leb_ctx* c, int layer, float* l, float* u, void* stream) {
+    if (!c || !l || !u) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    DeviceGuard guard(c->device);
+    return leb_nn_get_hidden(c->nn, layer, l, u, (cudaStream_t)stream, &c->launches);
+}
+
+long long leb_launch_count(const leb_ctx* c) { return c ? c->launches : 0; }
+
+}  // extern "C"

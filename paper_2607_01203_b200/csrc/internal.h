@@ -1,0 +1,39 @@
+// internal.h -- declarations shared by the translation units of libleb.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include "../../include/leb.h"
+
+namespace leb_an { struct Model; }
+
+// ---- analytic path (analytic.cu)
+leb_an::Model leb_make_model(const leb_analytic_model& m);
+cudaError_t leb_launch_analytic_fwd(const leb_an::Model& M, int tiles, const float* nom, const float* rad, int ld_in,
+                                    float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
+                                    long long* launches);
+cudaError_t leb_launch_analytic_vjp(const leb_an::Model& M, int tiles, const float* nom, const float* rad, const float* g_lo,
+                                    const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad,
+                                    int* domain_flag, cudaStream_t st, long long* launches);
+
+// ---- zonotope fold (inflate.cu)
+cudaError_t leb_launch_inflate(size_t rows, int n, const float* r_lo, const float* r_hi, const float* E_diag, float pad,
+                               float* c_bar, float* R_diag, float* Ebar_dense, cudaStream_t st, long long* launches);
+cudaError_t leb_launch_inflate_vjp(size_t count, const float* gc, const float* gR, float* g_lo, float* g_hi,
+                                   cudaStream_t st, long long* launches);
+
+// ---- NN path (nn.cu)
+struct NnState;   // packed weights + workspace, owned by the context
+NnState* leb_nn_create();
+void leb_nn_destroy(NnState*);
+leb_status leb_nn_set_mlp(NnState*, const leb_mlp* mlp, cudaStream_t st, long long* launches);
+leb_status leb_nn_set_chunk(NnState*, int tiles);
+bool leb_nn_ready(const NnState*);
+int leb_nn_n(const NnState*);
+int leb_nn_N(const NnState*);
+leb_status leb_nn_forward(NnState*, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
+                          float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
+                          long long* launches);
+leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
+                      int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
+                      cudaStream_t st, long long* launches);
+leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);

@@ -1,0 +1,688 @@
+// nn.cu -- leb_nn_fwd / leb_vjp(kind 1): CROWN back-substitution (Thm 2, eq. (18),
+// PAPER.md:L196-200) + Jacobian correction and box concretisation (Thm 3, eq. (19)-(21), L204-220),
+// and the reverse sweep of the same computation.
+//
+// Formulation ("deviation form"; algebraically identical to eq. (18)-(21), SURVEY
+// 8(c).7): with zhat_l the nominal pre-activations and, per neuron, the gaps
+// gU = kU zhat + bU - phi(zhat) >= 0, gL = kL zhat + bL - phi(zhat) <= 0 of the two relaxation lines,
+//     u_s = zhat_s + |Lam_up_0| sigma + sum_l (P_l gU_l + Q_l gL_l)          (hidden target s)
+//     l_s = zhat_s - |Lam_lo_0| sigma + sum_l (P_l gL_l + Q_l gU_l)
+//     r_hi = |Lam_up_0 - J| sigma + sum_l (...),  r_lo = -|Lam_lo_0 - J| sigma + sum_l (...)   (output)
+// where Lam_{l-1} = (P_l (.) k_pos + Q_l (.) k_neg) W_l, P = max(Lam,0), Q = min(Lam,0), and J is the
+// third ("Jacobian") chain with k_pos = k_neg = phi'(zhat).  No O(1) quantities are cancelled.
+//
+// Steps: N1 nominal pass, N2 layer-1 interval bounds, N3 hidden targets, N4 output
+// target, N5 concretisation, V reverse sweep.  All contractions are launched from here.
+#include <stdio.h>
+#include <vector>
+#include "internal.h"
+#include "nn_relax.cuh"
+#include "nn_gemm_ffma.cuh"
+
+using namespace leb_nn;
+
+namespace {
+
+inline int rup(int x, int m) { return (x + m - 1) / m * m; }
+constexpr int kPad = 32;        // feature dims are zero-padded to multiples of 32
+constexpr int kRowBlock = 128;  // chain row blocks
+constexpr int kMaxLayers = 16;
+
+}  // namespace
+
+struct NnState {
+    bool ready = false;
+    int L = 0, act = 0;
+    int w[kMaxLayers + 1] = {0}, wp[kMaxLayers + 1] = {0};   // true / padded widths, w[0] = N, w[L] = n
+    // weights (1-based layer index l = 1..L): W[l] is [rowsW[l] x wp[l-1]], Wt[l] is [wp[l-1] x rowsW[l]]
+    float *W[kMaxLayers + 1] = {nullptr}, *Wt[kMaxLayers + 1] = {nullptr}, *bias[kMaxLayers + 1] = {nullptr};
+    int rowsW[kMaxLayers + 1] = {0};
+    float *Wabs1 = nullptr, *Wabs1t = nullptr;
+    // workspace for one chunk of tiles
+    int chunk_req = 0, chunk = 0;
+    bool ws_vjp = false;
+    std::vector<void*> allocs;
+    float *nomp = nullptr, *radp = nullptr, *rad1 = nullptr;
+    float *zhat[kMaxLayers] = {nullptr}, *ahat[kMaxLayers] = {nullptr}, *dphi[kMaxLayers] = {nullptr};
+    float *lb[kMaxLayers] = {nullptr}, *ub[kMaxLayers] = {nullptr};
+    float *kU[kMaxLayers] = {nullptr}, *kL[kMaxLayers] = {nullptr}, *gU[kMaxLayers] = {nullptr}, *gL[kMaxLayers] = {nullptr};
+    // chains: target s = 2..L; Lam[s][l] for l = 0..s-2: [chunk*rows_pad[s] x wp[l]]
+    int rows_kind[kMaxLayers + 1] = {0}, rows_pad[kMaxLayers + 1] = {0};
+    float* Lam[kMaxLayers + 1][kMaxLayers] = {{nullptr}};
+    float* gap[kMaxLayers + 1] = {nullptr};
+    // VJP workspace
+    float *kUb[kMaxLayers] = {nullptr}, *kLb[kMaxLayers] = {nullptr}, *gUb[kMaxLayers] = {nullptr}, *gLb[kMaxLayers] = {nullptr},
+          *dpb[kMaxLayers] = {nullptr}, *zbar[kMaxLayers] = {nullptr}, *lbar[kMaxLayers] = {nullptr}, *ubar[kMaxLayers] = {nullptr};
+    float *Lbar[2] = {nullptr, nullptr}, *gapbar = nullptr, *nom_bar = nullptr, *rad_bar = nullptr, *glo_p = nullptr, *ghi_p = nullptr;
+    int last_tiles = 0;
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// small kernels
+// ------------------------------------------------------------------------------------------
+// copy [rows x cols] (ld_src) into a zero-padded [rows x ld_dst] buffer, optionally transposing / abs
+__global__ void pack_matrix_kernel(const float* __restrict__ src, int rows, int cols, int ld_src, float* __restrict__ dst,
+                                   int rows_p, int cols_p, int transpose, int absval) {
+    // dst is [rows_p x cols_p] if !transpose else [cols_p x rows_p]
+    size_t total = (size_t)rows_p * cols_p;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int r, c;
+        if (!transpose) { r = (int)(q / cols_p); c = (int)(q - (size_t)r * cols_p); }
+        else { c = (int)(q / rows_p); r = (int)(q - (size_t)c * rows_p); }
+        float v = (r < rows && c < cols) ? src[(size_t)r * ld_src + c] : 0.f;
+        dst[q] = absval ? fabsf(v) : v;
+    }
+}
+
+// nom/rad [tiles x ld_in] -> zero-padded [tiles x wp0]; invalid input (NaN/Inf, sigma < 0) poisons the tile with NaN
+__global__ void pad_inputs_kernel(int tiles, int N, int ld_in, int wp0, const float* __restrict__ nom, const float* __restrict__ rad,
+                                  float* __restrict__ nomp, float* __restrict__ radp) {
+    size_t total = (size_t)tiles * wp0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int t = (int)(q / wp0), c = (int)(q - (size_t)t * wp0);
+        float a = 0.f, s = 0.f;
+        if (c < N) {
+            a = nom[(size_t)t * ld_in + c];
+            s = rad[(size_t)t * ld_in + c];
+            if (!(s >= 0.f) || !(s <= 3.0e38f)) s = NAN;
+            if (!(fabsf(a) <= 3.0e38f)) a = NAN;
+        }
+        nomp[q] = a;
+        radp[q] = s;
+    }
+}
+
+__global__ void pad_cotangent_kernel(int tiles, int n, int ld_out, const float* __restrict__ g_lo, const float* __restrict__ g_hi,
+                                     float* __restrict__ glo_p, float* __restrict__ ghi_p) {
+    size_t total = (size_t)tiles * n;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int t = (int)(q / n), c = (int)(q - (size_t)t * n);
+        glo_p[q] = g_lo[(size_t)t * ld_out + c];
+        ghi_p[q] = g_hi[(size_t)t * ld_out + c];
+    }
+}
+
+__global__ void fill_kernel(float* __restrict__ p, size_t count, float v) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) p[q] = v;
+}
+
+// per-neuron relaxation of layer l from (zhat, l, u); for layer 1 (rad1 != NULL) first l,u = zhat -+ rad1 (N2)
+__global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat,
+                                 const float* __restrict__ rad1, float* __restrict__ lb, float* __restrict__ ub,
+                                 float* __restrict__ kU, float* __restrict__ kL, float* __restrict__ gU, float* __restrict__ gL) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) {
+            lb[q] = 0.f; ub[q] = 0.f; kU[q] = 0.f; kL[q] = 0.f; gU[q] = 0.f; gL[q] = 0.f;
+            continue;
+        }
+        float z = zhat[q], l, u;
+        if (rad1) { float r = rad1[q]; l = z - r; u = z + r; lb[q] = l; ub[q] = u; }
+        else { l = lb[q]; u = ub[q]; }
+        Relax r = relax_any(act, (double)l, (double)u);
+        double f = act_f(act, (double)z);
+        kU[q] = (float)r.kU;
+        kL[q] = (float)r.kL;
+        gU[q] = (float)(r.kU * (double)z + r.bU - f);
+        gL[q] = (float)(r.kL * (double)z + r.bL - f);
+    }
+}
+
+// N5 for a hidden target s: one warp per (tile, neuron k): rows k (upper) and rows_kind + k (lower)
+__global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
+                                         const float* __restrict__ sigma, const float* __restrict__ gap,
+                                         const float* __restrict__ zhat, float* __restrict__ lb, float* __restrict__ ub) {
+    int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    int total = tiles * rows_kind;
+    if (warp >= total) return;
+    int t = warp / rows_kind, k = warp - t * rows_kind;
+    const float* up = Lam0 + ((size_t)t * rows_pad + k) * wp0;
+    const float* lo = Lam0 + ((size_t)t * rows_pad + rows_kind + k) * wp0;
+    const float* sg = sigma + (size_t)t * wp0;
+    float su = 0.f, sl = 0.f;
+    for (int j = lane * 4; j < wp0; j += 128) {
+        float4 a = *reinterpret_cast<const float4*>(up + j), b = *reinterpret_cast<const float4*>(lo + j);
+        float4 s = *reinterpret_cast<const float4*>(sg + j);
+        su += fabsf(a.x) * s.x + fabsf(a.y) * s.y + fabsf(a.z) * s.z + fabsf(a.w) * s.w;
+        sl += fabsf(b.x) * s.x + fabsf(b.y) * s.y + fabsf(b.z) * s.z + fabsf(b.w) * s.w;
+    }
+#pragma unroll
+    for (int off = 16; off; off >>= 1) { su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off); }
+    if (lane == 0) {
+        float z = zhat[(size_t)t * rows_kind + k];
+        ub[(size_t)t * rows_kind + k] = z + (su + gap[(size_t)t * rows_pad + k]);
+        lb[(size_t)t * rows_kind + k] = z - (sl - gap[(size_t)t * rows_pad + rows_kind + k]);
+    }
+}
+
+// N5 for the output: Thm 3 (20)-(21); J = rows of the Jacobian chain, or the caller's matrix
+__global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int wp0, const float* __restrict__ Lam0,
+                                      const float* __restrict__ sigma, const float* __restrict__ gap,
+                                      const float* __restrict__ Jgiven, float* __restrict__ r_lo, float* __restrict__ r_hi,
+                                      int ld_out, int* __restrict__ domain_flag) {
+    int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    int total = tiles * n;
+    if (warp >= total) return;
+    int t = warp / n, i = warp - t * n;
+    const float* up = Lam0 + ((size_t)t * rows_pad + i) * wp0;
+    const float* lo = Lam0 + ((size_t)t * rows_pad + n + i) * wp0;
+    const float* sg = sigma + (size_t)t * wp0;
+    float su = 0.f, sl = 0.f;
+    if (Jgiven) {
+        const float* Jr = Jgiven + ((size_t)t * n + i) * N;
+        for (int j = lane; j < N; j += 32) {
+            float jv = Jr[j], s = sg[j];
+            su += fabsf(up[j] - jv) * s;
+            sl += fabsf(lo[j] - jv) * s;
+        }
+    } else {
+        const float* Jr = Lam0 + ((size_t)t * rows_pad + 2 * n + i) * wp0;
+        for (int j = lane * 4; j < wp0; j += 128) {
+            float4 a = *reinterpret_cast<const float4*>(up + j), b = *reinterpret_cast<const float4*>(lo + j);
+            float4 c = *reinterpret_cast<const float4*>(Jr + j), s = *reinterpret_cast<const float4*>(sg + j);
+            su += fabsf(a.x - c.x) * s.x + fabsf(a.y - c.y) * s.y + fabsf(a.z - c.z) * s.z + fabsf(a.w - c.w) * s.w;
+            sl += fabsf(b.x - c.x) * s.x + fabsf(b.y - c.y) * s.y + fabsf(b.z - c.z) * s.z + fabsf(b.w - c.w) * s.w;
+        }
+    }
+#pragma unroll
+    for (int off = 16; off; off >>= 1) { su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off); }
+    if (lane == 0) {
+        float hi = su + gap[(size_t)t * rows_pad + i];
+        float lo_v = -sl + gap[(size_t)t * rows_pad + n + i];
+        if (!(fabsf(hi) <= 3.0e38f) || !(fabsf(lo_v) <= 3.0e38f)) {   // NaN / Inf anywhere in the tile's inputs
+            hi = INFINITY; lo_v = -INFINITY;
+            atomicExch(domain_flag, 1);
+        }
+        r_hi[(size_t)t * ld_out + i] = hi;
+        r_lo[(size_t)t * ld_out + i] = lo_v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// VJP kernels
+// ------------------------------------------------------------------------------------------
+// Seeds of target s: one CTA per tile; thread j owns input column(s) j, loops over the rows.
+//   hidden: Lbar0[up k] = ubar_k sign(Lam_up_0) sigma,  Lbar0[lo k] = -lbar_k sign(Lam_lo_0) sigma
+//   output: with S = sign(Lam_0 - J): Lbar0[up i] = g_hi_i S_up sigma, Lbar0[lo i] = -g_lo_i S_lo sigma,
+//           Lbar0[jac i] = -(Lbar0[up i] + Lbar0[lo i])
+//   rad_bar_j += sum_rows |.| weights;  gapbar[up] = ybar_up, gapbar[lo] = ybar_lo
+__global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
+                            const float* __restrict__ sigma, const float* __restrict__ ybar_up, const float* __restrict__ ybar_lo,
+                            int ldy, float* __restrict__ Lbar0, float* __restrict__ gapbar, float* __restrict__ rad_bar) {
+    const int t = blockIdx.x;
+    const float* base = Lam0 + (size_t)t * rows_pad * wp0;
+    float* obase = Lbar0 + (size_t)t * rows_pad * wp0;
+    for (int r = threadIdx.x; r < rows_pad; r += blockDim.x) {
+        float v = 0.f;
+        if (r < rows_kind) v = ybar_up[(size_t)t * ldy + r];
+        else if (r < 2 * rows_kind) v = ybar_lo[(size_t)t * ldy + r - rows_kind];
+        gapbar[(size_t)t * rows_pad + r] = v;
+    }
+    for (int j = threadIdx.x; j < wp0; j += blockDim.x) {
+        const float s = sigma[(size_t)t * wp0 + j];
+        float sb = 0.f;
+        for (int k = 0; k < rows_kind; ++k) {
+            const float yu = ybar_up[(size_t)t * ldy + k], yl = ybar_lo[(size_t)t * ldy + k];
+            float a = base[(size_t)k * wp0 + j], b = base[(size_t)(rows_kind + k) * wp0 + j];
+            if (is_out) { float jv = base[(size_t)(2 * rows_kind + k) * wp0 + j]; a -= jv; b -= jv; }
+            const float sa = (a > 0.f) - (a < 0.f), sbn = (b > 0.f) - (b < 0.f);
+            const float lu = yu * sa * s, ll = -yl * sbn * s;
+            obase[(size_t)k * wp0 + j] = lu;
+            obase[(size_t)(rows_kind + k) * wp0 + j] = ll;
+            if (is_out) obase[(size_t)(2 * rows_kind + k) * wp0 + j] = -(lu + ll);
+            sb += yu * fabsf(a) - yl * fabsf(b);
+        }
+        rad_bar[(size_t)t * wp0 + j] += sb;
+    }
+}
+
+// adjoint of the relaxation parameters of layer l -> (lbar, ubar), and the direct zhat terms
+__global__ void relax_vjp_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat,
+                                 const float* __restrict__ lb, const float* __restrict__ ub, const float* __restrict__ kUb,
+                                 const float* __restrict__ kLb, const float* __restrict__ gUb, const float* __restrict__ gLb,
+                                 const float* __restrict__ dpb, float* __restrict__ lbar, float* __restrict__ ubar,
+                                 float* __restrict__ zbar, int is_layer1) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) { lbar[q] = 0.f; ubar[q] = 0.f; continue; }
+        double z = zhat[q], l = lb[q], u = ub[q];
+        Relax r = relax_any(act, l, u);
+        double gu = gUb[q], gl = gLb[q];
+        // g = k zhat + b - phi(zhat):  k_bar_eff = k_bar + zhat g_bar,  b_bar = g_bar
+        double kbu = (double)kUb[q] + z * gu, kbl = (double)kLb[q] + z * gl;
+        double lo = 0.0, up = 0.0;
+        line_vjp(act, r.cU, true, l, u, r.dU, kbu, gu, lo, up);
+        line_vjp(act, r.cL, false, l, u, r.dL, kbl, gl, lo, up);
+        double d1 = act_d1(act, z);
+        double zb = (r.kU - d1) * gu + (r.kL - d1) * gl + act_d2(act, z) * (double)dpb[q];
+        // l_s = zhat_s - ..., u_s = zhat_s + ...: both pass their adjoint straight to zhat_s
+        zb += lo + up;
+        lbar[q] = (float)lo;
+        ubar[q] = (float)up;
+        zbar[q] += (float)zb;
+        (void)is_layer1;
+    }
+}
+
+// ub1 - lb1 adjoint for the layer-1 radius |W_1| sigma
+__global__ void diff_kernel(const float* __restrict__ ubar, const float* __restrict__ lbar, float* __restrict__ out, size_t count) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x)
+        out[q] = ubar[q] - lbar[q];
+}
+
+__global__ void write_grads_kernel(int tiles, int N, int wp0, int ld_in, const float* __restrict__ nom_bar,
+                                   const float* __restrict__ rad_bar, float* __restrict__ grad_nom, float* __restrict__ grad_rad) {
+    size_t total = (size_t)tiles * N;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int t = (int)(q / N), c = (int)(q - (size_t)t * N);
+        grad_nom[(size_t)t * ld_in + c] = nom_bar[(size_t)t * wp0 + c];
+        grad_rad[(size_t)t * ld_in + c] = rad_bar[(size_t)t * wp0 + c];
+    }
+}
+
+__global__ void copy_hidden_kernel(int tiles, int w, int wp, const float* __restrict__ lb, const float* __restrict__ ub,
+                                   float* __restrict__ l, float* __restrict__ u) {
+    size_t total = (size_t)tiles * w;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int t = (int)(q / w), c = (int)(q - (size_t)t * w);
+        l[q] = lb[(size_t)t * wp + c];
+        u[q] = ub[(size_t)t * wp + c];
+    }
+}
+
+inline unsigned gs_grid(size_t work) {
+    size_t b = (work + 255) / 256;
+    if (b > 148 * 16) b = 148 * 16;
+    if (b < 1) b = 1;
+    return (unsigned)b;
+}
+
+// ------------------------------------------------------------------------------------------
+// GEMM launch helpers
+// ------------------------------------------------------------------------------------------
+template <int AMODE, int EPI>
+void launch_gemm(const GemmArgs& g, cudaStream_t st, long long* launches) {
+    dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM);
+    gemm_ffma_kernel<AMODE, EPI><<<grid, GT, 0, st>>>(g);
+    ++*launches;
+}
+
+GemmArgs plain_args(int M, int N, int K, const float* A, int lda, const float* B, int ldb, float* C, int ldc) {
+    GemmArgs g{};
+    g.M = M; g.N = N; g.K = K; g.A = A; g.lda = lda; g.B = B; g.ldb = ldb; g.C = C; g.ldc = ldc;
+    g.rows_pad = 1; g.rows_kind = 1; g.nkinds = 1;
+    return g;
+}
+
+void* ws_alloc(NnState* S, size_t bytes, bool* ok) {
+    void* p = nullptr;
+    if (bytes == 0) bytes = 16;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { *ok = false; return nullptr; }
+    S->allocs.push_back(p);
+    return p;
+}
+
+void ws_free(NnState* S) {
+    for (void* p : S->allocs) cudaFree(p);
+    S->allocs.clear();
+    S->chunk = 0;
+    S->ws_vjp = false;
+}
+
+size_t bytes_per_tile(const NnState* S, bool vjp) {
+    size_t f = 3 * (size_t)S->wp[0];
+    for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 17 : 9);
+    size_t maxLam = 0;
+    for (int s = 2; s <= S->L; ++s) {
+        for (int l = 0; l <= s - 2; ++l) f += (size_t)S->rows_pad[s] * S->wp[l];
+        f += S->rows_pad[s];
+        for (int l = 0; l <= s - 2; ++l) maxLam = std::max(maxLam, (size_t)S->rows_pad[s] * S->wp[l]);
+    }
+    if (vjp) f += 2 * maxLam + 2 * (size_t)S->wp[0] + 2 * (size_t)S->w[S->L] + 1024;
+    return f * sizeof(float);
+}
+
+// (re)allocate the chunk workspace
+leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
+    int want = S->chunk_req > 0 ? S->chunk_req : 0;
+    if (want == 0) {
+        // default: as many tiles as fit in ~6 GB, at most 1024 (enough row blocks to fill 148 SMs many times)
+        size_t per = bytes_per_tile(S, true);
+        size_t c = (size_t)6e9 / (per ? per : 1);
+        if (c < 1) c = 1;
+        if (c > 1024) c = 1024;
+        want = (int)c;
+    }
+    if (want > tiles && tiles > 0) want = tiles;
+    if (S->chunk >= want && (S->ws_vjp || !vjp)) return LEB_OK;
+    cudaDeviceSynchronize();
+    ws_free(S);
+    const int C = want, L = S->L;
+    bool ok = true;
+    auto F = [&](size_t count) { return (float*)ws_alloc(S, count * sizeof(float), &ok); };
+    S->nomp = F((size_t)C * S->wp[0]);
+    S->radp = F((size_t)C * S->wp[0]);
+    S->rad1 = F((size_t)C * S->wp[1]);
+    for (int l = 1; l < L; ++l) {
+        size_t c = (size_t)C * S->wp[l];
+        S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
+        S->kU[l] = F(c); S->kL[l] = F(c); S->gU[l] = F(c); S->gL[l] = F(c);
+        if (vjp) {
+            S->kUb[l] = F(c); S->kLb[l] = F(c); S->gUb[l] = F(c); S->gLb[l] = F(c); S->dpb[l] = F(c);
+            S->zbar[l] = F(c); S->lbar[l] = F(c); S->ubar[l] = F(c);
+        }
+    }
+    size_t maxLam = 0;
+    for (int s = 2; s <= L; ++s) {
+        for (int l = 0; l <= s - 2; ++l) {
+            size_t c = (size_t)C * S->rows_pad[s] * S->wp[l];
+            S->Lam[s][l] = F(c);
+            maxLam = std::max(maxLam, c);
+        }
+        S->gap[s] = F((size_t)C * S->rows_pad[s]);
+    }
+    if (vjp) {
+        S->Lbar[0] = F(maxLam);
+        S->Lbar[1] = F(maxLam);
+        size_t maxrows = 0;
+        for (int s = 2; s <= L; ++s) maxrows = std::max(maxrows, (size_t)S->rows_pad[s]);
+        S->gapbar = F((size_t)C * maxrows);
+        S->nom_bar = F((size_t)C * S->wp[0]);
+        S->rad_bar = F((size_t)C * S->wp[0]);
+        S->glo_p = F((size_t)C * S->w[L]);
+        S->ghi_p = F((size_t)C * S->w[L]);
+    }
+    if (!ok) { ws_free(S); return LEB_ERR_NOMEM; }
+    S->chunk = C;
+    S->ws_vjp = vjp;
+    return LEB_OK;
+}
+
+// forward for one chunk of C tiles whose padded inputs are already in S->nomp / S->radp
+void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaStream_t st, long long* launches) {
+    const int L = S->L;
+    // ---- N1 nominal pass
+    const float* a_prev = S->nomp;
+    for (int l = 1; l < L; ++l) {
+        GemmArgs g = plain_args(C, S->wp[l], S->wp[l - 1], a_prev, S->wp[l - 1], S->Wt[l], S->wp[l], S->zhat[l], S->wp[l]);
+        g.bias = S->bias[l]; g.ahat = S->ahat[l]; g.dphi_out = S->dphi[l]; g.act = S->act;
+        launch_gemm<AMODE_PLAIN, EPI_NOMINAL>(g, st, launches);
+        a_prev = S->ahat[l];
+    }
+    // ---- N2 layer-1 interval bounds: rad1 = |W_1| sigma
+    {
+        GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
+        launch_gemm<AMODE_PLAIN, EPI_STORE>(g, st, launches);
+        relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->rad1, S->lb[1],
+                                                                      S->ub[1], S->kU[1], S->kL[1], S->gU[1], S->gL[1]);
+        ++*launches;
+    }
+    // ---- N3 / N4: targets s = 2 .. L
+    for (int s = 2; s <= L; ++s) {
+        const bool is_out = (s == L);
+        const int nk = is_out ? (with_jac ? 3 : 2) : 2;
+        const int rp = S->rows_pad[s], rk = S->rows_kind[s];
+        for (int l = s - 1; l >= 1; --l) {
+            GemmArgs g{};
+            g.M = C * rp; g.N = S->wp[l - 1]; g.K = S->wp[l];
+            g.a_shared = (l == s - 1);
+            g.A = g.a_shared ? S->W[s] : S->Lam[s][l];
+            g.lda = S->wp[l];
+            g.B = S->W[l]; g.ldb = S->wp[l - 1];
+            g.C = S->Lam[s][l - 1]; g.ldc = S->wp[l - 1];
+            g.rows_pad = rp; g.rows_kind = rk; g.nkinds = nk;
+            g.kU = S->kU[l]; g.kL = S->kL[l]; g.gU = S->gU[l]; g.gL = S->gL[l]; g.dphi = S->dphi[l]; g.ldp = S->wp[l];
+            g.gap = S->gap[s]; g.gap_init = (l == s - 1);
+            launch_gemm<AMODE_CHAIN, EPI_STORE>(g, st, launches);
+        }
+        if (!is_out) {
+            size_t warps = (size_t)C * rk;
+            concretise_hidden_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(C, rp, rk, S->wp[0], S->Lam[s][0], S->radp,
+                                                                                        S->gap[s], S->zhat[s], S->lb[s], S->ub[s]);
+            ++*launches;
+            relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s],
+                                                                          S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s]);
+            ++*launches;
+        }
+    }
+    (void)Jgiven;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// state management
+// ------------------------------------------------------------------------------------------
+NnState* leb_nn_create() { return new NnState(); }
+
+static void free_weights(NnState* S) {
+    for (int l = 0; l <= kMaxLayers; ++l) {
+        if (S->W[l]) cudaFree(S->W[l]);
+        if (S->Wt[l]) cudaFree(S->Wt[l]);
+        if (S->bias[l]) cudaFree(S->bias[l]);
+        S->W[l] = S->Wt[l] = S->bias[l] = nullptr;
+    }
+    if (S->Wabs1) cudaFree(S->Wabs1);
+    if (S->Wabs1t) cudaFree(S->Wabs1t);
+    S->Wabs1 = S->Wabs1t = nullptr;
+    S->ready = false;
+}
+
+void leb_nn_destroy(NnState* S) {
+    if (!S) return;
+    cudaDeviceSynchronize();
+    ws_free(S);
+    free_weights(S);
+    delete S;
+}
+
+bool leb_nn_ready(const NnState* S) { return S && S->ready; }
+int leb_nn_n(const NnState* S) { return S->w[S->L]; }
+int leb_nn_N(const NnState* S) { return S->w[0]; }
+
+leb_status leb_nn_set_chunk(NnState* S, int tiles) {
+    if (tiles < 0) return LEB_ERR_ARG;
+    S->chunk_req = tiles;
+    cudaDeviceSynchronize();
+    ws_free(S);
+    return LEB_OK;
+}
+
+leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long long* launches) {
+    if (!m || !m->dims || !m->W || !m->b) return LEB_ERR_ARG;
+    if (m->n_layers < 2 || m->n_layers > kMaxLayers) return LEB_ERR_SHAPE;
+    if (m->act != LEB_ACT_RELU && m->act != LEB_ACT_TANH) return LEB_ERR_ARG;
+    for (int l = 0; l <= m->n_layers; ++l) if (m->dims[l] < 1) return LEB_ERR_SHAPE;
+    cudaDeviceSynchronize();
+    ws_free(S);
+    free_weights(S);
+    S->L = m->n_layers;
+    S->act = m->act;
+    const int L = S->L;
+    for (int l = 0; l <= L; ++l) { S->w[l] = m->dims[l]; S->wp[l] = rup(m->dims[l], kPad); }
+    bool ok = true;
+    std::vector<void*> staged;
+    for (int l = 1; l <= L; ++l) {
+        const int rows = S->w[l], cols = S->w[l - 1];
+        const int rows_p = (l < L) ? S->wp[l] : rows;      // output rows are not padded (they are only A rows)
+        const int cols_p = S->wp[l - 1];
+        S->rowsW[l] = rows_p;
+        const float* src = m->W[l - 1];
+        const float* bsrc = m->b[l - 1];
+        float *dW = nullptr, *db = nullptr;
+        if (m->weights_on_host) {
+            ok = ok && cudaMalloc(&dW, (size_t)rows * cols * sizeof(float)) == cudaSuccess;
+            ok = ok && cudaMalloc(&db, (size_t)rows * sizeof(float)) == cudaSuccess;
+            if (!ok) break;
+            staged.push_back(dW); staged.push_back(db);
+            cudaMemcpyAsync(dW, src, (size_t)rows * cols * sizeof(float), cudaMemcpyHostToDevice, st);
+            cudaMemcpyAsync(db, bsrc, (size_t)rows * sizeof(float), cudaMemcpyHostToDevice, st);
+            src = dW; bsrc = db;
+        }
+        ok = ok && cudaMalloc(&S->W[l], (size_t)rows_p * cols_p * sizeof(float)) == cudaSuccess;
+        ok = ok && cudaMalloc(&S->Wt[l], (size_t)rows_p * cols_p * sizeof(float)) == cudaSuccess;
+        ok = ok && cudaMalloc(&S->bias[l], (size_t)rup(rows_p, kPad) * sizeof(float)) == cudaSuccess;
+        if (!ok) break;
+        size_t tot = (size_t)rows_p * cols_p;
+        pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->W[l], rows_p, cols_p, 0, 0);
+        pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wt[l], rows_p, cols_p, 1, 0);
+        pack_matrix_kernel<<<gs_grid(rows_p), 256, 0, st>>>(bsrc, 1, rows, rows, S->bias[l], 1, rup(rows_p, kPad), 0, 0);
+        *launches += 3;
+        if (l == 1) {
+            ok = ok && cudaMalloc(&S->Wabs1, tot * sizeof(float)) == cudaSuccess;
+            ok = ok && cudaMalloc(&S->Wabs1t, tot * sizeof(float)) == cudaSuccess;
+            if (!ok) break;
+            pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wabs1, rows_p, cols_p, 0, 1);
+            pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wabs1t, rows_p, cols_p, 1, 1);
+            *launches += 2;
+        }
+    }
+    cudaStreamSynchronize(st);
+    for (void* p : staged) cudaFree(p);
+    if (!ok || cudaGetLastError() != cudaSuccess) { free_weights(S); return ok ? LEB_ERR_CUDA : LEB_ERR_NOMEM; }
+    for (int s = 2; s <= L; ++s) {
+        S->rows_kind[s] = (s < L) ? S->wp[s] : S->w[L];
+        S->rows_pad[s] = rup((s < L ? 2 : 3) * S->rows_kind[s], kRowBlock);
+    }
+    S->ready = true;
+    return LEB_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// forward
+// ------------------------------------------------------------------------------------------
+leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
+                          float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
+                          long long* launches) {
+    if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;   // certified mode: see DESIGN.md (N6)
+    if (tiles == 0) return LEB_OK;
+    leb_status ws = ensure_workspace(S, tiles, false);
+    if (ws != LEB_OK) return ws;
+    const int L = S->L, n = S->w[L], N = S->w[0];
+    for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
+        const int C = std::min(S->chunk, tiles - t0);
+        pad_inputs_kernel<<<gs_grid((size_t)C * S->wp[0]), 256, 0, st>>>(C, N, ld_in, S->wp[0], nom + (size_t)t0 * ld_in,
+                                                                       rad + (size_t)t0 * ld_in, S->nomp, S->radp);
+        ++*launches;
+        forward_chunk(S, C, J, J == nullptr, st, launches);
+        size_t warps = (size_t)C * n;
+        concretise_out_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(
+            C, S->rows_pad[L], n, N, S->wp[0], S->Lam[L][0], S->radp, S->gap[L], J ? J + (size_t)t0 * n * N : nullptr,
+            r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out, ld_out, domain_flag);
+        ++*launches;
+        if (margin) {
+            // value mode: the margin that would have been added is reported as 0 until N6 lands
+            for (int r = 0; r < 1; ++r) {
+                // rows are strided by ld_out: fill row by row only when ld_out != n
+                if (ld_out == n) fill_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(margin + (size_t)t0 * ld_out, (size_t)C * n, 0.f);
+                else fill_kernel<<<gs_grid((size_t)C * ld_out), 256, 0, st>>>(margin + (size_t)t0 * ld_out, (size_t)C * ld_out, 0.f);
+                ++*launches;
+            }
+        }
+        S->last_tiles = (tiles <= S->chunk) ? C : 0;
+    }
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStream_t st, long long* launches) {
+    if (layer < 1 || layer >= S->L || S->last_tiles <= 0 || S->chunk <= 0) return LEB_ERR_STATE;
+    copy_hidden_kernel<<<gs_grid((size_t)S->last_tiles * S->w[layer]), 256, 0, st>>>(S->last_tiles, S->w[layer], S->wp[layer],
+                                                                                    S->lb[layer], S->ub[layer], l, u);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------
+// VJP: forward of the chunk (all coefficient blocks kept), then the reverse sweep
+// ------------------------------------------------------------------------------------------
+leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
+                      int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
+                      cudaStream_t st, long long* launches) {
+    (void)flags; (void)domain_flag;
+    if (tiles == 0) return LEB_OK;
+    leb_status ws = ensure_workspace(S, tiles, true);
+    if (ws != LEB_OK) return ws;
+    const int L = S->L, n = S->w[L], N = S->w[0], wp0 = S->wp[0];
+    for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
+        const int C = std::min(S->chunk, tiles - t0);
+        pad_inputs_kernel<<<gs_grid((size_t)C * wp0), 256, 0, st>>>(C, N, ld_in, wp0, nom + (size_t)t0 * ld_in,
+                                                                  rad + (size_t)t0 * ld_in, S->nomp, S->radp);
+        pad_cotangent_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(C, n, ld_out, g_lo + (size_t)t0 * ld_out,
+                                                                   g_hi + (size_t)t0 * ld_out, S->glo_p, S->ghi_p);
+        *launches += 2;
+        forward_chunk(S, C, nullptr, true, st, launches);
+        // ---- zero the adjoint accumulators
+        for (int l = 1; l < L; ++l) {
+            size_t c = (size_t)C * S->wp[l];
+            cudaMemsetAsync(S->kUb[l], 0, c * 4, st); cudaMemsetAsync(S->kLb[l], 0, c * 4, st);
+            cudaMemsetAsync(S->gUb[l], 0, c * 4, st); cudaMemsetAsync(S->gLb[l], 0, c * 4, st);
+            cudaMemsetAsync(S->dpb[l], 0, c * 4, st); cudaMemsetAsync(S->zbar[l], 0, c * 4, st);
+        }
+        cudaMemsetAsync(S->nom_bar, 0, (size_t)C * wp0 * 4, st);
+        cudaMemsetAsync(S->rad_bar, 0, (size_t)C * wp0 * 4, st);
+        // ---- targets s = L .. 2
+        for (int s = L; s >= 2; --s) {
+            const bool is_out = (s == L);
+            const int rp = S->rows_pad[s], rk = S->rows_kind[s], nk = is_out ? 3 : 2;
+            if (!is_out) {
+                relax_vjp_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], S->lb[s],
+                                                                              S->ub[s], S->kUb[s], S->kLb[s], S->gUb[s], S->gLb[s],
+                                                                              S->dpb[s], S->lbar[s], S->ubar[s], S->zbar[s], 0);
+                ++*launches;
+            }
+            const float* yu = is_out ? S->ghi_p : S->ubar[s];
+            const float* yl = is_out ? S->glo_p : S->lbar[s];
+            seed_kernel<<<C, 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
+                                           S->Lbar[0], S->gapbar, S->rad_bar);
+            ++*launches;
+            int cur = 0;
+            for (int l = 1; l <= s - 1; ++l) {
+                GemmArgs g{};
+                g.M = C * rp; g.N = S->wp[l]; g.K = S->wp[l - 1];
+                g.A = S->Lbar[cur]; g.lda = S->wp[l - 1];
+                g.B = S->Wt[l]; g.ldb = S->rowsW[l];
+                g.C = S->Lbar[cur ^ 1]; g.ldc = S->wp[l];
+                g.rows_pad = rp; g.rows_kind = rk; g.nkinds = nk;
+                g.kU = S->kU[l]; g.kL = S->kL[l]; g.gU = S->gU[l]; g.gL = S->gL[l]; g.dphi = S->dphi[l]; g.ldp = S->wp[l];
+                g.lam_shared = (l == s - 1);
+                g.Lam = g.lam_shared ? S->W[s] : S->Lam[s][l];
+                g.ldl = S->wp[l];
+                g.gapbar = S->gapbar;
+                g.kUb = S->kUb[l]; g.kLb = S->kLb[l]; g.gUb = S->gUb[l]; g.gLb = S->gLb[l]; g.db = S->dpb[l];
+                g.write_c = (l < s - 1);
+                launch_gemm<AMODE_PLAIN, EPI_CHAIN_BWD>(g, st, launches);
+                cur ^= 1;
+            }
+        }
+        // ---- layer 1: l_1, u_1 = zhat_1 -+ |W_1| sigma
+        relax_vjp_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->lb[1], S->ub[1],
+                                                                      S->kUb[1], S->kLb[1], S->gUb[1], S->gLb[1], S->dpb[1],
+                                                                      S->lbar[1], S->ubar[1], S->zbar[1], 1);
+        diff_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->ubar[1], S->lbar[1], S->rad1, (size_t)C * S->wp[1]);
+        *launches += 2;
+        {
+            GemmArgs g = plain_args(C, wp0, S->wp[1], S->rad1, S->wp[1], S->Wabs1, wp0, S->rad_bar, wp0);
+            launch_gemm<AMODE_PLAIN, EPI_ACC>(g, st, launches);
+        }
+        // ---- nominal back-propagation: abar_{l-1} = zbar_l W_l; zbar_{l-1} += phi'(zhat_{l-1}) abar_{l-1}
+        for (int l = L - 1; l >= 1; --l) {
+            if (l > 1) {
+                GemmArgs g = plain_args(C, S->wp[l - 1], S->wp[l], S->zbar[l], S->wp[l], S->W[l], S->wp[l - 1], S->zbar[l - 1], S->wp[l - 1]);
+                g.dphi = S->dphi[l - 1]; g.ldp = S->wp[l - 1];
+                launch_gemm<AMODE_PLAIN, EPI_ACC_DPHI>(g, st, launches);
+            } else {
+                GemmArgs g = plain_args(C, wp0, S->wp[1], S->zbar[1], S->wp[1], S->W[1], wp0, S->nom_bar, wp0);
+                launch_gemm<AMODE_PLAIN, EPI_ACC>(g, st, launches);
+            }
+        }
+        write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,
+                                                                 grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in);
+        ++*launches;
+        S->last_tiles = 0;
+    }
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}

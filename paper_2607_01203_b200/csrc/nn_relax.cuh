@@ -1,0 +1,144 @@
+// nn_relax.cuh -- per-neuron linear relaxations  kL z + bL <= phi(z) <= kU z + bU  on [l, u]
+// (the activation step of CROWN, Thm 2 / eq. (18); the paper cites [26] and
+// gives no formulas -- DESIGN.md readings R8/R9), in "deviation form":
+//     gU = kU zhat + bU - phi(zhat) >= 0,   gL = kL zhat + bL - phi(zhat) <= 0
+// are the gaps of the two lines at the nominal pre-activation zhat.  O(width) work per layer, so it
+// is done in FP64 (removes the per-neuron cancellations) and stored as FP32.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace leb_nn {
+
+constexpr int ACT_RELU = 1, ACT_TANH = 2;
+constexpr int kBisect = 52;
+constexpr double kTanhD2Max = 0.76980035891950104;   // max |tanh''| = 4 / (3 sqrt 3)
+constexpr double kDegenerate = 1e-12;
+
+// how each line was built (needed again by the VJP)
+enum { LINE_ZERO = 0, LINE_IDENT, LINE_CHORD, LINE_TAN_MID, LINE_TAN_IMPL, LINE_RELU_LOW, LINE_DEGEN };
+
+struct Relax {
+    double kU, bU, kL, bL;
+    int cU, cL;        // LINE_* of the upper / lower line
+    double dU, dL;     // tangent points where applicable
+};
+
+__device__ __forceinline__ double th(double x) { return tanh(x); }
+__device__ __forceinline__ double th1(double x) { double t = tanh(x); return 1.0 - t * t; }
+__device__ __forceinline__ double th2(double x) { double t = tanh(x); return -2.0 * t * (1.0 - t * t); }
+
+__device__ inline Relax relax_relu(double l, double u) {
+    Relax r{};
+    if (u <= 0.0) { r.cU = r.cL = LINE_ZERO; return r; }
+    if (l >= 0.0) { r.kU = r.kL = 1.0; r.cU = r.cL = LINE_IDENT; return r; }
+    double w = u - l;
+    r.kU = u / w;
+    r.bU = -u * l / w;
+    r.cU = LINE_CHORD;
+    r.kL = (u > -l) ? 1.0 : 0.0;     // adaptive lower slope; tie u == -l -> 0 (reading R8)
+    r.bL = 0.0;
+    r.cL = LINE_RELU_LOW;
+    return r;
+}
+
+// tangent point of the upper line through (l, tanh l), l < 0 < u: root of
+// h(d) = t'(d)(d - l) - (t(d) - t(l)) on (0, u); h > 0 left of the root.  Returns the bracket end
+// d >= d*, the side on which the tangent stays above tanh on [l, u] (sound side).
+__device__ inline double tangent_upper(double l, double u) {
+    double tl = th(l), a = 0.0, b = u;
+    for (int it = 0; it < kBisect; ++it) {
+        double m = 0.5 * (a + b), t = tanh(m);
+        if ((1.0 - t * t) * (m - l) - (t - tl) > 0.0) a = m; else b = m;
+    }
+    return b;
+}
+// tangent point of the lower line through (u, tanh u): root of h(d) = t'(d)(u - d) - (t(u) - t(d))
+// on (l, 0); h > 0 right of the root.  Returns the end d <= d* (sound side).
+__device__ inline double tangent_lower(double l, double u) {
+    double tu = th(u), a = l, b = 0.0;
+    for (int it = 0; it < kBisect; ++it) {
+        double m = 0.5 * (a + b), t = tanh(m);
+        if ((1.0 - t * t) * (u - m) - (tu - t) > 0.0) b = m; else a = m;
+    }
+    return a;
+}
+
+__device__ inline Relax relax_tanh(double l, double u) {
+    Relax r{};
+    double w = u - l;
+    if (w < kDegenerate) {           // point interval: tangent at the midpoint, widened by the curvature bound
+        double d = 0.5 * (l + u), k = th1(d), b = th(d) - k * d, e = 0.5 * kTanhD2Max * w * w;
+        r.kU = r.kL = k; r.bU = b + e; r.bL = b - e; r.cU = r.cL = LINE_DEGEN; r.dU = r.dL = d;
+        return r;
+    }
+    double tl = th(l), tu = th(u);
+    double kc = (tu - tl) / w, bc = tl - kc * l;
+    if (l >= 0.0) {                  // concave part: tangent above, chord below
+        double d = 0.5 * (l + u), k = th1(d);
+        r.kU = k; r.bU = th(d) - k * d; r.cU = LINE_TAN_MID; r.dU = d;
+        r.kL = kc; r.bL = bc; r.cL = LINE_CHORD;
+        return r;
+    }
+    if (u <= 0.0) {                  // convex part: chord above, tangent below
+        double d = 0.5 * (l + u), k = th1(d);
+        r.kL = k; r.bL = th(d) - k * d; r.cL = LINE_TAN_MID; r.dL = d;
+        r.kU = kc; r.bU = bc; r.cU = LINE_CHORD;
+        return r;
+    }
+    if (kc <= 1.0 - tu * tu) { r.kU = kc; r.bU = bc; r.cU = LINE_CHORD; }
+    else { double d = tangent_upper(l, u), k = th1(d); r.kU = k; r.bU = th(d) - k * d; r.cU = LINE_TAN_IMPL; r.dU = d; }
+    if (kc <= 1.0 - tl * tl) { r.kL = kc; r.bL = bc; r.cL = LINE_CHORD; }
+    else { double d = tangent_lower(l, u), k = th1(d); r.kL = k; r.bL = th(d) - k * d; r.cL = LINE_TAN_IMPL; r.dL = d; }
+    return r;
+}
+
+__device__ inline Relax relax_any(int act, double l, double u) { return act == ACT_RELU ? relax_relu(l, u) : relax_tanh(l, u); }
+
+__device__ __forceinline__ double act_f(int act, double z) { return act == ACT_RELU ? fmax(z, 0.0) : tanh(z); }
+__device__ __forceinline__ double act_d1(int act, double z) { return act == ACT_RELU ? (z > 0.0 ? 1.0 : 0.0) : th1(z); }   // phi'(0)=0 (R12)
+__device__ __forceinline__ double act_d2(int act, double z) { return act == ACT_RELU ? 0.0 : th2(z); }
+
+// Adjoint of one line's (k, b) with respect to (l, u):  (lb, ub) += d(k,b)/d(l,u)^T (kb, bb).
+__device__ inline void line_vjp(int act, int how, bool upper, double l, double u, double d, double kb, double bb,
+                                double& lb, double& ub) {
+    switch (how) {
+        case LINE_CHORD: {
+            double w = u - l;
+            if (act == ACT_RELU) {      // k = u/(u-l), b = -u l/(u-l)
+                double w2 = w * w;
+                lb += kb * (u / w2) + bb * (-u * u / w2);
+                ub += kb * (-l / w2) + bb * (l * l / w2);
+            } else {                    // k = (t(u)-t(l))/(u-l), b = t(l) - k l
+                double k = (th(u) - th(l)) / w;
+                double dk_du = (th1(u) - k) / w, dk_dl = (k - th1(l)) / w;
+                double db_dl = th1(l) - k - l * dk_dl, db_du = -l * dk_du;
+                lb += kb * dk_dl + bb * db_dl;
+                ub += kb * dk_du + bb * db_du;
+            }
+            break;
+        }
+        case LINE_TAN_MID: {            // k = t'(d), b = t(d) - t'(d) d, d = (l+u)/2
+            double ad = th2(d) * (kb - d * bb);
+            lb += 0.5 * ad;
+            ub += 0.5 * ad;
+            break;
+        }
+        case LINE_TAN_IMPL: {           // tangent point defined implicitly by l (upper) or by u (lower)
+            double ad = th2(d) * (kb - d * bb);
+            if (upper) lb += ad * (th1(d) - th1(l)) / (th2(d) * (d - l));
+            else ub += ad * (th1(u) - th1(d)) / (th2(d) * (u - d));
+            break;
+        }
+        case LINE_DEGEN: {              // b = t(d) - k d +- c (u-l)^2, c = kTanhD2Max/2
+            double ad = th2(d) * (kb - d * bb);
+            double dw = kTanhD2Max * (u - l) * bb * (upper ? 1.0 : -1.0);
+            lb += 0.5 * ad - dw;
+            ub += 0.5 * ad + dw;
+            break;
+        }
+        default: break;                 // LINE_ZERO, LINE_IDENT, LINE_RELU_LOW: constants
+    }
+}
+
+}  // namespace leb_nn

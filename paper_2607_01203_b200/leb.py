@@ -1,0 +1,248 @@
+"""Thin Python binding of the C ABI in include/leb.h (argument marshalling only).
+
+Every numerical step runs in libleb.so's sm_100a kernels; torch is used for device memory and
+streams.  There is no CPU fallback: if the library is missing or no CUDA device is present the
+calls raise.  Function names mirror the C entry points.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libleb.so")
+
+LEB_OK = 0
+LEB_ERR_UNSUPPORTED = 5
+LEB_ERR_STATE = 8
+FLAG_NO_MARGIN = 1
+FLAG_FFMA_ONLY = 2
+FLAG_HOST_IO = 4
+
+EXPORTS = [
+    "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
+    "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_launch_count",
+]
+
+
+class LebError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: leb_status {status} ({_status_str(status)})")
+
+
+class _AnalyticModel(ctypes.Structure):
+    _fields_ = [("model_id", ctypes.c_int), ("integ", ctypes.c_int), ("n_units", ctypes.c_int),
+                ("dt", ctypes.c_float), ("mass", ctypes.c_float), ("g", ctypes.c_float),
+                ("Jx", ctypes.c_float), ("Jy", ctypes.c_float), ("Jz", ctypes.c_float),
+                ("k1", ctypes.c_float), ("k3", ctypes.c_float)]
+
+
+class _Mlp(ctypes.Structure):
+    _fields_ = [("n_layers", ctypes.c_int), ("dims", ctypes.POINTER(ctypes.c_int)),
+                ("W", ctypes.POINTER(ctypes.c_void_p)), ("b", ctypes.POINTER(ctypes.c_void_p)),
+                ("act", ctypes.c_int), ("residual", ctypes.c_int), ("weights_on_host", ctypes.c_int)]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libleb.so (built in-tree by paper_2607_01203_b200.build); fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not built: run `python -m paper_2607_01203_b200.build` (no CPU fallback exists)")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name in EXPORTS:
+            getattr(lib, name).restype = ctypes.c_int
+        lib.leb_status_str.restype = ctypes.c_char_p
+        lib.leb_launch_count.restype = ctypes.c_longlong
+        lib.leb_launch_count.argtypes = [ctypes.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _status_str(s: int) -> str:
+    try:
+        return load_library().leb_status_str(ctypes.c_int(s)).decode()
+    except Exception:
+        return "?"
+
+
+def _chk(status: int, where: str):
+    if status != LEB_OK:
+        raise LebError(status, where)
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream_ptr(device) -> ctypes.c_void_p:
+    return ctypes.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _check_f32(*tensors):
+    for t in tensors:
+        if t is not None and (t.dtype != torch.float32 or not t.is_contiguous()):
+            raise ValueError("tensors must be contiguous float32")
+
+
+class Context:
+    """Owns one leb_ctx on one CUDA device.  Inputs are CUDA tensors on that device, or (host_io=True
+    calls) CPU tensors, ideally pinned."""
+
+    def __init__(self, device: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the LEB library has no CPU fallback")
+        self.lib = load_library()
+        self.device = int(device)
+        self._ctx = ctypes.c_void_p()
+        _chk(self.lib.leb_create(ctypes.byref(self._ctx), ctypes.c_int(self.device)), "leb_create")
+        self.n = self.N = None
+        self.nn_n = self.nn_N = None
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx:
+            self.lib.leb_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ model set-up
+    def leb_set_analytic(self, model_id: int, integ: int, dt: float, n_units: int = 1, mass=1.0, g=9.81,
+                         Jx=0.010, Jy=0.015, Jz=0.020, k1=1.0, k3=0.1):
+        m = _AnalyticModel(int(model_id), int(integ), int(n_units), dt, mass, g, Jx, Jy, Jz, k1, k3)
+        _chk(self.lib.leb_set_analytic(self._ctx, ctypes.byref(m)), "leb_set_analytic")
+        if model_id == 1:
+            self.n, self.N = 3, 5
+        else:
+            u = n_units if model_id == 3 else 1
+            self.n, self.N = 12 * u, 16 * u
+
+    def leb_set_mlp(self, dims: Sequence[int], W: Sequence[torch.Tensor], b: Sequence[torch.Tensor], act: int,
+                    residual: bool = True):
+        L = len(W)
+        assert len(dims) == L + 1 and len(b) == L
+        on_host = not W[0].is_cuda
+        W = [w.contiguous().float() for w in W]
+        b = [x.contiguous().float() for x in b]
+        for l in range(L):
+            assert tuple(W[l].shape) == (dims[l + 1], dims[l]) and tuple(b[l].shape) == (dims[l + 1],)
+            assert W[l].is_cuda != on_host and b[l].is_cuda != on_host
+        dims_a = (ctypes.c_int * (L + 1))(*[int(d) for d in dims])
+        W_a = (ctypes.c_void_p * L)(*[w.data_ptr() for w in W])
+        b_a = (ctypes.c_void_p * L)(*[x.data_ptr() for x in b])
+        m = _Mlp(L, dims_a, W_a, b_a, int(act), int(bool(residual)), int(on_host))
+        _chk(self.lib.leb_set_mlp(self._ctx, ctypes.byref(m), _stream_ptr(self.device)), "leb_set_mlp")
+        self.nn_N, self.nn_n = int(dims[0]), int(dims[-1])
+
+    def leb_set_nn_chunk(self, tiles: int):
+        _chk(self.lib.leb_set_nn_chunk(self._ctx, ctypes.c_int(int(tiles))), "leb_set_nn_chunk")
+
+    # ------------------------------------------------------------------ helpers
+    def _out(self, like: torch.Tensor, shape, host_io: bool):
+        if host_io:
+            return torch.empty(shape, dtype=torch.float32, pin_memory=True)
+        return torch.empty(shape, dtype=torch.float32, device=like.device)
+
+    @staticmethod
+    def _bt(nom: torch.Tensor):
+        if nom.dim() != 3:
+            raise ValueError("expected [B, T, ld] tensors")
+        return int(nom.shape[0]), int(nom.shape[1]), int(nom.shape[2])
+
+    # ------------------------------------------------------------------ entry points
+    def leb_analytic_fwd(self, nom, rad, r_lo=None, r_hi=None, flags: int = 0):
+        _check_f32(nom, rad, r_lo, r_hi)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        if r_lo is None:
+            r_lo = self._out(nom, (B, T, self.n), host)
+            r_hi = self._out(nom, (B, T, self.n), host)
+        _chk(self.lib.leb_analytic_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), None, ld_in, _ptr(r_lo), _ptr(r_hi),
+                                       int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_fwd")
+        return r_lo, r_hi
+
+    def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = FLAG_NO_MARGIN):
+        _check_f32(nom, rad, J, r_lo, r_hi, margin)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        if r_lo is None:
+            r_lo = self._out(nom, (B, T, self.nn_n), host)
+            r_hi = self._out(nom, (B, T, self.nn_n), host)
+        _chk(self.lib.leb_nn_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), None, _ptr(J), ld_in, _ptr(r_lo), _ptr(r_hi),
+                                 _ptr(margin), int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_nn_fwd")
+        return r_lo, r_hi
+
+    def leb_vjp(self, kind: int, nom, rad, g_lo, g_hi, grad_nom=None, grad_rad=None, flags: int = FLAG_NO_MARGIN):
+        _check_f32(nom, rad, g_lo, g_hi, grad_nom, grad_rad)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        if grad_nom is None:
+            grad_nom = self._out(nom, (B, T, ld_in), host)
+            grad_rad = self._out(nom, (B, T, ld_in), host)
+        _chk(self.lib.leb_vjp(self._ctx, int(kind), B, T, _ptr(nom), _ptr(rad), _ptr(g_lo), _ptr(g_hi), ld_in,
+                              int(g_lo.shape[2]), _ptr(grad_nom), _ptr(grad_rad), ctypes.c_uint(flags),
+                              _stream_ptr(self.device)), "leb_vjp")
+        return grad_nom, grad_rad
+
+    def leb_zonotope_inflate(self, r_lo, r_hi, pad: float = 1e-6, E_diag=None, dense: bool = False, flags: int = 0):
+        _check_f32(r_lo, r_hi, E_diag)
+        B, T, n = self._bt(r_lo)
+        host = bool(flags & FLAG_HOST_IO)
+        c_bar = self._out(r_lo, (B, T, n), host)
+        R_diag = self._out(r_lo, (B, T, n), host)
+        Ebar = self._out(r_lo, (B, T, n, 2 * n), host) if dense else None
+        _chk(self.lib.leb_zonotope_inflate(self._ctx, B, T, n, _ptr(r_lo), _ptr(r_hi), _ptr(E_diag), ctypes.c_float(pad),
+                                           _ptr(c_bar), _ptr(R_diag), _ptr(Ebar), ctypes.c_uint(flags),
+                                           _stream_ptr(self.device)), "leb_zonotope_inflate")
+        return (c_bar, R_diag, Ebar) if dense else (c_bar, R_diag)
+
+    def leb_zonotope_inflate_vjp(self, gc, gR, flags: int = 0):
+        _check_f32(gc, gR)
+        B, T, n = self._bt(gc)
+        host = bool(flags & FLAG_HOST_IO)
+        g_lo = self._out(gc, (B, T, n), host)
+        g_hi = self._out(gc, (B, T, n), host)
+        _chk(self.lib.leb_zonotope_inflate_vjp(self._ctx, B, T, n, _ptr(gc), _ptr(gR), _ptr(g_lo), _ptr(g_hi),
+                                               ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_zonotope_inflate_vjp")
+        return g_lo, g_hi
+
+    def leb_domain_flag(self) -> int:
+        flag = ctypes.c_int(0)
+        _chk(self.lib.leb_domain_flag(self._ctx, ctypes.byref(flag), _stream_ptr(self.device)), "leb_domain_flag")
+        return int(flag.value)
+
+    def leb_nn_hidden_bounds(self, layer: int, tiles: int, width: int):
+        dev = torch.device("cuda", self.device)
+        l = torch.empty((tiles, width), dtype=torch.float32, device=dev)
+        u = torch.empty((tiles, width), dtype=torch.float32, device=dev)
+        _chk(self.lib.leb_nn_hidden_bounds(self._ctx, int(layer), _ptr(l), _ptr(u), _stream_ptr(self.device)),
+             "leb_nn_hidden_bounds")
+        return l, u
+
+    def leb_launch_count(self) -> int:
+        return int(self.lib.leb_launch_count(self._ctx))
+
+
+def context_for_workload(w, device: int = 0) -> Context:
+    """Context with the model of a workloads.Workload installed."""
+    ctx = Context(device)
+    if w.kind == "analytic":
+        a = w.analytic
+        ctx.leb_set_analytic(a.model_id, a.integ, a.dt, a.n_units, a.mass, a.g, a.Jx, a.Jy, a.Jz, a.k1, a.k3)
+    else:
+        dev = torch.device("cuda", device)
+        ctx.leb_set_mlp(w.mlp.dims, [torch.from_numpy(x).to(dev) for x in w.mlp.W],
+                        [torch.from_numpy(x).to(dev) for x in w.mlp.b], w.mlp.act, w.mlp.residual)
+    return ctx
