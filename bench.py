@@ -1,0 +1,293 @@
+#!/usr/bin/env python
+"""bench.py -- the LEB hot path on BASELINE.json's headline workload (config 5: 168-state tanh MLP,
+B=64 candidate trajectories x T=100 timesteps, forward + VJP), one process per GPU.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input (DESIGN.md
+"Measurement"): leb_nn_fwd -> leb_zonotope_inflate -> leb_zonotope_inflate_vjp -> leb_vjp.
+Rank 0 prints ONE JSON line.  `value` = bounded (timestep x state-dim) entries per second over all
+ranks with inputs resident in HBM; `e2e` = the same through the C ABI with host buffers
+(LEB_FLAG_HOST_IO: H2D/D2H copies inside the timed region); `roofline` = the dominant kernel's
+algorithmic flops / its CUDA-event time, measured during the timed steps; `cpu_baseline` = the
+oracle timed on this box's host cores on a bounded sample of the same workload.
+
+--impl reference times the oracle (oracle/nn_oracle.py, as it stands) instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bounded (timestep x state-dim) entries/sec incl. VJP"
+UNIT = "entries/s"
+CONFIG_ID = 5
+WORKLOAD = ("config5: MLP 224->512x4->168 tanh residual, Xavier-normal weights, B=64 x T=100 tiles per GPU, "
+            "radii U[0.005,0.03], forward + VJP")
+KC_NAMES = {0: "gemm_chain_fwd (CROWN back-substitution step)", 1: "gemm_chain_bwd (reverse-sweep step)"}
+
+
+def _clock_sampler(gpu_index: int):
+    q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    try:
+        return subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                 "-i", str(gpu_index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+    except Exception:
+        return None
+
+
+def _clock_summary(proc):
+    if proc is None:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+    proc.terminate()
+    try:
+        out, _ = proc.communicate(timeout=5)
+    except Exception:
+        proc.kill()
+        out = ""
+    sm, smax, reasons = [], [], set()
+    names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    for line in out.strip().splitlines():
+        f = [x.strip() for x in line.split(",")]
+        if len(f) < 7:
+            continue
+        try:
+            sm.append(float(f[0])); smax.append(float(f[1]))
+        except ValueError:
+            continue
+        for name, v in zip(names, f[3:7]):
+            if v.lower().startswith("active"):
+                reasons.add(name)
+    sm.sort()
+    return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(smax) if smax else None,
+            "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
+
+
+def _traffic(kernel_key: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = line.strip().split(",")
+        if len(f) >= 2 and f[0] == kernel_key:
+            try:
+                return float(f[1])
+            except ValueError:
+                return None
+    return None
+
+
+def _cpu_oracle_sample(w, tiles: int):
+    """Oracle forward + VJP on `tiles` seeded tiles of the workload; returns (entries/s, seconds, threads)."""
+    import numpy as np
+    from oracle import inflate_oracle, nn_oracle
+    threads = 1
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([int(i.get("num_threads", 1)) for i in threadpool_info()] + [1])
+    except Exception:
+        pass
+    idx = np.linspace(0, w.B * w.T - 1, tiles).astype(int)
+    nom, rad = w.nom.reshape(-1, w.N)[idx], w.rad.reshape(-1, w.N)[idx]
+    gc, gR = w.g_lo.reshape(-1, w.n)[idx], w.g_hi.reshape(-1, w.n)[idx]
+    t0 = time.perf_counter()
+    r_lo, r_hi = nn_oracle.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom, rad)
+    inflate_oracle.inflate(r_lo, r_hi, 1e-6)
+    g_lo, g_hi = inflate_oracle.inflate_vjp(gc, gR)
+    nn_oracle.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom, rad, g_lo, g_hi)
+    dt = time.perf_counter() - t0
+    return tiles * w.n / dt, dt, threads
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2607_01203_b200 import workloads as wl
+    w = wl.make_config(CONFIG_ID)
+    tiles_per_step = 3
+    for _ in range(args.warmup):
+        _cpu_oracle_sample(w, 1)
+    t0 = time.perf_counter()
+    threads = 1
+    for _ in range(args.steps):
+        _, _, threads = _cpu_oracle_sample(w, tiles_per_step)
+    dt = time.perf_counter() - t0
+    value = args.steps * tiles_per_step * w.n / dt
+    sample = f"{tiles_per_step} seeded tiles of config 5 per step (forward + fold + VJP), numpy FP64"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_01203_b200 import leb, sharding, workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the LEB library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    # weak scaling: every rank owns one full config-5 batch (B=64 x T=100); tiles are independent, so there
+    # is no collective on the data path
+    w = wl.make_config(CONFIG_ID)
+    ctx = leb.context_for_workload(w, local)
+    nom, rad = torch.from_numpy(w.nom).to(dev), torch.from_numpy(w.rad).to(dev)
+    gc, gR = torch.from_numpy(w.g_lo).to(dev), torch.from_numpy(w.g_hi).to(dev)     # cotangents of (c_bar, R_diag)
+    h_nom, h_rad = torch.from_numpy(w.nom).pin_memory(), torch.from_numpy(w.rad).pin_memory()
+    h_gc, h_gR = torch.from_numpy(w.g_lo).pin_memory(), torch.from_numpy(w.g_hi).pin_memory()
+
+    def step_device():
+        r_lo, r_hi = ctx.leb_nn_fwd(nom, rad)
+        ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
+        g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
+        return ctx.leb_vjp(1, nom, rad, g_lo, g_hi)
+
+    HOST = leb.FLAG_HOST_IO
+    e2e_bytes = {"h2d": 0, "d2h": 0}
+    pin = lambda *shape: torch.empty(shape, dtype=torch.float32, pin_memory=True)
+    hb = {k: pin(w.B, w.T, w.n) for k in ("r_lo", "r_hi", "c", "R", "g_lo", "g_hi")}
+    hb.update({k: pin(w.B, w.T, w.N) for k in ("gn", "gr")})
+
+    def step_host(count=False):
+        r_lo, r_hi = ctx.leb_nn_fwd(h_nom, h_rad, r_lo=hb["r_lo"], r_hi=hb["r_hi"], flags=leb.FLAG_NO_MARGIN | HOST)
+        c, R = ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6, flags=HOST, c_bar=hb["c"], R_diag=hb["R"])
+        g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(h_gc, h_gR, flags=HOST, g_lo=hb["g_lo"], g_hi=hb["g_hi"])
+        gn, gr = ctx.leb_vjp(1, h_nom, h_rad, g_lo, g_hi, grad_nom=hb["gn"], grad_rad=hb["gr"], flags=leb.FLAG_NO_MARGIN | HOST)
+        if count:
+            nb = lambda *ts: sum(t.numel() * t.element_size() for t in ts)
+            e2e_bytes["h2d"] = nb(h_nom, h_rad) + nb(r_lo, r_hi) + nb(h_gc, h_gR) + nb(h_nom, h_rad, g_lo, g_hi)
+            e2e_bytes["d2h"] = nb(r_lo, r_hi) + nb(c, R) + nb(g_lo, g_hi) + nb(gn, gr)
+        return gn, gr
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        step_device()
+    barrier()
+    sampler = _clock_sampler(local) if rank == 0 else None
+    ctx.leb_profile_reset()
+    ctx.leb_profile(True)
+    launches0 = ctx.leb_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step_device()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.leb_launch_count() - launches0
+    ctx.leb_profile(False)
+    kstats = {kc: ctx.leb_profile_read(kc) for kc in (0, 1, 5)}
+    clocks = _clock_summary(sampler) if rank == 0 else None
+    ms_max = sharding.max_over_ranks(ms, dev)
+    launches_total = int(sharding.sum_over_ranks(launches, dev))
+    entries_per_rank = w.entries * args.steps
+    value = world * entries_per_rank / (ms_max * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers
+    for _ in range(max(1, min(args.warmup, 2))):
+        step_host(count=True)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_host()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    dt_max = sharding.max_over_ranks(dt, dev)
+    e2e_value = world * entries_per_rank / dt_max
+
+    if rank == 0:
+        peaks = _peaks()
+        dom = max((0, 1), key=lambda kc: kstats[kc][0])
+        k_ms, k_flops, k_n = kstats[dom]
+        tot_ms = sum(kstats[kc][0] for kc in kstats)
+        sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+        # FP32 FFMA path: plain-ALU bound, peak = 148 SMs x 128 FP32 lanes x 2 flop x max SM clock
+        alu_peak = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+        achieved = (k_flops / 1e12) / (k_ms * 1e-3) if k_ms > 0 else 0.0
+        roofline = {"bound": "alu", "kernel": KC_NAMES[dom], "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                    "frac": achieved / alu_peak, "traffic": _traffic("chain_fwd" if dom == 0 else "chain_bwd"),
+                    "peak_source": f"148 SM x 128 lanes x 2 x {sm_max_mhz:.0f} MHz ({peaks['_source']} max SM clock)",
+                    "launches": k_n, "avg_launch_ms": k_ms / max(k_n, 1),
+                    "kernel_share_of_step": k_ms / ms if ms > 0 else None,
+                    "all_chain_gemm_share_of_step": (kstats[0][0] + kstats[1][0]) / ms if ms > 0 else None,
+                    "other_kernel": {"kernel": KC_NAMES[1 - dom], "achieved": (kstats[1 - dom][1] / 1e12) / max(kstats[1 - dom][0] * 1e-3, 1e-12),
+                                     "launches": kstats[1 - dom][2]},
+                    "algorithmic_tflop_per_step": (kstats[0][1] + kstats[1][1]) / 1e12 / max(args.steps, 1)}
+        cpu = None
+        if world == 1:
+            tiles = 12
+            v, secs, threads = _cpu_oracle_sample(w, tiles)
+            cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                   "sample": f"{tiles} seeded tiles of config 5 (forward + fold + VJP), {secs:.1f} s, numpy FP64"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_max / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOAD, "global_batch": 64 * world, "horizon": 100, "tiles": w.B * w.T * world,
+                           "parallelism": f"dp{world} (independent tiles, no collective)",
+                           "l2": "working set (>= 6 GB of coefficient blocks per chunk) exceeds the 126 MB L2; no flush needed",
+                           "mode": "value mode (LEB_FLAG_NO_MARGIN), FP32 FFMA contractions"},
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e_bytes["h2d"], "d2h_bytes_per_step": e2e_bytes["d2h"],
+                        "ms_per_step": 1e3 * dt_max / max(args.steps, 1)},
+                "gpu_launches": launches_total, "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -164,6 +164,18 @@ leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, voi
 /* Number of kernel launches the library has enqueued on this context so far. */
 long long leb_launch_count(const leb_ctx* ctx);
 
+/* Measurement aid (bench.py "roofline"): while enabled, every launch of
+ * the library's kernels is bracketed by CUDA events on the launching stream.  Kernel classes:
+ * 0 CROWN chain contraction (forward), 1 chain contraction (reverse sweep), 2 analytic forward,
+ * 3 analytic VJP, 4 zonotope fold, 5 other NN kernels' GEMMs.
+ * leb_profile_read synchronises `stream` and returns, for one class and since the last
+ * leb_profile_reset: the summed device time in ms, the summed ALGORITHMIC work (flops computed
+ * from the true, unpadded shapes; bytes for class 4; 0 for classes 2, 3) and the launch count. */
+leb_status leb_profile(leb_ctx* ctx, int enable);
+leb_status leb_profile_read(leb_ctx* ctx, int kernel_class, double* ms, double* work, long long* launches,
+                            void* stream);
+leb_status leb_profile_reset(leb_ctx* ctx);
+
 #ifdef __cplusplus
 }
 #endif

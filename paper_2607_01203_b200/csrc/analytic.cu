@@ -220,7 +220,7 @@ Model leb_make_model(const leb_analytic_model& m) {
 
 cudaError_t leb_launch_analytic_fwd(const Model& M, int tiles, const float* nom, const float* rad, int ld_in,
                                     float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
-                                    long long* launches) {
+                                    long long* launches, LebProf* prof) {
     if (tiles == 0) return cudaSuccess;
     size_t smem = 2 * (size_t)M.N * sizeof(float);
     // gridDim.y is limited to 65535: slice the tile range
@@ -230,10 +230,12 @@ cudaError_t leb_launch_analytic_fwd(const Model& M, int tiles, const float* nom,
         const float* s = rad + (size_t)t0 * ld_in;
         float* lo = r_lo + (size_t)t0 * ld_out;
         float* hi = r_hi + (size_t)t0 * ld_out;
+        prof->begin(LEB_KC_ANALYTIC_FWD, st);
         if (M.id == LEB_MODEL_UNICYCLE)
             analytic_fwd_kernel<3, true><<<dim3(1, nt), kThreads, smem, st>>>(M, a, s, ld_in, lo, hi, ld_out, domain_flag);
         else
             analytic_fwd_kernel<12, false><<<dim3(M.n_units, nt), kThreads, smem, st>>>(M, a, s, ld_in, lo, hi, ld_out, domain_flag);
+        prof->end(LEB_KC_ANALYTIC_FWD, st, 0.0);
         ++*launches;
     }
     return cudaGetLastError();
@@ -241,7 +243,7 @@ cudaError_t leb_launch_analytic_fwd(const Model& M, int tiles, const float* nom,
 
 cudaError_t leb_launch_analytic_vjp(const Model& M, int tiles, const float* nom, const float* rad, const float* g_lo,
                                     const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad,
-                                    int* domain_flag, cudaStream_t st, long long* launches) {
+                                    int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
     if (tiles == 0) return cudaSuccess;
     size_t smem = 2 * (size_t)M.N * sizeof(float);
     size_t total = (size_t)tiles * M.N;
@@ -250,6 +252,7 @@ cudaError_t leb_launch_analytic_vjp(const Model& M, int tiles, const float* nom,
     for (int t0 = 0; t0 < tiles; t0 += 65535) {
         int nt = tiles - t0 < 65535 ? tiles - t0 : 65535;
         size_t oi = (size_t)t0 * ld_in, oo = (size_t)t0 * ld_out;
+        prof->begin(LEB_KC_ANALYTIC_VJP, st);
         if (M.id == LEB_MODEL_UNICYCLE)
             analytic_vjp_kernel<3, true><<<dim3(1, nt), kThreads, smem, st>>>(M, nom + oi, rad + oi, g_lo + oo, g_hi + oo, ld_in,
                                                                              ld_out, grad_nom + oi, grad_rad + oi, domain_flag);
@@ -257,6 +260,7 @@ cudaError_t leb_launch_analytic_vjp(const Model& M, int tiles, const float* nom,
             analytic_vjp_kernel<12, false><<<dim3(M.n_units, nt), kThreads, smem, st>>>(M, nom + oi, rad + oi, g_lo + oo, g_hi + oo,
                                                                                        ld_in, ld_out, grad_nom + oi, grad_rad + oi,
                                                                                        domain_flag);
+        prof->end(LEB_KC_ANALYTIC_VJP, st, 0.0);
         ++*launches;
     }
     return cudaGetLastError();

@@ -13,6 +13,7 @@ struct leb_ctx {
     NnState* nn = nullptr;
     int* domain_flag = nullptr;     // device
     long long launches = 0;
+    LebProf prof;
     // staging for LEB_FLAG_HOST_IO (grown on demand)
     float* stage[8] = {nullptr};
     size_t stage_bytes[8] = {0};
@@ -104,6 +105,7 @@ leb_status leb_destroy(leb_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     leb_nn_destroy(c->nn);
+    c->prof.destroy();
     for (int i = 0; i < 8; ++i) if (c->stage[i]) cudaFree(c->stage[i]);
     if (c->domain_flag) cudaFree(c->domain_flag);
     delete c;
@@ -152,7 +154,7 @@ leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const fl
     float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
     float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
-    if (leb_launch_analytic_fwd(c->model, (int)tiles, d_nom, d_rad, ld_in, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches) != cudaSuccess)
+    if (leb_launch_analytic_fwd(c->model, (int)tiles, d_nom, d_rad, ld_in, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches, &c->prof) != cudaSuccess)
         return LEB_ERR_CUDA;
     out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
     out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
@@ -180,7 +182,7 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
     float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
     float* d_mg = out_ptr(c, 5, margin, tiles * ld_out, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
-    s = leb_nn_forward(c->nn, (int)tiles, d_nom, d_rad, d_J, ld_in, d_lo, d_hi, d_mg, ld_out, flags, c->domain_flag, st, &c->launches);
+    s = leb_nn_forward(c->nn, (int)tiles, d_nom, d_rad, d_J, ld_in, d_lo, d_hi, d_mg, ld_out, flags, c->domain_flag, st, &c->launches, &c->prof);
     if (s != LEB_OK) return s;
     out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
     out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
@@ -217,10 +219,10 @@ leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const f
     if (!ok) return LEB_ERR_NOMEM;
     if (kind == 0) {
         if (leb_launch_analytic_vjp(c->model, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, c->domain_flag, st,
-                                    &c->launches) != cudaSuccess)
+                                    &c->launches, &c->prof) != cudaSuccess)
             return LEB_ERR_CUDA;
     } else {
-        s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, flags, c->domain_flag, st, &c->launches);
+        s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, flags, c->domain_flag, st, &c->launches, &c->prof);
         if (s != LEB_OK) return s;
     }
     out_copy(grad_nom, d_gn, tiles * ld_in, host, st, &ok);
@@ -245,7 +247,7 @@ leb_status leb_zonotope_inflate(leb_ctx* c, int B, int T, int n, const float* r_
     float* d_R = out_ptr(c, 3, R_diag, rows, host, &ok);
     float* d_Eb = out_ptr(c, 5, Ebar_dense, rows * 2 * n, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
-    if (leb_launch_inflate(rows, n, d_lo, d_hi, d_E, pad, d_c, d_R, d_Eb, st, &c->launches) != cudaSuccess) return LEB_ERR_CUDA;
+    if (leb_launch_inflate(rows, n, d_lo, d_hi, d_E, pad, d_c, d_R, d_Eb, st, &c->launches, &c->prof) != cudaSuccess) return LEB_ERR_CUDA;
     out_copy(c_bar, d_c, rows, host, st, &ok);
     out_copy(R_diag, d_R, rows, host, st, &ok);
     out_copy(Ebar_dense, d_Eb, rows * 2 * n, host, st, &ok);
@@ -292,5 +294,36 @@ leb_status leb_nn_hidden_bounds(leb_ctx* c, int layer, float* l, float* u, void*
 }
 
 long long leb_launch_count(const leb_ctx* c) { return c ? c->launches : 0; }
+
+leb_status leb_profile(leb_ctx* c, int enable) {
+    if (!c) return LEB_ERR_ARG;
+    c->prof.on = enable != 0;
+    return LEB_OK;
+}
+
+leb_status leb_profile_read(leb_ctx* c, int kernel_class, double* ms, double* work, long long* launches, void* stream) {
+    if (!c || !ms || !work || !launches) return LEB_ERR_ARG;
+    if (kernel_class < 0 || kernel_class >= LEB_KC_COUNT) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return LEB_ERR_CUDA;
+    double total = 0.0;
+    for (size_t i = 0; i < c->prof.used; ++i) {
+        if (c->prof.recs[i].kc != kernel_class) continue;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, c->prof.recs[i].a, c->prof.recs[i].b) != cudaSuccess) return LEB_ERR_CUDA;
+        total += t;
+    }
+    *ms = total;
+    *work = c->prof.work[kernel_class];
+    *launches = c->prof.count[kernel_class];
+    return LEB_OK;
+}
+
+leb_status leb_profile_reset(leb_ctx* c) {
+    if (!c) return LEB_ERR_ARG;
+    c->prof.used = 0;
+    for (int k = 0; k < LEB_KC_COUNT; ++k) { c->prof.work[k] = 0.0; c->prof.count[k] = 0; }
+    return LEB_OK;
+}
 
 }  // extern "C"

@@ -97,16 +97,21 @@ inline unsigned grid_for(size_t work, int threads) {
 }  // namespace
 
 cudaError_t leb_launch_inflate(size_t rows, int n, const float* r_lo, const float* r_hi, const float* E_diag, float pad,
-                               float* c_bar, float* R_diag, float* Ebar_dense, cudaStream_t st, long long* launches) {
+                               float* c_bar, float* R_diag, float* Ebar_dense, cudaStream_t st, long long* launches,
+                               LebProf* prof) {
     if (rows == 0) return cudaSuccess;
     int vec = al16(r_lo) && al16(r_hi) && al16(c_bar) && al16(R_diag);
     size_t work = vec ? rows / 4 + 1 : rows;
+    prof->begin(LEB_KC_INFLATE, st);
     inflate_kernel<<<grid_for(work, 256), 256, 0, st>>>(rows, r_lo, r_hi, pad, c_bar, R_diag, vec);
+    prof->end(LEB_KC_INFLATE, st, 16.0 * (double)rows);   // algorithmic bytes: 2 arrays in, 2 out
     ++*launches;
     if (Ebar_dense) {
         int v2 = al16(Ebar_dense) && ((2 * n) % 4 == 0);
         size_t w2 = v2 ? rows * (size_t)(2 * n / 4) : rows * (size_t)(2 * n);
+        prof->begin(LEB_KC_INFLATE, st);
         ebar_kernel<<<grid_for(w2, 256), 256, 0, st>>>(rows, n, R_diag, E_diag, Ebar_dense, v2);
+        prof->end(LEB_KC_INFLATE, st, 4.0 * (double)rows * (2.0 * n + 1.0));
         ++*launches;
     }
     return cudaGetLastError();

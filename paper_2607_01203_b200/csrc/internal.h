@@ -4,20 +4,60 @@
 #include <stddef.h>
 #include "../../include/leb.h"
 
+#include <vector>
+
 namespace leb_an { struct Model; }
+
+// ---- profiling aid (leb_profile / leb_profile_read): CUDA events around the launches of each
+// kernel class, on the launching stream, so that bench.py can report the dominant kernel's average
+// launch duration measured live over the timed region.
+enum { LEB_KC_CHAIN_FWD = 0, LEB_KC_CHAIN_BWD = 1, LEB_KC_ANALYTIC_FWD = 2, LEB_KC_ANALYTIC_VJP = 3,
+       LEB_KC_INFLATE = 4, LEB_KC_NN_OTHER = 5, LEB_KC_COUNT = 6 };
+struct LebProf {
+    bool on = false;
+    struct Rec { cudaEvent_t a, b; int kc; };
+    std::vector<Rec> recs;        // pool (events are reused after leb_profile_read)
+    size_t used = 0;
+    double work[LEB_KC_COUNT] = {0};   // algorithmic flops (or bytes for LEB_KC_INFLATE)
+    long long count[LEB_KC_COUNT] = {0};
+    void begin(int kc, cudaStream_t st) {
+        if (!on) return;
+        if (used == recs.size()) {
+            Rec r{};
+            cudaEventCreate(&r.a);
+            cudaEventCreate(&r.b);
+            recs.push_back(r);
+        }
+        recs[used].kc = kc;
+        cudaEventRecord(recs[used].a, st);
+    }
+    void end(int kc, cudaStream_t st, double w) {
+        if (!on) return;
+        cudaEventRecord(recs[used].b, st);
+        ++used;
+        work[kc] += w;
+        ++count[kc];
+    }
+    void destroy() {
+        for (auto& r : recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+        recs.clear();
+        used = 0;
+    }
+};
 
 // ---- analytic path (analytic.cu)
 leb_an::Model leb_make_model(const leb_analytic_model& m);
 cudaError_t leb_launch_analytic_fwd(const leb_an::Model& M, int tiles, const float* nom, const float* rad, int ld_in,
                                     float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
-                                    long long* launches);
+                                    long long* launches, LebProf* prof);
 cudaError_t leb_launch_analytic_vjp(const leb_an::Model& M, int tiles, const float* nom, const float* rad, const float* g_lo,
                                     const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad,
-                                    int* domain_flag, cudaStream_t st, long long* launches);
+                                    int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
 
 // ---- zonotope fold (inflate.cu)
 cudaError_t leb_launch_inflate(size_t rows, int n, const float* r_lo, const float* r_hi, const float* E_diag, float pad,
-                               float* c_bar, float* R_diag, float* Ebar_dense, cudaStream_t st, long long* launches);
+                               float* c_bar, float* R_diag, float* Ebar_dense, cudaStream_t st, long long* launches,
+                               LebProf* prof);
 cudaError_t leb_launch_inflate_vjp(size_t count, const float* gc, const float* gR, float* g_lo, float* g_hi,
                                    cudaStream_t st, long long* launches);
 
@@ -32,8 +72,8 @@ int leb_nn_n(const NnState*);
 int leb_nn_N(const NnState*);
 leb_status leb_nn_forward(NnState*, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
                           float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
-                          long long* launches);
+                          long long* launches, LebProf* prof);
 leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
                       int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
-                      cudaStream_t st, long long* launches);
+                      cudaStream_t st, long long* launches, LebProf* prof);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);

@@ -55,6 +55,7 @@ struct NnState {
           *dpb[kMaxLayers] = {nullptr}, *zbar[kMaxLayers] = {nullptr}, *lbar[kMaxLayers] = {nullptr}, *ubar[kMaxLayers] = {nullptr};
     float *Lbar[2] = {nullptr, nullptr}, *gapbar = nullptr, *nom_bar = nullptr, *rad_bar = nullptr, *glo_p = nullptr, *ghi_p = nullptr;
     int last_tiles = 0;
+    LebProf* prof = nullptr;
 };
 
 namespace {
@@ -304,10 +305,13 @@ inline unsigned gs_grid(size_t work) {
 // ------------------------------------------------------------------------------------------
 // GEMM launch helpers
 // ------------------------------------------------------------------------------------------
+// kc / flops: kernel class and algorithmic flops (true, unpadded dims) for the profiling aid
 template <int AMODE, int EPI>
-void launch_gemm(const GemmArgs& g, cudaStream_t st, long long* launches) {
+void launch_gemm(NnState* S, const GemmArgs& g, cudaStream_t st, long long* launches, int kc = LEB_KC_NN_OTHER, double flops = 0.0) {
     dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM);
+    S->prof->begin(kc, st);
     gemm_ffma_kernel<AMODE, EPI><<<grid, GT, 0, st>>>(g);
+    S->prof->end(kc, st, flops);
     ++*launches;
 }
 
@@ -410,13 +414,13 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
     for (int l = 1; l < L; ++l) {
         GemmArgs g = plain_args(C, S->wp[l], S->wp[l - 1], a_prev, S->wp[l - 1], S->Wt[l], S->wp[l], S->zhat[l], S->wp[l]);
         g.bias = S->bias[l]; g.ahat = S->ahat[l]; g.dphi_out = S->dphi[l]; g.act = S->act;
-        launch_gemm<AMODE_PLAIN, EPI_NOMINAL>(g, st, launches);
+        launch_gemm<AMODE_PLAIN, EPI_NOMINAL>(S, g, st, launches);
         a_prev = S->ahat[l];
     }
     // ---- N2 layer-1 interval bounds: rad1 = |W_1| sigma
     {
         GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
-        launch_gemm<AMODE_PLAIN, EPI_STORE>(g, st, launches);
+        launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g, st, launches);
         relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->rad1, S->lb[1],
                                                                       S->ub[1], S->kU[1], S->kL[1], S->gU[1], S->gL[1]);
         ++*launches;
@@ -437,7 +441,8 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
             g.rows_pad = rp; g.rows_kind = rk; g.nkinds = nk;
             g.kU = S->kU[l]; g.kL = S->kL[l]; g.gU = S->gU[l]; g.gL = S->gL[l]; g.dphi = S->dphi[l]; g.ldp = S->wp[l];
             g.gap = S->gap[s]; g.gap_init = (l == s - 1);
-            launch_gemm<AMODE_CHAIN, EPI_STORE>(g, st, launches);
+            launch_gemm<AMODE_CHAIN, EPI_STORE>(S, g, st, launches, LEB_KC_CHAIN_FWD,
+                                                2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1]);
         }
         if (!is_out) {
             size_t warps = (size_t)C * rk;
@@ -557,7 +562,8 @@ leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long lo
 // ------------------------------------------------------------------------------------------
 leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
                           float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
-                          long long* launches) {
+                          long long* launches, LebProf* prof) {
+    S->prof = prof;
     if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;   // certified mode: see DESIGN.md (N6)
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, false);
@@ -601,8 +607,9 @@ leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStre
 // ------------------------------------------------------------------------------------------
 leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
                       int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
-                      cudaStream_t st, long long* launches) {
+                      cudaStream_t st, long long* launches, LebProf* prof) {
     (void)flags; (void)domain_flag;
+    S->prof = prof;
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;
@@ -654,7 +661,8 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                 g.gapbar = S->gapbar;
                 g.kUb = S->kUb[l]; g.kLb = S->kLb[l]; g.gUb = S->gUb[l]; g.gLb = S->gLb[l]; g.db = S->dpb[l];
                 g.write_c = (l < s - 1);
-                launch_gemm<AMODE_PLAIN, EPI_CHAIN_BWD>(g, st, launches);
+                launch_gemm<AMODE_PLAIN, EPI_CHAIN_BWD>(S, g, st, launches, LEB_KC_CHAIN_BWD,
+                                                        2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1]);
                 cur ^= 1;
             }
         }
@@ -666,17 +674,17 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         *launches += 2;
         {
             GemmArgs g = plain_args(C, wp0, S->wp[1], S->rad1, S->wp[1], S->Wabs1, wp0, S->rad_bar, wp0);
-            launch_gemm<AMODE_PLAIN, EPI_ACC>(g, st, launches);
+            launch_gemm<AMODE_PLAIN, EPI_ACC>(S, g, st, launches);
         }
         // ---- nominal back-propagation: abar_{l-1} = zbar_l W_l; zbar_{l-1} += phi'(zhat_{l-1}) abar_{l-1}
         for (int l = L - 1; l >= 1; --l) {
             if (l > 1) {
                 GemmArgs g = plain_args(C, S->wp[l - 1], S->wp[l], S->zbar[l], S->wp[l], S->W[l], S->wp[l - 1], S->zbar[l - 1], S->wp[l - 1]);
                 g.dphi = S->dphi[l - 1]; g.ldp = S->wp[l - 1];
-                launch_gemm<AMODE_PLAIN, EPI_ACC_DPHI>(g, st, launches);
+                launch_gemm<AMODE_PLAIN, EPI_ACC_DPHI>(S, g, st, launches);
             } else {
                 GemmArgs g = plain_args(C, wp0, S->wp[1], S->zbar[1], S->wp[1], S->W[1], wp0, S->nom_bar, wp0);
-                launch_gemm<AMODE_PLAIN, EPI_ACC>(g, st, launches);
+                launch_gemm<AMODE_PLAIN, EPI_ACC>(S, g, st, launches);
             }
         }
         write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,

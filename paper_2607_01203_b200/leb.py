@@ -25,7 +25,8 @@ FLAG_HOST_IO = 4
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_launch_count",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_profile_reset",
 ]
 
 
@@ -196,24 +197,27 @@ class Context:
                               _stream_ptr(self.device)), "leb_vjp")
         return grad_nom, grad_rad
 
-    def leb_zonotope_inflate(self, r_lo, r_hi, pad: float = 1e-6, E_diag=None, dense: bool = False, flags: int = 0):
-        _check_f32(r_lo, r_hi, E_diag)
+    def leb_zonotope_inflate(self, r_lo, r_hi, pad: float = 1e-6, E_diag=None, dense: bool = False, flags: int = 0,
+                             c_bar=None, R_diag=None):
+        _check_f32(r_lo, r_hi, E_diag, c_bar, R_diag)
         B, T, n = self._bt(r_lo)
         host = bool(flags & FLAG_HOST_IO)
-        c_bar = self._out(r_lo, (B, T, n), host)
-        R_diag = self._out(r_lo, (B, T, n), host)
+        if c_bar is None:
+            c_bar = self._out(r_lo, (B, T, n), host)
+            R_diag = self._out(r_lo, (B, T, n), host)
         Ebar = self._out(r_lo, (B, T, n, 2 * n), host) if dense else None
         _chk(self.lib.leb_zonotope_inflate(self._ctx, B, T, n, _ptr(r_lo), _ptr(r_hi), _ptr(E_diag), ctypes.c_float(pad),
                                            _ptr(c_bar), _ptr(R_diag), _ptr(Ebar), ctypes.c_uint(flags),
                                            _stream_ptr(self.device)), "leb_zonotope_inflate")
         return (c_bar, R_diag, Ebar) if dense else (c_bar, R_diag)
 
-    def leb_zonotope_inflate_vjp(self, gc, gR, flags: int = 0):
-        _check_f32(gc, gR)
+    def leb_zonotope_inflate_vjp(self, gc, gR, flags: int = 0, g_lo=None, g_hi=None):
+        _check_f32(gc, gR, g_lo, g_hi)
         B, T, n = self._bt(gc)
         host = bool(flags & FLAG_HOST_IO)
-        g_lo = self._out(gc, (B, T, n), host)
-        g_hi = self._out(gc, (B, T, n), host)
+        if g_lo is None:
+            g_lo = self._out(gc, (B, T, n), host)
+            g_hi = self._out(gc, (B, T, n), host)
         _chk(self.lib.leb_zonotope_inflate_vjp(self._ctx, B, T, n, _ptr(gc), _ptr(gR), _ptr(g_lo), _ptr(g_hi),
                                                ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_zonotope_inflate_vjp")
         return g_lo, g_hi
@@ -233,6 +237,19 @@ class Context:
 
     def leb_launch_count(self) -> int:
         return int(self.lib.leb_launch_count(self._ctx))
+
+    def leb_profile(self, enable: bool):
+        _chk(self.lib.leb_profile(self._ctx, ctypes.c_int(int(bool(enable)))), "leb_profile")
+
+    def leb_profile_read(self, kernel_class: int):
+        """(ms, algorithmic work, launches) of one kernel class since the last leb_profile_reset."""
+        ms, work, n = ctypes.c_double(0), ctypes.c_double(0), ctypes.c_longlong(0)
+        _chk(self.lib.leb_profile_read(self._ctx, ctypes.c_int(int(kernel_class)), ctypes.byref(ms), ctypes.byref(work),
+                                       ctypes.byref(n), _stream_ptr(self.device)), "leb_profile_read")
+        return float(ms.value), float(work.value), int(n.value)
+
+    def leb_profile_reset(self):
+        _chk(self.lib.leb_profile_reset(self._ctx), "leb_profile_reset")
 
 
 def context_for_workload(w, device: int = 0) -> Context:

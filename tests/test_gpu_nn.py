@@ -1,0 +1,201 @@
+"""GPU parity: leb_nn_fwd / leb_vjp(kind 1) through the C ABI against the FP64 numpy oracle
+(CROWN Thm 2 eq. (18) PAPER.md:L196-200 + Thm 3 eq. (19)-(21) L204-220), on the same seeded inputs."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+from parity_util import assert_bounds_close, assert_grads_close, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    from paper_2607_01203_b200 import build, leb, workloads
+    from oracle import nn_oracle
+    build.build()
+    return leb, workloads, nn_oracle
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _flat(w):
+    return (w.nom.reshape(-1, w.N), w.rad.reshape(-1, w.N), w.g_lo.reshape(-1, w.n), w.g_hi.reshape(-1, w.n))
+
+
+SMALL = [  # dims, act: ragged widths (not multiples of 4 / 32), 1-4 hidden layers, both activations
+    ([5, 9, 3], 1), ([5, 9, 3], 2), ([6, 10, 10, 10, 4], 1), ([6, 10, 10, 10, 4], 2),
+    ([7, 33, 20, 11, 5], 2), ([3, 40, 2], 1), ([40, 64, 64, 64, 64, 33], 2), ([24, 130, 70, 20], 1),
+]
+
+
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_fwd_small_nets_match_oracle(mods, dims, act):
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    ctx = leb.context_for_workload(w)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
+    nom, rad, _, _ = _flat(w)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad)
+    assert_bounds_close(to_np(lo).reshape(-1, w.n), olo, f"{dims} r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n), ohi, f"{dims} r_hi")
+    # hidden-layer pre-activation bounds (N2/N3) against the oracle's
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    for layer in range(1, len(dims) - 1):
+        l, u = ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])
+        for t in (0, w.B * w.T - 1):
+            fw = O.crown_forward(Ws, bs, act, nom[t].astype(np.float64), rad[t].astype(np.float64))
+            assert np.allclose(to_np(l)[t], fw["ls"][layer - 1], rtol=2e-5, atol=2e-6)
+            assert np.allclose(to_np(u)[t], fw["us"][layer - 1], rtol=2e-5, atol=2e-6)
+    ctx.close()
+
+
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_vjp_small_nets_match_oracle(mods, dims, act):
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    ctx = leb.context_for_workload(w)
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi))
+    nom, rad, g_lo, g_hi = _flat(w)
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, act, nom, rad, g_lo, g_hi)
+    assert_grads_close(to_np(gn), to_np(gr), ogn, ogr, f"{dims}")
+    ctx.close()
+
+
+def test_config3_full_size_sampled_tiles(mods):
+    """Config 3 at BASELINE size (1280 tiles: two workspace chunks), oracle on 24 sampled tiles."""
+    leb, wl, O = mods
+    w = wl.make_config(3)
+    ctx = leb.context_for_workload(w)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi))
+    nom, rad, g_lo, g_hi = _flat(w)
+    idx = np.linspace(0, w.B * w.T - 1, 24).astype(int)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
+    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg3 r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg3 r_hi")
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx], g_lo[idx], g_hi[idx])
+    assert_grads_close(to_np(gn).reshape(-1, w.N)[idx], to_np(gr).reshape(-1, w.N)[idx], ogn, ogr, "cfg3")
+    ctx.close()
+
+
+def test_config5_full_size_sampled_tiles(mods):
+    """Config 5 in the launch configuration bench.py times (B=64, T=100), oracle on sampled tiles
+    (0.4 s forward + 0.6 s VJP each on the host)."""
+    leb, wl, O = mods
+    w = wl.make_config(5)
+    ctx = leb.context_for_workload(w)
+    nom_d, rad_d = _dev(w.nom), _dev(w.rad)
+    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d)
+    assert ctx.leb_domain_flag() == 0
+    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi))
+    nom, rad, g_lo, g_hi = _flat(w)
+    idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1])        # chunk boundaries, middle, last
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
+    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg5 r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg5 r_hi")
+    vi = idx[[0, 2, 4]]
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[vi], rad[vi], g_lo[vi], g_hi[vi])
+    assert_grads_close(to_np(gn).reshape(-1, w.N)[vi], to_np(gr).reshape(-1, w.N)[vi], ogn, ogr, "cfg5")
+    # properties that hold at any size: lo <= 0 <= hi (r(a~) = 0 lies in the enclosure), all finite
+    assert bool((lo <= 0).all()) and bool((hi >= 0).all()) and bool(torch.isfinite(gn).all()) and bool(torch.isfinite(gr).all())
+    ctx.close()
+
+
+def test_fwd_never_below_sampled_maximum_and_exact_range(mods):
+    """Soundness where it is sharp: tiny ReLU nets (<= 4 inputs): >= 1e5 samples + all box vertices."""
+    leb, wl, O = mods
+    for dims, act, seed in (([3, 12, 2], 1, 1), ([4, 10, 3], 1, 2), ([4, 8, 8, 2], 2, 3), ([2, 16, 16, 2], 1, 4)):
+        w = wl.make_small_mlp(dims, act, 2, 2, seed=seed, rad_lo=0.05, rad_hi=0.4)
+        ctx = leb.context_for_workload(w)
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
+        glo, ghi = to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        rng = np.random.default_rng(seed)
+        N = dims[0]
+        verts = np.array(list(itertools.product((-1.0, 1.0), repeat=N)))
+        for t in range(w.B * w.T):
+            a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+            U = np.concatenate([rng.uniform(-1, 1, (100000, N)), verts])
+            X = a0[None, :] + U * sg[None, :]
+            zs, p, J = O.nominal(Ws, bs, act, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(act, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J.T
+            # FP32 value mode vs FP64 truth: allow the parity tolerance below the sampled extremum
+            assert np.all(r.max(0) <= ghi[t] + 1e-5 * np.abs(ghi[t]) + 1e-7), (dims, t)
+            assert np.all(r.min(0) >= glo[t] - 1e-5 * np.abs(glo[t]) - 1e-7), (dims, t)
+        ctx.close()
+
+
+def test_given_jacobian(mods):
+    """J != NULL: the bound is with respect to the caller's matrix (Thm 3 holds for any J)."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp([6, 20, 20, 4], 2, 2, 3)
+    ctx = leb.context_for_workload(w)
+    rng = np.random.default_rng(9)
+    J = rng.standard_normal((w.B, w.T, w.n, w.N)).astype(np.float32) * 0.3
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J))
+    nom, rad, _, _ = _flat(w)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom, rad, J=J.reshape(-1, w.n, w.N))
+    # with an arbitrary J the bound is O(|W - J| sigma), computed from O(1) coefficients: tolerance
+    # relative to that scale
+    assert np.allclose(to_np(lo).reshape(-1, w.n), olo, rtol=1e-5, atol=2e-6)
+    assert np.allclose(to_np(hi).reshape(-1, w.n), ohi, rtol=1e-5, atol=2e-6)
+    ctx.close()
+
+
+def test_edge_cases(mods):
+    leb, wl, O = mods
+    w = wl.make_small_mlp([6, 10, 10, 4], 1, 2, 3)
+    ctx = leb.context_for_workload(w)
+    nom, rad = _dev(w.nom), _dev(w.rad)
+    # empty batch
+    lo, hi = ctx.leb_nn_fwd(nom[:0], rad[:0])
+    assert lo.shape == (0, 3, 4)
+    # zero radius: ReLU bound exactly 0 when no nominal pre-activation is exactly 0
+    lo, hi = ctx.leb_nn_fwd(nom, torch.zeros_like(rad))
+    assert float(lo.abs().max()) == 0.0 and float(hi.abs().max()) == 0.0
+    # padded leading dimensions
+    nomp = torch.zeros(2, 3, 8, device="cuda"); nomp[..., :6] = nom
+    radp = torch.zeros(2, 3, 8, device="cuda"); radp[..., :6] = rad
+    lop = torch.full((2, 3, 8), 7.0, device="cuda"); hip = torch.full((2, 3, 8), 7.0, device="cuda")
+    ctx.leb_nn_fwd(nomp, radp, r_lo=lop, r_hi=hip)
+    lo, hi = ctx.leb_nn_fwd(nom, rad)
+    assert torch.equal(lop[..., :4], lo) and torch.equal(hip[..., :4], hi) and float((lop[..., 4:] - 7).abs().max()) == 0.0
+    # chunking does not change results
+    ctx.leb_set_nn_chunk(4)
+    lo2, hi2 = ctx.leb_nn_fwd(nom, rad)
+    gn2, gr2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    ctx.leb_set_nn_chunk(0)
+    gn, gr = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    assert torch.equal(lo2, lo) and torch.equal(hi2, hi)
+    assert torch.allclose(gn2, gn, rtol=1e-5, atol=1e-7) and torch.allclose(gr2, gr, rtol=1e-5, atol=1e-7)
+    # NaN input / negative radius poison only their tile and raise the flag
+    assert ctx.leb_domain_flag() == 0
+    n2 = w.nom.copy(); n2[1, 0, 2] = np.nan
+    lo, hi = ctx.leb_nn_fwd(_dev(n2), rad)
+    assert ctx.leb_domain_flag() == 1
+    assert bool(torch.isinf(lo[1, 0]).all()) and bool(torch.isinf(hi[1, 0]).all()) and bool(torch.isfinite(lo[0]).all())
+    r2 = w.rad.copy(); r2[0, 2, 5] = -0.1
+    lo, hi = ctx.leb_nn_fwd(nom, _dev(r2))
+    assert ctx.leb_domain_flag() == 1 and bool(torch.isinf(hi[0, 2]).all()) and bool(torch.isfinite(hi[1]).all())
+    # host IO
+    hlo, hhi = ctx.leb_nn_fwd(torch.from_numpy(w.nom).pin_memory(), torch.from_numpy(w.rad).pin_memory(),
+                              flags=leb.FLAG_NO_MARGIN | leb.FLAG_HOST_IO)
+    torch.cuda.synchronize()
+    lo, hi = ctx.leb_nn_fwd(nom, rad)
+    assert torch.equal(hlo, lo.cpu()) and torch.equal(hhi, hi.cpu())
+    # model not set
+    ctx2 = leb.Context(0)
+    with pytest.raises(leb.LebError) as e:
+        ctx2.nn_n = 4
+        ctx2.leb_nn_fwd(nom, rad)
+    assert e.value.status == leb.LEB_ERR_STATE
+    ctx2.close()
+    ctx.close()
