@@ -32,6 +32,8 @@
  *     analytic box on which cos(theta) contains 0, so 1/cos is unbounded) gets r_lo = -inf,
  *     r_hi = +inf for all its dimensions and raises the context's domain flag, readable after
  *     synchronising the stream with leb_domain_flag().  A finite bound is never silently wrong.
+ *   - An empty batch (B == 0 or T == 0) is legal: the call returns LEB_OK, launches nothing and
+ *     does not look at the data pointers (they may be NULL).
  *   - There is no CPU fallback: every numerical step runs in the library's sm_100a kernels.
  */
 #ifndef LEB_H_

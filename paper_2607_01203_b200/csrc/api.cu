@@ -138,9 +138,11 @@ leb_status leb_set_nn_chunk(leb_ctx* c, int tiles) {
 
 leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, int ld_in,
                             float* r_lo, float* r_hi, int ld_out, unsigned flags, void* stream) {
-    if (!c || !nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
+    if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (!c->has_analytic) return LEB_ERR_STATE;
     if (mu) return LEB_ERR_UNSUPPORTED;
+    if (B == 0 || T == 0) return LEB_OK;            // empty batch: nothing to do, pointers may be NULL
+    if (!nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
     leb_status s = check_traj(B, T, c->model.N, c->model.n, ld_in, ld_out);
     if (s != LEB_OK) return s;
     if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
@@ -163,9 +165,11 @@ leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const fl
 
 leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, const float* J, int ld_in,
                       float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, void* stream) {
-    if (!c || !nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
+    if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
     if (mu) return LEB_ERR_UNSUPPORTED;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
     const int n = leb_nn_n(c->nn), N = leb_nn_N(c->nn);
     leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
     if (s != LEB_OK) return s;
@@ -192,8 +196,10 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
 
 leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
                    int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, void* stream) {
-    if (!c || !nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad) return LEB_ERR_ARG;
+    if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (kind != 0 && kind != 1) return LEB_ERR_ARG;
+    if ((B == 0 || T == 0) && (kind == 0 ? c->has_analytic : leb_nn_ready(c->nn))) return LEB_OK;
+    if (!nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad) return LEB_ERR_ARG;
     int n, N;
     if (kind == 0) {
         if (!c->has_analytic) return LEB_ERR_STATE;
@@ -232,8 +238,9 @@ leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const f
 
 leb_status leb_zonotope_inflate(leb_ctx* c, int B, int T, int n, const float* r_lo, const float* r_hi, const float* E_diag,
                                 float pad, float* c_bar, float* R_diag, float* Ebar_dense, unsigned flags, void* stream) {
-    if (!c || !r_lo || !r_hi || !c_bar || !R_diag) return LEB_ERR_ARG;
-    if (B < 0 || T < 0 || n < 1 || !(pad >= 0.f)) return LEB_ERR_ARG;
+    if (!c || B < 0 || T < 0 || n < 1 || !(pad >= 0.f)) return LEB_ERR_ARG;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!r_lo || !r_hi || !c_bar || !R_diag) return LEB_ERR_ARG;
     if (!al4(r_lo) || !al4(r_hi) || !al4(c_bar) || !al4(R_diag) || !al4(Ebar_dense) || !al4(E_diag)) return LEB_ERR_ALIGN;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
@@ -256,8 +263,9 @@ leb_status leb_zonotope_inflate(leb_ctx* c, int B, int T, int n, const float* r_
 
 leb_status leb_zonotope_inflate_vjp(leb_ctx* c, int B, int T, int n, const float* gc, const float* gR, float* g_lo, float* g_hi,
                                     unsigned flags, void* stream) {
-    if (!c || !gc || !gR || !g_lo || !g_hi) return LEB_ERR_ARG;
-    if (B < 0 || T < 0 || n < 1) return LEB_ERR_ARG;
+    if (!c || B < 0 || T < 0 || n < 1) return LEB_ERR_ARG;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!gc || !gR || !g_lo || !g_hi) return LEB_ERR_ARG;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     const bool host = flags & LEB_FLAG_HOST_IO;
