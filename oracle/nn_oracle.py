@@ -391,8 +391,24 @@ def _chain_reverse(Ws, bs, relaxs, s, Lams, Lbar0, cbar, upper, padj):
     # adjoint of Lambda_{s-1} = W_s is dropped (weights are not differentiated)
 
 
-def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None):
-    """Returns (grad_nom, grad_rad) for one tile."""
+def output_sign_ties(Ws, bs, act, a0, sig, rel=1e-6):
+    """Entries (chain, i, j) of W_up - J / W_lo - J whose magnitude is below rel * max|W|: the
+    |.| of eq. (21) L220 sits on its kink there, so the branch (reading R20) cannot be
+    resolved in FP32 and both one-sided gradients are valid results.  Test plumbing only."""
+    fw = crown_forward(Ws, bs, act, a0, sig)
+    ties = []
+    for chain, Wm in (("up", fw["W_up"]), ("lo", fw["W_lo"])):
+        D = Wm - fw["J"]
+        thr = rel * max(np.abs(Wm).max(), 1e-300)
+        for i, j in zip(*np.nonzero(np.abs(D) < thr)):
+            if sig[j] > 0:
+                ties.append((chain, int(i), int(j)))
+    return ties
+
+
+def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None, flips=()):
+    """Returns (grad_nom, grad_rad) for one tile.  `flips`: entries (chain, i, j) from
+    output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink)."""
     L = len(Ws)
     fw = crown_forward(Ws, bs, act, a0, sig, J_given, keep=True)
     relaxs, ls, us, zs, J = fw["relaxs"], fw["ls"], fw["us"], fw["zs"], fw["J"]
@@ -404,6 +420,8 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None):
     Lams_up, Lams_lo = fw["kept"][L]
     Lu0, Ll0 = Lams_up[0], Lams_lo[0]
     Su, Sl = np.sign(Lu0 - J), np.sign(Ll0 - J)
+    for chain, i, j in flips:
+        (Su if chain == "up" else Sl)[i, j] *= -1.0
     a_bar += Lu0.T @ g_hi + Ll0.T @ g_lo
     s_bar += np.abs(Lu0 - J).T @ g_hi - np.abs(Ll0 - J).T @ g_lo
     Lbar_up = g_hi[:, None] * (Su * sig[None, :] + a0[None, :])

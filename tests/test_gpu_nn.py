@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 import torch
 
-from parity_util import assert_bounds_close, assert_grads_close, to_np
+from parity_util import assert_bounds_close, assert_grads_close, assert_nn_grads_close, to_np
 
 pytestmark = pytest.mark.gpu
 
@@ -78,8 +78,8 @@ def test_config3_full_size_sampled_tiles(mods):
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
     assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg3 r_lo")
     assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg3 r_hi")
-    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx], g_lo[idx], g_hi[idx])
-    assert_grads_close(to_np(gn).reshape(-1, w.N)[idx], to_np(gr).reshape(-1, w.N)[idx], ogn, ogr, "cfg3")
+    assert_nn_grads_close(O, w.mlp, nom[idx], rad[idx], g_lo[idx], g_hi[idx], to_np(gn).reshape(-1, w.N)[idx],
+                          to_np(gr).reshape(-1, w.N)[idx], "cfg3")
     ctx.close()
 
 
@@ -99,8 +99,8 @@ def test_config5_full_size_sampled_tiles(mods):
     assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg5 r_lo")
     assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg5 r_hi")
     vi = idx[[0, 2, 4]]
-    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[vi], rad[vi], g_lo[vi], g_hi[vi])
-    assert_grads_close(to_np(gn).reshape(-1, w.N)[vi], to_np(gr).reshape(-1, w.N)[vi], ogn, ogr, "cfg5")
+    assert_nn_grads_close(O, w.mlp, nom[vi], rad[vi], g_lo[vi], g_hi[vi], to_np(gn).reshape(-1, w.N)[vi],
+                          to_np(gr).reshape(-1, w.N)[vi], "cfg5")
     # properties that hold at any size: lo <= 0 <= hi (r(a~) = 0 lies in the enclosure), all finite
     assert bool((lo <= 0).all()) and bool((hi >= 0).all()) and bool(torch.isfinite(gn).all()) and bool(torch.isfinite(gr).all())
     ctx.close()
