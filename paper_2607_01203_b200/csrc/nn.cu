@@ -18,6 +18,7 @@
 #include "internal.h"
 #include "nn_relax.cuh"
 #include "nn_gemm_ffma.cuh"
+#include "nn_gemm_tc.cuh"
 
 using namespace leb_nn;
 
@@ -38,6 +39,11 @@ struct NnState {
     float *W[kMaxLayers + 1] = {nullptr}, *Wt[kMaxLayers + 1] = {nullptr}, *bias[kMaxLayers + 1] = {nullptr};
     int rowsW[kMaxLayers + 1] = {0};
     float *Wabs1 = nullptr, *Wabs1t = nullptr;
+    // 3xTF32 tensor-core path: hi/lo splits of W[l] (reverse sweep) and Wt[l] (forward chain), l = 1..L-1, and their TMA maps
+    float *Whi[kMaxLayers + 1] = {nullptr}, *Wlo[kMaxLayers + 1] = {nullptr}, *Wthi[kMaxLayers + 1] = {nullptr}, *Wtlo[kMaxLayers + 1] = {nullptr};
+    CUtensorMap mapW_hi[kMaxLayers + 1], mapW_lo[kMaxLayers + 1], mapWt_hi[kMaxLayers + 1], mapWt_lo[kMaxLayers + 1];
+    bool tc_ready = false, use_tc = false;
+    int num_sms = 148;
     // workspace for one chunk of tiles
     int chunk_req = 0, chunk = 0;
     bool ws_vjp = false;
@@ -107,6 +113,15 @@ __global__ void pad_cotangent_kernel(int tiles, int n, int ld_out, const float* 
 
 __global__ void fill_kernel(float* __restrict__ p, size_t count, float v) {
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) p[q] = v;
+}
+
+// x = hi + lo with hi = tf32(x), lo = tf32(x - hi) (round to nearest, ties away): operands of the 3xTF32 contraction
+__global__ void split_tf32_kernel(const float* __restrict__ src, float* __restrict__ hi, float* __restrict__ lo, size_t count) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) {
+        const float x = src[q], h = tc::to_tf32(x);
+        hi[q] = h;
+        lo[q] = tc::to_tf32(x - h);
+    }
 }
 
 // per-neuron relaxation of layer l from (zhat, l, u); for layer 1 (rad1 != NULL) first l,u = zhat -+ rad1 (N2)
@@ -441,8 +456,15 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
             g.rows_pad = rp; g.rows_kind = rk; g.nkinds = nk;
             g.kU = S->kU[l]; g.kL = S->kL[l]; g.gU = S->gU[l]; g.gL = S->gL[l]; g.dphi = S->dphi[l]; g.ldp = S->wp[l];
             g.gap = S->gap[s]; g.gap_init = (l == s - 1);
-            launch_gemm<AMODE_CHAIN, EPI_STORE>(S, g, st, launches, LEB_KC_CHAIN_FWD,
-                                                2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1]);
+            const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
+            if (S->use_tc) {
+                S->prof->begin(LEB_KC_CHAIN_FWD, st);
+                tc::launch_chain_gemm_tc<tc::MODE_FWD>(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st);
+                S->prof->end(LEB_KC_CHAIN_FWD, st, flops);
+                ++*launches;
+            } else {
+                launch_gemm<AMODE_CHAIN, EPI_STORE>(S, g, st, launches, LEB_KC_CHAIN_FWD, flops);
+            }
         }
         if (!is_out) {
             size_t warps = (size_t)C * rk;
@@ -470,7 +492,9 @@ static void free_weights(NnState* S) {
         if (S->Wt[l]) cudaFree(S->Wt[l]);
         if (S->bias[l]) cudaFree(S->bias[l]);
         S->W[l] = S->Wt[l] = S->bias[l] = nullptr;
+        for (float** p : {&S->Whi[l], &S->Wlo[l], &S->Wthi[l], &S->Wtlo[l]}) { if (*p) cudaFree(*p); *p = nullptr; }
     }
+    S->tc_ready = false;
     if (S->Wabs1) cudaFree(S->Wabs1);
     if (S->Wabs1t) cudaFree(S->Wabs1t);
     S->Wabs1 = S->Wabs1t = nullptr;
@@ -537,6 +561,13 @@ leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long lo
         pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wt[l], rows_p, cols_p, 1, 0);
         pack_matrix_kernel<<<gs_grid(rows_p), 256, 0, st>>>(bsrc, 1, rows, rows, S->bias[l], 1, rup(rows_p, kPad), 0, 0);
         *launches += 3;
+        if (l < L) {
+            for (float** p : {&S->Whi[l], &S->Wlo[l], &S->Wthi[l], &S->Wtlo[l]}) ok = ok && cudaMalloc(p, tot * sizeof(float)) == cudaSuccess;
+            if (!ok) break;
+            split_tf32_kernel<<<gs_grid(tot), 256, 0, st>>>(S->W[l], S->Whi[l], S->Wlo[l], tot);
+            split_tf32_kernel<<<gs_grid(tot), 256, 0, st>>>(S->Wt[l], S->Wthi[l], S->Wtlo[l], tot);
+            *launches += 2;
+        }
         if (l == 1) {
             ok = ok && cudaMalloc(&S->Wabs1, tot * sizeof(float)) == cudaSuccess;
             ok = ok && cudaMalloc(&S->Wabs1t, tot * sizeof(float)) == cudaSuccess;
@@ -553,6 +584,20 @@ leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long lo
         S->rows_kind[s] = (s < L) ? S->wp[s] : S->w[L];
         S->rows_pad[s] = rup((s < L ? 2 : 3) * S->rows_kind[s], kRowBlock);
     }
+    // TMA maps of the split weights (K-major B operands): W[l] is [wp[l] x wp[l-1]], Wt[l] is [wp[l-1] x wp[l]]
+    S->tc_ready = true;
+    for (int l = 1; l < L; ++l) {
+        S->tc_ready = S->tc_ready && tc::make_weight_map(&S->mapW_hi[l], S->Whi[l], S->wp[l], S->wp[l - 1]);
+        S->tc_ready = S->tc_ready && tc::make_weight_map(&S->mapW_lo[l], S->Wlo[l], S->wp[l], S->wp[l - 1]);
+        S->tc_ready = S->tc_ready && tc::make_weight_map(&S->mapWt_hi[l], S->Wthi[l], S->wp[l - 1], S->wp[l]);
+        S->tc_ready = S->tc_ready && tc::make_weight_map(&S->mapWt_lo[l], S->Wtlo[l], S->wp[l - 1], S->wp[l]);
+    }
+    if (!S->tc_ready) { free_weights(S); return LEB_ERR_CUDA; }   // no silent fallback: the driver must provide cuTensorMapEncodeTiled
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&S->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     S->ready = true;
     return LEB_OK;
 }
@@ -564,6 +609,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
                           float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
                           long long* launches, LebProf* prof) {
     S->prof = prof;
+    S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
     if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;   // certified mode: see DESIGN.md (N6)
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, false);
@@ -608,8 +654,9 @@ leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStre
 leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
                       int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
                       cudaStream_t st, long long* launches, LebProf* prof) {
-    (void)flags; (void)domain_flag;
+    (void)domain_flag;
     S->prof = prof;
+    S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;
@@ -661,8 +708,15 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                 g.gapbar = S->gapbar;
                 g.kUb = S->kUb[l]; g.kLb = S->kLb[l]; g.gUb = S->gUb[l]; g.gLb = S->gLb[l]; g.db = S->dpb[l];
                 g.write_c = (l < s - 1);
-                launch_gemm<AMODE_PLAIN, EPI_CHAIN_BWD>(S, g, st, launches, LEB_KC_CHAIN_BWD,
-                                                        2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1]);
+                const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
+                if (S->use_tc) {
+                    S->prof->begin(LEB_KC_CHAIN_BWD, st);
+                    tc::launch_chain_gemm_tc<tc::MODE_BWD>(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st);
+                    S->prof->end(LEB_KC_CHAIN_BWD, st, flops);
+                    ++*launches;
+                } else {
+                    launch_gemm<AMODE_PLAIN, EPI_CHAIN_BWD>(S, g, st, launches, LEB_KC_CHAIN_BWD, flops);
+                }
                 cur ^= 1;
             }
         }

@@ -27,18 +27,23 @@ def _flat(w):
     return (w.nom.reshape(-1, w.N), w.rad.reshape(-1, w.N), w.g_lo.reshape(-1, w.n), w.g_hi.reshape(-1, w.n))
 
 
+# both contraction paths: 3xTF32 tcgen05 (default) and FP32 FFMA (LEB_FLAG_FFMA_ONLY); value mode in both
+PATHS = {"tc": 1, "ffma": 1 | 2}
+
+
 SMALL = [  # dims, act: ragged widths (not multiples of 4 / 32), 1-4 hidden layers, both activations
     ([5, 9, 3], 1), ([5, 9, 3], 2), ([6, 10, 10, 10, 4], 1), ([6, 10, 10, 10, 4], 2),
     ([7, 33, 20, 11, 5], 2), ([3, 40, 2], 1), ([40, 64, 64, 64, 64, 33], 2), ([24, 130, 70, 20], 1),
 ]
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("dims,act", SMALL)
-def test_fwd_small_nets_match_oracle(mods, dims, act):
+def test_fwd_small_nets_match_oracle(mods, dims, act, path):
     leb, wl, O = mods
     w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
     ctx = leb.context_for_workload(w)
-    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
     nom, rad, _, _ = _flat(w)
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad)
     assert_bounds_close(to_np(lo).reshape(-1, w.n), olo, f"{dims} r_lo")
@@ -54,25 +59,27 @@ def test_fwd_small_nets_match_oracle(mods, dims, act):
     ctx.close()
 
 
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("dims,act", SMALL)
-def test_vjp_small_nets_match_oracle(mods, dims, act):
+def test_vjp_small_nets_match_oracle(mods, dims, act, path):
     leb, wl, O = mods
     w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
     ctx = leb.context_for_workload(w)
-    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi))
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
     nom, rad, g_lo, g_hi = _flat(w)
     ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, act, nom, rad, g_lo, g_hi)
     assert_grads_close(to_np(gn), to_np(gr), ogn, ogr, f"{dims}")
     ctx.close()
 
 
-def test_config3_full_size_sampled_tiles(mods):
+@pytest.mark.parametrize("path", list(PATHS))
+def test_config3_full_size_sampled_tiles(mods, path):
     """Config 3 at BASELINE size (1280 tiles: two workspace chunks), oracle on 24 sampled tiles."""
     leb, wl, O = mods
     w = wl.make_config(3)
     ctx = leb.context_for_workload(w)
-    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
-    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi))
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
     nom, rad, g_lo, g_hi = _flat(w)
     idx = np.linspace(0, w.B * w.T - 1, 24).astype(int)
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
@@ -83,16 +90,17 @@ def test_config3_full_size_sampled_tiles(mods):
     ctx.close()
 
 
-def test_config5_full_size_sampled_tiles(mods):
+@pytest.mark.parametrize("path", list(PATHS))
+def test_config5_full_size_sampled_tiles(mods, path):
     """Config 5 in the launch configuration bench.py times (B=64, T=100), oracle on sampled tiles
     (0.4 s forward + 0.6 s VJP each on the host)."""
     leb, wl, O = mods
     w = wl.make_config(5)
     ctx = leb.context_for_workload(w)
     nom_d, rad_d = _dev(w.nom), _dev(w.rad)
-    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d)
+    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d, flags=PATHS[path])
     assert ctx.leb_domain_flag() == 0
-    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi))
+    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
     nom, rad, g_lo, g_hi = _flat(w)
     idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1])        # chunk boundaries, middle, last
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
