@@ -26,7 +26,7 @@ namespace {
 
 inline int rup(int x, int m) { return (x + m - 1) / m * m; }
 constexpr int kPad = 32;        // feature dims are zero-padded to multiples of 32
-constexpr int kRowBlock = 128;  // chain row blocks
+constexpr int kRowBlock = 256;  // chain row blocks (the tensor-core kernel takes 256 coefficient rows per tile)
 constexpr int kMaxLayers = 16;
 
 }  // namespace
@@ -42,7 +42,7 @@ struct NnState {
     // 3xTF32 tensor-core path: hi/lo splits of W[l] (reverse sweep) and Wt[l] (forward chain), l = 1..L-1, and their TMA maps
     float *Whi[kMaxLayers + 1] = {nullptr}, *Wlo[kMaxLayers + 1] = {nullptr}, *Wthi[kMaxLayers + 1] = {nullptr}, *Wtlo[kMaxLayers + 1] = {nullptr};
     CUtensorMap mapW_hi[kMaxLayers + 1], mapW_lo[kMaxLayers + 1], mapWt_hi[kMaxLayers + 1], mapWt_lo[kMaxLayers + 1];
-    bool tc_ready = false, use_tc = false;
+    bool tc_ready = false, use_tc = false, launch_failed = false;
     int num_sms = 148;
     // workspace for one chunk of tiles
     int chunk_req = 0, chunk = 0;
@@ -459,7 +459,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
             const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
             if (S->use_tc) {
                 S->prof->begin(LEB_KC_CHAIN_FWD, st);
-                tc::launch_chain_gemm_tc<tc::MODE_FWD>(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st);
+                if (tc::launch_chain_gemm_tc<tc::MODE_FWD>(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st) != cudaSuccess) S->launch_failed = true;
                 S->prof->end(LEB_KC_CHAIN_FWD, st, flops);
                 ++*launches;
             } else {
@@ -637,6 +637,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         }
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
     }
+    if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
 
@@ -711,7 +712,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                 const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
                 if (S->use_tc) {
                     S->prof->begin(LEB_KC_CHAIN_BWD, st);
-                    tc::launch_chain_gemm_tc<tc::MODE_BWD>(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st);
+                    if (tc::launch_chain_gemm_tc<tc::MODE_BWD>(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st) != cudaSuccess) S->launch_failed = true;
                     S->prof->end(LEB_KC_CHAIN_BWD, st, flops);
                     ++*launches;
                 } else {
@@ -746,5 +747,6 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         ++*launches;
         S->last_tiles = 0;
     }
+    if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }

@@ -1,23 +1,29 @@
 // nn_gemm_tc.cuh -- the CROWN chain contraction on the 5th-generation tensor cores (tcgen05), 3xTF32.
 //
 // One step of the back-substitution (eq. (18)) and one step of
-// its reverse sweep are dense contractions  C[M x N] = T(A)[M x K] * B[K x N]  with
-// M = tiles * rows (10^5 .. 10^6), K, N = layer widths, and B a weight matrix shared by all tiles.
-// FP32 operands are split  x = hi + lo  (hi = tf32(x), lo = tf32(x - hi)) and the product is
-// accumulated in FP32 in tensor memory as  Ahi*Bhi + Ahi*Blo + Alo*Bhi  (the dropped Alo*Blo term and
-// the rounding of lo are <= 3 * 2^-22 |a||b| per product).
+// its reverse sweep are dense contractions  C[R x N] = T(A)[R x K] * W[K x N]  with
+// R = tiles * rows (10^5 .. 10^6) coefficient rows, K, N = layer widths, W a weight matrix shared by
+// all tiles.  FP32 operands are split  x = hi + lo  (hi = tf32(x), lo = tf32(x - hi)); the main term
+// Whi*Ahi and the correction Whi*Alo + Wlo*Ahi are accumulated in FP32 in two separate tensor-memory
+// accumulators and added in the epilogue (the tensor core truncates every accumulation, so the 2K/8
+// correction MMAs must not touch the large accumulator).
 //
-// Kernel layout (persistent, one CTA per SM, 384 threads):
-//   warp 0      TMA producer: pre-split weight tiles Bhi, Blo [256 x 32] (K-major, 128B swizzle)
-//   warp 1      MMA issuer: 12 tcgen05.mma (M128 x N<=256 x K8) per 32-wide K slab, accumulators in TMEM
-//   warp 2      TMEM allocation (2 x 256 columns: the epilogue of tile i overlaps the main loop of i+1)
-//   warps 4-7   epilogue: tcgen05.ld -> registers -> global (forward: Lambda_{l-1};
-//               reverse: sign-masked adjoint + column sums of the relaxation-parameter adjoints)
-//   warps 8-11  A producers: global FP32 rows -> (forward: D = Lam^+ k_pos + Lam^- k_neg and the
-//               deviation-form constant  gap += Lam^+ g_pos + Lam^- g_neg) -> hi/lo split ->
-//               128B-swizzled K-major shared-memory tiles (generic-proxy stores + async-proxy fence)
-// Stages are handed over with mbarriers: full[s] (128 producer arrivals + the TMA transaction),
-// empty[s] (tcgen05.commit), tmem_full[a] (tcgen05.commit), tmem_empty[a] (128 epilogue arrivals).
+// The product is computed TRANSPOSED, D[n, r] = sum_k W^T[n, k] T(A)[r, k]: the weights are the
+// M-side operand (128 output columns per tile, TMA-staged), the coefficient rows the N-side operand
+// (256 rows per tile).  A TMEM lane is then an output column: an epilogue thread owns one column,
+// walks the rows, stores coalesced rows of C and -- in the reverse sweep -- keeps the column sums of
+// the relaxation-parameter adjoints in registers (no cross-lane reduction).
+//
+// Kernel layout (persistent, one CTA per SM, 512 threads):
+//   warp 0       TMA producer: pre-split weight tiles Whi, Wlo [128 x 32] (K-major, 128B swizzle)
+//   warp 1       MMA issuer: 12 tcgen05.mma (M128 x N256 x K8) per 32-wide K slab
+//   warp 2       TMEM allocation (512 columns: main [0,256), correction [256,512))
+//   warps 4-7    epilogue: tcgen05.ld -> registers -> global
+//   warps 8-15   row producers: global FP32 rows -> (forward: D = Lam^+ k_pos + Lam^- k_neg and the
+//                deviation-form constant  gap += Lam^+ g_pos + Lam^- g_neg) -> hi/lo split ->
+//                128B-swizzled K-major shared-memory tiles (generic-proxy stores + async-proxy fence)
+// Stages are handed over with mbarriers: full[s] (256 producer arrivals + the TMA transaction),
+// empty[s] (tcgen05.commit), tmem_full (tcgen05.commit), tmem_empty (128 epilogue arrivals).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -29,14 +35,16 @@ namespace tc {
 
 enum { MODE_FWD = 0, MODE_BWD = 1 };
 
-constexpr int TBM = 128, TBN = 256, TBK = 32, STAGES = 2;
-constexpr int A_TILE_BYTES = TBM * TBK * 4;                         // 16 KB
-constexpr int B_TILE_BYTES = TBN * TBK * 4;                         // 32 KB
-constexpr int STAGE_BYTES = 2 * A_TILE_BYTES + 2 * B_TILE_BYTES;    // 96 KB
-constexpr int RED_BYTES = 5 * TBN * 4;                              // reverse epilogue column sums
+constexpr int TBM = 128;      // output columns per tile (MMA M, weights)
+constexpr int TBN = 256;      // coefficient rows per tile (MMA N)
+constexpr int TBK = 32, STAGES = 2;
+constexpr int W_TILE_BYTES = TBM * TBK * 4;                         // 16 KB
+constexpr int R_TILE_BYTES = TBN * TBK * 4;                         // 32 KB
+constexpr int STAGE_BYTES = 2 * W_TILE_BYTES + 2 * R_TILE_BYTES;    // 96 KB
 constexpr int BAR_BYTES = 128;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + RED_BYTES + BAR_BYTES + 1024;   // + 1024-byte alignment slack
-constexpr int THREADS = 384;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;   // + 1024-byte alignment slack
+constexpr int THREADS = 512;
+constexpr int PRODUCERS = 256;
 constexpr int TMEM_COLS = 512;
 constexpr unsigned long long kSpinLimit = 4000000000ull;            // ~2 s of SM clocks: trap instead of hanging
 
@@ -110,8 +118,22 @@ __device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint6
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-// 32 lanes x 32 columns of FP32: thread t of the warp gets lane (warp%4)*32 + t, columns [c, c+32)
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
+// NX consecutive FP32 columns of this warp's 32 TMEM lanes: thread t gets lane (warp%4)*32 + t, columns [c, c+NX).
+// Asynchronous: tmem_ld_wait() before the registers are read.
+template <int NX> __device__ __forceinline__ void tmem_ld(uint32_t taddr, float* v);
+template <> __device__ __forceinline__ void tmem_ld<16>(uint32_t taddr, float* v) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+template <> __device__ __forceinline__ void tmem_ld<32>(uint32_t taddr, float* v) {
     uint32_t r[32];
     asm volatile(
         "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -123,10 +145,10 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
           "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
         : "r"(taddr)
         : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ float to_tf32(float x) {
     uint32_t r;
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
@@ -149,18 +171,25 @@ __device__ __forceinline__ uint32_t make_idesc(int mma_m, int mma_n) {
     return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(mma_n >> 3) << 17) | ((uint32_t)(mma_m >> 4) << 24);
 }
 
-// butterfly transpose-reduce: on return v[0] of lane L holds sum over the warp's lanes of v[L]
-__device__ __forceinline__ void warp_transpose_sum32(float* v, int lane) {
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        const bool up = (lane & off) != 0;
-#pragma unroll
-        for (int j = 0; j < off; ++j) {
-            const float send = up ? v[j] : v[j + off];
-            const float keep = up ? v[j + off] : v[j];
-            v[j] = keep + __shfl_xor_sync(0xffffffffu, send, off);
-        }
-    }
+
+// per-tile geometry shared by the roles.  Tiles are numbered with the column block fastest, so the CTAs
+// that run concurrently share coefficient rows (L2 reuse).  rows_pad % 256 == 0: a row block never
+// straddles two trajectory tiles, so one slope-vector offset `po` serves the whole block.
+struct TileGeo {
+    int r0;        // first coefficient row of the block (global row index)
+    int n0;        // first output column
+    int rbase;     // r0 relative to its trajectory tile
+    size_t po;     // offset of the tile's per-neuron parameter vectors
+};
+__device__ __forceinline__ TileGeo tile_geo(const GemmArgs& g, int tile, int col_blocks) {
+    TileGeo t;
+    const int rb = tile / col_blocks;
+    t.n0 = (tile - rb * col_blocks) * TBM;
+    t.r0 = rb * TBN;
+    const int tl = t.r0 / g.rows_pad;
+    t.rbase = t.r0 - tl * g.rows_pad;
+    t.po = (size_t)tl * g.ldp;
+    return t;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -172,21 +201,19 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     extern __shared__ uint8_t smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* sgen = smem_raw + (sbase - smem_u32(smem_raw));           // generic pointer to the aligned base
-    // stage s: [Ahi | Alo | Bhi | Blo]
-    auto sA = [&](int s, int part) { return sbase + s * STAGE_BYTES + part * A_TILE_BYTES; };
-    auto sB = [&](int s, int part) { return sbase + s * STAGE_BYTES + 2 * A_TILE_BYTES + part * B_TILE_BYTES; };
-    float* s_red = reinterpret_cast<float*>(sgen + STAGES * STAGE_BYTES);
-    const uint32_t bar0 = sbase + STAGES * STAGE_BYTES + RED_BYTES;
+    // stage s: [Whi | Wlo | Rhi | Rlo]
+    auto sW = [&](int s, int part) { return sbase + s * STAGE_BYTES + part * W_TILE_BYTES; };
+    auto sR = [&](int s, int part) { return sbase + s * STAGE_BYTES + 2 * W_TILE_BYTES + part * R_TILE_BYTES; };
+    const uint32_t bar0 = sbase + STAGES * STAGE_BYTES;
     auto bar_full = [&](int s) { return bar0 + 8 * s; };
     auto bar_empty = [&](int s) { return bar0 + 8 * (STAGES + s); };
-    auto bar_tfull = [&](int a) { return bar0 + 8 * (2 * STAGES + a); };
-    auto bar_tempty = [&](int a) { return bar0 + 8 * (2 * STAGES + 2 + a); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + STAGES * STAGE_BYTES + RED_BYTES + 8 * (2 * STAGES + 4));
+    const uint32_t bar_tfull = bar0 + 8 * (2 * STAGES), bar_tempty = bar0 + 8 * (2 * STAGES + 1);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 2));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_blocks = (g.N + TBN - 1) / TBN;
-    const int m_blocks = g.M / TBM;
-    const int num_tiles = m_blocks * n_blocks;
+    const int col_blocks = (g.N + TBM - 1) / TBM;
+    const int row_blocks = g.M / TBN;                 // g.M % 256 == 0 (rows_pad % 256 == 0)
+    const int num_tiles = row_blocks * col_blocks;
     const int nk = g.K / TBK;
 
     if (warp == 0 && lane == 0) {
@@ -194,8 +221,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         tma_prefetch_desc(&tm_lo);
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full(s), 128 + 1); mbar_init(bar_empty(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), 128); }
+        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full(s), PRODUCERS + 1); mbar_init(bar_empty(s), 1); }
+        mbar_init(bar_tfull, 1);
+        mbar_init(bar_tempty, 128);
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
@@ -208,13 +236,13 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         // ===================== TMA producer (weights) =====================
         int stage = 0; uint32_t phase = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-            const int n0 = (tile % n_blocks) * TBN;
+            const int n0 = (tile % col_blocks) * TBM;
             for (int kt = 0; kt < nk; ++kt) {
                 mbar_wait(bar_empty(stage), phase ^ 1);
                 if (lane == 0) {
-                    mbar_arrive_expect_tx(bar_full(stage), 2 * B_TILE_BYTES);
-                    tma_load_2d(sB(stage, 0), &tm_hi, kt * TBK, n0, bar_full(stage));
-                    tma_load_2d(sB(stage, 1), &tm_lo, kt * TBK, n0, bar_full(stage));
+                    mbar_arrive_expect_tx(bar_full(stage), 2 * W_TILE_BYTES);
+                    tma_load_2d(sW(stage, 0), &tm_hi, kt * TBK, n0, bar_full(stage));
+                    tma_load_2d(sW(stage, 1), &tm_lo, kt * TBK, n0, bar_full(stage));
                 }
                 __syncwarp();
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -223,173 +251,161 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
         int stage = 0; uint32_t phase = 0;
+        const uint32_t idesc = make_idesc(TBM, TBN);
+        const uint32_t d_main = tmem_base, d_corr = tmem_base + TBN;
         int tcount = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
-            const int n0 = (tile % n_blocks) * TBN;
-            const int n_mma = min(TBN, g.N - n0);
-            const uint32_t idesc = make_idesc(TBM, n_mma);
-            const int acc = tcount & 1;
-            mbar_wait(bar_tempty(acc), ((tcount >> 1) & 1) ^ 1);
+            mbar_wait(bar_tempty, (tcount & 1) ^ 1);          // the epilogue has drained the previous tile
             tc_fence_after();
-            const uint32_t d_tmem = tmem_base + acc * TBN;
             for (int kt = 0; kt < nk; ++kt) {
                 mbar_wait(bar_full(stage), phase);
                 tc_fence_after();
                 if (lane == 0) {
-                    const uint64_t ahi = make_smem_desc(sA(stage, 0)), alo = make_smem_desc(sA(stage, 1));
-                    const uint64_t bhi = make_smem_desc(sB(stage, 0)), blo = make_smem_desc(sB(stage, 1));
+                    const uint64_t whi = make_smem_desc(sW(stage, 0)), wlo = make_smem_desc(sW(stage, 1));
+                    const uint64_t rhi = make_smem_desc(sR(stage, 0)), rlo = make_smem_desc(sR(stage, 1));
 #pragma unroll
                     for (int k = 0; k < TBK / 8; ++k) {
                         const uint64_t ko = (uint64_t)(k * 32 >> 4);     // 8 tf32 = 32 bytes along K inside the swizzle atom
-                        umma_tf32(d_tmem, alo + ko, bhi + ko, idesc, (kt | k) != 0);
-                        umma_tf32(d_tmem, ahi + ko, blo + ko, idesc, 1u);
-                        umma_tf32(d_tmem, ahi + ko, bhi + ko, idesc, 1u);
+                        umma_tf32(d_main, whi + ko, rhi + ko, idesc, (kt | k) != 0);
+                        umma_tf32(d_corr, whi + ko, rlo + ko, idesc, (kt | k) != 0);
+                        umma_tf32(d_corr, wlo + ko, rhi + ko, idesc, 1u);
                     }
                     umma_commit(bar_empty(stage));                       // frees the stage when these MMAs retire
-                    if (kt == nk - 1) umma_commit(bar_tfull(acc));       // accumulator complete
+                    if (kt == nk - 1) umma_commit(bar_tfull);            // accumulators complete
                 }
                 __syncwarp();
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp >= 4 && warp < 8) {
-        // ===================== epilogue =====================
-        const int q = warp - 4;                    // TMEM lane quadrant of this warp (warp % 4)
-        const int etid = threadIdx.x - 128;
+        // ===================== epilogue: TMEM lane = output column, TMEM column = coefficient row =====================
+        const int q = warp - 4;                                  // TMEM lane quadrant of this warp (warp % 4)
+        const uint32_t t_lane = tmem_base + ((uint32_t)(q * 32) << 16);
         int tcount = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
-            const int mb = tile / n_blocks, n0 = (tile - mb * n_blocks) * TBN;
-            const int n_mma = min(TBN, g.N - n0);
-            const int acc = tcount & 1;
-            const int m = mb * TBM + q * 32 + lane;
-            int tl = 0, kind = 0, rk = 0;
-            chain_row(g, m, tl, kind, rk);
-            const size_t po = (size_t)tl * g.ldp;
-            if (MODE == MODE_BWD) {
-                for (int i = etid; i < 5 * TBN; i += 128) s_red[i] = 0.f;
-                named_bar_sync(1, 128);
-            }
-            mbar_wait(bar_tfull(acc), (tcount >> 1) & 1);
-            tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * TBN;
+            const TileGeo t = tile_geo(g, tile, col_blocks);
+            const int n = t.n0 + q * 32 + lane;                  // this thread's output column
+            const bool n_ok = n < g.N;
             if (MODE == MODE_FWD) {
-                float* crow = g.C + (size_t)m * g.ldc + n0;
-                for (int c = 0; c < n_mma; c += 32) {
-                    float v[32];
-                    tmem_ld32(taddr + c, v);
+                mbar_wait(bar_tfull, tcount & 1);
+                tc_fence_after();
+                float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
+#pragma unroll 1
+                for (int c = 0; c < TBN; c += 32) {
+                    float a[32], b[32];
+                    tmem_ld<32>(t_lane + c, a);
+                    tmem_ld<32>(t_lane + TBN + c, b);
+                    tmem_ld_wait();
+                    if (n_ok) {
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4)
-                        *reinterpret_cast<float4*>(crow + c + j) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+                        for (int j = 0; j < 32; ++j) cbase[(size_t)(c + j) * g.ldc] = a[j] + b[j];   // 128 B per warp and row
+                    }
                 }
+                tc_fence_before();
+                mbar_arrive(bar_tempty);
             } else {
-                const float gb = (kind >= 0 && kind < 2) ? g.gapbar[m] : 0.f;
-                const float* lrow = g.Lam + (size_t)(g.lam_shared ? rk : m) * g.ldl + n0;
-                float* crow = g.C + (size_t)m * g.ldc + n0;
-                for (int c = 0; c < n_mma; c += 32) {
-                    float v[32], lam[32], t[32];
-                    tmem_ld32(taddr + c, v);
+                // row kinds inside the block: [0,kb1) upper chain, [kb1,kb2) lower, [kb2,kbe) Jacobian, then padding
+                const int kb1 = g.rows_kind - t.rbase, kb2 = 2 * g.rows_kind - t.rbase, kbe = g.nkinds * g.rows_kind - t.rbase;
+                float kU = 0.f, kL = 0.f, gU = 0.f, gL = 0.f, dp = 0.f;
+                if (n_ok) {
+                    kU = __ldg(g.kU + t.po + n); kL = __ldg(g.kL + t.po + n);
+                    gU = __ldg(g.gU + t.po + n); gL = __ldg(g.gL + t.po + n);
+                    dp = __ldg(g.dphi + t.po + n);
+                }
+                float skU = 0.f, skL = 0.f, sgU = 0.f, sgL = 0.f, sdb = 0.f;
+                auto load_lam = [&](float* dst, int c) {
 #pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        const float4 x = (kind >= 0) ? __ldg(reinterpret_cast<const float4*>(lrow + c + j)) : make_float4(0.f, 0.f, 0.f, 0.f);
-                        lam[j] = x.x; lam[j + 1] = x.y; lam[j + 2] = x.z; lam[j + 3] = x.w;
+                    for (int j = 0; j < 16; ++j) {
+                        const int jj = c + j;
+                        const int kind = (jj >= kb1) + (jj >= kb2);
+                        const int row = g.lam_shared ? (t.rbase + jj - kind * g.rows_kind) : (t.r0 + jj);
+                        dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
+                    }
+                };
+                float lam[16], lamn[16];
+                load_lam(lam, 0);                                // overlaps the tail of the main loop
+                mbar_wait(bar_tfull, tcount & 1);
+                tc_fence_after();
+                float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
+#pragma unroll 1
+                for (int c = 0; c < TBN; c += 16) {
+                    float a[16], b[16];
+                    tmem_ld<16>(t_lane + c, a);
+                    tmem_ld<16>(t_lane + TBN + c, b);
+                    if (c + 16 < TBN) load_lam(lamn, c + 16);
+                    // the row's gap adjoint: lane j < 16 fetches row c + j, broadcast below
+                    float gbv = 0.f;
+                    {
+                        const int jj = c + (lane & 15);
+                        const int kind = (jj >= kb1) + (jj >= kb2);
+                        if (jj < kbe && kind < 2) gbv = __ldg(g.gapbar + t.r0 + jj);
+                    }
+                    tmem_ld_wait();
+                    if (c + 16 >= TBN) {                         // last read of this tile's accumulators: release them
+                        tc_fence_before();
+                        mbar_arrive(bar_tempty);
                     }
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) v[j] = (kind >= 0) ? v[j] : 0.f;     // padding rows may hold anything
-                    // ---- column sums over the rows of this warp, one adjoint at a time (register pressure)
-                    // kUb: upper rows Db*P, lower rows Db*Q;  kLb: the other way round
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) t[j] = (kind == 0) ? v[j] * fmaxf(lam[j], 0.f) : ((kind == 1) ? v[j] * fminf(lam[j], 0.f) : 0.f);
-                    warp_transpose_sum32(t, lane);
-                    atomicAdd(&s_red[0 * TBN + c + lane], t[0]);
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) t[j] = (kind == 0) ? v[j] * fminf(lam[j], 0.f) : ((kind == 1) ? v[j] * fmaxf(lam[j], 0.f) : 0.f);
-                    warp_transpose_sum32(t, lane);
-                    atomicAdd(&s_red[1 * TBN + c + lane], t[0]);
-                    // gUb / gLb: the same with the row's gap adjoint in place of Db
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) t[j] = (kind == 0) ? gb * fmaxf(lam[j], 0.f) : ((kind == 1) ? gb * fminf(lam[j], 0.f) : 0.f);
-                    warp_transpose_sum32(t, lane);
-                    atomicAdd(&s_red[2 * TBN + c + lane], t[0]);
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) t[j] = (kind == 0) ? gb * fminf(lam[j], 0.f) : ((kind == 1) ? gb * fmaxf(lam[j], 0.f) : 0.f);
-                    warp_transpose_sum32(t, lane);
-                    atomicAdd(&s_red[3 * TBN + c + lane], t[0]);
-                    if (g.nkinds == 3) {       // Jacobian chain: adjoint of phi'(zhat)
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) t[j] = (kind == 2) ? v[j] * lam[j] : 0.f;
-                        warp_transpose_sum32(t, lane);
-                        atomicAdd(&s_red[4 * TBN + c + lane], t[0]);
-                    }
-                    // ---- the masked adjoint of Lambda_l
-                    if (g.write_c) {
-                        const float* pk = (kind == 0 ? g.kU : (kind == 1 ? g.kL : g.dphi)) + po + n0 + c;   // slope on Lam > 0
-                        const float* nk_ = (kind == 0 ? g.kL : (kind == 1 ? g.kU : g.dphi)) + po + n0 + c;  // slope on Lam < 0
-                        const float* pg = (kind == 0 ? g.gU : g.gL) + po + n0 + c;
-                        const float* ng = (kind == 0 ? g.gL : g.gU) + po + n0 + c;
-                        const float gbe = (kind == 2) ? 0.f : gb;
-#pragma unroll
-                        for (int j = 0; j < 32; j += 4) {
-                            const float4 kp = __ldg(reinterpret_cast<const float4*>(pk + j)), kn = __ldg(reinterpret_cast<const float4*>(nk_ + j));
-                            const float4 gp = __ldg(reinterpret_cast<const float4*>(pg + j)), gn = __ldg(reinterpret_cast<const float4*>(ng + j));
-                            float4 o;
-                            o.x = lam[j] > 0.f ? fmaf(v[j], kp.x, gbe * gp.x) : (lam[j] < 0.f ? fmaf(v[j], kn.x, gbe * gn.x) : 0.f);
-                            o.y = lam[j + 1] > 0.f ? fmaf(v[j + 1], kp.y, gbe * gp.y) : (lam[j + 1] < 0.f ? fmaf(v[j + 1], kn.y, gbe * gn.y) : 0.f);
-                            o.z = lam[j + 2] > 0.f ? fmaf(v[j + 2], kp.z, gbe * gp.z) : (lam[j + 2] < 0.f ? fmaf(v[j + 2], kn.z, gbe * gn.z) : 0.f);
-                            o.w = lam[j + 3] > 0.f ? fmaf(v[j + 3], kp.w, gbe * gp.w) : (lam[j + 3] < 0.f ? fmaf(v[j + 3], kn.w, gbe * gn.w) : 0.f);
-                            if (kind == 2) {   // Jacobian chain: Db * phi' irrespective of the sign of Lam (FFMA path: out = Db * d1)
-                                o.x = v[j] * kp.x; o.y = v[j + 1] * kp.y; o.z = v[j + 2] * kp.z; o.w = v[j + 3] * kp.w;
+                    for (int j = 0; j < 16; ++j) {
+                        const int jj = c + j;
+                        const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
+                        const float gb = __shfl_sync(0xffffffffu, gbv, j);
+                        const float Db = a[j] + b[j], lv = lam[j];
+                        float out = 0.f;
+                        if (jj < kbe) {
+                            if (kind == 2) {
+                                sdb = fmaf(Db, lv, sdb);
+                                out = Db * dp;
+                            } else {
+                                const bool up = (kind == 0);
+                                const float P = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                                const float dP = Db * P, dQ = Db * Q, gP = gb * P, gQ = gb * Q;
+                                skU += up ? dP : dQ; skL += up ? dQ : dP;
+                                sgU += up ? gP : gQ; sgL += up ? gQ : gP;
+                                const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
+                                out = lv > 0.f ? fmaf(Db, kp, gb * gp) : (lv < 0.f ? fmaf(Db, kn, gb * gn) : 0.f);
                             }
-                            if (kind < 0) o = make_float4(0.f, 0.f, 0.f, 0.f);
-                            *reinterpret_cast<float4*>(crow + c + j) = o;
                         }
+                        if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
                     }
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) lam[j] = lamn[j];
                 }
-            }
-            // release the accumulator to the MMA warp
-            tc_fence_before();
-            mbar_arrive(bar_tempty(acc));
-            if (MODE == MODE_BWD) {
-                named_bar_sync(1, 128);
-                const int nq = (g.nkinds == 3) ? 5 : 4;
-                for (int i = etid; i < nq * TBN; i += 128) {
-                    const int a = i / TBN, col = i - a * TBN;
-                    if (col >= n_mma) continue;
-                    float* dst = (a == 0 ? g.kUb : a == 1 ? g.kLb : a == 2 ? g.gUb : a == 3 ? g.gLb : g.db) + po + n0 + col;
-                    atomicAdd(dst, s_red[i]);
+                if (n_ok) {
+                    atomicAdd(g.kUb + t.po + n, skU);
+                    atomicAdd(g.kLb + t.po + n, skL);
+                    atomicAdd(g.gUb + t.po + n, sgU);
+                    atomicAdd(g.gLb + t.po + n, sgL);
+                    if (g.nkinds == 3) atomicAdd(g.db + t.po + n, sdb);
                 }
-                named_bar_sync(1, 128);
             }
         }
     } else if (warp >= 8) {
-        // ===================== A producers =====================
-        const int ptid = threadIdx.x - 256, pw = ptid >> 5;
-        const int r4 = lane >> 3, c4 = lane & 7;
+        // ===================== row producers =====================
+        const int pw = warp - 8;                   // 0..7: this warp owns rows [pw*32, pw*32 + 32) of the block
+        const int r4 = lane >> 3, c4 = lane & 7;   // 8 threads per row (one float4 each = 128 B), 4 rows per warp instruction
         int stage = 0; uint32_t phase = 0;
         const float* aptr[8];
-        uint32_t kinds_cur = 0, kinds_nxt = 0;
-        size_t po_cur = 0, po_nxt = 0;
-        int m0_cur = 0, m0_nxt = 0, nb_cur = 0, nb_nxt = 0;
+        uint32_t kinds_cur = 0, kinds_nxt = 0;     // 2 bits per row: 0 upper, 1 lower, 2 Jacobian chain, 3 padding
+        TileGeo t_cur{}, t_nxt{};
         float4 cur[8], nxt[8];
-        auto setup_tile = [&](int tile, uint32_t& kinds, size_t& po, int& m0, int& nb) {
-            const int mb = tile / n_blocks;
-            nb = tile - mb * n_blocks;
-            m0 = mb * TBM;
+        auto setup_tile = [&](int tile, uint32_t& kinds, TileGeo& t) {
+            t = tile_geo(g, tile, col_blocks);
             kinds = 0;
-            int tl = 0;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const int m = m0 + pw * 32 + i * 4 + r4;
-                int kind = 0, rk = 0;
+                const int j = pw * 32 + i * 4 + r4;
                 if (MODE == MODE_FWD) {
-                    chain_row(g, m, tl, kind, rk);
-                    if (kind < 0) { kind = 3; rk = 0; }
-                    aptr[i] = g.A + (size_t)(g.a_shared ? rk : m) * g.lda + c4 * 4;
+                    const int rin = t.rbase + j;
+                    int kind = rin / g.rows_kind;
+                    int rk = rin - kind * g.rows_kind;
+                    if (kind >= g.nkinds) { kind = 3; rk = 0; }
+                    aptr[i] = g.A + (size_t)(g.a_shared ? rk : (t.r0 + j)) * g.lda + c4 * 4;
+                    kinds |= (uint32_t)kind << (2 * i);
                 } else {
-                    aptr[i] = g.A + (size_t)m * g.lda + c4 * 4;
+                    aptr[i] = g.A + (size_t)(t.r0 + j) * g.lda + c4 * 4;
                 }
-                kinds |= (uint32_t)kind << (2 * i);
             }
-            po = (size_t)(m0 / g.rows_pad) * g.ldp;
         };
         auto load_slab = [&](float4* dst, uint32_t kinds, int kt) {
 #pragma unroll
@@ -398,10 +414,28 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 dst[i] = ok ? __ldg(reinterpret_cast<const float4*>(aptr[i] + kt * TBK)) : make_float4(0.f, 0.f, 0.f, 0.f);
             }
         };
+        auto split_store = [&](const float4& v, uint32_t r_hi, uint32_t r_lo, int row) {
+            float4 hi, lo;
+            hi.x = to_tf32(v.x); hi.y = to_tf32(v.y); hi.z = to_tf32(v.z); hi.w = to_tf32(v.w);
+            lo.x = to_tf32(v.x - hi.x); lo.y = to_tf32(v.y - hi.y); lo.z = to_tf32(v.z - hi.z); lo.w = to_tf32(v.w - hi.w);
+            const uint32_t off = (uint32_t)row * 128u + (uint32_t)((c4 ^ (row & 7)) << 4);     // 128B swizzle
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_hi + off), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_lo + off), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w) : "memory");
+        };
+        auto relax4 = [&](float4& v, const float4& kp, const float4& kn) {
+            v.x *= v.x > 0.f ? kp.x : kn.x;
+            v.y *= v.y > 0.f ? kp.y : kn.y;
+            v.z *= v.z > 0.f ? kp.z : kn.z;
+            v.w *= v.w > 0.f ? kp.w : kn.w;
+        };
+        auto gap4 = [&](const float4& v, const float4& gp, const float4& gn) {
+            return (v.x > 0.f ? v.x * gp.x : v.x * gn.x) + (v.y > 0.f ? v.y * gp.y : v.y * gn.y) +
+                   (v.z > 0.f ? v.z * gp.z : v.z * gn.z) + (v.w > 0.f ? v.w * gp.w : v.w * gn.w);
+        };
         int tile = blockIdx.x, kt = 0;
         bool have = tile < num_tiles;
         if (have) {
-            setup_tile(tile, kinds_cur, po_cur, m0_cur, nb_cur);
+            setup_tile(tile, kinds_cur, t_cur);
             load_slab(cur, kinds_cur, 0);
         }
         float gsum[8];
@@ -412,52 +446,52 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             int ntile = tile, nkt = kt + 1;
             if (nkt == nk) { nkt = 0; ntile = tile + gridDim.x; }
             const bool nhave = ntile < num_tiles;
-            kinds_nxt = kinds_cur; po_nxt = po_cur; m0_nxt = m0_cur; nb_nxt = nb_cur;
+            kinds_nxt = kinds_cur; t_nxt = t_cur;
             if (nhave) {
-                if (nkt == 0) setup_tile(ntile, kinds_nxt, po_nxt, m0_nxt, nb_nxt);
+                if (nkt == 0) setup_tile(ntile, kinds_nxt, t_nxt);
                 load_slab(nxt, kinds_nxt, nkt);
             }
             // ---- transform + split the current slab into the stage
             const int col = kt * TBK + c4 * 4;
             float4 kU4 = make_float4(0.f, 0.f, 0.f, 0.f), kL4 = kU4, dp4 = kU4, gU4 = kU4, gL4 = kU4;
-            const bool do_gap = (MODE == MODE_FWD) && (nb_cur == 0) && (g.gap != nullptr);
+            const bool do_gap = (MODE == MODE_FWD) && (t_cur.n0 == 0) && (g.gap != nullptr);
             if (MODE == MODE_FWD) {
-                kU4 = __ldg(reinterpret_cast<const float4*>(g.kU + po_cur + col));
-                kL4 = __ldg(reinterpret_cast<const float4*>(g.kL + po_cur + col));
-                if (g.nkinds == 3) dp4 = __ldg(reinterpret_cast<const float4*>(g.dphi + po_cur + col));
+                kU4 = __ldg(reinterpret_cast<const float4*>(g.kU + t_cur.po + col));
+                kL4 = __ldg(reinterpret_cast<const float4*>(g.kL + t_cur.po + col));
+                if (g.nkinds == 3) dp4 = __ldg(reinterpret_cast<const float4*>(g.dphi + t_cur.po + col));
                 if (do_gap) {
-                    gU4 = __ldg(reinterpret_cast<const float4*>(g.gU + po_cur + col));
-                    gL4 = __ldg(reinterpret_cast<const float4*>(g.gL + po_cur + col));
+                    gU4 = __ldg(reinterpret_cast<const float4*>(g.gU + t_cur.po + col));
+                    gL4 = __ldg(reinterpret_cast<const float4*>(g.gL + t_cur.po + col));
                 }
             }
             mbar_wait(bar_empty(stage), phase ^ 1);
-            const uint32_t a_hi = sA(stage, 0), a_lo = sA(stage, 1);
+            const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
+            if (MODE == MODE_FWD && (kinds_cur == 0u || kinds_cur == 0x5555u)) {
+                // all 8 rows of this thread on one chain (always the case for hidden-layer targets)
+                const float4 kp = kinds_cur == 0u ? kU4 : kL4, kn = kinds_cur == 0u ? kL4 : kU4;
+                const float4 gp = kinds_cur == 0u ? gU4 : gL4, gn = kinds_cur == 0u ? gL4 : gU4;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                float4 v = cur[i];
-                if (MODE == MODE_FWD) {
-                    const uint32_t kind = (kinds_cur >> (2 * i)) & 3u;
-                    const float4 kp = kind == 0 ? kU4 : (kind == 1 ? kL4 : dp4);
-                    const float4 kn = kind == 0 ? kL4 : (kind == 1 ? kU4 : dp4);
-                    if (do_gap && kind < 2) {
-                        const float4 gp = kind == 0 ? gU4 : gL4, gn = kind == 0 ? gL4 : gU4;
-                        gsum[i] += (v.x > 0.f ? v.x * gp.x : v.x * gn.x) + (v.y > 0.f ? v.y * gp.y : v.y * gn.y) +
-                                   (v.z > 0.f ? v.z * gp.z : v.z * gn.z) + (v.w > 0.f ? v.w * gp.w : v.w * gn.w);
-                    }
-                    if (kind != 3u) {
-                        v.x = v.x > 0.f ? v.x * kp.x : v.x * kn.x;
-                        v.y = v.y > 0.f ? v.y * kp.y : v.y * kn.y;
-                        v.z = v.z > 0.f ? v.z * kp.z : v.z * kn.z;
-                        v.w = v.w > 0.f ? v.w * kp.w : v.w * kn.w;
-                    }
+                for (int i = 0; i < 8; ++i) {
+                    float4 v = cur[i];
+                    if (do_gap) gsum[i] += gap4(v, gp, gn);
+                    relax4(v, kp, kn);
+                    split_store(v, r_hi, r_lo, pw * 32 + i * 4 + r4);
                 }
-                float4 hi, lo;
-                hi.x = to_tf32(v.x); hi.y = to_tf32(v.y); hi.z = to_tf32(v.z); hi.w = to_tf32(v.w);
-                lo.x = to_tf32(v.x - hi.x); lo.y = to_tf32(v.y - hi.y); lo.z = to_tf32(v.z - hi.z); lo.w = to_tf32(v.w - hi.w);
-                const int row = pw * 32 + i * 4 + r4;
-                const uint32_t off = (uint32_t)row * 128u + (uint32_t)((c4 ^ (row & 7)) << 4);
-                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a_hi + off), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
-                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a_lo + off), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w) : "memory");
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    float4 v = cur[i];
+                    if (MODE == MODE_FWD) {
+                        const uint32_t kind = (kinds_cur >> (2 * i)) & 3u;
+                        if (kind < 2u) {
+                            if (do_gap) gsum[i] += gap4(v, kind == 0u ? gU4 : gL4, kind == 0u ? gL4 : gU4);
+                            relax4(v, kind == 0u ? kU4 : kL4, kind == 0u ? kL4 : kU4);
+                        } else if (kind == 2u) {
+                            relax4(v, dp4, dp4);
+                        }
+                    }
+                    split_store(v, r_hi, r_lo, pw * 32 + i * 4 + r4);
+                }
             }
             fence_proxy_async();                 // generic-proxy stores -> visible to the tensor core's async proxy
             mbar_arrive(bar_full(stage));
@@ -471,7 +505,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         s += __shfl_xor_sync(0xffffffffu, s, 1);
                         s += __shfl_xor_sync(0xffffffffu, s, 2);
                         s += __shfl_xor_sync(0xffffffffu, s, 4);
-                        const int m = m0_cur + pw * 32 + i * 4 + r4;
+                        const int m = t_cur.r0 + pw * 32 + i * 4 + r4;
                         if (c4 == 0) g.gap[m] = (g.gap_init ? 0.f : g.gap[m]) + s;
                     }
                 }
@@ -480,7 +514,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             }
             // ---- advance
             tile = ntile; kt = nkt; have = nhave;
-            kinds_cur = kinds_nxt; po_cur = po_nxt; m0_cur = m0_nxt; nb_cur = nb_nxt;
+            kinds_cur = kinds_nxt; t_cur = t_nxt;
 #pragma unroll
             for (int i = 0; i < 8; ++i) cur[i] = nxt[i];
         }
@@ -514,13 +548,14 @@ inline EncodeTiledFn encode_fn() {
     return fn;
 }
 
-// tensor map of a row-major FP32 matrix [rows x cols] (cols contiguous, cols % 32 == 0): box = 32 cols x 256 rows, 128B swizzle
+// tensor map of a row-major FP32 matrix [rows x cols] (cols contiguous, cols % 32 == 0): box = 32 cols x 128 rows,
+// 128B swizzle; rows beyond the matrix are zero-filled
 inline bool make_weight_map(CUtensorMap* map, const float* dptr, int rows, int cols) {
     EncodeTiledFn fn = encode_fn();
     if (!fn) return false;
     cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
     cuuint64_t strides[1] = {(cuuint64_t)cols * sizeof(float)};
-    cuuint32_t box[2] = {(cuuint32_t)TBK, (cuuint32_t)TBN};
+    cuuint32_t box[2] = {(cuuint32_t)TBK, (cuuint32_t)TBM};
     cuuint32_t estr[2] = {1, 1};
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(dptr), dims, strides, box, estr,
                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -528,6 +563,7 @@ inline bool make_weight_map(CUtensorMap* map, const float* dptr, int rows, int c
     return r == CUDA_SUCCESS;
 }
 
+// g.M (coefficient rows) must be a multiple of 256, g.K and g.N multiples of 32
 template <int MODE>
 inline cudaError_t launch_chain_gemm_tc(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
     static bool attr_done = false;
@@ -536,7 +572,8 @@ inline cudaError_t launch_chain_gemm_tc(const GemmArgs& g, const CUtensorMap& hi
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int tiles = (g.M / TBM) * ((g.N + TBN - 1) / TBN);
+    if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
+    const int tiles = (g.M / TBN) * ((g.N + TBM - 1) / TBM);
     const int grid = tiles < num_sms ? tiles : num_sms;
     chain_gemm_tc_kernel<MODE><<<grid, THREADS, SMEM_BYTES, st>>>(g, hi, lo);
     return cudaGetLastError();
