@@ -37,12 +37,15 @@ enum { MODE_FWD = 0, MODE_BWD = 1 };
 
 constexpr int TBM = 128;      // output columns per tile (MMA M, weights)
 constexpr int TBN = 256;      // coefficient rows per tile (MMA N)
-constexpr int TBK = 32, STAGES = 2;
-constexpr int W_TILE_BYTES = TBM * TBK * 4;                         // 16 KB
-constexpr int R_TILE_BYTES = TBN * TBK * 4;                         // 32 KB
-constexpr int STAGE_BYTES = 2 * W_TILE_BYTES + 2 * R_TILE_BYTES;    // 96 KB
+constexpr int TBK = 32;
+constexpr int WSTAGES = 3;    // weight ring (TMA: L2 latency ~ one K slab of MMA time, so one stage deeper than the rows)
+constexpr int RSTAGES = 2;    // coefficient-row ring (register path, prefetched one slab ahead)
+constexpr int W_TILE_BYTES = TBM * TBK * 4;                         // 16 KB (hi) + 16 KB (lo) per stage
+constexpr int R_TILE_BYTES = TBN * TBK * 4;                         // 32 KB (hi) + 32 KB (lo) per stage
+constexpr int RING_BYTES = WSTAGES * 2 * W_TILE_BYTES + RSTAGES * 2 * R_TILE_BYTES;   // 96 KB + 128 KB
+constexpr int PAR_BYTES = 5 * TBK * 4;                              // per-neuron parameters of one K slab: kU, kL, phi', gU, gL
 constexpr int BAR_BYTES = 128;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;   // + 1024-byte alignment slack
+constexpr int SMEM_BYTES = RING_BYTES + WSTAGES * PAR_BYTES + BAR_BYTES + 1024;   // + 1024-byte alignment slack (= 227 KB)
 constexpr int THREADS = 512;
 constexpr int PRODUCERS = 256;
 constexpr int TMEM_COLS = 512;
@@ -92,6 +95,11 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar)
         : "memory");
+}
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -156,6 +164,10 @@ __device__ __forceinline__ float to_tf32(float x) {
 }
 __device__ __forceinline__ void named_bar_sync(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
 
+// register re-distribution between the warp roles (warpgroup granularity; 512 threads start with 128 registers each)
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
 // K-major, 128B-swizzled operand tile: rows of 128 bytes, 8-row groups 1024 bytes apart
 __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
     uint64_t d = 0;
@@ -201,14 +213,23 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     extern __shared__ uint8_t smem_raw[];
     const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* sgen = smem_raw + (sbase - smem_u32(smem_raw));           // generic pointer to the aligned base
-    // stage s: [Whi | Wlo | Rhi | Rlo]
-    auto sW = [&](int s, int part) { return sbase + s * STAGE_BYTES + part * W_TILE_BYTES; };
-    auto sR = [&](int s, int part) { return sbase + s * STAGE_BYTES + 2 * W_TILE_BYTES + part * R_TILE_BYTES; };
-    const uint32_t bar0 = sbase + STAGES * STAGE_BYTES;
-    auto bar_full = [&](int s) { return bar0 + 8 * s; };
-    auto bar_empty = [&](int s) { return bar0 + 8 * (STAGES + s); };
-    const uint32_t bar_tfull = bar0 + 8 * (2 * STAGES), bar_tempty = bar0 + 8 * (2 * STAGES + 1);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + STAGES * STAGE_BYTES + 8 * (2 * STAGES + 2));
+    // weight ring: stage s = [Whi | Wlo]; row ring: stage s = [Rhi | Rlo]
+    auto sW = [&](int s, int part) { return sbase + (2 * s + part) * W_TILE_BYTES; };
+    auto sR = [&](int s, int part) { return sbase + WSTAGES * 2 * W_TILE_BYTES + (2 * s + part) * R_TILE_BYTES; };
+    // the slab's per-neuron parameters travel with the weight stage (forward only): [kU | kL | phi' | gU | gL] x 32 floats
+    auto sP = [&](int s) { return sbase + RING_BYTES + s * PAR_BYTES; };
+    const uint32_t bar0 = sbase + RING_BYTES + WSTAGES * PAR_BYTES;
+    auto bar_wfull = [&](int s) { return bar0 + 8 * s; };
+    auto bar_wempty = [&](int s) { return bar0 + 8 * (WSTAGES + s); };
+    auto bar_rfull = [&](int s) { return bar0 + 8 * (2 * WSTAGES + s); };
+    auto bar_rempty = [&](int s) { return bar0 + 8 * (2 * WSTAGES + RSTAGES + s); };
+    auto bar_tfull = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + a); };
+    auto bar_tempty = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + 2 + a); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + RING_BYTES + WSTAGES * PAR_BYTES + 8 * (2 * WSTAGES + 2 * RSTAGES + 4));
+    // forward: one accumulator pair (main [0,256), correction [256,512)); reverse sweep: the gradient tolerance
+    // (1e-4) leaves room for the truncation of a single accumulator, so two of them alternate and the epilogue
+    // of tile i overlaps the main loop of tile i+1
+    constexpr int NACC = (MODE == MODE_BWD) ? 2 : 1;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int col_blocks = (g.N + TBM - 1) / TBM;
@@ -221,9 +242,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         tma_prefetch_desc(&tm_lo);
     }
     if (warp == 1 && lane == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(bar_full(s), PRODUCERS + 1); mbar_init(bar_empty(s), 1); }
-        mbar_init(bar_tfull, 1);
-        mbar_init(bar_tempty, 128);
+        for (int s = 0; s < WSTAGES; ++s) { mbar_init(bar_wfull(s), 1); mbar_init(bar_wempty(s), 1); }
+        for (int s = 0; s < RSTAGES; ++s) { mbar_init(bar_rfull(s), PRODUCERS); mbar_init(bar_rempty(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), 128); }
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
@@ -231,54 +252,79 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    // registers per thread: control warps 40; forward: epilogue 104, producers 184 (three slabs of rows in flight
+    // plus the slopes of two); reverse sweep: epilogue 168 (four steps of forward coefficients in flight), producers 152
+    constexpr int kEpiRegs = (MODE == MODE_FWD) ? 104 : 168, kProdRegs = (MODE == MODE_FWD) ? 184 : 152;
 
+    if (warp < 4) reg_dec<40>();
     if (warp == 0) {
         // ===================== TMA producer (weights) =====================
         int stage = 0; uint32_t phase = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-            const int n0 = (tile % col_blocks) * TBM;
+            const TileGeo t = tile_geo(g, tile, col_blocks);
+            const int n0 = t.n0;
             for (int kt = 0; kt < nk; ++kt) {
-                mbar_wait(bar_empty(stage), phase ^ 1);
+                mbar_wait(bar_wempty(stage), phase ^ 1);
                 if (lane == 0) {
-                    mbar_arrive_expect_tx(bar_full(stage), 2 * W_TILE_BYTES);
-                    tma_load_2d(sW(stage, 0), &tm_hi, kt * TBK, n0, bar_full(stage));
-                    tma_load_2d(sW(stage, 1), &tm_lo, kt * TBK, n0, bar_full(stage));
+                    mbar_arrive_expect_tx(bar_wfull(stage), 2 * W_TILE_BYTES + (MODE == MODE_FWD ? PAR_BYTES : 0));
+                    tma_load_2d(sW(stage, 0), &tm_hi, kt * TBK, n0, bar_wfull(stage));
+                    tma_load_2d(sW(stage, 1), &tm_lo, kt * TBK, n0, bar_wfull(stage));
+                    if (MODE == MODE_FWD) {
+                        const size_t o = t.po + (size_t)kt * TBK;
+                        bulk_load_1d(sP(stage) + 0 * TBK * 4, g.kU + o, TBK * 4, bar_wfull(stage));
+                        bulk_load_1d(sP(stage) + 1 * TBK * 4, g.kL + o, TBK * 4, bar_wfull(stage));
+                        bulk_load_1d(sP(stage) + 2 * TBK * 4, g.dphi + o, TBK * 4, bar_wfull(stage));
+                        bulk_load_1d(sP(stage) + 3 * TBK * 4, g.gU + o, TBK * 4, bar_wfull(stage));
+                        bulk_load_1d(sP(stage) + 4 * TBK * 4, g.gL + o, TBK * 4, bar_wfull(stage));
+                    }
                 }
                 __syncwarp();
-                if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                if (++stage == WSTAGES) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer =====================
-        int stage = 0; uint32_t phase = 0;
+        int ws = 0, rs = 0; uint32_t wphase = 0, rphase = 0;
         const uint32_t idesc = make_idesc(TBM, TBN);
-        const uint32_t d_main = tmem_base, d_corr = tmem_base + TBN;
         int tcount = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
-            mbar_wait(bar_tempty, (tcount & 1) ^ 1);          // the epilogue has drained the previous tile
+            const int acc = tcount % NACC;
+            mbar_wait(bar_tempty(acc), ((tcount / NACC) & 1) ^ 1);          // the epilogue has drained this accumulator
             tc_fence_after();
+            const uint32_t d_main = tmem_base + acc * TBN;
+            const uint32_t d_corr = (MODE == MODE_BWD) ? d_main : tmem_base + TBN;
             for (int kt = 0; kt < nk; ++kt) {
-                mbar_wait(bar_full(stage), phase);
+                mbar_wait(bar_wfull(ws), wphase);
+                mbar_wait(bar_rfull(rs), rphase);
                 tc_fence_after();
                 if (lane == 0) {
-                    const uint64_t whi = make_smem_desc(sW(stage, 0)), wlo = make_smem_desc(sW(stage, 1));
-                    const uint64_t rhi = make_smem_desc(sR(stage, 0)), rlo = make_smem_desc(sR(stage, 1));
+                    const uint64_t whi = make_smem_desc(sW(ws, 0)), wlo = make_smem_desc(sW(ws, 1));
+                    const uint64_t rhi = make_smem_desc(sR(rs, 0)), rlo = make_smem_desc(sR(rs, 1));
 #pragma unroll
                     for (int k = 0; k < TBK / 8; ++k) {
                         const uint64_t ko = (uint64_t)(k * 32 >> 4);     // 8 tf32 = 32 bytes along K inside the swizzle atom
-                        umma_tf32(d_main, whi + ko, rhi + ko, idesc, (kt | k) != 0);
-                        umma_tf32(d_corr, whi + ko, rlo + ko, idesc, (kt | k) != 0);
-                        umma_tf32(d_corr, wlo + ko, rhi + ko, idesc, 1u);
+                        if (MODE == MODE_BWD) {
+                            umma_tf32(d_main, whi + ko, rlo + ko, idesc, (kt | k) != 0);
+                            umma_tf32(d_main, wlo + ko, rhi + ko, idesc, 1u);
+                            umma_tf32(d_main, whi + ko, rhi + ko, idesc, 1u);
+                        } else {
+                            umma_tf32(d_main, whi + ko, rhi + ko, idesc, (kt | k) != 0);
+                            umma_tf32(d_corr, whi + ko, rlo + ko, idesc, (kt | k) != 0);
+                            umma_tf32(d_corr, wlo + ko, rhi + ko, idesc, 1u);
+                        }
                     }
-                    umma_commit(bar_empty(stage));                       // frees the stage when these MMAs retire
-                    if (kt == nk - 1) umma_commit(bar_tfull);            // accumulators complete
+                    umma_commit(bar_wempty(ws));                         // both stages are free when these MMAs retire
+                    umma_commit(bar_rempty(rs));
+                    if (kt == nk - 1) umma_commit(bar_tfull(acc));       // accumulators complete
                 }
                 __syncwarp();
-                if (++stage == STAGES) { stage = 0; phase ^= 1; }
+                if (++ws == WSTAGES) { ws = 0; wphase ^= 1; }
+                if (++rs == RSTAGES) { rs = 0; rphase ^= 1; }
             }
         }
     } else if (warp >= 4 && warp < 8) {
         // ===================== epilogue: TMEM lane = output column, TMEM column = coefficient row =====================
+        if (kEpiRegs < 128) reg_dec<kEpiRegs>(); else reg_inc<kEpiRegs>();
         const int q = warp - 4;                                  // TMEM lane quadrant of this warp (warp % 4)
         const uint32_t t_lane = tmem_base + ((uint32_t)(q * 32) << 16);
         int tcount = 0;
@@ -286,23 +332,38 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             const TileGeo t = tile_geo(g, tile, col_blocks);
             const int n = t.n0 + q * 32 + lane;                  // this thread's output column
             const bool n_ok = n < g.N;
+            const int acc = tcount % NACC;
+            const uint32_t acc_parity = (tcount / NACC) & 1;
             if (MODE == MODE_FWD) {
-                mbar_wait(bar_tfull, tcount & 1);
+                mbar_wait(bar_tfull(acc), acc_parity);
                 tc_fence_after();
                 float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
+                // 16 rows per step, the TMEM loads of step i+1 in flight while step i is stored
+                float a0[16], b0[16], a1[16], b1[16];
+                tmem_ld<16>(t_lane, a0);
+                tmem_ld<16>(t_lane + TBN, b0);
 #pragma unroll 1
                 for (int c = 0; c < TBN; c += 32) {
-                    float a[32], b[32];
-                    tmem_ld<32>(t_lane + c, a);
-                    tmem_ld<32>(t_lane + TBN + c, b);
                     tmem_ld_wait();
+                    tmem_ld<16>(t_lane + c + 16, a1);
+                    tmem_ld<16>(t_lane + TBN + c + 16, b1);
                     if (n_ok) {
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) cbase[(size_t)(c + j) * g.ldc] = a[j] + b[j];   // 128 B per warp and row
+                        for (int j = 0; j < 16; ++j) cbase[(size_t)(c + j) * g.ldc] = a0[j] + b0[j];   // 128 B per warp and row
+                    }
+                    tmem_ld_wait();
+                    if (c + 32 < TBN) {
+                        tmem_ld<16>(t_lane + c + 32, a0);
+                        tmem_ld<16>(t_lane + TBN + c + 32, b0);
+                    } else {                                             // last read of this tile's accumulators: release them
+                        tc_fence_before();
+                        mbar_arrive(bar_tempty(acc));
+                    }
+                    if (n_ok) {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) cbase[(size_t)(c + 16 + j) * g.ldc] = a1[j] + b1[j];
                     }
                 }
-                tc_fence_before();
-                mbar_arrive(bar_tempty);
             } else {
                 // row kinds inside the block: [0,kb1) upper chain, [kb1,kb2) lower, [kb2,kbe) Jacobian, then padding
                 const int kb1 = g.rows_kind - t.rbase, kb2 = 2 * g.rows_kind - t.rbase, kbe = g.nkinds * g.rows_kind - t.rbase;
@@ -322,35 +383,43 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
                     }
                 };
-                float lam[16], lamn[16];
-                load_lam(lam, 0);                                // overlaps the tail of the main loop
-                mbar_wait(bar_tfull, tcount & 1);
+                auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
+                    const int jj = c + (lane & 15);
+                    const int kind = (jj >= kb1) + (jj >= kb2);
+                    return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
+                };
+                // forward coefficients three steps (48 rows) ahead of their use -- they come from HBM; the first three
+                // steps are requested before the accumulator is complete and overlap the main loop
+                float lam0[16], lam1[16], lam2[16], lam3[16];
+                float gb0, gb1, gb2, gb3 = 0.f;
+                load_lam(lam0, 0); gb0 = load_gb(0);
+                load_lam(lam1, 16); gb1 = load_gb(16);
+                load_lam(lam2, 32); gb2 = load_gb(32);
+                mbar_wait(bar_tfull(acc), acc_parity);
                 tc_fence_after();
+                const uint32_t t_acc = t_lane + acc * TBN;
                 float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
-#pragma unroll 1
-                for (int c = 0; c < TBN; c += 16) {
-                    float a[16], b[16];
-                    tmem_ld<16>(t_lane + c, a);
-                    tmem_ld<16>(t_lane + TBN + c, b);
-                    if (c + 16 < TBN) load_lam(lamn, c + 16);
-                    // the row's gap adjoint: lane j < 16 fetches row c + j, broadcast below
-                    float gbv = 0.f;
-                    {
-                        const int jj = c + (lane & 15);
-                        const int kind = (jj >= kb1) + (jj >= kb2);
-                        if (jj < kbe && kind < 2) gbv = __ldg(g.gapbar + t.r0 + jj);
-                    }
+                float a[16];
+                tmem_ld<16>(t_acc, a);
+                // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+48, c+64) into L
+                auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
+                    if (c + 48 < TBN) { load_lam(L, c + 48); gbL = load_gb(c + 48); }
                     tmem_ld_wait();
-                    if (c + 16 >= TBN) {                         // last read of this tile's accumulators: release them
+                    float d[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) d[j] = a[j];
+                    if (c + 16 < TBN) {
+                        tmem_ld<16>(t_acc + c + 16, a);
+                    } else {                                             // last read of this accumulator: release it
                         tc_fence_before();
-                        mbar_arrive(bar_tempty);
+                        mbar_arrive(bar_tempty(acc));
                     }
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
                         const int jj = c + j;
                         const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
-                        const float gb = __shfl_sync(0xffffffffu, gbv, j);
-                        const float Db = a[j] + b[j], lv = lam[j];
+                        const float gb = __shfl_sync(0xffffffffu, gbP, j);
+                        const float Db = d[j], lv = P[j];
                         float out = 0.f;
                         if (jj < kbe) {
                             if (kind == 2) {
@@ -358,8 +427,8 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                                 out = Db * dp;
                             } else {
                                 const bool up = (kind == 0);
-                                const float P = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
-                                const float dP = Db * P, dQ = Db * Q, gP = gb * P, gQ = gb * Q;
+                                const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                                const float dP = Db * Pp, dQ = Db * Q, gP = gb * Pp, gQ = gb * Q;
                                 skU += up ? dP : dQ; skL += up ? dQ : dP;
                                 sgU += up ? gP : gQ; sgL += up ? gQ : gP;
                                 const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
@@ -368,8 +437,13 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                         if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
                     }
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) lam[j] = lamn[j];
+                };
+#pragma unroll 1
+                for (int c = 0; c < TBN; c += 64) {
+                    estep(c, lam0, gb0, lam3, gb3);
+                    estep(c + 16, lam1, gb1, lam0, gb0);
+                    estep(c + 32, lam2, gb2, lam1, gb1);
+                    estep(c + 48, lam3, gb3, lam2, gb2);
                 }
                 if (n_ok) {
                     atomicAdd(g.kUb + t.po + n, skU);
@@ -382,16 +456,23 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         }
     } else if (warp >= 8) {
         // ===================== row producers =====================
+        // Two cursors walk the CTA's sequence of (tile, K slab): the LOADER issues the global loads of a slab
+        // into one of three register buffers two slabs ahead of the TRANSFORMER, which relaxes, splits and
+        // stores the oldest buffer into the stage the MMA warp has released.  HBM latency (~1.5 slabs of MMA
+        // time) is covered by the two slabs in flight; the per-neuron slopes are fetched one slab ahead.
+        reg_inc<kProdRegs>();
         const int pw = warp - 8;                   // 0..7: this warp owns rows [pw*32, pw*32 + 32) of the block
         const int r4 = lane >> 3, c4 = lane & 7;   // 8 threads per row (one float4 each = 128 B), 4 rows per warp instruction
-        int stage = 0; uint32_t phase = 0;
-        const float* aptr[8];
-        uint32_t kinds_cur = 0, kinds_nxt = 0;     // 2 bits per row: 0 upper, 1 lower, 2 Jacobian chain, 3 padding
-        TileGeo t_cur{}, t_nxt{};
-        float4 cur[8], nxt[8];
-        auto setup_tile = [&](int tile, uint32_t& kinds, TileGeo& t) {
-            t = tile_geo(g, tile, col_blocks);
-            kinds = 0;
+        const float4* const A4 = reinterpret_cast<const float4*>(g.A);
+        const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        // ---- loader cursor
+        int ltile = blockIdx.x, lkt = 0;
+        bool lhave = ltile < num_tiles;
+        uint32_t aoff[8];                          // row offsets into A in float4 units
+        uint32_t lkinds = 0;                       // 2 bits per row: 0 upper, 1 lower, 2 Jacobian chain, 3 padding
+        auto setup_load = [&]() {
+            const TileGeo t = tile_geo(g, ltile, col_blocks);
+            lkinds = 0;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const int j = pw * 32 + i * 4 + r4;
@@ -400,19 +481,38 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     int kind = rin / g.rows_kind;
                     int rk = rin - kind * g.rows_kind;
                     if (kind >= g.nkinds) { kind = 3; rk = 0; }
-                    aptr[i] = g.A + (size_t)(g.a_shared ? rk : (t.r0 + j)) * g.lda + c4 * 4;
-                    kinds |= (uint32_t)kind << (2 * i);
+                    aoff[i] = (uint32_t)(((size_t)(g.a_shared ? rk : (t.r0 + j)) * g.lda) >> 2) + c4;
+                    lkinds |= (uint32_t)kind << (2 * i);
                 } else {
-                    aptr[i] = g.A + (size_t)(t.r0 + j) * g.lda + c4 * 4;
+                    aoff[i] = (uint32_t)(((size_t)(t.r0 + j) * g.lda) >> 2) + c4;
                 }
             }
         };
-        auto load_slab = [&](float4* dst, uint32_t kinds, int kt) {
+        auto issue = [&](float4* buf, uint32_t& bkinds) {
+            bkinds = lkinds;
+            if (!lhave) return;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const bool ok = ((kinds >> (2 * i)) & 3u) != 3u;
-                dst[i] = ok ? __ldg(reinterpret_cast<const float4*>(aptr[i] + kt * TBK)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const bool ok = ((lkinds >> (2 * i)) & 3u) != 3u;
+                buf[i] = ok ? __ldg(A4 + aoff[i] + lkt * (TBK / 4)) : zero4;
             }
+            if (++lkt == nk) {
+                lkt = 0;
+                ltile += gridDim.x;
+                lhave = ltile < num_tiles;
+                if (lhave) setup_load();
+            }
+        };
+        // ---- transformer cursor
+        int ptile = blockIdx.x, pkt = 0;
+        bool phave = ptile < num_tiles;
+        TileGeo t_cur = tile_geo(g, phave ? ptile : 0, col_blocks);
+        int stage = 0; uint32_t phase = 0;
+        int ws = 0; uint32_t wphase = 0;           // weight/parameter stage of the slab being transformed
+        auto lds4 = [&](uint32_t addr) {
+            float4 v;
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+            return v;
         };
         auto split_store = [&](const float4& v, uint32_t r_hi, uint32_t r_lo, int row) {
             float4 hi, lo;
@@ -432,47 +532,40 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             return (v.x > 0.f ? v.x * gp.x : v.x * gn.x) + (v.y > 0.f ? v.y * gp.y : v.y * gn.y) +
                    (v.z > 0.f ? v.z * gp.z : v.z * gn.z) + (v.w > 0.f ? v.w * gp.w : v.w * gn.w);
         };
-        int tile = blockIdx.x, kt = 0;
-        bool have = tile < num_tiles;
-        if (have) {
-            setup_tile(tile, kinds_cur, t_cur);
-            load_slab(cur, kinds_cur, 0);
-        }
         float gsum[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) gsum[i] = 0.f;
-        while (have) {
-            // ---- prefetch the next slab (possibly of the next tile) into registers
-            int ntile = tile, nkt = kt + 1;
-            if (nkt == nk) { nkt = 0; ntile = tile + gridDim.x; }
+
+        // one step: prefetch into L (two slabs ahead), transform P (kinds kP); returns false after the last slab
+        auto step = [&](float4* P, uint32_t kP, float4* L, uint32_t& kL) -> bool {
+            issue(L, kL);
+            // position of the next slab to transform
+            int ntile = ptile, nkt = pkt + 1;
+            TileGeo t_nxt = t_cur;
+            if (nkt == nk) { nkt = 0; ntile = ptile + gridDim.x; }
             const bool nhave = ntile < num_tiles;
-            kinds_nxt = kinds_cur; t_nxt = t_cur;
-            if (nhave) {
-                if (nkt == 0) setup_tile(ntile, kinds_nxt, t_nxt);
-                load_slab(nxt, kinds_nxt, nkt);
-            }
-            // ---- transform + split the current slab into the stage
-            const int col = kt * TBK + c4 * 4;
-            float4 kU4 = make_float4(0.f, 0.f, 0.f, 0.f), kL4 = kU4, dp4 = kU4, gU4 = kU4, gL4 = kU4;
+            if (nhave && nkt == 0) t_nxt = tile_geo(g, ntile, col_blocks);
             const bool do_gap = (MODE == MODE_FWD) && (t_cur.n0 == 0) && (g.gap != nullptr);
+            float4 kUc = zero4, kLc = zero4, dpc = zero4, gU4 = zero4, gL4 = zero4;
             if (MODE == MODE_FWD) {
-                kU4 = __ldg(reinterpret_cast<const float4*>(g.kU + t_cur.po + col));
-                kL4 = __ldg(reinterpret_cast<const float4*>(g.kL + t_cur.po + col));
-                if (g.nkinds == 3) dp4 = __ldg(reinterpret_cast<const float4*>(g.dphi + t_cur.po + col));
-                if (do_gap) {
-                    gU4 = __ldg(reinterpret_cast<const float4*>(g.gU + t_cur.po + col));
-                    gL4 = __ldg(reinterpret_cast<const float4*>(g.gL + t_cur.po + col));
-                }
+                // the slab's parameters arrived with its weight stage (TMA warp); the stage is not recycled before
+                // the MMAs of this slab retire, i.e. long after these reads
+                mbar_wait(bar_wfull(ws), wphase);
+                const uint32_t pp = sP(ws) + c4 * 16;
+                kUc = lds4(pp); kLc = lds4(pp + TBK * 4);
+                if (g.nkinds == 3) dpc = lds4(pp + 2 * TBK * 4);
+                if (do_gap) { gU4 = lds4(pp + 3 * TBK * 4); gL4 = lds4(pp + 4 * TBK * 4); }
+                if (++ws == WSTAGES) { ws = 0; wphase ^= 1; }
             }
-            mbar_wait(bar_empty(stage), phase ^ 1);
+            mbar_wait(bar_rempty(stage), phase ^ 1);
             const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
-            if (MODE == MODE_FWD && (kinds_cur == 0u || kinds_cur == 0x5555u)) {
+            if (MODE == MODE_FWD && (kP == 0u || kP == 0x5555u)) {
                 // all 8 rows of this thread on one chain (always the case for hidden-layer targets)
-                const float4 kp = kinds_cur == 0u ? kU4 : kL4, kn = kinds_cur == 0u ? kL4 : kU4;
-                const float4 gp = kinds_cur == 0u ? gU4 : gL4, gn = kinds_cur == 0u ? gL4 : gU4;
+                const float4 kp = kP == 0u ? kUc : kLc, kn = kP == 0u ? kLc : kUc;
+                const float4 gp = kP == 0u ? gU4 : gL4, gn = kP == 0u ? gL4 : gU4;
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    float4 v = cur[i];
+                    float4 v = P[i];
                     if (do_gap) gsum[i] += gap4(v, gp, gn);
                     relax4(v, kp, kn);
                     split_store(v, r_hi, r_lo, pw * 32 + i * 4 + r4);
@@ -480,24 +573,24 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             } else {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    float4 v = cur[i];
+                    float4 v = P[i];
                     if (MODE == MODE_FWD) {
-                        const uint32_t kind = (kinds_cur >> (2 * i)) & 3u;
+                        const uint32_t kind = (kP >> (2 * i)) & 3u;
                         if (kind < 2u) {
                             if (do_gap) gsum[i] += gap4(v, kind == 0u ? gU4 : gL4, kind == 0u ? gL4 : gU4);
-                            relax4(v, kind == 0u ? kU4 : kL4, kind == 0u ? kL4 : kU4);
+                            relax4(v, kind == 0u ? kUc : kLc, kind == 0u ? kLc : kUc);
                         } else if (kind == 2u) {
-                            relax4(v, dp4, dp4);
+                            relax4(v, dpc, dpc);
                         }
                     }
                     split_store(v, r_hi, r_lo, pw * 32 + i * 4 + r4);
                 }
             }
             fence_proxy_async();                 // generic-proxy stores -> visible to the tensor core's async proxy
-            mbar_arrive(bar_full(stage));
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            mbar_arrive(bar_rfull(stage));
+            if (++stage == RSTAGES) { stage = 0; phase ^= 1; }
             // ---- end of a tile: the deviation-form constant (row sums over K; 8 threads per row)
-            if (kt == nk - 1) {
+            if (pkt == nk - 1) {
                 if (do_gap) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
@@ -512,11 +605,20 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
 #pragma unroll
                 for (int i = 0; i < 8; ++i) gsum[i] = 0.f;
             }
-            // ---- advance
-            tile = ntile; kt = nkt; have = nhave;
-            kinds_cur = kinds_nxt; t_cur = t_nxt;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) cur[i] = nxt[i];
+            ptile = ntile; pkt = nkt; t_cur = t_nxt;
+            return nhave;
+        };
+        if (phave) {
+            float4 b0[8], b1[8], b2[8];
+            uint32_t k0 = 0, k1 = 0, k2 = 0;
+            setup_load();
+            issue(b0, k0);
+            issue(b1, k1);
+            while (true) {
+                if (!step(b0, k0, b2, k2)) break;
+                if (!step(b1, k1, b0, k0)) break;
+                if (!step(b2, k2, b1, k1)) break;
+            }
         }
     }
 
