@@ -79,10 +79,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
     return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
+    // try_wait suspends the thread for a hardware-defined time slice, so this is not a hot spin; the clock is only
+    // consulted every 4096 slices to turn a protocol bug into a trap instead of a hung GPU
+    uint32_t spins = 0;
+    long long t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if ((unsigned long long)(clock64() - t0) > kSpinLimit) __trap();   // never hang the GPU
+        if ((++spins & 4095u) == 0u) {
+            const long long now = clock64();
+            if (t0 == 0) t0 = now;
+            else if ((unsigned long long)(now - t0) > kSpinLimit) __trap();
+        }
     }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
@@ -157,10 +163,10 @@ template <> __device__ __forceinline__ void tmem_ld<32>(uint32_t taddr, float* v
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// round to TF32 (10-bit mantissa), nearest with ties away from zero -- what cvt.rna.tf32.f32 computes for finite
+// inputs, in two integer instructions (the PTX conversion expands to a longer NaN/Inf-aware sequence)
 __device__ __forceinline__ float to_tf32(float x) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-    return __uint_as_float(r);
+    return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
 }
 __device__ __forceinline__ void named_bar_sync(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
 
@@ -286,6 +292,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         // ===================== MMA issuer =====================
         int ws = 0, rs = 0; uint32_t wphase = 0, rphase = 0;
         const uint32_t idesc = make_idesc(TBM, TBN);
+        const uint64_t dW0 = make_smem_desc(sW(0, 0)), dR0 = make_smem_desc(sR(0, 0));   // stage 0, hi part; the others are offsets
         int tcount = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
             const int acc = tcount % NACC;
@@ -298,8 +305,8 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 mbar_wait(bar_rfull(rs), rphase);
                 tc_fence_after();
                 if (lane == 0) {
-                    const uint64_t whi = make_smem_desc(sW(ws, 0)), wlo = make_smem_desc(sW(ws, 1));
-                    const uint64_t rhi = make_smem_desc(sR(rs, 0)), rlo = make_smem_desc(sR(rs, 1));
+                    const uint64_t whi = dW0 + (uint64_t)((2 * ws * W_TILE_BYTES) >> 4), wlo = whi + (W_TILE_BYTES >> 4);
+                    const uint64_t rhi = dR0 + (uint64_t)((2 * rs * R_TILE_BYTES) >> 4), rlo = rhi + (R_TILE_BYTES >> 4);
 #pragma unroll
                     for (int k = 0; k < TBK / 8; ++k) {
                         const uint64_t ko = (uint64_t)(k * 32 >> 4);     // 8 tf32 = 32 bytes along K inside the swizzle atom
@@ -491,10 +498,16 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         auto issue = [&](float4* buf, uint32_t& bkinds) {
             bkinds = lkinds;
             if (!lhave) return;
+            const uint32_t ko = (uint32_t)lkt * (TBK / 4);
+            if ((lkinds & (lkinds >> 1) & 0x5555u) == 0u) {          // no padding row among this thread's eight
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const bool ok = ((lkinds >> (2 * i)) & 3u) != 3u;
-                buf[i] = ok ? __ldg(A4 + aoff[i] + lkt * (TBK / 4)) : zero4;
+                for (int i = 0; i < 8; ++i) buf[i] = __ldg(A4 + aoff[i] + ko);
+            } else {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const bool ok = ((lkinds >> (2 * i)) & 3u) != 3u;
+                    buf[i] = ok ? __ldg(A4 + aoff[i] + ko) : zero4;
+                }
             }
             if (++lkt == nk) {
                 lkt = 0;
@@ -515,9 +528,11 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             return v;
         };
         auto split_store = [&](const float4& v, uint32_t r_hi, uint32_t r_lo, int row) {
+            // hi = tf32(v) (nearest); lo = v - hi exactly (|lo| <= 2^-11 |v|, at most 13 significant bits); the tensor
+            // core reads the upper 19 bits of lo, i.e. lo to within 2^-10 |lo| <= 2^-21 |v|
             float4 hi, lo;
             hi.x = to_tf32(v.x); hi.y = to_tf32(v.y); hi.z = to_tf32(v.z); hi.w = to_tf32(v.w);
-            lo.x = to_tf32(v.x - hi.x); lo.y = to_tf32(v.y - hi.y); lo.z = to_tf32(v.z - hi.z); lo.w = to_tf32(v.w - hi.w);
+            lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
             const uint32_t off = (uint32_t)row * 128u + (uint32_t)((c4 ^ (row & 7)) << 4);     // 128B swizzle
             asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_hi + off), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
             asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_lo + off), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w) : "memory");
