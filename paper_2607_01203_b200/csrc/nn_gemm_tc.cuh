@@ -43,9 +43,10 @@ constexpr int RSTAGES = 2;    // coefficient-row ring (register path, prefetched
 constexpr int W_TILE_BYTES = TBM * TBK * 4;                         // 16 KB (hi) + 16 KB (lo) per stage
 constexpr int R_TILE_BYTES = TBN * TBK * 4;                         // 32 KB (hi) + 32 KB (lo) per stage
 constexpr int RING_BYTES = WSTAGES * 2 * W_TILE_BYTES + RSTAGES * 2 * R_TILE_BYTES;   // 96 KB + 128 KB
-constexpr int PAR_BYTES = 5 * TBK * 4;                              // per-neuron parameters of one K slab: kU, kL, phi', gU, gL
-constexpr int BAR_BYTES = 128;
-constexpr int SMEM_BYTES = RING_BYTES + WSTAGES * PAR_BYTES + BAR_BYTES + 1024;   // + 1024-byte alignment slack (= 227 KB)
+constexpr int PSTAGES = 4;    // per-neuron parameter ring (tiny; four slabs ahead so that its latency never shows)
+constexpr int PAR_BYTES = 5 * TBK * 4;                              // parameters of one K slab: kU, kL, phi', gU, gL
+constexpr int BAR_BYTES = 192;
+constexpr int SMEM_BYTES = RING_BYTES + PSTAGES * PAR_BYTES + BAR_BYTES;   // 226.7 KB of the 227 KB a CTA can have
 constexpr int THREADS = 512;
 constexpr int PRODUCERS = 256;
 constexpr int TMEM_COLS = 512;
@@ -78,12 +79,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
+// SLEEP_NS > 0: back off between probes (the roles that wait for a whole tile or slab must not take issue slots
+// from the MMA warp that shares their scheduler)
+template <int SLEEP_NS = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     // try_wait suspends the thread for a hardware-defined time slice, so this is not a hot spin; the clock is only
     // consulted every 4096 slices to turn a protocol bug into a trap instead of a hung GPU
     uint32_t spins = 0;
     long long t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
+        if (SLEEP_NS > 0) __nanosleep(SLEEP_NS);
         if ((++spins & 4095u) == 0u) {
             const long long now = clock64();
             if (t0 == 0) t0 = now;
@@ -216,22 +221,25 @@ __device__ __forceinline__ TileGeo tile_geo(const GemmArgs& g, int tile, int col
 template <int MODE>
 __global__ void __launch_bounds__(THREADS, 1)
 chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo) {
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    uint8_t* sgen = smem_raw + (sbase - smem_u32(smem_raw));           // generic pointer to the aligned base
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t sbase = smem_u32(smem_raw);
+    if ((sbase & 1023u) != 0u) __trap();                               // the 128B-swizzled tiles need 1024-byte alignment
+    uint8_t* sgen = smem_raw;
     // weight ring: stage s = [Whi | Wlo]; row ring: stage s = [Rhi | Rlo]
     auto sW = [&](int s, int part) { return sbase + (2 * s + part) * W_TILE_BYTES; };
     auto sR = [&](int s, int part) { return sbase + WSTAGES * 2 * W_TILE_BYTES + (2 * s + part) * R_TILE_BYTES; };
-    // the slab's per-neuron parameters travel with the weight stage (forward only): [kU | kL | phi' | gU | gL] x 32 floats
+    // parameter ring (forward only): stage s = [kU | kL | phi' | gU | gL] x 32 floats of one K slab
     auto sP = [&](int s) { return sbase + RING_BYTES + s * PAR_BYTES; };
-    const uint32_t bar0 = sbase + RING_BYTES + WSTAGES * PAR_BYTES;
+    const uint32_t bar0 = sbase + RING_BYTES + PSTAGES * PAR_BYTES;
     auto bar_wfull = [&](int s) { return bar0 + 8 * s; };
     auto bar_wempty = [&](int s) { return bar0 + 8 * (WSTAGES + s); };
     auto bar_rfull = [&](int s) { return bar0 + 8 * (2 * WSTAGES + s); };
     auto bar_rempty = [&](int s) { return bar0 + 8 * (2 * WSTAGES + RSTAGES + s); };
     auto bar_tfull = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + a); };
     auto bar_tempty = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + 2 + a); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + RING_BYTES + WSTAGES * PAR_BYTES + 8 * (2 * WSTAGES + 2 * RSTAGES + 4));
+    auto bar_pfull = [&](int s) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + 4 + s); };
+    auto bar_pempty = [&](int s) { return bar0 + 8 * (2 * WSTAGES + 2 * RSTAGES + 4 + PSTAGES + s); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + RING_BYTES + PSTAGES * PAR_BYTES + 8 * (2 * WSTAGES + 2 * RSTAGES + 4 + 2 * PSTAGES));
     // forward: one accumulator pair (main [0,256), correction [256,512)); reverse sweep: the gradient tolerance
     // (1e-4) leaves room for the truncation of a single accumulator, so two of them alternate and the epilogue
     // of tile i overlaps the main loop of tile i+1
@@ -251,6 +259,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         for (int s = 0; s < WSTAGES; ++s) { mbar_init(bar_wfull(s), 1); mbar_init(bar_wempty(s), 1); }
         for (int s = 0; s < RSTAGES; ++s) { mbar_init(bar_rfull(s), PRODUCERS); mbar_init(bar_rempty(s), 1); }
         for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), 128); }
+        for (int s = 0; s < PSTAGES; ++s) { mbar_init(bar_pfull(s), 1); mbar_init(bar_pempty(s), PRODUCERS / 32); }
         fence_barrier_init();
     }
     if (warp == 2) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
@@ -270,22 +279,36 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             const TileGeo t = tile_geo(g, tile, col_blocks);
             const int n0 = t.n0;
             for (int kt = 0; kt < nk; ++kt) {
-                mbar_wait(bar_wempty(stage), phase ^ 1);
+                mbar_wait<100>(bar_wempty(stage), phase ^ 1);
                 if (lane == 0) {
-                    mbar_arrive_expect_tx(bar_wfull(stage), 2 * W_TILE_BYTES + (MODE == MODE_FWD ? PAR_BYTES : 0));
+                    mbar_arrive_expect_tx(bar_wfull(stage), 2 * W_TILE_BYTES);
                     tma_load_2d(sW(stage, 0), &tm_hi, kt * TBK, n0, bar_wfull(stage));
                     tma_load_2d(sW(stage, 1), &tm_lo, kt * TBK, n0, bar_wfull(stage));
-                    if (MODE == MODE_FWD) {
-                        const size_t o = t.po + (size_t)kt * TBK;
-                        bulk_load_1d(sP(stage) + 0 * TBK * 4, g.kU + o, TBK * 4, bar_wfull(stage));
-                        bulk_load_1d(sP(stage) + 1 * TBK * 4, g.kL + o, TBK * 4, bar_wfull(stage));
-                        bulk_load_1d(sP(stage) + 2 * TBK * 4, g.dphi + o, TBK * 4, bar_wfull(stage));
-                        bulk_load_1d(sP(stage) + 3 * TBK * 4, g.gU + o, TBK * 4, bar_wfull(stage));
-                        bulk_load_1d(sP(stage) + 4 * TBK * 4, g.gL + o, TBK * 4, bar_wfull(stage));
-                    }
                 }
                 __syncwarp();
                 if (++stage == WSTAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 3) {
+        // ===================== parameter loader (forward): the slab's slopes and gaps, four slabs ahead =====================
+        if (MODE == MODE_FWD) {
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+                const TileGeo t = tile_geo(g, tile, col_blocks);
+                for (int kt = 0; kt < nk; ++kt) {
+                    mbar_wait<100>(bar_pempty(stage), phase ^ 1);
+                    if (lane == 0) {
+                        const size_t o = t.po + (size_t)kt * TBK;
+                        mbar_arrive_expect_tx(bar_pfull(stage), PAR_BYTES);
+                        bulk_load_1d(sP(stage) + 0 * TBK * 4, g.kU + o, TBK * 4, bar_pfull(stage));
+                        bulk_load_1d(sP(stage) + 1 * TBK * 4, g.kL + o, TBK * 4, bar_pfull(stage));
+                        bulk_load_1d(sP(stage) + 2 * TBK * 4, g.dphi + o, TBK * 4, bar_pfull(stage));
+                        bulk_load_1d(sP(stage) + 3 * TBK * 4, g.gU + o, TBK * 4, bar_pfull(stage));
+                        bulk_load_1d(sP(stage) + 4 * TBK * 4, g.gL + o, TBK * 4, bar_pfull(stage));
+                    }
+                    __syncwarp();
+                    if (++stage == PSTAGES) { stage = 0; phase ^= 1; }
+                }
             }
         }
     } else if (warp == 1) {
@@ -304,9 +327,10 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 mbar_wait(bar_wfull(ws), wphase);
                 mbar_wait(bar_rfull(rs), rphase);
                 tc_fence_after();
+                // warp-uniform descriptor arithmetic stays outside the single-lane region (uniform datapath)
+                const uint64_t whi = dW0 + (uint64_t)((2 * ws * W_TILE_BYTES) >> 4), wlo = whi + (W_TILE_BYTES >> 4);
+                const uint64_t rhi = dR0 + (uint64_t)((2 * rs * R_TILE_BYTES) >> 4), rlo = rhi + (R_TILE_BYTES >> 4);
                 if (lane == 0) {
-                    const uint64_t whi = dW0 + (uint64_t)((2 * ws * W_TILE_BYTES) >> 4), wlo = whi + (W_TILE_BYTES >> 4);
-                    const uint64_t rhi = dR0 + (uint64_t)((2 * rs * R_TILE_BYTES) >> 4), rlo = rhi + (R_TILE_BYTES >> 4);
 #pragma unroll
                     for (int k = 0; k < TBK / 8; ++k) {
                         const uint64_t ko = (uint64_t)(k * 32 >> 4);     // 8 tf32 = 32 bytes along K inside the swizzle atom
@@ -342,7 +366,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             const int acc = tcount % NACC;
             const uint32_t acc_parity = (tcount / NACC) & 1;
             if (MODE == MODE_FWD) {
-                mbar_wait(bar_tfull(acc), acc_parity);
+                mbar_wait<200>(bar_tfull(acc), acc_parity);
                 tc_fence_after();
                 float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
                 // 16 rows per step, the TMEM loads of step i+1 in flight while step i is stored
@@ -402,7 +426,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 load_lam(lam0, 0); gb0 = load_gb(0);
                 load_lam(lam1, 16); gb1 = load_gb(16);
                 load_lam(lam2, 32); gb2 = load_gb(32);
-                mbar_wait(bar_tfull(acc), acc_parity);
+                mbar_wait<200>(bar_tfull(acc), acc_parity);
                 tc_fence_after();
                 const uint32_t t_acc = t_lane + acc * TBN;
                 float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
@@ -521,7 +545,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
         bool phave = ptile < num_tiles;
         TileGeo t_cur = tile_geo(g, phave ? ptile : 0, col_blocks);
         int stage = 0; uint32_t phase = 0;
-        int ws = 0; uint32_t wphase = 0;           // weight/parameter stage of the slab being transformed
+        int ps = 0; uint32_t pphase = 0;           // parameter stage of the slab being transformed
         auto lds4 = [&](uint32_t addr) {
             float4 v;
             asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
@@ -563,14 +587,17 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             const bool do_gap = (MODE == MODE_FWD) && (t_cur.n0 == 0) && (g.gap != nullptr);
             float4 kUc = zero4, kLc = zero4, dpc = zero4, gU4 = zero4, gL4 = zero4;
             if (MODE == MODE_FWD) {
-                // the slab's parameters arrived with its weight stage (TMA warp); the stage is not recycled before
-                // the MMAs of this slab retire, i.e. long after these reads
-                mbar_wait(bar_wfull(ws), wphase);
-                const uint32_t pp = sP(ws) + c4 * 16;
+                mbar_wait(bar_pfull(ps), pphase);
+                const uint32_t pp = sP(ps) + c4 * 16;
                 kUc = lds4(pp); kLc = lds4(pp + TBK * 4);
                 if (g.nkinds == 3) dpc = lds4(pp + 2 * TBK * 4);
                 if (do_gap) { gU4 = lds4(pp + 3 * TBK * 4); gL4 = lds4(pp + 4 * TBK * 4); }
-                if (++ws == WSTAGES) { ws = 0; wphase ^= 1; }
+                // the loads must have returned before the stage is handed back to the async proxy
+                asm volatile("" ::"f"(kUc.x), "f"(kLc.x), "f"(dpc.x), "f"(gU4.x), "f"(gL4.x));
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_pempty(ps));              // values are in registers: recycle the stage
+                if (++ps == PSTAGES) { ps = 0; pphase ^= 1; }
             }
             mbar_wait(bar_rempty(stage), phase ^ 1);
             const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
