@@ -405,76 +405,137 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     dp = __ldg(g.dphi + t.po + n);
                 }
                 float skU = 0.f, skL = 0.f, sgU = 0.f, sgL = 0.f, sdb = 0.f;
-                auto load_lam = [&](float* dst, int c) {
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const int jj = c + j;
-                        const int kind = (jj >= kb1) + (jj >= kb2);
-                        const int row = g.lam_shared ? (t.rbase + jj - kind * g.rows_kind) : (t.r0 + jj);
-                        dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
-                    }
-                };
-                auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
-                    const int jj = c + (lane & 15);
-                    const int kind = (jj >= kb1) + (jj >= kb2);
-                    return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
-                };
-                // forward coefficients three steps (48 rows) ahead of their use -- they come from HBM; the first three
-                // steps are requested before the accumulator is complete and overlap the main loop
-                float lam0[16], lam1[16], lam2[16], lam3[16];
-                float gb0, gb1, gb2, gb3 = 0.f;
-                load_lam(lam0, 0); gb0 = load_gb(0);
-                load_lam(lam1, 16); gb1 = load_gb(16);
-                load_lam(lam2, 32); gb2 = load_gb(32);
-                mbar_wait<200>(bar_tfull(acc), acc_parity);
-                tc_fence_after();
                 const uint32_t t_acc = t_lane + acc * TBN;
                 float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
-                float a[16];
-                tmem_ld<16>(t_acc, a);
-                // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+48, c+64) into L
-                auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                    if (c + 48 < TBN) { load_lam(L, c + 48); gbL = load_gb(c + 48); }
-                    tmem_ld_wait();
-                    float d[16];
+                const int kind0 = (0 >= kb1) + (0 >= kb2);
+                const bool uniform = (kind0 == (TBN - 1 >= kb1) + (TBN - 1 >= kb2)) && (TBN - 1 < kbe) && (kind0 < 2);
+                if (uniform) {
+                    // ---- all 256 rows on one chain (every hidden-layer target): no per-row selection
+                    const bool up = (kind0 == 0);
+                    const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
+                    const float* lp = g.Lam + (size_t)(g.lam_shared ? (t.rbase - kind0 * g.rows_kind) : t.r0) * g.ldl + (n_ok ? n : 0);
+                    const float* gbp = g.gapbar + t.r0 + (lane & 15);
+                    auto ld16 = [&](float* dst, int c) {
+                        const float* q = lp + (size_t)c * g.ldl;
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) d[j] = a[j];
-                    if (c + 16 < TBN) {
-                        tmem_ld<16>(t_acc + c + 16, a);
-                    } else {                                             // last read of this accumulator: release it
-                        tc_fence_before();
-                        mbar_arrive(bar_tempty(acc));
-                    }
+                        for (int j = 0; j < 16; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
+                    };
+                    float sP = 0.f, sQ = 0.f, hP = 0.f, hQ = 0.f;
+                    float lam0[16], lam1[16], lam2[16], lam3[16];
+                    float gb0, gb1, gb2, gb3 = 0.f;
+                    ld16(lam0, 0); gb0 = __ldg(gbp);
+                    ld16(lam1, 16); gb1 = __ldg(gbp + 16);
+                    ld16(lam2, 32); gb2 = __ldg(gbp + 32);
+                    mbar_wait<200>(bar_tfull(acc), acc_parity);
+                    tc_fence_after();
+                    float a[16];
+                    tmem_ld<16>(t_acc, a);
+                    float* cp = cbase;
+                    auto fstep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
+                        if (c + 48 < TBN) { ld16(L, c + 48); gbL = __ldg(gbp + c + 48); }
+                        tmem_ld_wait();
+                        float d[16];
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const int jj = c + j;
-                        const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
-                        const float gb = __shfl_sync(0xffffffffu, gbP, j);
-                        const float Db = d[j], lv = P[j];
-                        float out = 0.f;
-                        if (jj < kbe) {
-                            if (kind == 2) {
-                                sdb = fmaf(Db, lv, sdb);
-                                out = Db * dp;
-                            } else {
-                                const bool up = (kind == 0);
-                                const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
-                                const float dP = Db * Pp, dQ = Db * Q, gP = gb * Pp, gQ = gb * Q;
-                                skU += up ? dP : dQ; skL += up ? dQ : dP;
-                                sgU += up ? gP : gQ; sgL += up ? gQ : gP;
-                                const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
-                                out = lv > 0.f ? fmaf(Db, kp, gb * gp) : (lv < 0.f ? fmaf(Db, kn, gb * gn) : 0.f);
-                            }
+                        for (int j = 0; j < 16; ++j) d[j] = a[j];
+                        if (c + 16 < TBN) {
+                            tmem_ld<16>(t_acc + c + 16, a);
+                        } else {                                         // last read of this accumulator: release it
+                            tc_fence_before();
+                            mbar_arrive(bar_tempty(acc));
                         }
-                        if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
-                    }
-                };
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const float gb = __shfl_sync(0xffffffffu, gbP, j);
+                            const float Db = d[j], lv = P[j];
+                            const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                            sP = fmaf(Db, Pp, sP); sQ = fmaf(Db, Q, sQ);
+                            hP = fmaf(gb, Pp, hP); hQ = fmaf(gb, Q, hQ);
+                            const bool pos = lv > 0.f;
+                            float out = fmaf(Db, pos ? kp : kn, gb * (pos ? gp : gn));
+                            out = (lv == 0.f) ? 0.f : out;
+                            if (g.write_c && n_ok) *cp = out;
+                            cp += g.ldc;
+                        }
+                    };
 #pragma unroll 1
-                for (int c = 0; c < TBN; c += 64) {
-                    estep(c, lam0, gb0, lam3, gb3);
-                    estep(c + 16, lam1, gb1, lam0, gb0);
-                    estep(c + 32, lam2, gb2, lam1, gb1);
-                    estep(c + 48, lam3, gb3, lam2, gb2);
+                    for (int c = 0; c < TBN; c += 64) {
+                        fstep(c, lam0, gb0, lam3, gb3);
+                        fstep(c + 16, lam1, gb1, lam0, gb0);
+                        fstep(c + 32, lam2, gb2, lam1, gb1);
+                        fstep(c + 48, lam3, gb3, lam2, gb2);
+                    }
+                    skU = up ? sP : sQ; skL = up ? sQ : sP;
+                    sgU = up ? hP : hQ; sgL = up ? hQ : hP;
+                } else {
+                    auto load_lam = [&](float* dst, int c) {
+    #pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int jj = c + j;
+                            const int kind = (jj >= kb1) + (jj >= kb2);
+                            const int row = g.lam_shared ? (t.rbase + jj - kind * g.rows_kind) : (t.r0 + jj);
+                            dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
+                        }
+                    };
+                    auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
+                        const int jj = c + (lane & 15);
+                        const int kind = (jj >= kb1) + (jj >= kb2);
+                        return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
+                    };
+                    // forward coefficients three steps (48 rows) ahead of their use -- they come from HBM; the first three
+                    // steps are requested before the accumulator is complete and overlap the main loop
+                    float lam0[16], lam1[16], lam2[16], lam3[16];
+                    float gb0, gb1, gb2, gb3 = 0.f;
+                    load_lam(lam0, 0); gb0 = load_gb(0);
+                    load_lam(lam1, 16); gb1 = load_gb(16);
+                    load_lam(lam2, 32); gb2 = load_gb(32);
+                    mbar_wait<200>(bar_tfull(acc), acc_parity);
+                    tc_fence_after();
+                    float a[16];
+                    tmem_ld<16>(t_acc, a);
+                    // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+48, c+64) into L
+                    auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
+                        if (c + 48 < TBN) { load_lam(L, c + 48); gbL = load_gb(c + 48); }
+                        tmem_ld_wait();
+                        float d[16];
+    #pragma unroll
+                        for (int j = 0; j < 16; ++j) d[j] = a[j];
+                        if (c + 16 < TBN) {
+                            tmem_ld<16>(t_acc + c + 16, a);
+                        } else {                                             // last read of this accumulator: release it
+                            tc_fence_before();
+                            mbar_arrive(bar_tempty(acc));
+                        }
+    #pragma unroll
+                        for (int j = 0; j < 16; ++j) {
+                            const int jj = c + j;
+                            const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
+                            const float gb = __shfl_sync(0xffffffffu, gbP, j);
+                            const float Db = d[j], lv = P[j];
+                            float out = 0.f;
+                            if (jj < kbe) {
+                                if (kind == 2) {
+                                    sdb = fmaf(Db, lv, sdb);
+                                    out = Db * dp;
+                                } else {
+                                    const bool up = (kind == 0);
+                                    const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                                    const float dP = Db * Pp, dQ = Db * Q, gP = gb * Pp, gQ = gb * Q;
+                                    skU += up ? dP : dQ; skL += up ? dQ : dP;
+                                    sgU += up ? gP : gQ; sgL += up ? gQ : gP;
+                                    const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
+                                    out = lv > 0.f ? fmaf(Db, kp, gb * gp) : (lv < 0.f ? fmaf(Db, kn, gb * gn) : 0.f);
+                                }
+                            }
+                            if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
+                        }
+                    };
+    #pragma unroll 1
+                    for (int c = 0; c < TBN; c += 64) {
+                        estep(c, lam0, gb0, lam3, gb3);
+                        estep(c + 16, lam1, gb1, lam0, gb0);
+                        estep(c + 32, lam2, gb2, lam1, gb1);
+                        estep(c + 48, lam3, gb3, lam2, gb2);
+                    }
                 }
                 if (n_ok) {
                     atomicAdd(g.kUb + t.po + n, skU);
