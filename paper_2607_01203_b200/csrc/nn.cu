@@ -228,19 +228,21 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
 __global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
                             const float* __restrict__ sigma, const float* __restrict__ ybar_up, const float* __restrict__ ybar_lo,
                             int ldy, float* __restrict__ Lbar0, float* __restrict__ gapbar, float* __restrict__ rad_bar) {
-    const int t = blockIdx.x;
+    // grid (tiles, ceil(rows_kind / 32)): a block takes 32 bound indices k of one tile; thread j owns input column j
+    const int t = blockIdx.x, k0 = blockIdx.y * 32, k1 = min(k0 + 32, rows_kind);
     const float* base = Lam0 + (size_t)t * rows_pad * wp0;
     float* obase = Lbar0 + (size_t)t * rows_pad * wp0;
-    for (int r = threadIdx.x; r < rows_pad; r += blockDim.x) {
-        float v = 0.f;
-        if (r < rows_kind) v = ybar_up[(size_t)t * ldy + r];
-        else if (r < 2 * rows_kind) v = ybar_lo[(size_t)t * ldy + r - rows_kind];
-        gapbar[(size_t)t * rows_pad + r] = v;
+    for (int k = k0 + threadIdx.x; k < k1; k += blockDim.x) {
+        gapbar[(size_t)t * rows_pad + k] = ybar_up[(size_t)t * ldy + k];
+        gapbar[(size_t)t * rows_pad + rows_kind + k] = ybar_lo[(size_t)t * ldy + k];
     }
+    if (blockIdx.y == 0)
+        for (int r = 2 * rows_kind + threadIdx.x; r < rows_pad; r += blockDim.x) gapbar[(size_t)t * rows_pad + r] = 0.f;
     for (int j = threadIdx.x; j < wp0; j += blockDim.x) {
         const float s = sigma[(size_t)t * wp0 + j];
         float sb = 0.f;
-        for (int k = 0; k < rows_kind; ++k) {
+#pragma unroll 4
+        for (int k = k0; k < k1; ++k) {
             const float yu = ybar_up[(size_t)t * ldy + k], yl = ybar_lo[(size_t)t * ldy + k];
             float a = base[(size_t)k * wp0 + j], b = base[(size_t)(rows_kind + k) * wp0 + j];
             if (is_out) { float jv = base[(size_t)(2 * rows_kind + k) * wp0 + j]; a -= jv; b -= jv; }
@@ -251,7 +253,7 @@ __global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, co
             if (is_out) obase[(size_t)(2 * rows_kind + k) * wp0 + j] = -(lu + ll);
             sb += yu * fabsf(a) - yl * fabsf(b);
         }
-        rad_bar[(size_t)t * wp0 + j] += sb;
+        atomicAdd(&rad_bar[(size_t)t * wp0 + j], sb);
     }
 }
 
@@ -691,7 +693,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
             }
             const float* yu = is_out ? S->ghi_p : S->ubar[s];
             const float* yl = is_out ? S->glo_p : S->lbar[s];
-            seed_kernel<<<C, 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
+            seed_kernel<<<dim3(C, (rk + 31) / 32), 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
                                            S->Lbar[0], S->gapbar, S->rad_bar);
             ++*launches;
             int cur = 0;
