@@ -406,6 +406,23 @@ def output_sign_ties(Ws, bs, act, a0, sig, rel=1e-6):
     return ties
 
 
+def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
+    """Hidden neurons (layer, k) whose pre-activation bound sits on a case switch of the relaxation
+    table (readings R8/R9/R21): an endpoint l or u within rel * (|l| + |u|) of 0, or (ReLU)
+    |u + l| that close to the u > -l switch.  The relaxation -- and with it the bound -- is
+    discontinuous there, so an FP32 evaluation may legitimately take the other case.  Test
+    plumbing only: calls crown_forward, changes no arithmetic."""
+    fw = crown_forward(Ws, bs, act, a0, sig)
+    ties = []
+    for layer, (l, u) in enumerate(zip(fw["ls"], fw["us"]), start=1):
+        scale = rel * (np.abs(l) + np.abs(u))
+        near = (np.abs(l) < scale) | (np.abs(u) < scale)
+        if act == ACT_RELU:
+            near |= (l < 0) & (u > 0) & (np.abs(u + l) < scale)
+        ties += [(layer, int(k)) for k in np.nonzero(near)[0]]
+    return ties
+
+
 def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None, flips=()):
     """Returns (grad_nom, grad_rad) for one tile.  `flips`: entries (chain, i, j) from
     output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink)."""

@@ -654,7 +654,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 if (g.nkinds == 3) dpc = lds4(pp + 2 * TBK * 4);
                 if (do_gap) { gU4 = lds4(pp + 3 * TBK * 4); gL4 = lds4(pp + 4 * TBK * 4); }
                 // the loads must have returned before the stage is handed back to the async proxy
-                asm volatile("" ::"f"(kUc.x), "f"(kLc.x), "f"(dpc.x), "f"(gU4.x), "f"(gL4.x));
+                // generic-proxy reads, then the async proxy (bulk TMA) overwrites the stage: the cross-proxy fence is
+                // required (without it ~10 % of config-5 tiles came out wrong, non-deterministically)
+                asm volatile("" ::"f"(kUc.x), "f"(kLc.x), "f"(dpc.x), "f"(gU4.x), "f"(gL4.x) : "memory");
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_pempty(ps));              // values are in registers: recycle the stage
