@@ -371,11 +371,11 @@ size_t bytes_per_tile(const NnState* S, bool vjp) {
 leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
     int want = S->chunk_req > 0 ? S->chunk_req : 0;
     if (want == 0) {
-        // default: as many tiles as fit in ~6 GB, at most 1024 (enough row blocks to fill 148 SMs many times)
+        // default: as many tiles as fit in ~24 GB of the 180 GB HBM, at most 2048: fewer, longer launches (tail and launch gaps amortised)
         size_t per = bytes_per_tile(S, true);
-        size_t c = (size_t)6e9 / (per ? per : 1);
+        size_t c = (size_t)24e9 / (per ? per : 1);
         if (c < 1) c = 1;
-        if (c > 1024) c = 1024;
+        if (c > 2048) c = 2048;
         want = (int)c;
     }
     if (want > tiles && tiles > 0) want = tiles;

@@ -279,7 +279,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             const TileGeo t = tile_geo(g, tile, col_blocks);
             const int n0 = t.n0;
             for (int kt = 0; kt < nk; ++kt) {
-                mbar_wait<100>(bar_wempty(stage), phase ^ 1);
+                mbar_wait<32>(bar_wempty(stage), phase ^ 1);
                 if (lane == 0) {
                     mbar_arrive_expect_tx(bar_wfull(stage), 2 * W_TILE_BYTES);
                     tma_load_2d(sW(stage, 0), &tm_hi, kt * TBK, n0, bar_wfull(stage));
@@ -647,6 +647,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             if (nhave && nkt == 0) t_nxt = tile_geo(g, ntile, col_blocks);
             const bool do_gap = (MODE == MODE_FWD) && (t_cur.n0 == 0) && (g.gap != nullptr);
             float4 kUc = zero4, kLc = zero4, dpc = zero4, gU4 = zero4, gL4 = zero4;
+            int p_used = 0;
             if (MODE == MODE_FWD) {
                 mbar_wait(bar_pfull(ps), pphase);
                 const uint32_t pp = sP(ps) + c4 * 16;
@@ -654,12 +655,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 if (g.nkinds == 3) dpc = lds4(pp + 2 * TBK * 4);
                 if (do_gap) { gU4 = lds4(pp + 3 * TBK * 4); gL4 = lds4(pp + 4 * TBK * 4); }
                 // the loads must have returned before the stage is handed back to the async proxy
-                // generic-proxy reads, then the async proxy (bulk TMA) overwrites the stage: the cross-proxy fence is
-                // required (without it ~10 % of config-5 tiles came out wrong, non-deterministically)
-                asm volatile("" ::"f"(kUc.x), "f"(kLc.x), "f"(dpc.x), "f"(gU4.x), "f"(gL4.x) : "memory");
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_pempty(ps));              // values are in registers: recycle the stage
+                p_used = ps;                                             // released below, behind the step's proxy fence
                 if (++ps == PSTAGES) { ps = 0; pphase ^= 1; }
             }
             mbar_wait(bar_rempty(stage), phase ^ 1);
@@ -691,9 +687,16 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     split_store(v, r_hi, r_lo, pw * 32 + i * 4 + r4);
                 }
             }
-            fence_proxy_async();                 // generic-proxy stores -> visible to the tensor core's async proxy
+            // one cross-proxy fence for both hand-overs: the row stores become visible to the tensor core, and the
+            // parameter reads above are ordered before the bulk TMA that recycles their stage (without a fence on that
+            // path ~10 % of config-5 tiles came out wrong, non-deterministically)
+            fence_proxy_async();
             mbar_arrive(bar_rfull(stage));
             if (++stage == RSTAGES) { stage = 0; phase ^= 1; }
+            if (MODE == MODE_FWD) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_pempty(p_used));
+            }
             // ---- end of a tile: the deviation-form constant (row sums over K; 8 threads per row)
             if (pkt == nk - 1) {
                 if (do_gap) {
