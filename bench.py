@@ -172,7 +172,7 @@ def run_ours(args):
     h_gc, h_gR = torch.from_numpy(w.g_lo).pin_memory(), torch.from_numpy(w.g_hi).pin_memory()
 
     def step_device():
-        r_lo, r_hi = ctx.leb_nn_fwd(nom, rad)
+        r_lo, r_hi = ctx.leb_nn_fwd(nom, rad, flags=0)          # certified mode: rounding margin added outward (N6)
         ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
         g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
         return ctx.leb_vjp(1, nom, rad, g_lo, g_hi)
@@ -184,7 +184,7 @@ def run_ours(args):
     hb.update({k: pin(w.B, w.T, w.N) for k in ("gn", "gr")})
 
     def step_host(count=False):
-        r_lo, r_hi = ctx.leb_nn_fwd(h_nom, h_rad, r_lo=hb["r_lo"], r_hi=hb["r_hi"], flags=leb.FLAG_NO_MARGIN | HOST)
+        r_lo, r_hi = ctx.leb_nn_fwd(h_nom, h_rad, r_lo=hb["r_lo"], r_hi=hb["r_hi"], flags=HOST)
         c, R = ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6, flags=HOST, c_bar=hb["c"], R_diag=hb["R"])
         g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(h_gc, h_gR, flags=HOST, g_lo=hb["g_lo"], g_hi=hb["g_hi"])
         gn, gr = ctx.leb_vjp(1, h_nom, h_rad, g_lo, g_hi, grad_nom=hb["gn"], grad_rad=hb["gr"], flags=leb.FLAG_NO_MARGIN | HOST)
@@ -235,6 +235,15 @@ def run_ours(args):
     dt_max = sharding.max_over_ranks(dt, dev)
     e2e_value = world * entries_per_rank / dt_max
 
+    certified = None
+    if rank == 0:
+        # outside the timed region: what the certified margin costs in tightness, against the value-mode (parity) result
+        c_lo, c_hi = ctx.leb_nn_fwd(nom, rad, flags=0)
+        v_lo, v_hi = ctx.leb_nn_fwd(nom, rad, flags=leb.FLAG_NO_MARGIN)
+        width = (v_hi - v_lo).clamp_min(1e-12)
+        ex = torch.maximum(c_hi - v_hi, v_lo - c_lo) / width
+        certified = {"excess_over_value_mode_median": float(ex.median()), "excess_over_value_mode_max": float(ex.max()),
+                     "unit": "fraction of the enclosure width", "contains_value_mode": bool((ex >= -1e-5).all())}
     if rank == 0:
         peaks = _peaks()
         dom = max((0, 1), key=lambda kc: kstats[kc][0])
@@ -271,11 +280,12 @@ def run_ours(args):
                 "config": {"workload": WORKLOAD, "global_batch": 64 * world, "horizon": 100, "tiles": w.B * w.T * world,
                            "parallelism": f"dp{world} (independent tiles, no collective)",
                            "l2": "working set (>= 6 GB of coefficient blocks per chunk) exceeds the 126 MB L2; no flush needed",
-                           "mode": "value mode (LEB_FLAG_NO_MARGIN), 3xTF32 tcgen05 contractions"},
+                           "mode": "forward in certified mode (rounding margin added outward, DESIGN.md section 6), VJP of the value-mode "
+                                   "bound; 3xTF32 tcgen05 contractions"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e_bytes["h2d"], "d2h_bytes_per_step": e2e_bytes["d2h"],
                         "ms_per_step": 1e3 * dt_max / max(args.steps, 1)},
-                "gpu_launches": launches_total, "roofline": roofline, "cpu_baseline": cpu}
+                "gpu_launches": launches_total, "roofline": roofline, "cpu_baseline": cpu, "certified": certified}
         print(json.dumps(line))
     ctx.close()
     if world > 1:

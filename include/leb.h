@@ -89,7 +89,10 @@ typedef struct {
 } leb_mlp;
 
 enum {
-    LEB_FLAG_NO_MARGIN = 1u, /* NN: do not add the FP rounding margin (value mode; parity tests) */
+    LEB_FLAG_NO_MARGIN = 1u, /* NN: value mode -- plain FP32 / 3xTF32 result with no rounding margin (the mode the
+                                parity tests compare with the oracle).  Without it leb_nn_fwd runs in CERTIFIED mode:
+                                every rounding error of the path is bounded and added outward,
+                                so r_lo <= r(a) <= r_hi holds in exact arithmetic for the FP32 weights as given */
     LEB_FLAG_FFMA_ONLY = 2u, /* NN: FP32 FFMA contractions instead of 3xTF32 tcgen05 */
     LEB_FLAG_HOST_IO = 4u    /* data pointers of this call are host pointers */
 };
@@ -121,14 +124,18 @@ leb_status leb_analytic_fwd(leb_ctx* ctx, int B, int T, const float* nom, const 
 /* CROWN + Thm 3 bound, eq. (18)-(21) L196-220, for every tile.
  *   J      : NULL => the network's own Jacobian at a~ (eq. (7)); otherwise [B, T, n, N]
  *            dense, and the bound is with respect to that matrix (Thm 3 holds for any J).
- *   margin : NULL or [B, T, ld_out]: the rounding margin that was (or, with
- *            LEB_FLAG_NO_MARGIN, would have been) added outward to each of r_lo, r_hi. */
+ *   margin : NULL or [B, T, ld_out].  Certified mode: the outward pad contained in r_lo / r_hi of the entry (the
+ *            larger of the two sides): rounding pads of the output rows' chain steps, the nominal drift eta and the
+ *            rounding of the final sums.  (The pads of the hidden-layer bounds act through looser relaxations and
+ *            are not part of this number; certified minus value-mode bound is the total cost.)  Value mode: 0.
+ * Certified mode returns LEB_ERR_UNSUPPORTED for layers wider than 2048 (padded). */
 leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad,
                       const float* mu, const float* J, int ld_in, float* r_lo, float* r_hi,
                       float* margin, int ld_out, unsigned flags, void* stream);
 
 /* VJP of the bounds: grad = d/d(a~, sigma) sum_i g_hi[i] r_hi[i] + g_lo[i] r_lo[i], per tile
- * (block-diagonal over tiles).  Recomputes the forward pass internally (stateless).
+ * (block-diagonal over tiles).  Recomputes the forward pass internally (stateless).  kind 1: always the VJP of
+ * the value-mode bound -- the certified margin is a rounding-level pad and is treated as a constant.
  *   kind: 0 analytic (model from leb_set_analytic), 1 NN (model from leb_set_mlp)
  *   g_lo, g_hi       : [B, T, ld_out] cotangents
  *   grad_nom,grad_rad: [B, T, ld_in] outputs (columns >= N are left untouched).
@@ -162,6 +169,13 @@ leb_status leb_domain_flag(leb_ctx* ctx, int* flag, void* stream);
  * in the workspace by the LAST leb_nn_fwd call whose B*T fitted one chunk.
  * l, u: device [B*T, dims[layer]] contiguous. */
 leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, void* stream);
+
+/* Inspection (tests): the back-substituted coefficient rows Lambda_0 (coefficients on the input a = [x; u],
+ * eq. (18)) of target layer `target` (2 .. L; L = the output target) left in the workspace by the
+ * LAST leb_nn_fwd call whose B*T fitted one chunk.  out: device [B*T, 2, rows, dims[0]] contiguous, rows =
+ * dims[target]; index 0 = upper chain, 1 = lower chain.  Used to measure the contraction's rounding error
+ * against the model behind the certified margin. */
+leb_status leb_nn_chain_coeffs(leb_ctx* ctx, int target, float* out, void* stream);
 
 /* Number of kernel launches the library has enqueued on this context so far. */
 long long leb_launch_count(const leb_ctx* ctx);

@@ -301,6 +301,13 @@ leb_status leb_nn_hidden_bounds(leb_ctx* c, int layer, float* l, float* u, void*
     return leb_nn_get_hidden(c->nn, layer, l, u, (cudaStream_t)stream, &c->launches);
 }
 
+leb_status leb_nn_chain_coeffs(leb_ctx* c, int target, float* out, void* stream) {
+    if (!c || !out) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    DeviceGuard guard(c->device);
+    return leb_nn_get_coeffs(c->nn, target, out, (cudaStream_t)stream, &c->launches);
+}
+
 long long leb_launch_count(const leb_ctx* c) { return c ? c->launches : 0; }
 
 leb_status leb_profile(leb_ctx* c, int enable) {

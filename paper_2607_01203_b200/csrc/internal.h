@@ -77,3 +77,4 @@ leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, c
                       int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
                       cudaStream_t st, long long* launches, LebProf* prof);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);
+leb_status leb_nn_get_coeffs(NnState*, int target, float* out, cudaStream_t st, long long* launches);

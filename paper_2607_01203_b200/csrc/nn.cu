@@ -56,6 +56,11 @@ struct NnState {
     int rows_kind[kMaxLayers + 1] = {0}, rows_pad[kMaxLayers + 1] = {0};
     float* Lam[kMaxLayers + 1][kMaxLayers] = {{nullptr}};
     float* gap[kMaxLayers + 1] = {nullptr};
+    // certified mode (N6, DESIGN.md §6 "Certified margin"): per layer the centre residual e, the nominal drift t, the
+    // interval radius v of z_l - zhat_l, the activation deviation adev and the gap pads mU, mL ([chunk x wp[l]]);
+    // the chain margin of the output rows (report only, [chunk x rows_pad[L]]); eta for the output ([chunk x wpL])
+    float *ce[kMaxLayers] = {nullptr}, *ct[kMaxLayers] = {nullptr}, *cv[kMaxLayers] = {nullptr}, *adev[kMaxLayers] = {nullptr};
+    float *mU[kMaxLayers] = {nullptr}, *mL[kMaxLayers] = {nullptr}, *marg = nullptr, *eta = nullptr;
     // VJP workspace
     float *kUb[kMaxLayers] = {nullptr}, *kLb[kMaxLayers] = {nullptr}, *gUb[kMaxLayers] = {nullptr}, *gLb[kMaxLayers] = {nullptr},
           *dpb[kMaxLayers] = {nullptr}, *zbar[kMaxLayers] = {nullptr}, *lbar[kMaxLayers] = {nullptr}, *ubar[kMaxLayers] = {nullptr};
@@ -147,10 +152,170 @@ __global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const 
     }
 }
 
+// certified mode (N6): the same relaxation, made sound for the numbers as STORED.  With c = zhat (the FP32 centre),
+// a = ahat (the FP32 centre of the activation) and the FP32 slopes kU, kL, the stored gaps satisfy, for every z in [l, u],
+//     kL (z - c) + gL  <=  phi(z) - a  <=  kU (z - c) + gU            in exact arithmetic:
+// the slope's rounding moves the line by at most |k32 - k64| max|z - c|, and the FP64 construction of the line by at most
+// d64 (libm tanh within 2 ulp); both are added outward, gU is rounded up and kept >= 0, gL rounded down and kept <= 0.
+// Layer 1 (layer1 != 0): l, u = c -+ (|W_1| sigma + e_1) = c -+ (v + e), outward.  adev >= |phi(z) - a| over [l, u].
+//
+// The rounding of the chain step through this layer is carried by the gaps as well.  A coefficient row Lam on a_l turns
+// into D = Lam^+ kU + Lam^- kL (lower chain: kL, kU) and then into D W_l, computed in FP32 / 3xTF32; what the step can lose
+// is at most sum_j |D_j| x_j with x_j = gamma_j v_j + e_j (v = |W_l| adev_{l-1}: radius of z_l - zhat_l; e: centre residual;
+// gamma_j: see gamma_of()), and |D_j| x_j = Lam_j^+ |kU_j| x_j - Lam_j^- |kL_j| x_j has exactly the form of the gap sum.  So
+//     gU += |kU| x,   gL -= |kL| x
+// adds the step's margin outward to both chains, on either contraction path, with no work in the contraction kernels.
+// mU, mL keep the two pads by themselves (for the margin report).
+__device__ __forceinline__ float gamma_of(int tensor, int K, int j) {
+    // rounding error that the product D_j W_l[j,k] can cause in the contraction over j (K terms, taken in index order by
+    // both kernels): the term is part of every partial sum from its own step on.
+    //   tensor path: (4.5 (K/8 - floor(j/8)) + 17) 2^-23 -- per accumulating MMA (8 terms) at most 4.5 ulp of the running
+    //                magnitude (measured adder: addends truncated at 2^-25 of the largest, result truncated to FP32; taken
+    //                twice over in case the 8 terms are added in two halves), + 2^-19 for the hi/lo split, the dropped
+    //                lo*lo term and the correction accumulator, + 2^-23 for the rounding of D_j itself and the final FADD
+    //   FFMA path:   (K - j + 4) 2^-24 + 2^-23         -- one rounding to nearest per fused multiply-add
+    // (DESIGN.md section 6 "Certified margin"; tests/test_gpu_nn_certified.py probes both models on adversarial operands)
+    const float g = tensor ? (4.5f * (float)(K / 8 - j / 8) + 17.f) * 1.1920930e-07f : (float)(K - j + 4) * 5.9604652e-08f + 1.1920930e-07f;
+    return g * 1.000001f;
+}
+__global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, int layer1, int tensor, const float* __restrict__ zhat,
+                                      const float* __restrict__ ahat, const float* __restrict__ v, const float* __restrict__ e,
+                                      float* __restrict__ lb, float* __restrict__ ub, float* __restrict__ kU, float* __restrict__ kL,
+                                      float* __restrict__ gU, float* __restrict__ gL, float* __restrict__ adev,
+                                      float* __restrict__ mU, float* __restrict__ mL) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) {
+            lb[q] = 0.f; ub[q] = 0.f; kU[q] = 0.f; kL[q] = 0.f; gU[q] = 0.f; gL[q] = 0.f; adev[q] = 0.f; mU[q] = 0.f; mL[q] = 0.f;
+            continue;
+        }
+        float z = zhat[q], l, u;
+        if (layer1) {
+            float r = __fadd_ru(v[q], e[q]);
+            l = __fadd_rd(z, -r); u = __fadd_ru(z, r);
+            lb[q] = l; ub[q] = u;
+        } else { l = lb[q]; u = ub[q]; }
+        const double zd = (double)z, ld = (double)l, ud = (double)u, a = (double)ahat[q];
+        Relax r = relax_any(act, ld, ud);
+        const float kU32 = (float)r.kU, kL32 = (float)r.kL;
+        const double zdev = fmax(ud - zd, zd - ld);
+        const double d64 = 5.7e-14 * (1.0 + fabs(zd) + fabs(ld) + fabs(ud));          // 2^-44 (1 + |c| + |l| + |u|)
+        const double gu = (r.kU * zd + r.bU - a) + fabs((double)kU32 - r.kU) * zdev + d64;
+        const double gl = (r.kL * zd + r.bL - a) - fabs((double)kL32 - r.kL) * zdev - d64;
+        const float x = __fmaf_ru(gamma_of(tensor, wp, c), v[q], e[q]);
+        const float pu = __fmul_ru(fabsf(kU32), x), pl = __fmul_ru(fabsf(kL32), x);
+        kU[q] = kU32;
+        kL[q] = kL32;
+        gU[q] = __fadd_ru(fmaxf(__double2float_ru(gu), 0.f), pu);
+        gL[q] = __fadd_rd(fminf(__double2float_rd(gl), 0.f), -pl);
+        mU[q] = pu;
+        mL[q] = pl;
+        adev[q] = __double2float_ru(fmax(act_f(act, ud) - a, a - act_f(act, ld)) + 1e-15);
+    }
+}
+
+// certified mode (N6): one layer's rounding bookkeeping from the stored centres.  For tile m and neuron j of layer l,
+//   e[m,j] >= | W_l ahat_{l-1} + b_l - zhat_l |      FP64 dot product (a product of two floats is exact in FP64) + its own
+//                                                     accumulation bound (K + 2) 2^-52 (|W_l| |ahat_{l-1}| + |b_l|)
+//   t[m,j] >= | a_l(nominal input) - ahat_l |         = (|W_l| t_{l-1} + e) + |phi(zhat_l) - ahat_l|   (phi is 1-Lipschitz)
+//   v[m,j] >= |W_l| adev_{l-1}                        radius of z_l - zhat_l - (centre residual) over the box
+// the two |W_l| products are FP32 with every operation rounded up.  out_only (layer L): t = eta = |W_L| t_{L-1}.
+// Wt is [K x ldw] (K-major: Wt[k][j]).  Block: 16 tiles x 64 neurons, K slabs of 32.
+constexpr int CM = 16, CJ = 64, CK = 32;
+__global__ void __launch_bounds__(256) cert_layer_kernel(int C, int J, int K, const float* __restrict__ Wt, int ldw,
+                                                         const float* __restrict__ bias, const float* __restrict__ X,
+                                                         const float* __restrict__ T, const float* __restrict__ A, int ldx,
+                                                         const float* __restrict__ zhat, const float* __restrict__ ahat, int act,
+                                                         int out_only, float* __restrict__ e, float* __restrict__ t,
+                                                         float* __restrict__ v, int ldo) {
+    __shared__ __align__(16) float Ws[CK][CJ];
+    __shared__ float Xs[CM][CK], Ts[CM][CK], As[CM][CK];
+    const int tid = threadIdx.x, tj = tid & 15, tm = tid >> 4;
+    const int m0 = blockIdx.y * CM, j0 = blockIdx.x * CJ;
+    double s[4] = {0.0, 0.0, 0.0, 0.0}, sa[4] = {0.0, 0.0, 0.0, 0.0};
+    float zt[4] = {0.f, 0.f, 0.f, 0.f}, vv[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int k0 = 0; k0 < K; k0 += CK) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int idx = tid + i * 256, kk = idx >> 6, jj = idx & 63;
+            Ws[kk][jj] = (k0 + kk < K && j0 + jj < J) ? Wt[(size_t)(k0 + kk) * ldw + j0 + jj] : 0.f;
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int idx = tid + i * 256, mm = idx >> 5, kk = idx & 31;
+            const bool ok = (m0 + mm < C) && (k0 + kk < K);
+            const size_t o = (size_t)(m0 + mm) * ldx + k0 + kk;
+            Xs[mm][kk] = (ok && X) ? X[o] : 0.f;
+            Ts[mm][kk] = (ok && T) ? T[o] : 0.f;
+            As[mm][kk] = (ok && A) ? A[o] : 0.f;
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int kk = 0; kk < CK; ++kk) {
+            const float4 w4 = *reinterpret_cast<const float4*>(&Ws[kk][tj * 4]);
+            const float w[4] = {w4.x, w4.y, w4.z, w4.w};
+            const float x = Xs[tm][kk], tt = Ts[tm][kk], a = As[tm][kk];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float wa = fabsf(w[c]);
+                if (!out_only) {
+                    s[c] = fma((double)w[c], (double)x, s[c]);
+                    sa[c] = fma((double)wa, fabs((double)x), sa[c]);
+                    vv[c] = __fmaf_ru(wa, a, vv[c]);
+                }
+                zt[c] = __fmaf_ru(wa, tt, zt[c]);
+            }
+        }
+        __syncthreads();
+    }
+    const int m = m0 + tm;
+    if (m >= C) return;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const int j = j0 + tj * 4 + c;
+        if (j >= J) continue;
+        const size_t o = (size_t)m * ldo + j;
+        if (out_only) { t[o] = zt[c]; continue; }
+        const double b = (double)bias[j], c0 = (double)zhat[o];
+        const double fuzz = (sa[c] + fabs(b)) * (double)(K + 2) * 2.220446049250313e-16;
+        const float ee = __double2float_ru(fabs(s[c] + b - c0) + fuzz);
+        const double ep = fabs(act_f(act, c0) - (double)ahat[o]) + 1e-15;
+        e[o] = ee;
+        t[o] = __fadd_ru(__fadd_ru(zt[c], ee), __double2float_ru(ep));
+        v[o] = vv[c];
+    }
+}
+
+// certified mode, margin report: the share of the output rows' gap sums that is rounding pad,
+//   marg[row] (+)= sum_j Lam_j^+ m_pos[j] - Lam_j^- m_neg[j]      (upper rows: (mU, mL); lower rows: (mL, mU))
+// for one chain step of the output target; one warp per row (upper and lower rows only).  Rounded up.
+__global__ void row_margin_kernel(int tiles, int rows_pad, int rows_kind, int K, const float* __restrict__ Lam, int a_shared,
+                                  const float* __restrict__ mU, const float* __restrict__ mL, float* __restrict__ marg, int init) {
+    int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (warp >= tiles * 2 * rows_kind) return;
+    const int t = warp / (2 * rows_kind), r = warp - t * 2 * rows_kind, kind = r / rows_kind, rk = r - kind * rows_kind;
+    const float* row = Lam + (size_t)(a_shared ? rk : (size_t)t * rows_pad + r) * K;
+    const float* mp = (kind == 0 ? mU : mL) + (size_t)t * K;
+    const float* mn = (kind == 0 ? mL : mU) + (size_t)t * K;
+    float s = 0.f;
+    for (int j = lane; j < K; j += 32) {
+        const float lv = row[j];
+        s = __fmaf_ru(fabsf(lv), lv > 0.f ? mp[j] : mn[j], s);
+    }
+#pragma unroll
+    for (int off = 16; off; off >>= 1) s = __fadd_ru(s, __shfl_xor_sync(0xffffffffu, s, off));
+    if (lane == 0) marg[(size_t)t * rows_pad + r] = init ? s : __fadd_ru(marg[(size_t)t * rows_pad + r], s);
+}
+
 // N5 for a hidden target s: one warp per (tile, neuron k): rows k (upper) and rows_kind + k (lower)
+// certified mode (e_s != NULL): every term rounded outward -- the |Lam| sigma sums and the gap sums (which carry the
+// chain steps' rounding pads, see relax_fwd_cert_kernel) are sums of same-signed terms, so their FP32 rounding error is
+// relative (factors kap_sum, kap_gap); plus the centre residual e_s of the target neuron (DESIGN.md §6 "Certified margin")
 __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
                                          const float* __restrict__ sigma, const float* __restrict__ gap,
-                                         const float* __restrict__ zhat, float* __restrict__ lb, float* __restrict__ ub) {
+                                         const float* __restrict__ zhat, float* __restrict__ lb, float* __restrict__ ub,
+                                         const float* __restrict__ e_s, float kap_sum, float kap_gap) {
     int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     int total = tiles * rows_kind;
     if (warp >= total) return;
@@ -169,8 +334,17 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
     for (int off = 16; off; off >>= 1) { su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off); }
     if (lane == 0) {
         float z = zhat[(size_t)t * rows_kind + k];
-        ub[(size_t)t * rows_kind + k] = z + (su + gap[(size_t)t * rows_pad + k]);
-        lb[(size_t)t * rows_kind + k] = z - (sl - gap[(size_t)t * rows_pad + rows_kind + k]);
+        const float gu = gap[(size_t)t * rows_pad + k], gl = gap[(size_t)t * rows_pad + rows_kind + k];
+        if (e_s) {
+            const float e = e_s[(size_t)t * rows_kind + k];
+            const float pu = __fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), e);
+            const float pl = __fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), e);
+            ub[(size_t)t * rows_kind + k] = __fadd_ru(z, pu);
+            lb[(size_t)t * rows_kind + k] = __fadd_rd(z, -pl);
+        } else {
+            ub[(size_t)t * rows_kind + k] = z + (su + gu);
+            lb[(size_t)t * rows_kind + k] = z - (sl - gl);
+        }
     }
 }
 
@@ -178,7 +352,9 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
 __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int wp0, const float* __restrict__ Lam0,
                                       const float* __restrict__ sigma, const float* __restrict__ gap,
                                       const float* __restrict__ Jgiven, float* __restrict__ r_lo, float* __restrict__ r_hi,
-                                      int ld_out, int* __restrict__ domain_flag) {
+                                      int ld_out, int* __restrict__ domain_flag, int cert, const float* __restrict__ marg,
+                                      const float* __restrict__ eta, int ld_eta, float kap_sum, float kap_gap,
+                                      float* __restrict__ margin_out) {
     int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     int total = tiles * n;
     if (warp >= total) return;
@@ -208,12 +384,25 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
     if (lane == 0) {
         float hi = su + gap[(size_t)t * rows_pad + i];
         float lo_v = -sl + gap[(size_t)t * rows_pad + n + i];
+        float mg = 0.f;
+        if (cert) {
+            // certified mode: outward-rounded terms (the gap sums carry the chain steps' pads) + eta (the exact nominal
+            // output against the centre the chain was developed around); margin_out = eta, the rounding of these sums and
+            // the chain pads inside the gap sum (marg, gathered by row_margin_kernel when a margin report is asked for)
+            const float gu = gap[(size_t)t * rows_pad + i], gl = gap[(size_t)t * rows_pad + n + i], et = eta[(size_t)t * ld_eta + i];
+            const float pu = __fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), et);
+            const float pl = __fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), et);
+            mg = fmaxf(__fadd_ru(pu, -hi), __fadd_ru(pl, lo_v));
+            if (margin_out) mg = __fadd_ru(mg, fmaxf(marg[(size_t)t * rows_pad + i], marg[(size_t)t * rows_pad + n + i]));
+            hi = pu; lo_v = -pl;
+        }
         if (!(fabsf(hi) <= 3.0e38f) || !(fabsf(lo_v) <= 3.0e38f)) {   // NaN / Inf anywhere in the tile's inputs
-            hi = INFINITY; lo_v = -INFINITY;
+            hi = INFINITY; lo_v = -INFINITY; mg = INFINITY;
             atomicExch(domain_flag, 1);
         }
         r_hi[(size_t)t * ld_out + i] = hi;
         r_lo[(size_t)t * ld_out + i] = lo_v;
+        if (margin_out) margin_out[(size_t)t * ld_out + i] = mg;
     }
 }
 
@@ -312,6 +501,18 @@ __global__ void copy_hidden_kernel(int tiles, int w, int wp, const float* __rest
     }
 }
 
+// Lambda_0 rows of one target: [tiles x rows_pad x wp0] (upper | lower | ...) -> [tiles x 2 x rows x N]
+__global__ void copy_coeffs_kernel(int tiles, int rows, int rows_kind, int rows_pad, int N, int wp0, const float* __restrict__ Lam0,
+                                   float* __restrict__ out) {
+    size_t total = (size_t)tiles * 2 * rows * N;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % N);
+        size_t r = q / N;
+        int k = (int)(r % rows), chain = (int)((r / rows) % 2), t = (int)(r / ((size_t)2 * rows));
+        out[q] = Lam0[((size_t)t * rows_pad + (size_t)chain * rows_kind + k) * wp0 + c];
+    }
+}
+
 inline unsigned gs_grid(size_t work) {
     size_t b = (work + 255) / 256;
     if (b > 148 * 16) b = 148 * 16;
@@ -356,11 +557,11 @@ void ws_free(NnState* S) {
 
 size_t bytes_per_tile(const NnState* S, bool vjp) {
     size_t f = 3 * (size_t)S->wp[0];
-    for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 17 : 9);
+    for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 23 : 15);
     size_t maxLam = 0;
     for (int s = 2; s <= S->L; ++s) {
         for (int l = 0; l <= s - 2; ++l) f += (size_t)S->rows_pad[s] * S->wp[l];
-        f += S->rows_pad[s];
+        f += (size_t)S->rows_pad[s] + (s == S->L ? S->rows_pad[s] : 0);
         for (int l = 0; l <= s - 2; ++l) maxLam = std::max(maxLam, (size_t)S->rows_pad[s] * S->wp[l]);
     }
     if (vjp) f += 2 * maxLam + 2 * (size_t)S->wp[0] + 2 * (size_t)S->w[S->L] + 1024;
@@ -392,6 +593,7 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
         size_t c = (size_t)C * S->wp[l];
         S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
         S->kU[l] = F(c); S->kL[l] = F(c); S->gU[l] = F(c); S->gL[l] = F(c);
+        S->ce[l] = F(c); S->ct[l] = F(c); S->cv[l] = F(c); S->adev[l] = F(c); S->mU[l] = F(c); S->mL[l] = F(c);
         if (vjp) {
             S->kUb[l] = F(c); S->kLb[l] = F(c); S->gUb[l] = F(c); S->gLb[l] = F(c); S->dpb[l] = F(c);
             S->zbar[l] = F(c); S->lbar[l] = F(c); S->ubar[l] = F(c);
@@ -406,6 +608,8 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
         }
         S->gap[s] = F((size_t)C * S->rows_pad[s]);
     }
+    S->marg = F((size_t)C * S->rows_pad[L]);
+    S->eta = F((size_t)C * S->wp[L]);
     if (vjp) {
         S->Lbar[0] = F(maxLam);
         S->Lbar[1] = F(maxLam);
@@ -424,8 +628,27 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
 }
 
 // forward for one chunk of C tiles whose padded inputs are already in S->nomp / S->radp
-void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaStream_t st, long long* launches) {
+void launch_cert_layer(NnState* S, int C, int l, bool out_only, cudaStream_t st, long long* launches) {
+    const int J = out_only ? S->w[l] : S->wp[l], K = S->wp[l - 1];
+    dim3 grid((J + CJ - 1) / CJ, (C + CM - 1) / CM);
+    const float* X = (l == 1) ? S->nomp : S->ahat[l - 1];
+    const float* T = (l == 1) ? nullptr : S->ct[l - 1];
+    const float* A = (l == 1) ? S->radp : S->adev[l - 1];
+    if (out_only)
+        cert_layer_kernel<<<grid, 256, 0, st>>>(C, J, K, S->Wt[l], S->rowsW[l], S->bias[l], nullptr, T, nullptr, K, nullptr, nullptr, S->act, 1,
+                                               nullptr, S->eta, nullptr, S->wp[l]);
+    else
+        cert_layer_kernel<<<grid, 256, 0, st>>>(C, J, K, S->Wt[l], S->rowsW[l], S->bias[l], X, T, A, K, S->zhat[l], S->ahat[l], S->act, 0,
+                                               S->ce[l], S->ct[l], S->cv[l], S->wp[l]);
+    ++*launches;
+}
+
+void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool cert, bool marg_report, cudaStream_t st,
+                   long long* launches) {
     const int L = S->L;
+    int ksum = 0;                                   // total contraction length of the gap sums of the deepest chain
+    for (int l = 1; l < L; ++l) ksum += S->wp[l];
+    const float kap_sum = 1.f + (float)(S->wp[0] + 8) * 1.1920929e-07f, kap_gap = 1.f + (float)(ksum + 64) * 1.1920929e-07f;
     // ---- N1 nominal pass
     const float* a_prev = S->nomp;
     for (int l = 1; l < L; ++l) {
@@ -435,7 +658,14 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
         a_prev = S->ahat[l];
     }
     // ---- N2 layer-1 interval bounds: rad1 = |W_1| sigma
-    {
+    if (cert) {
+        // certified: the radius is the rounded-up product v_1 = |W_1| sigma, widened by the centre residual e_1
+        launch_cert_layer(S, C, 1, false, st, launches);
+        relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(
+            S->act, C, S->w[1], S->wp[1], 1, S->use_tc ? 1 : 0, S->zhat[1], S->ahat[1], S->cv[1], S->ce[1], S->lb[1], S->ub[1], S->kU[1],
+            S->kL[1], S->gU[1], S->gL[1], S->adev[1], S->mU[1], S->mL[1]);
+        ++*launches;
+    } else {
         GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
         launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g, st, launches);
         relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->rad1, S->lb[1],
@@ -447,6 +677,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
         const bool is_out = (s == L);
         const int nk = is_out ? (with_jac ? 3 : 2) : 2;
         const int rp = S->rows_pad[s], rk = S->rows_kind[s];
+        if (cert) launch_cert_layer(S, C, s, is_out, st, launches);     // e_s, t_s, v_s (eta for the output) -- needs adev_{s-1}
         for (int l = s - 1; l >= 1; --l) {
             GemmArgs g{};
             g.M = C * rp; g.N = S->wp[l - 1]; g.K = S->wp[l];
@@ -458,6 +689,12 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
             g.rows_pad = rp; g.rows_kind = rk; g.nkinds = nk;
             g.kU = S->kU[l]; g.kL = S->kL[l]; g.gU = S->gU[l]; g.gL = S->gL[l]; g.dphi = S->dphi[l]; g.ldp = S->wp[l];
             g.gap = S->gap[s]; g.gap_init = (l == s - 1);
+            if (cert && is_out && marg_report) {
+                const size_t warps = (size_t)C * 2 * rk;
+                row_margin_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(C, rp, rk, S->wp[l], g.A, g.a_shared, S->mU[l], S->mL[l],
+                                                                                     S->marg, l == s - 1);
+                ++*launches;
+            }
             const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
             if (S->use_tc) {
                 S->prof->begin(LEB_KC_CHAIN_FWD, st);
@@ -470,11 +707,18 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, cudaSt
         }
         if (!is_out) {
             size_t warps = (size_t)C * rk;
-            concretise_hidden_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(C, rp, rk, S->wp[0], S->Lam[s][0], S->radp,
-                                                                                        S->gap[s], S->zhat[s], S->lb[s], S->ub[s]);
+            concretise_hidden_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(
+                C, rp, rk, S->wp[0], S->Lam[s][0], S->radp, S->gap[s], S->zhat[s], S->lb[s], S->ub[s], cert ? S->ce[s] : nullptr,
+                kap_sum, kap_gap);
             ++*launches;
-            relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s],
-                                                                          S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s]);
+            if (cert) {
+                relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(
+                    S->act, C, S->w[s], S->wp[s], 0, S->use_tc ? 1 : 0, S->zhat[s], S->ahat[s], S->cv[s], S->ce[s], S->lb[s], S->ub[s],
+                    S->kU[s], S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s]);
+            } else {
+                relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s],
+                                                                              S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s]);
+            }
             ++*launches;
         }
     }
@@ -612,7 +856,9 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
                           long long* launches, LebProf* prof) {
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
-    if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;   // certified mode: see DESIGN.md (N6)
+    const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
+    if (cert)
+        for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, false);
     if (ws != LEB_OK) return ws;
@@ -622,21 +868,15 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         pad_inputs_kernel<<<gs_grid((size_t)C * S->wp[0]), 256, 0, st>>>(C, N, ld_in, S->wp[0], nom + (size_t)t0 * ld_in,
                                                                        rad + (size_t)t0 * ld_in, S->nomp, S->radp);
         ++*launches;
-        forward_chunk(S, C, J, J == nullptr, st, launches);
+        forward_chunk(S, C, J, J == nullptr, cert, cert && margin != nullptr, st, launches);
         size_t warps = (size_t)C * n;
+        const int ks = [&] { int k = 0; for (int l = 1; l < L; ++l) k += S->wp[l]; return k; }();
         concretise_out_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(
             C, S->rows_pad[L], n, N, S->wp[0], S->Lam[L][0], S->radp, S->gap[L], J ? J + (size_t)t0 * n * N : nullptr,
-            r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out, ld_out, domain_flag);
+            r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out, ld_out, domain_flag, cert ? 1 : 0, S->marg, S->eta, S->wp[L],
+            1.f + (float)(S->wp[0] + 8) * 1.1920929e-07f, 1.f + (float)(ks + 64) * 1.1920929e-07f,
+            margin ? margin + (size_t)t0 * ld_out : nullptr);     // value mode: no margin is added, 0 is reported
         ++*launches;
-        if (margin) {
-            // value mode: the margin that would have been added is reported as 0 until N6 lands
-            for (int r = 0; r < 1; ++r) {
-                // rows are strided by ld_out: fill row by row only when ld_out != n
-                if (ld_out == n) fill_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(margin + (size_t)t0 * ld_out, (size_t)C * n, 0.f);
-                else fill_kernel<<<gs_grid((size_t)C * ld_out), 256, 0, st>>>(margin + (size_t)t0 * ld_out, (size_t)C * ld_out, 0.f);
-                ++*launches;
-            }
-        }
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
@@ -647,6 +887,15 @@ leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStre
     if (layer < 1 || layer >= S->L || S->last_tiles <= 0 || S->chunk <= 0) return LEB_ERR_STATE;
     copy_hidden_kernel<<<gs_grid((size_t)S->last_tiles * S->w[layer]), 256, 0, st>>>(S->last_tiles, S->w[layer], S->wp[layer],
                                                                                     S->lb[layer], S->ub[layer], l, u);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_nn_get_coeffs(NnState* S, int target, float* out, cudaStream_t st, long long* launches) {
+    if (target < 2 || target > S->L || S->last_tiles <= 0 || S->chunk <= 0) return LEB_ERR_STATE;
+    const int rows = S->w[target];
+    copy_coeffs_kernel<<<gs_grid((size_t)S->last_tiles * 2 * rows * S->w[0]), 256, 0, st>>>(
+        S->last_tiles, rows, S->rows_kind[target], S->rows_pad[target], S->w[0], S->wp[0], S->Lam[target][0], out);
     ++*launches;
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
@@ -671,7 +920,8 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         pad_cotangent_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(C, n, ld_out, g_lo + (size_t)t0 * ld_out,
                                                                    g_hi + (size_t)t0 * ld_out, S->glo_p, S->ghi_p);
         *launches += 2;
-        forward_chunk(S, C, nullptr, true, st, launches);
+        // the VJP is that of the value-mode bound: the certified margin is a rounding-level outward pad, treated as constant
+        forward_chunk(S, C, nullptr, true, false, false, st, launches);
         // ---- zero the adjoint accumulators
         for (int l = 1; l < L; ++l) {
             size_t c = (size_t)C * S->wp[l];

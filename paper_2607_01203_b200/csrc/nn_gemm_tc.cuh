@@ -203,11 +203,15 @@ struct TileGeo {
     int n0;        // first output column
     int rbase;     // r0 relative to its trajectory tile
     size_t po;     // offset of the tile's per-neuron parameter vectors
+    bool rowsums;  // this column-block tile takes the row block's row sums (the gap)
 };
 __device__ __forceinline__ TileGeo tile_geo(const GemmArgs& g, int tile, int col_blocks) {
     TileGeo t;
     const int rb = tile / col_blocks;
     t.n0 = (tile - rb * col_blocks) * TBM;
+    // a CTA's column block is fixed (grid % col_blocks == 0): rotate the tile that takes the row sums with the row block,
+    // so that the extra work does not always land on the same CTAs
+    t.rowsums = (tile - rb * col_blocks) == (rb % col_blocks);
     t.r0 = rb * TBN;
     const int tl = t.r0 / g.rows_pad;
     t.rbase = t.r0 - tl * g.rows_pad;
@@ -645,7 +649,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
             if (nkt == nk) { nkt = 0; ntile = ptile + gridDim.x; }
             const bool nhave = ntile < num_tiles;
             if (nhave && nkt == 0) t_nxt = tile_geo(g, ntile, col_blocks);
-            const bool do_gap = (MODE == MODE_FWD) && (t_cur.n0 == 0) && (g.gap != nullptr);
+            const bool do_gap = (MODE == MODE_FWD) && t_cur.rowsums && (g.gap != nullptr);
             float4 kUc = zero4, kLc = zero4, dpc = zero4, gU4 = zero4, gL4 = zero4;
             int p_used = 0;
             if (MODE == MODE_FWD) {

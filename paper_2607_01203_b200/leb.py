@@ -25,7 +25,7 @@ FLAG_HOST_IO = 4
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
 
@@ -234,6 +234,11 @@ class Context:
         _chk(self.lib.leb_nn_hidden_bounds(self._ctx, int(layer), _ptr(l), _ptr(u), _stream_ptr(self.device)),
              "leb_nn_hidden_bounds")
         return l, u
+
+    def leb_nn_chain_coeffs(self, target: int, tiles: int, rows: int, N: int):
+        out = torch.empty((tiles, 2, rows, N), dtype=torch.float32, device=torch.device("cuda", self.device))
+        _chk(self.lib.leb_nn_chain_coeffs(self._ctx, int(target), _ptr(out), _stream_ptr(self.device)), "leb_nn_chain_coeffs")
+        return out
 
     def leb_launch_count(self) -> int:
         return int(self.lib.leb_launch_count(self._ctx))

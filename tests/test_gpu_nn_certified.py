@@ -1,0 +1,199 @@
+"""GPU tests of the certified mode of leb_nn_fwd (step N6 of SURVEY 8(a); flags without LEB_FLAG_NO_MARGIN): the FP32 /
+3xTF32 rounding error of the CROWN path (Thm 2 eq. (18), Thm 3 eq. (19)-(21) L204-220) is bounded
+and added outward (DESIGN.md §6 "Certified margin").  Checked against the FP64 oracle and against the true remainder:
+* the certified enclosure contains the oracle's (exact-arithmetic CROWN) enclosure, hidden layers and output;
+* it is never below the sampled maximum of the remainder -- with NO tolerance (that is the point of the mode);
+* its looseness over the oracle is small and is reported."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+from parity_util import to_np
+
+pytestmark = pytest.mark.gpu
+
+PATHS = {"tc": 0, "ffma": 2}          # certified mode on both contraction paths
+
+
+@pytest.fixture(scope="module")
+def mods():
+    from paper_2607_01203_b200 import build, leb, workloads
+    from oracle import nn_oracle
+    build.build()
+    return leb, workloads, nn_oracle
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+SMALL = [([5, 9, 3], 1), ([5, 9, 3], 2), ([6, 10, 10, 10, 4], 1), ([6, 10, 10, 10, 4], 2), ([7, 33, 20, 11, 5], 2),
+         ([40, 64, 64, 64, 64, 33], 2), ([24, 130, 70, 20], 1)]
+
+
+def _looseness(clo, chi, olo, ohi):
+    """largest outward excess of the certified enclosure, as a fraction of the tile's widest oracle enclosure"""
+    w = np.maximum((ohi - olo).max(axis=1, keepdims=True), 1e-3)      # a tile whose bound is exactly [0, 0]: absolute scale
+    return float(np.max(np.maximum(chi - ohi, olo - clo) / w))
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_certified_contains_oracle_enclosure(mods, dims, act, path):
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    ctx = leb.context_for_workload(w)
+    nom_d, rad_d = _dev(w.nom), _dev(w.rad)
+    mg = torch.full((w.B, w.T, w.n), -1.0, device="cuda")
+    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d, margin=mg, flags=PATHS[path])
+    nom, rad = w.nom.reshape(-1, w.N), w.rad.reshape(-1, w.N)
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+    hidden = [ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer]) for layer in range(1, len(dims) - 1)]
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad)
+    # the certified enclosure contains the exact-arithmetic one
+    assert np.all(chi >= ohi) and np.all(clo <= olo), (dims, float((ohi - chi).max()), float((clo - olo).max()))
+    for t in range(w.B * w.T):
+        fw = O.crown_forward(Ws, bs, act, nom[t].astype(np.float64), rad[t].astype(np.float64))
+        for layer, (l, u) in enumerate(hidden, start=1):
+            assert np.all(to_np(l)[t] <= fw["ls"][layer - 1]) and np.all(to_np(u)[t] >= fw["us"][layer - 1]), (dims, t, layer)
+    # ... and is not much wider (fraction of the enclosure's width)
+    assert _looseness(clo, chi, olo, ohi) < 2e-2, _looseness(clo, chi, olo, ohi)
+    # the reported margin is what was added over the plain FP32 value; value mode reports 0
+    m = to_np(mg)
+    assert np.all(m > 0) and np.all(m < 1e-2 * (1 + np.abs(to_np(hi))))
+    vlo, vhi = ctx.leb_nn_fwd(nom_d, rad_d, margin=mg, flags=PATHS[path] | leb.FLAG_NO_MARGIN)
+    assert float(mg.abs().max()) == 0.0
+    ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_certified_never_below_sampled_maximum_strict(mods, path):
+    """Tiny nets (<= 4 inputs), >= 1e5 samples + all box vertices per tile, no tolerance.  The caller passes J (FP32),
+    so the remainder is defined with exactly that matrix (Thm 3 holds for any J, reading R12)."""
+    leb, wl, O = mods
+    for dims, act, seed in (([3, 12, 2], 1, 1), ([4, 10, 3], 1, 2), ([4, 8, 8, 2], 2, 3), ([2, 16, 16, 2], 1, 4), ([1, 6, 1], 1, 5)):
+        w = wl.make_small_mlp(dims, act, 2, 2, seed=seed, rad_lo=0.05, rad_hi=0.4)
+        ctx = leb.context_for_workload(w)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        N = dims[0]
+        J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in w.nom.reshape(-1, N)]).astype(np.float32)
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path])
+        clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+        rng = np.random.default_rng(seed)
+        verts = np.array(list(itertools.product((-1.0, 1.0), repeat=N)))
+        for t in range(w.B * w.T):
+            a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+            U = np.concatenate([rng.uniform(-1, 1, (100000, N)), verts])
+            X = a0[None, :] + U * sg[None, :]
+            _, p, _ = O.nominal(Ws, bs, act, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(act, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
+            assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
+        ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("cfg", [3, 5])
+def test_certified_config_sampled_tiles(mods, cfg, path):
+    """Configs 3 and 5 at BASELINE size in the launch configuration bench.py uses; oracle on sampled tiles."""
+    leb, wl, O = mods
+    w = wl.make_config(cfg)
+    ctx = leb.context_for_workload(w)
+    nom_d, rad_d = _dev(w.nom), _dev(w.rad)
+    mg = torch.empty((w.B, w.T, w.n), device="cuda")
+    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d, margin=mg, flags=PATHS[path])
+    assert ctx.leb_domain_flag() == 0
+    vlo, vhi = ctx.leb_nn_fwd(nom_d, rad_d, flags=PATHS[path] | leb.FLAG_NO_MARGIN)
+    nom, rad = w.nom.reshape(-1, w.N), w.rad.reshape(-1, w.N)
+    idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1]) if cfg == 5 else np.linspace(0, w.B * w.T - 1, 16).astype(int)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
+    clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64)[idx], to_np(hi).reshape(-1, w.n).astype(np.float64)[idx]
+    assert np.all(chi >= ohi) and np.all(clo <= olo), (float((ohi - chi).max()), float((clo - olo).max()))
+    loose = _looseness(clo, chi, olo, ohi)
+    print(f"config {cfg} {path}: certified looseness over the oracle enclosure = {loose:.3e} of its width")
+    assert loose < 5e-2
+    # at any size: contains the value-mode result up to the parity tolerance, finite, margin positive
+    # (a widened hidden bound can flip a relaxation case, e.g. the ReLU lower slope at u = -l, to an equally valid
+    # one that happens to be tighter for some output -- reading R21 -- so a few entries may lie inside the value result)
+    inside = ((hi < vhi - 1e-5 * vhi.abs() - 1e-7) | (lo > vlo + 1e-5 * vlo.abs() + 1e-7)).float().mean()
+    print(f"config {cfg} {path}: fraction of entries tighter than value mode (case flips) = {float(inside):.2e}")
+    assert float(inside) < 5e-3
+    assert bool(torch.isfinite(hi).all()) and bool(torch.isfinite(lo).all()) and bool((mg > 0).all())
+    ctx.close()
+
+
+def test_certified_edge_cases(mods):
+    leb, wl, O = mods
+    w = wl.make_small_mlp([6, 10, 10, 4], 1, 2, 3)
+    ctx = leb.context_for_workload(w)
+    nom, rad = _dev(w.nom), _dev(w.rad)
+    # zero radius: the exact bound is [0, 0]; the certified one is a rounding-level enclosure of it
+    lo, hi = ctx.leb_nn_fwd(nom, torch.zeros_like(rad), flags=0)
+    assert bool((lo <= 0).all()) and bool((hi >= 0).all()) and float(hi.max()) < 1e-4 and float(lo.min()) > -1e-4
+    # chunking does not change results
+    lo1, hi1 = ctx.leb_nn_fwd(nom, rad, flags=0)
+    ctx.leb_set_nn_chunk(4)
+    lo2, hi2 = ctx.leb_nn_fwd(nom, rad, flags=0)
+    ctx.leb_set_nn_chunk(0)
+    assert torch.equal(lo1, lo2) and torch.equal(hi1, hi2)
+    # NaN input poisons its tile only
+    n2 = w.nom.copy(); n2[1, 0, 2] = np.nan
+    lo, hi = ctx.leb_nn_fwd(_dev(n2), rad, flags=0)
+    assert ctx.leb_domain_flag() == 1
+    assert bool(torch.isinf(lo[1, 0]).all()) and bool(torch.isinf(hi[1, 0]).all()) and bool(torch.isfinite(lo[0]).all())
+    # the VJP is that of the value-mode bound whichever mode is asked for
+    g1 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=0)
+    g2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN)
+    assert torch.equal(g1[0], g2[0]) and torch.equal(g1[1], g2[1])
+    ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_contraction_error_model(mods, path):
+    """The rounding model behind the margin, probed on one chain step Lambda_0 = W_2 W_1 (ReLU, every
+    hidden neuron stably active so that D = W_2 exactly; K = 512): |computed - exact| <= sum_j gamma_j |W_2[i,j]| |W_1[j,k]|
+    elementwise, on operands built to be bad for a truncating block adder -- all-positive terms (every truncation loses),
+    one large term followed by terms just below each candidate truncation grid, a large term in every block of 8 -- and on
+    random ones.  Reports how much of the bound the worst case uses."""
+    leb, wl, O = mods
+    K, N0, n = 512, 64, 64
+    j = np.arange(K)
+    if path == "tc":
+        gam = (4.5 * (K // 8 - j // 8) + 17.0) * 2.0 ** -23
+    else:
+        gam = (K - j + 4.0) * 2.0 ** -24 + 2.0 ** -23
+    rng = np.random.default_rng(0)
+    cases = {"pos": (rng.uniform(0.5, 1, (n, K)), rng.uniform(0.5, 1, (K, N0))),
+             "rand": (rng.standard_normal((n, K)), rng.standard_normal((K, N0)))}
+    for p in range(22, 31):
+        tiny = 2.0 ** -p * (1 - 2.0 ** -9)
+        W2 = np.full((n, K), tiny); W2[:, 0] = 1.0
+        cases[f"one large, rest 2^-{p}"] = (W2, np.ones((K, N0)))
+        W2 = np.full((n, K), tiny); W2[:, ::8] = 1.0
+        cases[f"large every 8, rest 2^-{p}"] = (W2, np.ones((K, N0)))
+        W2 = np.full((n, K), tiny); W2[:, K // 2] = 1.0
+        cases[f"large in the middle, rest 2^-{p}"] = (W2, np.ones((K, N0)))
+    dev = torch.device("cuda", 0)
+    worst = 0.0
+    for name, (W2, W1) in cases.items():
+        W2 = W2.astype(np.float32); W1 = W1.astype(np.float32)
+        ctx = leb.Context(0)
+        ctx.leb_set_mlp([N0, K, n], [torch.from_numpy(W1).to(dev), torch.from_numpy(W2).to(dev)],
+                        [torch.full((K,), 4.0, device=dev), torch.zeros(n, device=dev)], 1, 1)
+        # hidden pre-activation z_1 = W_1 a + 4 > 0 on the whole box (|a| <= 1e-3): slopes exactly 1
+        nom = torch.zeros((1, 1, N0), device=dev); rad = torch.full((1, 1, N0), 1e-3, device=dev)
+        ctx.leb_nn_fwd(nom, rad, flags=PATHS[path] | leb.FLAG_NO_MARGIN)
+        lam = to_np(ctx.leb_nn_chain_coeffs(2, 1, n, N0)).astype(np.float64)
+        ctx.close()
+        ref = W2.astype(np.float64) @ W1.astype(np.float64)
+        bound = (np.abs(W2).astype(np.float64) * gam[None, :]) @ np.abs(W1).astype(np.float64)
+        for chain in (0, 1):
+            ratio = float(np.max(np.abs(lam[0, chain] - ref) / bound))
+            worst = max(worst, ratio)
+            assert ratio <= 1.0, (name, chain, ratio)
+    print(f"{path}: worst observed contraction error = {worst:.3f} of the model bound")
