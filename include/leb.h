@@ -94,7 +94,12 @@ enum {
                                 every rounding error of the path is bounded and added outward,
                                 so r_lo <= r(a) <= r_hi holds in exact arithmetic for the FP32 weights as given */
     LEB_FLAG_FFMA_ONLY = 2u, /* NN: FP32 FFMA contractions instead of 3xTF32 tcgen05 */
-    LEB_FLAG_HOST_IO = 4u    /* data pointers of this call are host pointers */
+    LEB_FLAG_HOST_IO = 4u,   /* data pointers of this call are host pointers */
+    LEB_FLAG_REUSE_FWD = 8u  /* leb_vjp(kind 1): the caller states that (nom, rad) are those of the previous leb_nn_fwd
+                                call on this context (J == NULL); if the workspace still holds that call's complete
+                                forward state (the batch fitted one chunk) the reverse sweep starts from it instead of
+                                recomputing the forward, otherwise the flag has no effect.  The gradient is then that
+                                of the bound leb_nn_fwd returned (certified mode: its pads held constant). */
 };
 
 leb_status leb_create(leb_ctx** ctx, int device);

@@ -46,6 +46,7 @@ struct NnState {
     int num_sms = 148;
     // workspace for one chunk of tiles
     int chunk_req = 0, chunk = 0;
+    bool chunk_capped = false;   // the default chunk was limited by free memory
     bool ws_vjp = false;
     std::vector<void*> allocs;
     float *nomp = nullptr, *radp = nullptr, *rad1 = nullptr;
@@ -65,7 +66,8 @@ struct NnState {
     float *kUb[kMaxLayers] = {nullptr}, *kLb[kMaxLayers] = {nullptr}, *gUb[kMaxLayers] = {nullptr}, *gLb[kMaxLayers] = {nullptr},
           *dpb[kMaxLayers] = {nullptr}, *zbar[kMaxLayers] = {nullptr}, *lbar[kMaxLayers] = {nullptr}, *ubar[kMaxLayers] = {nullptr};
     float *Lbar[2] = {nullptr, nullptr}, *gapbar = nullptr, *nom_bar = nullptr, *rad_bar = nullptr, *glo_p = nullptr, *ghi_p = nullptr;
-    int last_tiles = 0;
+    int last_tiles = 0;          // > 0: the workspace holds the complete forward state of that many tiles (one chunk)
+    bool last_with_jac = false;  // ... including the Jacobian chain rows (needed by the reverse sweep)
     LebProf* prof = nullptr;
 };
 
@@ -553,6 +555,7 @@ void ws_free(NnState* S) {
     S->allocs.clear();
     S->chunk = 0;
     S->ws_vjp = false;
+    S->last_tiles = 0;
 }
 
 size_t bytes_per_tile(const NnState* S, bool vjp) {
@@ -570,19 +573,29 @@ size_t bytes_per_tile(const NnState* S, bool vjp) {
 
 // (re)allocate the chunk workspace
 leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
-    int want = S->chunk_req > 0 ? S->chunk_req : 0;
-    if (want == 0) {
-        // default: as many tiles as fit in ~24 GB of the 180 GB HBM, at most 2048: fewer, longer launches (tail and launch gaps amortised)
-        size_t per = bytes_per_tile(S, true);
-        size_t c = (size_t)24e9 / (per ? per : 1);
-        if (c < 1) c = 1;
-        if (c > 2048) c = 2048;
-        want = (int)c;
-    }
+    // Default: the whole batch resident (config 5: 6 400 tiles x 17 MB = 108 GB of the 180 GB HBM) -- one launch per chain
+    // step, and leb_vjp can reuse the forward's coefficient blocks (LEB_FLAG_REUSE_FWD) -- capped by 85 % of the free
+    // memory.  The workspace is always sized for the reverse sweep too, so that a later leb_vjp does not reallocate.
+    (void)vjp;
+    int want = S->chunk_req > 0 ? S->chunk_req : tiles;
     if (want > tiles && tiles > 0) want = tiles;
-    if (S->chunk >= want && (S->ws_vjp || !vjp)) return LEB_OK;
+    if (S->chunk >= want || (S->chunk > 0 && S->chunk_capped && S->chunk_req == 0)) return LEB_OK;
     cudaDeviceSynchronize();
     ws_free(S);
+    S->chunk_capped = false;
+    {
+        size_t free_b = 0, total_b = 0;
+        const size_t per = bytes_per_tile(S, true);
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && per > 0) {
+            const size_t fit = (size_t)(0.85 * (double)free_b) / per;
+            if ((size_t)want > fit) { want = fit < 1 ? 1 : (int)fit; S->chunk_capped = true; }
+        }
+        int maxrows = 1;                                   // the FFMA kernels put M / 128 row blocks on grid.y (<= 65535)
+        for (int s = 2; s <= S->L; ++s) maxrows = std::max(maxrows, S->rows_pad[s]);
+        const int lim = (int)((size_t)65535 * 128 / (size_t)maxrows);
+        if (want > lim) { want = lim; S->chunk_capped = true; }
+    }
+    vjp = true;
     const int C = want, L = S->L;
     bool ok = true;
     auto F = [&](size_t count) { return (float*)ws_alloc(S, count * sizeof(float), &ok); };
@@ -878,6 +891,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
             margin ? margin + (size_t)t0 * ld_out : nullptr);     // value mode: no margin is added, 0 is reported
         ++*launches;
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
+        S->last_with_jac = (J == nullptr);
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
@@ -913,15 +927,19 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;
     const int L = S->L, n = S->w[L], N = S->w[0], wp0 = S->wp[0];
+    // LEB_FLAG_REUSE_FWD: the caller states that (nom, rad) are those of the previous leb_nn_fwd call on this context; if the
+    // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
+    const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk;
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
-        pad_inputs_kernel<<<gs_grid((size_t)C * wp0), 256, 0, st>>>(C, N, ld_in, wp0, nom + (size_t)t0 * ld_in,
-                                                                  rad + (size_t)t0 * ld_in, S->nomp, S->radp);
+        if (!reuse)
+            pad_inputs_kernel<<<gs_grid((size_t)C * wp0), 256, 0, st>>>(C, N, ld_in, wp0, nom + (size_t)t0 * ld_in,
+                                                                      rad + (size_t)t0 * ld_in, S->nomp, S->radp);
         pad_cotangent_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(C, n, ld_out, g_lo + (size_t)t0 * ld_out,
                                                                    g_hi + (size_t)t0 * ld_out, S->glo_p, S->ghi_p);
         *launches += 2;
         // the VJP is that of the value-mode bound: the certified margin is a rounding-level outward pad, treated as constant
-        forward_chunk(S, C, nullptr, true, false, false, st, launches);
+        if (!reuse) forward_chunk(S, C, nullptr, true, false, false, st, launches);
         // ---- zero the adjoint accumulators
         for (int l = 1; l < L; ++l) {
             size_t c = (size_t)C * S->wp[l];
@@ -997,7 +1015,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,
                                                                  grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in);
         ++*launches;
-        S->last_tiles = 0;
+        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;

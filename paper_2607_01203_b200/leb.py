@@ -21,6 +21,7 @@ LEB_ERR_STATE = 8
 FLAG_NO_MARGIN = 1
 FLAG_FFMA_ONLY = 2
 FLAG_HOST_IO = 4
+FLAG_REUSE_FWD = 8
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",

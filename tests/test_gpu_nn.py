@@ -100,7 +100,14 @@ def test_config5_full_size_sampled_tiles(mods, path):
     nom_d, rad_d = _dev(w.nom), _dev(w.rad)
     lo, hi = ctx.leb_nn_fwd(nom_d, rad_d, flags=PATHS[path])
     assert ctx.leb_domain_flag() == 0
-    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
+    # as bench.py runs it: the whole batch resident, the VJP starts from the forward's coefficient blocks
+    launches0 = ctx.leb_launch_count()
+    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path] | leb.FLAG_REUSE_FWD)
+    launches_reuse = ctx.leb_launch_count() - launches0
+    gn2, gr2 = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])      # stateless: recomputes
+    assert launches_reuse < ctx.leb_launch_count() - launches0 - launches_reuse, "LEB_FLAG_REUSE_FWD did not skip the forward"
+    for a, b in ((gn, gn2), (gr, gr2)):      # same forward state; column sums are atomic adds, so not bit-identical
+        assert float((a - b).abs().max()) <= 1e-5 * float(b.abs().max())
     nom, rad, g_lo, g_hi = _flat(w)
     idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1])        # chunk boundaries, middle, last
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
@@ -210,10 +217,18 @@ def test_edge_cases(mods):
     ctx.leb_nn_fwd(nomp, radp, r_lo=lop, r_hi=hip)
     lo, hi = ctx.leb_nn_fwd(nom, rad)
     assert torch.equal(lop[..., :4], lo) and torch.equal(hip[..., :4], hi) and float((lop[..., 4:] - 7).abs().max()) == 0.0
+    # LEB_FLAG_REUSE_FWD: same gradient; no effect when the forward state is not there (other batch, chunked batch)
+    ctx.leb_nn_fwd(nom, rad)
+    gA = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
+    gB = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    assert torch.allclose(gA[0], gB[0], rtol=1e-5, atol=1e-7) and torch.allclose(gA[1], gB[1], rtol=1e-5, atol=1e-7)
+    ctx.leb_nn_fwd(nom[:1], rad[:1])
+    gC = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
+    assert torch.allclose(gC[0], gB[0], rtol=1e-5, atol=1e-7) and torch.allclose(gC[1], gB[1], rtol=1e-5, atol=1e-7)
     # chunking does not change results
     ctx.leb_set_nn_chunk(4)
     lo2, hi2 = ctx.leb_nn_fwd(nom, rad)
-    gn2, gr2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    gn2, gr2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
     ctx.leb_set_nn_chunk(0)
     gn, gr = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
     assert torch.equal(lo2, lo) and torch.equal(hi2, hi)
