@@ -248,6 +248,12 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     // (1e-4) leaves room for the truncation of a single accumulator, so two of them alternate and the epilogue
     // of tile i overlaps the main loop of tile i+1
     constexpr int NACC = (MODE == MODE_BWD) ? 2 : 1;
+    // Warp roles.  Forward: the row producers (transform + split) are the critical role: 4 epilogue warps (4..7), 8 producer
+    // warps (8..15).  Reverse sweep: the producers only split, but the epilogue does ~35 instructions per row and one warp
+    // per scheduler cannot issue them fast enough (ncu: producers 67 % idle, epilogue never): 8 epilogue warps (4..11, two
+    // per TMEM lane quadrant, each taking half of the tile's 256 rows) and 4 producer warps (12..15, 16 rows per thread).
+    constexpr int kEpiWarps = (MODE == MODE_BWD) ? 8 : 4, kProdWarps = 12 - kEpiWarps;
+    constexpr int kEpiRows = TBN * 4 / kEpiWarps;             // rows of the tile per epilogue warp
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int col_blocks = (g.N + TBM - 1) / TBM;
@@ -261,8 +267,8 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     }
     if (warp == 1 && lane == 0) {
         for (int s = 0; s < WSTAGES; ++s) { mbar_init(bar_wfull(s), 1); mbar_init(bar_wempty(s), 1); }
-        for (int s = 0; s < RSTAGES; ++s) { mbar_init(bar_rfull(s), PRODUCERS); mbar_init(bar_rempty(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), 128); }
+        for (int s = 0; s < RSTAGES; ++s) { mbar_init(bar_rfull(s), kProdWarps * 32); mbar_init(bar_rempty(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), kEpiWarps * 32); }
         for (int s = 0; s < PSTAGES; ++s) { mbar_init(bar_pfull(s), 1); mbar_init(bar_pempty(s), PRODUCERS / 32); }
         fence_barrier_init();
     }
@@ -273,7 +279,7 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     const uint32_t tmem_base = *tmem_slot;
     // registers per thread: control warps 40; forward: epilogue 104, producers 184 (three slabs of rows in flight
     // plus the slopes of two); reverse sweep: epilogue 168 (four steps of forward coefficients in flight), producers 152
-    constexpr int kEpiRegs = (MODE == MODE_FWD) ? 104 : 168, kProdRegs = (MODE == MODE_FWD) ? 184 : 152;
+    constexpr int kEpiRegs = (MODE == MODE_FWD) ? 104 : 152, kProdRegs = (MODE == MODE_FWD) ? 184 : 168;
 
     if (warp < 4) reg_dec<40>();
     if (warp == 0) {
@@ -357,10 +363,11 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 if (++rs == RSTAGES) { rs = 0; rphase ^= 1; }
             }
         }
-    } else if (warp >= 4 && warp < 8) {
+    } else if (warp >= 4 && warp < 4 + kEpiWarps) {
         // ===================== epilogue: TMEM lane = output column, TMEM column = coefficient row =====================
         if (kEpiRegs < 128) reg_dec<kEpiRegs>(); else reg_inc<kEpiRegs>();
-        const int q = warp - 4;                                  // TMEM lane quadrant of this warp (warp % 4)
+        const int q = (MODE == MODE_BWD) ? (warp & 3) : (warp - 4);          // TMEM lane quadrant of this warp (warp % 4)
+        const int c_lo = (MODE == MODE_BWD) ? ((warp - 4) >> 2) * kEpiRows : 0, c_hi = c_lo + kEpiRows;   // this warp's rows of the tile
         const uint32_t t_lane = tmem_base + ((uint32_t)(q * 32) << 16);
         int tcount = 0;
         for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
@@ -425,23 +432,23 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         for (int j = 0; j < 16; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
                     };
                     float sP = 0.f, sQ = 0.f, hP = 0.f, hQ = 0.f;
-                    float lam0[16], lam1[16], lam2[16], lam3[16];
-                    float gb0, gb1, gb2, gb3 = 0.f;
-                    ld16(lam0, 0); gb0 = __ldg(gbp);
-                    ld16(lam1, 16); gb1 = __ldg(gbp + 16);
-                    ld16(lam2, 32); gb2 = __ldg(gbp + 32);
+                    // two coefficient buffers, 32 rows per loop trip: with 8 epilogue warps the 64-row / four-buffer version
+                    // spent 35-50 % of its samples on instruction-cache misses (stall_no_inst)
+                    float lam0[16], lam1[16];
+                    float gb0, gb1 = 0.f;
+                    ld16(lam0, c_lo); gb0 = __ldg(gbp + c_lo);
                     mbar_wait<200>(bar_tfull(acc), acc_parity);
                     tc_fence_after();
                     float a[16];
-                    tmem_ld<16>(t_acc, a);
-                    float* cp = cbase;
+                    tmem_ld<16>(t_acc + c_lo, a);
+                    float* cp = cbase + (size_t)c_lo * g.ldc;
                     auto fstep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                        if (c + 48 < TBN) { ld16(L, c + 48); gbL = __ldg(gbp + c + 48); }
+                        if (c + 16 < c_hi) { ld16(L, c + 16); gbL = __ldg(gbp + c + 16); }
                         tmem_ld_wait();
                         float d[16];
 #pragma unroll
                         for (int j = 0; j < 16; ++j) d[j] = a[j];
-                        if (c + 16 < TBN) {
+                        if (c + 16 < c_hi) {
                             tmem_ld<16>(t_acc + c + 16, a);
                         } else {                                         // last read of this accumulator: release it
                             tc_fence_before();
@@ -462,11 +469,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                     };
 #pragma unroll 1
-                    for (int c = 0; c < TBN; c += 64) {
-                        fstep(c, lam0, gb0, lam3, gb3);
+                    for (int c = c_lo; c < c_hi; c += 32) {
+                        fstep(c, lam0, gb0, lam1, gb1);
                         fstep(c + 16, lam1, gb1, lam0, gb0);
-                        fstep(c + 32, lam2, gb2, lam1, gb1);
-                        fstep(c + 48, lam3, gb3, lam2, gb2);
                     }
                     skU = up ? sP : sQ; skL = up ? sQ : sP;
                     sgU = up ? hP : hQ; sgL = up ? hQ : hP;
@@ -485,25 +490,23 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         const int kind = (jj >= kb1) + (jj >= kb2);
                         return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
                     };
-                    // forward coefficients three steps (48 rows) ahead of their use -- they come from HBM; the first three
+                    // forward coefficients one step (16 rows) ahead of their use -- they come from HBM; the first
                     // steps are requested before the accumulator is complete and overlap the main loop
-                    float lam0[16], lam1[16], lam2[16], lam3[16];
-                    float gb0, gb1, gb2, gb3 = 0.f;
-                    load_lam(lam0, 0); gb0 = load_gb(0);
-                    load_lam(lam1, 16); gb1 = load_gb(16);
-                    load_lam(lam2, 32); gb2 = load_gb(32);
+                    float lam0[16], lam1[16];
+                    float gb0, gb1 = 0.f;
+                    load_lam(lam0, c_lo); gb0 = load_gb(c_lo);
                     mbar_wait<200>(bar_tfull(acc), acc_parity);
                     tc_fence_after();
                     float a[16];
-                    tmem_ld<16>(t_acc, a);
-                    // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+48, c+64) into L
+                    tmem_ld<16>(t_acc + c_lo, a);
+                    // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+16, c+32) into L
                     auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                        if (c + 48 < TBN) { load_lam(L, c + 48); gbL = load_gb(c + 48); }
+                        if (c + 16 < c_hi) { load_lam(L, c + 16); gbL = load_gb(c + 16); }
                         tmem_ld_wait();
                         float d[16];
     #pragma unroll
                         for (int j = 0; j < 16; ++j) d[j] = a[j];
-                        if (c + 16 < TBN) {
+                        if (c + 16 < c_hi) {
                             tmem_ld<16>(t_acc + c + 16, a);
                         } else {                                             // last read of this accumulator: release it
                             tc_fence_before();
@@ -534,11 +537,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                     };
     #pragma unroll 1
-                    for (int c = 0; c < TBN; c += 64) {
-                        estep(c, lam0, gb0, lam3, gb3);
+                    for (int c = c_lo; c < c_hi; c += 32) {
+                        estep(c, lam0, gb0, lam1, gb1);
                         estep(c + 16, lam1, gb1, lam0, gb0);
-                        estep(c + 32, lam2, gb2, lam1, gb1);
-                        estep(c + 48, lam3, gb3, lam2, gb2);
                     }
                 }
                 if (n_ok) {
@@ -550,7 +551,66 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 }
             }
         }
-    } else if (warp >= 8) {
+    } else if (MODE == MODE_BWD && warp >= 12) {
+        // ===================== row producers, reverse sweep: plain rows, hi/lo split only =====================
+        // 4 warps; warp pw owns rows [pw*64, pw*64 + 64) of the block, a thread 16 of them (8 threads per row, one float4
+        // each).  Two register buffers: the loads of slab i+1 are in flight while slab i is split and stored.
+        reg_inc<kProdRegs>();
+        const int pw = warp - 12;
+        const int r4 = lane >> 3, c4 = lane & 7;
+        const float4* const A4 = reinterpret_cast<const float4*>(g.A);
+        const uint32_t rstride = (uint32_t)(g.lda >> 2) * 4u;          // 4 rows, in float4 units
+        int ltile = blockIdx.x, lkt = 0;
+        bool lhave = ltile < num_tiles;
+        uint32_t lbase = 0;
+        auto set_base = [&]() { lbase = (uint32_t)(((size_t)(ltile / col_blocks * TBN + pw * 64 + r4) * g.lda) >> 2) + c4; };
+        auto issue = [&](float4* buf) {
+            if (!lhave) return;
+            const float4* src = A4 + lbase + (uint32_t)lkt * (TBK / 4);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) buf[i] = __ldg(src + (size_t)i * rstride);
+            if (++lkt == nk) {
+                lkt = 0;
+                ltile += gridDim.x;
+                lhave = ltile < num_tiles;
+                if (lhave) set_base();
+            }
+        };
+        int stage = 0; uint32_t phase = 0;
+        int remaining = 0;
+        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) remaining += nk;
+        auto put = [&](const float4* buf) {
+            mbar_wait(bar_rempty(stage), phase ^ 1);
+            const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const float4 v = buf[i];
+                float4 hi, lo;
+                hi.x = to_tf32(v.x); hi.y = to_tf32(v.y); hi.z = to_tf32(v.z); hi.w = to_tf32(v.w);
+                lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
+                const int row = pw * 64 + i * 4 + r4;
+                const uint32_t off = (uint32_t)row * 128u + (uint32_t)((c4 ^ (row & 7)) << 4);     // 128B swizzle
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_hi + off), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_lo + off), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w) : "memory");
+            }
+            fence_proxy_async();
+            mbar_arrive(bar_rfull(stage));
+            if (++stage == RSTAGES) { stage = 0; phase ^= 1; }
+        };
+        if (lhave) {
+            float4 b0[16], b1[16];
+            set_base();
+            issue(b0);
+            while (true) {
+                issue(b1);
+                put(b0);
+                if (--remaining == 0) break;
+                issue(b0);
+                put(b1);
+                if (--remaining == 0) break;
+            }
+        }
+    } else if (MODE == MODE_FWD && warp >= 8) {
         // ===================== row producers =====================
         // Two cursors walk the CTA's sequence of (tile, K slab): the LOADER issues the global loads of a slab
         // into one of three register buffers two slabs ahead of the TRANSFORMER, which relaxes, splits and
