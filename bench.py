@@ -307,15 +307,69 @@ def run_ours(args):
     return 0
 
 
+def run_other_config(args):
+    """--config 1..4: the same step (forward -> fold -> fold VJP -> VJP) on one of the other BASELINE.json configurations,
+    1 GPU, device-resident inputs.  These are parity-test cases, not the bench line (the contract's line is config 5);
+    this mode exists so that the numbers quoted in DESIGN.md / profiles/ come from a committed command."""
+    import torch
+    from paper_2607_01203_b200 import leb, workloads as wl
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the LEB library has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    w = wl.make_config(args.config)
+    ctx = leb.context_for_workload(w, 0)
+    nom, rad = torch.from_numpy(w.nom).to(dev), torch.from_numpy(w.rad).to(dev)
+    gc, gR = torch.from_numpy(w.g_lo).to(dev), torch.from_numpy(w.g_hi).to(dev)
+    kind = 0 if w.kind == "analytic" else 1
+
+    def fwd():
+        return ctx.leb_analytic_fwd(nom, rad) if kind == 0 else ctx.leb_nn_fwd(nom, rad, flags=leb.FLAG_NO_MARGIN)
+
+    def step():
+        r_lo, r_hi = fwd()
+        ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
+        g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
+        return ctx.leb_vjp(kind, nom, rad, g_lo, g_hi, flags=(leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD) if kind else 0)
+
+    def timed(f, n):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / max(n, 1)
+
+    for _ in range(args.warmup):
+        step()
+    launches0 = ctx.leb_launch_count()
+    ms = timed(step, args.steps)
+    launches = ctx.leb_launch_count() - launches0
+    ms_fwd = timed(fwd, args.steps)
+    line = {"metric": METRIC, "value": w.entries / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "ms_forward_only": ms_fwd, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"config{args.config}: {w.kind}, B={w.B} x T={w.T} tiles, n={w.n}, N={w.N} (parity-test case, not the bench line)"},
+            "gpu_launches": launches}
+    print(json.dumps(line))
+    ctx.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=CONFIG_ID, choices=[1, 2, 3, 4, 5],
+                    help="5 (default) = the bench line; 1-4 = the other BASELINE.json configurations, timing only")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.config != CONFIG_ID:
+        return run_other_config(args)
     return run_ours(args)
 
 
