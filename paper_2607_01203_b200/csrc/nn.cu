@@ -14,11 +14,13 @@
 // Steps: N1 nominal pass, N2 layer-1 interval bounds, N3 hidden targets, N4 output
 // target, N5 concretisation, V reverse sweep.  All contractions are launched from here.
 #include <stdio.h>
+#include <stdlib.h>
 #include <vector>
 #include "internal.h"
 #include "nn_relax.cuh"
 #include "nn_gemm_ffma.cuh"
 #include "nn_gemm_tc.cuh"
+#include "nn_gemm_tc2.cuh"
 
 using namespace leb_nn;
 
@@ -43,6 +45,7 @@ struct NnState {
     float *Whi[kMaxLayers + 1] = {nullptr}, *Wlo[kMaxLayers + 1] = {nullptr}, *Wthi[kMaxLayers + 1] = {nullptr}, *Wtlo[kMaxLayers + 1] = {nullptr};
     CUtensorMap mapW_hi[kMaxLayers + 1], mapW_lo[kMaxLayers + 1], mapWt_hi[kMaxLayers + 1], mapWt_lo[kMaxLayers + 1];
     bool tc_ready = false, use_tc = false, launch_failed = false;
+    bool use_pairs = false;      // forward chain steps on CTA pairs (nn_gemm_tc2.cuh)
     int num_sms = 148;
     // workspace for one chunk of tiles
     int chunk_req = 0, chunk = 0;
@@ -711,7 +714,9 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
             const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
             if (S->use_tc) {
                 S->prof->begin(LEB_KC_CHAIN_FWD, st);
-                if (tc::launch_chain_gemm_tc<tc::MODE_FWD>(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st) != cudaSuccess) S->launch_failed = true;
+                const cudaError_t le = S->use_pairs ? tc2::launch_chain_gemm_tc2_fwd(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st)
+                                                    : tc::launch_chain_gemm_tc<tc::MODE_FWD>(g, S->mapWt_hi[l], S->mapWt_lo[l], S->num_sms, st);
+                if (le != cudaSuccess) S->launch_failed = true;
                 S->prof->end(LEB_KC_CHAIN_FWD, st, flops);
                 ++*launches;
             } else {
@@ -739,6 +744,13 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
 }
 
 }  // namespace
+
+// forward chain steps on CTA pairs (nn_gemm_tc2.cuh); LEB_TC_PAIRS=0 in the environment selects the single-CTA kernel
+static bool pairs_enabled() {
+    static int v = -1;
+    if (v < 0) { const char* e = getenv("LEB_TC_PAIRS"); v = (e && e[0] == '0') ? 0 : 1; }
+    return v == 1;
+}
 
 // ------------------------------------------------------------------------------------------
 // state management
@@ -869,6 +881,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
                           long long* launches, LebProf* prof) {
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
+    S->use_pairs = S->use_tc && pairs_enabled();
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
@@ -923,6 +936,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     (void)domain_flag;
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
+    S->use_pairs = S->use_tc && pairs_enabled();
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;
