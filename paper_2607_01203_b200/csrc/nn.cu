@@ -745,13 +745,6 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
 
 }  // namespace
 
-// forward chain steps on CTA pairs (nn_gemm_tc2.cuh); LEB_TC_PAIRS=0 in the environment selects the single-CTA kernel
-static bool pairs_enabled() {
-    static int v = -1;
-    if (v < 0) { const char* e = getenv("LEB_TC_PAIRS"); v = (e && e[0] == '0') ? 0 : 1; }
-    return v == 1;
-}
-
 // ------------------------------------------------------------------------------------------
 // state management
 // ------------------------------------------------------------------------------------------
@@ -881,7 +874,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
                           long long* launches, LebProf* prof) {
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
-    S->use_pairs = S->use_tc && pairs_enabled();
+    S->use_pairs = S->use_tc && !(flags & LEB_FLAG_SINGLE_CTA);
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
@@ -936,7 +929,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     (void)domain_flag;
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
-    S->use_pairs = S->use_tc && pairs_enabled();
+    S->use_pairs = S->use_tc && !(flags & LEB_FLAG_SINGLE_CTA);
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;

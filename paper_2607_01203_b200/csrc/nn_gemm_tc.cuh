@@ -18,12 +18,15 @@
 //   warp 0       TMA producer: pre-split weight tiles Whi, Wlo [128 x 32] (K-major, 128B swizzle)
 //   warp 1       MMA issuer: 12 tcgen05.mma (M128 x N256 x K8) per 32-wide K slab
 //   warp 2       TMEM allocation (512 columns: main [0,256), correction [256,512))
-//   warps 4-7    epilogue: tcgen05.ld -> registers -> global
-//   warps 8-15   row producers: global FP32 rows -> (forward: D = Lam^+ k_pos + Lam^- k_neg and the
-//                deviation-form constant  gap += Lam^+ g_pos + Lam^- g_neg) -> hi/lo split ->
-//                128B-swizzled K-major shared-memory tiles (generic-proxy stores + async-proxy fence)
-// Stages are handed over with mbarriers: full[s] (256 producer arrivals + the TMA transaction),
-// empty[s] (tcgen05.commit), tmem_full (tcgen05.commit), tmem_empty (128 epilogue arrivals).
+//   warp 3       forward: bulk-TMA loader of the K slab's per-neuron parameters
+//   forward:       warps 4-7 epilogue (tcgen05.ld -> registers -> global), warps 8-15 row producers: global FP32 rows
+//                  -> D = Lam^+ k_pos + Lam^- k_neg and the deviation-form constant gap += Lam^+ g_pos + Lam^- g_neg
+//                  -> hi/lo split -> 128B-swizzled K-major shared-memory tiles (generic-proxy stores + async-proxy fence)
+//   reverse sweep: warps 4-11 epilogue (two per TMEM lane quadrant, half of the tile's rows each), warps 12-15 row
+//                  producers (plain rows, split only, 16 rows per thread)
+// Stages are handed over with mbarriers: full[s] (producer arrivals + the TMA transaction), empty[s] (tcgen05.commit),
+// tmem_full (tcgen05.commit), tmem_empty (epilogue arrivals).
+// The forward step normally runs on CTA pairs instead (nn_gemm_tc2.cuh); this file's forward is LEB_FLAG_SINGLE_CTA.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>

@@ -28,7 +28,7 @@ def _flat(w):
 
 
 # both contraction paths: 3xTF32 tcgen05 (default) and FP32 FFMA (LEB_FLAG_FFMA_ONLY); value mode in both
-PATHS = {"tc": 1, "ffma": 1 | 2}
+PATHS = {"tc": 1, "tc_single_cta": 1 | 16, "ffma": 1 | 2}
 
 
 SMALL = [  # dims, act: ragged widths (not multiples of 4 / 32), 1-4 hidden layers, both activations
@@ -136,6 +136,7 @@ def test_config5_every_tile_both_paths(mods):
         res[path] = (to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n))
     bad = np.zeros(w.B * w.T, dtype=bool)
     for q in (0, 1):
+        assert np.array_equal(res["tc"][q], res["tc_single_cta"][q]), "CTA-pair and single-CTA forward kernels differ"
         a, b = res["tc"][q], res["ffma"][q]
         bad |= (np.abs(a - b) > 3 * (1e-5 * np.abs(b) + 1e-7)).any(1)
     idx = np.nonzero(bad)[0]
