@@ -51,6 +51,7 @@ constexpr int PAR_BYTES = 5 * TBK * 4;                              // parameter
 constexpr int BAR_BYTES = 192;
 constexpr int SMEM_BYTES = RING_BYTES + PSTAGES * PAR_BYTES + BAR_BYTES;   // 226.7 KB of the 227 KB a CTA can have
 constexpr int THREADS = 512;
+constexpr int THREADS_BWD = 768;          // reverse sweep: 4 control + 16 epilogue + 4 producer warps
 constexpr int PRODUCERS = 256;
 constexpr int TMEM_COLS = 512;
 constexpr unsigned long long kSpinLimit = 4000000000ull;            // ~2 s of SM clocks: trap instead of hanging
@@ -115,6 +116,10 @@ __device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
+// hint: bring `bytes` (multiple of 16, 16-byte aligned) of global memory into L2
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
 }
@@ -154,6 +159,15 @@ template <> __device__ __forceinline__ void tmem_ld<16>(uint32_t taddr, float* v
         : "memory");
 #pragma unroll
     for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+template <> __device__ __forceinline__ void tmem_ld<8>(uint32_t taddr, float* v) {
+    uint32_t r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
 }
 template <> __device__ __forceinline__ void tmem_ld<32>(uint32_t taddr, float* v) {
     uint32_t r[32];
@@ -226,7 +240,7 @@ __device__ __forceinline__ TileGeo tile_geo(const GemmArgs& g, int tile, int col
 // the kernel
 // ---------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(THREADS, 1)
+__global__ void __launch_bounds__(MODE == MODE_BWD ? THREADS_BWD : THREADS, 1)
 chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t sbase = smem_u32(smem_raw);
@@ -253,9 +267,10 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     constexpr int NACC = (MODE == MODE_BWD) ? 2 : 1;
     // Warp roles.  Forward: the row producers (transform + split) are the critical role: 4 epilogue warps (4..7), 8 producer
     // warps (8..15).  Reverse sweep: the producers only split, but the epilogue does ~35 instructions per row and one warp
-    // per scheduler cannot issue them fast enough (ncu: producers 67 % idle, epilogue never): 8 epilogue warps (4..11, two
-    // per TMEM lane quadrant, each taking half of the tile's 256 rows) and 4 producer warps (12..15, 16 rows per thread).
-    constexpr int kEpiWarps = (MODE == MODE_BWD) ? 8 : 4, kProdWarps = 12 - kEpiWarps;
+    // per scheduler cannot issue them fast enough (ncu: producers 67 % idle, epilogue never): 768 threads -- 16 epilogue warps
+    // (4..19, four per TMEM lane quadrant, each taking a quarter of the tile's 256 rows, 8 rows per step to fit 72 registers)
+    // and 4 producer warps (20..23, 16 rows per thread).
+    constexpr int kEpiWarps = (MODE == MODE_BWD) ? 16 : 4, kProdWarps = (MODE == MODE_BWD) ? 4 : 8;
     constexpr int kEpiRows = TBN * 4 / kEpiWarps;             // rows of the tile per epilogue warp
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -282,7 +297,10 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
     const uint32_t tmem_base = *tmem_slot;
     // registers per thread: control warps 40; forward: epilogue 104, producers 184 (three slabs of rows in flight
     // plus the slopes of two); reverse sweep: epilogue 168 (four steps of forward coefficients in flight), producers 152
-    constexpr int kEpiRegs = (MODE == MODE_FWD) ? 104 : 152, kProdRegs = (MODE == MODE_FWD) ? 184 : 168;
+    // (the pool setmaxnreg redistributes is what the CTA got at launch: 512 x 128 registers forward, 768 x 80 = 61 440 in the
+    // reverse sweep: 128 x 40 + 512 x 72 + 128 x 152 = 61 440)
+    constexpr int kEpiRegs = (MODE == MODE_FWD) ? 104 : 72, kProdRegs = (MODE == MODE_FWD) ? 184 : 152;
+    constexpr int RB = (MODE == MODE_BWD) ? 8 : 16;           // rows per step of the reverse-sweep epilogue
 
     if (warp < 4) reg_dec<40>();
     if (warp == 0) {
@@ -322,6 +340,21 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     __syncwarp();
                     if (++stage == PSTAGES) { stage = 0; phase ^= 1; }
                 }
+            }
+        } else if (!g.lam_shared) {
+            // ===================== reverse sweep: L2 prefetch of the forward coefficients the epilogue will read =====================
+            // The epilogue reads its tile's 256 x 128 block of Lambda_l from HBM with short register prefetch (ncu: half of its
+            // samples wait on those loads).  When the accumulator of tile i becomes free -- i.e. as its main loop starts -- this
+            // warp asks for the block to be brought into L2 (512 B per row), a whole main loop ahead of the epilogue.
+            int tcount = 0;
+            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++tcount) {
+                const int acc = tcount % NACC;
+                const uint32_t par = (uint32_t)(((tcount / NACC) & 1) ^ 1);
+                for (int probe = 0; probe < 200000 && !mbar_try_wait(bar_tempty(acc), par); ++probe) __nanosleep(100);   // a hint: never block
+                const TileGeo t = tile_geo(g, tile, col_blocks);
+                const int cols = (g.N - t.n0) < TBM ? (g.N - t.n0) : TBM;
+                const float* base = g.Lam + (size_t)t.r0 * g.ldl + t.n0;
+                for (int j = lane; j < TBN; j += 32) bulk_prefetch_l2(base + (size_t)j * g.ldl, (uint32_t)cols * 4u);
             }
         }
     } else if (warp == 1) {
@@ -428,38 +461,41 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     const bool up = (kind0 == 0);
                     const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
                     const float* lp = g.Lam + (size_t)(g.lam_shared ? (t.rbase - kind0 * g.rows_kind) : t.r0) * g.ldl + (n_ok ? n : 0);
-                    const float* gbp = g.gapbar + t.r0 + (lane & 15);
-                    auto ld16 = [&](float* dst, int c) {
+                    // the gap adjoints of this warp's rows (kEpiRows <= 64): lane l holds rows c_lo + l and c_lo + 32 + l
+                    const float gbA = __ldg(g.gapbar + t.r0 + c_lo + lane);
+                    const float gbB = (kEpiRows > 32) ? __ldg(g.gapbar + t.r0 + c_lo + 32 + lane) : 0.f;
+                    auto ldr = [&](float* dst, int c) {
                         const float* q = lp + (size_t)c * g.ldl;
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
+                        for (int j = 0; j < RB; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
                     };
                     float sP = 0.f, sQ = 0.f, hP = 0.f, hQ = 0.f;
                     // two coefficient buffers, 32 rows per loop trip: with 8 epilogue warps the 64-row / four-buffer version
                     // spent 35-50 % of its samples on instruction-cache misses (stall_no_inst)
-                    float lam0[16], lam1[16];
-                    float gb0, gb1 = 0.f;
-                    ld16(lam0, c_lo); gb0 = __ldg(gbp + c_lo);
+                    float lam0[RB], lam1[RB];
+                    ldr(lam0, c_lo);
                     mbar_wait<200>(bar_tfull(acc), acc_parity);
                     tc_fence_after();
-                    float a[16];
-                    tmem_ld<16>(t_acc + c_lo, a);
+                    float a[RB];
+                    tmem_ld<RB>(t_acc + c_lo, a);
                     float* cp = cbase + (size_t)c_lo * g.ldc;
-                    auto fstep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                        if (c + 16 < c_hi) { ld16(L, c + 16); gbL = __ldg(gbp + c + 16); }
+                    auto fstep = [&](int c, const float* P, float* L) {
+                        if (c + RB < c_hi) ldr(L, c + RB);
+                        const int rl = c - c_lo;                              // first row of the step inside the warp's range
+                        const float gbsrc = rl < 32 ? gbA : gbB;
                         tmem_ld_wait();
-                        float d[16];
+                        float d[RB];
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) d[j] = a[j];
-                        if (c + 16 < c_hi) {
-                            tmem_ld<16>(t_acc + c + 16, a);
+                        for (int j = 0; j < RB; ++j) d[j] = a[j];
+                        if (c + RB < c_hi) {
+                            tmem_ld<RB>(t_acc + c + RB, a);
                         } else {                                         // last read of this accumulator: release it
                             tc_fence_before();
                             mbar_arrive(bar_tempty(acc));
                         }
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
-                            const float gb = __shfl_sync(0xffffffffu, gbP, j);
+                        for (int j = 0; j < RB; ++j) {
+                            const float gb = __shfl_sync(0xffffffffu, gbsrc, (rl & 31) + j);
                             const float Db = d[j], lv = P[j];
                             const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
                             sP = fmaf(Db, Pp, sP); sQ = fmaf(Db, Q, sQ);
@@ -472,16 +508,16 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                     };
 #pragma unroll 1
-                    for (int c = c_lo; c < c_hi; c += 32) {
-                        fstep(c, lam0, gb0, lam1, gb1);
-                        fstep(c + 16, lam1, gb1, lam0, gb0);
+                    for (int c = c_lo; c < c_hi; c += 2 * RB) {
+                        fstep(c, lam0, lam1);
+                        fstep(c + RB, lam1, lam0);
                     }
                     skU = up ? sP : sQ; skL = up ? sQ : sP;
                     sgU = up ? hP : hQ; sgL = up ? hQ : hP;
                 } else {
                     auto load_lam = [&](float* dst, int c) {
     #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
+                        for (int j = 0; j < RB; ++j) {
                             const int jj = c + j;
                             const int kind = (jj >= kb1) + (jj >= kb2);
                             const int row = g.lam_shared ? (t.rbase + jj - kind * g.rows_kind) : (t.r0 + jj);
@@ -489,34 +525,34 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                     };
                     auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
-                        const int jj = c + (lane & 15);
+                        const int jj = c + (lane & (RB - 1));
                         const int kind = (jj >= kb1) + (jj >= kb2);
                         return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
                     };
                     // forward coefficients one step (16 rows) ahead of their use -- they come from HBM; the first
                     // steps are requested before the accumulator is complete and overlap the main loop
-                    float lam0[16], lam1[16];
+                    float lam0[RB], lam1[RB];
                     float gb0, gb1 = 0.f;
                     load_lam(lam0, c_lo); gb0 = load_gb(c_lo);
                     mbar_wait<200>(bar_tfull(acc), acc_parity);
                     tc_fence_after();
-                    float a[16];
-                    tmem_ld<16>(t_acc + c_lo, a);
+                    float a[RB];
+                    tmem_ld<RB>(t_acc + c_lo, a);
                     // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+16, c+32) into L
                     auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                        if (c + 16 < c_hi) { load_lam(L, c + 16); gbL = load_gb(c + 16); }
+                        if (c + RB < c_hi) { load_lam(L, c + RB); gbL = load_gb(c + RB); }
                         tmem_ld_wait();
-                        float d[16];
+                        float d[RB];
     #pragma unroll
-                        for (int j = 0; j < 16; ++j) d[j] = a[j];
-                        if (c + 16 < c_hi) {
-                            tmem_ld<16>(t_acc + c + 16, a);
+                        for (int j = 0; j < RB; ++j) d[j] = a[j];
+                        if (c + RB < c_hi) {
+                            tmem_ld<RB>(t_acc + c + RB, a);
                         } else {                                             // last read of this accumulator: release it
                             tc_fence_before();
                             mbar_arrive(bar_tempty(acc));
                         }
     #pragma unroll
-                        for (int j = 0; j < 16; ++j) {
+                        for (int j = 0; j < RB; ++j) {
                             const int jj = c + j;
                             const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
                             const float gb = __shfl_sync(0xffffffffu, gbP, j);
@@ -540,9 +576,9 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                         }
                     };
     #pragma unroll 1
-                    for (int c = c_lo; c < c_hi; c += 32) {
+                    for (int c = c_lo; c < c_hi; c += 2 * RB) {
                         estep(c, lam0, gb0, lam1, gb1);
-                        estep(c + 16, lam1, gb1, lam0, gb0);
+                        estep(c + RB, lam1, gb1, lam0, gb0);
                     }
                 }
                 if (n_ok) {
@@ -554,12 +590,12 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                 }
             }
         }
-    } else if (MODE == MODE_BWD && warp >= 12) {
+    } else if (MODE == MODE_BWD && warp >= 4 + kEpiWarps) {
         // ===================== row producers, reverse sweep: plain rows, hi/lo split only =====================
         // 4 warps; warp pw owns rows [pw*64, pw*64 + 64) of the block, a thread 16 of them (8 threads per row, one float4
         // each).  Two register buffers: the loads of slab i+1 are in flight while slab i is split and stored.
         reg_inc<kProdRegs>();
-        const int pw = warp - 12;
+        const int pw = warp - (4 + kEpiWarps);
         const int r4 = lane >> 3, c4 = lane & 7;
         const float4* const A4 = reinterpret_cast<const float4*>(g.A);
         const uint32_t rstride = (uint32_t)(g.lda >> 2) * 4u;          // 4 rows, in float4 units
@@ -852,7 +888,7 @@ inline cudaError_t launch_chain_gemm_tc(const GemmArgs& g, const CUtensorMap& hi
     if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
     const int tiles = (g.M / TBN) * ((g.N + TBM - 1) / TBM);
     const int grid = tiles < num_sms ? tiles : num_sms;
-    chain_gemm_tc_kernel<MODE><<<grid, THREADS, SMEM_BYTES, st>>>(g, hi, lo);
+    chain_gemm_tc_kernel<MODE><<<grid, MODE == MODE_BWD ? THREADS_BWD : THREADS, SMEM_BYTES, st>>>(g, hi, lo);
     return cudaGetLastError();
 }
 
