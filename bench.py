@@ -32,7 +32,7 @@ UNIT = "entries/s"
 CONFIG_ID = 5
 WORKLOAD = ("config5: MLP 224->512x4->168 tanh residual, Xavier-normal weights, B=64 x T=100 tiles per GPU, "
             "radii U[0.005,0.03], forward + VJP")
-KC_NAMES = {0: "chain_gemm_tc2_fwd_kernel (CROWN back-substitution step, CTA pairs)", 1: "chain_gemm_tc_kernel<1> (reverse-sweep step)"}
+KC_NAMES = {0: "chain_gemm_tc2_fwd_kernel (CROWN back-substitution step, CTA pairs)", 1: "chain_gemm_tc2_bwd_kernel (reverse-sweep step, CTA pairs)"}
 
 
 def _clock_sampler(gpu_index: int):

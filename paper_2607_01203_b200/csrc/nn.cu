@@ -989,7 +989,9 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                 const double flops = 2.0 * C * nk * (is_out ? S->w[L] : S->w[s]) * (double)S->w[l] * S->w[l - 1];
                 if (S->use_tc) {
                     S->prof->begin(LEB_KC_CHAIN_BWD, st);
-                    if (tc::launch_chain_gemm_tc<tc::MODE_BWD>(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st) != cudaSuccess) S->launch_failed = true;
+                    const cudaError_t le = S->use_pairs ? tc2::launch_chain_gemm_tc2_bwd(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st)
+                                                        : tc::launch_chain_gemm_tc<tc::MODE_BWD>(g, S->mapW_hi[l], S->mapW_lo[l], S->num_sms, st);
+                    if (le != cudaSuccess) S->launch_failed = true;
                     S->prof->end(LEB_KC_CHAIN_BWD, st, flops);
                     ++*launches;
                 } else {

@@ -237,6 +237,162 @@ __device__ __forceinline__ TileGeo tile_geo(const GemmArgs& g, int tile, int col
 }
 
 // ---------------------------------------------------------------------------------------------
+// reverse-sweep epilogue of one tile for one warp (shared by the single-CTA and the CTA-pair kernel): rows [c_lo, c_hi) of
+// the tile's accumulator (TMEM address t_acc: this warp's lane quadrant, the tile's accumulator), output column n = lane.
+// Masks the adjoint with the forward coefficients, writes C, keeps the five column sums in registers and
+// adds them to the parameter adjoints.  release_acc() is called once, after the last TMEM read.
+// ---------------------------------------------------------------------------------------------
+template <int RB, int EPI_ROWS, class ReleaseFn>
+__device__ __forceinline__ void bwd_epilogue_tile(const GemmArgs& g, int r0, int rbase, size_t po, int n, bool n_ok, int lane,
+                                                  uint32_t t_acc, int c_lo, int c_hi, uint32_t tfull_bar, uint32_t acc_parity,
+                                                  ReleaseFn release_acc) {
+    // row kinds inside the block: [0,kb1) upper chain, [kb1,kb2) lower, [kb2,kbe) Jacobian, then padding
+    const int kb1 = g.rows_kind - rbase, kb2 = 2 * g.rows_kind - rbase, kbe = g.nkinds * g.rows_kind - rbase;
+    float kU = 0.f, kL = 0.f, gU = 0.f, gL = 0.f, dp = 0.f;
+    if (n_ok) {
+        kU = __ldg(g.kU + po + n); kL = __ldg(g.kL + po + n);
+        gU = __ldg(g.gU + po + n); gL = __ldg(g.gL + po + n);
+        dp = __ldg(g.dphi + po + n);
+    }
+    float skU = 0.f, skL = 0.f, sgU = 0.f, sgL = 0.f, sdb = 0.f;
+    float* cbase = g.C + (size_t)r0 * g.ldc + n;
+    const int kind0 = (0 >= kb1) + (0 >= kb2);
+    const bool uniform = (kind0 == (TBN - 1 >= kb1) + (TBN - 1 >= kb2)) && (TBN - 1 < kbe) && (kind0 < 2);
+    if (uniform) {
+        // ---- all 256 rows on one chain (every hidden-layer target): no per-row selection
+        const bool up = (kind0 == 0);
+        const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
+        const float* lp = g.Lam + (size_t)(g.lam_shared ? (rbase - kind0 * g.rows_kind) : r0) * g.ldl + (n_ok ? n : 0);
+        // the gap adjoints of this warp's rows (EPI_ROWS <= 64): lane l holds rows c_lo + l and c_lo + 32 + l
+        const float gbA = __ldg(g.gapbar + r0 + c_lo + lane);
+        const float gbB = (EPI_ROWS > 32) ? __ldg(g.gapbar + r0 + c_lo + 32 + lane) : 0.f;
+        auto ldr = [&](float* dst, int c) {
+            const float* q = lp + (size_t)c * g.ldl;
+#pragma unroll
+            for (int j = 0; j < RB; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
+        };
+        float sP = 0.f, sQ = 0.f, hP = 0.f, hQ = 0.f;
+        // two coefficient buffers, 32 rows per loop trip: with 8 epilogue warps the 64-row / four-buffer version
+        // spent 35-50 % of its samples on instruction-cache misses (stall_no_inst)
+        float lam0[RB], lam1[RB];
+        ldr(lam0, c_lo);
+        mbar_wait<200>(tfull_bar, acc_parity);
+        tc_fence_after();
+        float a[RB];
+        tmem_ld<RB>(t_acc + c_lo, a);
+        float* cp = cbase + (size_t)c_lo * g.ldc;
+        auto fstep = [&](int c, const float* P, float* L) {
+            if (c + RB < c_hi) ldr(L, c + RB);
+            const int rl = c - c_lo;                              // first row of the step inside the warp's range
+            const float gbsrc = rl < 32 ? gbA : gbB;
+            tmem_ld_wait();
+            float d[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) d[j] = a[j];
+            if (c + RB < c_hi) {
+                tmem_ld<RB>(t_acc + c + RB, a);
+            } else {                                         // last read of this accumulator: release it
+                tc_fence_before();
+                release_acc();
+            }
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const float gb = __shfl_sync(0xffffffffu, gbsrc, (rl & 31) + j);
+                const float Db = d[j], lv = P[j];
+                const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                sP = fmaf(Db, Pp, sP); sQ = fmaf(Db, Q, sQ);
+                hP = fmaf(gb, Pp, hP); hQ = fmaf(gb, Q, hQ);
+                const bool pos = lv > 0.f;
+                float out = fmaf(Db, pos ? kp : kn, gb * (pos ? gp : gn));
+                out = (lv == 0.f) ? 0.f : out;
+                if (g.write_c && n_ok) *cp = out;
+                cp += g.ldc;
+            }
+        };
+#pragma unroll 1
+        for (int c = c_lo; c < c_hi; c += 2 * RB) {
+            fstep(c, lam0, lam1);
+            fstep(c + RB, lam1, lam0);
+        }
+        skU = up ? sP : sQ; skL = up ? sQ : sP;
+        sgU = up ? hP : hQ; sgL = up ? hQ : hP;
+    } else {
+        auto load_lam = [&](float* dst, int c) {
+    #pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int jj = c + j;
+                const int kind = (jj >= kb1) + (jj >= kb2);
+                const int row = g.lam_shared ? (rbase + jj - kind * g.rows_kind) : (r0 + jj);
+                dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
+            }
+        };
+        auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
+            const int jj = c + (lane & (RB - 1));
+            const int kind = (jj >= kb1) + (jj >= kb2);
+            return (jj < kbe && kind < 2) ? __ldg(g.gapbar + r0 + jj) : 0.f;
+        };
+        // forward coefficients one step (16 rows) ahead of their use -- they come from HBM; the first
+        // steps are requested before the accumulator is complete and overlap the main loop
+        float lam0[RB], lam1[RB];
+        float gb0, gb1 = 0.f;
+        load_lam(lam0, c_lo); gb0 = load_gb(c_lo);
+        mbar_wait<200>(tfull_bar, acc_parity);
+        tc_fence_after();
+        float a[RB];
+        tmem_ld<RB>(t_acc + c_lo, a);
+        // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+16, c+32) into L
+        auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
+            if (c + RB < c_hi) { load_lam(L, c + RB); gbL = load_gb(c + RB); }
+            tmem_ld_wait();
+            float d[RB];
+    #pragma unroll
+            for (int j = 0; j < RB; ++j) d[j] = a[j];
+            if (c + RB < c_hi) {
+                tmem_ld<RB>(t_acc + c + RB, a);
+            } else {                                             // last read of this accumulator: release it
+                tc_fence_before();
+                release_acc();
+            }
+    #pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int jj = c + j;
+                const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
+                const float gb = __shfl_sync(0xffffffffu, gbP, j);
+                const float Db = d[j], lv = P[j];
+                float out = 0.f;
+                if (jj < kbe) {
+                    if (kind == 2) {
+                        sdb = fmaf(Db, lv, sdb);
+                        out = Db * dp;
+                    } else {
+                        const bool up = (kind == 0);
+                        const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
+                        const float dP = Db * Pp, dQ = Db * Q, gP = gb * Pp, gQ = gb * Q;
+                        skU += up ? dP : dQ; skL += up ? dQ : dP;
+                        sgU += up ? gP : gQ; sgL += up ? gQ : gP;
+                        const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
+                        out = lv > 0.f ? fmaf(Db, kp, gb * gp) : (lv < 0.f ? fmaf(Db, kn, gb * gn) : 0.f);
+                    }
+                }
+                if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
+            }
+        };
+    #pragma unroll 1
+        for (int c = c_lo; c < c_hi; c += 2 * RB) {
+            estep(c, lam0, gb0, lam1, gb1);
+            estep(c + RB, lam1, gb1, lam0, gb0);
+        }
+    }
+    if (n_ok) {
+        atomicAdd(g.kUb + po + n, skU);
+        atomicAdd(g.kLb + po + n, skL);
+        atomicAdd(g.gUb + po + n, sgU);
+        atomicAdd(g.gLb + po + n, sgL);
+        if (g.nkinds == 3) atomicAdd(g.db + po + n, sdb);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
 template <int MODE>
@@ -443,151 +599,8 @@ chain_gemm_tc_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi
                     }
                 }
             } else {
-                // row kinds inside the block: [0,kb1) upper chain, [kb1,kb2) lower, [kb2,kbe) Jacobian, then padding
-                const int kb1 = g.rows_kind - t.rbase, kb2 = 2 * g.rows_kind - t.rbase, kbe = g.nkinds * g.rows_kind - t.rbase;
-                float kU = 0.f, kL = 0.f, gU = 0.f, gL = 0.f, dp = 0.f;
-                if (n_ok) {
-                    kU = __ldg(g.kU + t.po + n); kL = __ldg(g.kL + t.po + n);
-                    gU = __ldg(g.gU + t.po + n); gL = __ldg(g.gL + t.po + n);
-                    dp = __ldg(g.dphi + t.po + n);
-                }
-                float skU = 0.f, skL = 0.f, sgU = 0.f, sgL = 0.f, sdb = 0.f;
-                const uint32_t t_acc = t_lane + acc * TBN;
-                float* cbase = g.C + (size_t)t.r0 * g.ldc + n;
-                const int kind0 = (0 >= kb1) + (0 >= kb2);
-                const bool uniform = (kind0 == (TBN - 1 >= kb1) + (TBN - 1 >= kb2)) && (TBN - 1 < kbe) && (kind0 < 2);
-                if (uniform) {
-                    // ---- all 256 rows on one chain (every hidden-layer target): no per-row selection
-                    const bool up = (kind0 == 0);
-                    const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
-                    const float* lp = g.Lam + (size_t)(g.lam_shared ? (t.rbase - kind0 * g.rows_kind) : t.r0) * g.ldl + (n_ok ? n : 0);
-                    // the gap adjoints of this warp's rows (kEpiRows <= 64): lane l holds rows c_lo + l and c_lo + 32 + l
-                    const float gbA = __ldg(g.gapbar + t.r0 + c_lo + lane);
-                    const float gbB = (kEpiRows > 32) ? __ldg(g.gapbar + t.r0 + c_lo + 32 + lane) : 0.f;
-                    auto ldr = [&](float* dst, int c) {
-                        const float* q = lp + (size_t)c * g.ldl;
-#pragma unroll
-                        for (int j = 0; j < RB; ++j) dst[j] = __ldg(q + (size_t)j * g.ldl);
-                    };
-                    float sP = 0.f, sQ = 0.f, hP = 0.f, hQ = 0.f;
-                    // two coefficient buffers, 32 rows per loop trip: with 8 epilogue warps the 64-row / four-buffer version
-                    // spent 35-50 % of its samples on instruction-cache misses (stall_no_inst)
-                    float lam0[RB], lam1[RB];
-                    ldr(lam0, c_lo);
-                    mbar_wait<200>(bar_tfull(acc), acc_parity);
-                    tc_fence_after();
-                    float a[RB];
-                    tmem_ld<RB>(t_acc + c_lo, a);
-                    float* cp = cbase + (size_t)c_lo * g.ldc;
-                    auto fstep = [&](int c, const float* P, float* L) {
-                        if (c + RB < c_hi) ldr(L, c + RB);
-                        const int rl = c - c_lo;                              // first row of the step inside the warp's range
-                        const float gbsrc = rl < 32 ? gbA : gbB;
-                        tmem_ld_wait();
-                        float d[RB];
-#pragma unroll
-                        for (int j = 0; j < RB; ++j) d[j] = a[j];
-                        if (c + RB < c_hi) {
-                            tmem_ld<RB>(t_acc + c + RB, a);
-                        } else {                                         // last read of this accumulator: release it
-                            tc_fence_before();
-                            mbar_arrive(bar_tempty(acc));
-                        }
-#pragma unroll
-                        for (int j = 0; j < RB; ++j) {
-                            const float gb = __shfl_sync(0xffffffffu, gbsrc, (rl & 31) + j);
-                            const float Db = d[j], lv = P[j];
-                            const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
-                            sP = fmaf(Db, Pp, sP); sQ = fmaf(Db, Q, sQ);
-                            hP = fmaf(gb, Pp, hP); hQ = fmaf(gb, Q, hQ);
-                            const bool pos = lv > 0.f;
-                            float out = fmaf(Db, pos ? kp : kn, gb * (pos ? gp : gn));
-                            out = (lv == 0.f) ? 0.f : out;
-                            if (g.write_c && n_ok) *cp = out;
-                            cp += g.ldc;
-                        }
-                    };
-#pragma unroll 1
-                    for (int c = c_lo; c < c_hi; c += 2 * RB) {
-                        fstep(c, lam0, lam1);
-                        fstep(c + RB, lam1, lam0);
-                    }
-                    skU = up ? sP : sQ; skL = up ? sQ : sP;
-                    sgU = up ? hP : hQ; sgL = up ? hQ : hP;
-                } else {
-                    auto load_lam = [&](float* dst, int c) {
-    #pragma unroll
-                        for (int j = 0; j < RB; ++j) {
-                            const int jj = c + j;
-                            const int kind = (jj >= kb1) + (jj >= kb2);
-                            const int row = g.lam_shared ? (t.rbase + jj - kind * g.rows_kind) : (t.r0 + jj);
-                            dst[j] = (n_ok && jj < kbe) ? __ldg(g.Lam + (size_t)row * g.ldl + n) : 0.f;
-                        }
-                    };
-                    auto load_gb = [&](int c) {      // the rows' gap adjoints: lane j < 16 fetches row c + j, broadcast by shuffle
-                        const int jj = c + (lane & (RB - 1));
-                        const int kind = (jj >= kb1) + (jj >= kb2);
-                        return (jj < kbe && kind < 2) ? __ldg(g.gapbar + t.r0 + jj) : 0.f;
-                    };
-                    // forward coefficients one step (16 rows) ahead of their use -- they come from HBM; the first
-                    // steps are requested before the accumulator is complete and overlap the main loop
-                    float lam0[RB], lam1[RB];
-                    float gb0, gb1 = 0.f;
-                    load_lam(lam0, c_lo); gb0 = load_gb(c_lo);
-                    mbar_wait<200>(bar_tfull(acc), acc_parity);
-                    tc_fence_after();
-                    float a[RB];
-                    tmem_ld<RB>(t_acc + c_lo, a);
-                    // one step: rows [c, c+16) with coefficients P / gap adjoints gbP; prefetch rows [c+16, c+32) into L
-                    auto estep = [&](int c, const float* P, float gbP, float* L, float& gbL) {
-                        if (c + RB < c_hi) { load_lam(L, c + RB); gbL = load_gb(c + RB); }
-                        tmem_ld_wait();
-                        float d[RB];
-    #pragma unroll
-                        for (int j = 0; j < RB; ++j) d[j] = a[j];
-                        if (c + RB < c_hi) {
-                            tmem_ld<RB>(t_acc + c + RB, a);
-                        } else {                                             // last read of this accumulator: release it
-                            tc_fence_before();
-                            mbar_arrive(bar_tempty(acc));
-                        }
-    #pragma unroll
-                        for (int j = 0; j < RB; ++j) {
-                            const int jj = c + j;
-                            const int kind = (jj >= kb1) + (jj >= kb2);            // warp-uniform
-                            const float gb = __shfl_sync(0xffffffffu, gbP, j);
-                            const float Db = d[j], lv = P[j];
-                            float out = 0.f;
-                            if (jj < kbe) {
-                                if (kind == 2) {
-                                    sdb = fmaf(Db, lv, sdb);
-                                    out = Db * dp;
-                                } else {
-                                    const bool up = (kind == 0);
-                                    const float Pp = fmaxf(lv, 0.f), Q = fminf(lv, 0.f);
-                                    const float dP = Db * Pp, dQ = Db * Q, gP = gb * Pp, gQ = gb * Q;
-                                    skU += up ? dP : dQ; skL += up ? dQ : dP;
-                                    sgU += up ? gP : gQ; sgL += up ? gQ : gP;
-                                    const float kp = up ? kU : kL, kn = up ? kL : kU, gp = up ? gU : gL, gn = up ? gL : gU;
-                                    out = lv > 0.f ? fmaf(Db, kp, gb * gp) : (lv < 0.f ? fmaf(Db, kn, gb * gn) : 0.f);
-                                }
-                            }
-                            if (g.write_c && n_ok) cbase[(size_t)jj * g.ldc] = out;
-                        }
-                    };
-    #pragma unroll 1
-                    for (int c = c_lo; c < c_hi; c += 2 * RB) {
-                        estep(c, lam0, gb0, lam1, gb1);
-                        estep(c + RB, lam1, gb1, lam0, gb0);
-                    }
-                }
-                if (n_ok) {
-                    atomicAdd(g.kUb + t.po + n, skU);
-                    atomicAdd(g.kLb + t.po + n, skL);
-                    atomicAdd(g.gUb + t.po + n, sgU);
-                    atomicAdd(g.gLb + t.po + n, sgL);
-                    if (g.nkinds == 3) atomicAdd(g.db + t.po + n, sdb);
-                }
+                bwd_epilogue_tile<RB, kEpiRows>(g, t.r0, t.rbase, t.po, n, n_ok, lane, t_lane + acc * TBN, c_lo, c_hi, bar_tfull(acc),
+                                                acc_parity, [&]() { mbar_arrive(bar_tempty(acc)); });
             }
         }
     } else if (MODE == MODE_BWD && warp >= 4 + kEpiWarps) {

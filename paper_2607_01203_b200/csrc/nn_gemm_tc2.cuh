@@ -459,6 +459,209 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// reverse-sweep step on CTA pairs: D_l = Lbar_{l-1} W_l^T with the sign-masked epilogue.  Same pair protocol
+// as the forward; 768 threads per CTA: 4 control warps, 16 epilogue warps (bwd_epilogue_tile of nn_gemm_tc.cuh, this CTA's
+// 128 output columns x all 256 rows, two alternating accumulators), 4 producer warps (this CTA's 128 rows, split only).
+// ---------------------------------------------------------------------------------------------
+constexpr int SMEM2B_BYTES = RING2_BYTES + 256;
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS_BWD, 1)
+chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap tm_hi, const __grid_constant__ CUtensorMap tm_lo) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t sbase = smem_u32(smem_raw);
+    if ((sbase & 1023u) != 0u) __trap();
+    uint8_t* sgen = smem_raw;
+    auto sW = [&](int s, int part) { return sbase + (2 * s + part) * W_TILE_BYTES; };
+    auto sR = [&](int s, int part) { return sbase + WSTAGES * 2 * W_TILE_BYTES + (2 * s + part) * R2_TILE_BYTES; };
+    const uint32_t bar0 = sbase + RING2_BYTES;
+    auto bar_wfull = [&](int s) { return bar0 + 8 * s; };
+    auto bar_wempty = [&](int s) { return bar0 + 8 * (WSTAGES + s); };
+    auto bar_rfull = [&](int s) { return bar0 + 8 * (2 * WSTAGES + s); };
+    auto bar_rempty = [&](int s) { return bar0 + 8 * (2 * WSTAGES + R2STAGES + s); };
+    auto bar_tfull = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * R2STAGES + a); };
+    auto bar_tempty = [&](int a) { return bar0 + 8 * (2 * WSTAGES + 2 * R2STAGES + 2 + a); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sgen + RING2_BYTES + 8 * (2 * WSTAGES + 2 * R2STAGES + 4));
+    constexpr int kEpiWarps = 16, kProdWarps = 4, kEpiRows = TBN * 4 / kEpiWarps, RB = 8;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const bool leader = rank == 0;
+    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    const int col_pairs = (g.N + 2 * TBM - 1) / (2 * TBM);
+    const int row_blocks = g.M / TBN;
+    const int num_tiles = row_blocks * col_pairs;
+    const int nk = g.K / TBK;
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tm_hi);
+        tma_prefetch_desc(&tm_lo);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < WSTAGES; ++s) { mbar_init(bar_wfull(s), 1); mbar_init(bar_wempty(s), 1); }
+        for (int s = 0; s < R2STAGES; ++s) { mbar_init(bar_rfull(s), 2 * kProdWarps); mbar_init(bar_rempty(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(bar_tfull(a), 1); mbar_init(bar_tempty(a), 2 * kEpiWarps); }
+        fence_barrier_init();
+    }
+    if (warp == 2) tmem_alloc_pair(smem_u32(tmem_slot), TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    // register pool of the CTA: 768 x 80 = 61 440 = 128 x 40 (control) + 512 x 72 (epilogue) + 128 x 152 (producers)
+    if (warp < 4) reg_dec<40>();
+    if (warp == 0) {
+        int stage = 0; uint32_t phase = 0;
+        for (int tile = pair; tile < num_tiles; tile += npairs) {
+            const PairGeo t = pair_geo(g, tile, col_pairs, (int)rank);
+            for (int kt = 0; kt < nk; ++kt) {
+                mbar_wait<32>(bar_wempty(stage), phase ^ 1);
+                if (lane == 0) {
+                    if (leader) mbar_arrive_expect_tx(bar_wfull(stage), 4 * W_TILE_BYTES);
+                    tma_load_2d_pair(sW(stage, 0), &tm_hi, kt * TBK, t.n0, bar_wfull(stage));
+                    tma_load_2d_pair(sW(stage, 1), &tm_lo, kt * TBK, t.n0, bar_wfull(stage));
+                }
+                __syncwarp();
+                if (++stage == WSTAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 1) {
+        if (leader) {
+            int ws = 0, rs = 0; uint32_t wphase = 0, rphase = 0;
+            const uint32_t idesc = make_idesc(2 * TBM, TBN);
+            const uint64_t dW0 = make_smem_desc(sW(0, 0)), dR0 = make_smem_desc(sR(0, 0));
+            int tcount = 0;
+            for (int tile = pair; tile < num_tiles; tile += npairs, ++tcount) {
+                const int acc = tcount & 1;
+                mbar_wait(bar_tempty(acc), ((tcount >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_main = tmem_base + acc * TBN;
+                for (int kt = 0; kt < nk; ++kt) {
+                    mbar_wait(bar_wfull(ws), wphase);
+                    mbar_wait(bar_rfull(rs), rphase);
+                    tc_fence_after();
+                    const uint64_t whi = dW0 + (uint64_t)((2 * ws * W_TILE_BYTES) >> 4), wlo = whi + (W_TILE_BYTES >> 4);
+                    const uint64_t rhi = dR0 + (uint64_t)((2 * rs * R2_TILE_BYTES) >> 4), rlo = rhi + (R2_TILE_BYTES >> 4);
+                    if (lane == 0) {
+#pragma unroll
+                        for (int k = 0; k < TBK / 8; ++k) {
+                            const uint64_t ko = (uint64_t)(k * 32 >> 4);
+                            umma_tf32_pair(d_main, whi + ko, rlo + ko, idesc, (kt | k) != 0);
+                            umma_tf32_pair(d_main, wlo + ko, rhi + ko, idesc, 1u);
+                            umma_tf32_pair(d_main, whi + ko, rhi + ko, idesc, 1u);
+                        }
+                        umma_commit_pair(bar_wempty(ws));
+                        umma_commit_pair(bar_rempty(rs));
+                        if (kt == nk - 1) umma_commit_pair(bar_tfull(acc));
+                    }
+                    __syncwarp();
+                    if (++ws == WSTAGES) { ws = 0; wphase ^= 1; }
+                    if (++rs == R2STAGES) { rs = 0; rphase ^= 1; }
+                }
+            }
+        }
+    } else if (warp >= 4 && warp < 4 + kEpiWarps) {
+        reg_dec<72>();
+        const int q = warp & 3;
+        const uint32_t t_lane = tmem_base + ((uint32_t)(q * 32) << 16);
+        const int c_lo = ((warp - 4) >> 2) * kEpiRows, c_hi = c_lo + kEpiRows;
+        int tcount = 0;
+        for (int tile = pair; tile < num_tiles; tile += npairs, ++tcount) {
+            const PairGeo t = pair_geo(g, tile, col_pairs, (int)rank);
+            const int n = t.n0 + q * 32 + lane;
+            const bool n_ok = n < g.N;
+            const int acc = tcount & 1;
+            const uint32_t tempty = bar_tempty(acc);
+            bwd_epilogue_tile<RB, kEpiRows>(g, t.r0, t.rbase, t.po, n, n_ok, lane, t_lane + acc * TBN, c_lo, c_hi, bar_tfull(acc),
+                                            (uint32_t)((tcount >> 1) & 1), [&]() {
+                                                __syncwarp();
+                                                if (lane == 0) { if (leader) mbar_arrive(tempty); else mbar_arrive_remote(tempty, 0); }
+                                            });
+        }
+    } else if (warp >= 4 + kEpiWarps) {
+        // ===================== row producers: this CTA's 128 rows, 8 rows per thread, split only =====================
+        reg_inc<152>();
+        const int pw = warp - (4 + kEpiWarps);
+        const int r4 = lane >> 3, c4 = lane & 7;
+        const float4* const A4 = reinterpret_cast<const float4*>(g.A);
+        const uint32_t rstride = (uint32_t)(g.lda >> 2) * 4u;
+        const int rofs = (int)rank * HROWS;
+        int ltile = pair, lkt = 0;
+        bool lhave = ltile < num_tiles;
+        uint32_t lbase = 0;
+        auto set_base = [&]() { lbase = (uint32_t)(((size_t)(ltile / col_pairs * TBN + rofs + pw * 32 + r4) * g.lda) >> 2) + c4; };
+        auto issue = [&](float4* buf) {
+            if (!lhave) return;
+            const float4* src = A4 + lbase + (uint32_t)lkt * (TBK / 4);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) buf[i] = __ldg(src + (size_t)i * rstride);
+            if (++lkt == nk) {
+                lkt = 0;
+                ltile += npairs;
+                lhave = ltile < num_tiles;
+                if (lhave) set_base();
+            }
+        };
+        int stage = 0; uint32_t phase = 0;
+        long long remaining = 0;
+        for (int tile = pair; tile < num_tiles; tile += npairs) remaining += nk;
+        auto put = [&](const float4* buf) {
+            mbar_wait(bar_rempty(stage), phase ^ 1);
+            const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float4 v = buf[i];
+                float4 hi, lo;
+                hi.x = to_tf32(v.x); hi.y = to_tf32(v.y); hi.z = to_tf32(v.z); hi.w = to_tf32(v.w);
+                lo.x = v.x - hi.x; lo.y = v.y - hi.y; lo.z = v.z - hi.z; lo.w = v.w - hi.w;
+                const int row = pw * 32 + i * 4 + r4;
+                const uint32_t off = (uint32_t)row * 128u + (uint32_t)((c4 ^ (row & 7)) << 4);
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_hi + off), "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(r_lo + off), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w) : "memory");
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) { if (leader) mbar_arrive(bar_rfull(stage)); else mbar_arrive_remote(bar_rfull(stage), 0); }
+            if (++stage == R2STAGES) { stage = 0; phase ^= 1; }
+        };
+        if (lhave) {
+            float4 b0[8], b1[8], b2[8];
+            set_base();
+            issue(b0);
+            issue(b1);
+            while (true) {
+                issue(b2); put(b0); if (--remaining == 0) break;
+                issue(b0); put(b1); if (--remaining == 0) break;
+                issue(b1); put(b2); if (--remaining == 0) break;
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc_pair(tmem_base, TMEM_COLS);
+    }
+}
+
+inline cudaError_t launch_chain_gemm_tc2_bwd(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(chain_gemm_tc2_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2B_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
+    const int tiles = (g.M / TBN) * ((g.N + 2 * TBM - 1) / (2 * TBM));
+    int grid = 2 * tiles < num_sms ? 2 * tiles : (num_sms & ~1);
+    chain_gemm_tc2_bwd_kernel<<<grid, THREADS_BWD, SMEM2B_BYTES, st>>>(g, hi, lo);
+    return cudaGetLastError();
+}
+
 // g.M (coefficient rows) must be a multiple of 256, g.K a multiple of 32
 inline cudaError_t launch_chain_gemm_tc2_fwd(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
     static bool attr_done = false;
