@@ -295,6 +295,8 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
         // ===================== row producers: this CTA's 128 rows of the block, 4 rows per thread =====================
         reg_inc<184>();
         const int pw = warp - 8;                   // warp pw owns local rows [pw*16, pw*16 + 16)
+        // a thread owns 4 CONSECUTIVE rows (pw*16 + r4*4 + i): when the chain boundaries are multiples of 4 (n = 168, 20, ...)
+        // its rows all lie on one chain and it takes the selection-free path even in blocks that mix chains
         const int r4 = lane >> 3, c4 = lane & 7;
         const float4* const A4 = reinterpret_cast<const float4*>(g.A);
         const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -308,7 +310,7 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
             lkinds = 0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                const int j = rofs + pw * 16 + i * 4 + r4;
+                const int j = rofs + pw * 16 + r4 * 4 + i;
                 const int rin = t.rbase + j;
                 int kind = rin / g.rows_kind;
                 int rk = rin - kind * g.rows_kind;
@@ -380,15 +382,17 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
             if (++ps == PSTAGES) { ps = 0; pphase ^= 1; }
             mbar_wait(bar_rempty(stage), phase ^ 1);
             const uint32_t r_hi = sR(stage, 0), r_lo = sR(stage, 1);
-            if (kP == 0u || kP == 0x55u) {
-                const float4 kp = kP == 0u ? kUc : kLc, kn = kP == 0u ? kLc : kUc;
-                const float4 gp = kP == 0u ? gU4 : gL4, gn = kP == 0u ? gL4 : gU4;
+            if (kP == 0u || kP == 0x55u || kP == 0xAAu || kP == 0xFFu) {
+                // all four rows of this thread on one chain (upper / lower / Jacobian; padding rows are zero anyway)
+                const bool jac = kP >= 0xAAu;
+                const float4 kp = kP == 0u ? kUc : (jac ? dpc : kLc), kn = kP == 0u ? kLc : (jac ? dpc : kUc);
+                const float4 gp = kP == 0u ? gU4 : (jac ? zero4 : gL4), gn = kP == 0u ? gL4 : (jac ? zero4 : gU4);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
                     float4 v = P[i];
                     if (do_gap) gsum[i] += gap4(v, gp, gn);
                     relax4(v, kp, kn);
-                    split_store(v, r_hi, r_lo, pw * 16 + i * 4 + r4);
+                    split_store(v, r_hi, r_lo, pw * 16 + r4 * 4 + i);
                 }
             } else {
 #pragma unroll
@@ -401,7 +405,7 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
                     } else if (kind == 2u) {
                         relax4(v, dpc, dpc);
                     }
-                    split_store(v, r_hi, r_lo, pw * 16 + i * 4 + r4);
+                    split_store(v, r_hi, r_lo, pw * 16 + r4 * 4 + i);
                 }
             }
             // generic-proxy stores -> visible to the tensor core of the LEADER's SM (async proxy), then the hand-over
@@ -422,7 +426,7 @@ chain_gemm_tc2_fwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
                         s += __shfl_xor_sync(0xffffffffu, s, 1);
                         s += __shfl_xor_sync(0xffffffffu, s, 2);
                         s += __shfl_xor_sync(0xffffffffu, s, 4);
-                        const int m = t_cur.r0 + rofs + pw * 16 + i * 4 + r4;
+                        const int m = t_cur.r0 + rofs + pw * 16 + r4 * 4 + i;
                         if (c4 == 0) g.gap[m] = (g.gap_init ? 0.f : g.gap[m]) + s;
                     }
                 }
