@@ -146,6 +146,14 @@ def test_certified_edge_cases(mods):
     lo, hi = ctx.leb_nn_fwd(_dev(n2), rad, flags=0)
     assert ctx.leb_domain_flag() == 1
     assert bool(torch.isinf(lo[1, 0]).all()) and bool(torch.isinf(hi[1, 0]).all()) and bool(torch.isfinite(lo[0]).all())
+    # layers wider than 2048 (padded): the norm / sum inflation factors of the certificate are derived for K <= 2048
+    wide = wl.make_small_mlp([4, 2100, 3], 1, 1, 1)
+    cw = leb.context_for_workload(wide)
+    with pytest.raises(leb.LebError) as e:
+        cw.leb_nn_fwd(_dev(wide.nom), _dev(wide.rad), flags=0)
+    assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+    cw.leb_nn_fwd(_dev(wide.nom), _dev(wide.rad), flags=leb.FLAG_NO_MARGIN)      # value mode has no such limit
+    cw.close()
     # the VJP is that of the value-mode bound whichever mode is asked for
     g1 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=0)
     g2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN)
