@@ -514,7 +514,7 @@ chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    // register pool of the CTA: 768 x 80 = 61 440 = 128 x 40 (control) + 512 x 72 (epilogue) + 128 x 152 (producers)
+    // register pool of the CTA: 768 x 80 = 61 440 >= 128 x 40 (control) + 512 x 80 (epilogue) + 128 x 120 (producers)
     if (warp < 4) reg_dec<40>();
     if (warp == 0) {
         int stage = 0; uint32_t phase = 0;
@@ -567,7 +567,7 @@ chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
             }
         }
     } else if (warp >= 4 && warp < 4 + kEpiWarps) {
-        reg_dec<72>();
+        reg_dec<80>();                              // (keeps its 80 registers; without the statement ptxas spills 770 bytes here)
         const int q = warp & 3;
         const uint32_t t_lane = tmem_base + ((uint32_t)(q * 32) << 16);
         const int c_lo = ((warp - 4) >> 2) * kEpiRows, c_hi = c_lo + kEpiRows;
@@ -586,7 +586,7 @@ chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
         }
     } else if (warp >= 4 + kEpiWarps) {
         // ===================== row producers: this CTA's 128 rows, 8 rows per thread, split only =====================
-        reg_inc<152>();
+        reg_inc<120>();
         const int pw = warp - (4 + kEpiWarps);
         const int r4 = lane >> 3, c4 = lane & 7;
         const float4* const A4 = reinterpret_cast<const float4*>(g.A);
@@ -631,14 +631,12 @@ chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
             if (++stage == R2STAGES) { stage = 0; phase ^= 1; }
         };
         if (lhave) {
-            float4 b0[8], b1[8], b2[8];
+            float4 b0[8], b1[8];
             set_base();
             issue(b0);
-            issue(b1);
             while (true) {
-                issue(b2); put(b0); if (--remaining == 0) break;
+                issue(b1); put(b0); if (--remaining == 0) break;
                 issue(b0); put(b1); if (--remaining == 0) break;
-                issue(b1); put(b2); if (--remaining == 0) break;
             }
         }
     }
