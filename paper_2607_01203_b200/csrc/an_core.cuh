@@ -397,6 +397,14 @@ LEB_HD int window_vars(const Model& M, int i, int* vars /* >= 54 */) {
     return L;
 }
 
+// off-diagonal item t in [0, L(L-1)/2) -> positions (a < b), row-major over a
+LEB_HD void item_decode_offdiag(int t, int L, int* a, int* b) {
+    int row = 0, rem = t;
+    while (rem >= L - 1 - row) { rem -= L - 1 - row; ++row; }
+    *a = row;
+    *b = row + 1 + rem;
+}
+
 // item t in [0, L(L+1)/2) -> positions (a <= b) in the window list, row-major over a
 LEB_HD void item_decode(int t, int L, int* a, int* b) {
     int row = 0, rem = t;

@@ -126,6 +126,7 @@ analytic_vjp_kernel(Model M, const float* __restrict__ nom, const float* __restr
     __shared__ int nvars;
     __shared__ float gl_s[NOUT], gh_s[NOUT];
     __shared__ float grad_s[2 * kMaxVars];
+    __shared__ int rad_off[kMaxVars + 1];      // prefix counts of the radius work units per item row a
 
     const int tile = blockIdx.y, unit = blockIdx.x;
     bool bad = load_tile(nom + (size_t)tile * ld_in, rad + (size_t)tile * ld_in, M.N, nom_s, rad_s);
@@ -141,17 +142,41 @@ analytic_vjp_kernel(Model M, const float* __restrict__ nom, const float* __restr
     for (int d = threadIdx.x; d < 2 * kMaxVars; d += blockDim.x) grad_s[d] = 0.f;
     __syncthreads();
     const int L = nvars, nitems = L * (L + 1) / 2, ndirs = 2 * L;
+    // Work units.  Every item (a <= b) needs all L nominal directions.  A RADIUS direction p matters only if the box of the
+    // item depends on sigma_p -- positions p <= a of the prefix box A^(j) (Thm 1: coordinates after j are pinned at the
+    // nominal point, L162) -- or if sigma_p is one of the explicit factors (p == b; p == a is already counted): for every
+    // other p the tangent is identically zero, so those (item, direction) pairs are not enumerated at all
+    // (L = 54: 109 341 units instead of 160 380).  Row a of the item table has L - a items, each with a + 1 box directions.
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int a = 0; a < L; ++a) { rad_off[a] = acc; acc += (L - a) * (a + 1); }
+        rad_off[L] = acc;
+    }
+    __syncthreads();
+    const int n_nom = nitems * L, n_box = rad_off[L], n_fac = nitems - L;      // n_fac: off-diagonal items, direction p == b
     bool dom = false;
     if (!bad) {
-        const int nwork = nitems * ndirs;
+        const int nwork = n_nom + n_box + n_fac;
         for (int w = threadIdx.x; w < nwork; w += blockDim.x) {
-            int t = w / ndirs, d = w - t * ndirs;
-            int a, b;
-            item_decode(t, L, &a, &b);
+            int a, b, d;                       // item (a, b) and direction d in [0, 2L): nominal d, radius L + position
+            if (w < n_nom) {
+                const int t = w / L;
+                d = w - t * L;
+                item_decode(t, L, &a, &b);
+            } else if (w < n_nom + n_box) {
+                const int r = w - n_nom;
+                int lo = 0, hi = L - 1;        // largest a with rad_off[a] <= r
+                while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (rad_off[mid] <= r) lo = mid; else hi = mid - 1; }
+                a = lo;
+                const int rem = r - rad_off[a], p = rem / (L - a);
+                b = a + (rem - p * (L - a));
+                d = L + p;
+            } else {
+                item_decode_offdiag(w - n_nom - n_box, L, &a, &b);
+                d = L + b;
+            }
             const int j = vars[a], k = vars[b];
             const int dvar = vars[d < L ? d : d - L];
-            // a tangent on a coordinate outside {<= k} cannot reach item (j,k)'s box or seeds only if
-            // the coordinate is not an input of the cone at all; every window variable is, so no skip.
             Inputs<Du> in{DuArr{nom_s, d < L ? dvar : -1}, DuArr{rad_s, d < L ? -1 : dvar}, j, k};
             Jet<Du> f[NOUT];
             if (UNICYCLE) unicycle_f(M, in, f);
