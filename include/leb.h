@@ -97,11 +97,16 @@ enum {
     LEB_FLAG_HOST_IO = 4u,   /* data pointers of this call are host pointers */
     LEB_FLAG_SINGLE_CTA = 16u, /* NN: forward chain steps on single CTAs (nn_gemm_tc.cuh) instead of CTA pairs
                                   (tcgen05.mma.cta_group::2, nn_gemm_tc2.cuh, the default); same results bit for bit */
-    LEB_FLAG_REUSE_FWD = 8u  /* leb_vjp(kind 1): the caller states that (nom, rad) are those of the previous leb_nn_fwd
-                                call on this context (J == NULL); if the workspace still holds that call's complete
-                                forward state (the batch fitted one chunk) the reverse sweep starts from it instead of
-                                recomputing the forward, otherwise the flag has no effect.  The gradient is then that
-                                of the bound leb_nn_fwd returned (certified mode: its pads held constant). */
+    LEB_FLAG_REUSE_FWD = 8u  /* leb_vjp(kind 1) becomes STATEFUL: the caller states that (nom, rad) are those of the previous
+                                leb_nn_fwd call on this context (J == NULL).  If the workspace still holds that call's complete
+                                forward state (the batch fitted one chunk) AND that state was computed in the mode this
+                                leb_vjp call names (LEB_FLAG_NO_MARGIN set: a value-mode forward; clear: a certified one), the
+                                reverse sweep starts from it instead of recomputing the forward.  Otherwise the flag has no
+                                effect: the call recomputes a value-mode forward, exactly as the stateless call does.
+                                leb_nn_state() reports which of the two happened.  Reverse sweep over a CERTIFIED state: the
+                                derivative of the value-mode formulas evaluated on the certified forward's (widened) hidden
+                                bounds and padded gaps, i.e. the gradient of the certified bound with its rounding pads and
+                                outward-rounding factors (<= 3e-4 relative) treated as constants. */
 };
 
 leb_status leb_create(leb_ctx** ctx, int device);
@@ -141,8 +146,11 @@ leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float*
                       float* margin, int ld_out, unsigned flags, void* stream);
 
 /* VJP of the bounds: grad = d/d(a~, sigma) sum_i g_hi[i] r_hi[i] + g_lo[i] r_lo[i], per tile
- * (block-diagonal over tiles).  Recomputes the forward pass internally (stateless).  kind 1: always the VJP of
- * the value-mode bound -- the certified margin is a rounding-level pad and is treated as a constant.
+ * (block-diagonal over tiles).  Stateless by default: the forward pass is recomputed internally, and for kind 1 it
+ * is recomputed in value mode whatever the flags say -- the certified margin is a rounding-level pad and is treated
+ * as a constant.  The one stateful variant is LEB_FLAG_REUSE_FWD (see the flag).
+ * Reproducibility: both kinds reduce in a fixed order except the NN reverse sweep's column sums (FP32 atomicAdd, one
+ * per column and row block), so kind-1 gradients repeat to ~1e-6 relative, kind-0 gradients bit for bit.
  *   kind: 0 analytic (model from leb_set_analytic), 1 NN (model from leb_set_mlp)
  *   g_lo, g_hi       : [B, T, ld_out] cotangents
  *   grad_nom,grad_rad: [B, T, ld_in] outputs (columns >= N are left untouched).
@@ -183,6 +191,12 @@ leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, voi
  * dims[target]; index 0 = upper chain, 1 = lower chain.  Used to measure the contraction's rounding error
  * against the model behind the certified margin. */
 leb_status leb_nn_chain_coeffs(leb_ctx* ctx, int target, float* out, void* stream);
+
+/* State of the NN workspace (host-side query, no synchronisation): *tiles = number of tiles whose complete forward
+ * state the last leb_nn_fwd / leb_vjp left resident (0: none, e.g. the batch was processed in chunks); *certified =
+ * 1 if that state is a certified-mode one; *vjp_reused = 1 if the last leb_vjp(kind 1) call started from the
+ * resident state (LEB_FLAG_REUSE_FWD honoured), 0 if it recomputed the forward. */
+leb_status leb_nn_state(leb_ctx* ctx, int* tiles, int* certified, int* vjp_reused);
 
 /* Number of kernel launches the library has enqueued on this context so far. */
 long long leb_launch_count(const leb_ctx* ctx);

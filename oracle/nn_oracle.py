@@ -423,11 +423,12 @@ def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
     return ties
 
 
-def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None, flips=()):
-    """Returns (grad_nom, grad_rad) for one tile.  `flips`: entries (chain, i, j) from
+def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=()):
+    """Returns (grad_nom, grad_rad) for one tile; J is the network's own Jacobian at a~ (the
+    product's leb_vjp takes no J argument).  `flips`: entries (chain, i, j) from
     output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink)."""
     L = len(Ws)
-    fw = crown_forward(Ws, bs, act, a0, sig, J_given, keep=True)
+    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True)
     relaxs, ls, us, zs, J = fw["relaxs"], fw["ls"], fw["us"], fw["zs"], fw["J"]
     a_bar = np.zeros_like(a0)
     s_bar = np.zeros_like(sig)
@@ -451,19 +452,17 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, J_given=None, flips=()):
     # ---- J_bar and p_bar back through the nominal network
     #   J = G_l diag(phi'(z_l)) W_l F_{l-1},  G_l = dp/da_l,  F_l = da_l/da
     abar_l = Ws[L - 1].T @ pbar                 # adjoint of a_{L-1}
-    if J_given is None:
-        F = [np.eye(a0.shape[0])]
-        for l in range(1, L):
-            F.append((dphi(act, zs[l - 1])[:, None] * Ws[l - 1]) @ F[l - 1])
-        G = {L - 1: Ws[L - 1]}
-        for l in range(L - 2, 0, -1):
-            G[l] = (G[l + 1] * dphi(act, zs[l])[None, :]) @ Ws[l]
+    F = [np.eye(a0.shape[0])]
+    for l in range(1, L):
+        F.append((dphi(act, zs[l - 1])[:, None] * Ws[l - 1]) @ F[l - 1])
+    G = {L - 1: Ws[L - 1]}
+    for l in range(L - 2, 0, -1):
+        G[l] = (G[l + 1] * dphi(act, zs[l])[None, :]) @ Ws[l]
     for l in range(L - 1, 0, -1):
         zbar = dphi(act, zs[l - 1]) * abar_l
-        if J_given is None:
-            WF = Ws[l - 1] @ F[l - 1]                       # [w_l, N]
-            q = np.einsum("ik,ij,kj->k", G[l], Jbar, WF)    # diag(G^T Jbar WF^T)
-            zbar = zbar + d2phi(act, zs[l - 1]) * q
+        WF = Ws[l - 1] @ F[l - 1]                       # [w_l, N]
+        q = np.einsum("ik,ij,kj->k", G[l], Jbar, WF)    # diag(G^T Jbar WF^T)
+        zbar = zbar + d2phi(act, zs[l - 1]) * q
         abar_l = Ws[l - 1].T @ zbar
     a_bar += abar_l
 

@@ -308,6 +308,13 @@ leb_status leb_nn_chain_coeffs(leb_ctx* c, int target, float* out, void* stream)
     return leb_nn_get_coeffs(c->nn, target, out, (cudaStream_t)stream, &c->launches);
 }
 
+leb_status leb_nn_state(leb_ctx* c, int* tiles, int* certified, int* vjp_reused) {
+    if (!c || !tiles || !certified || !vjp_reused) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    leb_nn_query(c->nn, tiles, certified, vjp_reused);
+    return LEB_OK;
+}
+
 long long leb_launch_count(const leb_ctx* c) { return c ? c->launches : 0; }
 
 leb_status leb_profile(leb_ctx* c, int enable) {

@@ -71,6 +71,8 @@ struct NnState {
     float *Lbar[2] = {nullptr, nullptr}, *gapbar = nullptr, *nom_bar = nullptr, *rad_bar = nullptr, *glo_p = nullptr, *ghi_p = nullptr;
     int last_tiles = 0;          // > 0: the workspace holds the complete forward state of that many tiles (one chunk)
     bool last_with_jac = false;  // ... including the Jacobian chain rows (needed by the reverse sweep)
+    bool last_cert = false;      // ... computed in certified mode (widened hidden bounds, padded gaps)
+    bool last_vjp_reused = false;   // the last leb_vjp(kind 1) started from the resident forward state
     LebProf* prof = nullptr;
 };
 
@@ -898,9 +900,16 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         ++*launches;
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
         S->last_with_jac = (J == nullptr);
+        S->last_cert = cert;
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+void leb_nn_query(const NnState* S, int* tiles, int* certified, int* vjp_reused) {
+    *tiles = S->last_tiles > 0 ? S->last_tiles : 0;
+    *certified = (S->last_tiles > 0 && S->last_cert) ? 1 : 0;
+    *vjp_reused = S->last_vjp_reused ? 1 : 0;
 }
 
 leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStream_t st, long long* launches) {
@@ -936,7 +945,11 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     const int L = S->L, n = S->w[L], N = S->w[0], wp0 = S->wp[0];
     // LEB_FLAG_REUSE_FWD: the caller states that (nom, rad) are those of the previous leb_nn_fwd call on this context; if the
     // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
-    const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk;
+    // and was computed in the mode this call names (LEB_FLAG_NO_MARGIN: a value-mode state; otherwise a certified one).
+    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN);
+    const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
+                       S->last_cert == want_cert;
+    S->last_vjp_reused = reuse;
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
         if (!reuse)
@@ -1024,7 +1037,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,
                                                                  grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in);
         ++*launches;
-        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; }   // a value-mode forward state
+        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;

@@ -28,6 +28,7 @@
 // tmem_full (tcgen05.commit), tmem_empty (epilogue arrivals).
 // The forward step normally runs on CTA pairs instead (nn_gemm_tc2.cuh); this file's forward is LEB_FLAG_SINGLE_CTA.
 #pragma once
+#include <atomic>
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -892,11 +893,15 @@ inline bool make_weight_map(CUtensorMap* map, const float* dptr, int rows, int c
 // g.M (coefficient rows) must be a multiple of 256, g.K and g.N multiples of 32
 template <int MODE>
 inline cudaError_t launch_chain_gemm_tc(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the attribute is per device: one bit per device ordinal (a context may live on any GPU of the process)
+    static std::atomic<unsigned long long> attr_done{0ull};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & bit)) {
         cudaError_t e = cudaFuncSetAttribute(chain_gemm_tc_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done.fetch_or(bit, std::memory_order_release);
     }
     if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
     const int tiles = (g.M / TBN) * ((g.N + TBM - 1) / TBM);

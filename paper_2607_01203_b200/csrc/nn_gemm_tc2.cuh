@@ -20,6 +20,7 @@
 //   wempty[s], rempty[s], tfull  exist in BOTH CTAs and are signalled together by the leader's
 //                                tcgen05.commit.cta_group::2 ... .multicast::cluster (mask 0b11)
 #pragma once
+#include <atomic>
 #include "nn_gemm_tc.cuh"
 
 namespace leb_nn {
@@ -651,11 +652,15 @@ chain_gemm_tc2_bwd_kernel(const GemmArgs g, const __grid_constant__ CUtensorMap 
 }
 
 inline cudaError_t launch_chain_gemm_tc2_bwd(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the attribute is per device: one bit per device ordinal (a context may live on any GPU of the process)
+    static std::atomic<unsigned long long> attr_done{0ull};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & bit)) {
         cudaError_t e = cudaFuncSetAttribute(chain_gemm_tc2_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2B_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done.fetch_or(bit, std::memory_order_release);
     }
     if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
     const int tiles = (g.M / TBN) * ((g.N + 2 * TBM - 1) / (2 * TBM));
@@ -666,11 +671,15 @@ inline cudaError_t launch_chain_gemm_tc2_bwd(const GemmArgs& g, const CUtensorMa
 
 // g.M (coefficient rows) must be a multiple of 256, g.K a multiple of 32
 inline cudaError_t launch_chain_gemm_tc2_fwd(const GemmArgs& g, const CUtensorMap& hi, const CUtensorMap& lo, int num_sms, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the attribute is per device: one bit per device ordinal (a context may live on any GPU of the process)
+    static std::atomic<unsigned long long> attr_done{0ull};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & bit)) {
         cudaError_t e = cudaFuncSetAttribute(chain_gemm_tc2_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        attr_done.fetch_or(bit, std::memory_order_release);
     }
     if (g.M % TBN != 0 || g.K % TBK != 0) return cudaErrorInvalidValue;
     const int tiles = (g.M / TBN) * ((g.N + 2 * TBM - 1) / (2 * TBM));

@@ -27,7 +27,7 @@ FLAG_SINGLE_CTA = 16
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
 
@@ -176,7 +176,9 @@ class Context:
                                        int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_fwd")
         return r_lo, r_hi
 
-    def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = FLAG_NO_MARGIN):
+    def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = 0):
+        """flags = 0 is the C ABI's default: CERTIFIED mode (rounding errors bounded and added outward).
+        FLAG_NO_MARGIN selects value mode, the plain FP32 result the parity tests compare with the oracle."""
         _check_f32(nom, rad, J, r_lo, r_hi, margin)
         B, T, ld_in = self._bt(nom)
         host = bool(flags & FLAG_HOST_IO)
@@ -187,7 +189,7 @@ class Context:
                                  _ptr(margin), int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_nn_fwd")
         return r_lo, r_hi
 
-    def leb_vjp(self, kind: int, nom, rad, g_lo, g_hi, grad_nom=None, grad_rad=None, flags: int = FLAG_NO_MARGIN):
+    def leb_vjp(self, kind: int, nom, rad, g_lo, g_hi, grad_nom=None, grad_rad=None, flags: int = 0):
         _check_f32(nom, rad, g_lo, g_hi, grad_nom, grad_rad)
         B, T, ld_in = self._bt(nom)
         host = bool(flags & FLAG_HOST_IO)
@@ -241,6 +243,12 @@ class Context:
         out = torch.empty((tiles, 2, rows, N), dtype=torch.float32, device=torch.device("cuda", self.device))
         _chk(self.lib.leb_nn_chain_coeffs(self._ctx, int(target), _ptr(out), _stream_ptr(self.device)), "leb_nn_chain_coeffs")
         return out
+
+    def leb_nn_state(self):
+        """(resident tiles, certified?, last leb_vjp reused the resident forward state?)"""
+        t, c, r = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0)
+        _chk(self.lib.leb_nn_state(self._ctx, ctypes.byref(t), ctypes.byref(c), ctypes.byref(r)), "leb_nn_state")
+        return int(t.value), bool(c.value), bool(r.value)
 
     def leb_launch_count(self) -> int:
         return int(self.lib.leb_launch_count(self._ctx))

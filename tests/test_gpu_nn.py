@@ -28,6 +28,7 @@ def _flat(w):
 
 
 # both contraction paths: 3xTF32 tcgen05 (default) and FP32 FFMA (LEB_FLAG_FFMA_ONLY); value mode in both
+VAL = 1      # LEB_FLAG_NO_MARGIN: value mode, the mode compared with the oracle (the binding's default is certified)
 PATHS = {"tc": 1, "tc_single_cta": 1 | 16, "ffma": 1 | 2}
 
 
@@ -162,7 +163,7 @@ def test_fwd_never_below_sampled_maximum_and_exact_range(mods):
     for dims, act, seed in (([3, 12, 2], 1, 1), ([4, 10, 3], 1, 2), ([4, 8, 8, 2], 2, 3), ([2, 16, 16, 2], 1, 4)):
         w = wl.make_small_mlp(dims, act, 2, 2, seed=seed, rad_lo=0.05, rad_hi=0.4)
         ctx = leb.context_for_workload(w)
-        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad))
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=VAL)
         glo, ghi = to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n)
         Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
         rng = np.random.default_rng(seed)
@@ -190,7 +191,7 @@ def test_given_jacobian(mods):
     ctx = leb.context_for_workload(w)
     rng = np.random.default_rng(9)
     J = rng.standard_normal((w.B, w.T, w.n, w.N)).astype(np.float32) * 0.3
-    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J))
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J), flags=VAL)
     nom, rad, _, _ = _flat(w)
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom, rad, J=J.reshape(-1, w.n, w.N))
     # with an arbitrary J the bound is O(|W - J| sigma), computed from O(1) coefficients: tolerance
@@ -206,54 +207,57 @@ def test_edge_cases(mods):
     ctx = leb.context_for_workload(w)
     nom, rad = _dev(w.nom), _dev(w.rad)
     # empty batch
-    lo, hi = ctx.leb_nn_fwd(nom[:0], rad[:0])
+    lo, hi = ctx.leb_nn_fwd(nom[:0], rad[:0], flags=VAL)
     assert lo.shape == (0, 3, 4)
     # zero radius: ReLU bound exactly 0 when no nominal pre-activation is exactly 0
-    lo, hi = ctx.leb_nn_fwd(nom, torch.zeros_like(rad))
+    lo, hi = ctx.leb_nn_fwd(nom, torch.zeros_like(rad), flags=VAL)
     assert float(lo.abs().max()) == 0.0 and float(hi.abs().max()) == 0.0
     # padded leading dimensions
     nomp = torch.zeros(2, 3, 8, device="cuda"); nomp[..., :6] = nom
     radp = torch.zeros(2, 3, 8, device="cuda"); radp[..., :6] = rad
     lop = torch.full((2, 3, 8), 7.0, device="cuda"); hip = torch.full((2, 3, 8), 7.0, device="cuda")
-    ctx.leb_nn_fwd(nomp, radp, r_lo=lop, r_hi=hip)
-    lo, hi = ctx.leb_nn_fwd(nom, rad)
+    ctx.leb_nn_fwd(nomp, radp, r_lo=lop, r_hi=hip, flags=VAL)
+    lo, hi = ctx.leb_nn_fwd(nom, rad, flags=VAL)
     assert torch.equal(lop[..., :4], lo) and torch.equal(hip[..., :4], hi) and float((lop[..., 4:] - 7).abs().max()) == 0.0
     # LEB_FLAG_REUSE_FWD: same gradient; no effect when the forward state is not there (other batch, chunked batch)
-    ctx.leb_nn_fwd(nom, rad)
+    ctx.leb_nn_fwd(nom, rad, flags=VAL)
     gA = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
-    gB = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    assert ctx.leb_nn_state() == (w.B * w.T, False, True)
+    gB = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=VAL)
+    assert ctx.leb_nn_state()[2] is False
     assert torch.allclose(gA[0], gB[0], rtol=1e-5, atol=1e-7) and torch.allclose(gA[1], gB[1], rtol=1e-5, atol=1e-7)
-    ctx.leb_nn_fwd(nom[:1], rad[:1])
+    ctx.leb_nn_fwd(nom[:1], rad[:1], flags=VAL)
     gC = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state()[2] is False                    # another batch is resident: recomputed
     assert torch.allclose(gC[0], gB[0], rtol=1e-5, atol=1e-7) and torch.allclose(gC[1], gB[1], rtol=1e-5, atol=1e-7)
     # chunking does not change results
     ctx.leb_set_nn_chunk(4)
-    lo2, hi2 = ctx.leb_nn_fwd(nom, rad)
+    lo2, hi2 = ctx.leb_nn_fwd(nom, rad, flags=VAL)
     gn2, gr2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
     ctx.leb_set_nn_chunk(0)
-    gn, gr = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi))
+    gn, gr = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=VAL)
     assert torch.equal(lo2, lo) and torch.equal(hi2, hi)
     assert torch.allclose(gn2, gn, rtol=1e-5, atol=1e-7) and torch.allclose(gr2, gr, rtol=1e-5, atol=1e-7)
     # NaN input / negative radius poison only their tile and raise the flag
     assert ctx.leb_domain_flag() == 0
     n2 = w.nom.copy(); n2[1, 0, 2] = np.nan
-    lo, hi = ctx.leb_nn_fwd(_dev(n2), rad)
+    lo, hi = ctx.leb_nn_fwd(_dev(n2), rad, flags=VAL)
     assert ctx.leb_domain_flag() == 1
     assert bool(torch.isinf(lo[1, 0]).all()) and bool(torch.isinf(hi[1, 0]).all()) and bool(torch.isfinite(lo[0]).all())
     r2 = w.rad.copy(); r2[0, 2, 5] = -0.1
-    lo, hi = ctx.leb_nn_fwd(nom, _dev(r2))
+    lo, hi = ctx.leb_nn_fwd(nom, _dev(r2), flags=VAL)
     assert ctx.leb_domain_flag() == 1 and bool(torch.isinf(hi[0, 2]).all()) and bool(torch.isfinite(hi[1]).all())
     # host IO
     hlo, hhi = ctx.leb_nn_fwd(torch.from_numpy(w.nom).pin_memory(), torch.from_numpy(w.rad).pin_memory(),
                               flags=leb.FLAG_NO_MARGIN | leb.FLAG_HOST_IO)
     torch.cuda.synchronize()
-    lo, hi = ctx.leb_nn_fwd(nom, rad)
+    lo, hi = ctx.leb_nn_fwd(nom, rad, flags=VAL)
     assert torch.equal(hlo, lo.cpu()) and torch.equal(hhi, hi.cpu())
     # model not set
     ctx2 = leb.Context(0)
     with pytest.raises(leb.LebError) as e:
         ctx2.nn_n = 4
-        ctx2.leb_nn_fwd(nom, rad)
+        ctx2.leb_nn_fwd(nom, rad, flags=VAL)
     assert e.value.status == leb.LEB_ERR_STATE
     ctx2.close()
     ctx.close()

@@ -158,6 +158,18 @@ def test_certified_edge_cases(mods):
     g1 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=0)
     g2 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN)
     assert torch.equal(g1[0], g2[0]) and torch.equal(g1[1], g2[1])
+    # LEB_FLAG_REUSE_FWD is honoured only when the resident forward state has the mode the VJP call names (leb.h):
+    ctx.leb_nn_fwd(nom, rad, flags=0)                                   # certified state resident
+    assert ctx.leb_nn_state()[:2] == (w.B * w.T, True)
+    g3 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state()[2] is False                               # value-mode VJP asked: recomputed, not reused
+    assert torch.allclose(g3[0], g2[0], rtol=1e-5, atol=1e-7) and torch.allclose(g3[1], g2[1], rtol=1e-5, atol=1e-7)
+    ctx.leb_nn_fwd(nom, rad, flags=0)
+    g4 = ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state() == (w.B * w.T, True, True)                # reverse sweep over the certified state
+    # ... the gradient of the certified bound with its pads held constant: that of the value-mode bound up to the pads' size
+    for a, b in zip(g4, g2):
+        assert float((a - b).abs().max()) <= 2e-2 * float(b.abs().max())
     ctx.close()
 
 

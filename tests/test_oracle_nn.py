@@ -270,3 +270,52 @@ def test_vjp_random_directions_config3_shape():
         good += 1
         assert np.isclose((fp - fm) / (2 * h), gn @ dn + gr @ dr, rtol=1e-5, atol=1e-7)
     assert good >= 16
+
+
+def test_vjp_through_degenerate_tanh_neurons():
+    """Pin of relax_vjp_scalar's "degenerate" branch (u - l < 1e-12, reading R9): inputs 0..2 have
+    zero radius and feed, alone, hidden neurons 0..3 of layer 1, which feed, alone, neurons 0..2 of
+    layer 2 -- those neurons' pre-activation intervals are points, in both layers, and the output
+    reads them next to ordinary neurons.  Central differences in every direction that keeps the
+    structure (all nominal coordinates; the radii of the non-degenerate inputs) must match, and the
+    branch itself must return (numerically) nothing: at l = u = d the tangent's parameter adjoints
+    cancel, t''(d)(k_bar - d b_bar) = 0, and the widening term carries the factor (u - l)."""
+    rng = np.random.default_rng(77)
+    dims = [6, 9, 8, 7, 3]
+    Ws, bs = _net(rng, dims, scale=1.5)
+    Ws[0][:4, 3:] = 0.0          # layer-1 neurons 0..3 see only the zero-radius inputs
+    Ws[1][:3, 4:] = 0.0          # layer-2 neurons 0..2 see only those
+    a0 = rng.standard_normal(6)
+    sig = np.concatenate([np.zeros(3), rng.uniform(0.05, 0.3, 3)])
+    g_lo, g_hi = rng.standard_normal(3), rng.standard_normal(3)
+    fw = O.crown_forward(Ws, bs, O.ACT_TANH, a0, sig)
+    kinds = [[a[0] for a in r[4]] for r in fw["relaxs"]]
+    assert kinds[0][:4] == ["degenerate"] * 4 and kinds[1][:3] == ["degenerate"] * 3
+    assert "degenerate" not in kinds[0][4:] + kinds[1][3:] + kinds[2]
+    # the branch's own output: zero to rounding, for arbitrary parameter cotangents consistent with l = u = d
+    for l in (-0.7, 0.0, 1.3):
+        aux = O.relax_tanh_scalar(l, l)[4]
+        yb, lam = 0.83, -1.9                       # k_bar = y_bar * lam * z, b_bar = y_bar * lam at z = d
+        lb, ub = O.relax_vjp_scalar(O.ACT_TANH, l, l, aux, yb * lam * l, yb * lam, 0.3 * yb * lam * l, 0.3 * yb * lam)
+        assert abs(lb) < 1e-12 and abs(ub) < 1e-12
+    gn, gr = O.crown_vjp(Ws, bs, O.ACT_TANH, a0, sig, g_lo, g_hi)
+
+    def F(a, s):
+        f = O.crown_forward(Ws, bs, O.ACT_TANH, a, s)
+        return g_hi @ f["r_hi"] + g_lo @ f["r_lo"]
+    scale = max(np.abs(gn).max(), np.abs(gr).max())
+    checked = 0
+    for i in range(6):
+        for is_rad in (False, True):
+            if is_rad and i < 3:
+                continue                             # sigma = 0: one-sided, unpinned (SURVEY 8(c).4)
+            e = np.zeros(6)
+            e[i] = 1e-6
+            fp, fm, F0 = (F(a0, sig + e), F(a0, sig - e), F(a0, sig)) if is_rad else (F(a0 + e, sig), F(a0 - e, sig), F(a0, sig))
+            if abs((fp - F0) - (F0 - fm)) > 1e-3 * abs(fp - fm) + 1e-12:
+                continue                             # kink
+            g = (gr if is_rad else gn)[i]
+            assert abs((fp - fm) / 2e-6 - g) <= 1e-6 * scale + 1e-5 * abs(g), (i, is_rad)
+            checked += 1
+    assert checked >= 7
+    assert np.abs(gn[:3]).max() > 1e-3 * scale       # the zero-radius coordinates do carry gradient
