@@ -6,7 +6,7 @@
  *
  *     r_i(a) = f_i(a) - f_i(a~) - J(a~)(a - a~),   a = [x; u] in the tube box A_t     (10) L133
  *
- * where A_t = [a~ - sigma, a~ + sigma] is the centred tube box ((25a) L272 with mu = 0),
+ * where A_t = a~ + mu + [-sigma, sigma] is the tube box (25a) L272 (mu = NULL: the centred box, mu = 0),
  *   - for analytic dynamics by the path-based interval-Hessian bound, Thm 1 eq. (15);
  *   - for MLP dynamics by CROWN affine relaxations (Thm 2, eq. (18)) followed by the
  *     local Jacobian correction and box concretisation of Thm 3, eq. (19)-(21) L204-220;
@@ -51,13 +51,14 @@ typedef enum {
     LEB_ERR_SHAPE = 2,       /* ld too small, model/shape mismatch */
     LEB_ERR_ALIGN = 3,       /* pointer not 4-byte aligned */
     LEB_ERR_DOMAIN = 4,      /* reported by leb_domain_flag(): some tile hit a domain error */
-    LEB_ERR_UNSUPPORTED = 5, /* mu != NULL (non-centred boxes: SURVEY 8(f).1), unknown model */
+    LEB_ERR_UNSUPPORTED = 5, /* NN path with mu != NULL (non-centred boxes), unknown model, certified mode wider than 2048 */
     LEB_ERR_CUDA = 6,
     LEB_ERR_NOMEM = 7,
     LEB_ERR_STATE = 8        /* model not set before the call that needs it */
 } leb_status;
 
-typedef enum { LEB_MODEL_UNICYCLE = 1, LEB_MODEL_QUAD12 = 2, LEB_MODEL_QUADCHAIN = 3 } leb_model_id;
+typedef enum { LEB_MODEL_UNICYCLE = 1, LEB_MODEL_QUAD12 = 2, LEB_MODEL_QUADCHAIN = 3, LEB_MODEL_PLANAR_QUAD = 4,
+               LEB_MODEL_SATELLITE = 5 } leb_model_id;
 typedef enum { LEB_INTEG_EULER = 1, LEB_INTEG_RK4 = 2 } leb_integ;
 typedef enum { LEB_ACT_RELU = 1, LEB_ACT_TANH = 2 } leb_act;
 
@@ -67,6 +68,9 @@ typedef enum { LEB_ACT_RELU = 1, LEB_ACT_TANH = 2 } leb_act;
  *              nu = (T, tau[3]); ZYX rigid-body vector field (eq. (38), de-garbled).
  *   QUADCHAIN: n_units copies of QUAD12, x = (xi_1..xi_U), u = (nu_1..nu_U) ((39) L540-543),
  *              neighbours joined per axis by the spring k1 d + k3 d^3 (BASELINE config 4).
+ *   PLANAR_QUAD: x = (px, py, phi, vx, vy, phidot), u = (u1, u2), eq. (37a);
+ *              mass = m, g, Jx = moment of inertia J, k1 = arm length L.
+ *   SATELLITE: x = (q[4], om[3]), u = torque[3], eq. (36); (Jx, Jy, Jz) = diag of I_S.
  * integ = EULER: f = x + dt g(x,u) (the paper's choice, L505); RK4: classical 4 stages, u held. */
 typedef struct {
     int model_id; /* leb_model_id */
@@ -126,8 +130,10 @@ leb_status leb_set_mlp(leb_ctx* ctx, const leb_mlp* mlp, void* stream);
 leb_status leb_set_nn_chunk(leb_ctx* ctx, int tiles_per_chunk);
 
 /* Path-based interval-Hessian bound, Thm 1 eq. (15), for every tile.
- *   nom, rad : [B, T, ld_in]  nominal a~ and radii sigma >= 0 (box (25a) L272, mu = 0)
- *   mu       : must be NULL (LEB_ERR_UNSUPPORTED otherwise)
+ *   nom, rad : [B, T, ld_in]  nominal a~ and radii sigma >= 0
+ *   mu       : NULL (centred box) or [B, T, ld_in]: the box is a~ + mu + [-sigma, sigma] (25a) L272, D = A (-) a~ =
+ *              [mu - sigma, mu + sigma] (L164), and the Hessian enclosures of (15) are taken on the prefix sets of
+ *              hull(A u {a~}) (reading R4: Thm 1 needs the whole segment from a~ to a point of A)
  *   r_lo,r_hi: [B, T, ld_out] outputs, r_lo <= r(a) <= r_hi on the box, outward-rounded FP32. */
 leb_status leb_analytic_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad,
                             const float* mu, int ld_in, float* r_lo, float* r_hi, int ld_out,
@@ -159,6 +165,13 @@ leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float*
 leb_status leb_vjp(leb_ctx* ctx, int kind, int B, int T, const float* nom, const float* rad,
                    const float* g_lo, const float* g_hi, int ld_in, int ld_out, float* grad_nom,
                    float* grad_rad, unsigned flags, void* stream);
+
+/* leb_vjp for non-centred boxes: the same, with the box offsets mu [B, T, ld_in] as a third argument of the bound and
+ * its gradient grad_mu [B, T, ld_in] as a third output (grad_mu may be NULL).  mu == NULL: identical to leb_vjp.
+ * kind 1 (NN) with mu != NULL: LEB_ERR_UNSUPPORTED (the NN path takes centred boxes only). */
+leb_status leb_vjp_mu(leb_ctx* ctx, int kind, int B, int T, const float* nom, const float* rad, const float* mu,
+                      const float* g_lo, const float* g_hi, int ld_in, int ld_out, float* grad_nom,
+                      float* grad_rad, float* grad_mu, unsigned flags, void* stream);
 
 /* Zonotope fold, L229-231 and (25b,c) L274-281: c_bar = (r_lo + r_hi)/2,
  * R_diag = (r_hi - r_lo)/2 + pad (padding L347), rounded so that

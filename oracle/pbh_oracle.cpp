@@ -191,7 +191,8 @@ inline double cube_(double a) { return a * a * a; }
 
 // ----------------------------------------------------------------- models
 struct Params { double dt, mass, g, Jx, Jy, Jz, k1, k3; };
-enum { MODEL_UNICYCLE = 1, MODEL_QUAD12 = 2, MODEL_QUADCHAIN = 3, MODEL_QUADRATIC = 100, MODEL_LINEAR = 101 };
+enum { MODEL_UNICYCLE = 1, MODEL_QUAD12 = 2, MODEL_QUADCHAIN = 3, MODEL_PLANAR_QUAD = 4, MODEL_SATELLITE = 5,
+       MODEL_QUADRATIC = 100, MODEL_LINEAR = 101 };
 enum { INTEG_EULER = 1, INTEG_RK4 = 2 };
 
 // quad12 vector field g(xi, nu), DESIGN.md "Model SLPs" (state order PAPER.md:L538;
@@ -245,6 +246,37 @@ void chain_field(const Params& P, int U, const X* x, const X* u, X* out) {
     }
 }
 
+// planar quadrotor, eq. (37a): x = (px, py, phi, vx, vy, phidot), u = (u1, u2);
+// xdot = (vx, vy, phidot, -(u1+u2) sin(phi)/m, (u1+u2) cos(phi)/m - g, (L/J)(u2 - u1))   ("L/T" at L524 is a garble of L/J).
+// Params: mass = m, g, Jx = J, k1 = L.
+template <class X>
+void planar_quad_field(const Params& P, const X* x, const X* u, X* out) {
+    X s = sin_(x[2]), c = cos_(x[2]);
+    X thrust = scale(1.0 / P.mass, u[0] + u[1]);
+    out[0] = x[3];
+    out[1] = x[4];
+    out[2] = x[5];
+    out[3] = -(thrust * s);
+    out[4] = addc(thrust * c, -P.g);
+    out[5] = scale(P.k1 / P.Jx, u[1] - u[0]);
+}
+
+// satellite, eq. (36): x = (q[4], om[3]), u = torque[3];
+// qdot = zeta(om) q (the 4x4 matrix printed at L514), omdot = I^-1 (u - om x (I om)), I = diag(Jx, Jy, Jz).
+template <class X>
+void satellite_field(const Params& P, const X* x, const X* u, X* out) {
+    const X* q = x;
+    const X* om = x + 4;
+    out[0] = scale(0.5, ((-(om[0] * q[1])) - om[1] * q[2]) - om[2] * q[3]);
+    out[1] = scale(0.5, (om[0] * q[0] + om[2] * q[2]) - om[1] * q[3]);
+    out[2] = scale(0.5, (om[1] * q[0] - om[2] * q[1]) + om[0] * q[3]);
+    out[3] = scale(0.5, (om[2] * q[0] + om[1] * q[1]) - om[0] * q[2]);
+    // (om x I om) = ((Jz - Jy) om2 om3, (Jx - Jz) om3 om1, (Jy - Jx) om1 om2)
+    out[4] = scale((P.Jy - P.Jz) / P.Jx, om[1] * om[2]) + scale(1.0 / P.Jx, u[0]);
+    out[5] = scale((P.Jz - P.Jx) / P.Jy, om[0] * om[2]) + scale(1.0 / P.Jy, u[1]);
+    out[6] = scale((P.Jx - P.Jy) / P.Jz, om[0] * om[1]) + scale(1.0 / P.Jz, u[2]);
+}
+
 struct Model {
     int id, integ, n_units;
     Params P;
@@ -256,6 +288,8 @@ struct Model {
 template <class X>
 void vector_field(const Model& M, const X* x, const X* u, X* out) {
     if (M.id == MODEL_QUAD12) quad12_field<X>(M.P, x, u, nullptr, out);
+    else if (M.id == MODEL_PLANAR_QUAD) planar_quad_field<X>(M.P, x, u, out);
+    else if (M.id == MODEL_SATELLITE) satellite_field<X>(M.P, x, u, out);
     else chain_field<X>(M.P, M.n_units, x, u, out);
 }
 
@@ -331,14 +365,26 @@ void hessian_entry(const Model& M, const std::vector<Iv<S>>& box, int j, int k, 
     for (int l = 0; l < n; ++l) H[l] = f[l].wjk;
 }
 
-// one tile.  nom, rad: N scalars (S carries tangents for the VJP).  mu = NULL.
+// one tile.  nom, rad, mu: N scalars (S carries tangents for the VJP); mu may be NULL (= 0).
+//
+// Non-centred boxes (25a) L272: A_i = (a~_i + mu_i) + [-sigma_i, sigma_i], so Delta_i = A_i (-) a~_i =
+// [mu_i - sigma_i, mu_i + sigma_i] (L164).  Thm 1 needs a~ in the set the Hessian is enclosed on (L164: the path
+// runs from a~ to a point of A one coordinate at a time), which (25a) does not give when |mu_i| > sigma_i; reading
+// R4: the enclosure is taken on hull(A_i u {a~_i}) = a~_i + [min(mu_i - sigma_i, 0), max(mu_i + sigma_i, 0)]
+// -- every point of the segment from a~_i to a point of A_i.  With mu = 0 this is A_i itself.
 template <class S>
-void pbh_tile(const Model& M, const S* nom, const S* rad, int mode, S* r_lo, S* r_hi) {
+void pbh_tile(const Model& M, const S* nom, const S* rad, const S* mu, int mode, S* r_lo, S* r_hi) {
     const int N = M.N, n = M.n;
     std::vector<Iv<S>> A(N), D(N), box(N), H(n);
     for (int i = 0; i < N; ++i) {
-        A[i] = {nom[i] - rad[i], nom[i] + rad[i]};          // (25a) with mu = 0
-        D[i] = {-rad[i], rad[i]};                           // Delta = A (-) a~
+        if (mu) {
+            D[i] = {mu[i] - rad[i], mu[i] + rad[i]};        // Delta = A (-) a~
+            // ties keep the first candidate (the VJP then follows mu -+ sigma)
+            A[i] = {nom[i] + min_(D[i].lo, cst<S>(0.0)), nom[i] + max_(D[i].hi, cst<S>(0.0))};
+        } else {
+            A[i] = {nom[i] - rad[i], nom[i] + rad[i]};      // (25a) with mu = 0
+            D[i] = {-rad[i], rad[i]};                       // Delta = A (-) a~
+        }
     }
     std::vector<Iv<S>> R(n, iconst<S>(0.0));
     if (mode == MODE_CLASSIC) {
@@ -376,6 +422,8 @@ Model make_model(int id, int integ, int n_units, const double* params, const dou
     if (id == MODEL_UNICYCLE) { M.n = 3; M.N = 5; }
     else if (id == MODEL_QUAD12) { M.n = 12; M.N = 16; }
     else if (id == MODEL_QUADCHAIN) { M.n = 12 * n_units; M.N = 16 * n_units; }
+    else if (id == MODEL_PLANAR_QUAD) { M.n = 6; M.N = 8; }
+    else if (id == MODEL_SATELLITE) { M.n = 7; M.N = 10; }
     else { M.n = n; M.N = N; }
     return M;
 }
@@ -387,7 +435,7 @@ extern "C" {
 // status: 0 ok, 4 domain error (0 in cos(theta) box) in some tile -> that tile's bounds are -/+inf
 int pbh_oracle_eval(int model_id, int integ, int n_units, const double* params,
                     const double* Q, const double* C, int n_gen, int N_gen,
-                    int tiles, const double* nom, const double* rad, int mode,
+                    int tiles, const double* nom, const double* rad, const double* mu, int mode,
                     double* r_lo, double* r_hi, int threads) {
     Model M = make_model(model_id, integ, n_units, params, Q, C, n_gen, N_gen);
     int status = 0;
@@ -397,7 +445,7 @@ int pbh_oracle_eval(int model_id, int integ, int n_units, const double* params,
 #pragma omp parallel for schedule(dynamic, 1)
     for (int t = 0; t < tiles; ++t) {
         try {
-            pbh_tile<double>(M, nom + (size_t)t * M.N, rad + (size_t)t * M.N, mode,
+            pbh_tile<double>(M, nom + (size_t)t * M.N, rad + (size_t)t * M.N, mu ? mu + (size_t)t * M.N : nullptr, mode,
                              r_lo + (size_t)t * M.n, r_hi + (size_t)t * M.n);
         } catch (DomainError&) {
             for (int l = 0; l < M.n; ++l) { r_lo[(size_t)t * M.n + l] = -INFINITY; r_hi[(size_t)t * M.n + l] = INFINITY; }
@@ -408,12 +456,13 @@ int pbh_oracle_eval(int model_id, int integ, int n_units, const double* params,
     return status;
 }
 
-// VJP by forward-mode duals.  dirs: list of n_dirs direction indices in [0, 2N):
-// d < N -> d/d nom[d], d >= N -> d/d rad[d-N].  out[t*n_dirs + i] =
+// VJP by forward-mode duals.  dirs: list of n_dirs direction indices in [0, 3N):
+// d < N -> d/d nom[d], N <= d < 2N -> d/d rad[d-N], d >= 2N -> d/d mu[d-2N] (mu != NULL only).
+// out[t*n_dirs + i] =
 // sum_l g_hi[l] d r_hi[l] + g_lo[l] d r_lo[l]  along direction dirs[i].
 int pbh_oracle_vjp(int model_id, int integ, int n_units, const double* params,
                    const double* Q, const double* C, int n_gen, int N_gen,
-                   int tiles, const double* nom, const double* rad,
+                   int tiles, const double* nom, const double* rad, const double* mu,
                    const double* g_lo, const double* g_hi,
                    int n_dirs, const int* dirs, double* out, int threads) {
     Model M = make_model(model_id, integ, n_units, params, Q, C, n_gen, N_gen);
@@ -425,14 +474,15 @@ int pbh_oracle_vjp(int model_id, int integ, int n_units, const double* params,
 #pragma omp parallel for schedule(dynamic, 1) collapse(2)
     for (int t = 0; t < tiles; ++t)
         for (int i = 0; i < n_dirs; ++i) {
-            std::vector<Dual> a(N), s(N), lo(n), hi(n);
+            std::vector<Dual> a(N), s(N), m(N), lo(n), hi(n);
             const int d = dirs[i];
             for (int q = 0; q < N; ++q) {
                 a[q] = Dual{nom[(size_t)t * N + q], (d == q) ? 1.0 : 0.0};
                 s[q] = Dual{rad[(size_t)t * N + q], (d == N + q) ? 1.0 : 0.0};
+                m[q] = Dual{mu ? mu[(size_t)t * N + q] : 0.0, (d == 2 * N + q) ? 1.0 : 0.0};
             }
             try {
-                pbh_tile<Dual>(M, a.data(), s.data(), MODE_PATH, lo.data(), hi.data());
+                pbh_tile<Dual>(M, a.data(), s.data(), mu ? m.data() : nullptr, MODE_PATH, lo.data(), hi.data());
                 double acc = 0.0;
                 for (int l = 0; l < n; ++l)
                     acc += g_hi[(size_t)t * n + l] * hi[l].d + g_lo[(size_t)t * n + l] * lo[l].d;

@@ -15,7 +15,8 @@ _SRC = os.path.join(_HERE, "pbh_oracle.cpp")
 _LIB = os.path.join(_HERE, "libpbh_oracle.so")
 
 MODE_PATH, MODE_EXPAND, MODE_CLASSIC = 0, 1, 2
-MODEL_UNICYCLE, MODEL_QUAD12, MODEL_QUADCHAIN, MODEL_QUADRATIC, MODEL_LINEAR = 1, 2, 3, 100, 101
+MODEL_UNICYCLE, MODEL_QUAD12, MODEL_QUADCHAIN, MODEL_PLANAR_QUAD, MODEL_SATELLITE = 1, 2, 3, 4, 5
+MODEL_QUADRATIC, MODEL_LINEAR = 100, 101
 INTEG_EULER, INTEG_RK4 = 1, 2
 
 
@@ -57,6 +58,10 @@ class ModelSpec:
             self.n, self.N = 12, 16
         elif model_id == MODEL_QUADCHAIN:
             self.n, self.N = 12 * n_units, 16 * n_units
+        elif model_id == MODEL_PLANAR_QUAD:
+            self.n, self.N = 6, 8
+        elif model_id == MODEL_SATELLITE:
+            self.n, self.N = 7, 10
         else:
             self.n, self.N = self.C.shape
 
@@ -65,30 +70,34 @@ class ModelSpec:
                 _p(self.params), _p(self.Q), _p(self.C), ctypes.c_int(self.n), ctypes.c_int(self.N))
 
 
-def pbh(spec: ModelSpec, nom, rad, mode=MODE_PATH, threads=0):
-    """nom, rad [tiles, N] -> (r_lo, r_hi) [tiles, n] FP64, status."""
+def pbh(spec: ModelSpec, nom, rad, mode=MODE_PATH, threads=0, mu=None):
+    """nom, rad (, mu) [tiles, N] -> (r_lo, r_hi) [tiles, n] FP64, status.  mu: box offsets of (25a)."""
     nom = np.ascontiguousarray(nom, dtype=np.float64).reshape(-1, spec.N)
     rad = np.ascontiguousarray(rad, dtype=np.float64).reshape(-1, spec.N)
+    if mu is not None:
+        mu = np.ascontiguousarray(mu, dtype=np.float64).reshape(-1, spec.N)
     tiles = nom.shape[0]
     r_lo = np.empty((tiles, spec.n))
     r_hi = np.empty((tiles, spec.n))
-    st = lib().pbh_oracle_eval(*spec._head(), ctypes.c_int(tiles), _p(nom), _p(rad), ctypes.c_int(mode),
+    st = lib().pbh_oracle_eval(*spec._head(), ctypes.c_int(tiles), _p(nom), _p(rad), _p(mu), ctypes.c_int(mode),
                                _p(r_lo), _p(r_hi), ctypes.c_int(threads))
     return r_lo, r_hi, st
 
 
-def pbh_vjp(spec: ModelSpec, nom, rad, g_lo, g_hi, dirs=None, threads=0):
-    """Gradient entries along `dirs` (indices in [0,2N): <N nominal, >=N radius);
-    default all 2N.  Returns array [tiles, len(dirs)]."""
+def pbh_vjp(spec: ModelSpec, nom, rad, g_lo, g_hi, dirs=None, threads=0, mu=None):
+    """Gradient entries along `dirs` (indices in [0,3N): <N nominal, [N,2N) radius, >=2N mu);
+    default all 2N (3N with mu).  Returns array [tiles, len(dirs)]."""
     nom = np.ascontiguousarray(nom, dtype=np.float64).reshape(-1, spec.N)
     rad = np.ascontiguousarray(rad, dtype=np.float64).reshape(-1, spec.N)
+    if mu is not None:
+        mu = np.ascontiguousarray(mu, dtype=np.float64).reshape(-1, spec.N)
     g_lo = np.ascontiguousarray(g_lo, dtype=np.float64).reshape(-1, spec.n)
     g_hi = np.ascontiguousarray(g_hi, dtype=np.float64).reshape(-1, spec.n)
     if dirs is None:
-        dirs = np.arange(2 * spec.N)
+        dirs = np.arange((2 if mu is None else 3) * spec.N)
     dirs = np.ascontiguousarray(dirs, dtype=np.int32)
     out = np.empty((nom.shape[0], dirs.shape[0]))
-    st = lib().pbh_oracle_vjp(*spec._head(), ctypes.c_int(nom.shape[0]), _p(nom), _p(rad), _p(g_lo), _p(g_hi),
+    st = lib().pbh_oracle_vjp(*spec._head(), ctypes.c_int(nom.shape[0]), _p(nom), _p(rad), _p(mu), _p(g_lo), _p(g_hi),
                               ctypes.c_int(dirs.shape[0]), _p(dirs), _p(out), ctypes.c_int(threads))
     return out, st
 

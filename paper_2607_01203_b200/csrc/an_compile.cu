@@ -1,0 +1,546 @@
+// an_compile.cu -- host side of the analytic path: symbolic evaluation of a model's straight-line program
+// (SLP) into the interval tape of an_tape.h.  Structure only -- no interval is evaluated here; every number
+// of the bound is computed by the device interpreter (analytic.cu).
+//
+// For every path index j (eq. (14)-(15)) the model SLP is run on symbolic second-order
+// jets (reading R1): a component is `zero`, a constant c (the seeds e_j, e_k are the constant 1), or a slot
+// of the tape.  0 * x = 0, 0 + x = x, 1 * x = x and c * [lo, hi] = the hull of the endpoint products are exact
+// identities of the interval extension (also under directed rounding), so dropping / folding them leaves
+// the enclosure the contract defines; two constants are folded only when the FP32 result is exact.
+//   pass WJ(j)   : w and w_j of every SLP variable on the prefix box A^(j); results memoised in evaluation order
+//   pass K(j,k)  : the same SLP again for every k >= j that shares an output with j; w and w_j come from the
+//                  memo (the SLP is straight-line: the sequence of operations is the same), w_k and w_jk are new
+// then dead code is removed (backwards from the OUT instructions) and slots are renumbered.
+#include <math.h>
+#include <string.h>
+#include <algorithm>
+#include <unordered_map>
+#include "an_tape.h"
+#include "internal.h"
+
+namespace leb_an {
+namespace {
+
+enum SK : uint8_t { SK_Z = 0, SK_C = 1, SK_S = 2 };
+struct Sym {
+    SK k = SK_Z;
+    float c = 0.f;     // SK_C
+    uint32_t s = 0;    // SK_S: slot id; bit 30 set = slot of the current K segment, else of WJ
+};
+constexpr uint32_t KTAG = 1u << 30;
+
+inline Sym Z() { return Sym{}; }
+inline Sym C(float c) { Sym r; if (c == 0.f) return r; r.k = SK_C; r.c = c; return r; }
+inline Sym S(uint32_t s) { Sym r; r.k = SK_S; r.s = s; return r; }
+inline uint32_t fbits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+inline bool exact_f32(double v) { return (double)(float)v == v && fabs(v) < 3.0e38; }
+
+struct SJet { Sym w, wj, wk, wjk; };
+
+class Builder {
+public:
+    // ---- emission state
+    std::vector<Ins> wj_ins, k_ins;
+    bool kphase = false, diag = false;
+    std::vector<Sym> memo;
+    size_t mpos = 0;
+    std::unordered_map<uint32_t, uint32_t> const_wj, const_k;     // float bits -> slot
+    int j = 0, k = 0;
+    bool use_mu = false;
+    std::vector<int> in_slot;        // input coordinate -> slot of its w in WJ (or -1)
+
+    uint32_t emit(uint32_t op, uint32_t a, uint32_t b) {
+        std::vector<Ins>& v = kphase ? k_ins : wj_ins;
+        uint32_t slot = (uint32_t)v.size() | (kphase ? KTAG : 0u);
+        // an operand slot is stored with its tag; resolved to a final index when the task is laid out
+        v.push_back(Ins{op, a});      // temporarily: w0 = op, w1 = a ; b kept in the side array
+        (kphase ? k_b : wj_b).push_back(b);
+        return slot;
+    }
+    std::vector<uint32_t> wj_b, k_b;
+
+    Sym mat(Sym a) {                 // constants become slots when an instruction needs one
+        if (a.k != SK_C) return a;
+        auto& cache = kphase ? const_k : const_wj;
+        auto it = cache.find(fbits(a.c));
+        if (it != cache.end()) return S(it->second);
+        // a constant needed in a K segment may already exist in WJ
+        if (kphase) { auto iw = const_wj.find(fbits(a.c)); if (iw != const_wj.end()) return S(iw->second); }
+        uint32_t s = emit(OP_CONST, 0, fbits(a.c));
+        cache[fbits(a.c)] = s;
+        return S(s);
+    }
+    Sym un(uint32_t op, Sym a) { a = mat(a); return S(emit(op, a.s, 0)); }
+    Sym neg(Sym a) {
+        if (a.k == SK_Z) return a;
+        if (a.k == SK_C) return C(-a.c);
+        return S(emit(OP_NEG, a.s, 0));
+    }
+    Sym scale(float c, Sym a) {
+        if (c == 0.f || a.k == SK_Z) return Z();
+        if (c == 1.f) return a;
+        if (a.k == SK_C) {
+            double p = (double)c * (double)a.c;
+            if (exact_f32(p)) return C((float)p);
+            a = mat(a);
+        }
+        return S(emit(OP_SCALE, a.s, fbits(c)));
+    }
+    Sym addc(Sym a, float c) {
+        if (c == 0.f) return a;
+        if (a.k == SK_Z) return C(c);
+        if (a.k == SK_C) {
+            double s = (double)a.c + (double)c;
+            if (exact_f32(s)) return C((float)s);
+            a = mat(a);
+        }
+        return S(emit(OP_ADDC, a.s, fbits(c)));
+    }
+    Sym add(Sym a, Sym b) {
+        if (a.k == SK_Z) return b;
+        if (b.k == SK_Z) return a;
+        if (a.k == SK_C && b.k == SK_C) {
+            double s = (double)a.c + (double)b.c;
+            if (exact_f32(s)) return C((float)s);
+            a = mat(a);
+        }
+        if (a.k == SK_C) return addc(b, a.c);
+        if (b.k == SK_C) return addc(a, b.c);
+        return S(emit(OP_ADD, a.s, b.s));
+    }
+    Sym sub(Sym a, Sym b) {
+        if (b.k == SK_Z) return a;
+        if (a.k == SK_Z) return neg(b);
+        if (b.k == SK_C) return add(a, C(-b.c));
+        if (a.k == SK_C) return addc(neg(b), a.c);
+        return S(emit(OP_SUB, a.s, b.s));
+    }
+    Sym mul(Sym a, Sym b) {
+        if (a.k == SK_Z || b.k == SK_Z) return Z();
+        if (a.k == SK_C) return scale(a.c, b);
+        if (b.k == SK_C) return scale(b.c, a);
+        return S(emit(OP_MUL, a.s, b.s));
+    }
+    Sym sqr(Sym a) {
+        if (a.k == SK_Z) return a;
+        if (a.k == SK_C) {
+            double p = (double)a.c * (double)a.c;
+            if (exact_f32(p)) return C((float)p);
+            a = mat(a);
+        }
+        return S(emit(OP_SQR, a.s, 0));
+    }
+
+    // w / w_j components: computed in pass WJ, replayed from the memo in pass K
+    template <class F> Sym M(F&& f) {
+        if (kphase) return memo[mpos++];
+        Sym r = f();
+        memo.push_back(r);
+        return r;
+    }
+
+    // ---- inputs: prefix box A^(j) (14) L157-162
+    SJet in(int g) {
+        SJet r;
+        r.w = M([&] {
+            if (in_slot[g] < 0) {
+                uint32_t op = g <= j ? (use_mu ? OP_BOXMU : OP_BOX) : OP_PT;
+                in_slot[g] = (int)emit(op, (uint32_t)g, 0);
+            }
+            return S((uint32_t)in_slot[g]);
+        });
+        r.wj = g == j ? C(1.f) : Z();
+        r.wk = g == k ? C(1.f) : Z();
+        r.wjk = Z();
+        return r;
+    }
+    SJet cst(float c) { SJet r; r.w = C(c); return r; }
+
+    // ---- jet arithmetic (reading R1)
+    SJet jadd(const SJet& a, const SJet& b) {
+        SJet r;
+        r.w = M([&] { return add(a.w, b.w); });
+        r.wj = M([&] { return add(a.wj, b.wj); });
+        if (kphase) { r.wk = diag ? r.wj : add(a.wk, b.wk); r.wjk = add(a.wjk, b.wjk); }
+        return r;
+    }
+    SJet jsub(const SJet& a, const SJet& b) {
+        SJet r;
+        r.w = M([&] { return sub(a.w, b.w); });
+        r.wj = M([&] { return sub(a.wj, b.wj); });
+        if (kphase) { r.wk = diag ? r.wj : sub(a.wk, b.wk); r.wjk = sub(a.wjk, b.wjk); }
+        return r;
+    }
+    SJet jneg(const SJet& a) {
+        SJet r;
+        r.w = M([&] { return neg(a.w); });
+        r.wj = M([&] { return neg(a.wj); });
+        if (kphase) { r.wk = diag ? r.wj : neg(a.wk); r.wjk = neg(a.wjk); }
+        return r;
+    }
+    SJet jscale(float c, const SJet& a) {
+        SJet r;
+        r.w = M([&] { return scale(c, a.w); });
+        r.wj = M([&] { return scale(c, a.wj); });
+        if (kphase) { r.wk = diag ? r.wj : scale(c, a.wk); r.wjk = scale(c, a.wjk); }
+        return r;
+    }
+    SJet jaddc(const SJet& a, float c) {
+        SJet r = a;
+        r.w = M([&] { return addc(a.w, c); });
+        return r;
+    }
+    // product rule; on the diagonal (j == k) the cross term is 2 a_j b_j
+    SJet jmul(const SJet& a, const SJet& b) {
+        SJet r;
+        r.w = M([&] { return mul(a.w, b.w); });
+        r.wj = M([&] { return add(mul(a.wj, b.w), mul(a.w, b.wj)); });
+        if (kphase) {
+            r.wk = diag ? r.wj : add(mul(a.wk, b.w), mul(a.w, b.wk));
+            Sym cross = diag ? scale(2.f, mul(a.wj, b.wj)) : add(mul(a.wj, b.wk), mul(a.wk, b.wj));
+            r.wjk = add(add(mul(a.wjk, b.w), cross), mul(a.w, b.wjk));
+        }
+        return r;
+    }
+    // w = phi(a) from enclosures f, f1, f2 of phi, phi', phi'' on a.w; on the diagonal a_j a_k = sqr(a_j)
+    SJet junary(const SJet& a, Sym f, Sym f1, Sym f2) {
+        SJet r;
+        r.w = f;
+        r.wj = M([&] { return mul(f1, a.wj); });
+        if (kphase) {
+            r.wk = diag ? r.wj : mul(f1, a.wk);
+            Sym jk = diag ? sqr(a.wj) : mul(a.wj, a.wk);
+            r.wjk = add(mul(f2, jk), mul(f1, a.wjk));
+        }
+        return r;
+    }
+    void jsincos(const SJet& a, SJet* s_out, SJet* c_out) {
+        Sym s = M([&] { return un(OP_SIN, a.w); });
+        Sym c = M([&] { return un(OP_COS, a.w); });
+        Sym ns = M([&] { return neg(s); });
+        Sym nc = M([&] { return neg(c); });
+        *s_out = junary(a, s, c, ns);        // (sin)' = cos, (sin)'' = -sin
+        *c_out = junary(a, c, ns, nc);       // (cos)' = -sin, (cos)'' = -cos
+    }
+    SJet jrecip(const SJet& a) {
+        Sym r = M([&] { return un(OP_RECIP, a.w); });
+        Sym f1 = M([&] { return neg(sqr(r)); });                     // (1/a)' = -1/a^2
+        Sym f2 = M([&] { return scale(2.f, un(OP_CUBE, r)); });      // (1/a)'' = 2/a^3
+        return junary(a, r, f1, f2);
+    }
+    SJet jcube(const SJet& a) {
+        Sym f = M([&] { return un(OP_CUBE, a.w); });
+        Sym f1 = M([&] { return scale(3.f, sqr(a.w)); });
+        Sym f2 = M([&] { return scale(6.f, a.w); });
+        return junary(a, f, f1, f2);
+    }
+    SJet jsqr(const SJet& a) {
+        Sym f = M([&] { return sqr(a.w); });
+        Sym f1 = M([&] { return scale(2.f, a.w); });
+        return junary(a, f, f1, C(2.f));
+    }
+};
+
+// ------------------------------------------------------------------------------------------ model SLPs
+// (restated from the paper, shared with nothing)
+using JV = std::vector<SJet>;
+
+// quad12 vector field, state order of PAPER.md:L538: xi = (p[3], phi, theta, psi, v[3], p, q, r), nu = (T, tau[3]);
+// eq. (38a) L534 is garbled, the standard ZYX rigid-body form is used (reading R6).  coup: spring force per axis or NULL.
+void quad12_field(Builder& B, const Model& M, const SJet* xi, const SJet* nu, const SJet* coup, SJet* out) {
+    SJet sphi, cphi, sth, cth, spsi, cpsi;
+    B.jsincos(xi[3], &sphi, &cphi);
+    B.jsincos(xi[4], &sth, &cth);
+    B.jsincos(xi[5], &spsi, &cpsi);
+    SJet rcth = B.jrecip(cth);
+    const SJet &p = xi[9], &q = xi[10], &r = xi[11];
+    SJet a = B.jadd(B.jmul(q, sphi), B.jmul(r, cphi));
+    out[0] = xi[6];
+    out[1] = xi[7];
+    out[2] = xi[8];
+    out[3] = B.jadd(p, B.jmul(a, B.jmul(sth, rcth)));
+    out[4] = B.jsub(B.jmul(q, cphi), B.jmul(r, sphi));
+    out[5] = B.jmul(a, rcth);
+    SJet Tm = B.jscale(M.inv_m, nu[0]);
+    out[6] = B.jmul(Tm, B.jadd(B.jmul(B.jmul(cpsi, sth), cphi), B.jmul(spsi, sphi)));
+    out[7] = B.jmul(Tm, B.jsub(B.jmul(B.jmul(spsi, sth), cphi), B.jmul(cpsi, sphi)));
+    out[8] = B.jaddc(B.jmul(Tm, B.jmul(cth, cphi)), -M.g);
+    out[9] = B.jadd(B.jscale(M.cp, B.jmul(q, r)), B.jscale(M.iJx, nu[1]));
+    out[10] = B.jadd(B.jscale(M.cq, B.jmul(p, r)), B.jscale(M.iJy, nu[2]));
+    out[11] = B.jadd(B.jscale(M.cr, B.jmul(p, q)), B.jscale(M.iJz, nu[3]));
+    if (coup)
+        for (int c = 0; c < 3; ++c) out[6 + c] = B.jadd(out[6 + c], B.jscale(M.inv_m, coup[c]));
+}
+
+// chain vector field (BASELINE config 4): spring i joins units i and i+1 per axis, s = k1 d + k3 d^3, d = p_{i+1} - p_i;
+// force +s on unit i, -s on unit i+1 (open chain, zero rest length)
+void chain_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
+    const int U = M.n_units;
+    JV s(3 * std::max(U - 1, 1));
+    for (int i = 0; i + 1 < U; ++i)
+        for (int c = 0; c < 3; ++c) {
+            SJet d = B.jsub(x[12 * (i + 1) + c], x[12 * i + c]);
+            s[3 * i + c] = B.jadd(B.jscale(M.k1, d), B.jscale(M.k3, B.jcube(d)));
+        }
+    for (int i = 0; i < U; ++i) {
+        SJet coup[3];
+        bool any = false;
+        for (int c = 0; c < 3; ++c) {
+            if (i + 1 < U && i > 0) { coup[c] = B.jsub(s[3 * i + c], s[3 * (i - 1) + c]); any = true; }
+            else if (i + 1 < U) { coup[c] = s[3 * i + c]; any = true; }
+            else if (i > 0) { coup[c] = B.jneg(s[3 * (i - 1) + c]); any = true; }
+        }
+        quad12_field(B, M, &x[12 * i], &u[4 * i], any ? coup : nullptr, &out[12 * i]);
+    }
+}
+
+// planar quadrotor (37a) PAPER.md:L521-528: x = (px, py, phi, vx, vy, phidot), u = (u1, u2)
+void planar_quad_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
+    SJet s, c;
+    B.jsincos(x[2], &s, &c);
+    SJet thrust = B.jscale(M.inv_m, B.jadd(u[0], u[1]));
+    out[0] = x[3];
+    out[1] = x[4];
+    out[2] = x[5];
+    out[3] = B.jneg(B.jmul(thrust, s));
+    out[4] = B.jaddc(B.jmul(thrust, c), -M.g);
+    out[5] = B.jscale(M.k1, B.jsub(u[1], u[0]));      // k1 holds L / J
+}
+
+// satellite (36) PAPER.md:L507-519: x = (q[4], om[3]), u = torque[3];
+// qdot = zeta(om) q, omdot = I^-1 (u - om x (I om)), I = diag(Jx, Jy, Jz)
+void satellite_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
+    const SJet *q = &x[0], *om = &x[4];
+    auto half = [&](const SJet& a) { return B.jscale(0.5f, a); };
+    out[0] = half(B.jsub(B.jsub(B.jneg(B.jmul(om[0], q[1])), B.jmul(om[1], q[2])), B.jmul(om[2], q[3])));
+    out[1] = half(B.jsub(B.jadd(B.jmul(om[0], q[0]), B.jmul(om[2], q[2])), B.jmul(om[1], q[3])));
+    out[2] = half(B.jadd(B.jsub(B.jmul(om[1], q[0]), B.jmul(om[2], q[1])), B.jmul(om[0], q[3])));
+    out[3] = half(B.jsub(B.jadd(B.jmul(om[2], q[0]), B.jmul(om[1], q[1])), B.jmul(om[0], q[2])));
+    // om x (I om) = ((Jz - Jy) om2 om3, (Jx - Jz) om3 om1, (Jy - Jx) om1 om2); cp, cq, cr hold -(that)/J*
+    out[4] = B.jadd(B.jscale(M.cp, B.jmul(om[1], om[2])), B.jscale(M.iJx, u[0]));
+    out[5] = B.jadd(B.jscale(M.cq, B.jmul(om[0], om[2])), B.jscale(M.iJy, u[1]));
+    out[6] = B.jadd(B.jscale(M.cr, B.jmul(om[0], om[1])), B.jscale(M.iJz, u[2]));
+}
+
+void vector_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
+    if (M.id == LEB_MODEL_PLANAR_QUAD) planar_quad_field(B, M, x, u, out);
+    else if (M.id == LEB_MODEL_SATELLITE) satellite_field(B, M, x, u, out);
+    else chain_field(B, M, x, u, out);
+}
+
+// discrete-time map f(a), a = [x; u]; Euler (the paper's choice, L505) or classical RK4 with u held
+void model_f(Builder& B, const Model& M, JV& f) {
+    const int n = M.n, N = M.N;
+    JV al(N);
+    for (int g = 0; g < N; ++g) al[g] = B.in(g);
+    if (M.id == LEB_MODEL_UNICYCLE) {
+        // a = (px, py, th, v, om); f = (px + dt v cos th, py + dt v sin th, th + dt om)
+        SJet s, c;
+        B.jsincos(al[2], &s, &c);
+        f[0] = B.jadd(al[0], B.jscale(M.dt, B.jmul(al[3], c)));
+        f[1] = B.jadd(al[1], B.jscale(M.dt, B.jmul(al[3], s)));
+        f[2] = B.jadd(al[2], B.jscale(M.dt, al[4]));
+        return;
+    }
+    JV x(al.begin(), al.begin() + n), u(al.begin() + n, al.end());
+    JV k1(n), k2(n), k3(n), k4(n), xs(n);
+    vector_field(B, M, x, u, k1);
+    if (M.integ == LEB_INTEG_EULER) {
+        for (int i = 0; i < n; ++i) f[i] = B.jadd(x[i], B.jscale(M.dt, k1[i]));
+        return;
+    }
+    for (int i = 0; i < n; ++i) xs[i] = B.jadd(x[i], B.jscale(M.half_dt, k1[i]));
+    vector_field(B, M, xs, u, k2);
+    for (int i = 0; i < n; ++i) xs[i] = B.jadd(x[i], B.jscale(M.half_dt, k2[i]));
+    vector_field(B, M, xs, u, k3);
+    for (int i = 0; i < n; ++i) xs[i] = B.jadd(x[i], B.jscale(M.dt, k3[i]));
+    vector_field(B, M, xs, u, k4);
+    for (int i = 0; i < n; ++i)
+        f[i] = B.jadd(x[i], B.jscale(M.dt6, B.jadd(B.jadd(B.jadd(k1[i], B.jscale(2.f, k2[i])), B.jscale(2.f, k3[i])), k4[i])));
+}
+
+// ------------------------------------------------------------------------------------------ layout
+struct RawSeg { std::vector<Ins> ins; std::vector<uint32_t> b; };      // ins: w0 = op, w1 = a (tagged)
+
+inline bool op_has_a(uint32_t op) { return op >= OP_ADD && op != OP_COUNT; }      // a is a slot
+inline bool op_has_b(uint32_t op) { return op == OP_ADD || op == OP_SUB || op == OP_MUL; }   // b is a slot
+
+}  // namespace
+
+// Compile the model into a tape.  with_mu: non-centred boxes (25a) L272 (reading R4: prefix hull sets).
+void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
+    const int n = M.n, N = M.N;
+    T->n = n; T->N = N; T->uses_mu = with_mu;
+    T->ins.clear(); T->segs.clear(); T->tasks.clear();
+
+    // ---- first-order dependencies: which outputs read coordinate g at all (pass WJ in direction g)
+    std::vector<std::vector<uint8_t>> dep(N, std::vector<uint8_t>(n, 0));
+    {
+        for (int g = 0; g < N; ++g) {
+            Builder B;
+            B.j = g; B.k = -1; B.use_mu = with_mu;
+            B.in_slot.assign(N, -1);
+            JV f(n);
+            model_f(B, M, f);
+            for (int l = 0; l < n; ++l) dep[g][l] = f[l].wj.k != SK_Z;
+        }
+    }
+
+    std::vector<std::vector<uint32_t>> out_rows(n), var_rows(N);
+    uint32_t acc_rows = 0, grad_rows = 0;
+
+    for (int j = 0; j < N; ++j) {
+        Builder B;
+        B.j = j; B.k = -1; B.use_mu = with_mu;
+        B.in_slot.assign(N, -1);
+        JV f(n);
+        model_f(B, M, f);                       // pass WJ: memo filled
+        Sym Dj = S(B.emit(with_mu ? OP_DELTAMU : OP_DELTA, (uint32_t)j, 0));
+        const size_t wj_len0 = B.wj_ins.size();
+        (void)wj_len0;
+
+        std::vector<RawSeg> ksegs;
+        std::vector<uint8_t> wj_live(B.wj_ins.size() + 64, 0);
+        std::vector<int> acc_of(n, -1);
+        int n_acc = 0;
+        for (int k = j; k < N; ++k) {
+            bool share = false;
+            for (int l = 0; l < n && !share; ++l) share = dep[j][l] && dep[k][l];
+            if (!share) continue;
+            B.kphase = true; B.diag = (k == j); B.k = k; B.mpos = 0;
+            B.k_ins.clear(); B.k_b.clear(); B.const_k.clear();
+            JV fk(n);
+            model_f(B, M, fk);
+            // terms of eq. (15): off-diagonal [H_kj] D_j D_k, diagonal 1/2 [H_kk] sqr(D_k)   (D_k^2 >= 0, L152)
+            Sym fac;
+            bool have_fac = false;
+            for (int l = 0; l < n; ++l) {
+                if (fk[l].wjk.k == SK_Z) continue;
+                if (!have_fac) {
+                    if (B.diag) fac = B.sqr(Dj);
+                    else fac = B.mul(Dj, S(B.emit(with_mu ? OP_DELTAMU : OP_DELTA, (uint32_t)k, 0)));
+                    have_fac = true;
+                }
+                Sym t = B.mul(fk[l].wjk, fac);
+                if (B.diag) t = B.scale(0.5f, t);
+                t = B.mat(t);
+                if (acc_of[l] < 0) acc_of[l] = n_acc++;
+                B.emit(OP_OUT, t.s, ((uint32_t)l << 16) | (uint32_t)acc_of[l]);
+            }
+            B.kphase = false;
+            if (!have_fac) continue;
+            // ---- dead code: keep what the OUT instructions read
+            const size_t nk = B.k_ins.size();
+            std::vector<uint8_t> live(nk, 0);
+            if (wj_live.size() < B.wj_ins.size()) wj_live.resize(B.wj_ins.size() + 64, 0);   // constants may be added to WJ? (no: kphase emits to K)
+            auto touch = [&](uint32_t s) { if (s & KTAG) live[s & ~KTAG] = 1; else wj_live[s] = 1; };
+            for (size_t i = nk; i-- > 0;) {
+                const uint32_t op = B.k_ins[i].w0;
+                if (op == OP_OUT) live[i] = 1;
+                if (!live[i]) continue;
+                if (op_has_a(op)) touch(B.k_ins[i].w1);
+                if (op_has_b(op)) touch(B.k_b[i]);
+            }
+            RawSeg seg;
+            std::vector<uint32_t> remap(nk, 0);
+            for (size_t i = 0; i < nk; ++i) {
+                if (!live[i]) continue;
+                remap[i] = (uint32_t)seg.ins.size();
+                seg.ins.push_back(B.k_ins[i]);
+                seg.b.push_back(B.k_b[i]);
+            }
+            for (size_t i = 0; i < seg.ins.size(); ++i) {
+                const uint32_t op = seg.ins[i].w0;
+                if (op_has_a(op) && (seg.ins[i].w1 & KTAG)) seg.ins[i].w1 = KTAG | remap[seg.ins[i].w1 & ~KTAG];
+                if (op_has_b(op) && (seg.b[i] & KTAG)) seg.b[i] = KTAG | remap[seg.b[i] & ~KTAG];
+            }
+            ksegs.push_back(std::move(seg));
+        }
+        if (ksegs.empty()) continue;
+        // ---- dead code in WJ
+        const size_t nw = B.wj_ins.size();
+        wj_live.resize(nw, 0);
+        for (size_t i = nw; i-- > 0;) {
+            if (!wj_live[i]) continue;
+            const uint32_t op = B.wj_ins[i].w0;
+            if (op_has_a(op)) wj_live[B.wj_ins[i].w1] = 1;
+            if (op_has_b(op)) wj_live[B.wj_b[i]] = 1;
+        }
+        std::vector<uint32_t> wremap(nw, 0);
+        Task task{};
+        task.j = (uint32_t)j;
+        task.wj_begin = (uint32_t)T->ins.size();
+        uint32_t nwj = 0;
+        for (size_t i = 0; i < nw; ++i) if (wj_live[i]) wremap[i] = nwj++;
+        task.wj_count = nwj;
+        // gradient rows: one per input coordinate this task reads
+        std::vector<int> grow(N, -1);
+        int n_grad = 0;
+        auto grad_row = [&](uint32_t g) { if (grow[g] < 0) grow[g] = n_grad++; return (uint32_t)grow[g]; };
+        auto is_input = [](uint32_t op) { return op == OP_BOX || op == OP_PT || op == OP_DELTA || op == OP_BOXMU || op == OP_DELTAMU; };
+        uint64_t cost = 0;
+        double flops = 0.0;
+        for (size_t i = 0; i < nw; ++i) {
+            if (!wj_live[i]) continue;
+            const uint32_t op = B.wj_ins[i].w0;
+            uint32_t a = B.wj_ins[i].w1, b = B.wj_b[i];
+            if (op_has_a(op)) a = wremap[a];
+            if (op_has_b(op)) b = wremap[b];
+            if (is_input(op)) b = grad_row(a);
+            T->ins.push_back(Ins{op | (a << 8), b});
+            ++cost; flops += op_flops(op);
+        }
+        task.seg_begin = (uint32_t)T->segs.size();
+        uint32_t max_k = 0;
+        for (auto& seg : ksegs) {
+            Seg sg{(uint32_t)T->ins.size(), (uint32_t)seg.ins.size()};
+            max_k = std::max(max_k, sg.count);
+            auto fix = [&](uint32_t s) { return (s & KTAG) ? nwj + (s & ~KTAG) : wremap[s]; };
+            for (size_t i = 0; i < seg.ins.size(); ++i) {
+                const uint32_t op = seg.ins[i].w0;
+                uint32_t a = seg.ins[i].w1, b = seg.b[i];
+                if (op_has_a(op)) a = fix(a);
+                if (op_has_b(op)) b = fix(b);
+                if (is_input(op)) b = grad_row(a);
+                T->ins.push_back(Ins{op | (a << 8), b});
+                ++cost; flops += op_flops(op);
+            }
+            T->segs.push_back(sg);
+        }
+        task.seg_count = (uint32_t)ksegs.size();
+        task.n_slots = nwj + max_k;
+        task.acc_base = acc_rows; task.n_acc = (uint32_t)n_acc;
+        task.grad_base = grad_rows; task.n_grad = (uint32_t)n_grad;
+        task.cost = (uint32_t)std::min<uint64_t>(cost, 0xffffffffu);
+        for (int l = 0; l < n; ++l) if (acc_of[l] >= 0) out_rows[l].push_back(acc_rows + (uint32_t)acc_of[l]);
+        for (int g = 0; g < N; ++g) if (grow[g] >= 0) var_rows[g].push_back(grad_rows + (uint32_t)grow[g]);
+        acc_rows += (uint32_t)n_acc;
+        grad_rows += (uint32_t)n_grad;
+        T->flops_fwd += flops;
+        T->ins_fwd += cost;
+        T->max_slots = std::max(T->max_slots, task.n_slots);
+        T->max_acc = std::max(T->max_acc, task.n_acc);
+        T->max_grad = std::max(T->max_grad, task.n_grad);
+        T->tasks.push_back(task);
+    }
+    T->acc_rows = acc_rows;
+    T->grad_rows = grad_rows;
+    T->out_ptr.assign(n + 1, 0);
+    T->out_rows.clear();
+    for (int l = 0; l < n; ++l) {
+        T->out_ptr[l] = (uint32_t)T->out_rows.size();
+        T->out_rows.insert(T->out_rows.end(), out_rows[l].begin(), out_rows[l].end());
+    }
+    T->out_ptr[n] = (uint32_t)T->out_rows.size();
+    T->var_ptr.assign(N + 1, 0);
+    T->var_rows.clear();
+    for (int g = 0; g < N; ++g) {
+        T->var_ptr[g] = (uint32_t)T->var_rows.size();
+        T->var_rows.insert(T->var_rows.end(), var_rows[g].begin(), var_rows[g].end());
+    }
+    T->var_ptr[N] = (uint32_t)T->var_rows.size();
+    // heavy tasks first (the device pulls tasks from a counter)
+    std::stable_sort(T->tasks.begin(), T->tasks.end(), [](const Task& a, const Task& b) { return a.cost > b.cost; });
+}
+
+}  // namespace leb_an

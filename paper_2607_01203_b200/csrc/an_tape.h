@@ -1,0 +1,98 @@
+// an_tape.h -- the interval tape of the analytic path (leb_analytic_fwd / leb_vjp kind 0).
+//
+// The path-based interval-Hessian bound (Thm 1, eq. (15)) needs, for every pair
+// j <= k of coordinates of a = [x; u], the enclosure [H_{l,kj}](A^(j)) of all outputs l over the prefix
+// box A^(j) (eq. (14)).  Reading R1 fixes the inclusion function: the natural
+// interval extension of second-order forward-mode AD of the model's straight-line program, every
+// SLP variable carrying the intervals (w, w_j, w_k, w_jk).
+//
+// Almost all of those jet components are STRUCTURALLY zero (config 4: 3.3e8 interval products per tile
+// if evaluated densely, 2e6 that are not identically zero), and 0 * x = 0, 0 + x = x, 1 * x = x hold
+// exactly under directed rounding.  So the model SLP is not evaluated by device code written per model:
+// at leb_set_analytic time the host evaluates it SYMBOLICALLY (an_compile.cu: every jet component is
+// `zero`, a constant, or a slot), emits only the interval operations that can be non-zero, removes what
+// no output reads, and hands the device a tape.  The tape of one path index j is
+//     segment WJ(j)  : the w and w_j components on A^(j)           (shared by every k >= j)
+//     segments K(j,k): the w_k, w_jk components and the terms [H_kj] D_j D_k of eq. (15)
+// in static single assignment form: instruction i of a segment writes slot (segment base + i).
+// The device (analytic.cu) is an interpreter of that tape, one (trajectory, timestep) tile per lane,
+// one (tile group, j) task per warp -- the tape is the same for every tile, so a warp never diverges --
+// and its reverse sweep (adjoint slots, branch selections re-derived from the stored primal values) is
+// the VJP.  No numerical step of the method runs on the host: the compiler handles structure only.
+#pragma once
+#include <stdint.h>
+#include <vector>
+
+namespace leb_an {
+
+enum Op : uint32_t {
+    OP_NOP = 0,
+    OP_BOX,      // d = [nom[a] - rad[a], nom[a] + rad[a]]   (25a) L272, mu = 0;   b = gradient row of the task
+    OP_PT,       // d = [nom[a], nom[a]]                      coordinates > j are pinned, L162
+    OP_DELTA,    // d = [-rad[a], rad[a]]                     D = A (-) a~, L164
+    OP_BOXMU,    // d = hull([nom + mu - rad, nom + mu + rad], nom)   non-centred box (25a), prefix hull (reading R4)
+    OP_DELTAMU,  // d = [mu[a] - rad[a], mu[a] + rad[a]]
+    OP_CONST,    // d = [c, c]                                b = float bits
+    OP_ADD,      // d = a + b
+    OP_SUB,      // d = a - b
+    OP_NEG,      // d = -a
+    OP_SCALE,    // d = c * a                                 b = float bits
+    OP_ADDC,     // d = a + c                                 b = float bits
+    OP_MUL,      // d = a * b       hull of the four endpoint products
+    OP_SQR,      // d = a^2 >= 0
+    OP_CUBE,     // d = a^3
+    OP_RECIP,    // d = 1 / a       domain error if 0 in a
+    OP_SIN,      // range-exact
+    OP_COS,
+    OP_OUT,      // acc[b & 0xffff] += a     (RD / RU);  b >> 16 = output index l (the VJP's cotangent)
+    OP_COUNT
+};
+
+struct Ins { uint32_t w0, w1; };   // w0 = op | a << 8 ; w1 = b (slot, float bits, or row)
+
+inline uint32_t ins_op(const Ins& i) { return i.w0 & 255u; }
+inline uint32_t ins_a(const Ins& i) { return i.w0 >> 8; }
+
+struct Seg { uint32_t begin, count; };          // instruction range in Tape::ins
+
+struct Task {                                    // one path index j
+    uint32_t j;
+    uint32_t wj_begin, wj_count;                 // segment WJ(j); its slots are [0, wj_count)
+    uint32_t seg_begin, seg_count;               // K segments (Tape::segs); their slots start at wj_count
+    uint32_t n_slots;                            // wj_count + longest K segment
+    uint32_t acc_base, n_acc;                    // rows of the partial-bound buffer (one per output this j touches)
+    uint32_t grad_base, n_grad;                  // rows of the partial-gradient buffer (one per input this j reads)
+    uint32_t cost;                               // instructions executed (forward)
+};
+
+// real FP32 operations per interval instruction (the algorithmic work the roofline counts; directed-rounding
+// add / mul / fma and min / max count one each, sin / cos / rcp one each)
+inline int op_flops(uint32_t op) {
+    switch (op) {
+        case OP_BOX: case OP_ADD: case OP_SUB: case OP_SCALE: case OP_ADDC: case OP_OUT: case OP_DELTAMU: return 2;
+        case OP_BOXMU: return 4;
+        case OP_MUL: return 14;
+        case OP_SQR: return 5;
+        case OP_CUBE: return 4;
+        case OP_RECIP: return 2;
+        case OP_SIN: case OP_COS: return 10;
+        default: return 0;
+    }
+}
+
+struct Tape {
+    int n = 0, N = 0;
+    std::vector<Ins> ins;
+    std::vector<Seg> segs;
+    std::vector<Task> tasks;                     // sorted by descending cost
+    // fixed-order reductions: bound l = sum of partial rows out_rows[out_ptr[l] .. out_ptr[l+1]) (ascending j)
+    std::vector<uint32_t> out_ptr, out_rows;
+    // gradient of input v = sum of partial-gradient rows var_rows[var_ptr[v] .. var_ptr[v+1])
+    std::vector<uint32_t> var_ptr, var_rows;
+    uint32_t acc_rows = 0, grad_rows = 0, max_slots = 0, max_acc = 0, max_grad = 0;
+    double flops_fwd = 0.0;                      // algorithmic FP32 operations per tile, forward
+    uint64_t ins_fwd = 0;                        // instructions executed per tile, forward
+    bool uses_mu = false;
+};
+
+}  // namespace leb_an

@@ -1,234 +1,586 @@
-// analytic.cu -- leb_analytic_fwd / leb_vjp(kind 0): path-based interval-Hessian bound
-// (Thm 1, eq. (15)) and its VJP, FP32 with directed rounding.
+// analytic.cu -- leb_analytic_fwd / leb_vjp(kind 0): path-based interval-Hessian bound (Thm 1, eq. (15),
+// PAPER.md:L164-167) and its VJP, as an interpreter of the interval tape of an_tape.h / an_compile.cu.
 //
-// Launch shape: one CTA per (tile, centre unit).  A tile is one (trajectory, timestep); a "unit"
-// is one quadrotor of the chain (1 for unicycle / quad12).  The CTA's work items are the pairs
-// (j <= k) of variables in the dependency cone of the unit; each thread evaluates, for its items,
-// the second-order interval jets of the unit's outputs over the prefix box A^(j) (steps A1-A2 of
-// SURVEY 8(a)) and folds H_kj D_j D_k into per-output partial sums (A3), which are combined by
-// directed-rounding warp shuffles.  Nothing but the 2N inputs and 2n outputs of a tile touches HBM.
-#include "an_core.cuh"
+// Work decomposition: a TASK is one path index j of the tape (its segment WJ(j) and its segments K(j,k));
+// a warp takes a (task, group of 32 tiles) work item from a counter, heavy tasks first.  Lane = tile: the tape is
+// the same for every tile, so a warp executes one instruction stream on 32 sets of intervals -- no divergence
+// except on data-dependent selections inside an instruction.  Slots live in a per-warp region of a global
+// workspace laid out [slot][lane] (256-byte coalesced accesses, L1/L2 resident while hot).  FP32 with directed
+// rounding throughout: lower endpoints round down, upper endpoints round up, sinf / cosf are padded by their
+// 2-ulp error bound, so every enclosure contains the exact-arithmetic enclosure of the same tape (steps A1-A3 of
+// SURVEY 8(a)).  A task leaves its partial sums of eq. (15) in a buffer; a second kernel adds the partial rows of
+// every output in ascending j with RD / RU (a fixed order: results are bitwise reproducible).
+//
+// VJP: the same forward sweep keeps every slot (SSA), then the tape is walked backwards with one adjoint per slot
+// endpoint; min / max / hull selections are re-derived from the stored primal values (ties -> the first candidate
+// in the order lo*lo, lo*hi, hi*lo, hi*hi; reading R20).  The K segments are run forward and backward one
+// at a time, their adjoints flowing into WJ(j)'s, which is reversed once at the end of the task.  Per-task input
+// adjoints go to a partial-gradient buffer and are summed in a fixed order as well.
+#include <new>
+#include "an_tape.h"
 #include "internal.h"
 
 namespace leb_an {
 
-constexpr int kThreads = 128;
-constexpr int kMaxVars = 64;
+constexpr int kWarpsPerBlock = 4;
+constexpr unsigned FULL = 0xffffffffu;
 
-__device__ __forceinline__ float shfl_add_dn(float v, int off) { return __fadd_rd(v, __shfl_xor_sync(0xffffffffu, v, off)); }
-__device__ __forceinline__ float shfl_add_up(float v, int off) { return __fadd_ru(v, __shfl_xor_sync(0xffffffffu, v, off)); }
+struct DevTape {
+    const uint2* ins;
+    const Seg* segs;
+    const Task* tasks;
+    const uint32_t *out_ptr, *out_rows, *var_ptr, *var_rows;
+    int ntasks, n, N;
+};
 
-// loads the tile's nominal point and radii into shared memory and validates them
-__device__ bool load_tile(const float* __restrict__ nom, const float* __restrict__ rad, int N, float* nom_s, float* rad_s) {
+struct VmArgs {
+    int tiles, ngroups, tiles_pad;
+    const float *nom, *rad, *mu;
+    int ld_in;
+    const float *g_lo, *g_hi;
+    int ld_out;
+    float2* partial;        // forward: [acc_rows][tiles_pad] (lo, hi); VJP: [grad_rows][tiles_pad] (nom_bar, rad_bar)
+    float* partial_mu;      // VJP with mu: [grad_rows][tiles_pad]
+    float2* ws;             // per-warp slot regions
+    size_t ws_stride;       // float2 elements per warp region
+    uint32_t adj_off, acc_off, gm_off;   // slot offsets inside a region: adjoint file; accumulator rows (forward) or
+                                         // (nom_bar, rad_bar) rows (VJP); (mu_bar, -) rows (VJP)
+    unsigned* counter;
+    int* tile_bad;
+};
+
+// ------------------------------------------------------------------ interval primitives (directed rounding)
+__device__ __forceinline__ float pad_dn(float s) { return fmaxf(-1.f, __fadd_rd(s, -(fabsf(s) * 3.0e-7f + 1e-30f))); }
+__device__ __forceinline__ float pad_up(float s) { return fminf(1.f, __fadd_ru(s, (fabsf(s) * 3.0e-7f + 1e-30f))); }
+// does [lo, hi] contain a point c + 2 pi k ?  (FP64 test with a tiny outward slack: when in doubt say yes,
+// which only widens the enclosure by O(slack^2))
+__device__ __forceinline__ bool contains_2pik(float lo, float hi, double c) {
+    const double INV_TWO_PI = 0.15915494309189533576888376337251;
+    double a = ((double)lo - c) * INV_TWO_PI - 1e-9, b = ((double)hi - c) * INV_TWO_PI + 1e-9;
+    return floor(b) >= ceil(a);
+}
+__device__ __forceinline__ float2 iv_mul(float2 a, float2 b) {
+    float lo = fminf(fminf(__fmul_rd(a.x, b.x), __fmul_rd(a.x, b.y)), fminf(__fmul_rd(a.y, b.x), __fmul_rd(a.y, b.y)));
+    float hi = fmaxf(fmaxf(__fmul_ru(a.x, b.x), __fmul_ru(a.x, b.y)), fmaxf(__fmul_ru(a.y, b.x), __fmul_ru(a.y, b.y)));
+    return make_float2(lo, hi);
+}
+__device__ __forceinline__ float2 iv_sqr(float2 a) {
+    if (a.x >= 0.f) return make_float2(__fmul_rd(a.x, a.x), __fmul_ru(a.y, a.y));
+    if (a.y <= 0.f) return make_float2(__fmul_rd(a.y, a.y), __fmul_ru(a.x, a.x));
+    return make_float2(0.f, fmaxf(__fmul_ru(a.x, a.x), __fmul_ru(a.y, a.y)));
+}
+// x^3 is increasing; for x < 0 the lower bound is -(up(|x|^3))
+__device__ __forceinline__ float cube_dn(float x) {
+    if (x >= 0.f) return __fmul_rd(__fmul_rd(x, x), x);
+    float m = -x;
+    return -__fmul_ru(__fmul_ru(m, m), m);
+}
+__device__ __forceinline__ float cube_up(float x) {
+    if (x >= 0.f) return __fmul_ru(__fmul_ru(x, x), x);
+    float m = -x;
+    return -__fmul_rd(__fmul_rd(m, m), m);
+}
+constexpr double HALF_PI = 1.5707963267948966192313216916398;
+constexpr double PI_D = 3.1415926535897932384626433832795;
+
+__device__ __forceinline__ float2 iv_sin(float2 a) {
+    const bool has_max = contains_2pik(a.x, a.y, HALF_PI), has_min = contains_2pik(a.x, a.y, -HALF_PI);
+    const float sl = sinf(a.x), sh = sinf(a.y);
+    return make_float2(has_min ? -1.f : fminf(pad_dn(sl), pad_dn(sh)), has_max ? 1.f : fmaxf(pad_up(sl), pad_up(sh)));
+}
+__device__ __forceinline__ float2 iv_cos(float2 a) {
+    const bool has_max = contains_2pik(a.x, a.y, 0.0), has_min = contains_2pik(a.x, a.y, PI_D);
+    const float cl = cosf(a.x), ch = cosf(a.y);
+    return make_float2(has_min ? -1.f : fminf(pad_dn(cl), pad_dn(ch)), has_max ? 1.f : fmaxf(pad_up(cl), pad_up(ch)));
+}
+
+__device__ __forceinline__ float as_f(uint32_t u) { return __uint_as_float(u); }
+
+// ------------------------------------------------------------------ forward sweep of one segment
+// S: slot file of this lane (slot s at S[s * 32]); dst0: slot of the segment's first instruction.
+// VJP: the adjoint slot is cleared as the primal one is written and OUT does nothing.
+template <bool VJP>
+__device__ __forceinline__ void run_fwd(const uint2* __restrict__ ins, uint32_t begin, uint32_t count, uint32_t dst0,
+                                        float2* __restrict__ S, const VmArgs& A, const float* __restrict__ nom,
+                                        const float* __restrict__ rad, const float* __restrict__ mu, bool& bad, int lane) {
+    float2* ADJ = S + (size_t)A.adj_off * 32;
+    float2* ACC = S + (size_t)A.acc_off * 32;
+    float2 prev = make_float2(0.f, 0.f);
+    uint32_t dst = dst0;
+    for (uint32_t base = 0; base < count; base += 32) {
+        uint2 mine = make_uint2(0u, 0u);
+        if (base + lane < count) mine = __ldg(ins + begin + base + lane);
+        const int m = min(32u, count - base);
+        for (int i = 0; i < m; ++i, ++dst) {
+            const uint32_t w0 = __shfl_sync(FULL, mine.x, i), w1 = __shfl_sync(FULL, mine.y, i);
+            const uint32_t op = w0 & 255u, a = w0 >> 8;
+            float2 r, x;
+            if (op >= OP_ADD) x = (a + 1 == dst && dst != dst0) ? prev : S[(size_t)a * 32];
+            switch (op) {
+                case OP_BOX: { float c = nom[a], s = rad[a]; r = make_float2(__fadd_rd(c, -s), __fadd_ru(c, s)); break; }
+                case OP_PT: { float c = nom[a]; r = make_float2(c, c); break; }
+                case OP_DELTA: { float s = rad[a]; r = make_float2(-s, s); break; }
+                case OP_BOXMU: {   // hull of [c + mu - s, c + mu + s] and {c}: the segment from a~ to a point of the box
+                    float c = nom[a], s = rad[a], u = mu[a];
+                    r = make_float2(__fadd_rd(c, fminf(__fadd_rd(u, -s), 0.f)), __fadd_ru(c, fmaxf(__fadd_ru(u, s), 0.f)));
+                    break;
+                }
+                case OP_DELTAMU: { float s = rad[a], u = mu[a]; r = make_float2(__fadd_rd(u, -s), __fadd_ru(u, s)); break; }
+                case OP_CONST: { float c = as_f(w1); r = make_float2(c, c); break; }
+                case OP_ADD: { float2 y = S[(size_t)w1 * 32]; r = make_float2(__fadd_rd(x.x, y.x), __fadd_ru(x.y, y.y)); break; }
+                case OP_SUB: { float2 y = S[(size_t)w1 * 32]; r = make_float2(__fadd_rd(x.x, -y.y), __fadd_ru(x.y, -y.x)); break; }
+                case OP_NEG: r = make_float2(-x.y, -x.x); break;
+                case OP_SCALE: {
+                    float c = as_f(w1);
+                    r = c >= 0.f ? make_float2(__fmul_rd(c, x.x), __fmul_ru(c, x.y)) : make_float2(__fmul_rd(c, x.y), __fmul_ru(c, x.x));
+                    break;
+                }
+                case OP_ADDC: { float c = as_f(w1); r = make_float2(__fadd_rd(x.x, c), __fadd_ru(x.y, c)); break; }
+                case OP_MUL: { float2 y = (w1 + 1 == dst && dst != dst0) ? prev : S[(size_t)w1 * 32]; r = iv_mul(x, y); break; }
+                case OP_SQR: r = iv_sqr(x); break;
+                case OP_CUBE: r = make_float2(cube_dn(x.x), cube_up(x.y)); break;
+                case OP_RECIP:
+                    if (x.x <= 0.f && x.y >= 0.f) { bad = true; r = make_float2(1.f, 1.f); }
+                    else r = make_float2(__frcp_rd(x.y), __frcp_ru(x.x));
+                    break;
+                case OP_SIN: r = iv_sin(x); break;
+                case OP_COS: r = iv_cos(x); break;
+                case OP_OUT:
+                    r = x;
+                    if (!VJP) {
+                        float2* p = ACC + (size_t)(w1 & 0xffffu) * 32;
+                        float2 c = *p;
+                        *p = make_float2(__fadd_rd(c.x, x.x), __fadd_ru(c.y, x.y));
+                    }
+                    break;
+                default: r = make_float2(0.f, 0.f); break;
+            }
+            if (op != OP_OUT) S[(size_t)dst * 32] = r;
+            if (VJP) ADJ[(size_t)dst * 32] = make_float2(0.f, 0.f);
+            prev = r;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ reverse sweep of one segment
+__device__ __forceinline__ void adj_add(float2* p, float dl, float dh) { float2 v = *p; v.x += dl; v.y += dh; *p = v; }
+
+__device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t begin, uint32_t count, uint32_t dst0,
+                                        float2* __restrict__ S, const VmArgs& A, const float* __restrict__ rad,
+                                        const float* __restrict__ mu, const float* __restrict__ g_lo,
+                                        const float* __restrict__ g_hi, int lane) {
+    float2* ADJ = S + (size_t)A.adj_off * 32;
+    float2* G0 = S + (size_t)A.acc_off * 32;                 // (nom_bar, rad_bar) per gradient row
+    float2* GM = S + (size_t)A.gm_off * 32;                  // (mu_bar, -) per gradient row
+    if (count == 0) return;
+    for (int base = (int)((count - 1) / 32) * 32; base >= 0; base -= 32) {
+        uint2 mine = make_uint2(0u, 0u);
+        if ((uint32_t)base + lane < count) mine = __ldg(ins + begin + base + lane);
+        const int m = min(32u, count - (uint32_t)base);
+        for (int i = m - 1; i >= 0; --i) {
+            const uint32_t w0 = __shfl_sync(FULL, mine.x, i), w1 = __shfl_sync(FULL, mine.y, i);
+            const uint32_t op = w0 & 255u, a = w0 >> 8;
+            const uint32_t dst = dst0 + (uint32_t)base + (uint32_t)i;
+            if (op == OP_OUT) {
+                const uint32_t l = w1 >> 16;
+                adj_add(ADJ + (size_t)a * 32, g_lo[l], g_hi[l]);
+                continue;
+            }
+            const float2 d = ADJ[(size_t)dst * 32];
+            const float dl = d.x, dh = d.y;
+            if (dl == 0.f && dh == 0.f) continue;
+            switch (op) {
+                case OP_BOX: adj_add(G0 + (size_t)w1 * 32, dl + dh, dh - dl); break;
+                case OP_PT: adj_add(G0 + (size_t)w1 * 32, dl + dh, 0.f); break;
+                case OP_DELTA: adj_add(G0 + (size_t)w1 * 32, 0.f, dh - dl); break;
+                case OP_BOXMU: {
+                    // lo = c + min(mu - s, 0), hi = c + max(mu + s, 0); ties keep the first candidate
+                    const float s = rad[a], u = mu[a];
+                    const float fl = (0.f < __fadd_rd(u, -s)) ? 0.f : dl, fh = (0.f > __fadd_ru(u, s)) ? 0.f : dh;
+                    adj_add(G0 + (size_t)w1 * 32, dl + dh, fh - fl);
+                    adj_add(GM + (size_t)w1 * 32, fl + fh, 0.f);
+                    break;
+                }
+                case OP_DELTAMU:
+                    adj_add(G0 + (size_t)w1 * 32, 0.f, dh - dl);
+                    adj_add(GM + (size_t)w1 * 32, dl + dh, 0.f);
+                    break;
+                case OP_ADD: adj_add(ADJ + (size_t)a * 32, dl, dh); adj_add(ADJ + (size_t)w1 * 32, dl, dh); break;
+                case OP_SUB: adj_add(ADJ + (size_t)a * 32, dl, dh); adj_add(ADJ + (size_t)w1 * 32, -dh, -dl); break;
+                case OP_NEG: adj_add(ADJ + (size_t)a * 32, -dh, -dl); break;
+                case OP_SCALE: {
+                    const float c = as_f(w1);
+                    if (c >= 0.f) adj_add(ADJ + (size_t)a * 32, c * dl, c * dh);
+                    else adj_add(ADJ + (size_t)a * 32, c * dh, c * dl);
+                    break;
+                }
+                case OP_ADDC: adj_add(ADJ + (size_t)a * 32, dl, dh); break;
+                case OP_MUL: {
+                    const float2 x = S[(size_t)a * 32], y = S[(size_t)w1 * 32];
+                    // lower endpoint: first minimum of (xl yl, xl yh, xh yl, xh yh), products rounded down as in the forward
+                    float best = __fmul_rd(x.x, y.x); int sl = 0;
+                    float p = __fmul_rd(x.x, y.y); if (p < best) { best = p; sl = 1; }
+                    p = __fmul_rd(x.y, y.x); if (p < best) { best = p; sl = 2; }
+                    p = __fmul_rd(x.y, y.y); if (p < best) { best = p; sl = 3; }
+                    best = __fmul_ru(x.x, y.x); int sh = 0;
+                    p = __fmul_ru(x.x, y.y); if (p > best) { best = p; sh = 1; }
+                    p = __fmul_ru(x.y, y.x); if (p > best) { best = p; sh = 2; }
+                    p = __fmul_ru(x.y, y.y); if (p > best) { best = p; sh = 3; }
+                    const float xs_l = (sl & 2) ? x.y : x.x, ys_l = (sl & 1) ? y.y : y.x;
+                    const float xs_h = (sh & 2) ? x.y : x.x, ys_h = (sh & 1) ? y.y : y.x;
+                    float2 ax = make_float2(0.f, 0.f), ay = make_float2(0.f, 0.f);
+                    if (sl & 2) ax.y += dl * ys_l; else ax.x += dl * ys_l;
+                    if (sl & 1) ay.y += dl * xs_l; else ay.x += dl * xs_l;
+                    if (sh & 2) ax.y += dh * ys_h; else ax.x += dh * ys_h;
+                    if (sh & 1) ay.y += dh * xs_h; else ay.x += dh * xs_h;
+                    adj_add(ADJ + (size_t)a * 32, ax.x, ax.y);
+                    adj_add(ADJ + (size_t)w1 * 32, ay.x, ay.y);
+                    break;
+                }
+                case OP_SQR: {
+                    const float2 x = S[(size_t)a * 32];
+                    if (x.x >= 0.f) adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dl, 2.f * x.y * dh);
+                    else if (x.y <= 0.f) adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dh, 2.f * x.y * dl);
+                    else if (__fmul_ru(x.y, x.y) > __fmul_ru(x.x, x.x)) adj_add(ADJ + (size_t)a * 32, 0.f, 2.f * x.y * dh);
+                    else adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dh, 0.f);
+                    break;
+                }
+                case OP_CUBE: {
+                    const float2 x = S[(size_t)a * 32];
+                    adj_add(ADJ + (size_t)a * 32, 3.f * x.x * x.x * dl, 3.f * x.y * x.y * dh);
+                    break;
+                }
+                case OP_RECIP: {
+                    const float2 r = S[(size_t)dst * 32];          // (1/hi, 1/lo)
+                    adj_add(ADJ + (size_t)a * 32, -dh * r.y * r.y, -dl * r.x * r.x);
+                    break;
+                }
+                case OP_SIN: {
+                    const float2 x = S[(size_t)a * 32];
+                    const bool has_max = contains_2pik(x.x, x.y, HALF_PI), has_min = contains_2pik(x.x, x.y, -HALF_PI);
+                    const float sl = sinf(x.x), sh = sinf(x.y);
+                    float al = 0.f, ah = 0.f;
+                    if (!has_min) { if (pad_dn(sh) < pad_dn(sl)) ah += cosf(x.y) * dl; else al += cosf(x.x) * dl; }
+                    if (!has_max) { if (pad_up(sh) > pad_up(sl)) ah += cosf(x.y) * dh; else al += cosf(x.x) * dh; }
+                    adj_add(ADJ + (size_t)a * 32, al, ah);
+                    break;
+                }
+                case OP_COS: {
+                    const float2 x = S[(size_t)a * 32];
+                    const bool has_max = contains_2pik(x.x, x.y, 0.0), has_min = contains_2pik(x.x, x.y, PI_D);
+                    const float cl = cosf(x.x), ch = cosf(x.y);
+                    float al = 0.f, ah = 0.f;
+                    if (!has_min) { if (pad_dn(ch) < pad_dn(cl)) ah -= sinf(x.y) * dl; else al -= sinf(x.x) * dl; }
+                    if (!has_max) { if (pad_up(ch) > pad_up(cl)) ah -= sinf(x.y) * dh; else al -= sinf(x.x) * dh; }
+                    adj_add(ADJ + (size_t)a * 32, al, ah);
+                    break;
+                }
+                default: break;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------ the interpreter kernel
+template <bool VJP>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32) an_vm_kernel(DevTape P, VmArgs A) {
+    const int lane = threadIdx.x & 31;
+    const size_t wid = (size_t)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+    float2* S = A.ws + wid * A.ws_stride + lane;
+    const unsigned nwork = (unsigned)P.ntasks * (unsigned)A.ngroups;
+    for (;;) {
+        unsigned t = 0;
+        if (lane == 0) t = atomicAdd(A.counter, 1u);
+        t = __shfl_sync(FULL, t, 0);
+        if (t >= nwork) break;
+        const Task tk = P.tasks[t / A.ngroups];
+        const int tile = (int)(t % A.ngroups) * 32 + lane;
+        const bool valid = tile < A.tiles;
+        const size_t row = (size_t)(valid ? tile : A.tiles - 1);
+        const float* nom = A.nom + row * A.ld_in;
+        const float* rad = A.rad + row * A.ld_in;
+        const float* mu = A.mu ? A.mu + row * A.ld_in : nullptr;
+        bool bad = false;
+        if (!VJP) {
+            float2* ACC = S + (size_t)A.acc_off * 32;
+            for (uint32_t r = 0; r < tk.n_acc; ++r) ACC[(size_t)r * 32] = make_float2(0.f, 0.f);
+            run_fwd<false>(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, nom, rad, mu, bad, lane);
+            for (uint32_t q = 0; q < tk.seg_count; ++q) {
+                const Seg sg = P.segs[tk.seg_begin + q];
+                run_fwd<false>(P.ins, sg.begin, sg.count, tk.wj_count, S, A, nom, rad, mu, bad, lane);
+            }
+            if (valid)
+                for (uint32_t r = 0; r < tk.n_acc; ++r) A.partial[(size_t)(tk.acc_base + r) * A.tiles_pad + tile] = ACC[(size_t)r * 32];
+        } else {
+            float2* G0 = S + (size_t)A.acc_off * 32;
+            float2* GM = S + (size_t)A.gm_off * 32;
+            const float* g_lo = A.g_lo + row * A.ld_out;
+            const float* g_hi = A.g_hi + row * A.ld_out;
+            for (uint32_t r = 0; r < tk.n_grad; ++r) { G0[(size_t)r * 32] = make_float2(0.f, 0.f); GM[(size_t)r * 32] = make_float2(0.f, 0.f); }
+            run_fwd<true>(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, nom, rad, mu, bad, lane);
+            for (uint32_t q = 0; q < tk.seg_count; ++q) {
+                const Seg sg = P.segs[tk.seg_begin + q];
+                run_fwd<true>(P.ins, sg.begin, sg.count, tk.wj_count, S, A, nom, rad, mu, bad, lane);
+                run_bwd(P.ins, sg.begin, sg.count, tk.wj_count, S, A, rad, mu, g_lo, g_hi, lane);
+            }
+            run_bwd(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, rad, mu, g_lo, g_hi, lane);
+            if (valid)
+                for (uint32_t r = 0; r < tk.n_grad; ++r) {
+                    A.partial[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = G0[(size_t)r * 32];
+                    if (A.partial_mu) A.partial_mu[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = GM[(size_t)r * 32].x;
+                }
+        }
+        if (bad && valid) A.tile_bad[tile] = 1;
+    }
+}
+
+// ------------------------------------------------------------------ fixed-order reductions over the tasks
+// one block per tile: validates the tile's inputs, then thread l adds the partial rows of output l in ascending j
+__global__ void an_reduce_fwd_kernel(DevTape P, int tiles_pad, const float* __restrict__ nom, const float* __restrict__ rad,
+                                     const float* __restrict__ mu, int ld_in, const float2* __restrict__ partial,
+                                     const int* __restrict__ tile_bad, float* __restrict__ r_lo, float* __restrict__ r_hi,
+                                     int ld_out, int* __restrict__ domain_flag) {
+    const int tile = blockIdx.x;
     int bad = 0;
-    for (int g = threadIdx.x; g < N; g += blockDim.x) {
-        float a = nom[g], s = rad[g];
-        nom_s[g] = a;
-        rad_s[g] = s;
+    for (int g = threadIdx.x; g < P.N; g += blockDim.x) {
+        const float a = nom[(size_t)tile * ld_in + g], s = rad[(size_t)tile * ld_in + g];
         if (!(fabsf(a) <= 3.0e38f) || !(s >= 0.f) || !(s <= 3.0e38f)) bad = 1;
+        if (mu) { const float u = mu[(size_t)tile * ld_in + g]; if (!(fabsf(u) <= 3.0e38f)) bad = 1; }
     }
-    return __syncthreads_or(bad) != 0;
-}
-
-// ---------------------------------------------------------------------------------------------
-// forward
-// ---------------------------------------------------------------------------------------------
-template <int NOUT, bool UNICYCLE>
-__global__ void __launch_bounds__(kThreads)
-analytic_fwd_kernel(Model M, const float* __restrict__ nom, const float* __restrict__ rad, int ld_in,
-                    float* __restrict__ r_lo, float* __restrict__ r_hi, int ld_out, int* __restrict__ domain_flag) {
-    extern __shared__ float smem[];
-    float* nom_s = smem;
-    float* rad_s = smem + M.N;
-    __shared__ int vars[kMaxVars];
-    __shared__ int nvars;
-    __shared__ float red_lo[kThreads / 32][NOUT], red_hi[kThreads / 32][NOUT];
-
-    const int tile = blockIdx.y, unit = blockIdx.x;
-    bool bad = load_tile(nom + (size_t)tile * ld_in, rad + (size_t)tile * ld_in, M.N, nom_s, rad_s);
-    if (threadIdx.x == 0) {
-        if (UNICYCLE) { for (int g = 0; g < 5; ++g) vars[g] = g; nvars = 5; }
-        else nvars = window_vars(M, unit, vars);
-    }
-    __syncthreads();
-    const int L = nvars, nitems = L * (L + 1) / 2;
-
-    Iv<float> R[NOUT];
-#pragma unroll
-    for (int l = 0; l < NOUT; ++l) R[l] = iconst<float>(0.f);
-    bool dom = false;
-    if (!bad) {
-        for (int t = threadIdx.x; t < nitems; t += blockDim.x) {
-            int a, b;
-            item_decode(t, L, &a, &b);
-            Inputs<float> in{nom_s, rad_s, vars[a], vars[b]};
-            Jet<float> f[NOUT];
-            if (UNICYCLE) unicycle_f(M, in, f);
-            else chain_center_f(M, in, unit, f, &dom);
-#pragma unroll
-            for (int l = 0; l < NOUT; ++l)
-                R[l] = iadd(R[l], item_term(f[l].wjk, rad_s[in.j], rad_s[in.k], in.j == in.k));
+    bad = __syncthreads_or(bad | (threadIdx.x == 0 ? tile_bad[tile] : 0));
+    for (int l = threadIdx.x; l < P.n; l += blockDim.x) {
+        float lo = 0.f, hi = 0.f;
+        for (uint32_t q = P.out_ptr[l]; q < P.out_ptr[l + 1]; ++q) {
+            const float2 v = partial[(size_t)P.out_rows[q] * tiles_pad + tile];
+            lo = __fadd_rd(lo, v.x);
+            hi = __fadd_ru(hi, v.y);
         }
-    }
-    bad = (__syncthreads_or((int)dom) != 0) || bad;
-    // directed-rounding reduction: lanes -> warps -> thread l
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int l = 0; l < NOUT; ++l) {
-        float lo = R[l].lo, hi = R[l].hi;
-#pragma unroll
-        for (int off = 16; off; off >>= 1) { lo = shfl_add_dn(lo, off); hi = shfl_add_up(hi, off); }
-        if (lane == 0) { red_lo[warp][l] = lo; red_hi[warp][l] = hi; }
-    }
-    __syncthreads();
-    if (threadIdx.x < NOUT) {
-        float lo = red_lo[0][threadIdx.x], hi = red_hi[0][threadIdx.x];
-        for (int w = 1; w < kThreads / 32; ++w) { lo = __fadd_rd(lo, red_lo[w][threadIdx.x]); hi = __fadd_ru(hi, red_hi[w][threadIdx.x]); }
         if (bad) { lo = -INFINITY; hi = INFINITY; }
-        size_t o = (size_t)tile * ld_out + (size_t)unit * NOUT + threadIdx.x;
-        r_lo[o] = lo;
-        r_hi[o] = hi;
+        r_lo[(size_t)tile * ld_out + l] = lo;
+        r_hi[(size_t)tile * ld_out + l] = hi;
     }
     if (bad && threadIdx.x == 0) atomicExch(domain_flag, 1);
 }
 
-// ---------------------------------------------------------------------------------------------
-// VJP by forward-mode duals: work unit = (item, direction); direction = (window variable, nom|rad)
-// ---------------------------------------------------------------------------------------------
-struct DuArr {   // presents a float array as duals with a unit tangent at one index
-    const float* a;
-    int seed;
-    __device__ __forceinline__ Du operator[](int g) const { return Du{a[g], g == seed ? 1.f : 0.f}; }
-};
-template <> struct Inputs<Du> {
-    DuArr nom, rad;
-    int j, k;
-    __device__ __forceinline__ Jet<Du> operator()(int g) const {
-        Jet<Du> r;
-        if (g <= j) r.w = {add_dn(nom[g], neg(rad[g])), add_up(nom[g], rad[g])};
-        else r.w = {nom[g], nom[g]};
-        r.wj = iconst<Du>(g == j ? 1.f : 0.f);
-        r.wk = iconst<Du>(g == k ? 1.f : 0.f);
-        r.wjk = iconst<Du>(0.f);
-        return r;
+__global__ void an_reduce_vjp_kernel(DevTape P, int tiles_pad, const float* __restrict__ nom, const float* __restrict__ rad,
+                                     const float* __restrict__ mu, int ld_in, const float2* __restrict__ partial,
+                                     const float* __restrict__ partial_mu, const int* __restrict__ tile_bad,
+                                     float* __restrict__ grad_nom, float* __restrict__ grad_rad, float* __restrict__ grad_mu,
+                                     int* __restrict__ domain_flag) {
+    const int tile = blockIdx.x;
+    int bad = 0;
+    for (int g = threadIdx.x; g < P.N; g += blockDim.x) {
+        const float a = nom[(size_t)tile * ld_in + g], s = rad[(size_t)tile * ld_in + g];
+        if (!(fabsf(a) <= 3.0e38f) || !(s >= 0.f) || !(s <= 3.0e38f)) bad = 1;
+        if (mu) { const float u = mu[(size_t)tile * ld_in + g]; if (!(fabsf(u) <= 3.0e38f)) bad = 1; }
     }
-};
-
-template <int NOUT, bool UNICYCLE>
-__global__ void __launch_bounds__(kThreads)
-analytic_vjp_kernel(Model M, const float* __restrict__ nom, const float* __restrict__ rad,
-                    const float* __restrict__ g_lo, const float* __restrict__ g_hi, int ld_in, int ld_out,
-                    float* __restrict__ grad_nom, float* __restrict__ grad_rad, int* __restrict__ domain_flag) {
-    extern __shared__ float smem[];
-    float* nom_s = smem;
-    float* rad_s = smem + M.N;
-    __shared__ int vars[kMaxVars];
-    __shared__ int nvars;
-    __shared__ float gl_s[NOUT], gh_s[NOUT];
-    __shared__ float grad_s[2 * kMaxVars];
-    __shared__ int rad_off[kMaxVars + 1];      // prefix counts of the radius work units per item row a
-
-    const int tile = blockIdx.y, unit = blockIdx.x;
-    bool bad = load_tile(nom + (size_t)tile * ld_in, rad + (size_t)tile * ld_in, M.N, nom_s, rad_s);
-    if (threadIdx.x == 0) {
-        if (UNICYCLE) { for (int g = 0; g < 5; ++g) vars[g] = g; nvars = 5; }
-        else nvars = window_vars(M, unit, vars);
-    }
-    if (threadIdx.x < NOUT) {
-        size_t o = (size_t)tile * ld_out + (size_t)unit * NOUT + threadIdx.x;
-        gl_s[threadIdx.x] = g_lo[o];
-        gh_s[threadIdx.x] = g_hi[o];
-    }
-    for (int d = threadIdx.x; d < 2 * kMaxVars; d += blockDim.x) grad_s[d] = 0.f;
-    __syncthreads();
-    const int L = nvars, nitems = L * (L + 1) / 2, ndirs = 2 * L;
-    // Work units.  Every item (a <= b) needs all L nominal directions.  A RADIUS direction p matters only if the box of the
-    // item depends on sigma_p -- positions p <= a of the prefix box A^(j) (Thm 1: coordinates after j are pinned at the
-    // nominal point, L162) -- or if sigma_p is one of the explicit factors (p == b; p == a is already counted): for every
-    // other p the tangent is identically zero, so those (item, direction) pairs are not enumerated at all
-    // (L = 54: 109 341 units instead of 160 380).  Row a of the item table has L - a items, each with a + 1 box directions.
-    if (threadIdx.x == 0) {
-        int acc = 0;
-        for (int a = 0; a < L; ++a) { rad_off[a] = acc; acc += (L - a) * (a + 1); }
-        rad_off[L] = acc;
-    }
-    __syncthreads();
-    const int n_nom = nitems * L, n_box = rad_off[L], n_fac = nitems - L;      // n_fac: off-diagonal items, direction p == b
-    bool dom = false;
-    if (!bad) {
-        const int nwork = n_nom + n_box + n_fac;
-        for (int w = threadIdx.x; w < nwork; w += blockDim.x) {
-            int a, b, d;                       // item (a, b) and direction d in [0, 2L): nominal d, radius L + position
-            if (w < n_nom) {
-                const int t = w / L;
-                d = w - t * L;
-                item_decode(t, L, &a, &b);
-            } else if (w < n_nom + n_box) {
-                const int r = w - n_nom;
-                int lo = 0, hi = L - 1;        // largest a with rad_off[a] <= r
-                while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (rad_off[mid] <= r) lo = mid; else hi = mid - 1; }
-                a = lo;
-                const int rem = r - rad_off[a], p = rem / (L - a);
-                b = a + (rem - p * (L - a));
-                d = L + p;
-            } else {
-                item_decode_offdiag(w - n_nom - n_box, L, &a, &b);
-                d = L + b;
-            }
-            const int j = vars[a], k = vars[b];
-            const int dvar = vars[d < L ? d : d - L];
-            Inputs<Du> in{DuArr{nom_s, d < L ? dvar : -1}, DuArr{rad_s, d < L ? -1 : dvar}, j, k};
-            Jet<Du> f[NOUT];
-            if (UNICYCLE) unicycle_f(M, in, f);
-            else chain_center_f(M, in, unit, f, &dom);
-            float acc = 0.f;
-#pragma unroll
-            for (int l = 0; l < NOUT; ++l) {
-                Iv<Du> term = item_term(f[l].wjk, in.rad[j], in.rad[k], j == k);
-                acc = fmaf(gh_s[l], term.hi.d, acc);
-                acc = fmaf(gl_s[l], term.lo.d, acc);
-            }
-            atomicAdd(&grad_s[d], acc);
+    bad = __syncthreads_or(bad | (threadIdx.x == 0 ? tile_bad[tile] : 0));
+    for (int g = threadIdx.x; g < P.N; g += blockDim.x) {
+        float gn = 0.f, gr = 0.f, gm = 0.f;
+        for (uint32_t q = P.var_ptr[g]; q < P.var_ptr[g + 1]; ++q) {
+            const size_t o = (size_t)P.var_rows[q] * tiles_pad + tile;
+            const float2 v = partial[o];
+            gn += v.x;
+            gr += v.y;
+            if (partial_mu) gm += partial_mu[o];
         }
-    }
-    bad = (__syncthreads_or((int)dom) != 0) || bad;
-    for (int d = threadIdx.x; d < ndirs; d += blockDim.x) {
-        float v = bad ? NAN : grad_s[d];
-        int var = vars[d < L ? d : d - L];
-        float* dst = (d < L ? grad_nom : grad_rad) + (size_t)tile * ld_in + var;
-        atomicAdd(dst, v);
+        if (bad) { gn = NAN; gr = NAN; gm = NAN; }
+        grad_nom[(size_t)tile * ld_in + g] = gn;
+        grad_rad[(size_t)tile * ld_in + g] = gr;
+        if (grad_mu) grad_mu[(size_t)tile * ld_in + g] = gm;
     }
     if (bad && threadIdx.x == 0) atomicExch(domain_flag, 1);
-}
-
-// zero the first N columns of [tiles, ld] rows
-__global__ void zero_rows_kernel(float* __restrict__ a, float* __restrict__ b, int tiles, int N, int ld) {
-    size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    size_t total = (size_t)tiles * N;
-    if (idx < total) {
-        size_t t = idx / N, c = idx - t * N;
-        a[t * ld + c] = 0.f;
-        b[t * ld + c] = 0.f;
-    }
 }
 
 }  // namespace leb_an
 
+// ============================================================================================== host side
 using namespace leb_an;
+
+struct AnState {
+    bool ready = false;
+    Model model{};
+    Tape tape[2];                 // [0] centred boxes, [1] non-centred (mu != NULL), compiled on first use
+    bool have[2] = {false, false};
+    DevTape dev[2]{};
+    std::vector<void*> tape_allocs[2];
+    // buffers grown on demand
+    float2* ws = nullptr; size_t ws_bytes = 0;
+    float2* partial = nullptr; size_t partial_bytes = 0;
+    float* partial_mu = nullptr; size_t partial_mu_bytes = 0;
+    int* tile_bad = nullptr; size_t tile_bad_n = 0;
+    unsigned* counter = nullptr;
+    int num_sms = 148;
+};
+
+AnState* leb_an_create() {
+    AnState* S = new (std::nothrow) AnState();
+    if (!S) return nullptr;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&S->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    return S;
+}
+
+static void free_tape(AnState* S, int v) {
+    for (void* p : S->tape_allocs[v]) cudaFree(p);
+    S->tape_allocs[v].clear();
+    S->have[v] = false;
+}
+
+void leb_an_destroy(AnState* S) {
+    if (!S) return;
+    free_tape(S, 0); free_tape(S, 1);
+    if (S->ws) cudaFree(S->ws);
+    if (S->partial) cudaFree(S->partial);
+    if (S->partial_mu) cudaFree(S->partial_mu);
+    if (S->tile_bad) cudaFree(S->tile_bad);
+    if (S->counter) cudaFree(S->counter);
+    delete S;
+}
+
+bool leb_an_ready(const AnState* S) { return S && S->ready; }
+int leb_an_n(const AnState* S) { return S->model.n; }
+int leb_an_N(const AnState* S) { return S->model.N; }
+
+template <class T>
+static bool upload(AnState* S, int v, const std::vector<T>& h, const T** d) {
+    void* p = nullptr;
+    const size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
+    if (cudaMalloc(&p, bytes) != cudaSuccess) return false;
+    S->tape_allocs[v].push_back(p);
+    if (!h.empty() && cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+    *d = (const T*)p;
+    return true;
+}
+
+static leb_status ensure_tape(AnState* S, int v) {
+    if (S->have[v]) return LEB_OK;
+    Tape& T = S->tape[v];
+    leb_compile_tape(S->model, v == 1, &T);
+    DevTape& D = S->dev[v];
+    const uint2* ins = nullptr;
+    static_assert(sizeof(Ins) == sizeof(uint2), "Ins is two words");
+    std::vector<uint2> raw(T.ins.size());
+    for (size_t i = 0; i < T.ins.size(); ++i) raw[i] = make_uint2(T.ins[i].w0, T.ins[i].w1);
+    bool ok = upload(S, v, raw, &ins) && upload(S, v, T.segs, &D.segs) && upload(S, v, T.tasks, &D.tasks) &&
+              upload(S, v, T.out_ptr, &D.out_ptr) && upload(S, v, T.out_rows, &D.out_rows) &&
+              upload(S, v, T.var_ptr, &D.var_ptr) && upload(S, v, T.var_rows, &D.var_rows);
+    if (!ok) { free_tape(S, v); return LEB_ERR_NOMEM; }
+    D.ins = ins;
+    D.ntasks = (int)T.tasks.size();
+    D.n = T.n; D.N = T.N;
+    S->have[v] = true;
+    return LEB_OK;
+}
+
+leb_status leb_an_set_model(AnState* S, const Model& M) {
+    free_tape(S, 0); free_tape(S, 1);
+    S->model = M;
+    S->ready = true;
+    if (!S->counter && cudaMalloc(&S->counter, sizeof(unsigned)) != cudaSuccess) return LEB_ERR_NOMEM;
+    return ensure_tape(S, 0);
+}
+
+template <class T>
+static bool grow(T** p, size_t* have, size_t need_bytes) {
+    if (*have >= need_bytes) return true;
+    if (*p) { cudaDeviceSynchronize(); cudaFree(*p); *p = nullptr; *have = 0; }
+    if (cudaMalloc((void**)p, need_bytes) != cudaSuccess) return false;
+    *have = need_bytes;
+    return true;
+}
+
+void leb_an_stats(const AnState* S, double* flops_fwd, long long* ins_fwd, long long* tape_ins, int* ntasks, int* max_slots) {
+    const Tape& T = S->tape[0];
+    *flops_fwd = T.flops_fwd; *ins_fwd = (long long)T.ins_fwd; *tape_ins = (long long)T.ins.size();
+    *ntasks = (int)T.tasks.size(); *max_slots = (int)T.max_slots;
+}
+
+// forward (g_lo == NULL) or VJP
+static leb_status an_run(AnState* S, bool vjp, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                         float* r_lo, float* r_hi, const float* g_lo, const float* g_hi, int ld_out, float* grad_nom,
+                         float* grad_rad, float* grad_mu, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
+    if (tiles == 0) return LEB_OK;
+    const int v = mu ? 1 : 0;
+    leb_status es = ensure_tape(S, v);
+    if (es != LEB_OK) return es;
+    const Tape& T = S->tape[v];
+    const DevTape& D = S->dev[v];
+    VmArgs A{};
+    A.tiles = tiles; A.ngroups = (tiles + 31) / 32; A.tiles_pad = A.ngroups * 32;
+    A.nom = nom; A.rad = rad; A.mu = mu; A.ld_in = ld_in; A.g_lo = g_lo; A.g_hi = g_hi; A.ld_out = ld_out;
+    const size_t nwork = (size_t)T.tasks.size() * A.ngroups;
+    // slot regions
+    size_t region;     // float2 elements per lane
+    if (!vjp) { A.adj_off = 0; A.acc_off = T.max_slots; A.gm_off = 0; region = (size_t)T.max_slots + T.max_acc; }
+    else { A.adj_off = T.max_slots; A.acc_off = 2 * T.max_slots; A.gm_off = 2 * T.max_slots + T.max_grad; region = 2 * (size_t)T.max_slots + 2 * (size_t)T.max_grad; }
+    region = std::max<size_t>(region, 1);
+    A.ws_stride = region * 32;
+    int blocks = S->num_sms * (vjp ? 6 : 8);
+    const size_t need_blocks = (nwork + kWarpsPerBlock - 1) / kWarpsPerBlock;
+    if ((size_t)blocks > need_blocks) blocks = (int)std::max<size_t>(need_blocks, 1);
+    const size_t rows = vjp ? T.grad_rows : T.acc_rows;
+    if (!grow(&S->ws, &S->ws_bytes, (size_t)blocks * kWarpsPerBlock * A.ws_stride * sizeof(float2))) return LEB_ERR_NOMEM;
+    if (!grow(&S->partial, &S->partial_bytes, std::max<size_t>(rows, 1) * A.tiles_pad * sizeof(float2))) return LEB_ERR_NOMEM;
+    if (vjp && mu && !grow(&S->partial_mu, &S->partial_mu_bytes, std::max<size_t>(rows, 1) * A.tiles_pad * sizeof(float))) return LEB_ERR_NOMEM;
+    {
+        size_t have = S->tile_bad_n * sizeof(int);
+        if (!grow(&S->tile_bad, &have, (size_t)A.tiles_pad * sizeof(int))) return LEB_ERR_NOMEM;
+        S->tile_bad_n = have / sizeof(int);
+    }
+    A.ws = S->ws; A.partial = S->partial; A.partial_mu = (vjp && mu) ? S->partial_mu : nullptr;
+    A.counter = S->counter; A.tile_bad = S->tile_bad;
+    cudaMemsetAsync(S->counter, 0, sizeof(unsigned), st);
+    cudaMemsetAsync(S->tile_bad, 0, (size_t)A.tiles_pad * sizeof(int), st);
+    const int kc = vjp ? LEB_KC_ANALYTIC_VJP : LEB_KC_ANALYTIC_FWD;
+    prof->begin(kc, st);
+    if (nwork > 0) {
+        if (vjp) an_vm_kernel<true><<<blocks, kWarpsPerBlock * 32, 0, st>>>(D, A);
+        else an_vm_kernel<false><<<blocks, kWarpsPerBlock * 32, 0, st>>>(D, A);
+        ++*launches;
+    }
+    // algorithmic work: the tape's FP32 operations per tile (the reverse sweep is counted as twice the forward)
+    prof->end(kc, st, (vjp ? 3.0 : 1.0) * T.flops_fwd * tiles);
+    const int threads = 128;
+    if (vjp) an_reduce_vjp_kernel<<<tiles, threads, 0, st>>>(D, A.tiles_pad, nom, rad, mu, ld_in, S->partial, A.partial_mu, S->tile_bad, grad_nom, grad_rad, grad_mu, domain_flag);
+    else an_reduce_fwd_kernel<<<tiles, threads, 0, st>>>(D, A.tiles_pad, nom, rad, mu, ld_in, S->partial, S->tile_bad, r_lo, r_hi, ld_out, domain_flag);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_an_forward(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, int ld_in, float* r_lo,
+                          float* r_hi, int ld_out, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
+    return an_run(S, false, tiles, nom, rad, mu, ld_in, r_lo, r_hi, nullptr, nullptr, ld_out, nullptr, nullptr, nullptr, domain_flag, st, launches, prof);
+}
+
+leb_status leb_an_vjp(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo, const float* g_hi,
+                      int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, int* domain_flag, cudaStream_t st,
+                      long long* launches, LebProf* prof) {
+    return an_run(S, true, tiles, nom, rad, mu, ld_in, nullptr, nullptr, g_lo, g_hi, ld_out, grad_nom, grad_rad, grad_mu, domain_flag, st, launches, prof);
+}
 
 Model leb_make_model(const leb_analytic_model& m) {
     Model M{};
     M.id = m.model_id;
     M.integ = (m.model_id == LEB_MODEL_UNICYCLE) ? LEB_INTEG_EULER : m.integ;
     M.n_units = (m.model_id == LEB_MODEL_QUADCHAIN) ? m.n_units : 1;
-    if (m.model_id == LEB_MODEL_UNICYCLE) { M.n = 3; M.N = 5; }
-    else { M.n = 12 * M.n_units; M.N = 16 * M.n_units; }
+    switch (m.model_id) {
+        case LEB_MODEL_UNICYCLE: M.n = 3; M.N = 5; break;
+        case LEB_MODEL_PLANAR_QUAD: M.n = 6; M.N = 8; break;
+        case LEB_MODEL_SATELLITE: M.n = 7; M.N = 10; break;
+        default: M.n = 12 * M.n_units; M.N = 16 * M.n_units; break;
+    }
     // derived constants: evaluated in FP64 from the FP32 parameters, rounded once to FP32
-    double dt = m.dt;
+    const double dt = m.dt;
     M.dt = (float)dt;
     M.half_dt = (float)(0.5 * dt);
     M.dt6 = (float)(dt / 6.0);
-    if (m.model_id != LEB_MODEL_UNICYCLE) {
+    if (m.model_id == LEB_MODEL_PLANAR_QUAD) {
+        M.inv_m = (float)(1.0 / (double)m.mass);
+        M.g = m.g;
+        M.k1 = (float)((double)m.k1 / (double)m.Jx);      // arm length / moment of inertia
+    } else if (m.model_id != LEB_MODEL_UNICYCLE) {
         M.inv_m = (float)(1.0 / (double)m.mass);
         M.g = m.g;
         M.cp = (float)(((double)m.Jy - (double)m.Jz) / (double)m.Jx);
@@ -241,52 +593,4 @@ Model leb_make_model(const leb_analytic_model& m) {
         M.k3 = m.k3;
     }
     return M;
-}
-
-cudaError_t leb_launch_analytic_fwd(const Model& M, int tiles, const float* nom, const float* rad, int ld_in,
-                                    float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
-                                    long long* launches, LebProf* prof) {
-    if (tiles == 0) return cudaSuccess;
-    size_t smem = 2 * (size_t)M.N * sizeof(float);
-    // gridDim.y is limited to 65535: slice the tile range
-    for (int t0 = 0; t0 < tiles; t0 += 65535) {
-        int nt = tiles - t0 < 65535 ? tiles - t0 : 65535;
-        const float* a = nom + (size_t)t0 * ld_in;
-        const float* s = rad + (size_t)t0 * ld_in;
-        float* lo = r_lo + (size_t)t0 * ld_out;
-        float* hi = r_hi + (size_t)t0 * ld_out;
-        prof->begin(LEB_KC_ANALYTIC_FWD, st);
-        if (M.id == LEB_MODEL_UNICYCLE)
-            analytic_fwd_kernel<3, true><<<dim3(1, nt), kThreads, smem, st>>>(M, a, s, ld_in, lo, hi, ld_out, domain_flag);
-        else
-            analytic_fwd_kernel<12, false><<<dim3(M.n_units, nt), kThreads, smem, st>>>(M, a, s, ld_in, lo, hi, ld_out, domain_flag);
-        prof->end(LEB_KC_ANALYTIC_FWD, st, 0.0);
-        ++*launches;
-    }
-    return cudaGetLastError();
-}
-
-cudaError_t leb_launch_analytic_vjp(const Model& M, int tiles, const float* nom, const float* rad, const float* g_lo,
-                                    const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad,
-                                    int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
-    if (tiles == 0) return cudaSuccess;
-    size_t smem = 2 * (size_t)M.N * sizeof(float);
-    size_t total = (size_t)tiles * M.N;
-    zero_rows_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(grad_nom, grad_rad, tiles, M.N, ld_in);
-    ++*launches;
-    for (int t0 = 0; t0 < tiles; t0 += 65535) {
-        int nt = tiles - t0 < 65535 ? tiles - t0 : 65535;
-        size_t oi = (size_t)t0 * ld_in, oo = (size_t)t0 * ld_out;
-        prof->begin(LEB_KC_ANALYTIC_VJP, st);
-        if (M.id == LEB_MODEL_UNICYCLE)
-            analytic_vjp_kernel<3, true><<<dim3(1, nt), kThreads, smem, st>>>(M, nom + oi, rad + oi, g_lo + oo, g_hi + oo, ld_in,
-                                                                             ld_out, grad_nom + oi, grad_rad + oi, domain_flag);
-        else
-            analytic_vjp_kernel<12, false><<<dim3(M.n_units, nt), kThreads, smem, st>>>(M, nom + oi, rad + oi, g_lo + oo, g_hi + oo,
-                                                                                       ld_in, ld_out, grad_nom + oi, grad_rad + oi,
-                                                                                       domain_flag);
-        prof->end(LEB_KC_ANALYTIC_VJP, st, 0.0);
-        ++*launches;
-    }
-    return cudaGetLastError();
 }

@@ -3,13 +3,11 @@
 #include <stdio.h>
 #include <stdint.h>
 #include <new>
-#include "an_core.cuh"
 #include "internal.h"
 
 struct leb_ctx {
     int device = 0;
-    bool has_analytic = false;
-    leb_an::Model model{};
+    AnState* an = nullptr;
     NnState* nn = nullptr;
     int* domain_flag = nullptr;     // device
     long long launches = 0;
@@ -96,6 +94,8 @@ leb_status leb_create(leb_ctx** out, int device) {
     if (cudaMalloc(&c->domain_flag, sizeof(int)) != cudaSuccess) { delete c; return LEB_ERR_NOMEM; }
     cudaMemset(c->domain_flag, 0, sizeof(int));
     c->nn = leb_nn_create();
+    c->an = leb_an_create();
+    if (!c->nn || !c->an) { leb_nn_destroy(c->nn); leb_an_destroy(c->an); cudaFree(c->domain_flag); delete c; return LEB_ERR_NOMEM; }
     *out = c;
     return LEB_OK;
 }
@@ -105,6 +105,7 @@ leb_status leb_destroy(leb_ctx* c) {
     DeviceGuard guard(c->device);
     cudaDeviceSynchronize();
     leb_nn_destroy(c->nn);
+    leb_an_destroy(c->an);
     c->prof.destroy();
     for (int i = 0; i < 8; ++i) if (c->stage[i]) cudaFree(c->stage[i]);
     if (c->domain_flag) cudaFree(c->domain_flag);
@@ -114,14 +115,15 @@ leb_status leb_destroy(leb_ctx* c) {
 
 leb_status leb_set_analytic(leb_ctx* c, const leb_analytic_model* m) {
     if (!c || !m) return LEB_ERR_ARG;
-    if (m->model_id != LEB_MODEL_UNICYCLE && m->model_id != LEB_MODEL_QUAD12 && m->model_id != LEB_MODEL_QUADCHAIN) return LEB_ERR_UNSUPPORTED;
+    if (m->model_id < LEB_MODEL_UNICYCLE || m->model_id > LEB_MODEL_SATELLITE) return LEB_ERR_UNSUPPORTED;
     if (m->model_id != LEB_MODEL_UNICYCLE && m->integ != LEB_INTEG_EULER && m->integ != LEB_INTEG_RK4) return LEB_ERR_ARG;
     if (m->model_id == LEB_MODEL_QUADCHAIN && (m->n_units < 1 || m->n_units > 4096)) return LEB_ERR_SHAPE;
     if (!(m->dt > 0.f)) return LEB_ERR_ARG;
-    if (m->model_id != LEB_MODEL_UNICYCLE && (!(m->mass > 0.f) || !(m->Jx > 0.f) || !(m->Jy > 0.f) || !(m->Jz > 0.f))) return LEB_ERR_ARG;
-    c->model = leb_make_model(*m);
-    c->has_analytic = true;
-    return LEB_OK;
+    if (m->model_id != LEB_MODEL_UNICYCLE && !(m->Jx > 0.f)) return LEB_ERR_ARG;
+    if (m->model_id != LEB_MODEL_UNICYCLE && m->model_id != LEB_MODEL_SATELLITE && !(m->mass > 0.f)) return LEB_ERR_ARG;
+    if (m->model_id != LEB_MODEL_UNICYCLE && m->model_id != LEB_MODEL_PLANAR_QUAD && (!(m->Jy > 0.f) || !(m->Jz > 0.f))) return LEB_ERR_ARG;
+    DeviceGuard guard(c->device);
+    return leb_an_set_model(c->an, leb_make_model(*m));
 }
 
 leb_status leb_set_mlp(leb_ctx* c, const leb_mlp* m, void* stream) {
@@ -139,13 +141,12 @@ leb_status leb_set_nn_chunk(leb_ctx* c, int tiles) {
 leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, int ld_in,
                             float* r_lo, float* r_hi, int ld_out, unsigned flags, void* stream) {
     if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
-    if (!c->has_analytic) return LEB_ERR_STATE;
-    if (mu) return LEB_ERR_UNSUPPORTED;
+    if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
     if (B == 0 || T == 0) return LEB_OK;            // empty batch: nothing to do, pointers may be NULL
     if (!nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
-    leb_status s = check_traj(B, T, c->model.N, c->model.n, ld_in, ld_out);
+    leb_status s = check_traj(B, T, leb_an_N(c->an), leb_an_n(c->an), ld_in, ld_out);
     if (s != LEB_OK) return s;
-    if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
+    if (!al4(nom) || !al4(rad) || !al4(mu) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     const bool host = flags & LEB_FLAG_HOST_IO;
@@ -153,11 +154,12 @@ leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const fl
     bool ok = true;
     const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
     const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_mu = in_ptr(c, 4, mu, tiles * ld_in, host, st, &ok);
     float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
     float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
-    if (leb_launch_analytic_fwd(c->model, (int)tiles, d_nom, d_rad, ld_in, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches, &c->prof) != cudaSuccess)
-        return LEB_ERR_CUDA;
+    s = leb_an_forward(c->an, (int)tiles, d_nom, d_rad, d_mu, ld_in, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches, &c->prof);
+    if (s != LEB_OK) return s;
     out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
     out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
     return ok ? LEB_OK : LEB_ERR_CUDA;
@@ -194,23 +196,25 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
     return ok ? LEB_OK : LEB_ERR_CUDA;
 }
 
-leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
-                   int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, void* stream) {
+leb_status leb_vjp_mu(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* mu, const float* g_lo,
+                      const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags,
+                      void* stream) {
     if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (kind != 0 && kind != 1) return LEB_ERR_ARG;
-    if ((B == 0 || T == 0) && (kind == 0 ? c->has_analytic : leb_nn_ready(c->nn))) return LEB_OK;
+    if (kind == 1 && mu) return LEB_ERR_UNSUPPORTED;
+    if ((B == 0 || T == 0) && (kind == 0 ? leb_an_ready(c->an) : leb_nn_ready(c->nn))) return LEB_OK;
     if (!nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad) return LEB_ERR_ARG;
     int n, N;
     if (kind == 0) {
-        if (!c->has_analytic) return LEB_ERR_STATE;
-        n = c->model.n; N = c->model.N;
+        if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
+        n = leb_an_n(c->an); N = leb_an_N(c->an);
     } else {
         if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
         n = leb_nn_n(c->nn); N = leb_nn_N(c->nn);
     }
     leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
     if (s != LEB_OK) return s;
-    if (!al4(nom) || !al4(rad) || !al4(g_lo) || !al4(g_hi) || !al4(grad_nom) || !al4(grad_rad)) return LEB_ERR_ALIGN;
+    if (!al4(nom) || !al4(rad) || !al4(mu) || !al4(g_lo) || !al4(g_hi) || !al4(grad_nom) || !al4(grad_rad) || !al4(grad_mu)) return LEB_ERR_ALIGN;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     const bool host = flags & LEB_FLAG_HOST_IO;
@@ -220,20 +224,28 @@ leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const f
     const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
     const float* d_glo = in_ptr(c, 2, g_lo, tiles * ld_out, host, st, &ok);
     const float* d_ghi = in_ptr(c, 3, g_hi, tiles * ld_out, host, st, &ok);
+    const float* d_mu = in_ptr(c, 4, mu, tiles * ld_in, host, st, &ok);
     float* d_gn = out_ptr(c, 6, grad_nom, tiles * ld_in, host, &ok);
     float* d_gr = out_ptr(c, 7, grad_rad, tiles * ld_in, host, &ok);
+    float* d_gm = out_ptr(c, 5, (mu ? grad_mu : nullptr), tiles * ld_in, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
     if (kind == 0) {
-        if (leb_launch_analytic_vjp(c->model, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, c->domain_flag, st,
-                                    &c->launches, &c->prof) != cudaSuccess)
-            return LEB_ERR_CUDA;
+        s = leb_an_vjp(c->an, (int)tiles, d_nom, d_rad, d_mu, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, d_gm, c->domain_flag, st,
+                       &c->launches, &c->prof);
+        if (s != LEB_OK) return s;
     } else {
         s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, flags, c->domain_flag, st, &c->launches, &c->prof);
         if (s != LEB_OK) return s;
     }
     out_copy(grad_nom, d_gn, tiles * ld_in, host, st, &ok);
     out_copy(grad_rad, d_gr, tiles * ld_in, host, st, &ok);
+    if (mu) out_copy(grad_mu, d_gm, tiles * ld_in, host, st, &ok);
     return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_vjp(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
+                   int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, void* stream) {
+    return leb_vjp_mu(c, kind, B, T, nom, rad, nullptr, g_lo, g_hi, ld_in, ld_out, grad_nom, grad_rad, nullptr, flags, stream);
 }
 
 leb_status leb_zonotope_inflate(leb_ctx* c, int B, int T, int n, const float* r_lo, const float* r_hi, const float* E_diag,

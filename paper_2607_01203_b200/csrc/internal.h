@@ -6,7 +6,17 @@
 
 #include <vector>
 
-namespace leb_an { struct Model; }
+namespace leb_an {
+struct Tape;
+// analytic model with its derived constants (leb_make_model)
+struct Model {
+    int id, integ, n_units, n, N;
+    float dt, half_dt, dt6;                      // dt, dt/2, dt/6
+    float inv_m, g, cp, cq, cr, iJx, iJy, iJz;   // 1/m, g, (Jy-Jz)/Jx, (Jz-Jx)/Jy, (Jx-Jy)/Jz, 1/J*
+    float k1, k3;                                // chain spring; planar quadrotor: k1 = arm length / inertia
+};
+void leb_compile_tape(const Model& M, bool with_mu, Tape* T);      // an_compile.cu (host, structure only)
+}
 
 // ---- profiling aid (leb_profile / leb_profile_read): CUDA events around the launches of each
 // kernel class, on the launching stream, so that bench.py can report the dominant kernel's average
@@ -45,14 +55,21 @@ struct LebProf {
     }
 };
 
-// ---- analytic path (analytic.cu)
+// ---- analytic path (analytic.cu: interpreter of the interval tape compiled by an_compile.cu)
+struct AnState;   // model, tapes (host + device), workspace; owned by the context
 leb_an::Model leb_make_model(const leb_analytic_model& m);
-cudaError_t leb_launch_analytic_fwd(const leb_an::Model& M, int tiles, const float* nom, const float* rad, int ld_in,
-                                    float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
-                                    long long* launches, LebProf* prof);
-cudaError_t leb_launch_analytic_vjp(const leb_an::Model& M, int tiles, const float* nom, const float* rad, const float* g_lo,
-                                    const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad,
-                                    int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
+AnState* leb_an_create();
+void leb_an_destroy(AnState*);
+bool leb_an_ready(const AnState*);
+int leb_an_n(const AnState*);
+int leb_an_N(const AnState*);
+leb_status leb_an_set_model(AnState*, const leb_an::Model& M);
+leb_status leb_an_forward(AnState*, int tiles, const float* nom, const float* rad, const float* mu, int ld_in, float* r_lo,
+                          float* r_hi, int ld_out, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
+leb_status leb_an_vjp(AnState*, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo,
+                      const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu,
+                      int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
+void leb_an_stats(const AnState*, double* flops_fwd, long long* ins_fwd, long long* tape_ins, int* ntasks, int* max_slots);
 
 // ---- zonotope fold (inflate.cu)
 cudaError_t leb_launch_inflate(size_t rows, int n, const float* r_lo, const float* r_hi, const float* E_diag, float pad,

@@ -26,7 +26,7 @@ FLAG_SINGLE_CTA = 16
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
-    "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
+    "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
     "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
@@ -126,8 +126,8 @@ class Context:
                          Jx=0.010, Jy=0.015, Jz=0.020, k1=1.0, k3=0.1):
         m = _AnalyticModel(int(model_id), int(integ), int(n_units), dt, mass, g, Jx, Jy, Jz, k1, k3)
         _chk(self.lib.leb_set_analytic(self._ctx, ctypes.byref(m)), "leb_set_analytic")
-        if model_id == 1:
-            self.n, self.N = 3, 5
+        if model_id in (1, 4, 5):
+            self.n, self.N = {1: (3, 5), 4: (6, 8), 5: (7, 10)}[model_id]
         else:
             u = n_units if model_id == 3 else 1
             self.n, self.N = 12 * u, 16 * u
@@ -165,14 +165,14 @@ class Context:
         return int(nom.shape[0]), int(nom.shape[1]), int(nom.shape[2])
 
     # ------------------------------------------------------------------ entry points
-    def leb_analytic_fwd(self, nom, rad, r_lo=None, r_hi=None, flags: int = 0):
-        _check_f32(nom, rad, r_lo, r_hi)
+    def leb_analytic_fwd(self, nom, rad, r_lo=None, r_hi=None, flags: int = 0, mu=None):
+        _check_f32(nom, rad, r_lo, r_hi, mu)
         B, T, ld_in = self._bt(nom)
         host = bool(flags & FLAG_HOST_IO)
         if r_lo is None:
             r_lo = self._out(nom, (B, T, self.n), host)
             r_hi = self._out(nom, (B, T, self.n), host)
-        _chk(self.lib.leb_analytic_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), None, ld_in, _ptr(r_lo), _ptr(r_hi),
+        _chk(self.lib.leb_analytic_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), ld_in, _ptr(r_lo), _ptr(r_hi),
                                        int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_fwd")
         return r_lo, r_hi
 
@@ -200,6 +200,20 @@ class Context:
                               int(g_lo.shape[2]), _ptr(grad_nom), _ptr(grad_rad), ctypes.c_uint(flags),
                               _stream_ptr(self.device)), "leb_vjp")
         return grad_nom, grad_rad
+
+    def leb_vjp_mu(self, kind: int, nom, rad, mu, g_lo, g_hi, grad_nom=None, grad_rad=None, grad_mu=None, flags: int = 0):
+        _check_f32(nom, rad, mu, g_lo, g_hi, grad_nom, grad_rad, grad_mu)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        if grad_nom is None:
+            grad_nom = self._out(nom, (B, T, ld_in), host)
+            grad_rad = self._out(nom, (B, T, ld_in), host)
+        if grad_mu is None and mu is not None:
+            grad_mu = self._out(nom, (B, T, ld_in), host)
+        _chk(self.lib.leb_vjp_mu(self._ctx, int(kind), B, T, _ptr(nom), _ptr(rad), _ptr(mu), _ptr(g_lo), _ptr(g_hi), ld_in,
+                                 int(g_lo.shape[2]), _ptr(grad_nom), _ptr(grad_rad), _ptr(grad_mu), ctypes.c_uint(flags),
+                                 _stream_ptr(self.device)), "leb_vjp_mu")
+        return grad_nom, grad_rad, grad_mu
 
     def leb_zonotope_inflate(self, r_lo, r_hi, pad: float = 1e-6, E_diag=None, dense: bool = False, flags: int = 0,
                              c_bar=None, R_diag=None):

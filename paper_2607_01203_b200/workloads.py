@@ -28,6 +28,8 @@ BASE_SEED = 20260701
 MODEL_UNICYCLE = 1
 MODEL_QUAD12 = 2
 MODEL_QUADCHAIN = 3
+MODEL_PLANAR_QUAD = 4
+MODEL_SATELLITE = 5
 INTEG_EULER = 1
 INTEG_RK4 = 2
 ACT_RELU = 1
@@ -58,11 +60,13 @@ class AnalyticModel:
 
     @property
     def n(self) -> int:
-        return {MODEL_UNICYCLE: 3, MODEL_QUAD12: 12, MODEL_QUADCHAIN: 12 * self.n_units}[self.model_id]
+        return {MODEL_UNICYCLE: 3, MODEL_QUAD12: 12, MODEL_QUADCHAIN: 12 * self.n_units, MODEL_PLANAR_QUAD: 6,
+                MODEL_SATELLITE: 7}[self.model_id]
 
     @property
     def m(self) -> int:
-        return {MODEL_UNICYCLE: 2, MODEL_QUAD12: 4, MODEL_QUADCHAIN: 4 * self.n_units}[self.model_id]
+        return {MODEL_UNICYCLE: 2, MODEL_QUAD12: 4, MODEL_QUADCHAIN: 4 * self.n_units, MODEL_PLANAR_QUAD: 2,
+                MODEL_SATELLITE: 3}[self.model_id]
 
     def params(self) -> np.ndarray:
         """Flat fp64 parameter vector [dt, mass, g, Jx, Jy, Jz, k1, k3]."""
@@ -206,6 +210,40 @@ def make_small_chain(n_units: int, B: int, T: int, seed: int = 7) -> Workload:
     am = AnalyticModel(MODEL_QUADCHAIN, INTEG_RK4, 0.05, n_units=U)
     return Workload(40 + U, f"quadchain{12*U}_rk4", "analytic", B, T, 12 * U, 4 * U,
                     _f32(nom), _f32(rad), g_lo, g_hi, analytic=am)
+
+
+def make_paper_system(name: str, B: int, T: int, seed: int = 3) -> Workload:
+    """The paper's own analytic systems (App. I), forward Euler as in the paper, synthetic nominal
+    points: "satellite" (36) L507-519, 7 states (unit quaternion, body rates U[-1,1]) + 3 torques, I_S = diag(5,2,1),
+    dt 0.1; "planar_quad" (37) L521-528, 6 states + 2 rotor thrusts around hover, m = 2.0576, L = 0.25, J = 0.01,
+    dt 0.05; "quad12_euler": the 3-D quadrotor (38) with Euler.  Radii U[0.01, 0.2] (the local-set sizes of L372)."""
+    rng = np.random.Generator(np.random.PCG64(BASE_SEED + 300 + seed))
+    if name == "satellite":
+        q = rng.standard_normal((B, T, 4))
+        q /= np.linalg.norm(q, axis=-1, keepdims=True)
+        nom = np.concatenate([q, rng.uniform(-1, 1, (B, T, 3)), rng.uniform(-1, 1, (B, T, 3))], -1)
+        am = AnalyticModel(MODEL_SATELLITE, INTEG_EULER, 0.1, mass=1.0, g=0.0, Jx=5.0, Jy=2.0, Jz=1.0, k1=0.0, k3=0.0)
+    elif name == "planar_quad":
+        hover = 0.5 * 2.0576 * 9.81
+        nom = np.concatenate([rng.uniform(-1, 1, (B, T, 2)), rng.uniform(-0.5, 0.5, (B, T, 1)), rng.uniform(-1, 1, (B, T, 3)),
+                              hover * rng.uniform(0.8, 1.2, (B, T, 2))], -1)
+        am = AnalyticModel(MODEL_PLANAR_QUAD, INTEG_EULER, 0.05, mass=2.0576, g=9.81, Jx=0.01, Jy=1.0, Jz=1.0, k1=0.25, k3=0.0)
+    elif name == "quad12_euler":
+        xi, nu = _quad_unit_nominal(rng, (B, T))
+        nom = np.concatenate([xi, nu], -1)
+        am = AnalyticModel(MODEL_QUAD12, INTEG_EULER, 0.05)
+    else:
+        raise ValueError(name)
+    rad = rng.uniform(0.01, 0.2, nom.shape)
+    g_lo, g_hi = _cotangents(rng, B, T, am.n)
+    return Workload(60, name, "analytic", B, T, am.n, am.m, _f32(nom), _f32(rad), g_lo, g_hi, analytic=am)
+
+
+def make_mu(w: Workload, scale: float = 1.5, seed: int = 5) -> np.ndarray:
+    """Box offsets mu (25a) PAPER.md:L272 for a workload: mu = rad * U[-scale, scale] (for scale > 1 the nominal
+    point lies outside the box for some coordinates)."""
+    rng = np.random.Generator(np.random.PCG64(BASE_SEED + 400 + seed))
+    return _f32(w.rad * rng.uniform(-scale, scale, w.rad.shape))
 
 
 def make_small_mlp(dims, act, B, T, seed=11, rad_lo=0.01, rad_hi=0.05, init="xavier") -> Workload:

@@ -8,10 +8,30 @@ i.e. entrywise 1e-4 relative plus a normwise floor: grad_nom is the small differ
 and lower-bound adjoints (u_bar + l_bar) whose FP32 rounding scales with |u_bar| + |l_bar|, the size
 of grad_rad (u_bar - l_bar), so an FP32 evaluation cannot be entrywise-relative on it.
 """
+import json
+import os
+
 import numpy as np
 
 BOUND_RTOL, BOUND_ATOL = 1e-5, 1e-7
 GRAD_RTOL, GRAD_NORMWISE = 1e-4, 3e-5
+
+
+_LOG = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def report(what, worst):
+    """Every parity helper reports the worst err/tol it saw: printed (pytest -s / -rP shows it) and, on the GPU box,
+    appended to gpurun_out/parity_worst.jsonl so the numbers quoted in DESIGN.md section 6 can be read back."""
+    worst = float(worst)
+    print(f"[parity] {what}: worst err/tol = {worst:.3g}")
+    if os.path.isdir(_LOG):
+        try:
+            with open(os.path.join(_LOG, "parity_worst.jsonl"), "a") as f:
+                f.write(json.dumps({"what": what, "worst_err_over_tol": worst}) + "\n")
+        except OSError:
+            pass
+    return worst
 
 
 def to_np(t):
@@ -23,6 +43,7 @@ def assert_bounds_close(got, ref, what=""):
     err = np.abs(got - ref)
     tol = BOUND_RTOL * np.abs(ref) + BOUND_ATOL
     bad = ~(err <= tol)
+    report(what, np.nanmax(err / tol) if err.size else 0.0)
     assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} outside tolerance, worst err/tol {np.nanmax(err / tol):.3g}"
 
 
@@ -35,26 +56,36 @@ def assert_grads_close(gn, gr, ref_n, ref_r, what=""):
         err = np.abs(got - ref)
         tol = GRAD_RTOL * np.abs(ref) + GRAD_NORMWISE * S + 1e-12
         bad = ~(err <= tol)
+        report(f"{what} {name}", np.nanmax(err / tol) if err.size else 0.0)
         assert not bad.any(), f"{what} {name}: {bad.sum()} of {bad.size} outside tolerance, worst err/tol {np.nanmax(err / tol):.3g}"
+
+
+GRAD_NORMWISE_ANALYTIC = 1e-6      # SURVEY 8(c).5's proposal; the analytic path meets it
 
 
 def assert_grad_dirs_close(got, ref, S, what=""):
     """Analytic path, gradient entries along selected directions: got/ref [tiles, ndirs], S [tiles]."""
     err = np.abs(np.asarray(got, dtype=np.float64) - ref)
-    tol = GRAD_RTOL * np.abs(ref) + GRAD_NORMWISE * np.asarray(S)[:, None] + 1e-12
+    tol = GRAD_RTOL * np.abs(ref) + GRAD_NORMWISE_ANALYTIC * np.asarray(S)[:, None] + 1e-12
     bad = ~(err <= tol)
+    report(what, np.nanmax(err / tol) if err.size else 0.0)
     assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} outside tolerance, worst err/tol {np.nanmax(err / tol):.3g}"
+
+
+def grads_ratio(gn, gr, ref_n, ref_r):
+    """Per-tile worst err/tol of the assert_grads_close criterion."""
+    gn = np.asarray(gn, dtype=np.float64).reshape(ref_n.shape)
+    gr = np.asarray(gr, dtype=np.float64).reshape(ref_r.shape)
+    S = np.maximum(np.abs(ref_n).max(1), np.abs(ref_r).max(1))[:, None]
+    worst = np.zeros(ref_n.shape[0])
+    for got, ref in ((gn, ref_n), (gr, ref_r)):
+        worst = np.maximum(worst, (np.abs(got - ref) / (GRAD_RTOL * np.abs(ref) + GRAD_NORMWISE * S + 1e-12)).max(1))
+    return worst
 
 
 def grads_ok(gn, gr, ref_n, ref_r):
     """Per-tile boolean of the assert_grads_close criterion."""
-    gn = np.asarray(gn, dtype=np.float64).reshape(ref_n.shape)
-    gr = np.asarray(gr, dtype=np.float64).reshape(ref_r.shape)
-    S = np.maximum(np.abs(ref_n).max(1), np.abs(ref_r).max(1))[:, None]
-    ok = np.ones(ref_n.shape[0], dtype=bool)
-    for got, ref in ((gn, ref_n), (gr, ref_r)):
-        ok &= (np.abs(got - ref) <= GRAD_RTOL * np.abs(ref) + GRAD_NORMWISE * S + 1e-12).all(1)
-    return ok
+    return grads_ratio(gn, gr, ref_n, ref_r) <= 1.0
 
 
 def assert_nn_grads_close(O, mlp, nom, rad, g_lo, g_hi, gn, gr, what="", max_tie_tiles=2):
@@ -66,7 +97,9 @@ def assert_nn_grads_close(O, mlp, nom, rad, g_lo, g_hi, gn, gr, what="", max_tie
     ref_n, ref_r = O.leb_nn_vjp(mlp.W, mlp.b, mlp.act, nom, rad, g_lo, g_hi)
     gn = np.asarray(gn, dtype=np.float64).reshape(ref_n.shape)
     gr = np.asarray(gr, dtype=np.float64).reshape(ref_r.shape)
-    ok = grads_ok(gn, gr, ref_n, ref_r)
+    ratio = grads_ratio(gn, gr, ref_n, ref_r)
+    ok = ratio <= 1.0
+    report(f"{what} gradient (tiles off a kink of |W - J|)", ratio[ok].max() if ok.any() else 0.0)
     bad = np.nonzero(~ok)[0]
     assert len(bad) <= max_tie_tiles, f"{what}: {len(bad)} tiles miss the oracle gradient"
     Ws = [np.asarray(W, dtype=np.float64) for W in mlp.W]

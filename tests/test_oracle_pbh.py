@@ -360,3 +360,187 @@ def test_vjp_small_chain_directions():
     scale = np.abs(fd).max()
     assert ok.sum() >= 8
     assert np.all(np.abs(G[0] - fd)[ok] <= 1e-5 * np.abs(fd)[ok] + 1e-6 * scale)
+
+
+# ---------------------------------------------------------------- non-centred boxes (25a) PAPER.md:L272, reading R4
+def _iv_mul(a, b):
+    p = [a[0] * b[0], a[0] * b[1], a[1] * b[0], a[1] * b[1]]
+    return min(p), max(p)
+
+
+def _iv_sqr(a):
+    lo = 0.0 if a[0] <= 0.0 <= a[1] else min(a[0] ** 2, a[1] ** 2)
+    return lo, max(a[0] ** 2, a[1] ** 2)
+
+
+def test_mu_zero_is_the_centred_bound_bit_for_bit():
+    for cfg, tiles in ((1, 20), (2, 6)):
+        w = wl.make_config(cfg)
+        spec = P.spec_from_workload(w)
+        nom, rad = w.nom.reshape(-1, w.N)[:tiles], w.rad.reshape(-1, w.N)[:tiles]
+        for mode in (P.MODE_PATH, P.MODE_EXPAND):
+            a = P.pbh(spec, nom, rad, mode)
+            b = P.pbh(spec, nom, rad, mode, mu=np.zeros_like(nom))
+            assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_mu_quadratic_map_closed_form():
+    """Constant Hessian Q_l: R_l = sum_{j<k} Q_kj D_j D_k + 1/2 sum_k Q_kk D_k^2 with D = [mu - sigma, mu + sigma]
+    (L164): every term's range written out by hand (corner products; the square's range on a general interval)."""
+    rng = np.random.default_rng(11)
+    n, N = 3, 5
+    Q = rng.standard_normal((n, N, N))
+    Q = Q + Q.transpose(0, 2, 1)
+    C = rng.standard_normal((n, N))
+    spec = P.ModelSpec(P.MODEL_QUADRATIC, params=PARAMS, Q=Q, C=C)
+    nom, rad = rng.standard_normal((6, N)), rng.uniform(0.05, 0.5, (6, N))
+    mu = rng.uniform(-0.6, 0.6, (6, N))               # some |mu| > sigma: a~ outside the box
+    assert (np.abs(mu) > rad).any() and (np.abs(mu) < rad).any()
+    lo, hi, st = P.pbh(spec, nom, rad, mu=mu)
+    assert st == 0
+    for t in range(6):
+        D = [(mu[t, i] - rad[t, i], mu[t, i] + rad[t, i]) for i in range(N)]
+        for l in range(n):
+            up = dn = 0.0
+            for j in range(N):
+                for k in range(j + 1, N):
+                    a, b = _iv_mul((Q[l, k, j], Q[l, k, j]), _iv_mul(D[j], D[k]))
+                    dn += a
+                    up += b
+            for k in range(N):
+                a, b = _iv_mul((Q[l, k, k], Q[l, k, k]), _iv_sqr(D[k]))
+                dn += 0.5 * a
+                up += 0.5 * b
+            assert np.isclose(hi[t, l], up, rtol=1e-12, atol=1e-14) and np.isclose(lo[t, l], dn, rtol=1e-12, atol=1e-14)
+        # constant Hessian: r = 1/2 d^T Q d exactly for a = a~ + d; vertices of the shifted box
+        for s in itertools.product((-1.0, 1.0), repeat=N):
+            d = mu[t] + rad[t] * np.array(s)
+            r = 0.5 * np.einsum("lij,i,j->l", Q, d, d)
+            assert np.all(r <= hi[t] + 1e-12) and np.all(r >= lo[t] - 1e-12)
+
+
+@pytest.mark.parametrize("cfg,tiles", [(1, 8), (2, 4)])
+def test_mu_soundness_off_centre(cfg, tiles):
+    """Thm 1 with the nominal point off the box centre (and for some coordinates outside the box): the remainder
+    about a~, r(a) = f(a) - f(a~) - J(a~)(a - a~) (10) L133, sampled on A = a~ + mu + [-sigma, sigma] and at all its
+    vertices, lies in the enclosure; and the enclosure is not vacuous."""
+    w = wl.make_config(cfg)
+    spec = P.spec_from_workload(w)
+    rng = np.random.default_rng(50 + cfg)
+    N = w.N
+    nom, rad = w.nom.reshape(-1, N)[:tiles].astype(float), w.rad.reshape(-1, N)[:tiles].astype(float)
+    mu = rad * rng.uniform(-2.0, 2.0, rad.shape)
+    lo, hi, st = P.pbh(spec, nom, rad, mu=mu)
+    assert st == 0
+    verts = np.array(list(itertools.product((-1.0, 1.0), repeat=N)))
+    sharp = []
+    for t in range(tiles):
+        U = np.concatenate([rng.uniform(-1, 1, (100000, N)), verts])
+        r = _true_r(spec, nom[t], nom[t][None] + mu[t][None] + U * rad[t][None])
+        assert np.all(r.max(0) <= hi[t] + 1e-12) and np.all(r.min(0) >= lo[t] - 1e-12), t
+        nz = (hi[t] - lo[t]) > 1e-9
+        sharp.append(((r.max(0) - r.min(0))[nz] / (hi[t] - lo[t])[nz]).max())
+    assert max(sharp) > 0.3
+
+
+def test_mu_vjp_matches_central_differences():
+    w = wl.make_config(2, B=1, T=3)
+    spec = P.spec_from_workload(w)
+    rng = np.random.default_rng(8)
+    N, n = w.N, w.n
+    nom, rad = w.nom.reshape(-1, N).astype(float), w.rad.reshape(-1, N).astype(float)
+    mu = rad * rng.uniform(-1.5, 1.5, rad.shape)
+    g_lo, g_hi = w.g_lo.reshape(-1, n).astype(float), w.g_hi.reshape(-1, n).astype(float)
+    g, st = P.pbh_vjp(spec, nom, rad, g_lo, g_hi, mu=mu)
+    assert st == 0 and g.shape == (3, 3 * N)
+
+    def F(a, s, m):
+        lo, hi, _ = P.pbh(spec, a, s, mu=m)
+        return (g_hi * hi + g_lo * lo).sum(1)
+    h, checked = 1e-6, 0
+    F0 = F(nom, rad, mu)
+    for d in range(3 * N):
+        e = np.zeros((3, N))
+        e[:, d % N] = h
+        args = [(nom + e, rad, mu), (nom - e, rad, mu)] if d < N else \
+               [(nom, rad + e, mu), (nom, rad - e, mu)] if d < 2 * N else [(nom, rad, mu + e), (nom, rad, mu - e)]
+        fp, fm = F(*args[0]), F(*args[1])
+        for t in range(3):
+            if abs((fp[t] - F0[t]) - (F0[t] - fm[t])) > 1e-3 * abs(fp[t] - fm[t]) + 1e-14:
+                continue                                   # kink
+            fd = (fp[t] - fm[t]) / (2 * h)
+            assert abs(fd - g[t, d]) <= 1e-5 * abs(fd) + 1e-6 * np.abs(g[t]).max(), (t, d)
+            checked += 1
+    assert checked >= 2 * N * 3
+    assert np.abs(g[:, 2 * N:]).max() > 1e-3 * np.abs(g).max()      # mu does carry gradient
+
+
+# ---------------------------------------------------------------- the paper's own systems (App. I)
+SAT = [0.1, 1.0, 0.0, 5.0, 2.0, 1.0, 0.0, 0.0]        # dt; I_S = diag(5, 2, 1)  (PAPER.md:L519)
+PQ = [0.05, 2.0576, 9.81, 0.01, 1.0, 1.0, 0.25, 0.0]   # dt; m, g, J, -, -, L       (PAPER.md:L528)
+
+
+def test_satellite_constant_hessian_closed_form():
+    """Euler satellite (36) L507-519 is a quadratic map: the Hessian is constant, so (15) has the closed form of
+    SURVEY 8(c).6 with Q measured from the point function by second differences (exact for a quadratic)."""
+    spec = P.ModelSpec(P.MODEL_SATELLITE, P.INTEG_EULER, 1, SAT)
+    rng = np.random.default_rng(3)
+    n, N = 7, 10
+    a0 = rng.standard_normal(N)
+    h = 0.5
+    Q = np.zeros((n, N, N))
+    E = np.eye(N) * h
+    f0 = P.f(spec, a0[None])[0]
+    for i in range(N):
+        for k in range(N):
+            Q[:, i, k] = (P.f(spec, (a0 + E[i] + E[k])[None])[0] - P.f(spec, (a0 + E[i])[None])[0]
+                          - P.f(spec, (a0 + E[k])[None])[0] + f0) / h ** 2
+    # quaternion kinematics: d^2 f_0 / d om_1 d q_1 = -dt/2; Euler's equations: d^2 f_4 / d om_2 d om_3 = dt (Jy - Jz)/Jx
+    assert np.isclose(Q[0, 4, 1], -0.05) and np.isclose(Q[4, 5, 6], 0.1 * (2.0 - 1.0) / 5.0) and np.isclose(Q[6, 4, 5], 0.1 * 3.0)
+    nom, rad = rng.standard_normal((4, N)), rng.uniform(0.01, 0.2, (4, N))
+    lo, hi, st = P.pbh(spec, nom, rad)
+    assert st == 0
+    for t in range(4):
+        s = rad[t]
+        for l in range(n):
+            off = sum(abs(Q[l, k, j]) * s[j] * s[k] for j in range(N) for k in range(j + 1, N))
+            up = off + 0.5 * sum(max(Q[l, k, k], 0) * s[k] ** 2 for k in range(N))
+            dn = -off + 0.5 * sum(min(Q[l, k, k], 0) * s[k] ** 2 for k in range(N))
+            assert np.isclose(hi[t, l], up, rtol=1e-9, atol=1e-13) and np.isclose(lo[t, l], dn, rtol=1e-9, atol=1e-13)
+    lo2, hi2, _ = P.pbh(spec, nom, rad, P.MODE_EXPAND)
+    assert np.allclose(lo, lo2, rtol=1e-12, atol=1e-15) and np.allclose(hi, hi2, rtol=1e-12, atol=1e-15)
+
+
+def test_planar_quadrotor_closed_form():
+    """Planar quadrotor (37a) L521-528, Euler: only phi (index 2) meets u1, u2 (6, 7) non-linearly.
+    f_3 = vx - dt (u1+u2) sin(phi)/m:  H_phiphi = dt (u1+u2) sin(phi)/m on A^(2) -- u PINNED (indices 6, 7 > 2) --,
+    H_phi,u = -dt cos(phi)/m on A^(2);  f_4 likewise with (-cos, -sin).  All other outputs are linear."""
+    spec = P.ModelSpec(P.MODEL_PLANAR_QUAD, P.INTEG_EULER, 1, PQ)
+    rng = np.random.default_rng(4)
+    dt, m = PQ[0], PQ[1]
+    nom = np.concatenate([rng.uniform(-1, 1, (6, 2)), rng.uniform(0.2, 0.9, (6, 1)), rng.uniform(-1, 1, (6, 3)),
+                          rng.uniform(8, 12, (6, 2))], 1)
+    rad = rng.uniform(0.01, 0.1, (6, 8))
+    lo, hi, st = P.pbh(spec, nom, rad)
+    assert st == 0
+    for t in range(6):
+        ph, sp = nom[t, 2], rad[t, 2]
+        S = (np.sin(ph - sp), np.sin(ph + sp))           # 0 < phi - sp, phi + sp < pi/2: both monotone
+        Cc = (np.cos(ph + sp), np.cos(ph - sp))
+        ub = nom[t, 6] + nom[t, 7]
+        D = lambda i: (-rad[t, i], rad[t, i])
+        for out, hpp, hpu in ((3, (dt / m * ub * S[0], dt / m * ub * S[1]), (-dt / m * Cc[1], -dt / m * Cc[0])),
+                              (4, (-dt / m * ub * Cc[1], -dt / m * ub * Cc[0]), (-dt / m * S[1], -dt / m * S[0]))):
+            a = _iv_mul(hpp, _iv_sqr(D(2)))
+            dn, up = 0.5 * a[0], 0.5 * a[1]
+            for u in (6, 7):
+                b = _iv_mul(hpu, _iv_mul(D(2), D(u)))
+                dn += b[0]
+                up += b[1]
+            assert np.isclose(lo[t, out], dn, rtol=1e-12, atol=1e-16) and np.isclose(hi[t, out], up, rtol=1e-12, atol=1e-16)
+        for out in (0, 1, 2, 5):
+            assert lo[t, out] == 0.0 and hi[t, out] == 0.0
+    # soundness on one tile
+    U = np.concatenate([rng.uniform(-1, 1, (100000, 8)), np.array(list(itertools.product((-1.0, 1.0), repeat=8)))])
+    r = _true_r(spec, nom[0], nom[0][None] + U * rad[0][None])
+    assert np.all(r.max(0) <= hi[0] + 1e-12) and np.all(r.min(0) >= lo[0] - 1e-12)
