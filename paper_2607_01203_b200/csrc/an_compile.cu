@@ -371,7 +371,10 @@ inline bool op_has_b(uint32_t op) { return op == OP_ADD || op == OP_SUB || op ==
 void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
     const int n = M.n, N = M.N;
     T->n = n; T->N = N; T->uses_mu = with_mu;
-    T->ins.clear(); T->segs.clear(); T->tasks.clear();
+    *T = Tape();
+    T->n = n; T->N = N; T->uses_mu = with_mu;
+    auto& task_out = T->task_out;
+    auto& task_var = T->task_var;
 
     // ---- first-order dependencies: which outputs read coordinate g at all (pass WJ in direction g)
     std::vector<std::vector<uint8_t>> dep(N, std::vector<uint8_t>(n, 0));
@@ -508,39 +511,99 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
             T->segs.push_back(sg);
         }
         task.seg_count = (uint32_t)ksegs.size();
+        // ---- operand sources and FAR bits (an_tape.h)
+        {
+            Ins* base = T->ins.data();
+            auto src_of = [&](uint32_t slot, uint32_t user, uint32_t seg_dst0, uint32_t seg_begin) -> uint32_t {
+                if (slot < seg_dst0) { base[task.wj_begin + slot].w0 |= OP_FAR; return SRC_GLOBAL; }     // WJ slot read by a K segment
+                if (user - slot == 1 && (base[seg_begin + (slot - seg_dst0)].w0 & OP_MASK) != OP_OUT) return SRC_PREV;
+                if (user - slot < kRing) return SRC_RING;
+                base[seg_begin + (slot - seg_dst0)].w0 |= OP_FAR;
+                return SRC_GLOBAL;
+            };
+            auto scan = [&](uint32_t begin, uint32_t count, uint32_t dst0) {
+                for (uint32_t i = 0; i < count; ++i) {
+                    const uint32_t op = base[begin + i].w0 & OP_MASK;
+                    if (op_has_a(op)) base[begin + i].w0 |= src_of(base[begin + i].w0 >> 8, dst0 + i, dst0, begin) << SRC_SHIFT;
+                    if (op_has_b(op)) base[begin + i].w1 |= src_of(base[begin + i].w1 & B_MASK, dst0 + i, dst0, begin) << B_SRC_SHIFT;
+                }
+            };
+            scan(task.wj_begin, nwj, 0);
+            for (uint32_t q = 0; q < task.seg_count; ++q) scan(T->segs[task.seg_begin + q].begin, T->segs[task.seg_begin + q].count, nwj);
+        }
         task.n_slots = nwj + max_k;
         task.acc_base = acc_rows; task.n_acc = (uint32_t)n_acc;
         task.grad_base = grad_rows; task.n_grad = (uint32_t)n_grad;
         task.cost = (uint32_t)std::min<uint64_t>(cost, 0xffffffffu);
-        for (int l = 0; l < n; ++l) if (acc_of[l] >= 0) out_rows[l].push_back(acc_rows + (uint32_t)acc_of[l]);
-        for (int g = 0; g < N; ++g) if (grow[g] >= 0) var_rows[g].push_back(grad_rows + (uint32_t)grow[g]);
-        acc_rows += (uint32_t)n_acc;
-        grad_rows += (uint32_t)n_grad;
+        {   // which output / input each of this task's rows belongs to (for the reduction tables)
+            std::vector<uint32_t> to(n_acc), tv(n_grad);
+            for (int l = 0; l < n; ++l) if (acc_of[l] >= 0) to[acc_of[l]] = (uint32_t)l;
+            for (int g = 0; g < N; ++g) if (grow[g] >= 0) tv[grow[g]] = (uint32_t)g;
+            task_out.push_back(std::move(to));
+            task_var.push_back(std::move(tv));
+        }
         T->flops_fwd += flops;
-        T->ins_fwd += cost;
         T->max_slots = std::max(T->max_slots, task.n_slots);
         T->max_acc = std::max(T->max_acc, task.n_acc);
         T->max_grad = std::max(T->max_grad, task.n_grad);
-        T->tasks.push_back(task);
+        T->base.push_back(task);
+        T->ins_fwd += cost;
     }
-    T->acc_rows = acc_rows;
-    T->grad_rows = grad_rows;
-    T->out_ptr.assign(n + 1, 0);
-    T->out_rows.clear();
-    for (int l = 0; l < n; ++l) {
-        T->out_ptr[l] = (uint32_t)T->out_rows.size();
-        T->out_rows.insert(T->out_rows.end(), out_rows[l].begin(), out_rows[l].end());
+    (void)acc_rows; (void)grad_rows; (void)out_rows; (void)var_rows;
+}
+
+void leb_build_taskset(const Tape& T, uint32_t target, TaskSet* set) {
+    const int n = T.n, N = T.N;
+    *set = TaskSet();
+    std::vector<uint32_t> parent;
+    for (size_t q = 0; q < T.base.size(); ++q) {
+        const Task& tk = T.base[q];
+        if (tk.cost <= target) { set->tasks.push_back(tk); parent.push_back((uint32_t)q); continue; }
+        // parts of about equal K cost, each at most `target` (but never shorter than the WJ they repeat)
+        const uint32_t kcost = tk.cost - tk.wj_count;
+        const uint32_t room = std::max<uint32_t>(target > tk.wj_count ? target - tk.wj_count : 0, tk.wj_count);
+        const uint32_t parts = (kcost + room - 1) / room;
+        const uint32_t per = (kcost + parts - 1) / parts;
+        uint32_t s0 = 0;
+        while (s0 < tk.seg_count) {
+            uint32_t s1 = s0, c = 0, mk = 0;
+            while (s1 < tk.seg_count && (s1 == s0 || c + T.segs[tk.seg_begin + s1].count <= per)) {
+                c += T.segs[tk.seg_begin + s1].count;
+                mk = std::max(mk, T.segs[tk.seg_begin + s1].count);
+                ++s1;
+            }
+            Task part = tk;
+            part.seg_begin = tk.seg_begin + s0;
+            part.seg_count = s1 - s0;
+            part.n_slots = tk.wj_count + mk;
+            part.cost = tk.wj_count + c;
+            set->tasks.push_back(part);
+            parent.push_back((uint32_t)q);
+            s0 = s1;
+        }
     }
-    T->out_ptr[n] = (uint32_t)T->out_rows.size();
-    T->var_ptr.assign(N + 1, 0);
-    T->var_rows.clear();
-    for (int g = 0; g < N; ++g) {
-        T->var_ptr[g] = (uint32_t)T->var_rows.size();
-        T->var_rows.insert(T->var_rows.end(), var_rows[g].begin(), var_rows[g].end());
+    // rows are handed out in creation order (ascending j), so every reduction adds in ascending j
+    std::vector<std::vector<uint32_t>> orow(n), vrow(N);
+    uint32_t ar = 0, gr = 0;
+    for (size_t q = 0; q < set->tasks.size(); ++q) {
+        Task& tk = set->tasks[q];
+        tk.acc_base = ar; tk.grad_base = gr;
+        const auto& to = T.task_out[parent[q]];
+        const auto& tv = T.task_var[parent[q]];
+        for (uint32_t r = 0; r < tk.n_acc; ++r) orow[to[r]].push_back(ar + r);
+        for (uint32_t r = 0; r < tk.n_grad; ++r) vrow[tv[r]].push_back(gr + r);
+        ar += tk.n_acc; gr += tk.n_grad;
+        set->ins_fwd += tk.cost;
     }
-    T->var_ptr[N] = (uint32_t)T->var_rows.size();
+    set->acc_rows = ar; set->grad_rows = gr;
+    set->out_ptr.assign(n + 1, 0);
+    for (int l = 0; l < n; ++l) { set->out_ptr[l] = (uint32_t)set->out_rows.size(); set->out_rows.insert(set->out_rows.end(), orow[l].begin(), orow[l].end()); }
+    set->out_ptr[n] = (uint32_t)set->out_rows.size();
+    set->var_ptr.assign(N + 1, 0);
+    for (int g = 0; g < N; ++g) { set->var_ptr[g] = (uint32_t)set->var_rows.size(); set->var_rows.insert(set->var_rows.end(), vrow[g].begin(), vrow[g].end()); }
+    set->var_ptr[N] = (uint32_t)set->var_rows.size();
     // heavy tasks first (the device pulls tasks from a counter)
-    std::stable_sort(T->tasks.begin(), T->tasks.end(), [](const Task& a, const Task& b) { return a.cost > b.cost; });
+    std::stable_sort(set->tasks.begin(), set->tasks.end(), [](const Task& a, const Task& b) { return a.cost > b.cost; });
 }
 
 }  // namespace leb_an

@@ -48,9 +48,19 @@ enum Op : uint32_t {
     OP_COUNT
 };
 
-struct Ins { uint32_t w0, w1; };   // w0 = op | a << 8 ; w1 = b (slot, float bits, or row)
+// Instruction word: w0 = op (5 bits) | source of operand a (2 bits) | FAR (1 bit) | a (24 bits);
+// w1 = operand b: slot (30 bits) | source of b (2 bits) for ADD / SUB / MUL, else float bits or a row.
+// The interpreter keeps the last kRing results of a segment in shared memory (a ring indexed by slot % kRing) and the
+// last one in registers.  Where an operand is read from is decided here, by the compiler: SRC_PREV (defined by the
+// preceding instruction), SRC_RING (fewer than kRing instructions earlier in the same segment) or SRC_GLOBAL (the
+// global slot file).  A slot whose value -- in the reverse sweep: whose adjoint -- is needed through the global file
+// carries the FAR bit.
+struct Ins { uint32_t w0, w1; };
+constexpr uint32_t kRing = 64;
+constexpr uint32_t OP_MASK = 31u, OP_FAR = 0x80u, SRC_SHIFT = 5, SRC_GLOBAL = 0, SRC_RING = 1, SRC_PREV = 2;
+constexpr uint32_t B_MASK = 0x3fffffffu, B_SRC_SHIFT = 30;
 
-inline uint32_t ins_op(const Ins& i) { return i.w0 & 255u; }
+inline uint32_t ins_op(const Ins& i) { return i.w0 & OP_MASK; }
 inline uint32_t ins_a(const Ins& i) { return i.w0 >> 8; }
 
 struct Seg { uint32_t begin, count; };          // instruction range in Tape::ins
@@ -80,19 +90,32 @@ inline int op_flops(uint32_t op) {
     }
 }
 
+// A set of tasks with the fixed-order reduction tables that go with it.
+struct TaskSet {
+    std::vector<Task> tasks;                     // sorted by descending cost
+    // bound l = sum of partial rows out_rows[out_ptr[l] .. out_ptr[l+1]) (ascending j)
+    std::vector<uint32_t> out_ptr, out_rows;
+    // gradient of input v = sum of partial-gradient rows var_rows[var_ptr[v] .. var_ptr[v+1])
+    std::vector<uint32_t> var_ptr, var_rows;
+    uint32_t acc_rows = 0, grad_rows = 0;
+    uint64_t ins_fwd = 0;                        // instructions executed per tile, forward
+};
+
 struct Tape {
     int n = 0, N = 0;
     std::vector<Ins> ins;
     std::vector<Seg> segs;
-    std::vector<Task> tasks;                     // sorted by descending cost
-    // fixed-order reductions: bound l = sum of partial rows out_rows[out_ptr[l] .. out_ptr[l+1]) (ascending j)
-    std::vector<uint32_t> out_ptr, out_rows;
-    // gradient of input v = sum of partial-gradient rows var_rows[var_ptr[v] .. var_ptr[v+1])
-    std::vector<uint32_t> var_ptr, var_rows;
-    uint32_t acc_rows = 0, grad_rows = 0, max_slots = 0, max_acc = 0, max_grad = 0;
+    std::vector<Task> base;                      // one task per path index j, ascending j, rows not yet assigned
+    std::vector<std::vector<uint32_t>> task_out, task_var;   // per base task: output index of each acc row, input of each grad row
+    uint32_t max_slots = 0, max_acc = 0, max_grad = 0;
+    uint64_t ins_fwd = 0;                        // instructions per tile, forward, one task per j
     double flops_fwd = 0.0;                      // algorithmic FP32 operations per tile, forward
-    uint64_t ins_fwd = 0;                        // instructions executed per tile, forward
     bool uses_mu = false;
 };
+
+// Task set for a launch: the base tasks, those longer than `target` instructions cut into several tasks -- the K segments
+// of a task depend on WJ(j) only, so they can be dealt to several tasks that each re-run WJ(j).  The run time of a small
+// batch is the longest task's; cutting trades a little repeated work for a shorter critical path.
+void leb_build_taskset(const Tape& T, uint32_t target, TaskSet* set);
 
 }  // namespace leb_an

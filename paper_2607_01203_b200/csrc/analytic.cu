@@ -97,162 +97,239 @@ __device__ __forceinline__ float2 iv_cos(float2 a) {
 __device__ __forceinline__ float as_f(uint32_t u) { return __uint_as_float(u); }
 
 // ------------------------------------------------------------------ forward sweep of one segment
-// S: slot file of this lane (slot s at S[s * 32]); dst0: slot of the segment's first instruction.
-// VJP: the adjoint slot is cleared as the primal one is written and OUT does nothing.
+// S: global slot file of this lane (slot s at S[s * 32]); rb: shared-memory address of this lane's column of the warp's
+// ring (slot s at rb + (s % kRing) * 256); dst0: slot of the segment's first instruction.  Where an operand comes from
+// (the previous result, the ring, the global file) was decided by the compiler (an_tape.h).  VJP: every primal value
+// is also kept in the global file (the reverse sweep needs it), the adjoint of a FAR slot is cleared, OUT does nothing.
+__device__ __forceinline__ void prefetch_row(const float2* row) {
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(row));
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(row + 16));
+}
+__device__ __forceinline__ float2 lds2(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts2(uint32_t addr, float2 v) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y));
+}
+__device__ __forceinline__ float2 fetch(uint32_t src, uint32_t slot, const float2& prev, uint32_t rb, const float2* __restrict__ S) {
+    if (src == SRC_PREV) return prev;
+    if (src == SRC_RING) return lds2(rb + (slot & (kRing - 1)) * 256u);
+    return S[(size_t)slot * 32];
+}
+
 template <bool VJP>
 __device__ __forceinline__ void run_fwd(const uint2* __restrict__ ins, uint32_t begin, uint32_t count, uint32_t dst0,
-                                        float2* __restrict__ S, const VmArgs& A, const float* __restrict__ nom,
-                                        const float* __restrict__ rad, const float* __restrict__ mu, bool& bad, int lane) {
+                                        float2* __restrict__ S, uint32_t rb, const VmArgs& A,
+                                        const float* __restrict__ nom, const float* __restrict__ rad,
+                                        const float* __restrict__ mu, bool& bad, int lane) {
     float2* ADJ = S + (size_t)A.adj_off * 32;
     float2* ACC = S + (size_t)A.acc_off * 32;
+    const float2* row0 = S - lane;
     float2 prev = make_float2(0.f, 0.f);
     uint32_t dst = dst0;
+    uint2 nxt = make_uint2(0u, 0u);
+    if ((uint32_t)lane < count) nxt = __ldg(ins + begin + lane);
     for (uint32_t base = 0; base < count; base += 32) {
-        uint2 mine = make_uint2(0u, 0u);
-        if (base + lane < count) mine = __ldg(ins + begin + base + lane);
+        const uint2 mine = nxt;
+        nxt = make_uint2(0u, 0u);
+        if (base + 32 + lane < count) {
+            // next chunk: fetch its instructions and pull its global operands towards L1 while this chunk executes
+            nxt = __ldg(ins + begin + base + 32 + lane);
+            const uint32_t op = nxt.x & OP_MASK;
+            if (op >= OP_ADD && ((nxt.x >> SRC_SHIFT) & 3u) == SRC_GLOBAL) prefetch_row(row0 + (size_t)(nxt.x >> 8) * 32);
+            if ((op == OP_ADD || op == OP_SUB || op == OP_MUL) && (nxt.y >> B_SRC_SHIFT) == SRC_GLOBAL) prefetch_row(row0 + (size_t)(nxt.y & B_MASK) * 32);
+        }
         const int m = min(32u, count - base);
         for (int i = 0; i < m; ++i, ++dst) {
             const uint32_t w0 = __shfl_sync(FULL, mine.x, i), w1 = __shfl_sync(FULL, mine.y, i);
-            const uint32_t op = w0 & 255u, a = w0 >> 8;
-            float2 r, x;
-            if (op >= OP_ADD) x = (a + 1 == dst && dst != dst0) ? prev : S[(size_t)a * 32];
-            switch (op) {
-                case OP_BOX: { float c = nom[a], s = rad[a]; r = make_float2(__fadd_rd(c, -s), __fadd_ru(c, s)); break; }
-                case OP_PT: { float c = nom[a]; r = make_float2(c, c); break; }
-                case OP_DELTA: { float s = rad[a]; r = make_float2(-s, s); break; }
-                case OP_BOXMU: {   // hull of [c + mu - s, c + mu + s] and {c}: the segment from a~ to a point of the box
-                    float c = nom[a], s = rad[a], u = mu[a];
-                    r = make_float2(__fadd_rd(c, fminf(__fadd_rd(u, -s), 0.f)), __fadd_ru(c, fmaxf(__fadd_ru(u, s), 0.f)));
-                    break;
+            const uint32_t op = w0 & OP_MASK, a = w0 >> 8;
+            float2 r;
+            if (op == OP_MUL) {
+                const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S), y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
+                r = iv_mul(x, y);
+            } else if (op == OP_SCALE) {
+                const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S);
+                const float c = as_f(w1);
+                r = c >= 0.f ? make_float2(__fmul_rd(c, x.x), __fmul_ru(c, x.y)) : make_float2(__fmul_rd(c, x.y), __fmul_ru(c, x.x));
+            } else if (op == OP_ADD) {
+                const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S), y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
+                r = make_float2(__fadd_rd(x.x, y.x), __fadd_ru(x.y, y.y));
+            } else if (op == OP_OUT) {
+                const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S);
+                if (!VJP) {
+                    float2* p = ACC + (size_t)(w1 & 0xffffu) * 32;
+                    const float2 c = *p;
+                    *p = make_float2(__fadd_rd(c.x, x.x), __fadd_ru(c.y, x.y));
                 }
-                case OP_DELTAMU: { float s = rad[a], u = mu[a]; r = make_float2(__fadd_rd(u, -s), __fadd_ru(u, s)); break; }
-                case OP_CONST: { float c = as_f(w1); r = make_float2(c, c); break; }
-                case OP_ADD: { float2 y = S[(size_t)w1 * 32]; r = make_float2(__fadd_rd(x.x, y.x), __fadd_ru(x.y, y.y)); break; }
-                case OP_SUB: { float2 y = S[(size_t)w1 * 32]; r = make_float2(__fadd_rd(x.x, -y.y), __fadd_ru(x.y, -y.x)); break; }
-                case OP_NEG: r = make_float2(-x.y, -x.x); break;
-                case OP_SCALE: {
-                    float c = as_f(w1);
-                    r = c >= 0.f ? make_float2(__fmul_rd(c, x.x), __fmul_ru(c, x.y)) : make_float2(__fmul_rd(c, x.y), __fmul_ru(c, x.x));
-                    break;
-                }
-                case OP_ADDC: { float c = as_f(w1); r = make_float2(__fadd_rd(x.x, c), __fadd_ru(x.y, c)); break; }
-                case OP_MUL: { float2 y = (w1 + 1 == dst && dst != dst0) ? prev : S[(size_t)w1 * 32]; r = iv_mul(x, y); break; }
-                case OP_SQR: r = iv_sqr(x); break;
-                case OP_CUBE: r = make_float2(cube_dn(x.x), cube_up(x.y)); break;
-                case OP_RECIP:
-                    if (x.x <= 0.f && x.y >= 0.f) { bad = true; r = make_float2(1.f, 1.f); }
-                    else r = make_float2(__frcp_rd(x.y), __frcp_ru(x.x));
-                    break;
-                case OP_SIN: r = iv_sin(x); break;
-                case OP_COS: r = iv_cos(x); break;
-                case OP_OUT:
-                    r = x;
-                    if (!VJP) {
-                        float2* p = ACC + (size_t)(w1 & 0xffffu) * 32;
-                        float2 c = *p;
-                        *p = make_float2(__fadd_rd(c.x, x.x), __fadd_ru(c.y, x.y));
+                prev = x;
+                continue;
+            } else {
+                float2 x = make_float2(0.f, 0.f);
+                if (op >= OP_ADD) x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S);
+                switch (op) {
+                    case OP_BOX: { float c = nom[a], s = rad[a]; r = make_float2(__fadd_rd(c, -s), __fadd_ru(c, s)); break; }
+                    case OP_PT: { float c = nom[a]; r = make_float2(c, c); break; }
+                    case OP_DELTA: { float s = rad[a]; r = make_float2(-s, s); break; }
+                    case OP_BOXMU: {   // hull of [c + mu - s, c + mu + s] and {c}: the segment from a~ to a point of the box
+                        float c = nom[a], s = rad[a], u = mu[a];
+                        r = make_float2(__fadd_rd(c, fminf(__fadd_rd(u, -s), 0.f)), __fadd_ru(c, fmaxf(__fadd_ru(u, s), 0.f)));
+                        break;
                     }
-                    break;
-                default: r = make_float2(0.f, 0.f); break;
+                    case OP_DELTAMU: { float s = rad[a], u = mu[a]; r = make_float2(__fadd_rd(u, -s), __fadd_ru(u, s)); break; }
+                    case OP_CONST: { float c = as_f(w1); r = make_float2(c, c); break; }
+                    case OP_SUB: {
+                        const float2 y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
+                        r = make_float2(__fadd_rd(x.x, -y.y), __fadd_ru(x.y, -y.x));
+                        break;
+                    }
+                    case OP_NEG: r = make_float2(-x.y, -x.x); break;
+                    case OP_ADDC: { float c = as_f(w1); r = make_float2(__fadd_rd(x.x, c), __fadd_ru(x.y, c)); break; }
+                    case OP_SQR: r = iv_sqr(x); break;
+                    case OP_CUBE: r = make_float2(cube_dn(x.x), cube_up(x.y)); break;
+                    case OP_RECIP:
+                        if (x.x <= 0.f && x.y >= 0.f) { bad = true; r = make_float2(1.f, 1.f); }
+                        else r = make_float2(__frcp_rd(x.y), __frcp_ru(x.x));
+                        break;
+                    case OP_SIN: r = iv_sin(x); break;
+                    case OP_COS: r = iv_cos(x); break;
+                    default: r = make_float2(0.f, 0.f); break;
+                }
             }
-            if (op != OP_OUT) S[(size_t)dst * 32] = r;
-            if (VJP) ADJ[(size_t)dst * 32] = make_float2(0.f, 0.f);
+            sts2(rb + (dst & (kRing - 1)) * 256u, r);
+            if (VJP || (w0 & OP_FAR)) S[(size_t)dst * 32] = r;
+            if (VJP && (w0 & OP_FAR)) ADJ[(size_t)dst * 32] = make_float2(0.f, 0.f);
             prev = r;
         }
     }
 }
 
 // ------------------------------------------------------------------ reverse sweep of one segment
-__device__ __forceinline__ void adj_add(float2* p, float dl, float dh) { float2 v = *p; v.x += dl; v.y += dh; *p = v; }
+// The adjoint of a slot is the sum of what its uses send back.  Uses fewer than kRing instructions later (same segment:
+// operand sources PREV / RING) accumulate in the shared-memory ring; every other use adds into the global adjoint file
+// with a fire-and-forget reduction (each lane owns its column: no contention), and only FAR slots read it back.
+__device__ __forceinline__ void red_add(float2* p, float dl, float dh) { atomicAdd(p, make_float2(dl, dh)); }
+__device__ __forceinline__ void send(uint32_t src, uint32_t slot, float dl, float dh, uint32_t rb, float2* __restrict__ ADJ) {
+    if (src != SRC_GLOBAL) {
+        const uint32_t p = rb + (slot & (kRing - 1)) * 256u;
+        float2 v = lds2(p);
+        v.x += dl; v.y += dh;
+        sts2(p, v);
+    } else {
+        red_add(ADJ + (size_t)slot * 32, dl, dh);
+    }
+}
 
 __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t begin, uint32_t count, uint32_t dst0,
-                                        float2* __restrict__ S, const VmArgs& A, const float* __restrict__ rad,
-                                        const float* __restrict__ mu, const float* __restrict__ g_lo,
-                                        const float* __restrict__ g_hi, int lane) {
+                                        float2* __restrict__ S, uint32_t rb, const VmArgs& A,
+                                        const float* __restrict__ rad, const float* __restrict__ mu,
+                                        const float* __restrict__ g_lo, const float* __restrict__ g_hi, int lane) {
     float2* ADJ = S + (size_t)A.adj_off * 32;
     float2* G0 = S + (size_t)A.acc_off * 32;                 // (nom_bar, rad_bar) per gradient row
     float2* GM = S + (size_t)A.gm_off * 32;                  // (mu_bar, -) per gradient row
+    const float2* row0 = S - lane;
     if (count == 0) return;
-    for (int base = (int)((count - 1) / 32) * 32; base >= 0; base -= 32) {
-        uint2 mine = make_uint2(0u, 0u);
-        if ((uint32_t)base + lane < count) mine = __ldg(ins + begin + base + lane);
+    for (uint32_t q = 0; q < kRing; ++q) sts2(rb + q * 256u, make_float2(0.f, 0.f));
+    const int last = (int)((count - 1) / 32) * 32;
+    uint2 nxt = make_uint2(0u, 0u);
+    if ((uint32_t)last + lane < count) nxt = __ldg(ins + begin + last + lane);
+    for (int base = last; base >= 0; base -= 32) {
+        const uint2 mine = nxt;
+        // this chunk's primal operands towards L1 (they were written by the forward sweep, long ago)
+        if ((uint32_t)base + lane < count) {
+            const uint32_t op = mine.x & OP_MASK;
+            if (op == OP_MUL || op == OP_SQR || op == OP_CUBE || op == OP_SIN || op == OP_COS) prefetch_row(row0 + (size_t)(mine.x >> 8) * 32);
+            if (op == OP_MUL) prefetch_row(row0 + (size_t)(mine.y & B_MASK) * 32);
+            if (op == OP_RECIP) prefetch_row(row0 + (size_t)(dst0 + base + lane) * 32);
+        }
+        nxt = make_uint2(0u, 0u);
+        if (base >= 32) nxt = __ldg(ins + begin + base - 32 + lane);
         const int m = min(32u, count - (uint32_t)base);
         for (int i = m - 1; i >= 0; --i) {
             const uint32_t w0 = __shfl_sync(FULL, mine.x, i), w1 = __shfl_sync(FULL, mine.y, i);
-            const uint32_t op = w0 & 255u, a = w0 >> 8;
+            const uint32_t op = w0 & OP_MASK, a = w0 >> 8, sa = (w0 >> SRC_SHIFT) & 3u;
             const uint32_t dst = dst0 + (uint32_t)base + (uint32_t)i;
+            const uint32_t rp = rb + (dst & (kRing - 1)) * 256u;
             if (op == OP_OUT) {
                 const uint32_t l = w1 >> 16;
-                adj_add(ADJ + (size_t)a * 32, g_lo[l], g_hi[l]);
-                continue;
+                send(sa, a, g_lo[l], g_hi[l], rb, ADJ);
+                continue;                                    // an OUT slot has no uses: its ring entry is still zero
             }
-            const float2 d = ADJ[(size_t)dst * 32];
+            float2 d = lds2(rp);
+            sts2(rp, make_float2(0.f, 0.f));                 // the ring entry now belongs to slot dst - kRing
+            if (w0 & OP_FAR) { const float2 g = __ldcg(ADJ + (size_t)dst * 32); d.x += g.x; d.y += g.y; }
             const float dl = d.x, dh = d.y;
             if (dl == 0.f && dh == 0.f) continue;
+            if (op == OP_MUL) {
+                const uint32_t b = w1 & B_MASK, sb = w1 >> B_SRC_SHIFT;
+                const float2 x = S[(size_t)a * 32], y = S[(size_t)b * 32];
+                // lower endpoint: first minimum of (xl yl, xl yh, xh yl, xh yh), products rounded down as in the forward
+                float best = __fmul_rd(x.x, y.x); int sl = 0;
+                float p = __fmul_rd(x.x, y.y); if (p < best) { best = p; sl = 1; }
+                p = __fmul_rd(x.y, y.x); if (p < best) { best = p; sl = 2; }
+                p = __fmul_rd(x.y, y.y); if (p < best) { best = p; sl = 3; }
+                best = __fmul_ru(x.x, y.x); int sh = 0;
+                p = __fmul_ru(x.x, y.y); if (p > best) { best = p; sh = 1; }
+                p = __fmul_ru(x.y, y.x); if (p > best) { best = p; sh = 2; }
+                p = __fmul_ru(x.y, y.y); if (p > best) { best = p; sh = 3; }
+                const float xs_l = (sl & 2) ? x.y : x.x, ys_l = (sl & 1) ? y.y : y.x;
+                const float xs_h = (sh & 2) ? x.y : x.x, ys_h = (sh & 1) ? y.y : y.x;
+                float2 ax = make_float2(0.f, 0.f), ay = make_float2(0.f, 0.f);
+                if (sl & 2) ax.y += dl * ys_l; else ax.x += dl * ys_l;
+                if (sl & 1) ay.y += dl * xs_l; else ay.x += dl * xs_l;
+                if (sh & 2) ax.y += dh * ys_h; else ax.x += dh * ys_h;
+                if (sh & 1) ay.y += dh * xs_h; else ay.x += dh * xs_h;
+                send(sa, a, ax.x, ax.y, rb, ADJ);
+                send(sb, b, ay.x, ay.y, rb, ADJ);
+                continue;
+            }
+            if (op == OP_SCALE) {
+                const float c = as_f(w1);
+                if (c >= 0.f) send(sa, a, c * dl, c * dh, rb, ADJ);
+                else send(sa, a, c * dh, c * dl, rb, ADJ);
+                continue;
+            }
+            if (op == OP_ADD) {
+                send(sa, a, dl, dh, rb, ADJ);
+                send(w1 >> B_SRC_SHIFT, w1 & B_MASK, dl, dh, rb, ADJ);
+                continue;
+            }
             switch (op) {
-                case OP_BOX: adj_add(G0 + (size_t)w1 * 32, dl + dh, dh - dl); break;
-                case OP_PT: adj_add(G0 + (size_t)w1 * 32, dl + dh, 0.f); break;
-                case OP_DELTA: adj_add(G0 + (size_t)w1 * 32, 0.f, dh - dl); break;
+                case OP_BOX: red_add(G0 + (size_t)w1 * 32, dl + dh, dh - dl); break;
+                case OP_PT: red_add(G0 + (size_t)w1 * 32, dl + dh, 0.f); break;
+                case OP_DELTA: red_add(G0 + (size_t)w1 * 32, 0.f, dh - dl); break;
                 case OP_BOXMU: {
                     // lo = c + min(mu - s, 0), hi = c + max(mu + s, 0); ties keep the first candidate
                     const float s = rad[a], u = mu[a];
                     const float fl = (0.f < __fadd_rd(u, -s)) ? 0.f : dl, fh = (0.f > __fadd_ru(u, s)) ? 0.f : dh;
-                    adj_add(G0 + (size_t)w1 * 32, dl + dh, fh - fl);
-                    adj_add(GM + (size_t)w1 * 32, fl + fh, 0.f);
+                    red_add(G0 + (size_t)w1 * 32, dl + dh, fh - fl);
+                    red_add(GM + (size_t)w1 * 32, fl + fh, 0.f);
                     break;
                 }
                 case OP_DELTAMU:
-                    adj_add(G0 + (size_t)w1 * 32, 0.f, dh - dl);
-                    adj_add(GM + (size_t)w1 * 32, dl + dh, 0.f);
+                    red_add(G0 + (size_t)w1 * 32, 0.f, dh - dl);
+                    red_add(GM + (size_t)w1 * 32, dl + dh, 0.f);
                     break;
-                case OP_ADD: adj_add(ADJ + (size_t)a * 32, dl, dh); adj_add(ADJ + (size_t)w1 * 32, dl, dh); break;
-                case OP_SUB: adj_add(ADJ + (size_t)a * 32, dl, dh); adj_add(ADJ + (size_t)w1 * 32, -dh, -dl); break;
-                case OP_NEG: adj_add(ADJ + (size_t)a * 32, -dh, -dl); break;
-                case OP_SCALE: {
-                    const float c = as_f(w1);
-                    if (c >= 0.f) adj_add(ADJ + (size_t)a * 32, c * dl, c * dh);
-                    else adj_add(ADJ + (size_t)a * 32, c * dh, c * dl);
-                    break;
-                }
-                case OP_ADDC: adj_add(ADJ + (size_t)a * 32, dl, dh); break;
-                case OP_MUL: {
-                    const float2 x = S[(size_t)a * 32], y = S[(size_t)w1 * 32];
-                    // lower endpoint: first minimum of (xl yl, xl yh, xh yl, xh yh), products rounded down as in the forward
-                    float best = __fmul_rd(x.x, y.x); int sl = 0;
-                    float p = __fmul_rd(x.x, y.y); if (p < best) { best = p; sl = 1; }
-                    p = __fmul_rd(x.y, y.x); if (p < best) { best = p; sl = 2; }
-                    p = __fmul_rd(x.y, y.y); if (p < best) { best = p; sl = 3; }
-                    best = __fmul_ru(x.x, y.x); int sh = 0;
-                    p = __fmul_ru(x.x, y.y); if (p > best) { best = p; sh = 1; }
-                    p = __fmul_ru(x.y, y.x); if (p > best) { best = p; sh = 2; }
-                    p = __fmul_ru(x.y, y.y); if (p > best) { best = p; sh = 3; }
-                    const float xs_l = (sl & 2) ? x.y : x.x, ys_l = (sl & 1) ? y.y : y.x;
-                    const float xs_h = (sh & 2) ? x.y : x.x, ys_h = (sh & 1) ? y.y : y.x;
-                    float2 ax = make_float2(0.f, 0.f), ay = make_float2(0.f, 0.f);
-                    if (sl & 2) ax.y += dl * ys_l; else ax.x += dl * ys_l;
-                    if (sl & 1) ay.y += dl * xs_l; else ay.x += dl * xs_l;
-                    if (sh & 2) ax.y += dh * ys_h; else ax.x += dh * ys_h;
-                    if (sh & 1) ay.y += dh * xs_h; else ay.x += dh * xs_h;
-                    adj_add(ADJ + (size_t)a * 32, ax.x, ax.y);
-                    adj_add(ADJ + (size_t)w1 * 32, ay.x, ay.y);
-                    break;
-                }
+                case OP_SUB: send(sa, a, dl, dh, rb, ADJ); send(w1 >> B_SRC_SHIFT, w1 & B_MASK, -dh, -dl, rb, ADJ); break;
+                case OP_NEG: send(sa, a, -dh, -dl, rb, ADJ); break;
+                case OP_ADDC: send(sa, a, dl, dh, rb, ADJ); break;
                 case OP_SQR: {
                     const float2 x = S[(size_t)a * 32];
-                    if (x.x >= 0.f) adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dl, 2.f * x.y * dh);
-                    else if (x.y <= 0.f) adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dh, 2.f * x.y * dl);
-                    else if (__fmul_ru(x.y, x.y) > __fmul_ru(x.x, x.x)) adj_add(ADJ + (size_t)a * 32, 0.f, 2.f * x.y * dh);
-                    else adj_add(ADJ + (size_t)a * 32, 2.f * x.x * dh, 0.f);
+                    if (x.x >= 0.f) send(sa, a, 2.f * x.x * dl, 2.f * x.y * dh, rb, ADJ);
+                    else if (x.y <= 0.f) send(sa, a, 2.f * x.x * dh, 2.f * x.y * dl, rb, ADJ);
+                    else if (__fmul_ru(x.y, x.y) > __fmul_ru(x.x, x.x)) send(sa, a, 0.f, 2.f * x.y * dh, rb, ADJ);
+                    else send(sa, a, 2.f * x.x * dh, 0.f, rb, ADJ);
                     break;
                 }
                 case OP_CUBE: {
                     const float2 x = S[(size_t)a * 32];
-                    adj_add(ADJ + (size_t)a * 32, 3.f * x.x * x.x * dl, 3.f * x.y * x.y * dh);
+                    send(sa, a, 3.f * x.x * x.x * dl, 3.f * x.y * x.y * dh, rb, ADJ);
                     break;
                 }
                 case OP_RECIP: {
                     const float2 r = S[(size_t)dst * 32];          // (1/hi, 1/lo)
-                    adj_add(ADJ + (size_t)a * 32, -dh * r.y * r.y, -dl * r.x * r.x);
+                    send(sa, a, -dh * r.y * r.y, -dl * r.x * r.x, rb, ADJ);
                     break;
                 }
                 case OP_SIN: {
@@ -262,7 +339,7 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
                     float al = 0.f, ah = 0.f;
                     if (!has_min) { if (pad_dn(sh) < pad_dn(sl)) ah += cosf(x.y) * dl; else al += cosf(x.x) * dl; }
                     if (!has_max) { if (pad_up(sh) > pad_up(sl)) ah += cosf(x.y) * dh; else al += cosf(x.x) * dh; }
-                    adj_add(ADJ + (size_t)a * 32, al, ah);
+                    send(sa, a, al, ah, rb, ADJ);
                     break;
                 }
                 case OP_COS: {
@@ -272,7 +349,7 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
                     float al = 0.f, ah = 0.f;
                     if (!has_min) { if (pad_dn(ch) < pad_dn(cl)) ah -= sinf(x.y) * dl; else al -= sinf(x.x) * dl; }
                     if (!has_max) { if (pad_up(ch) > pad_up(cl)) ah -= sinf(x.y) * dh; else al -= sinf(x.x) * dh; }
-                    adj_add(ADJ + (size_t)a * 32, al, ah);
+                    send(sa, a, al, ah, rb, ADJ);
                     break;
                 }
                 default: break;
@@ -283,10 +360,12 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
 
 // ------------------------------------------------------------------ the interpreter kernel
 template <bool VJP>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32) an_vm_kernel(DevTape P, VmArgs A) {
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 3) an_vm_kernel(DevTape P, VmArgs A) {
+    extern __shared__ float2 ring[];                         // [kWarpsPerBlock][kRing][32]
     const int lane = threadIdx.x & 31;
     const size_t wid = (size_t)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
     float2* S = A.ws + wid * A.ws_stride + lane;
+    const uint32_t R = (uint32_t)__cvta_generic_to_shared(ring + (size_t)(threadIdx.x >> 5) * kRing * 32 + lane);
     const unsigned nwork = (unsigned)P.ntasks * (unsigned)A.ngroups;
     for (;;) {
         unsigned t = 0;
@@ -304,10 +383,10 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32) an_vm_kernel(DevTape P, V
         if (!VJP) {
             float2* ACC = S + (size_t)A.acc_off * 32;
             for (uint32_t r = 0; r < tk.n_acc; ++r) ACC[(size_t)r * 32] = make_float2(0.f, 0.f);
-            run_fwd<false>(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, nom, rad, mu, bad, lane);
+            run_fwd<false>(P.ins, tk.wj_begin, tk.wj_count, 0, S, R, A, nom, rad, mu, bad, lane);
             for (uint32_t q = 0; q < tk.seg_count; ++q) {
                 const Seg sg = P.segs[tk.seg_begin + q];
-                run_fwd<false>(P.ins, sg.begin, sg.count, tk.wj_count, S, A, nom, rad, mu, bad, lane);
+                run_fwd<false>(P.ins, sg.begin, sg.count, tk.wj_count, S, R, A, nom, rad, mu, bad, lane);
             }
             if (valid)
                 for (uint32_t r = 0; r < tk.n_acc; ++r) A.partial[(size_t)(tk.acc_base + r) * A.tiles_pad + tile] = ACC[(size_t)r * 32];
@@ -317,17 +396,17 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32) an_vm_kernel(DevTape P, V
             const float* g_lo = A.g_lo + row * A.ld_out;
             const float* g_hi = A.g_hi + row * A.ld_out;
             for (uint32_t r = 0; r < tk.n_grad; ++r) { G0[(size_t)r * 32] = make_float2(0.f, 0.f); GM[(size_t)r * 32] = make_float2(0.f, 0.f); }
-            run_fwd<true>(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, nom, rad, mu, bad, lane);
+            run_fwd<true>(P.ins, tk.wj_begin, tk.wj_count, 0, S, R, A, nom, rad, mu, bad, lane);
             for (uint32_t q = 0; q < tk.seg_count; ++q) {
                 const Seg sg = P.segs[tk.seg_begin + q];
-                run_fwd<true>(P.ins, sg.begin, sg.count, tk.wj_count, S, A, nom, rad, mu, bad, lane);
-                run_bwd(P.ins, sg.begin, sg.count, tk.wj_count, S, A, rad, mu, g_lo, g_hi, lane);
+                run_fwd<true>(P.ins, sg.begin, sg.count, tk.wj_count, S, R, A, nom, rad, mu, bad, lane);
+                run_bwd(P.ins, sg.begin, sg.count, tk.wj_count, S, R, A, rad, mu, g_lo, g_hi, lane);
             }
-            run_bwd(P.ins, tk.wj_begin, tk.wj_count, 0, S, A, rad, mu, g_lo, g_hi, lane);
+            run_bwd(P.ins, tk.wj_begin, tk.wj_count, 0, S, R, A, rad, mu, g_lo, g_hi, lane);
             if (valid)
                 for (uint32_t r = 0; r < tk.n_grad; ++r) {
-                    A.partial[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = G0[(size_t)r * 32];
-                    if (A.partial_mu) A.partial_mu[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = GM[(size_t)r * 32].x;
+                    A.partial[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = __ldcg(G0 + (size_t)r * 32);
+                    if (A.partial_mu) A.partial_mu[(size_t)(tk.grad_base + r) * A.tiles_pad + tile] = __ldcg(GM + (size_t)r * 32).x;
                 }
         }
         if (bad && valid) A.tile_bad[tile] = 1;
@@ -397,13 +476,22 @@ __global__ void an_reduce_vjp_kernel(DevTape P, int tiles_pad, const float* __re
 // ============================================================================================== host side
 using namespace leb_an;
 
+struct DevSet {                   // a TaskSet on the device
+    uint32_t target = 0;
+    DevTape dev{};
+    uint32_t acc_rows = 0, grad_rows = 0, ntasks = 0;
+    std::vector<void*> allocs;
+};
+
 struct AnState {
     bool ready = false;
     Model model{};
     Tape tape[2];                 // [0] centred boxes, [1] non-centred (mu != NULL), compiled on first use
     bool have[2] = {false, false};
-    DevTape dev[2]{};
+    const uint2* d_ins[2] = {nullptr, nullptr};
+    const Seg* d_segs[2] = {nullptr, nullptr};
     std::vector<void*> tape_allocs[2];
+    std::vector<DevSet> sets[2];  // task sets built so far (one per cost target, see leb_build_taskset)
     // buffers grown on demand
     float2* ws = nullptr; size_t ws_bytes = 0;
     float2* partial = nullptr; size_t partial_bytes = 0;
@@ -411,6 +499,7 @@ struct AnState {
     int* tile_bad = nullptr; size_t tile_bad_n = 0;
     unsigned* counter = nullptr;
     int num_sms = 148;
+    bool attr_done = false;
 };
 
 AnState* leb_an_create() {
@@ -425,6 +514,8 @@ AnState* leb_an_create() {
 static void free_tape(AnState* S, int v) {
     for (void* p : S->tape_allocs[v]) cudaFree(p);
     S->tape_allocs[v].clear();
+    for (DevSet& d : S->sets[v]) for (void* p : d.allocs) cudaFree(p);
+    S->sets[v].clear();
     S->have[v] = false;
 }
 
@@ -444,11 +535,11 @@ int leb_an_n(const AnState* S) { return S->model.n; }
 int leb_an_N(const AnState* S) { return S->model.N; }
 
 template <class T>
-static bool upload(AnState* S, int v, const std::vector<T>& h, const T** d) {
+static bool upload(std::vector<void*>& allocs, const std::vector<T>& h, const T** d) {
     void* p = nullptr;
     const size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(T);
     if (cudaMalloc(&p, bytes) != cudaSuccess) return false;
-    S->tape_allocs[v].push_back(p);
+    allocs.push_back(p);
     if (!h.empty() && cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
     *d = (const T*)p;
     return true;
@@ -458,20 +549,34 @@ static leb_status ensure_tape(AnState* S, int v) {
     if (S->have[v]) return LEB_OK;
     Tape& T = S->tape[v];
     leb_compile_tape(S->model, v == 1, &T);
-    DevTape& D = S->dev[v];
-    const uint2* ins = nullptr;
     static_assert(sizeof(Ins) == sizeof(uint2), "Ins is two words");
     std::vector<uint2> raw(T.ins.size());
     for (size_t i = 0; i < T.ins.size(); ++i) raw[i] = make_uint2(T.ins[i].w0, T.ins[i].w1);
-    bool ok = upload(S, v, raw, &ins) && upload(S, v, T.segs, &D.segs) && upload(S, v, T.tasks, &D.tasks) &&
-              upload(S, v, T.out_ptr, &D.out_ptr) && upload(S, v, T.out_rows, &D.out_rows) &&
-              upload(S, v, T.var_ptr, &D.var_ptr) && upload(S, v, T.var_rows, &D.var_rows);
-    if (!ok) { free_tape(S, v); return LEB_ERR_NOMEM; }
-    D.ins = ins;
-    D.ntasks = (int)T.tasks.size();
-    D.n = T.n; D.N = T.N;
+    if (!upload(S->tape_allocs[v], raw, &S->d_ins[v]) || !upload(S->tape_allocs[v], T.segs, &S->d_segs[v])) { free_tape(S, v); return LEB_ERR_NOMEM; }
     S->have[v] = true;
     return LEB_OK;
+}
+
+// the task set whose longest task has about `target` instructions (targets are rounded down to powers of two, at least
+// 1024, so that only a handful of sets ever exist)
+static const DevSet* ensure_set(AnState* S, int v, uint64_t target64) {
+    uint32_t target = 1024;
+    while ((uint64_t)target * 2 <= target64 && target < 0x40000000u) target <<= 1;
+    for (const DevSet& d : S->sets[v]) if (d.target == target) return &d;
+    const Tape& T = S->tape[v];
+    TaskSet set;
+    leb_build_taskset(T, target, &set);
+    S->sets[v].emplace_back();
+    DevSet& D = S->sets[v].back();
+    D.target = target;
+    D.acc_rows = set.acc_rows; D.grad_rows = set.grad_rows; D.ntasks = (uint32_t)set.tasks.size();
+    D.dev.ins = S->d_ins[v]; D.dev.segs = S->d_segs[v];
+    D.dev.ntasks = (int)set.tasks.size(); D.dev.n = T.n; D.dev.N = T.N;
+    const bool ok = upload(D.allocs, set.tasks, &D.dev.tasks) && upload(D.allocs, set.out_ptr, &D.dev.out_ptr) &&
+                    upload(D.allocs, set.out_rows, &D.dev.out_rows) && upload(D.allocs, set.var_ptr, &D.dev.var_ptr) &&
+                    upload(D.allocs, set.var_rows, &D.dev.var_rows);
+    if (!ok) { for (void* p : D.allocs) cudaFree(p); S->sets[v].pop_back(); return nullptr; }
+    return &D;
 }
 
 leb_status leb_an_set_model(AnState* S, const Model& M) {
@@ -494,7 +599,7 @@ static bool grow(T** p, size_t* have, size_t need_bytes) {
 void leb_an_stats(const AnState* S, double* flops_fwd, long long* ins_fwd, long long* tape_ins, int* ntasks, int* max_slots) {
     const Tape& T = S->tape[0];
     *flops_fwd = T.flops_fwd; *ins_fwd = (long long)T.ins_fwd; *tape_ins = (long long)T.ins.size();
-    *ntasks = (int)T.tasks.size(); *max_slots = (int)T.max_slots;
+    *ntasks = (int)T.base.size(); *max_slots = (int)T.max_slots;
 }
 
 // forward (g_lo == NULL) or VJP
@@ -506,21 +611,26 @@ static leb_status an_run(AnState* S, bool vjp, int tiles, const float* nom, cons
     leb_status es = ensure_tape(S, v);
     if (es != LEB_OK) return es;
     const Tape& T = S->tape[v];
-    const DevTape& D = S->dev[v];
     VmArgs A{};
     A.tiles = tiles; A.ngroups = (tiles + 31) / 32; A.tiles_pad = A.ngroups * 32;
     A.nom = nom; A.rad = rad; A.mu = mu; A.ld_in = ld_in; A.g_lo = g_lo; A.g_hi = g_hi; A.ld_out = ld_out;
-    const size_t nwork = (size_t)T.tasks.size() * A.ngroups;
+    // work items = (task, group of 32 tiles).  A small batch cannot fill the GPU with whole tasks -- its run time would be
+    // the longest task's -- so tasks longer than the per-warp share of the work are cut (leb_build_taskset)
+    const int warps_resident = S->num_sms * 3 * kWarpsPerBlock;
+    const DevSet* DS = ensure_set(S, v, T.ins_fwd * (uint64_t)A.ngroups / (uint64_t)warps_resident);
+    if (!DS) return LEB_ERR_NOMEM;
+    const DevTape& D = DS->dev;
+    const size_t nwork = (size_t)DS->ntasks * A.ngroups;
     // slot regions
     size_t region;     // float2 elements per lane
     if (!vjp) { A.adj_off = 0; A.acc_off = T.max_slots; A.gm_off = 0; region = (size_t)T.max_slots + T.max_acc; }
     else { A.adj_off = T.max_slots; A.acc_off = 2 * T.max_slots; A.gm_off = 2 * T.max_slots + T.max_grad; region = 2 * (size_t)T.max_slots + 2 * (size_t)T.max_grad; }
     region = std::max<size_t>(region, 1);
     A.ws_stride = region * 32;
-    int blocks = S->num_sms * (vjp ? 6 : 8);
+    int blocks = S->num_sms * 3;      // 64 KB of ring per block: three blocks (12 warps) per SM
     const size_t need_blocks = (nwork + kWarpsPerBlock - 1) / kWarpsPerBlock;
     if ((size_t)blocks > need_blocks) blocks = (int)std::max<size_t>(need_blocks, 1);
-    const size_t rows = vjp ? T.grad_rows : T.acc_rows;
+    const size_t rows = vjp ? DS->grad_rows : DS->acc_rows;
     if (!grow(&S->ws, &S->ws_bytes, (size_t)blocks * kWarpsPerBlock * A.ws_stride * sizeof(float2))) return LEB_ERR_NOMEM;
     if (!grow(&S->partial, &S->partial_bytes, std::max<size_t>(rows, 1) * A.tiles_pad * sizeof(float2))) return LEB_ERR_NOMEM;
     if (vjp && mu && !grow(&S->partial_mu, &S->partial_mu_bytes, std::max<size_t>(rows, 1) * A.tiles_pad * sizeof(float))) return LEB_ERR_NOMEM;
@@ -536,8 +646,15 @@ static leb_status an_run(AnState* S, bool vjp, int tiles, const float* nom, cons
     const int kc = vjp ? LEB_KC_ANALYTIC_VJP : LEB_KC_ANALYTIC_FWD;
     prof->begin(kc, st);
     if (nwork > 0) {
-        if (vjp) an_vm_kernel<true><<<blocks, kWarpsPerBlock * 32, 0, st>>>(D, A);
-        else an_vm_kernel<false><<<blocks, kWarpsPerBlock * 32, 0, st>>>(D, A);
+        const size_t smem = (size_t)kWarpsPerBlock * kRing * 32 * sizeof(float2);
+        if (!S->attr_done) {      // per context, hence per device
+            if (cudaFuncSetAttribute(an_vm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+                cudaFuncSetAttribute(an_vm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+                return LEB_ERR_CUDA;
+            S->attr_done = true;
+        }
+        if (vjp) an_vm_kernel<true><<<blocks, kWarpsPerBlock * 32, smem, st>>>(D, A);
+        else an_vm_kernel<false><<<blocks, kWarpsPerBlock * 32, smem, st>>>(D, A);
         ++*launches;
     }
     // algorithmic work: the tape's FP32 operations per tile (the reverse sweep is counted as twice the forward)
