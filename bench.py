@@ -5,12 +5,17 @@ B=64 candidate trajectories x T=100 timesteps, forward + VJP), one process per G
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input (DESIGN.md
-"Measurement"): leb_nn_fwd -> leb_zonotope_inflate -> leb_zonotope_inflate_vjp -> leb_vjp.
+"Measurement"): leb_nn_fwd -> leb_zonotope_inflate -> leb_zonotope_inflate_vjp -> leb_vjp, the forward in
+CERTIFIED mode (the library's default: every rounding error of the 3xTF32 path bounded and added outward).
 Rank 0 prints ONE JSON line.  `value` = bounded (timestep x state-dim) entries per second over all
 ranks with inputs resident in HBM; `e2e` = the same through the C ABI with host buffers
 (LEB_FLAG_HOST_IO: H2D/D2H copies inside the timed region); `roofline` = the dominant kernel's
-algorithmic flops / its CUDA-event time, measured during the timed steps; `cpu_baseline` = the
-oracle timed on this box's host cores on a bounded sample of the same workload.
+algorithmic flops / its CUDA-event time, measured during the timed steps; `value_mode` = the same step with the
+plain (parity-tested) forward; `configs` = the other BASELINE.json configurations (1 GPU, few steps) with the
+analytic kernels' ALU roofline; `cpu_baseline` = the oracle timed on this box's host cores on a bounded sample.
+
+--gpus N without a torchrun environment starts N ranks itself (one process per GPU, NCCL for the barrier and the
+max-over-ranks only: tiles are independent, there is no collective on the data path).
 
 --impl reference times the oracle (oracle/nn_oracle.py, as it stands) instead.
 """
@@ -173,8 +178,9 @@ def run_ours(args):
 
     REUSE = leb.FLAG_REUSE_FWD      # the VJP starts from the coefficient blocks the step's forward left in HBM (108 GB resident)
 
-    def step_device(fwd_flags=leb.FLAG_NO_MARGIN):
-        # value mode = the mode the parity tests compare with the oracle at this size; fwd_flags=0: certified forward (N6)
+    def step_device(fwd_flags=0):
+        # fwd_flags = 0: certified forward (N6), the library's default and the mode north_star sanctions for tensor cores;
+        # LEB_FLAG_NO_MARGIN: value mode, the mode the parity tests compare with the oracle at this size
         r_lo, r_hi = ctx.leb_nn_fwd(nom, rad, flags=fwd_flags)
         ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
         g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
@@ -187,10 +193,10 @@ def run_ours(args):
     hb.update({k: pin(w.B, w.T, w.N) for k in ("gn", "gr")})
 
     def step_host(count=False):
-        r_lo, r_hi = ctx.leb_nn_fwd(h_nom, h_rad, r_lo=hb["r_lo"], r_hi=hb["r_hi"], flags=leb.FLAG_NO_MARGIN | HOST)
+        r_lo, r_hi = ctx.leb_nn_fwd(h_nom, h_rad, r_lo=hb["r_lo"], r_hi=hb["r_hi"], flags=HOST)
         c, R = ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6, flags=HOST, c_bar=hb["c"], R_diag=hb["R"])
         g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(h_gc, h_gR, flags=HOST, g_lo=hb["g_lo"], g_hi=hb["g_hi"])
-        gn, gr = ctx.leb_vjp(1, h_nom, h_rad, g_lo, g_hi, grad_nom=hb["gn"], grad_rad=hb["gr"], flags=leb.FLAG_NO_MARGIN | HOST | REUSE)
+        gn, gr = ctx.leb_vjp(1, h_nom, h_rad, g_lo, g_hi, grad_nom=hb["gn"], grad_rad=hb["gr"], flags=HOST | REUSE)
         if count:
             nb = lambda *ts: sum(t.numel() * t.element_size() for t in ts)
             e2e_bytes["h2d"] = nb(h_nom, h_rad) + nb(r_lo, r_hi) + nb(h_gc, h_gR) + nb(h_nom, h_rad, g_lo, g_hi)
@@ -238,26 +244,28 @@ def run_ours(args):
     dt_max = sharding.max_over_ranks(dt, dev)
     e2e_value = world * entries_per_rank / dt_max
 
-    certified = None
+    assert ctx.leb_nn_state()[1:] == (True, True), "the timed step did not reuse its certified forward state"
+    value_mode = None
     if rank == 0:
         # outside the timed region: what the certified margin costs in tightness, against the value-mode (parity) result
         c_lo, c_hi = ctx.leb_nn_fwd(nom, rad, flags=0)
         v_lo, v_hi = ctx.leb_nn_fwd(nom, rad, flags=leb.FLAG_NO_MARGIN)
         width = (v_hi - v_lo).clamp_min(1e-12)
         ex = torch.maximum(c_hi - v_hi, v_lo - c_lo) / width
-        # the same step with the forward in certified mode (the gradient is then that of the certified bound, pads constant)
-        step_device(0)
+        # the same step with the forward in value mode (the mode the parity tests compare with the oracle)
+        step_device(leb.FLAG_NO_MARGIN)
         torch.cuda.synchronize()
         c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         c0.record()
         for _ in range(args.steps):
-            step_device(0)
+            step_device(leb.FLAG_NO_MARGIN)
         c1.record()
         torch.cuda.synchronize()
-        cert_ms = c0.elapsed_time(c1) / max(args.steps, 1)
-        certified = {"ms_per_step": cert_ms, "value": w.entries / (cert_ms * 1e-3),
-                     "excess_over_value_mode_median": float(ex.median()), "excess_over_value_mode_max": float(ex.max()),
-                     "unit": "fraction of the enclosure width", "contains_value_mode": bool((ex >= -1e-5).all())}
+        vm_ms = c0.elapsed_time(c1) / max(args.steps, 1)
+        value_mode = {"ms_per_step": vm_ms, "value": w.entries / (vm_ms * 1e-3),
+                      "certified_excess_over_value_mode_median": float(ex.median()),
+                      "certified_excess_over_value_mode_max": float(ex.max()),
+                      "unit": "fraction of the enclosure width", "certified_contains_value_mode": bool((ex >= -1e-5).all())}
     if rank == 0:
         peaks = _peaks()
         dom = max((0, 1), key=lambda kc: kstats[kc][0])
@@ -294,17 +302,92 @@ def run_ours(args):
                 "config": {"workload": WORKLOAD, "global_batch": 64 * world, "horizon": 100, "tiles": w.B * w.T * world,
                            "parallelism": f"dp{world} (independent tiles, no collective)",
                            "l2": "working set (82 GB of coefficient blocks, streamed once per chain step) exceeds the 126 MB L2; no flush needed",
-                           "mode": "value mode (LEB_FLAG_NO_MARGIN: the parity-tested result), VJP from the step's resident forward state "
-                                   "(LEB_FLAG_REUSE_FWD), 3xTF32 tcgen05 contractions; `certified` = the same step with the certified forward"},
+                           "mode": "certified forward (rounding errors of the 3xTF32 tcgen05 contractions bounded and added outward), VJP "
+                                   "from the step's resident forward state (LEB_FLAG_REUSE_FWD); `value_mode` = the same step with the "
+                                   "plain forward the parity tests compare with the oracle"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e_bytes["h2d"], "d2h_bytes_per_step": e2e_bytes["d2h"],
                         "ms_per_step": 1e3 * dt_max / max(args.steps, 1)},
-                "gpu_launches": launches_total, "roofline": roofline, "cpu_baseline": cpu, "certified": certified}
+                "gpu_launches": launches_total, "roofline": roofline, "cpu_baseline": cpu, "value_mode": value_mode}
+        ctx.close()
+        ctx = None
+        if world == 1 and not args.no_configs:
+            line["configs"] = {f"config{c}": _config_record(c, 3, 2, peaks) for c in (1, 2, 3, 4)}
         print(json.dumps(line))
-    ctx.close()
+    if ctx is not None:
+        ctx.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def _alu_peak(peaks):
+    """FP32 ALU roofline of the analytic kernels: interval arithmetic is directed-rounding FADD / FMUL and FMNMX, one FP32
+    operation per lane and instruction (no FMA contraction: every endpoint product is rounded on its own and goes through a
+    min / max), so peak = 148 SMs x 128 FP32 lanes x sm_max clock."""
+    return 148 * 128 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+
+
+def _config_record(cfg, steps, warmup, peaks):
+    """One of the other BASELINE.json configurations on cuda:0: the same step (forward -> fold -> fold VJP -> VJP),
+    device-resident inputs, few steps.  Parity-test cases, not the bench line."""
+    import torch
+    from paper_2607_01203_b200 import leb, workloads as wl
+    dev = torch.device("cuda", 0)
+    w = wl.make_config(cfg)
+    ctx = leb.context_for_workload(w, 0)
+    nom, rad = torch.from_numpy(w.nom).to(dev), torch.from_numpy(w.rad).to(dev)
+    gc, gR = torch.from_numpy(w.g_lo).to(dev), torch.from_numpy(w.g_hi).to(dev)
+    kind = 0 if w.kind == "analytic" else 1
+
+    def fwd():
+        return ctx.leb_analytic_fwd(nom, rad) if kind == 0 else ctx.leb_nn_fwd(nom, rad)
+
+    def step():
+        r_lo, r_hi = fwd()
+        ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
+        g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
+        return ctx.leb_vjp(kind, nom, rad, g_lo, g_hi, flags=leb.FLAG_REUSE_FWD if kind else 0)
+
+    def timed(f, n):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / max(n, 1)
+
+    for _ in range(warmup):
+        step()
+    launches0 = ctx.leb_launch_count()
+    ctx.leb_profile_reset()
+    ctx.leb_profile(True)
+    ms = timed(step, steps)
+    ctx.leb_profile(False)
+    launches = ctx.leb_launch_count() - launches0
+    rec = {"workload": f"{w.name}: {w.kind}, B={w.B} x T={w.T} tiles, n={w.n}, N={w.N}", "ms_per_step": ms,
+           "entries_per_s": w.entries / (ms * 1e-3), "gpu_launches_per_step": launches // max(steps, 1)}
+    if kind == 0:
+        peak = _alu_peak(peaks)
+        st = ctx.leb_analytic_tape_stats()
+        rec["tape"] = st
+        for name, kc in (("fwd_kernel", 2), ("vjp_kernel", 3)):
+            k_ms, k_flops, k_n = ctx.leb_profile_read(kc)
+            ach = (k_flops / 1e12) / (k_ms * 1e-3) if k_ms > 0 else 0.0
+            rec[name] = {"bound": "alu", "avg_launch_ms": k_ms / max(k_n, 1), "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                         "frac": ach / peak, "algorithmic_gflop_per_launch": k_flops / max(k_n, 1) / 1e9}
+    rec["ms_forward_only"] = timed(fwd, steps)
+    ctx.close()
+    return rec
+
+
+def _spawn_worker(local_rank, world, port, argv):
+    os.environ.update({"RANK": str(local_rank), "LOCAL_RANK": str(local_rank), "WORLD_SIZE": str(world),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    sys.argv = argv
+    sys.exit(main())
 
 
 def run_other_config(args):
@@ -323,13 +406,13 @@ def run_other_config(args):
     kind = 0 if w.kind == "analytic" else 1
 
     def fwd():
-        return ctx.leb_analytic_fwd(nom, rad) if kind == 0 else ctx.leb_nn_fwd(nom, rad, flags=leb.FLAG_NO_MARGIN)
+        return ctx.leb_analytic_fwd(nom, rad) if kind == 0 else ctx.leb_nn_fwd(nom, rad)
 
     def step():
         r_lo, r_hi = fwd()
         ctx.leb_zonotope_inflate(r_lo, r_hi, 1e-6)
         g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(gc, gR)
-        return ctx.leb_vjp(kind, nom, rad, g_lo, g_hi, flags=(leb.FLAG_NO_MARGIN | leb.FLAG_REUSE_FWD) if kind else 0)
+        return ctx.leb_vjp(kind, nom, rad, g_lo, g_hi, flags=leb.FLAG_REUSE_FWD if kind else 0)
 
     def timed(f, n):
         torch.cuda.synchronize()
@@ -365,9 +448,22 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=CONFIG_ID, choices=[1, 2, 3, 4, 5],
                     help="5 (default) = the bench line; 1-4 = the other BASELINE.json configurations, timing only")
+    ap.add_argument("--no-configs", action="store_true", help="skip the `configs` record (configs 1-4) of the bench line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.config == CONFIG_ID:
+        # launched without torchrun: start the N ranks here, one process per GPU
+        import torch
+        import torch.multiprocessing as mp
+        if torch.cuda.device_count() < args.gpus:
+            raise RuntimeError(f"--gpus {args.gpus} but only {torch.cuda.device_count()} CUDA devices are visible")
+        import socket
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+        mp.spawn(_spawn_worker, args=(args.gpus, port, list(sys.argv)), nprocs=args.gpus, join=True)
+        return 0
     if args.config != CONFIG_ID:
         return run_other_config(args)
     return run_ours(args)

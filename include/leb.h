@@ -211,6 +211,13 @@ leb_status leb_nn_chain_coeffs(leb_ctx* ctx, int target, float* out, void* strea
  * resident state (LEB_FLAG_REUSE_FWD honoured), 0 if it recomputed the forward. */
 leb_status leb_nn_state(leb_ctx* ctx, int* tiles, int* certified, int* vjp_reused);
 
+/* Statistics of the analytic model's interval tape (host-side query; roofline bookkeeping):
+ * *flops_per_tile = FP32 operations of one forward pass over one tile (directed-rounding add / mul, min / max, one
+ * per sin / cos / reciprocal), *ins_per_tile = interval instructions executed per tile (forward), *tape_ins =
+ * instructions stored, *tasks = path indices j with any non-zero Hessian entry, *max_slots = slots of the largest task. */
+leb_status leb_analytic_tape_stats(leb_ctx* ctx, double* flops_per_tile, long long* ins_per_tile, long long* tape_ins,
+                                   int* tasks, int* max_slots);
+
 /* Number of kernel launches the library has enqueued on this context so far. */
 long long leb_launch_count(const leb_ctx* ctx);
 
@@ -219,8 +226,9 @@ long long leb_launch_count(const leb_ctx* ctx);
  * 0 CROWN chain contraction (forward), 1 chain contraction (reverse sweep), 2 analytic forward,
  * 3 analytic VJP, 4 zonotope fold, 5 other NN kernels' GEMMs.
  * leb_profile_read synchronises `stream` and returns, for one class and since the last
- * leb_profile_reset: the summed device time in ms, the summed ALGORITHMIC work (flops computed
- * from the true, unpadded shapes; bytes for class 4; 0 for classes 2, 3) and the launch count. */
+ * leb_profile_reset: the summed device time in ms, the summed ALGORITHMIC work (classes 0, 1, 5: flops computed
+ * from the true, unpadded shapes; class 2: the tape's FP32 operations; class 3: three times that, the reverse sweep
+ * counted as twice the forward; class 4: bytes) and the launch count. */
 leb_status leb_profile(leb_ctx* ctx, int enable);
 leb_status leb_profile_read(leb_ctx* ctx, int kernel_class, double* ms, double* work, long long* launches,
                             void* stream);

@@ -327,6 +327,14 @@ leb_status leb_nn_state(leb_ctx* c, int* tiles, int* certified, int* vjp_reused)
     return LEB_OK;
 }
 
+leb_status leb_analytic_tape_stats(leb_ctx* c, double* flops_per_tile, long long* ins_per_tile, long long* tape_ins, int* tasks,
+                                   int* max_slots) {
+    if (!c || !flops_per_tile || !ins_per_tile || !tape_ins || !tasks || !max_slots) return LEB_ERR_ARG;
+    if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
+    leb_an_stats(c->an, flops_per_tile, ins_per_tile, tape_ins, tasks, max_slots);
+    return LEB_OK;
+}
+
 long long leb_launch_count(const leb_ctx* c) { return c ? c->launches : 0; }
 
 leb_status leb_profile(leb_ctx* c, int enable) {

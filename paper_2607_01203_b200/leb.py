@@ -27,7 +27,7 @@ FLAG_SINGLE_CTA = 16
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
 
@@ -263,6 +263,13 @@ class Context:
         t, c, r = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0)
         _chk(self.lib.leb_nn_state(self._ctx, ctypes.byref(t), ctypes.byref(c), ctypes.byref(r)), "leb_nn_state")
         return int(t.value), bool(c.value), bool(r.value)
+
+    def leb_analytic_tape_stats(self) -> dict:
+        f, i, t, k, m = ctypes.c_double(0), ctypes.c_longlong(0), ctypes.c_longlong(0), ctypes.c_int(0), ctypes.c_int(0)
+        _chk(self.lib.leb_analytic_tape_stats(self._ctx, ctypes.byref(f), ctypes.byref(i), ctypes.byref(t), ctypes.byref(k),
+                                              ctypes.byref(m)), "leb_analytic_tape_stats")
+        return {"flops_per_tile": float(f.value), "ins_per_tile": int(i.value), "tape_ins": int(t.value),
+                "tasks": int(k.value), "max_slots": int(m.value)}
 
     def leb_launch_count(self) -> int:
         return int(self.lib.leb_launch_count(self._ctx))

@@ -63,3 +63,53 @@ def test_world_size_2_gloo_partition_and_reductions():
         assert p.exitcode == 0
     assert t == 2.0 and n == total
     assert np.all(cover == 1)
+
+
+def _two_device_worker(rank, world, port, q):
+    """One process per GPU: its own leb context on its own device, its slice of the batch, NCCL for the reductions."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    import numpy as np
+    from paper_2607_01203_b200 import leb, workloads as wl
+    torch.cuda.set_device(rank)
+    dev = torch.device("cuda", rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+    w = wl.make_small_mlp([40, 64, 64, 64, 33], wl.ACT_TANH, 4, 6)       # wide enough for the tcgen05 path (200 KB smem launches)
+    a, b = sharding.shard_range(w.B, rank, world)
+    ctx = leb.context_for_workload(w, rank)
+    lo, hi = ctx.leb_nn_fwd(torch.from_numpy(w.nom[a:b]).to(dev), torch.from_numpy(w.rad[a:b]).to(dev), flags=leb.FLAG_NO_MARGIN)
+    torch.cuda.synchronize()
+    n = sharding.sum_over_ranks(b - a, dev)
+    q.put((rank, a, b, lo.cpu().numpy(), hi.cpu().numpy(), n))
+    ctx.close()
+    dist.destroy_process_group()
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_two_contexts_on_two_devices():
+    """weights replicated, tiles partitioned, no collective on the data path.  Needs >= 2 GPUs (skipped on the
+    1-GPU boxes this round has); also covers the per-device dynamic shared-memory attribute of the tcgen05 launches."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    from paper_2607_01203_b200 import build, leb, workloads as wl
+    build.build()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_two_device_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted([q.get(timeout=300) for _ in range(2)], key=lambda x: x[0])
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    w = wl.make_small_mlp([40, 64, 64, 64, 33], wl.ACT_TANH, 4, 6)
+    one = leb.context_for_workload(w, 0)
+    lo, hi = one.leb_nn_fwd(torch.from_numpy(w.nom).cuda(), torch.from_numpy(w.rad).cuda(), flags=leb.FLAG_NO_MARGIN)
+    got_lo = np.concatenate([r[3] for r in res]); got_hi = np.concatenate([r[4] for r in res])
+    assert np.array_equal(got_lo, lo.cpu().numpy()) and np.array_equal(got_hi, hi.cpu().numpy())
+    assert res[0][5] == w.B
+    one.close()
