@@ -110,13 +110,31 @@ def test_config5_full_size_sampled_tiles(mods, path):
     for a, b in ((gn, gn2), (gr, gr2)):      # same forward state; column sums are atomic adds, so not bit-identical
         assert float((a - b).abs().max()) <= 1e-5 * float(b.abs().max())
     nom, rad, g_lo, g_hi = _flat(w)
-    idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1])        # chunk boundaries, middle, last
+    if path == "tc":
+        # the default path (the one bench.py times): one tile of every trajectory forward (64 tiles),
+        # every fourth of those through the VJP (16 tiles); ~1 s of oracle time per tile
+        idx = np.arange(w.B) * w.T + (np.arange(w.B) * 37) % w.T
+        idx[0], idx[-1] = 0, w.B * w.T - 1
+        vi = idx[::4]
+    else:
+        idx = np.array([0, 1023, 1024, 3777, w.B * w.T - 1])        # chunk boundaries, middle, last
+        vi = idx[[0, 2, 4]]
     olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
-    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg5 r_lo")
-    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg5 r_hi")
-    vi = idx[[0, 2, 4]]
+    glo, ghi = to_np(lo).reshape(-1, w.n)[idx], to_np(hi).reshape(-1, w.n)[idx]
+    # relaxation case switches (reading R21): a tile whose hidden bound sits on a switch may take the other, equally
+    # valid, case; such tiles must be reported as ties by the oracle and are few
+    tol = lambda ref: 1e-5 * np.abs(ref) + 1e-7
+    off = np.nonzero(((np.abs(glo - olo) > tol(olo)) | (np.abs(ghi - ohi) > tol(ohi))).any(1))[0]
+    assert len(off) <= 2, f"{len(off)} of {len(idx)} sampled tiles miss the oracle"
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    for q in off:
+        assert len(O.relax_case_ties(Ws, bs, w.mlp.act, nom[idx[q]].astype(np.float64), rad[idx[q]].astype(np.float64))) > 0
+    keep = np.setdiff1d(np.arange(len(idx)), off)
+    assert_bounds_close(glo[keep], olo[keep], f"cfg5 {path} r_lo ({len(keep)} tiles)")
+    assert_bounds_close(ghi[keep], ohi[keep], f"cfg5 {path} r_hi ({len(keep)} tiles)")
+    vi = np.array([t for t in vi if t not in set(idx[off])])
     assert_nn_grads_close(O, w.mlp, nom[vi], rad[vi], g_lo[vi], g_hi[vi], to_np(gn).reshape(-1, w.N)[vi],
-                          to_np(gr).reshape(-1, w.N)[vi], "cfg5")
+                          to_np(gr).reshape(-1, w.N)[vi], f"cfg5 {path} ({len(vi)} tiles)")
     # properties that hold at any size: lo <= 0 <= hi (r(a~) = 0 lies in the enclosure), all finite
     assert bool((lo <= 0).all()) and bool((hi >= 0).all()) and bool(torch.isfinite(gn).all()) and bool(torch.isfinite(gr).all())
     ctx.close()
@@ -154,6 +172,61 @@ def test_config5_every_tile_both_paths(mods):
             ok |= bool(np.all(np.abs(glo - fw["r_lo"]) <= 1e-5 * np.abs(fw["r_lo"]) + 1e-7) and
                        np.all(np.abs(ghi - fw["r_hi"]) <= 1e-5 * np.abs(fw["r_hi"]) + 1e-7))
         assert ok, f"tile {t}: neither path matches the oracle"
+    ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_ragged_tile_count_at_full_width(mods, path):
+    """Config-5 architecture with 37 tiles: 37 * 1024 / 37 * 504 coefficient rows are not multiples of the 256-row block
+    per launch boundary of the tensor path, forward and VJP (the batch tail)."""
+    leb, wl, O = mods
+    w = wl.make_config(5, B=1, T=37)
+    ctx = leb.context_for_workload(w)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path] | leb.FLAG_REUSE_FWD)
+    nom, rad, g_lo, g_hi = _flat(w)
+    idx = np.array([0, 17, 35, 36])
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx])
+    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, f"ragged {path} r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, f"ragged {path} r_hi")
+    assert_nn_grads_close(O, w.mlp, nom[idx], rad[idx], g_lo[idx], g_hi[idx], to_np(gn).reshape(-1, w.N)[idx],
+                          to_np(gr).reshape(-1, w.N)[idx], f"ragged {path}")
+    ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_tanh_zero_radius_coordinates(mods, path):
+    """tanh nets with sigma_j = 0 on some coordinates, and on all of them: neurons fed only by zero-radius inputs have
+    point pre-activation intervals (u - l = 0: the degenerate line of reading R9, LINE_DEGEN in nn_relax.cuh), next to
+    ordinary neurons.  Forward against the oracle; VJP in the directions the oracle pins (not d/d sigma_j at sigma_j = 0)."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp([6, 40, 36, 33, 4], 2, 2, 3, rad_lo=0.02, rad_hi=0.2)
+    Wz = [x.copy() for x in w.mlp.W]
+    Wz[0][:10, 3:] = 0.0          # layer-1 neurons 0..9 see only inputs 0..2
+    Wz[1][:8, 10:] = 0.0          # layer-2 neurons 0..7 see only those
+    w.mlp.W = Wz
+    rad = w.rad.copy()
+    rad[..., :3] = 0.0
+    ctx = leb.context_for_workload(w)
+    nom_f, _, g_lo, g_hi = _flat(w)
+    rad_f = rad.reshape(-1, w.N)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(rad), flags=PATHS[path])
+    assert ctx.leb_domain_flag() == 0
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, 2, nom_f, rad_f)
+    assert_bounds_close(to_np(lo).reshape(-1, w.n), olo, f"tanh sigma_j=0 {path} r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n), ohi, f"tanh sigma_j=0 {path} r_hi")
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, 2, nom_f, rad_f, g_lo, g_hi)
+    assert_grads_close(to_np(gn).reshape(-1, w.N), to_np(gr).reshape(-1, w.N)[:, 3:], ogn, ogr[:, 3:], f"tanh sigma_j=0 {path}")
+    # certified mode on the same inputs contains the oracle enclosure
+    clo, chi = ctx.leb_nn_fwd(_dev(w.nom), _dev(rad), flags=PATHS[path] & ~1)
+    assert np.all(to_np(clo).reshape(-1, w.n) <= olo) and np.all(to_np(chi).reshape(-1, w.n) >= ohi)
+    # all radii zero: the exact bound is [0, 0]; value mode returns it to rounding, certified mode encloses it
+    z = torch.zeros_like(_dev(rad))
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), z, flags=PATHS[path])
+    assert float(lo.abs().max()) < 1e-6 and float(hi.abs().max()) < 1e-6
+    clo, chi = ctx.leb_nn_fwd(_dev(w.nom), z, flags=PATHS[path] & ~1)
+    assert bool((clo <= 0).all()) and bool((chi >= 0).all()) and float(chi.max()) < 1e-4 and float(clo.min()) > -1e-4
     ctx.close()
 
 

@@ -174,22 +174,55 @@ def test_certified_edge_cases(mods):
 
 
 @pytest.mark.parametrize("path", list(PATHS))
-def test_contraction_error_model(mods, path):
+def test_certified_strict_soundness_wide_tanh_net(mods, path):
+    """A 3-hidden-layer tanh net of width 128 (config-3 shape, tanh): 1e5 samples of the box plus 1e5 of its vertices per
+    tile, no tolerance; J is passed in FP32 so the remainder is defined with exactly that matrix (reading R12).  (At this
+    size the sampled extremum is far inside the bound -- SURVEY 8(c).7 -- so this guards the sign and the direction of
+    every pad rather than its size; the size is what the tiny-net test and the containment tests check.)"""
+    leb, wl, O = mods
+    w = wl.make_small_mlp([24, 128, 128, 128, 20], 2, 1, 3, seed=21, rad_lo=0.01, rad_hi=0.05, init="xavier")
+    ctx = leb.context_for_workload(w)
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    N = 24
+    J32 = np.stack([O.nominal(Ws, bs, 2, a0.astype(np.float64))[2] for a0 in w.nom.reshape(-1, N)]).astype(np.float32)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path])
+    clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+    rng = np.random.default_rng(21)
+    for t in range(w.B * w.T):
+        a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+        U = np.concatenate([rng.uniform(-1, 1, (100000, N)), rng.choice([-1.0, 1.0], (100000, N))])
+        X = a0[None, :] + U * sg[None, :]
+        _, p, _ = O.nominal(Ws, bs, 2, a0)
+        A = X.T
+        for l in range(len(Ws) - 1):
+            A = O.phi(2, Ws[l] @ A + bs[l][:, None])
+        r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
+        assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), t
+    ctx.close()
+
+
+@pytest.mark.parametrize("K", [128, 224, 512, 2048])
+@pytest.mark.parametrize("path", list(PATHS))
+def test_contraction_error_model(mods, path, K):
     """The rounding model behind the margin, probed on one chain step Lambda_0 = W_2 W_1 (ReLU, every
     hidden neuron stably active so that D = W_2 exactly; K = 512): |computed - exact| <= sum_j gamma_j |W_2[i,j]| |W_1[j,k]|
     elementwise, on operands built to be bad for a truncating block adder -- all-positive terms (every truncation loses),
     one large term followed by terms just below each candidate truncation grid, a large term in every block of 8 -- and on
     random ones.  Reports how much of the bound the worst case uses."""
     leb, wl, O = mods
-    K, N0, n = 512, 64, 64
+    N0, n = 64, 64
     j = np.arange(K)
     if path == "tc":
         gam = (4.5 * (K // 8 - j // 8) + 17.0) * 2.0 ** -23
     else:
         gam = (K - j + 4.0) * 2.0 ** -24 + 2.0 ** -23
     rng = np.random.default_rng(0)
+    sgn = rng.choice([-1.0, 1.0], (n, K))
     cases = {"pos": (rng.uniform(0.5, 1, (n, K)), rng.uniform(0.5, 1, (K, N0))),
-             "rand": (rng.standard_normal((n, K)), rng.standard_normal((K, N0)))}
+             "rand": (rng.standard_normal((n, K)), rng.standard_normal((K, N0))),
+             # mixed signs with cancellation: the exact result is much smaller than the sum of magnitudes
+             "mixed": (sgn * rng.uniform(0.5, 1, (n, K)), rng.uniform(0.5, 1, (K, N0))),
+             "alternating": (np.where(j % 2 == 0, 1.0, -1.0)[None, :] * np.ones((n, K)), 1.0 + 2.0 ** -12 * rng.integers(0, 2048, (K, N0)))}
     for p in range(22, 31):
         tiny = 2.0 ** -p * (1 - 2.0 ** -9)
         W2 = np.full((n, K), tiny); W2[:, 0] = 1.0
@@ -216,4 +249,6 @@ def test_contraction_error_model(mods, path):
             ratio = float(np.max(np.abs(lam[0, chain] - ref) / bound))
             worst = max(worst, ratio)
             assert ratio <= 1.0, (name, chain, ratio)
-    print(f"{path}: worst observed contraction error = {worst:.3f} of the model bound")
+    print(f"{path} K={K}: worst observed contraction error = {worst:.3f} of the model bound")
+    from parity_util import report
+    report(f"contraction error model {path} K={K} (observed error / model bound)", worst)
