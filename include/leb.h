@@ -139,6 +139,26 @@ leb_status leb_analytic_fwd(leb_ctx* ctx, int B, int T, const float* nom, const 
                             const float* mu, int ld_in, float* r_lo, float* r_hi, int ld_out,
                             unsigned flags, void* stream);
 
+/* Input-domain partitioning (Sec. IV-D): the box of every tile is cut into a grid of sub-boxes, splits[g] >= 1 equal
+ * parts along coordinate g (HOST array of N ints; at most 65536 sub-boxes per tile); every sub-box is bounded as a
+ * non-centred box about the same nominal point and the hull of the sub-box enclosures is returned.  Sound (every point of
+ * the box lies in a sub-box; FP32 sub-boxes are padded to overlap) and never wider than leb_analytic_fwd's enclosure
+ * (inclusion isotonicity).  Forward only.  Other arguments as leb_analytic_fwd. */
+leb_status leb_analytic_partition_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad, const float* mu,
+                                      int ld_in, const int* splits, float* r_lo, float* r_hi, int ld_out,
+                                      unsigned flags, void* stream);
+
+/* Nominal-point refinement by projected gradient descent (Sec. IV-D, Table II).  The box of every tile is
+ * FIXED (centre, rad); the nominal point a~ moves inside |a~ - centre| <= eps (componentwise) so as to shrink the total
+ * width W(a~) = sum_i (r_hi_i - r_lo_i) of the enclosure of the remainder about a~ on that box (mu = centre - a~).
+ * `steps` plain gradient steps a~ <- proj(a~ - lr dW/da~) (the paper gives no step rule: DESIGN.md reading R22), all on
+ * the device; the best iterate is kept.
+ *   centre, rad, eps : [B, T, ld_in]
+ *   nom              : [B, T, ld_in] in: starting points (inside the neighbourhood); out: best nominal points
+ *   width0, width    : [B, T] total width at the start / at the returned point */
+leb_status leb_analytic_pgd(leb_ctx* ctx, int B, int T, const float* centre, const float* rad, const float* eps, int ld_in,
+                            int steps, float lr, float* nom, float* width0, float* width, unsigned flags, void* stream);
+
 /* CROWN + Thm 3 bound, eq. (18)-(21) L196-220, for every tile.
  *   J      : NULL => the network's own Jacobian at a~ (eq. (7)); otherwise [B, T, n, N]
  *            dense, and the bound is with respect to that matrix (Thm 3 holds for any J).
@@ -189,6 +209,32 @@ leb_status leb_zonotope_inflate_vjp(leb_ctx* ctx, int B, int T, int n, const flo
                                     const float* gR, float* g_lo, float* g_hi, unsigned flags,
                                     void* stream);
 
+/* Disturbance-error enclosure, eq. (22): r_dist = (E(x) - E_k) w in ([E](Omega^x) (-) E_k) E_nw, added IN PLACE to
+ * the linearization-error enclosure (r = r_lin + r_dist, L228), outward rounded.  The caller supplies the interval
+ * enclosure of the disturbance matrix over the state tube (the paper's systems all have constant E, for which this
+ * call adds nothing).
+ *   E_lo, E_hi, E_nom : [B, T, n, nw]  E_lo <= E(x) <= E_hi on the tube, E_nom = E(z_k)
+ *   r_lo, r_hi        : [B, T, n] contiguous, updated */
+leb_status leb_dist_add(leb_ctx* ctx, int B, int T, int n, int nw, const float* E_lo, const float* E_hi,
+                        const float* E_nom, float* r_lo, float* r_hi, unsigned flags, void* stream);
+
+/* Tube propagation, eq. (27)-(28) L289-291: for k = 1..T
+ *     h_mu_k = sum_{j<k} Phi_{k,j} c_bar_j,   h_sigma_k = sum_{j<k} || Phi_{k,j} [diag(E) diag(R_bar_j)] ||_{1,r}
+ * (row-wise 1-norm; every operation of h_sigma rounded up: it is a bound).
+ *   Phi          : [B, T (T+1) / 2, N, n], N = n + m: block (k-1) k / 2 + j holds Phi_{k,j} = [Phi^x; Phi^u], 0 <= j < k <= T
+ *   c_bar, R_diag: [B, T, n] (leb_zonotope_inflate's outputs);  E_diag: [n] or NULL (= 0)
+ *   h_mu, h_sigma: [B, T, N], row k-1 = time k.   n > 8192: LEB_ERR_UNSUPPORTED. */
+leb_status leb_tube_propagate(leb_ctx* ctx, int B, int T, int n, int m, const float* Phi, const float* c_bar,
+                              const float* R_diag, const float* E_diag, float* h_mu, float* h_sigma,
+                              unsigned flags, void* stream);
+
+/* Propagated-error penalty, eq. (35) L360 (the sum over k read as k = j+1..T: Phi_{j,j} does not exist in (26)-(28)):
+ *     J_err[b] = sum_j sum_{k>j} || Phi_{k,j} [diag(E) diag(R_bar_j)] ||_F^2,   grad_R = d J_err / d R_diag [B, T, n]
+ * grad_R (may be NULL) is the cotangent gR of leb_zonotope_inflate_vjp, which leb_vjp then takes to (a~, sigma).
+ *   J_err : [B].   n > 1024: LEB_ERR_UNSUPPORTED. */
+leb_status leb_jerr(leb_ctx* ctx, int B, int T, int n, int m, const float* Phi, const float* R_diag,
+                    const float* E_diag, float* J_err, float* grad_R, unsigned flags, void* stream);
+
 /* *flag = 1 if any tile of any call since the last leb_domain_flag() hit a domain error
  * (synchronises `stream`, then clears the flag). */
 leb_status leb_domain_flag(leb_ctx* ctx, int* flag, void* stream);
@@ -224,11 +270,11 @@ long long leb_launch_count(const leb_ctx* ctx);
 /* Measurement aid (bench.py "roofline"): while enabled, every launch of
  * the library's kernels is bracketed by CUDA events on the launching stream.  Kernel classes:
  * 0 CROWN chain contraction (forward), 1 chain contraction (reverse sweep), 2 analytic forward,
- * 3 analytic VJP, 4 zonotope fold, 5 other NN kernels' GEMMs.
+ * 3 analytic VJP, 4 zonotope fold, 5 other NN kernels' GEMMs, 6 disturbance error / tube propagation / J_err.
  * leb_profile_read synchronises `stream` and returns, for one class and since the last
  * leb_profile_reset: the summed device time in ms, the summed ALGORITHMIC work (classes 0, 1, 5: flops computed
  * from the true, unpadded shapes; class 2: the tape's FP32 operations; class 3: three times that, the reverse sweep
- * counted as twice the forward; class 4: bytes) and the launch count. */
+ * counted as twice the forward; classes 4, 6: bytes) and the launch count. */
 leb_status leb_profile(leb_ctx* ctx, int enable);
 leb_status leb_profile_read(leb_ctx* ctx, int kernel_class, double* ms, double* work, long long* launches,
                             void* stream);

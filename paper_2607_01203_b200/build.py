@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libleb.so")
-SOURCES = ["api.cu", "an_compile.cu", "analytic.cu", "inflate.cu", "nn.cu"]
+SOURCES = ["api.cu", "an_compile.cu", "analytic.cu", "inflate.cu", "tube.cu", "nn.cu"]
 HEADERS = ["an_tape.h", "internal.h", "nn_relax.cuh", "nn_gemm_ffma.cuh", "../../include/leb.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

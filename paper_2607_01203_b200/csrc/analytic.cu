@@ -413,6 +413,88 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 3) an_vm_kernel(DevTape P
     }
 }
 
+// ------------------------------------------------------------------ refinements built on forward + VJP (Table II)
+// input-domain partitioning: sub-box p of tile t along coordinate g: part q_g = (p / stride_g) % splits_g of splits_g equal
+// parts.  The sub-radius is rounded up and padded by a few ulps of the box so that the FP32 sub-boxes cover the box.
+__global__ void subbox_kernel(size_t tiles, int P, int N, int ld_in, const int* __restrict__ splits, const int* __restrict__ strides,
+                              const float* __restrict__ nom, const float* __restrict__ rad, const float* __restrict__ mu,
+                              float* __restrict__ nom_x, float* __restrict__ rad_x, float* __restrict__ mu_x) {
+    const size_t total = tiles * (size_t)P * N;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int g = (int)(idx % N);
+        const size_t tp = idx / N;
+        const int p = (int)(tp % P);
+        const size_t t = tp / P;
+        const int s = splits[g], q = (p / strides[g]) % s;
+        const float r = rad[t * ld_in + g], m = mu ? mu[t * ld_in + g] : 0.f;
+        nom_x[idx] = nom[t * ld_in + g];
+        if (s == 1) { rad_x[idx] = r; mu_x[idx] = m; continue; }
+        const float inv = 1.f / (float)s;
+        rad_x[idx] = __fadd_ru(__fmul_ru(r, inv), 4.f * 1.1920929e-07f * (fabsf(m) + r));
+        mu_x[idx] = fmaf(r, fmaf((float)(2 * q + 1), inv, -1.f), m);
+    }
+}
+
+// hull over the P sub-boxes of a tile
+__global__ void hull_kernel(size_t tiles, int P, int n, int ld_out, const float* __restrict__ lo_x, const float* __restrict__ hi_x,
+                            float* __restrict__ r_lo, float* __restrict__ r_hi) {
+    const size_t total = tiles * (size_t)n;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t t = idx / n;
+        const int l = (int)(idx - t * n);
+        float lo = INFINITY, hi = -INFINITY;
+        for (int p = 0; p < P; ++p) {
+            const size_t o = (t * P + p) * (size_t)n + l;
+            lo = fminf(lo, lo_x[o]);
+            hi = fmaxf(hi, hi_x[o]);
+            if (!(lo_x[o] == lo_x[o])) { lo = -INFINITY; hi = INFINITY; }
+        }
+        r_lo[t * ld_out + l] = lo;
+        r_hi[t * ld_out + l] = hi;
+    }
+}
+
+// PGD: mu = centre - nom
+__global__ void pgd_mu_kernel(size_t count, const float* __restrict__ centre, const float* __restrict__ nom, float* __restrict__ mu) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (size_t)gridDim.x * blockDim.x) mu[i] = centre[i] - nom[i];
+}
+__global__ void fill_kernel(size_t count, float v, float* __restrict__ a) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (size_t)gridDim.x * blockDim.x) a[i] = v;
+}
+// one block per tile: width of the enclosure, keep the best iterate, take the projected gradient step
+__global__ void pgd_step_kernel(int n, int N, int ld_in, int first, int last, float lr, const float* __restrict__ lo,
+                                const float* __restrict__ hi, const float* __restrict__ gn, const float* __restrict__ gm,
+                                const float* __restrict__ centre, const float* __restrict__ eps, float* __restrict__ cur,
+                                float* __restrict__ best_nom, float* __restrict__ w0, float* __restrict__ wbest) {
+    __shared__ float red[32];
+    __shared__ int take;
+    const size_t t = blockIdx.x;
+    float w = 0.f;
+    for (int l = threadIdx.x; l < n; l += blockDim.x) w += hi[t * n + l] - lo[t * n + l];
+    for (int off = 16; off; off >>= 1) w += __shfl_xor_sync(FULL, w, off);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = w;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float tot = 0.f;
+        for (int q = 0; q < (int)(blockDim.x >> 5); ++q) tot += red[q];
+        if (first) { w0[t] = tot; wbest[t] = tot; take = 1; }
+        else if (tot < wbest[t]) { wbest[t] = tot; take = 1; }
+        else take = 0;
+    }
+    __syncthreads();
+    for (int g = threadIdx.x; g < N; g += blockDim.x) {
+        const size_t o = t * ld_in + g;
+        const float x = cur[o];
+        if (take) best_nom[o] = x;
+        if (!last) {
+            const float d = gn[o] - gm[o];            // d W / d a~ with the box fixed (mu = centre - a~)
+            float y = x - lr * d;
+            y = fminf(fmaxf(y, centre[o] - eps[o]), centre[o] + eps[o]);
+            if (y == y) cur[o] = y;
+        }
+    }
+}
+
 // ------------------------------------------------------------------ fixed-order reductions over the tasks
 // one block per tile: validates the tile's inputs, then thread l adds the partial rows of output l in ascending j
 __global__ void an_reduce_fwd_kernel(DevTape P, int tiles_pad, const float* __restrict__ nom, const float* __restrict__ rad,
@@ -500,6 +582,11 @@ struct AnState {
     unsigned* counter = nullptr;
     int num_sms = 148;
     bool attr_done = false;
+    // scratch of the refinements (partitioning, PGD): grown on demand
+    float* scratch[12] = {nullptr};
+    size_t scratch_bytes[12] = {0};
+    int* d_splits = nullptr;      // [2][N]: splits, strides
+    size_t d_splits_n = 0;
 };
 
 AnState* leb_an_create() {
@@ -527,6 +614,8 @@ void leb_an_destroy(AnState* S) {
     if (S->partial_mu) cudaFree(S->partial_mu);
     if (S->tile_bad) cudaFree(S->tile_bad);
     if (S->counter) cudaFree(S->counter);
+    for (int i = 0; i < 12; ++i) if (S->scratch[i]) cudaFree(S->scratch[i]);
+    if (S->d_splits) cudaFree(S->d_splits);
     delete S;
 }
 
@@ -663,6 +752,79 @@ static leb_status an_run(AnState* S, bool vjp, int tiles, const float* nom, cons
     if (vjp) an_reduce_vjp_kernel<<<tiles, threads, 0, st>>>(D, A.tiles_pad, nom, rad, mu, ld_in, S->partial, A.partial_mu, S->tile_bad, grad_nom, grad_rad, grad_mu, domain_flag);
     else an_reduce_fwd_kernel<<<tiles, threads, 0, st>>>(D, A.tiles_pad, nom, rad, mu, ld_in, S->partial, S->tile_bad, r_lo, r_hi, ld_out, domain_flag);
     ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+static float* scratch(AnState* S, int slot, size_t count) {
+    if (!grow(&S->scratch[slot], &S->scratch_bytes[slot], std::max<size_t>(count, 4) * sizeof(float))) return nullptr;
+    return S->scratch[slot];
+}
+static unsigned gs_blocks(size_t work) { return (unsigned)std::min<size_t>((work + 255) / 256, 148 * 16); }
+
+// input-domain partitioning: hull of the bounds of the grid of sub-boxes, every sub-box a non-centred box
+// about the same nominal point
+leb_status leb_an_partition(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                            const int* splits_host, float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
+                            long long* launches, LebProf* prof) {
+    if (tiles == 0) return LEB_OK;
+    const int N = S->model.N, n = S->model.n;
+    std::vector<int> tab(2 * (size_t)N);
+    long long P = 1;
+    for (int g = N - 1; g >= 0; --g) {
+        if (splits_host[g] < 1) return LEB_ERR_ARG;
+        tab[g] = splits_host[g];
+        tab[N + g] = (int)P;
+        P *= splits_host[g];
+        if (P > 65536) return LEB_ERR_SHAPE;
+    }
+    if ((long long)tiles * P > 2000000000LL) return LEB_ERR_SHAPE;
+    if (S->d_splits_n < 2 * (size_t)N) {
+        if (S->d_splits) { cudaDeviceSynchronize(); cudaFree(S->d_splits); S->d_splits = nullptr; }
+        if (cudaMalloc(&S->d_splits, 2 * (size_t)N * sizeof(int)) != cudaSuccess) return LEB_ERR_NOMEM;
+        S->d_splits_n = 2 * (size_t)N;
+    }
+    cudaStreamSynchronize(st);        // the table of a previous call may still be in use
+    if (cudaMemcpy(S->d_splits, tab.data(), 2 * (size_t)N * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) return LEB_ERR_CUDA;
+    const size_t xt = (size_t)tiles * (size_t)P;
+    float *nx = scratch(S, 0, xt * N), *rx = scratch(S, 1, xt * N), *mx = scratch(S, 2, xt * N), *lx = scratch(S, 3, xt * n), *hx = scratch(S, 4, xt * n);
+    if (!nx || !rx || !mx || !lx || !hx) return LEB_ERR_NOMEM;
+    subbox_kernel<<<gs_blocks(xt * N), 256, 0, st>>>((size_t)tiles, (int)P, N, ld_in, S->d_splits, S->d_splits + N, nom, rad, mu, nx, rx, mx);
+    ++*launches;
+    leb_status es = an_run(S, false, (int)xt, nx, rx, mx, N, lx, hx, nullptr, nullptr, n, nullptr, nullptr, nullptr, domain_flag, st, launches, prof);
+    if (es != LEB_OK) return es;
+    hull_kernel<<<gs_blocks((size_t)tiles * n), 256, 0, st>>>((size_t)tiles, (int)P, n, ld_out, lx, hx, r_lo, r_hi);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+// nominal refinement by projected gradient descent (Table II): box (centre, rad) fixed, nominal point inside
+// |a~ - centre| <= eps, objective = total width of the enclosure of the remainder about a~
+leb_status leb_an_pgd(AnState* S, int tiles, const float* centre, const float* rad, const float* eps, int ld_in, int steps, float lr,
+                      float* nom, float* w0, float* wbest, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
+    if (tiles == 0) return LEB_OK;
+    const int N = S->model.N, n = S->model.n;
+    const size_t ci = (size_t)tiles * ld_in, co = (size_t)tiles * n;
+    float *cur = scratch(S, 0, ci), *mu = scratch(S, 1, ci), *gn = scratch(S, 2, ci), *gr = scratch(S, 5, ci), *gm = scratch(S, 6, ci);
+    float *lo = scratch(S, 3, co), *hi = scratch(S, 4, co), *glo = scratch(S, 7, co), *ghi = scratch(S, 8, co);
+    if (!cur || !mu || !gn || !gr || !gm || !lo || !hi || !glo || !ghi) return LEB_ERR_NOMEM;
+    if (cudaMemcpyAsync(cur, nom, ci * sizeof(float), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return LEB_ERR_CUDA;
+    fill_kernel<<<gs_blocks(co), 256, 0, st>>>(co, -1.f, glo);
+    fill_kernel<<<gs_blocks(co), 256, 0, st>>>(co, 1.f, ghi);
+    cudaMemsetAsync(gn, 0, ci * sizeof(float), st);
+    cudaMemsetAsync(gm, 0, ci * sizeof(float), st);
+    *launches += 2;
+    for (int it = 0; it <= steps; ++it) {
+        pgd_mu_kernel<<<gs_blocks(ci), 256, 0, st>>>(ci, centre, cur, mu);
+        ++*launches;
+        leb_status es = an_run(S, false, tiles, cur, rad, mu, ld_in, lo, hi, nullptr, nullptr, n, nullptr, nullptr, nullptr, domain_flag, st, launches, prof);
+        if (es != LEB_OK) return es;
+        if (it < steps) {
+            es = an_run(S, true, tiles, cur, rad, mu, ld_in, nullptr, nullptr, glo, ghi, n, gn, gr, gm, domain_flag, st, launches, prof);
+            if (es != LEB_OK) return es;
+        }
+        pgd_step_kernel<<<tiles, 128, 0, st>>>(n, N, ld_in, it == 0, it == steps, lr, lo, hi, gn, gm, centre, eps, cur, nom, w0, wbest);
+        ++*launches;
+    }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
 

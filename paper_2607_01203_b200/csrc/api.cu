@@ -165,6 +165,61 @@ leb_status leb_analytic_fwd(leb_ctx* c, int B, int T, const float* nom, const fl
     return ok ? LEB_OK : LEB_ERR_CUDA;
 }
 
+leb_status leb_analytic_partition_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, int ld_in,
+                                      const int* splits, float* r_lo, float* r_hi, int ld_out, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || !splits) return LEB_ERR_ARG;
+    if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
+    leb_status s = check_traj(B, T, leb_an_N(c->an), leb_an_n(c->an), ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(mu) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_mu = in_ptr(c, 4, mu, tiles * ld_in, host, st, &ok);
+    float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
+    float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    s = leb_an_partition(c->an, (int)tiles, d_nom, d_rad, d_mu, ld_in, splits, d_lo, d_hi, ld_out, c->domain_flag, st, &c->launches, &c->prof);
+    if (s != LEB_OK) return s;
+    out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
+    out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_analytic_pgd(leb_ctx* c, int B, int T, const float* centre, const float* rad, const float* eps, int ld_in, int steps,
+                            float lr, float* nom, float* width0, float* width, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || steps < 0 || !(lr >= 0.f)) return LEB_ERR_ARG;
+    if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!centre || !rad || !eps || !nom || !width0 || !width) return LEB_ERR_ARG;
+    if (ld_in < leb_an_N(c->an)) return LEB_ERR_SHAPE;
+    if (!al4(centre) || !al4(rad) || !al4(eps) || !al4(nom) || !al4(width0) || !al4(width)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_c = in_ptr(c, 0, centre, tiles * ld_in, host, st, &ok);
+    const float* d_r = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_e = in_ptr(c, 4, eps, tiles * ld_in, host, st, &ok);
+    float* d_n = const_cast<float*>(in_ptr(c, 2, nom, tiles * ld_in, host, st, &ok));
+    float* d_w0 = out_ptr(c, 6, width0, tiles, host, &ok);
+    float* d_w = out_ptr(c, 7, width, tiles, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    leb_status s = leb_an_pgd(c->an, (int)tiles, d_c, d_r, d_e, ld_in, steps, lr, d_n, d_w0, d_w, c->domain_flag, st, &c->launches, &c->prof);
+    if (s != LEB_OK) return s;
+    out_copy(nom, d_n, tiles * ld_in, host, st, &ok);
+    out_copy(width0, d_w0, tiles, host, st, &ok);
+    out_copy(width, d_w, tiles, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
 leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, const float* J, int ld_in,
                       float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, void* stream) {
     if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
@@ -291,6 +346,83 @@ leb_status leb_zonotope_inflate_vjp(leb_ctx* c, int B, int T, int n, const float
     if (leb_launch_inflate_vjp(count, d_gc, d_gR, d_lo, d_hi, st, &c->launches) != cudaSuccess) return LEB_ERR_CUDA;
     out_copy(g_lo, d_lo, count, host, st, &ok);
     out_copy(g_hi, d_hi, count, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_dist_add(leb_ctx* c, int B, int T, int n, int nw, const float* E_lo, const float* E_hi, const float* E_nom,
+                        float* r_lo, float* r_hi, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || n < 1 || nw < 1) return LEB_ERR_ARG;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!E_lo || !E_hi || !E_nom || !r_lo || !r_hi) return LEB_ERR_ARG;
+    if (!al4(E_lo) || !al4(E_hi) || !al4(E_nom) || !al4(r_lo) || !al4(r_hi)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t rows = (size_t)B * T * n;
+    bool ok = true;
+    const float* d_a = in_ptr(c, 0, E_lo, rows * nw, host, st, &ok);
+    const float* d_b = in_ptr(c, 1, E_hi, rows * nw, host, st, &ok);
+    const float* d_c = in_ptr(c, 4, E_nom, rows * nw, host, st, &ok);
+    float* d_lo = const_cast<float*>(in_ptr(c, 2, r_lo, rows, host, st, &ok));
+    float* d_hi = const_cast<float*>(in_ptr(c, 3, r_hi, rows, host, st, &ok));
+    if (!ok) return LEB_ERR_NOMEM;
+    if (leb_launch_dist_add(rows, nw, d_a, d_b, d_c, d_lo, d_hi, st, &c->launches, &c->prof) != cudaSuccess) return LEB_ERR_CUDA;
+    out_copy(r_lo, d_lo, rows, host, st, &ok);
+    out_copy(r_hi, d_hi, rows, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_tube_propagate(leb_ctx* c, int B, int T, int n, int m, const float* Phi, const float* c_bar, const float* R_diag,
+                              const float* E_diag, float* h_mu, float* h_sigma, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || n < 1 || m < 0) return LEB_ERR_ARG;
+    if (n > 8192) return LEB_ERR_UNSUPPORTED;
+    if (T > 65535 || B > 65535) return LEB_ERR_SHAPE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!Phi || !c_bar || !R_diag || !h_mu || !h_sigma) return LEB_ERR_ARG;
+    if (((uintptr_t)Phi & 15) || !al4(c_bar) || !al4(R_diag) || !al4(E_diag) || !al4(h_mu) || !al4(h_sigma)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const int N = n + m;
+    const size_t nphi = (size_t)B * ((size_t)T * (T + 1) / 2) * N * n, nv = (size_t)B * T * n, no = (size_t)B * T * N;
+    bool ok = true;
+    const float* d_P = in_ptr(c, 0, Phi, nphi, host, st, &ok);
+    const float* d_c = in_ptr(c, 1, c_bar, nv, host, st, &ok);
+    const float* d_R = in_ptr(c, 2, R_diag, nv, host, st, &ok);
+    const float* d_E = in_ptr(c, 4, E_diag, n, host, st, &ok);
+    float* d_m = out_ptr(c, 6, h_mu, no, host, &ok);
+    float* d_s = out_ptr(c, 7, h_sigma, no, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    if (leb_launch_tube(B, T, n, N, d_P, d_c, d_R, d_E, d_m, d_s, st, &c->launches, &c->prof) != cudaSuccess) return LEB_ERR_CUDA;
+    out_copy(h_mu, d_m, no, host, st, &ok);
+    out_copy(h_sigma, d_s, no, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_jerr(leb_ctx* c, int B, int T, int n, int m, const float* Phi, const float* R_diag, const float* E_diag,
+                    float* J_err, float* grad_R, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || n < 1 || m < 0) return LEB_ERR_ARG;
+    if (n > 1024) return LEB_ERR_UNSUPPORTED;
+    if (T > 65535 || B > 65535) return LEB_ERR_SHAPE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!Phi || !R_diag || !J_err) return LEB_ERR_ARG;
+    if (!al4(Phi) || !al4(R_diag) || !al4(E_diag) || !al4(J_err) || !al4(grad_R)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const int N = n + m;
+    const size_t nphi = (size_t)B * ((size_t)T * (T + 1) / 2) * N * n, nv = (size_t)B * T * n;
+    bool ok = true;
+    const float* d_P = in_ptr(c, 0, Phi, nphi, host, st, &ok);
+    const float* d_R = in_ptr(c, 2, R_diag, nv, host, st, &ok);
+    const float* d_E = in_ptr(c, 4, E_diag, n, host, st, &ok);
+    float* d_J = out_ptr(c, 6, J_err, (size_t)B, host, &ok);
+    float* d_g = out_ptr(c, 7, grad_R, nv, host, &ok);
+    float* d_part = stage_buf(c, 5, (size_t)B * T * sizeof(float));
+    if (!ok || !d_part) return LEB_ERR_NOMEM;
+    if (leb_launch_jerr(B, T, n, N, d_P, d_R, d_E, d_part, d_J, d_g, st, &c->launches, &c->prof) != cudaSuccess) return LEB_ERR_CUDA;
+    out_copy(J_err, d_J, (size_t)B, host, st, &ok);
+    out_copy(grad_R, d_g, nv, host, st, &ok);
     return ok ? LEB_OK : LEB_ERR_CUDA;
 }
 

@@ -22,7 +22,7 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T);      // an_compile
 // kernel class, on the launching stream, so that bench.py can report the dominant kernel's average
 // launch duration measured live over the timed region.
 enum { LEB_KC_CHAIN_FWD = 0, LEB_KC_CHAIN_BWD = 1, LEB_KC_ANALYTIC_FWD = 2, LEB_KC_ANALYTIC_VJP = 3,
-       LEB_KC_INFLATE = 4, LEB_KC_NN_OTHER = 5, LEB_KC_COUNT = 6 };
+       LEB_KC_INFLATE = 4, LEB_KC_NN_OTHER = 5, LEB_KC_TUBE = 6, LEB_KC_COUNT = 7 };
 struct LebProf {
     bool on = false;
     struct Rec { cudaEvent_t a, b; int kc; };
@@ -69,6 +69,11 @@ leb_status leb_an_forward(AnState*, int tiles, const float* nom, const float* ra
 leb_status leb_an_vjp(AnState*, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo,
                       const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu,
                       int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
+leb_status leb_an_partition(AnState*, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                            const int* splits_host, float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
+                            long long* launches, LebProf* prof);
+leb_status leb_an_pgd(AnState*, int tiles, const float* centre, const float* rad, const float* eps, int ld_in, int steps, float lr,
+                      float* nom, float* w0, float* wbest, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
 void leb_an_stats(const AnState*, double* flops_fwd, long long* ins_fwd, long long* tape_ins, int* ntasks, int* max_slots);
 
 // ---- zonotope fold (inflate.cu)
@@ -77,6 +82,15 @@ cudaError_t leb_launch_inflate(size_t rows, int n, const float* r_lo, const floa
                                LebProf* prof);
 cudaError_t leb_launch_inflate_vjp(size_t count, const float* gc, const float* gR, float* g_lo, float* g_hi,
                                    cudaStream_t st, long long* launches);
+
+// ---- disturbance error, tube propagation, J_err (tube.cu)
+cudaError_t leb_launch_dist_add(size_t rows, int nw, const float* E_lo, const float* E_hi, const float* E_nom, float* r_lo,
+                                float* r_hi, cudaStream_t st, long long* launches, LebProf* prof);
+cudaError_t leb_launch_tube(int B, int T, int n, int N, const float* Phi, const float* c_bar, const float* R_diag,
+                            const float* E_diag, float* h_mu, float* h_sigma, cudaStream_t st, long long* launches,
+                            LebProf* prof);
+cudaError_t leb_launch_jerr(int B, int T, int n, int N, const float* Phi, const float* R_diag, const float* E_diag,
+                            float* partial, float* J, float* grad_R, cudaStream_t st, long long* launches, LebProf* prof);
 
 // ---- NN path (nn.cu)
 struct NnState;   // packed weights + workspace, owned by the context

@@ -26,7 +26,7 @@ FLAG_SINGLE_CTA = 16
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
-    "leb_analytic_fwd", "leb_nn_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp",
+    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_pgd", "leb_nn_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
     "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
@@ -176,6 +176,32 @@ class Context:
                                        int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_fwd")
         return r_lo, r_hi
 
+    def leb_analytic_partition_fwd(self, nom, rad, splits, mu=None, flags: int = 0):
+        """Hull of the bounds of the grid of sub-boxes (splits[g] parts along coordinate g)."""
+        _check_f32(nom, rad, mu)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        r_lo = self._out(nom, (B, T, self.n), host)
+        r_hi = self._out(nom, (B, T, self.n), host)
+        sp = (ctypes.c_int * self.N)(*[int(x) for x in splits])
+        _chk(self.lib.leb_analytic_partition_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), ld_in, sp, _ptr(r_lo), _ptr(r_hi),
+                                                 self.n, ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_partition_fwd")
+        return r_lo, r_hi
+
+    def leb_analytic_pgd(self, centre, rad, eps, nom0, steps: int, lr: float, flags: int = 0):
+        """PGD refinement of the nominal point; returns (best nominal points, initial widths, best widths)."""
+        _check_f32(centre, rad, eps, nom0)
+        B, T, ld_in = self._bt(centre)
+        host = bool(flags & FLAG_HOST_IO)
+        nom = nom0.clone()
+        if host:
+            nom = nom.pin_memory()
+        w0 = self._out(centre, (B, T), host)
+        w = self._out(centre, (B, T), host)
+        _chk(self.lib.leb_analytic_pgd(self._ctx, B, T, _ptr(centre), _ptr(rad), _ptr(eps), ld_in, int(steps), ctypes.c_float(lr),
+                                       _ptr(nom), _ptr(w0), _ptr(w), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_pgd")
+        return nom, w0, w
+
     def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = 0):
         """flags = 0 is the C ABI's default: CERTIFIED mode (rounding errors bounded and added outward).
         FLAG_NO_MARGIN selects value mode, the plain FP32 result the parity tests compare with the oracle."""
@@ -239,6 +265,37 @@ class Context:
         _chk(self.lib.leb_zonotope_inflate_vjp(self._ctx, B, T, n, _ptr(gc), _ptr(gR), _ptr(g_lo), _ptr(g_hi),
                                                ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_zonotope_inflate_vjp")
         return g_lo, g_hi
+
+    def leb_dist_add(self, E_lo, E_hi, E_nom, r_lo, r_hi, flags: int = 0):
+        """(22): adds the disturbance-error enclosure to (r_lo, r_hi) in place.  E_*: [B, T, n, nw]."""
+        _check_f32(E_lo, E_hi, E_nom, r_lo, r_hi)
+        B, T, n, nw = (int(x) for x in E_lo.shape)
+        _chk(self.lib.leb_dist_add(self._ctx, B, T, n, nw, _ptr(E_lo), _ptr(E_hi), _ptr(E_nom), _ptr(r_lo), _ptr(r_hi),
+                                   ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_dist_add")
+        return r_lo, r_hi
+
+    def leb_tube_propagate(self, Phi, c_bar, R_diag, m: int, E_diag=None, flags: int = 0):
+        """(27)-(28): Phi [B, T(T+1)/2, n+m, n] packed; returns h_mu, h_sigma [B, T, n+m] (row k-1 = time k)."""
+        _check_f32(Phi, c_bar, R_diag, E_diag)
+        B, T, n = self._bt(c_bar)
+        host = bool(flags & FLAG_HOST_IO)
+        h_mu = self._out(c_bar, (B, T, n + m), host)
+        h_sigma = self._out(c_bar, (B, T, n + m), host)
+        _chk(self.lib.leb_tube_propagate(self._ctx, B, T, n, int(m), _ptr(Phi), _ptr(c_bar), _ptr(R_diag), _ptr(E_diag),
+                                         _ptr(h_mu), _ptr(h_sigma), ctypes.c_uint(flags), _stream_ptr(self.device)),
+             "leb_tube_propagate")
+        return h_mu, h_sigma
+
+    def leb_jerr(self, Phi, R_diag, m: int, E_diag=None, with_grad: bool = True, flags: int = 0):
+        """(35): returns J_err [B] and d J_err / d R_diag [B, T, n] (or None)."""
+        _check_f32(Phi, R_diag, E_diag)
+        B, T, n = self._bt(R_diag)
+        host = bool(flags & FLAG_HOST_IO)
+        J = self._out(R_diag, (B,), host)
+        g = self._out(R_diag, (B, T, n), host) if with_grad else None
+        _chk(self.lib.leb_jerr(self._ctx, B, T, n, int(m), _ptr(Phi), _ptr(R_diag), _ptr(E_diag), _ptr(J), _ptr(g),
+                               ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_jerr")
+        return J, g
 
     def leb_domain_flag(self) -> int:
         flag = ctypes.c_int(0)

@@ -1,0 +1,200 @@
+"""GPU parity of the consumers of the bounds against their oracles (oracle/tube_oracle.py, oracle/pbh_refine.py):
+leb_dist_add (22) L226, leb_tube_propagate (27)-(28) L289-291, leb_jerr (35) L360, leb_analytic_partition_fwd (L236),
+leb_analytic_pgd (Table II)."""
+import numpy as np
+import pytest
+import torch
+
+from parity_util import assert_bounds_close, report, to_np
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    from paper_2607_01203_b200 import build, leb, workloads
+    from oracle import pbh_oracle, pbh_refine, tube_oracle
+    build.build()
+    pbh_oracle.build()
+    return leb, workloads, pbh_oracle, pbh_refine, tube_oracle
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _responses(rng, B, T, n, m):
+    """Synthetic closed-loop responses with the structure of (34c): Phi^x_{j+1,j} = I, decaying in k - j."""
+    N = n + m
+    Phi = np.zeros((B, T * (T + 1) // 2, N, n), dtype=np.float32)
+    for k in range(1, T + 1):
+        for j in range(k):
+            blk = rng.standard_normal((B, N, n)) * (0.7 ** (k - 1 - j)) / np.sqrt(n)
+            if k == j + 1:
+                blk[:, :n] = np.eye(n)
+            Phi[:, (k - 1) * k // 2 + j] = blk
+    return Phi
+
+
+@pytest.mark.parametrize("B,T,n,m", [(2, 5, 6, 2), (1, 3, 7, 3), (3, 9, 168, 56), (2, 4, 33, 0)])
+def test_tube_and_jerr_match_oracle(mods, B, T, n, m):
+    leb, _, _, _, TU = mods
+    rng = np.random.default_rng(B * 100 + T)
+    Phi = _responses(rng, B, T, n, m)
+    c = (rng.standard_normal((B, T, n)) * 0.05).astype(np.float32)
+    Rd = rng.uniform(0.001, 0.1, (B, T, n)).astype(np.float32)
+    E = rng.uniform(0.0, 0.05, n).astype(np.float32)
+    ctx = leb.Context(0)
+    for Ed in (E, None):
+        h_mu, h_sg = ctx.leb_tube_propagate(_dev(Phi), _dev(c), _dev(Rd), m, None if Ed is None else _dev(Ed))
+        J, g = ctx.leb_jerr(_dev(Phi), _dev(Rd), m, None if Ed is None else _dev(Ed))
+        E0 = np.zeros(n) if Ed is None else Ed.astype(np.float64)
+        for b in range(B):
+            omu, osg = TU.tube_propagate(Phi[b], c[b].astype(np.float64), Rd[b].astype(np.float64), E0)
+            gmu, gsg = to_np(h_mu)[b], to_np(h_sg)[b]
+            scale = np.abs(omu).max() + 1e-30
+            assert np.all(np.abs(gmu - omu) <= 1e-5 * np.abs(omu) + 2e-6 * scale)        # h_mu: a signed sum, normwise floor
+            assert_bounds_close(gsg, osg, f"h_sigma n={n}")
+            assert np.all(gsg >= osg * (1 - 1e-12))                                      # rounded up: a bound
+            oJ = TU.j_err(Phi[b], Rd[b].astype(np.float64), E0)
+            og = TU.j_err_grad(Phi[b], Rd[b].astype(np.float64), E0)
+            assert abs(float(J[b]) - oJ) <= 1e-5 * oJ
+            assert np.all(np.abs(to_np(g)[b] - og) <= 1e-5 * np.abs(og) + 1e-7 * np.abs(og).max())
+    # empty batch; grad optional; host IO
+    Jn, gnone = ctx.leb_jerr(_dev(Phi), _dev(Rd), m, _dev(E), with_grad=False)
+    assert gnone is None and torch.equal(Jn, ctx.leb_jerr(_dev(Phi), _dev(Rd), m, _dev(E))[0])
+    hm, hs = ctx.leb_tube_propagate(torch.from_numpy(Phi).pin_memory(), torch.from_numpy(c).pin_memory(), torch.from_numpy(Rd).pin_memory(),
+                                    m, torch.from_numpy(E).pin_memory(), flags=leb.FLAG_HOST_IO)
+    torch.cuda.synchronize()
+    d_hm, d_hs = ctx.leb_tube_propagate(_dev(Phi), _dev(c), _dev(Rd), m, _dev(E))
+    assert torch.equal(hm, d_hm.cpu()) and torch.equal(hs, d_hs.cpu())
+    ctx.close()
+
+
+def test_jerr_gradient_chains_into_leb_vjp(mods):
+    """(35) -> d/dR_bar -> leb_zonotope_inflate_vjp -> leb_vjp: the gradient of J_err with respect to the nominal trajectory,
+    against central differences of the whole chain evaluated by the oracles."""
+    leb, wl, P, _, TU = mods
+    from oracle import inflate_oracle as I
+    w = wl.make_config(2, B=1, T=4)
+    spec = P.spec_from_workload(w)
+    rng = np.random.default_rng(3)
+    Phi = _responses(rng, 1, w.T, w.n, w.m)
+    ctx = leb.context_for_workload(w)
+    nom, rad = _dev(w.nom), _dev(w.rad)
+    lo, hi = ctx.leb_analytic_fwd(nom, rad)
+    c, R = ctx.leb_zonotope_inflate(lo, hi, 1e-6)
+    J, gR = ctx.leb_jerr(_dev(Phi), R, w.m)
+    g_lo, g_hi = ctx.leb_zonotope_inflate_vjp(torch.zeros_like(gR), gR)
+    gn, gr = ctx.leb_vjp(0, nom, rad, g_lo, g_hi)
+
+    def F(a, s):
+        olo, ohi, _ = P.pbh(spec, a, s)
+        _, oR = I.inflate(olo, ohi, 1e-6)
+        return TU.j_err(Phi[0], oR, np.zeros(w.n))
+    a0, s0 = w.nom.reshape(-1, w.N).astype(np.float64), w.rad.reshape(-1, w.N).astype(np.float64)
+    assert abs(float(J[0]) - F(a0, s0)) <= 1e-5 * F(a0, s0)
+    h, ok = 1e-6, 0
+    G = np.concatenate([to_np(gn).reshape(-1, w.N), to_np(gr).reshape(-1, w.N)], 1)
+    for t in range(w.T):
+        for d in range(2 * w.N):
+            e = np.zeros_like(a0)
+            e[t, d % w.N] = h
+            fp, fm = (F(a0 + e, s0), F(a0 - e, s0)) if d < w.N else (F(a0, s0 + e), F(a0, s0 - e))
+            f0 = F(a0, s0)
+            if abs((fp - f0) - (f0 - fm)) > 1e-3 * abs(fp - fm) + 1e-18:
+                continue
+            assert abs((fp - fm) / (2 * h) - G[t, d]) <= 2e-4 * abs(G[t, d]) + 1e-5 * np.abs(G[t]).max(), (t, d)
+            ok += 1
+    assert ok > w.T * w.N
+    ctx.close()
+
+
+def test_dist_add_matches_oracle(mods):
+    leb, _, _, _, TU = mods
+    rng = np.random.default_rng(4)
+    B, T, n, nw = 2, 3, 7, 5
+    E_nom = rng.standard_normal((B, T, n, nw)).astype(np.float32)
+    E_lo = (E_nom - rng.uniform(0, 0.3, E_nom.shape)).astype(np.float32)
+    E_hi = (E_nom + rng.uniform(0, 0.3, E_nom.shape)).astype(np.float32)
+    r_lo = (-rng.uniform(0, 0.1, (B, T, n))).astype(np.float32)
+    r_hi = rng.uniform(0, 0.1, (B, T, n)).astype(np.float32)
+    ctx = leb.Context(0)
+    lo, hi = ctx.leb_dist_add(_dev(E_lo), _dev(E_hi), _dev(E_nom), _dev(r_lo), _dev(r_hi))
+    dlo, dhi = TU.dist_bound(E_lo, E_hi, E_nom)
+    assert_bounds_close(to_np(lo), r_lo + dlo, "r_lo + r_dist_lo")
+    assert_bounds_close(to_np(hi), r_hi + dhi, "r_hi + r_dist_hi")
+    assert np.all(to_np(lo) <= r_lo.astype(np.float64) + dlo) and np.all(to_np(hi) >= r_hi.astype(np.float64) + dhi)   # outward
+    # constant E adds nothing
+    lo, hi = ctx.leb_dist_add(_dev(E_nom), _dev(E_nom), _dev(E_nom), _dev(r_lo), _dev(r_hi))
+    assert np.array_equal(to_np(lo), r_lo.astype(np.float64)) and np.array_equal(to_np(hi), r_hi.astype(np.float64))
+    ctx.close()
+
+
+def test_partition_matches_oracle_and_is_sound(mods):
+    leb, wl, P, R, _ = mods
+    w = wl.make_config(2, B=2, T=3)
+    spec = P.spec_from_workload(w)
+    N = w.N
+    rad = (4.0 * w.rad).astype(np.float32)
+    splits = np.ones(N, dtype=int)
+    splits[[3, 4, 12]] = (2, 3, 2)
+    ctx = leb.context_for_workload(w)
+    for mu in (None, wl.make_mu(w, 1.5)):
+        lo, hi = ctx.leb_analytic_partition_fwd(_dev(w.nom), _dev(rad), splits, None if mu is None else _dev(mu))
+        assert ctx.leb_domain_flag() == 0
+        olo, ohi, st = R.partition(spec, w.nom, rad, splits, mu=mu)
+        assert st == 0
+        glo, ghi = to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n)
+        assert_bounds_close(glo, olo, "partition r_lo")
+        assert_bounds_close(ghi, ohi, "partition r_hi")
+        plo, phi = ctx.leb_analytic_fwd(_dev(w.nom), _dev(rad), mu=None if mu is None else _dev(mu))
+        assert bool((lo >= plo - 1e-7 - 1e-5 * plo.abs()).all()) and bool((hi <= phi + 1e-7 + 1e-5 * phi.abs()).all())
+    # splits all 1 = the plain bound, bit for bit
+    lo1, hi1 = ctx.leb_analytic_partition_fwd(_dev(w.nom), _dev(rad), np.ones(N, dtype=int))
+    plo, phi = ctx.leb_analytic_fwd(_dev(w.nom), _dev(rad))
+    assert torch.equal(lo1, plo) and torch.equal(hi1, phi)
+    # soundness of the FP32 sub-box grid: samples of the whole box, incl. points on the cuts
+    lo, hi = ctx.leb_analytic_partition_fwd(_dev(w.nom), _dev(rad), splits)
+    glo, ghi = to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n)
+    rng = np.random.default_rng(6)
+    for t in range(3):
+        a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = rad.reshape(-1, N)[t].astype(np.float64)
+        U = rng.uniform(-1, 1, (100000, N))
+        U[:20000, 3] = 0.0                                   # on the cut of the 2-way split
+        U[20000:40000, 4] = rng.choice([-1 / 3, 1 / 3], 20000)
+        X = a0[None] + U * sg[None]
+        J = P.jac(spec, a0)
+        r = P.f(spec, X) - P.f(spec, a0[None]) - (X - a0) @ J.T
+        assert np.all(r.max(0) <= ghi[t] + 1e-12) and np.all(r.min(0) >= glo[t] - 1e-12)
+    ctx.close()
+
+
+def test_pgd_matches_oracle(mods):
+    leb, wl, P, R, _ = mods
+    w = wl.make_config(2, B=2, T=4)
+    spec = P.spec_from_workload(w)
+    centre, rad = w.nom, w.rad
+    rng = np.random.default_rng(1)
+    nom0 = (centre + 0.4 * rad * rng.uniform(-1, 1, rad.shape)).astype(np.float32)
+    eps = (0.5 * rad).astype(np.float32)
+    ctx = leb.context_for_workload(w)
+    steps, lr = 6, 0.03
+    best, w0, wb = ctx.leb_analytic_pgd(_dev(centre), _dev(rad), _dev(eps), _dev(nom0), steps, lr)
+    obest, ow0, owb = R.pgd(spec, centre.reshape(-1, w.N), rad.reshape(-1, w.N), nom0.reshape(-1, w.N), eps.reshape(-1, w.N).astype(np.float64),
+                            steps, lr)
+    gw0, gwb = to_np(w0).reshape(-1), to_np(wb).reshape(-1)
+    assert np.allclose(gw0, ow0, rtol=1e-5)
+    # an iteration amplifies rounding differences (and may pick another best iterate of equal width): widths to 1e-3,
+    # points to 1e-3 of the neighbourhood
+    report("pgd best width (rel err / 1e-3)", np.max(np.abs(gwb - owb) / owb) / 1e-3)
+    assert np.allclose(gwb, owb, rtol=1e-3)
+    assert np.all(gwb <= gw0) and np.all(gwb < 0.95 * gw0)
+    d = np.abs(to_np(best).reshape(-1, w.N) - obest) / eps.reshape(-1, w.N)
+    assert d.max() < 2e-2, d.max()
+    assert bool(((best - _dev(centre)).abs() <= _dev(eps) * (1 + 1e-6)).all())
+    # the returned point has the returned width
+    mu = _dev(centre) - best
+    lo, hi = ctx.leb_analytic_fwd(best, _dev(rad), mu=mu)
+    assert np.allclose(to_np((hi - lo).sum(-1)).reshape(-1), gwb, rtol=1e-5)
+    ctx.close()
