@@ -313,6 +313,7 @@ def run_ours(args):
         ctx = None
         if world == 1 and not args.no_configs:
             line["configs"] = {f"config{c}": _config_record(c, 3, 2, peaks) for c in (1, 2, 3, 4)}
+            line["configs"]["tube"] = _tube_record(peaks)
         print(json.dumps(line))
     if ctx is not None:
         ctx.close()
@@ -379,6 +380,42 @@ def _config_record(cfg, steps, warmup, peaks):
             rec[name] = {"bound": "alu", "avg_launch_ms": k_ms / max(k_n, 1), "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                          "frac": ach / peak, "algorithmic_gflop_per_launch": k_flops / max(k_n, 1) / 1e9}
     rec["ms_forward_only"] = timed(fwd, steps)
+    ctx.close()
+    return rec
+
+
+def _tube_record(peaks, B=16, T=100, n=168, m=56):
+    """Tube propagation (27)-(28) and J_err (35) at config-5 shape: HBM-bound streams over the closed-loop responses
+    (B = 16 trajectories: 12 GB of Phi, far beyond L2).  Synthetic responses drawn on the device, Phi^x_{j+1,j} = I."""
+    import torch
+    from paper_2607_01203_b200 import leb
+    dev = torch.device("cuda", 0)
+    g = torch.Generator(device=dev)
+    g.manual_seed(20260706)
+    nb = T * (T + 1) // 2
+    Phi = torch.empty((B, nb, n + m, n), dtype=torch.float32, device=dev)
+    for b in range(B):
+        Phi[b].normal_(0.0, 1.0 / n ** 0.5, generator=g)
+    for j in range(T):
+        Phi[:, (j + 1) * j // 2 + j, :n] = torch.eye(n, device=dev)
+    c = torch.randn((B, T, n), device=dev, generator=g) * 0.05
+    R = torch.rand((B, T, n), device=dev, generator=g) * 0.1 + 1e-3
+    E = torch.rand((n,), device=dev, generator=g) * 0.05
+    ctx = leb.Context(0)
+    rec = {"workload": f"tube propagation + J_err: B={B} x T={T}, n={n}, m={m}, Phi {Phi.numel() * 4 / 1e9:.1f} GB (synthetic)"}
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    for name, f in (("tube_kernel", lambda: ctx.leb_tube_propagate(Phi, c, R, m, E)), ("jerr_kernel", lambda: ctx.leb_jerr(Phi, R, m, E))):
+        for _ in range(2):
+            f()
+        ctx.leb_profile_reset()
+        ctx.leb_profile(True)
+        for _ in range(3):
+            f()
+        ctx.leb_profile(False)
+        k_ms, k_bytes, k_n = ctx.leb_profile_read(6)
+        ach = (k_bytes / 1e9) / (k_ms * 1e-3) if k_ms > 0 else 0.0
+        rec[name] = {"bound": "hbm", "avg_launch_ms": k_ms / max(k_n, 1), "achieved": ach, "peak": hbm, "unit": "GB/s",
+                     "frac": ach / hbm, "algorithmic_gb_per_launch": k_bytes / max(k_n, 1) / 1e9}
     ctx.close()
     return rec
 

@@ -39,115 +39,149 @@ __global__ void dist_add_kernel(size_t rows, int nw, const float* __restrict__ E
 }
 
 // ---------------------------------------------------------------- (27)-(28)
-// CTA = (trajectory b, time k, block of kRows output rows), 8 warps, each warp owns kRows / 8 rows and walks j = 0..k-1.
-// The per-j vectors c_bar_j and s_j = |E| + R_bar_j are staged in shared memory (every row of the block reads them).
-constexpr int kTubeWarps = 8, kRowsPerWarp = 4, kRows = kTubeWarps * kRowsPerWarp;
+// One warp per output row (b, k, i): it streams the k row segments Phi_{k,j}[i, :] (n floats each) as ONE flat sequence
+// of k * n / 4 16-byte items dealt round robin to the lanes -- every lane busy whatever n is -- kTubeUnroll items in
+// flight per lane (the kernel is a pure HBM stream: what matters is bytes in flight), against the per-j vectors c_bar_j
+// and s_j = |E| + R_bar_j, which every row of the same (b, k) re-reads from L1 / L2.
+constexpr int kTubeWarps = 8, kTubeUnroll = 4;
 
-__global__ void __launch_bounds__(kTubeWarps * 32)
+template <bool VEC>
+__global__ void __launch_bounds__(kTubeWarps * 32, 4)
 tube_kernel(int T, int n, int N, const float* __restrict__ Phi, const float* __restrict__ c_bar,
             const float* __restrict__ R_diag, const float* __restrict__ E_diag, float* __restrict__ h_mu,
             float* __restrict__ h_sigma) {
-    extern __shared__ float sm[];                 // [2][2][n]: double-buffered (c_bar_j, s_j)
     const int b = blockIdx.z;
-    const int k = T - (int)blockIdx.y;            // heavy (large k) CTAs first
-    const int row0 = blockIdx.x * kRows;
+    const int k = T - (int)blockIdx.y;            // heavy (large k) rows first
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = blockIdx.x * kTubeWarps + warp;
+    if (i >= N) return;
     const size_t blocks_per_traj = (size_t)T * (T + 1) / 2;
-    const float* P = Phi + ((size_t)b * blocks_per_traj + (size_t)(k - 1) * k / 2) * (size_t)N * n;
+    const float* P = Phi + (((size_t)b * blocks_per_traj + (size_t)(k - 1) * k / 2) * N + i) * (size_t)n;   // row i of Phi_{k,0}
+    const size_t jstride = (size_t)N * n;
     const float* cb = c_bar + (size_t)b * T * n;
     const float* Rb = R_diag + (size_t)b * T * n;
-    float mu[kRowsPerWarp], sg[kRowsPerWarp];
+    float mu = 0.f, sg = 0.f;
+    if (VEC) {
+        const int n4 = n >> 2;
+        // this lane's item: (j, c4); advancing by 32 items wraps c4 over the rows
+        int j = lane / n4, c4 = lane - j * n4;
+        const int dj = 32 / n4, dc = 32 - dj * n4;
+        while (j < k) {
+            float4 p[kTubeUnroll];
+            int jj[kTubeUnroll], cc[kTubeUnroll];
 #pragma unroll
-    for (int r = 0; r < kRowsPerWarp; ++r) { mu[r] = 0.f; sg[r] = 0.f; }
-    auto stage = [&](int j, int buf) {
-        float* dst = sm + (size_t)buf * 2 * n;
-        for (int c = threadIdx.x; c < n; c += blockDim.x) {
-            dst[c] = cb[(size_t)j * n + c];
-            dst[n + c] = __fadd_ru(E_diag ? fabsf(E_diag[c]) : 0.f, Rb[(size_t)j * n + c]);
-        }
-    };
-    stage(0, 0);
-    __syncthreads();
-    const bool vec = (n & 3) == 0;
-    for (int j = 0; j < k; ++j) {
-        if (j + 1 < k) stage(j + 1, (j + 1) & 1);
-        const float* cj = sm + (size_t)(j & 1) * 2 * n;
-        const float* sj = cj + n;
-        const float* Pj = P + (size_t)j * N * n;
+            for (int u = 0; u < kTubeUnroll; ++u) {
+                jj[u] = j; cc[u] = c4;
+                if (j < k) p[u] = __ldcs(reinterpret_cast<const float4*>(P + (size_t)j * jstride) + c4);
+                j += dj; c4 += dc;
+                if (c4 >= n4) { c4 -= n4; ++j; }
+            }
 #pragma unroll
-        for (int r = 0; r < kRowsPerWarp; ++r) {
-            const int i = row0 + warp * kRowsPerWarp + r;
-            if (i >= N) break;
-            const float* row = Pj + (size_t)i * n;
-            if (vec) {
-                const float4* row4 = reinterpret_cast<const float4*>(row);
-                for (int c4 = lane; c4 < n / 4; c4 += 32) {
-                    const float4 p = __ldcs(row4 + c4);               // streamed once
-                    const float4 cv = *reinterpret_cast<const float4*>(cj + 4 * c4), sv = *reinterpret_cast<const float4*>(sj + 4 * c4);
-                    mu[r] = fmaf(p.x, cv.x, fmaf(p.y, cv.y, fmaf(p.z, cv.z, fmaf(p.w, cv.w, mu[r]))));
-                    sg[r] = __fmaf_ru(fabsf(p.x), sv.x, __fmaf_ru(fabsf(p.y), sv.y, __fmaf_ru(fabsf(p.z), sv.z, __fmaf_ru(fabsf(p.w), sv.w, sg[r]))));
-                }
-            } else {
-                for (int c = lane; c < n; c += 32) {
-                    const float p = __ldcs(row + c);
-                    mu[r] = fmaf(p, cj[c], mu[r]);
-                    sg[r] = __fmaf_ru(fabsf(p), sj[c], sg[r]);
-                }
+            for (int u = 0; u < kTubeUnroll; ++u) {
+                if (jj[u] >= k) break;
+                const float4 cv = __ldg(reinterpret_cast<const float4*>(cb + (size_t)jj[u] * n) + cc[u]);
+                const float4 rv = __ldg(reinterpret_cast<const float4*>(Rb + (size_t)jj[u] * n) + cc[u]);
+                const float4 e = E_diag ? __ldg(reinterpret_cast<const float4*>(E_diag) + cc[u]) : make_float4(0.f, 0.f, 0.f, 0.f);
+                mu = fmaf(p[u].x, cv.x, fmaf(p[u].y, cv.y, fmaf(p[u].z, cv.z, fmaf(p[u].w, cv.w, mu))));
+                sg = __fmaf_ru(fabsf(p[u].x), __fadd_ru(fabsf(e.x), rv.x), sg);
+                sg = __fmaf_ru(fabsf(p[u].y), __fadd_ru(fabsf(e.y), rv.y), sg);
+                sg = __fmaf_ru(fabsf(p[u].z), __fadd_ru(fabsf(e.z), rv.z), sg);
+                sg = __fmaf_ru(fabsf(p[u].w), __fadd_ru(fabsf(e.w), rv.w), sg);
             }
         }
-        __syncthreads();
+    } else {
+        for (int c = lane; c < n; c += 32) {
+            const float e = E_diag ? fabsf(E_diag[c]) : 0.f;
+            for (int j = 0; j < k; ++j) {
+                const float p = __ldcs(P + (size_t)j * jstride + c);
+                mu = fmaf(p, cb[(size_t)j * n + c], mu);
+                sg = __fmaf_ru(fabsf(p), __fadd_ru(e, Rb[(size_t)j * n + c]), sg);
+            }
+        }
     }
 #pragma unroll
-    for (int r = 0; r < kRowsPerWarp; ++r) {
-        float a = mu[r], s = sg[r];
-#pragma unroll
-        for (int off = 16; off; off >>= 1) { a += __shfl_xor_sync(FULL, a, off); s = __fadd_ru(s, __shfl_xor_sync(FULL, s, off)); }
-        const int i = row0 + warp * kRowsPerWarp + r;
-        if (lane == 0 && i < N) {
-            const size_t o = ((size_t)b * T + (k - 1)) * N + i;
-            h_mu[o] = a;
-            h_sigma[o] = s;
-        }
+    for (int off = 16; off; off >>= 1) { mu += __shfl_xor_sync(FULL, mu, off); sg = __fadd_ru(sg, __shfl_xor_sync(FULL, sg, off)); }
+    if (lane == 0) {
+        const size_t o = ((size_t)b * T + (k - 1)) * N + i;
+        h_mu[o] = mu;
+        h_sigma[o] = sg;
     }
 }
 
 // ---------------------------------------------------------------- (35)
-// CTA = (trajectory b, disturbance index j): column energies S_c = sum_{k>j} sum_i Phi_{k,j}[i,c]^2, thread = column group,
-// warps split the rows; then partial J_err of (b, j) and d J_err / d R_bar_{j,c} = 2 R_bar_{j,c} S_c.
-constexpr int kJerrWarps = 8;
+// CTA = (trajectory b, disturbance index j): column energies S_c = sum_{k>j} sum_i Phi_{k,j}[i,c]^2.  A lane owns the
+// column quads c4 = lane, lane + 32, ... (register accumulators), the warps deal the rows of all blocks (k, j),
+// k = j+1..T, among themselves, kJerrUnroll rows in flight; then partial J_err of (b, j) and
+// d J_err / d R_bar_{j,c} = 2 R_bar_{j,c} S_c.
+constexpr int kJerrWarps = 8, kJerrQuads = 8, kJerrUnroll = 8;      // n <= 128 * kJerrQuads
 
-__global__ void __launch_bounds__(kJerrWarps * 32)
+template <bool VEC>
+__global__ void __launch_bounds__(kJerrWarps * 32, 3)
 jerr_kernel(int T, int n, int N, const float* __restrict__ Phi, const float* __restrict__ R_diag,
             const float* __restrict__ E_diag, float* __restrict__ partial /* [B, T] */, float* __restrict__ grad_R) {
-    extern __shared__ float sm[];                 // [kJerrWarps][n] column partials
+    extern __shared__ float sm[];                 // [kJerrWarps][4 * ceil(n / 4)] column partials
     const int b = blockIdx.y, j = blockIdx.x;     // j ascending = heavy first
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const size_t blocks_per_traj = (size_t)T * (T + 1) / 2;
     const float* base = Phi + (size_t)b * blocks_per_traj * (size_t)N * n;
-    float* mine = sm + (size_t)warp * n;
-    for (int c = lane; c < n; c += 32) mine[c] = 0.f;
-    __syncwarp();
-    // work items = rows of all blocks (k, j), k = j+1..T, dealt to the warps round robin
+    const int n4 = (n + 3) >> 2, nq = (n4 + 31) >> 5, np = 4 * n4;
+    float4 acc[kJerrQuads];
+#pragma unroll
+    for (int q = 0; q < kJerrQuads; ++q) acc[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     const int nrows = (T - j) * N;
-    for (int q = warp; q < nrows; q += kJerrWarps) {
-        const int k = j + 1 + q / N, i = q - (k - j - 1) * N;
-        const float* row = base + (((size_t)(k - 1) * k / 2 + j) * N + i) * (size_t)n;
-        for (int c = lane; c < n; c += 32) { const float p = __ldcs(row + c); mine[c] = fmaf(p, p, mine[c]); }
+    for (int q0 = warp * kJerrUnroll; q0 < nrows; q0 += kJerrWarps * kJerrUnroll) {
+        const float* row[kJerrUnroll];
+#pragma unroll
+        for (int u = 0; u < kJerrUnroll; ++u) {
+            const int q = min(q0 + u, nrows - 1);
+            const int k = j + 1 + q / N, i = q - (k - j - 1) * N;
+            row[u] = base + (((size_t)(k - 1) * k / 2 + j) * N + i) * (size_t)n;
+        }
+#pragma unroll
+        for (int cc = 0; cc < kJerrQuads; ++cc) {
+            if (cc >= nq) break;
+            const int c4 = lane + 32 * cc;
+            float4 p[kJerrUnroll];
+#pragma unroll
+            for (int u = 0; u < kJerrUnroll; ++u) {
+                p[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (c4 < n4 && q0 + u < nrows) {
+                    if (VEC) p[u] = __ldcs(reinterpret_cast<const float4*>(row[u]) + c4);
+                    else {
+                        const int c = 4 * c4;
+                        p[u].x = __ldcs(row[u] + c);
+                        if (c + 1 < n) p[u].y = __ldcs(row[u] + c + 1);
+                        if (c + 2 < n) p[u].z = __ldcs(row[u] + c + 2);
+                        if (c + 3 < n) p[u].w = __ldcs(row[u] + c + 3);
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < kJerrUnroll; ++u) {
+                acc[cc].x = fmaf(p[u].x, p[u].x, acc[cc].x); acc[cc].y = fmaf(p[u].y, p[u].y, acc[cc].y);
+                acc[cc].z = fmaf(p[u].z, p[u].z, acc[cc].z); acc[cc].w = fmaf(p[u].w, p[u].w, acc[cc].w);
+            }
+        }
+    }
+#pragma unroll
+    for (int cc = 0; cc < kJerrQuads; ++cc) {
+        const int c4 = lane + 32 * cc;
+        if (cc < nq && c4 < n4) reinterpret_cast<float4*>(sm + (size_t)warp * np)[c4] = acc[cc];
     }
     __syncthreads();
-    float acc = 0.f;
+    float tot = 0.f;
     for (int c = threadIdx.x; c < n; c += blockDim.x) {
         float S = 0.f;
 #pragma unroll
-        for (int w = 0; w < kJerrWarps; ++w) S += sm[(size_t)w * n + c];
+        for (int w = 0; w < kJerrWarps; ++w) S += sm[(size_t)w * np + c];
         const float R = R_diag[((size_t)b * T + j) * n + c], E = E_diag ? E_diag[c] : 0.f;
-        acc = fmaf(fmaf(E, E, R * R), S, acc);
+        tot = fmaf(fmaf(E, E, R * R), S, tot);
         if (grad_R) grad_R[((size_t)b * T + j) * n + c] = 2.f * R * S;
     }
     __syncthreads();
 #pragma unroll
-    for (int off = 16; off; off >>= 1) acc += __shfl_xor_sync(FULL, acc, off);
-    if (lane == 0) sm[warp] = acc;
+    for (int off = 16; off; off >>= 1) tot += __shfl_xor_sync(FULL, tot, off);
+    if (lane == 0) sm[warp] = tot;
     __syncthreads();
     if (threadIdx.x == 0) {
         float t = 0.f;
@@ -183,10 +217,11 @@ cudaError_t leb_launch_tube(int B, int T, int n, int N, const float* Phi, const 
                             const float* E_diag, float* h_mu, float* h_sigma, cudaStream_t st, long long* launches,
                             LebProf* prof) {
     if (B == 0 || T == 0) return cudaSuccess;
-    const dim3 grid((N + kRows - 1) / kRows, T, B);
-    const size_t smem = 4 * (size_t)n * sizeof(float);
+    const dim3 grid((N + kTubeWarps - 1) / kTubeWarps, T, B);
+    const bool vec = (n & 3) == 0 && (((size_t)Phi | (size_t)c_bar | (size_t)R_diag | (size_t)E_diag) & 15) == 0;
     prof->begin(LEB_KC_TUBE, st);
-    tube_kernel<<<grid, kTubeWarps * 32, smem, st>>>(T, n, N, Phi, c_bar, R_diag, E_diag, h_mu, h_sigma);
+    if (vec) tube_kernel<true><<<grid, kTubeWarps * 32, 0, st>>>(T, n, N, Phi, c_bar, R_diag, E_diag, h_mu, h_sigma);
+    else tube_kernel<false><<<grid, kTubeWarps * 32, 0, st>>>(T, n, N, Phi, c_bar, R_diag, E_diag, h_mu, h_sigma);
     // algorithmic bytes: Phi once, (c_bar, R_bar) once, two outputs
     prof->end(LEB_KC_TUBE, st, 4.0 * ((double)B * T * (T + 1) / 2 * N * n + 2.0 * B * T * n + 2.0 * B * T * N));
     ++*launches;
@@ -196,9 +231,11 @@ cudaError_t leb_launch_tube(int B, int T, int n, int N, const float* Phi, const 
 cudaError_t leb_launch_jerr(int B, int T, int n, int N, const float* Phi, const float* R_diag, const float* E_diag,
                             float* partial, float* J, float* grad_R, cudaStream_t st, long long* launches, LebProf* prof) {
     if (B == 0 || T == 0) return cudaSuccess;
-    const size_t smem = std::max<size_t>((size_t)kJerrWarps * n, 32) * sizeof(float);
+    const size_t smem = std::max<size_t>((size_t)kJerrWarps * 4 * ((n + 3) / 4), 32) * sizeof(float);
+    const bool vec = (n & 3) == 0 && ((size_t)Phi & 15) == 0;
     prof->begin(LEB_KC_TUBE, st);
-    jerr_kernel<<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
+    if (vec) jerr_kernel<true><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
+    else jerr_kernel<false><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
     prof->end(LEB_KC_TUBE, st, 4.0 * ((double)B * T * (T + 1) / 2 * N * n + 2.0 * B * T * n));
     jerr_finish_kernel<<<(B + 7) / 8, 256, 0, st>>>(B, T, partial, J);
     *launches += 2;
