@@ -58,7 +58,7 @@ typedef enum {
 } leb_status;
 
 typedef enum { LEB_MODEL_UNICYCLE = 1, LEB_MODEL_QUAD12 = 2, LEB_MODEL_QUADCHAIN = 3, LEB_MODEL_PLANAR_QUAD = 4,
-               LEB_MODEL_SATELLITE = 5 } leb_model_id;
+               LEB_MODEL_SATELLITE = 5, LEB_MODEL_QUADCENTROID = 6 } leb_model_id;
 typedef enum { LEB_INTEG_EULER = 1, LEB_INTEG_RK4 = 2 } leb_integ;
 typedef enum { LEB_ACT_RELU = 1, LEB_ACT_TANH = 2 } leb_act;
 
@@ -71,6 +71,8 @@ typedef enum { LEB_ACT_RELU = 1, LEB_ACT_TANH = 2 } leb_act;
  *   PLANAR_QUAD: x = (px, py, phi, vx, vy, phidot), u = (u1, u2), eq. (37a);
  *              mass = m, g, Jx = moment of inertia J, k1 = arm length L.
  *   SATELLITE: x = (q[4], om[3]), u = torque[3], eq. (36); (Jx, Jy, Jz) = diag of I_S.
+ *   QUADCENTROID: n_units copies of QUAD12 with the paper's centroid spring-damper coupling (40)-(42) L545-558;
+ *              k1 = alpha (stiffness), k3 = gamma (damping).
  * integ = EULER: f = x + dt g(x,u) (the paper's choice, L505); RK4: classical 4 stages, u held. */
 typedef struct {
     int model_id; /* leb_model_id */

@@ -192,6 +192,7 @@ inline double cube_(double a) { return a * a * a; }
 // ----------------------------------------------------------------- models
 struct Params { double dt, mass, g, Jx, Jy, Jz, k1, k3; };
 enum { MODEL_UNICYCLE = 1, MODEL_QUAD12 = 2, MODEL_QUADCHAIN = 3, MODEL_PLANAR_QUAD = 4, MODEL_SATELLITE = 5,
+       MODEL_QUADCENTROID = 6,
        MODEL_QUADRATIC = 100, MODEL_LINEAR = 101 };
 enum { INTEG_EULER = 1, INTEG_RK4 = 2 };
 
@@ -246,6 +247,27 @@ void chain_field(const Params& P, int U, const X* x, const X* u, X* out) {
     }
 }
 
+// coupled 3-D quadrotors of the paper, eq. (39)-(42) PAPER.md:L540-558: U quad12 units, centroid spring-damper
+//   a_i = -alpha U (p_i - pbar) - gamma (v_i - vbar),  pbar = (1/U) sum p_i,  vbar = (1/U) sum v_i        (40)-(41)
+// added to the translational acceleration of unit i (42).  Params: k1 = alpha, k3 = gamma.
+template <class X>
+void centroid_field(const Params& P, int U, const X* x, const X* u, X* out) {
+    X pbar[3] = {x[0], x[0], x[0]}, vbar[3] = {x[0], x[0], x[0]};
+    for (int c = 0; c < 3; ++c) {
+        X sp = x[c], sv = x[6 + c];
+        for (int i = 1; i < U; ++i) { sp = sp + x[12 * i + c]; sv = sv + x[12 * i + 6 + c]; }
+        pbar[c] = scale(1.0 / U, sp);
+        vbar[c] = scale(1.0 / U, sv);
+    }
+    for (int i = 0; i < U; ++i) {
+        quad12_field(P, x + 12 * i, u + 4 * i, (const X*)nullptr, out + 12 * i);
+        for (int c = 0; c < 3; ++c) {
+            X a = scale(-P.k1 * U, x[12 * i + c] - pbar[c]) + scale(-P.k3, x[12 * i + 6 + c] - vbar[c]);
+            out[12 * i + 6 + c] = out[12 * i + 6 + c] + a;
+        }
+    }
+}
+
 // planar quadrotor, eq. (37a): x = (px, py, phi, vx, vy, phidot), u = (u1, u2);
 // xdot = (vx, vy, phidot, -(u1+u2) sin(phi)/m, (u1+u2) cos(phi)/m - g, (L/J)(u2 - u1))   ("L/T" at L524 is a garble of L/J).
 // Params: mass = m, g, Jx = J, k1 = L.
@@ -290,6 +312,7 @@ void vector_field(const Model& M, const X* x, const X* u, X* out) {
     if (M.id == MODEL_QUAD12) quad12_field<X>(M.P, x, u, nullptr, out);
     else if (M.id == MODEL_PLANAR_QUAD) planar_quad_field<X>(M.P, x, u, out);
     else if (M.id == MODEL_SATELLITE) satellite_field<X>(M.P, x, u, out);
+    else if (M.id == MODEL_QUADCENTROID) centroid_field<X>(M.P, M.n_units, x, u, out);
     else chain_field<X>(M.P, M.n_units, x, u, out);
 }
 
@@ -421,7 +444,7 @@ Model make_model(int id, int integ, int n_units, const double* params, const dou
     M.Q = Q; M.C = C;
     if (id == MODEL_UNICYCLE) { M.n = 3; M.N = 5; }
     else if (id == MODEL_QUAD12) { M.n = 12; M.N = 16; }
-    else if (id == MODEL_QUADCHAIN) { M.n = 12 * n_units; M.N = 16 * n_units; }
+    else if (id == MODEL_QUADCHAIN || id == MODEL_QUADCENTROID) { M.n = 12 * n_units; M.N = 16 * n_units; }
     else if (id == MODEL_PLANAR_QUAD) { M.n = 6; M.N = 8; }
     else if (id == MODEL_SATELLITE) { M.n = 7; M.N = 10; }
     else { M.n = n; M.N = N; }

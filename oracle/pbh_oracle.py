@@ -15,7 +15,7 @@ _SRC = os.path.join(_HERE, "pbh_oracle.cpp")
 _LIB = os.path.join(_HERE, "libpbh_oracle.so")
 
 MODE_PATH, MODE_EXPAND, MODE_CLASSIC = 0, 1, 2
-MODEL_UNICYCLE, MODEL_QUAD12, MODEL_QUADCHAIN, MODEL_PLANAR_QUAD, MODEL_SATELLITE = 1, 2, 3, 4, 5
+MODEL_UNICYCLE, MODEL_QUAD12, MODEL_QUADCHAIN, MODEL_PLANAR_QUAD, MODEL_SATELLITE, MODEL_QUADCENTROID = 1, 2, 3, 4, 5, 6
 MODEL_QUADRATIC, MODEL_LINEAR = 100, 101
 INTEG_EULER, INTEG_RK4 = 1, 2
 
@@ -56,7 +56,7 @@ class ModelSpec:
             self.n, self.N = 3, 5
         elif model_id == MODEL_QUAD12:
             self.n, self.N = 12, 16
-        elif model_id == MODEL_QUADCHAIN:
+        elif model_id in (MODEL_QUADCHAIN, MODEL_QUADCENTROID):
             self.n, self.N = 12 * n_units, 16 * n_units
         elif model_id == MODEL_PLANAR_QUAD:
             self.n, self.N = 6, 8

@@ -294,6 +294,26 @@ void chain_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) 
     }
 }
 
+// coupled 3-D quadrotors (39)-(42) PAPER.md:L540-558: centroid spring-damper a_i = -alpha U (p_i - pbar) - gamma (v_i - vbar)
+// added to the acceleration of unit i; k1 = alpha, k3 = gamma
+void centroid_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
+    const int U = M.n_units;
+    SJet pbar[3], vbar[3];
+    for (int c = 0; c < 3; ++c) {
+        SJet sp = x[c], sv = x[6 + c];
+        for (int i = 1; i < U; ++i) { sp = B.jadd(sp, x[12 * i + c]); sv = B.jadd(sv, x[12 * i + 6 + c]); }
+        pbar[c] = B.jscale(1.f / (float)U, sp);
+        vbar[c] = B.jscale(1.f / (float)U, sv);
+    }
+    for (int i = 0; i < U; ++i) {
+        quad12_field(B, M, &x[12 * i], &u[4 * i], nullptr, &out[12 * i]);
+        for (int c = 0; c < 3; ++c) {
+            SJet a = B.jadd(B.jscale(-M.k1 * (float)U, B.jsub(x[12 * i + c], pbar[c])), B.jscale(-M.k3, B.jsub(x[12 * i + 6 + c], vbar[c])));
+            out[12 * i + 6 + c] = B.jadd(out[12 * i + 6 + c], a);
+        }
+    }
+}
+
 // planar quadrotor (37a) PAPER.md:L521-528: x = (px, py, phi, vx, vy, phidot), u = (u1, u2)
 void planar_quad_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
     SJet s, c;
@@ -325,6 +345,7 @@ void satellite_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& o
 void vector_field(Builder& B, const Model& M, const JV& x, const JV& u, JV& out) {
     if (M.id == LEB_MODEL_PLANAR_QUAD) planar_quad_field(B, M, x, u, out);
     else if (M.id == LEB_MODEL_SATELLITE) satellite_field(B, M, x, u, out);
+    else if (M.id == LEB_MODEL_QUADCENTROID) centroid_field(B, M, x, u, out);
     else chain_field(B, M, x, u, out);
 }
 

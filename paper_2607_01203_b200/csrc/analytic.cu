@@ -843,7 +843,7 @@ Model leb_make_model(const leb_analytic_model& m) {
     Model M{};
     M.id = m.model_id;
     M.integ = (m.model_id == LEB_MODEL_UNICYCLE) ? LEB_INTEG_EULER : m.integ;
-    M.n_units = (m.model_id == LEB_MODEL_QUADCHAIN) ? m.n_units : 1;
+    M.n_units = (m.model_id == LEB_MODEL_QUADCHAIN || m.model_id == LEB_MODEL_QUADCENTROID) ? m.n_units : 1;
     switch (m.model_id) {
         case LEB_MODEL_UNICYCLE: M.n = 3; M.N = 5; break;
         case LEB_MODEL_PLANAR_QUAD: M.n = 6; M.N = 8; break;

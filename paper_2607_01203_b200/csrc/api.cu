@@ -115,9 +115,9 @@ leb_status leb_destroy(leb_ctx* c) {
 
 leb_status leb_set_analytic(leb_ctx* c, const leb_analytic_model* m) {
     if (!c || !m) return LEB_ERR_ARG;
-    if (m->model_id < LEB_MODEL_UNICYCLE || m->model_id > LEB_MODEL_SATELLITE) return LEB_ERR_UNSUPPORTED;
+    if (m->model_id < LEB_MODEL_UNICYCLE || m->model_id > LEB_MODEL_QUADCENTROID) return LEB_ERR_UNSUPPORTED;
     if (m->model_id != LEB_MODEL_UNICYCLE && m->integ != LEB_INTEG_EULER && m->integ != LEB_INTEG_RK4) return LEB_ERR_ARG;
-    if (m->model_id == LEB_MODEL_QUADCHAIN && (m->n_units < 1 || m->n_units > 4096)) return LEB_ERR_SHAPE;
+    if ((m->model_id == LEB_MODEL_QUADCHAIN || m->model_id == LEB_MODEL_QUADCENTROID) && (m->n_units < 1 || m->n_units > 4096)) return LEB_ERR_SHAPE;
     if (!(m->dt > 0.f)) return LEB_ERR_ARG;
     if (m->model_id != LEB_MODEL_UNICYCLE && !(m->Jx > 0.f)) return LEB_ERR_ARG;
     if (m->model_id != LEB_MODEL_UNICYCLE && m->model_id != LEB_MODEL_SATELLITE && !(m->mass > 0.f)) return LEB_ERR_ARG;

@@ -129,7 +129,7 @@ class Context:
         if model_id in (1, 4, 5):
             self.n, self.N = {1: (3, 5), 4: (6, 8), 5: (7, 10)}[model_id]
         else:
-            u = n_units if model_id == 3 else 1
+            u = n_units if model_id in (3, 6) else 1
             self.n, self.N = 12 * u, 16 * u
 
     def leb_set_mlp(self, dims: Sequence[int], W: Sequence[torch.Tensor], b: Sequence[torch.Tensor], act: int,

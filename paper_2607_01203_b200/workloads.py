@@ -30,6 +30,7 @@ MODEL_QUAD12 = 2
 MODEL_QUADCHAIN = 3
 MODEL_PLANAR_QUAD = 4
 MODEL_SATELLITE = 5
+MODEL_QUADCENTROID = 6
 INTEG_EULER = 1
 INTEG_RK4 = 2
 ACT_RELU = 1
@@ -61,12 +62,12 @@ class AnalyticModel:
     @property
     def n(self) -> int:
         return {MODEL_UNICYCLE: 3, MODEL_QUAD12: 12, MODEL_QUADCHAIN: 12 * self.n_units, MODEL_PLANAR_QUAD: 6,
-                MODEL_SATELLITE: 7}[self.model_id]
+                MODEL_SATELLITE: 7, MODEL_QUADCENTROID: 12 * self.n_units}[self.model_id]
 
     @property
     def m(self) -> int:
         return {MODEL_UNICYCLE: 2, MODEL_QUAD12: 4, MODEL_QUADCHAIN: 4 * self.n_units, MODEL_PLANAR_QUAD: 2,
-                MODEL_SATELLITE: 3}[self.model_id]
+                MODEL_SATELLITE: 3, MODEL_QUADCENTROID: 4 * self.n_units}[self.model_id]
 
     def params(self) -> np.ndarray:
         """Flat fp64 parameter vector [dt, mass, g, Jx, Jy, Jz, k1, k3]."""
@@ -228,6 +229,11 @@ def make_paper_system(name: str, B: int, T: int, seed: int = 3) -> Workload:
         nom = np.concatenate([rng.uniform(-1, 1, (B, T, 2)), rng.uniform(-0.5, 0.5, (B, T, 1)), rng.uniform(-1, 1, (B, T, 3)),
                               hover * rng.uniform(0.8, 1.2, (B, T, 2))], -1)
         am = AnalyticModel(MODEL_PLANAR_QUAD, INTEG_EULER, 0.05, mass=2.0576, g=9.81, Jx=0.01, Jy=1.0, Jz=1.0, k1=0.25, k3=0.0)
+    elif name.startswith("quadcentroid"):          # "quadcentroid8": 8 coupled quadrotors (39)-(42) L540-558, alpha 0.75, gamma 0.25
+        U = int(name[len("quadcentroid"):])
+        xi, nu = _quad_unit_nominal(rng, (B, T, U))
+        nom = np.concatenate([xi.reshape(B, T, 12 * U), nu.reshape(B, T, 4 * U)], -1)
+        am = AnalyticModel(MODEL_QUADCENTROID, INTEG_EULER, 0.05, n_units=U, k1=0.75, k3=0.25)
     elif name == "quad12_euler":
         xi, nu = _quad_unit_nominal(rng, (B, T))
         nom = np.concatenate([xi, nu], -1)

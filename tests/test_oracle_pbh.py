@@ -544,3 +544,28 @@ def test_planar_quadrotor_closed_form():
     U = np.concatenate([rng.uniform(-1, 1, (100000, 8)), np.array(list(itertools.product((-1.0, 1.0), repeat=8)))])
     r = _true_r(spec, nom[0], nom[0][None] + U * rad[0][None])
     assert np.all(r.max(0) <= hi[0] + 1e-12) and np.all(r.min(0) >= lo[0] - 1e-12)
+
+
+def test_centroid_coupled_quadrotors():
+    """Coupled quadrotors (39)-(42) L540-558, forward Euler: the centroid spring-damper is linear, so it moves the Jacobian
+    but not the Hessian -- the enclosure of every unit equals that of the uncoupled quad12 on the same inputs -- and the
+    bound stays sound for the coupled map."""
+    U = 3
+    w = wl.make_paper_system(f"quadcentroid{U}", 1, 2)
+    spec = P.spec_from_workload(w)
+    nom, rad = w.nom.reshape(-1, w.N).astype(float), w.rad.reshape(-1, w.N).astype(float)
+    lo, hi, st = P.pbh(spec, nom, rad)
+    assert st == 0
+    q = P.ModelSpec(P.MODEL_QUAD12, P.INTEG_EULER, 1, spec.params)
+    for i in range(U):
+        sel = np.r_[12 * i:12 * i + 12, 12 * U + 4 * i:12 * U + 4 * i + 4]
+        qlo, qhi, _ = P.pbh(q, nom[:, sel], rad[:, sel])
+        assert np.allclose(lo[:, 12 * i:12 * i + 12], qlo, rtol=1e-13, atol=1e-18)
+        assert np.allclose(hi[:, 12 * i:12 * i + 12], qhi, rtol=1e-13, atol=1e-18)
+    # the coupling is there: unit 0's velocity row of J sees unit 1's position with -alpha U (-1/U) dt = alpha dt
+    J = P.jac(spec, nom[0])
+    assert np.isclose(J[6, 12], 0.75 * 0.05) and np.isclose(J[6, 0], -0.75 * U * (1 - 1 / U) * 0.05)
+    rng = np.random.default_rng(9)
+    X = nom[0][None] + rng.uniform(-1, 1, (50000, w.N)) * rad[0][None]
+    r = _true_r(spec, nom[0], X)
+    assert np.all(r.max(0) <= hi[0] + 1e-12) and np.all(r.min(0) >= lo[0] - 1e-12)
