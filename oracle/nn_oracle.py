@@ -51,6 +51,11 @@ def dphi(act, z):
     return 1.0 - t * t
 
 
+def dphi_at(act, z):
+    """phi' at a bound endpoint (interval propagation differentiates phi(l), phi(u)); ReLU: 1[z > 0] as in dphi."""
+    return dphi(act, z)
+
+
 def d2phi(act, z):
     if act == ACT_RELU:
         return np.zeros_like(z)
@@ -236,9 +241,22 @@ def backsub(Ws, bs, relaxs, s, keep=False):
     return Lu, cu, Ll, cl
 
 
-def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False):
-    """Full CROWN + Thm 3 for one tile.  Returns dict with r_lo, r_hi, the hidden
-    bounds (ls, us), the output affine bounds (W_up, b_up, W_lo, b_lo), J and p."""
+def ibp_layer(W, b, act, l_prev, u_prev):
+    """Interval propagation of one layer: z = W phi(z_prev) + b with z_prev in [l_prev, u_prev]; phi is monotone, so
+    phi(z_prev) in [phi(l_prev), phi(u_prev)] and the interval matrix-vector product is W+ lo + W- hi (lower end)."""
+    a_lo, a_hi = phi(act, l_prev), phi(act, u_prev)
+    Wp, Wn = np.maximum(W, 0.0), np.minimum(W, 0.0)
+    return Wp @ a_lo + Wn @ a_hi + b, Wp @ a_hi + Wn @ a_lo + b
+
+
+def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"):
+    """CROWN + Thm 3 for one tile.  Returns dict with r_lo, r_hi, the hidden
+    bounds (ls, us), the output affine bounds (W_up, b_up, W_lo, b_lo), J and p.
+
+    hidden = "crown": every hidden layer's pre-activation bounds by back-substitution to the input (full CROWN,
+    reading R11).  hidden = "ibp": hidden layers 2..L-1 by interval propagation of the previous layer's bounds
+    (CROWN-IBP: cheaper, looser intermediate bounds; the output is still back-substituted, Thm 2 holds for any valid
+    intermediate bounds).  PAPER.md:L194-196 leaves the CROWN variant open."""
     L = len(Ws)
     zs, p, J = nominal(Ws, bs, act, a0)
     if J_given is not None:
@@ -252,6 +270,12 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False):
     relaxs.append(relax(act, ls[0], us[0]))
     # hidden layers s = 2..L-1: full CROWN back-substitution to the input
     for s in range(2, L):
+        if hidden == "ibp":
+            lo_s, hi_s = ibp_layer(Ws[s - 1], bs[s - 1], act, ls[-1], us[-1])
+            ls.append(lo_s)
+            us.append(hi_s)
+            relaxs.append(relax(act, ls[-1], us[-1]))
+            continue
         res = backsub(Ws, bs, relaxs, s, keep=keep)
         Lu, cu, Ll, cl = res[:4]
         us.append(Lu @ a0 + np.abs(Lu) @ sig + cu)
@@ -270,7 +294,7 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False):
                 W_up=W_up, b_up=b_up, W_lo=W_lo, b_lo=b_lo, kept=kept)
 
 
-def leb_nn(Ws, bs, act, nom, rad, J=None):
+def leb_nn(Ws, bs, act, nom, rad, J=None, hidden="crown"):
     """Batch driver: nom, rad [tiles, N] -> r_lo, r_hi [tiles, n] (FP64)."""
     Ws = [np.asarray(W, dtype=np.float64) for W in Ws]
     bs = [np.asarray(b, dtype=np.float64) for b in bs]
@@ -280,7 +304,7 @@ def leb_nn(Ws, bs, act, nom, rad, J=None):
     r_lo = np.empty((nom.shape[0], n))
     r_hi = np.empty((nom.shape[0], n))
     for i in range(nom.shape[0]):
-        out = crown_forward(Ws, bs, act, nom[i], rad[i], None if J is None else np.asarray(J[i], dtype=np.float64))
+        out = crown_forward(Ws, bs, act, nom[i], rad[i], None if J is None else np.asarray(J[i], dtype=np.float64), hidden=hidden)
         r_lo[i], r_hi[i] = out["r_lo"], out["r_hi"]
     return r_lo, r_hi
 
@@ -423,12 +447,12 @@ def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
     return ties
 
 
-def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=()):
+def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown"):
     """Returns (grad_nom, grad_rad) for one tile; J is the network's own Jacobian at a~ (the
     product's leb_vjp takes no J argument).  `flips`: entries (chain, i, j) from
     output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink)."""
     L = len(Ws)
-    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True)
+    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True, hidden=hidden)
     relaxs, ls, us, zs, J = fw["relaxs"], fw["ls"], fw["us"], fw["zs"], fw["J"]
     a_bar = np.zeros_like(a0)
     s_bar = np.zeros_like(sig)
@@ -467,9 +491,22 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=()):
     a_bar += abar_l
 
     # ---- hidden targets s = L-1 .. 2 (seeds complete: only targets > s use layer s)
+    ibp_l = [np.zeros_like(x) for x in ls]      # hidden = "ibp": adjoints of (l_s, u_s) arriving from layer s+1's interval step
+    ibp_u = [np.zeros_like(x) for x in us]
     for s in range(L - 1, 1, -1):
         acc = padj[s - 1]
         lb, ub = relax_vjp(act, ls[s - 1], us[s - 1], relaxs[s - 1][4], acc[0], acc[1], acc[2], acc[3])
+        if hidden == "ibp":
+            # reverse of ibp_layer: l_s = W+ phi(l_{s-1}) + W- phi(u_{s-1}) + b, u_s = W+ phi(u_{s-1}) + W- phi(l_{s-1}) + b
+            lb = lb + ibp_l[s - 1]
+            ub = ub + ibp_u[s - 1]
+            W = Ws[s - 1]
+            Wp, Wn = np.maximum(W, 0.0), np.minimum(W, 0.0)
+            alo_bar = Wp.T @ lb + Wn.T @ ub
+            ahi_bar = Wp.T @ ub + Wn.T @ lb
+            ibp_l[s - 2] += dphi_at(act, ls[s - 2]) * alo_bar
+            ibp_u[s - 2] += dphi_at(act, us[s - 2]) * ahi_bar
+            continue
         Lams_up, Lams_lo = fw["kept"][s]
         Lu0, Ll0 = Lams_up[0], Lams_lo[0]
         a_bar += Lu0.T @ ub + Ll0.T @ lb
@@ -482,12 +519,14 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=()):
     # ---- layer 1: l_1, u_1 = W_1 a~ + b_1 -+ |W_1| sigma
     acc = padj[0]
     lb, ub = relax_vjp(act, ls[0], us[0], relaxs[0][4], acc[0], acc[1], acc[2], acc[3])
+    lb = lb + ibp_l[0]
+    ub = ub + ibp_u[0]
     a_bar += Ws[0].T @ (lb + ub)
     s_bar += np.abs(Ws[0]).T @ (ub - lb)
     return a_bar, s_bar
 
 
-def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi):
+def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi, hidden="crown"):
     """Batch driver: [tiles, N] inputs, [tiles, n] cotangents -> grads [tiles, N]."""
     Ws = [np.asarray(W, dtype=np.float64) for W in Ws]
     bs = [np.asarray(b, dtype=np.float64) for b in bs]
@@ -498,5 +537,5 @@ def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi):
     gn = np.empty_like(nom)
     gr = np.empty_like(rad)
     for i in range(nom.shape[0]):
-        gn[i], gr[i] = crown_vjp(Ws, bs, act, nom[i], rad[i], g_lo[i], g_hi[i])
+        gn[i], gr[i] = crown_vjp(Ws, bs, act, nom[i], rad[i], g_lo[i], g_hi[i], hidden=hidden)
     return gn, gr

@@ -319,3 +319,64 @@ def test_vjp_through_degenerate_tanh_neurons():
             checked += 1
     assert checked >= 7
     assert np.abs(gn[:3]).max() > 1e-3 * scale       # the zero-radius coordinates do carry gradient
+
+
+# ---------------------------------------------------------------- CROWN-IBP (hidden = "ibp"; PAPER.md:L194-196 leaves the variant open)
+@pytest.mark.parametrize("act,dims,seed", [(O.ACT_RELU, [6, 12, 12, 12, 4], 0), (O.ACT_TANH, [5, 16, 16, 16, 16, 3], 2)])
+def test_crown_ibp_sound_and_looser_hidden_bounds(act, dims, seed):
+    rng = np.random.default_rng(400 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    a0 = rng.standard_normal(dims[0])
+    sig = rng.uniform(0.05, 0.3, dims[0])
+    out = O.crown_forward(Ws, bs, act, a0, sig, hidden="ibp")
+    full = O.crown_forward(Ws, bs, act, a0, sig)
+    X = np.concatenate([a0 + sig * rng.uniform(-1, 1, (25000, dims[0])), _vertices(a0, sig)])
+    R = _true_r(Ws, bs, act, a0, X)
+    assert np.all(R.min(0) >= out["r_lo"] - 1e-12) and np.all(R.max(0) <= out["r_hi"] + 1e-12)
+    for x in X[::97]:
+        for z, l, u in zip(O.mlp_hidden(Ws, bs, act, x), out["ls"], out["us"]):
+            assert np.all(z >= l - 1e-12) and np.all(z <= u + 1e-12)
+    # layer 1 is the same; layer 2 by interval arithmetic is the textbook product [W][a] + b
+    assert np.array_equal(out["ls"][0], full["ls"][0]) and np.array_equal(out["us"][0], full["us"][0])
+    a_lo, a_hi = O.phi(act, out["ls"][0]), O.phi(act, out["us"][0])
+    c, r = 0.5 * (a_hi + a_lo), 0.5 * (a_hi - a_lo)
+    assert np.allclose(out["ls"][1], Ws[1] @ c - np.abs(Ws[1]) @ r + bs[1], atol=1e-13)
+    assert np.allclose(out["us"][1], Ws[1] @ c + np.abs(Ws[1]) @ r + bs[1], atol=1e-13)
+    # the interval bounds of the deeper layers are looser than full CROWN's on these nets, and so is the final bound
+    assert (out["us"][-1] - out["ls"][-1]).sum() > (full["us"][-1] - full["ls"][-1]).sum()
+    assert (out["r_hi"] - out["r_lo"]).sum() >= (full["r_hi"] - full["r_lo"]).sum() - 1e-12
+
+
+def test_crown_ibp_equals_crown_with_one_hidden_layer():
+    rng = np.random.default_rng(5)
+    Ws, bs = _net(rng, [5, 9, 3])
+    a0, sig = rng.standard_normal(5), rng.uniform(0.05, 0.3, 5)
+    a, b = O.crown_forward(Ws, bs, O.ACT_TANH, a0, sig, hidden="ibp"), O.crown_forward(Ws, bs, O.ACT_TANH, a0, sig)
+    assert np.array_equal(a["r_lo"], b["r_lo"]) and np.array_equal(a["r_hi"], b["r_hi"])
+
+
+@pytest.mark.parametrize("act,dims,seed", [(O.ACT_TANH, [6, 10, 10, 10, 4], 1), (O.ACT_RELU, [6, 10, 10, 10, 4], 0), (O.ACT_TANH, [5, 8, 8, 8, 8, 3], 3)])
+def test_crown_ibp_vjp_matches_central_differences(act, dims, seed):
+    rng = np.random.default_rng(500 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    a0 = rng.standard_normal(dims[0])
+    sig = rng.uniform(0.05, 0.3, dims[0])
+    g_lo, g_hi = rng.standard_normal(dims[-1]), rng.standard_normal(dims[-1])
+    gn, gr = O.crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, hidden="ibp")
+
+    def F(a, s):
+        f = O.crown_forward(Ws, bs, act, a, s, hidden="ibp")
+        return g_hi @ f["r_hi"] + g_lo @ f["r_lo"]
+    N, h, ok = dims[0], 1e-6, 0
+    F0 = F(a0, sig)
+    scale = max(np.abs(gn).max(), np.abs(gr).max())
+    for i in range(2 * N):
+        e = np.zeros(N)
+        e[i % N] = h
+        fp, fm = (F(a0 + e, sig), F(a0 - e, sig)) if i < N else (F(a0, sig + e), F(a0, sig - e))
+        if abs((fp - F0) - (F0 - fm)) > 1e-3 * abs(fp - fm) + 1e-12:
+            continue
+        g = gn[i] if i < N else gr[i - N]
+        assert abs((fp - fm) / (2 * h) - g) <= 1e-6 * scale + 1e-5 * abs(g), i
+        ok += 1
+    assert ok >= N
