@@ -103,6 +103,10 @@ enum {
     LEB_FLAG_HOST_IO = 4u,   /* data pointers of this call are host pointers */
     LEB_FLAG_SINGLE_CTA = 16u, /* NN: forward chain steps on single CTAs (nn_gemm_tc.cuh) instead of CTA pairs
                                   (tcgen05.mma.cta_group::2, nn_gemm_tc2.cuh, the default); same results bit for bit */
+    LEB_FLAG_IBP_HIDDEN = 32u, /* NN: CROWN-IBP -- the bounds of hidden layers 2..L-1 by interval propagation of the previous
+                                  layer's bounds instead of back-substitution (about 4x fewer flops at config 5, looser
+                                  bounds); the output is back-substituted as always.  Value mode only: without
+                                  LEB_FLAG_NO_MARGIN the call returns LEB_ERR_UNSUPPORTED.  leb_vjp takes the same flag. */
     LEB_FLAG_REUSE_FWD = 8u  /* leb_vjp(kind 1) becomes STATEFUL: the caller states that (nom, rad) are those of the previous
                                 leb_nn_fwd call on this context (J == NULL).  If the workspace still holds that call's complete
                                 forward state (the batch fitted one chunk) AND that state was computed in the mode this

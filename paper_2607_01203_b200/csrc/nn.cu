@@ -41,6 +41,7 @@ struct NnState {
     float *W[kMaxLayers + 1] = {nullptr}, *Wt[kMaxLayers + 1] = {nullptr}, *bias[kMaxLayers + 1] = {nullptr};
     int rowsW[kMaxLayers + 1] = {0};
     float *Wabs1 = nullptr, *Wabs1t = nullptr;
+    float *Wabs[kMaxLayers + 1] = {nullptr}, *Wabst[kMaxLayers + 1] = {nullptr};   // |W_l|, |W_l|^T for l = 2..L-1 (CROWN-IBP mode)
     // 3xTF32 tensor-core path: hi/lo splits of W[l] (reverse sweep) and Wt[l] (forward chain), l = 1..L-1, and their TMA maps
     float *Whi[kMaxLayers + 1] = {nullptr}, *Wlo[kMaxLayers + 1] = {nullptr}, *Wthi[kMaxLayers + 1] = {nullptr}, *Wtlo[kMaxLayers + 1] = {nullptr};
     CUtensorMap mapW_hi[kMaxLayers + 1], mapW_lo[kMaxLayers + 1], mapWt_hi[kMaxLayers + 1], mapWt_lo[kMaxLayers + 1];
@@ -72,6 +73,7 @@ struct NnState {
     int last_tiles = 0;          // > 0: the workspace holds the complete forward state of that many tiles (one chunk)
     bool last_with_jac = false;  // ... including the Jacobian chain rows (needed by the reverse sweep)
     bool last_cert = false;      // ... computed in certified mode (widened hidden bounds, padded gaps)
+    bool last_ibp = false;       // ... with hidden-layer bounds by interval propagation (LEB_FLAG_IBP_HIDDEN)
     bool last_vjp_reused = false;   // the last leb_vjp(kind 1) started from the resident forward state
     LebProf* prof = nullptr;
 };
@@ -482,6 +484,73 @@ __global__ void relax_vjp_kernel(int act, int tiles, int w_valid, int wp, const 
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// CROWN-IBP mode (LEB_FLAG_IBP_HIDDEN): hidden layers s = 2..L-1 bounded by interval propagation of the previous layer's
+// bounds instead of back-substitution (PAPER.md:L194-196 leaves the CROWN variant open).  In deviation form:
+// a_{s-1} - ahat_{s-1} in [dl, du] = [phi(l) - phi(zhat), phi(u) - phi(zhat)] (phi monotone), centre dc, radius dr;
+// z_s - zhat_s in W_s dc -+ |W_s| dr.
+// ------------------------------------------------------------------------------------------
+__global__ void ibp_dev_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ lb,
+                               const float* __restrict__ ub, float* __restrict__ dc, float* __restrict__ dr) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) { dc[q] = 0.f; dr[q] = 0.f; continue; }
+        const double f = act_f(act, (double)zhat[q]);
+        const double dl = act_f(act, (double)lb[q]) - f, du = act_f(act, (double)ub[q]) - f;
+        dc[q] = (float)(0.5 * (du + dl));
+        dr[q] = (float)(0.5 * (du - dl));
+    }
+}
+
+__global__ void ibp_bounds_kernel(int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ zc,
+                                  const float* __restrict__ zr, float* __restrict__ lb, float* __restrict__ ub) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) { lb[q] = 0.f; ub[q] = 0.f; continue; }
+        const float z = zhat[q], m = zc[q], r = zr[q];
+        lb[q] = z + (m - r);
+        ub[q] = z + (m + r);
+    }
+}
+
+// reverse: seeds of the two products from the (complete) adjoints of (l_s, u_s)
+__global__ void ibp_seed_kernel(size_t count, const float* __restrict__ lbar, const float* __restrict__ ubar, float* __restrict__ zcb,
+                                float* __restrict__ zrb) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) {
+        const float l = lbar[q], u = ubar[q];
+        zcb[q] = l + u;
+        zrb[q] = u - l;
+    }
+}
+
+// reverse: (dc_bar, dr_bar) of layer s-1 -> what layer s's interval step sends to (l_{s-1}, u_{s-1}) and to zhat_{s-1}
+__global__ void ibp_bwd_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ lb,
+                               const float* __restrict__ ub, const float* __restrict__ dcb, const float* __restrict__ drb,
+                               float* __restrict__ ibl, float* __restrict__ ibu, float* __restrict__ zbar) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) { ibl[q] = 0.f; ibu[q] = 0.f; continue; }
+        const double dlb = 0.5 * ((double)dcb[q] - (double)drb[q]), dub = 0.5 * ((double)dcb[q] + (double)drb[q]);
+        ibl[q] = (float)(act_d1(act, (double)lb[q]) * dlb);
+        ibu[q] = (float)(act_d1(act, (double)ub[q]) * dub);
+        zbar[q] += (float)(-act_d1(act, (double)zhat[q]) * (dlb + dub));
+    }
+}
+
+// reverse: add what the next layer's interval step sent; l = zhat + ..., u = zhat + ... pass it on to zhat as well
+__global__ void ibp_add_kernel(size_t count, float* __restrict__ lbar, float* __restrict__ ubar, float* __restrict__ zbar,
+                               const float* __restrict__ ibl, const float* __restrict__ ibu) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) {
+        const float a = ibl[q], b = ibu[q];
+        lbar[q] += a;
+        ubar[q] += b;
+        zbar[q] += a + b;
+    }
+}
+
 // ub1 - lb1 adjoint for the layer-1 radius |W_1| sigma
 __global__ void diff_kernel(const float* __restrict__ ubar, const float* __restrict__ lbar, float* __restrict__ out, size_t count) {
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x)
@@ -662,7 +731,7 @@ void launch_cert_layer(NnState* S, int C, int l, bool out_only, cudaStream_t st,
 }
 
 void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool cert, bool marg_report, cudaStream_t st,
-                   long long* launches) {
+                   long long* launches, bool ibp = false) {
     const int L = S->L;
     int ksum = 0;                                   // total contraction length of the gap sums of the deepest chain
     for (int l = 1; l < L; ++l) ksum += S->wp[l];
@@ -695,6 +764,22 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
         const bool is_out = (s == L);
         const int nk = is_out ? (with_jac ? 3 : 2) : 2;
         const int rp = S->rows_pad[s], rk = S->rows_kind[s];
+        if (ibp && !is_out) {
+            // CROWN-IBP: l_s, u_s = zhat_s + W_s dc -+ |W_s| dr (the cert-mode arrays serve as scratch: value mode only)
+            const size_t cp = (size_t)C * S->wp[s - 1], cs = (size_t)C * S->wp[s];
+            ibp_dev_kernel<<<gs_grid(cp), 256, 0, st>>>(S->act, C, S->w[s - 1], S->wp[s - 1], S->zhat[s - 1], S->lb[s - 1], S->ub[s - 1],
+                                                       S->ce[s - 1], S->ct[s - 1]);
+            ++*launches;
+            GemmArgs g1 = plain_args(C, S->wp[s], S->wp[s - 1], S->ce[s - 1], S->wp[s - 1], S->Wt[s], S->wp[s], S->cv[s], S->wp[s]);
+            launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g1, st, launches);
+            GemmArgs g2 = plain_args(C, S->wp[s], S->wp[s - 1], S->ct[s - 1], S->wp[s - 1], S->Wabst[s], S->wp[s], S->adev[s], S->wp[s]);
+            launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g2, st, launches);
+            ibp_bounds_kernel<<<gs_grid(cs), 256, 0, st>>>(C, S->w[s], S->wp[s], S->zhat[s], S->cv[s], S->adev[s], S->lb[s], S->ub[s]);
+            relax_fwd_kernel<<<gs_grid(cs), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s], S->ub[s], S->kU[s],
+                                                         S->kL[s], S->gU[s], S->gL[s]);
+            *launches += 2;
+            continue;
+        }
         if (cert) launch_cert_layer(S, C, s, is_out, st, launches);     // e_s, t_s, v_s (eta for the output) -- needs adev_{s-1}
         for (int l = s - 1; l >= 1; --l) {
             GemmArgs g{};
@@ -758,7 +843,7 @@ static void free_weights(NnState* S) {
         if (S->Wt[l]) cudaFree(S->Wt[l]);
         if (S->bias[l]) cudaFree(S->bias[l]);
         S->W[l] = S->Wt[l] = S->bias[l] = nullptr;
-        for (float** p : {&S->Whi[l], &S->Wlo[l], &S->Wthi[l], &S->Wtlo[l]}) { if (*p) cudaFree(*p); *p = nullptr; }
+        for (float** p : {&S->Whi[l], &S->Wlo[l], &S->Wthi[l], &S->Wtlo[l], &S->Wabs[l], &S->Wabst[l]}) { if (*p) cudaFree(*p); *p = nullptr; }
     }
     S->tc_ready = false;
     if (S->Wabs1) cudaFree(S->Wabs1);
@@ -834,6 +919,14 @@ leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long lo
             split_tf32_kernel<<<gs_grid(tot), 256, 0, st>>>(S->Wt[l], S->Wthi[l], S->Wtlo[l], tot);
             *launches += 2;
         }
+        if (l >= 2 && l < L) {
+            ok = ok && cudaMalloc(&S->Wabs[l], tot * sizeof(float)) == cudaSuccess;
+            ok = ok && cudaMalloc(&S->Wabst[l], tot * sizeof(float)) == cudaSuccess;
+            if (!ok) break;
+            pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wabs[l], rows_p, cols_p, 0, 1);
+            pack_matrix_kernel<<<gs_grid(tot), 256, 0, st>>>(src, rows, cols, cols, S->Wabst[l], rows_p, cols_p, 1, 1);
+            *launches += 2;
+        }
         if (l == 1) {
             ok = ok && cudaMalloc(&S->Wabs1, tot * sizeof(float)) == cudaSuccess;
             ok = ok && cudaMalloc(&S->Wabs1t, tot * sizeof(float)) == cudaSuccess;
@@ -878,6 +971,8 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
     S->use_pairs = S->use_tc && !(flags & LEB_FLAG_SINGLE_CTA);
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
+    const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
+    if (ibp && cert) return LEB_ERR_UNSUPPORTED;                       // the rounding bookkeeping covers the back-substituted hidden bounds only
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
     if (tiles == 0) return LEB_OK;
@@ -889,7 +984,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         pad_inputs_kernel<<<gs_grid((size_t)C * S->wp[0]), 256, 0, st>>>(C, N, ld_in, S->wp[0], nom + (size_t)t0 * ld_in,
                                                                        rad + (size_t)t0 * ld_in, S->nomp, S->radp);
         ++*launches;
-        forward_chunk(S, C, J, J == nullptr, cert, cert && margin != nullptr, st, launches);
+        forward_chunk(S, C, J, J == nullptr, cert, cert && margin != nullptr, st, launches, ibp);
         size_t warps = (size_t)C * n;
         const int ks = [&] { int k = 0; for (int l = 1; l < L; ++l) k += S->wp[l]; return k; }();
         concretise_out_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(
@@ -901,6 +996,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
         S->last_with_jac = (J == nullptr);
         S->last_cert = cert;
+        S->last_ibp = ibp;
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
@@ -946,9 +1042,10 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     // LEB_FLAG_REUSE_FWD: the caller states that (nom, rad) are those of the previous leb_nn_fwd call on this context; if the
     // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
     // and was computed in the mode this call names (LEB_FLAG_NO_MARGIN: a value-mode state; otherwise a certified one).
-    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN);
+    const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
+    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp;
     const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
-                       S->last_cert == want_cert;
+                       S->last_cert == want_cert && S->last_ibp == ibp;
     S->last_vjp_reused = reuse;
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
@@ -959,7 +1056,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                                                                    g_hi + (size_t)t0 * ld_out, S->glo_p, S->ghi_p);
         *launches += 2;
         // the VJP is that of the value-mode bound: the certified margin is a rounding-level outward pad, treated as constant
-        if (!reuse) forward_chunk(S, C, nullptr, true, false, false, st, launches);
+        if (!reuse) forward_chunk(S, C, nullptr, true, false, false, st, launches, ibp);
         // ---- zero the adjoint accumulators
         for (int l = 1; l < L; ++l) {
             size_t c = (size_t)C * S->wp[l];
@@ -978,6 +1075,20 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                                                                               S->ub[s], S->kUb[s], S->kLb[s], S->gUb[s], S->gLb[s],
                                                                               S->dpb[s], S->lbar[s], S->ubar[s], S->zbar[s], 0);
                 ++*launches;
+            }
+            if (ibp && !is_out) {
+                // CROWN-IBP: reverse of the interval step of layer s (see ibp_dev_kernel); mU / mL hold what layer s+1 sent
+                const size_t cs = (size_t)C * S->wp[s], cp = (size_t)C * S->wp[s - 1];
+                if (s < L - 1) { ibp_add_kernel<<<gs_grid(cs), 256, 0, st>>>(cs, S->lbar[s], S->ubar[s], S->zbar[s], S->mU[s], S->mL[s]); ++*launches; }
+                ibp_seed_kernel<<<gs_grid(cs), 256, 0, st>>>(cs, S->lbar[s], S->ubar[s], S->cv[s], S->adev[s]);
+                GemmArgs g1 = plain_args(C, S->wp[s - 1], S->wp[s], S->cv[s], S->wp[s], S->W[s], S->wp[s - 1], S->ce[s - 1], S->wp[s - 1]);
+                launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g1, st, launches);
+                GemmArgs g2 = plain_args(C, S->wp[s - 1], S->wp[s], S->adev[s], S->wp[s], S->Wabs[s], S->wp[s - 1], S->ct[s - 1], S->wp[s - 1]);
+                launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g2, st, launches);
+                ibp_bwd_kernel<<<gs_grid(cp), 256, 0, st>>>(S->act, C, S->w[s - 1], S->wp[s - 1], S->zhat[s - 1], S->lb[s - 1], S->ub[s - 1],
+                                                           S->ce[s - 1], S->ct[s - 1], S->mU[s - 1], S->mL[s - 1], S->zbar[s - 1]);
+                *launches += 2;
+                continue;
             }
             const float* yu = is_out ? S->ghi_p : S->ubar[s];
             const float* yl = is_out ? S->glo_p : S->lbar[s];
@@ -1017,6 +1128,11 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         relax_vjp_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->lb[1], S->ub[1],
                                                                       S->kUb[1], S->kLb[1], S->gUb[1], S->gLb[1], S->dpb[1],
                                                                       S->lbar[1], S->ubar[1], S->zbar[1], 1);
+        if (ibp && L > 2) {
+            const size_t c1 = (size_t)C * S->wp[1];
+            ibp_add_kernel<<<gs_grid(c1), 256, 0, st>>>(c1, S->lbar[1], S->ubar[1], S->zbar[1], S->mU[1], S->mL[1]);
+            ++*launches;
+        }
         diff_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->ubar[1], S->lbar[1], S->rad1, (size_t)C * S->wp[1]);
         *launches += 2;
         {
@@ -1037,7 +1153,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,
                                                                  grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in);
         ++*launches;
-        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; }   // a value-mode forward state
+        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;

@@ -23,6 +23,7 @@ FLAG_FFMA_ONLY = 2
 FLAG_HOST_IO = 4
 FLAG_REUSE_FWD = 8
 FLAG_SINGLE_CTA = 16
+FLAG_IBP_HIDDEN = 32
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",

@@ -334,3 +334,74 @@ def test_edge_cases(mods):
     assert e.value.status == leb.LEB_ERR_STATE
     ctx2.close()
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- CROWN-IBP (LEB_FLAG_IBP_HIDDEN)
+IBP = 32
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_crown_ibp_small_nets_match_oracle(mods, dims, act, path):
+    """Hidden layers 2..L-1 by interval propagation, output by back-substitution: forward, hidden bounds and VJP against
+    the oracle's hidden="ibp" branch."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    ctx = leb.context_for_workload(w)
+    flags = PATHS[path] | IBP
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=flags)
+    nom, rad, g_lo, g_hi = _flat(w)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, hidden="ibp")
+    assert_bounds_close(to_np(lo).reshape(-1, w.n), olo, f"crown-ibp {dims} r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n), ohi, f"crown-ibp {dims} r_hi")
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    for layer in range(1, len(dims) - 1):
+        l, u = ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])
+        fw = O.crown_forward(Ws, bs, act, nom[0].astype(np.float64), rad[0].astype(np.float64), hidden="ibp")
+        assert np.allclose(to_np(l)[0], fw["ls"][layer - 1], rtol=2e-5, atol=2e-6)
+        assert np.allclose(to_np(u)[0], fw["us"][layer - 1], rtol=2e-5, atol=2e-6)
+    # VJP: stateless and from the resident forward state
+    gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=flags)
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, act, nom, rad, g_lo, g_hi, hidden="ibp")
+    assert_grads_close(to_np(gn), to_np(gr), ogn, ogr, f"crown-ibp {dims}")
+    ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=flags)
+    g2 = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=flags | leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state()[2] is True
+    for a, b in ((g2[0], gn), (g2[1], gr)):          # column sums are atomic adds: equal to rounding, not bit for bit
+        assert float((a - b).abs().max()) <= 1e-5 * float(b.abs().max())
+    # a full-CROWN state is not reused for a CROWN-IBP gradient, and the certified mode refuses the flag
+    ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+    ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=flags | leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state()[2] is False
+    with pytest.raises(leb.LebError) as e:
+        ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=IBP)
+    assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,tiles", [(3, 16), (5, 8)])
+def test_crown_ibp_configs_sampled_tiles(mods, cfg, tiles):
+    leb, wl, O = mods
+    w = wl.make_config(cfg)
+    ctx = leb.context_for_workload(w)
+    nom_d, rad_d = _dev(w.nom), _dev(w.rad)
+    launches0 = ctx.leb_launch_count()
+    lo, hi = ctx.leb_nn_fwd(nom_d, rad_d, flags=VAL | IBP)
+    n_ibp = ctx.leb_launch_count() - launches0
+    gn, gr = ctx.leb_vjp(1, nom_d, rad_d, _dev(w.g_lo), _dev(w.g_hi), flags=VAL | IBP | leb.FLAG_REUSE_FWD)
+    flo, fhi = ctx.leb_nn_fwd(nom_d, rad_d, flags=VAL)
+    nom, rad, g_lo, g_hi = _flat(w)
+    idx = np.linspace(0, w.B * w.T - 1, tiles).astype(int)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx], hidden="ibp")
+    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, f"cfg{cfg} crown-ibp r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, f"cfg{cfg} crown-ibp r_hi")
+    vi = idx[::2]
+    ogn, ogr = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[vi], rad[vi], g_lo[vi], g_hi[vi], hidden="ibp")
+    from parity_util import grads_ratio
+    ratio = grads_ratio(to_np(gn).reshape(-1, w.N)[vi], to_np(gr).reshape(-1, w.N)[vi], ogn, ogr)
+    assert (ratio <= 1.0).sum() >= len(vi) - 1, ratio           # at most one tile on a kink of |W - J| (reading R20)
+    # looser than full CROWN, by a reported factor
+    wide = float(((hi - lo).sum() / (fhi - flo).sum()))
+    print(f"config {cfg}: CROWN-IBP enclosure width / full CROWN = {wide:.3f}")
+    assert wide >= 1.0 - 1e-6
+    ctx.close()
