@@ -266,6 +266,19 @@ def run_ours(args):
                       "certified_excess_over_value_mode_median": float(ex.median()),
                       "certified_excess_over_value_mode_max": float(ex.max()),
                       "unit": "fraction of the enclosure width", "certified_contains_value_mode": bool((ex >= -1e-5).all())}
+        # CROWN-IBP (LEB_FLAG_IBP_HIDDEN, value mode): the cheap, loose variant -- hidden bounds by interval propagation
+        IBPF = leb.FLAG_NO_MARGIN | leb.FLAG_IBP_HIDDEN
+        step_device(IBPF)
+        torch.cuda.synchronize()
+        c0.record()
+        for _ in range(args.steps):
+            step_device(IBPF)
+        c1.record()
+        torch.cuda.synchronize()
+        ib_ms = c0.elapsed_time(c1) / max(args.steps, 1)
+        i_lo, i_hi = ctx.leb_nn_fwd(nom, rad, flags=IBPF)
+        value_mode["crown_ibp"] = {"ms_per_step": ib_ms, "value": w.entries / (ib_ms * 1e-3),
+                                   "enclosure_width_over_full_crown": float((i_hi - i_lo).sum() / (v_hi - v_lo).sum())}
     if rank == 0:
         peaks = _peaks()
         dom = max((0, 1), key=lambda kc: kstats[kc][0])
