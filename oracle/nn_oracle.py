@@ -249,24 +249,30 @@ def ibp_layer(W, b, act, l_prev, u_prev):
     return Wp @ a_lo + Wn @ a_hi + b, Wp @ a_hi + Wn @ a_lo + b
 
 
-def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"):
+def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown", mu=None):
     """CROWN + Thm 3 for one tile.  Returns dict with r_lo, r_hi, the hidden
     bounds (ls, us), the output affine bounds (W_up, b_up, W_lo, b_lo), J and p.
 
     hidden = "crown": every hidden layer's pre-activation bounds by back-substitution to the input (full CROWN,
     reading R11).  hidden = "ibp": hidden layers 2..L-1 by interval propagation of the previous layer's bounds
     (CROWN-IBP: cheaper, looser intermediate bounds; the output is still back-substituted, Thm 2 holds for any valid
-    intermediate bounds).  PAPER.md:L194-196 leaves the CROWN variant open."""
+    intermediate bounds).  PAPER.md:L194-196 leaves the CROWN variant open.
+
+    mu: non-centred box (25a) PAPER.md:L272: the CROWN bounds are taken on the box c + [-sig, sig], c = a0 + mu, while
+    p(a~) and J(a~) of the remainder (10) stay at the nominal point a0; Thm 3's maximisation (21) of the affine r_up(a)
+    = (W_up - J) a + J a~ - p(a~) + b_up (20) then runs over that box.  (Thm 2 / Thm 3 need no a~ in the box.)"""
     L = len(Ws)
     zs, p, J = nominal(Ws, bs, act, a0)
     if J_given is not None:
         J = J_given
+    c = a0 if mu is None else a0 + mu
     ls, us, relaxs = [], [], []
     kept = {}
     # layer 1: interval affine
     A1 = np.abs(Ws[0]) @ sig
-    ls.append(zs[0] - A1)
-    us.append(zs[0] + A1)
+    z1c = zs[0] if mu is None else Ws[0] @ c + bs[0]
+    ls.append(z1c - A1)
+    us.append(z1c + A1)
     relaxs.append(relax(act, ls[0], us[0]))
     # hidden layers s = 2..L-1: full CROWN back-substitution to the input
     for s in range(2, L):
@@ -278,8 +284,8 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"
             continue
         res = backsub(Ws, bs, relaxs, s, keep=keep)
         Lu, cu, Ll, cl = res[:4]
-        us.append(Lu @ a0 + np.abs(Lu) @ sig + cu)
-        ls.append(Ll @ a0 - np.abs(Ll) @ sig + cl)
+        us.append(Lu @ c + np.abs(Lu) @ sig + cu)
+        ls.append(Ll @ c - np.abs(Ll) @ sig + cl)
         relaxs.append(relax(act, ls[-1], us[-1]))
         if keep:
             kept[s] = res[4:]
@@ -287,14 +293,18 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"
     W_up, b_up, W_lo, b_lo = res[:4]
     if keep:
         kept[L] = res[4:]
-    # Thm 3, eq. (20)-(21) on the centred box [a0 - sig, a0 + sig]
-    r_hi = np.abs(W_up - J) @ sig + (W_up @ a0 + b_up - p)
-    r_lo = -np.abs(W_lo - J) @ sig + (W_lo @ a0 + b_lo - p)
+    # Thm 3, eq. (20)-(21): box maximum of (W - J) a + J a~ - p(a~) + b over c + [-sig, sig] (c = a0: J a~ cancels)
+    if mu is None:
+        r_hi = np.abs(W_up - J) @ sig + (W_up @ a0 + b_up - p)
+        r_lo = -np.abs(W_lo - J) @ sig + (W_lo @ a0 + b_lo - p)
+    else:
+        r_hi = np.abs(W_up - J) @ sig + (W_up - J) @ c + J @ a0 - p + b_up
+        r_lo = -np.abs(W_lo - J) @ sig + (W_lo - J) @ c + J @ a0 - p + b_lo
     return dict(r_lo=r_lo, r_hi=r_hi, ls=ls, us=us, relaxs=relaxs, zs=zs, p=p, J=J,
                 W_up=W_up, b_up=b_up, W_lo=W_lo, b_lo=b_lo, kept=kept)
 
 
-def leb_nn(Ws, bs, act, nom, rad, J=None, hidden="crown"):
+def leb_nn(Ws, bs, act, nom, rad, J=None, hidden="crown", mu=None):
     """Batch driver: nom, rad [tiles, N] -> r_lo, r_hi [tiles, n] (FP64)."""
     Ws = [np.asarray(W, dtype=np.float64) for W in Ws]
     bs = [np.asarray(b, dtype=np.float64) for b in bs]
@@ -304,7 +314,8 @@ def leb_nn(Ws, bs, act, nom, rad, J=None, hidden="crown"):
     r_lo = np.empty((nom.shape[0], n))
     r_hi = np.empty((nom.shape[0], n))
     for i in range(nom.shape[0]):
-        out = crown_forward(Ws, bs, act, nom[i], rad[i], None if J is None else np.asarray(J[i], dtype=np.float64), hidden=hidden)
+        out = crown_forward(Ws, bs, act, nom[i], rad[i], None if J is None else np.asarray(J[i], dtype=np.float64), hidden=hidden,
+                            mu=None if mu is None else np.asarray(mu[i], dtype=np.float64))
         r_lo[i], r_hi[i] = out["r_lo"], out["r_hi"]
     return r_lo, r_hi
 
@@ -447,13 +458,16 @@ def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
     return ties
 
 
-def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown"):
-    """Returns (grad_nom, grad_rad) for one tile; J is the network's own Jacobian at a~ (the
-    product's leb_vjp takes no J argument).  `flips`: entries (chain, i, j) from
-    output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink)."""
+def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown", mu=None):
+    """Returns (grad_nom, grad_rad) -- with mu: (grad_nom, grad_rad, grad_mu) -- for one tile; J is the network's own
+    Jacobian at a~ (the product's leb_vjp takes no J argument).  `flips`: entries (chain, i, j) from
+    output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink).
+    Every bound depends on the box centre c = a~ + mu (adjoint a_bar below, shared by a~ and mu); p(a~), J(a~) and the
+    explicit terms J a~ - J c = -J mu depend on a~ and mu separately."""
     L = len(Ws)
-    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True, hidden=hidden)
+    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True, hidden=hidden, mu=mu)
     relaxs, ls, us, zs, J = fw["relaxs"], fw["ls"], fw["us"], fw["zs"], fw["J"]
+    a0 = a0 if mu is None else a0 + mu          # the box centre c: what the bounds below see
     a_bar = np.zeros_like(a0)
     s_bar = np.zeros_like(sig)
     padj = [[np.zeros(Ws[l].shape[0]) for _ in range(4)] for l in range(L - 1)]
@@ -469,6 +483,8 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown"):
     Lbar_up = g_hi[:, None] * (Su * sig[None, :] + a0[None, :])
     Lbar_lo = g_lo[:, None] * (-Sl * sig[None, :] + a0[None, :])
     Jbar = -g_hi[:, None] * Su * sig[None, :] + g_lo[:, None] * Sl * sig[None, :]
+    if mu is not None:
+        Jbar = Jbar - np.outer(g_hi + g_lo, mu)          # the explicit -J mu of (20)
     pbar = -(g_hi + g_lo)
     _chain_reverse(Ws, bs, relaxs, L, Lams_up, Lbar_up, g_hi.copy(), True, padj)
     _chain_reverse(Ws, bs, relaxs, L, Lams_lo, Lbar_lo, g_lo.copy(), False, padj)
@@ -488,7 +504,7 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown"):
         q = np.einsum("ik,ij,kj->k", G[l], Jbar, WF)    # diag(G^T Jbar WF^T)
         zbar = zbar + d2phi(act, zs[l - 1]) * q
         abar_l = Ws[l - 1].T @ zbar
-    a_bar += abar_l
+    nominal_bar = abar_l                       # through p(a~) and J(a~): the nominal point only
 
     # ---- hidden targets s = L-1 .. 2 (seeds complete: only targets > s use layer s)
     ibp_l = [np.zeros_like(x) for x in ls]      # hidden = "ibp": adjoints of (l_s, u_s) arriving from layer s+1's interval step
@@ -523,11 +539,13 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown"):
     ub = ub + ibp_u[0]
     a_bar += Ws[0].T @ (lb + ub)
     s_bar += np.abs(Ws[0]).T @ (ub - lb)
-    return a_bar, s_bar
+    if mu is None:
+        return a_bar + nominal_bar, s_bar
+    return a_bar + nominal_bar, s_bar, a_bar - J.T @ (g_hi + g_lo)
 
 
-def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi, hidden="crown"):
-    """Batch driver: [tiles, N] inputs, [tiles, n] cotangents -> grads [tiles, N]."""
+def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi, hidden="crown", mu=None):
+    """Batch driver: [tiles, N] inputs, [tiles, n] cotangents -> grads [tiles, N] (a third array with mu)."""
     Ws = [np.asarray(W, dtype=np.float64) for W in Ws]
     bs = [np.asarray(b, dtype=np.float64) for b in bs]
     nom = np.asarray(nom, dtype=np.float64)
@@ -536,6 +554,12 @@ def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi, hidden="crown"):
     g_hi = np.asarray(g_hi, dtype=np.float64)
     gn = np.empty_like(nom)
     gr = np.empty_like(rad)
+    if mu is not None:
+        mu = np.asarray(mu, dtype=np.float64)
+        gm = np.empty_like(nom)
+        for i in range(nom.shape[0]):
+            gn[i], gr[i], gm[i] = crown_vjp(Ws, bs, act, nom[i], rad[i], g_lo[i], g_hi[i], hidden=hidden, mu=mu[i])
+        return gn, gr, gm
     for i in range(nom.shape[0]):
         gn[i], gr[i] = crown_vjp(Ws, bs, act, nom[i], rad[i], g_lo[i], g_hi[i], hidden=hidden)
     return gn, gr

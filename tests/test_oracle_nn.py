@@ -380,3 +380,93 @@ def test_crown_ibp_vjp_matches_central_differences(act, dims, seed):
         assert abs((fp - fm) / (2 * h) - g) <= 1e-6 * scale + 1e-5 * abs(g), i
         ok += 1
     assert ok >= N
+
+
+# ---------------------------------------------------------------- non-centred boxes (25a) PAPER.md:L272 on the NN path
+def _true_r_about(Ws, bs, act, a0, X):
+    """remainder (10) about the nominal point a0 at the points X (which need not surround a0)"""
+    return _true_r(Ws, bs, act, a0, X)
+
+
+@pytest.mark.parametrize("act,dims,seed,hidden", [(O.ACT_RELU, [6, 12, 12, 12, 4], 0, "crown"), (O.ACT_TANH, [6, 12, 12, 12, 4], 1, "crown"),
+                                                  (O.ACT_TANH, [5, 16, 16, 16, 16, 3], 2, "ibp"), (O.ACT_RELU, [8, 10, 10, 5], 3, "crown")])
+def test_mu_soundness_and_reduction(act, dims, seed, hidden):
+    rng = np.random.default_rng(600 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    a0 = rng.standard_normal(dims[0])
+    sig = rng.uniform(0.05, 0.3, dims[0])
+    mu = sig * rng.uniform(-2.0, 2.0, dims[0])                 # some |mu| > sigma: the nominal point outside the box
+    assert (np.abs(mu) > sig).any()
+    z = O.crown_forward(Ws, bs, act, a0, sig, hidden=hidden, mu=np.zeros_like(a0))
+    c = O.crown_forward(Ws, bs, act, a0, sig, hidden=hidden)
+    assert np.allclose(z["r_lo"], c["r_lo"], rtol=0, atol=1e-13) and np.allclose(z["r_hi"], c["r_hi"], rtol=0, atol=1e-13)
+    out = O.crown_forward(Ws, bs, act, a0, sig, hidden=hidden, mu=mu)
+    X = np.concatenate([a0 + mu + sig * rng.uniform(-1, 1, (25000, dims[0])), _vertices(a0 + mu, sig)])
+    R = _true_r_about(Ws, bs, act, a0, X)
+    assert np.all(R.min(0) >= out["r_lo"] - 1e-12) and np.all(R.max(0) <= out["r_hi"] + 1e-12)
+    for x in X[::97]:
+        for zz, l, u in zip(O.mlp_hidden(Ws, bs, act, x), out["ls"], out["us"]):
+            assert np.all(zz >= l - 1e-12) and np.all(zz <= u + 1e-12)
+    # not vacuous: the sampled range fills a fair part of the enclosure on these small nets
+    if hidden == "crown":
+        assert ((R.max(0) - R.min(0)) / (out["r_hi"] - out["r_lo"])).max() > 0.2
+
+
+def test_mu_exact_range_1hidden_relu():
+    """1-hidden-layer ReLU net, 2 inputs, offset box: r about a0 is piecewise linear on the box c +- sigma; enumerate the
+    arrangement vertices (test helper above works on any box: it takes the box centre)."""
+    rng = np.random.default_rng(31)
+    Ws, bs = _net(rng, [2, 5, 3], scale=2.0)
+    a0 = rng.standard_normal(2) * 0.3
+    sig = rng.uniform(0.2, 0.6, 2)
+    mu = np.array([0.5, -0.7]) * sig * 2
+    c = a0 + mu
+    # vertices of the arrangement inside the offset box, remainder measured about a0
+    planes = [(Ws[0][k], -bs[0][k]) for k in range(5)]
+    for i in range(2):
+        e = np.zeros(2); e[i] = 1.0
+        planes += [(e, c[i] - sig[i]), (e, c[i] + sig[i])]
+    pts = []
+    for i, j in itertools.combinations(range(len(planes)), 2):
+        A = np.array([planes[i][0], planes[j][0]]); rhs = np.array([planes[i][1], planes[j][1]])
+        if abs(np.linalg.det(A)) < 1e-12:
+            continue
+        x = np.linalg.solve(A, rhs)
+        if np.all(np.abs(x - c) <= sig + 1e-12):
+            pts.append(np.clip(x, c - sig, c + sig))
+    R = _true_r(Ws, bs, O.ACT_RELU, a0, np.array(pts))
+    out = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig, mu=mu)
+    assert np.all(out["r_lo"] <= R.min(0) + 1e-12) and np.all(out["r_hi"] >= R.max(0) - 1e-12)
+    assert np.all((out["r_hi"] - out["r_lo"]) <= 8.0 * (R.max(0) - R.min(0)) + 1e-9)
+
+
+@pytest.mark.parametrize("act,dims,seed,hidden", [(O.ACT_TANH, [6, 10, 10, 10, 4], 1, "crown"), (O.ACT_RELU, [6, 10, 10, 10, 4], 0, "crown"),
+                                                  (O.ACT_TANH, [5, 8, 8, 8, 8, 3], 3, "ibp")])
+def test_mu_vjp_matches_central_differences(act, dims, seed, hidden):
+    rng = np.random.default_rng(700 + seed)
+    Ws, bs = _net(rng, dims, scale=1.5)
+    N = dims[0]
+    a0 = rng.standard_normal(N)
+    sig = rng.uniform(0.05, 0.3, N)
+    mu = sig * rng.uniform(-1.5, 1.5, N)
+    g_lo, g_hi = rng.standard_normal(dims[-1]), rng.standard_normal(dims[-1])
+    gn, gr, gm = O.crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, hidden=hidden, mu=mu)
+    g = np.concatenate([gn, gr, gm])
+
+    def F(a, s, m):
+        f = O.crown_forward(Ws, bs, act, a, s, hidden=hidden, mu=m)
+        return g_hi @ f["r_hi"] + g_lo @ f["r_lo"]
+    h, ok = 1e-6, 0
+    F0 = F(a0, sig, mu)
+    scale = np.abs(g).max()
+    for i in range(3 * N):
+        e = np.zeros(N)
+        e[i % N] = h
+        args = [(a0 + e, sig, mu), (a0 - e, sig, mu)] if i < N else [(a0, sig + e, mu), (a0, sig - e, mu)] if i < 2 * N else \
+               [(a0, sig, mu + e), (a0, sig, mu - e)]
+        fp, fm = F(*args[0]), F(*args[1])
+        if abs((fp - F0) - (F0 - fm)) > 1e-3 * abs(fp - fm) + 1e-12:
+            continue
+        assert abs((fp - fm) / (2 * h) - g[i]) <= 1e-6 * scale + 1e-5 * abs(g[i]), i
+        ok += 1
+    assert ok >= 2 * N
