@@ -51,7 +51,7 @@ typedef enum {
     LEB_ERR_SHAPE = 2,       /* ld too small, model/shape mismatch */
     LEB_ERR_ALIGN = 3,       /* pointer not 4-byte aligned */
     LEB_ERR_DOMAIN = 4,      /* reported by leb_domain_flag(): some tile hit a domain error */
-    LEB_ERR_UNSUPPORTED = 5, /* NN path with mu != NULL (non-centred boxes), unknown model, certified mode wider than 2048 */
+    LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048, with mu != NULL or with CROWN-IBP */
     LEB_ERR_CUDA = 6,
     LEB_ERR_NOMEM = 7,
     LEB_ERR_STATE = 8        /* model not set before the call that needs it */
@@ -166,6 +166,10 @@ leb_status leb_analytic_pgd(leb_ctx* ctx, int B, int T, const float* centre, con
                             int steps, float lr, float* nom, float* width0, float* width, unsigned flags, void* stream);
 
 /* CROWN + Thm 3 bound, eq. (18)-(21) L196-220, for every tile.
+ *   mu     : NULL (centred box) or [B, T, ld_in]: the box is a~ + mu + [-sigma, sigma] (25a) L272; the CROWN bounds are
+ *            taken on that box, p(a~) and J(a~) stay at the nominal point, and (21) maximises the affine bound (20) over
+ *            the box (in the kernels' deviation form: a - a~ in mu -+ sigma).  Value mode only: with mu != NULL and
+ *            without LEB_FLAG_NO_MARGIN the call returns LEB_ERR_UNSUPPORTED.
  *   J      : NULL => the network's own Jacobian at a~ (eq. (7)); otherwise [B, T, n, N]
  *            dense, and the bound is with respect to that matrix (Thm 3 holds for any J).
  *   margin : NULL or [B, T, ld_out].  Certified mode: the outward pad contained in r_lo / r_hi of the entry (the
@@ -194,7 +198,7 @@ leb_status leb_vjp(leb_ctx* ctx, int kind, int B, int T, const float* nom, const
 
 /* leb_vjp for non-centred boxes: the same, with the box offsets mu [B, T, ld_in] as a third argument of the bound and
  * its gradient grad_mu [B, T, ld_in] as a third output (grad_mu may be NULL).  mu == NULL: identical to leb_vjp.
- * kind 1 (NN) with mu != NULL: LEB_ERR_UNSUPPORTED (the NN path takes centred boxes only). */
+ * Both kinds (kind 1: the gradient of the value-mode bound). */
 leb_status leb_vjp_mu(leb_ctx* ctx, int kind, int B, int T, const float* nom, const float* rad, const float* mu,
                       const float* g_lo, const float* g_hi, int ld_in, int ld_out, float* grad_nom,
                       float* grad_rad, float* grad_mu, unsigned flags, void* stream);

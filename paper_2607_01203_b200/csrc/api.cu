@@ -224,13 +224,12 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
                       float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, void* stream) {
     if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
-    if (mu) return LEB_ERR_UNSUPPORTED;
     if (B == 0 || T == 0) return LEB_OK;
     if (!nom || !rad || !r_lo || !r_hi) return LEB_ERR_ARG;
     const int n = leb_nn_n(c->nn), N = leb_nn_N(c->nn);
     leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
     if (s != LEB_OK) return s;
-    if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi) || !al4(J) || !al4(margin)) return LEB_ERR_ALIGN;
+    if (!al4(nom) || !al4(rad) || !al4(mu) || !al4(r_lo) || !al4(r_hi) || !al4(J) || !al4(margin)) return LEB_ERR_ALIGN;
     DeviceGuard guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     const bool host = flags & LEB_FLAG_HOST_IO;
@@ -239,11 +238,12 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
     const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
     const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
     const float* d_J = in_ptr(c, 4, J, tiles * (size_t)n * N, host, st, &ok);
+    const float* d_mu = in_ptr(c, 6, mu, tiles * ld_in, host, st, &ok);
     float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
     float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
     float* d_mg = out_ptr(c, 5, margin, tiles * ld_out, host, &ok);
     if (!ok) return LEB_ERR_NOMEM;
-    s = leb_nn_forward(c->nn, (int)tiles, d_nom, d_rad, d_J, ld_in, d_lo, d_hi, d_mg, ld_out, flags, c->domain_flag, st, &c->launches, &c->prof);
+    s = leb_nn_forward(c->nn, (int)tiles, d_nom, d_rad, d_mu, d_J, ld_in, d_lo, d_hi, d_mg, ld_out, flags, c->domain_flag, st, &c->launches, &c->prof);
     if (s != LEB_OK) return s;
     out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
     out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
@@ -256,7 +256,6 @@ leb_status leb_vjp_mu(leb_ctx* c, int kind, int B, int T, const float* nom, cons
                       void* stream) {
     if (!c || B < 0 || T < 0) return LEB_ERR_ARG;
     if (kind != 0 && kind != 1) return LEB_ERR_ARG;
-    if (kind == 1 && mu) return LEB_ERR_UNSUPPORTED;
     if ((B == 0 || T == 0) && (kind == 0 ? leb_an_ready(c->an) : leb_nn_ready(c->nn))) return LEB_OK;
     if (!nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad) return LEB_ERR_ARG;
     int n, N;
@@ -289,7 +288,7 @@ leb_status leb_vjp_mu(leb_ctx* c, int kind, int B, int T, const float* nom, cons
                        &c->launches, &c->prof);
         if (s != LEB_OK) return s;
     } else {
-        s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, flags, c->domain_flag, st, &c->launches, &c->prof);
+        s = leb_nn_vjp(c->nn, (int)tiles, d_nom, d_rad, d_mu, d_glo, d_ghi, ld_in, ld_out, d_gn, d_gr, d_gm, flags, c->domain_flag, st, &c->launches, &c->prof);
         if (s != LEB_OK) return s;
     }
     out_copy(grad_nom, d_gn, tiles * ld_in, host, st, &ok);

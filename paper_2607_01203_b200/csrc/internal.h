@@ -101,12 +101,12 @@ leb_status leb_nn_set_chunk(NnState*, int tiles);
 bool leb_nn_ready(const NnState*);
 int leb_nn_n(const NnState*);
 int leb_nn_N(const NnState*);
-leb_status leb_nn_forward(NnState*, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
-                          float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
+leb_status leb_nn_forward(NnState*, int tiles, const float* nom, const float* rad, const float* mu, const float* J, int ld_in,
+                          float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
                           long long* launches, LebProf* prof);
-leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
-                      int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
-                      cudaStream_t st, long long* launches, LebProf* prof);
+leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo,
+                      const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags,
+                      int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
 void leb_nn_query(const NnState*, int* tiles, int* certified, int* vjp_reused);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);
 leb_status leb_nn_get_coeffs(NnState*, int target, float* out, cudaStream_t st, long long* launches);

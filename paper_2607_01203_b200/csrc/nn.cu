@@ -54,6 +54,8 @@ struct NnState {
     bool ws_vjp = false;
     std::vector<void*> allocs;
     float *nomp = nullptr, *radp = nullptr, *rad1 = nullptr;
+    float *mup = nullptr, *mu1 = nullptr, *mu_bar = nullptr;   // non-centred boxes: padded mu, W_1 mu, and its adjoint
+    const float* mu_cur = nullptr;                             // = mup while the chunk in flight has box offsets, else NULL
     float *zhat[kMaxLayers] = {nullptr}, *ahat[kMaxLayers] = {nullptr}, *dphi[kMaxLayers] = {nullptr};
     float *lb[kMaxLayers] = {nullptr}, *ub[kMaxLayers] = {nullptr};
     float *kU[kMaxLayers] = {nullptr}, *kL[kMaxLayers] = {nullptr}, *gU[kMaxLayers] = {nullptr}, *gL[kMaxLayers] = {nullptr};
@@ -74,6 +76,7 @@ struct NnState {
     bool last_with_jac = false;  // ... including the Jacobian chain rows (needed by the reverse sweep)
     bool last_cert = false;      // ... computed in certified mode (widened hidden bounds, padded gaps)
     bool last_ibp = false;       // ... with hidden-layer bounds by interval propagation (LEB_FLAG_IBP_HIDDEN)
+    bool last_mu = false;        // ... on non-centred boxes (mu != NULL)
     bool last_vjp_reused = false;   // the last leb_vjp(kind 1) started from the resident forward state
     LebProf* prof = nullptr;
 };
@@ -99,7 +102,8 @@ __global__ void pack_matrix_kernel(const float* __restrict__ src, int rows, int 
 
 // nom/rad [tiles x ld_in] -> zero-padded [tiles x wp0]; invalid input (NaN/Inf, sigma < 0) poisons the tile with NaN
 __global__ void pad_inputs_kernel(int tiles, int N, int ld_in, int wp0, const float* __restrict__ nom, const float* __restrict__ rad,
-                                  float* __restrict__ nomp, float* __restrict__ radp) {
+                                  float* __restrict__ nomp, float* __restrict__ radp, const float* __restrict__ mu = nullptr,
+                                  float* __restrict__ mup = nullptr) {
     size_t total = (size_t)tiles * wp0;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int t = (int)(q / wp0), c = (int)(q - (size_t)t * wp0);
@@ -112,6 +116,11 @@ __global__ void pad_inputs_kernel(int tiles, int N, int ld_in, int wp0, const fl
         }
         nomp[q] = a;
         radp[q] = s;
+        if (mup) {
+            float m = (c < N) ? mu[(size_t)t * ld_in + c] : 0.f;
+            if (!(fabsf(m) <= 3.0e38f)) m = NAN;
+            mup[q] = m;
+        }
     }
 }
 
@@ -141,7 +150,8 @@ __global__ void split_tf32_kernel(const float* __restrict__ src, float* __restri
 // per-neuron relaxation of layer l from (zhat, l, u); for layer 1 (rad1 != NULL) first l,u = zhat -+ rad1 (N2)
 __global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat,
                                  const float* __restrict__ rad1, float* __restrict__ lb, float* __restrict__ ub,
-                                 float* __restrict__ kU, float* __restrict__ kL, float* __restrict__ gU, float* __restrict__ gL) {
+                                 float* __restrict__ kU, float* __restrict__ kL, float* __restrict__ gU, float* __restrict__ gL,
+                                 const float* __restrict__ mu1 = nullptr) {
     size_t total = (size_t)tiles * wp;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int c = (int)(q % wp);
@@ -150,7 +160,10 @@ __global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const 
             continue;
         }
         float z = zhat[q], l, u;
-        if (rad1) { float r = rad1[q]; l = z - r; u = z + r; lb[q] = l; ub[q] = u; }
+        if (rad1) {     // layer 1: z_1 - zhat_1 = W_1 (a - a~) in W_1 mu -+ |W_1| sigma   (mu1 = W_1 mu, non-centred boxes)
+            const float r = rad1[q], m = mu1 ? mu1[q] : 0.f;
+            l = z + (m - r); u = z + (m + r); lb[q] = l; ub[q] = u;
+        }
         else { l = lb[q]; u = ub[q]; }
         Relax r = relax_any(act, (double)l, (double)u);
         double f = act_f(act, (double)z);
@@ -324,7 +337,8 @@ __global__ void row_margin_kernel(int tiles, int rows_pad, int rows_kind, int K,
 __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
                                          const float* __restrict__ sigma, const float* __restrict__ gap,
                                          const float* __restrict__ zhat, float* __restrict__ lb, float* __restrict__ ub,
-                                         const float* __restrict__ e_s, float kap_sum, float kap_gap) {
+                                         const float* __restrict__ e_s, float kap_sum, float kap_gap,
+                                         const float* __restrict__ mu = nullptr) {
     int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     int total = tiles * rows_kind;
     if (warp >= total) return;
@@ -332,15 +346,23 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
     const float* up = Lam0 + ((size_t)t * rows_pad + k) * wp0;
     const float* lo = Lam0 + ((size_t)t * rows_pad + rows_kind + k) * wp0;
     const float* sg = sigma + (size_t)t * wp0;
-    float su = 0.f, sl = 0.f;
+    float su = 0.f, sl = 0.f, du = 0.f, dl = 0.f;        // du, dl: Lam_0 mu (non-centred boxes: a - a~ in mu -+ sigma)
     for (int j = lane * 4; j < wp0; j += 128) {
         float4 a = *reinterpret_cast<const float4*>(up + j), b = *reinterpret_cast<const float4*>(lo + j);
         float4 s = *reinterpret_cast<const float4*>(sg + j);
         su += fabsf(a.x) * s.x + fabsf(a.y) * s.y + fabsf(a.z) * s.z + fabsf(a.w) * s.w;
         sl += fabsf(b.x) * s.x + fabsf(b.y) * s.y + fabsf(b.z) * s.z + fabsf(b.w) * s.w;
+        if (mu) {
+            float4 m = *reinterpret_cast<const float4*>(mu + (size_t)t * wp0 + j);
+            du += a.x * m.x + a.y * m.y + a.z * m.z + a.w * m.w;
+            dl += b.x * m.x + b.y * m.y + b.z * m.z + b.w * m.w;
+        }
     }
 #pragma unroll
-    for (int off = 16; off; off >>= 1) { su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off); }
+    for (int off = 16; off; off >>= 1) {
+        su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off);
+        du += __shfl_xor_sync(0xffffffffu, du, off); dl += __shfl_xor_sync(0xffffffffu, dl, off);
+    }
     if (lane == 0) {
         float z = zhat[(size_t)t * rows_kind + k];
         const float gu = gap[(size_t)t * rows_pad + k], gl = gap[(size_t)t * rows_pad + rows_kind + k];
@@ -351,8 +373,8 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
             ub[(size_t)t * rows_kind + k] = __fadd_ru(z, pu);
             lb[(size_t)t * rows_kind + k] = __fadd_rd(z, -pl);
         } else {
-            ub[(size_t)t * rows_kind + k] = z + (su + gu);
-            lb[(size_t)t * rows_kind + k] = z - (sl - gl);
+            ub[(size_t)t * rows_kind + k] = z + ((su + du) + gu);
+            lb[(size_t)t * rows_kind + k] = z - ((sl - dl) - gl);
         }
     }
 }
@@ -363,7 +385,7 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
                                       const float* __restrict__ Jgiven, float* __restrict__ r_lo, float* __restrict__ r_hi,
                                       int ld_out, int* __restrict__ domain_flag, int cert, const float* __restrict__ marg,
                                       const float* __restrict__ eta, int ld_eta, float kap_sum, float kap_gap,
-                                      float* __restrict__ margin_out) {
+                                      float* __restrict__ margin_out, const float* __restrict__ mu = nullptr) {
     int warp = (int)(((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     int total = tiles * n;
     if (warp >= total) return;
@@ -371,13 +393,15 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
     const float* up = Lam0 + ((size_t)t * rows_pad + i) * wp0;
     const float* lo = Lam0 + ((size_t)t * rows_pad + n + i) * wp0;
     const float* sg = sigma + (size_t)t * wp0;
-    float su = 0.f, sl = 0.f;
+    float su = 0.f, sl = 0.f, du = 0.f, dl = 0.f;        // du, dl: (Lam_0 - J) mu   (non-centred boxes)
+    const float* mt = mu ? mu + (size_t)t * wp0 : nullptr;
     if (Jgiven) {
         const float* Jr = Jgiven + ((size_t)t * n + i) * N;
         for (int j = lane; j < N; j += 32) {
             float jv = Jr[j], s = sg[j];
             su += fabsf(up[j] - jv) * s;
             sl += fabsf(lo[j] - jv) * s;
+            if (mt) { du += (up[j] - jv) * mt[j]; dl += (lo[j] - jv) * mt[j]; }
         }
     } else {
         const float* Jr = Lam0 + ((size_t)t * rows_pad + 2 * n + i) * wp0;
@@ -386,13 +410,21 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
             float4 c = *reinterpret_cast<const float4*>(Jr + j), s = *reinterpret_cast<const float4*>(sg + j);
             su += fabsf(a.x - c.x) * s.x + fabsf(a.y - c.y) * s.y + fabsf(a.z - c.z) * s.z + fabsf(a.w - c.w) * s.w;
             sl += fabsf(b.x - c.x) * s.x + fabsf(b.y - c.y) * s.y + fabsf(b.z - c.z) * s.z + fabsf(b.w - c.w) * s.w;
+            if (mt) {
+                float4 m = *reinterpret_cast<const float4*>(mt + j);
+                du += (a.x - c.x) * m.x + (a.y - c.y) * m.y + (a.z - c.z) * m.z + (a.w - c.w) * m.w;
+                dl += (b.x - c.x) * m.x + (b.y - c.y) * m.y + (b.z - c.z) * m.z + (b.w - c.w) * m.w;
+            }
         }
     }
 #pragma unroll
-    for (int off = 16; off; off >>= 1) { su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off); }
+    for (int off = 16; off; off >>= 1) {
+        su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off);
+        du += __shfl_xor_sync(0xffffffffu, du, off); dl += __shfl_xor_sync(0xffffffffu, dl, off);
+    }
     if (lane == 0) {
-        float hi = su + gap[(size_t)t * rows_pad + i];
-        float lo_v = -sl + gap[(size_t)t * rows_pad + n + i];
+        float hi = (su + du) + gap[(size_t)t * rows_pad + i];
+        float lo_v = (dl - sl) + gap[(size_t)t * rows_pad + n + i];
         float mg = 0.f;
         if (cert) {
             // certified mode: outward-rounded terms (the gap sums carry the chain steps' pads) + eta (the exact nominal
@@ -425,7 +457,8 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
 //   rad_bar_j += sum_rows |.| weights;  gapbar[up] = ybar_up, gapbar[lo] = ybar_lo
 __global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
                             const float* __restrict__ sigma, const float* __restrict__ ybar_up, const float* __restrict__ ybar_lo,
-                            int ldy, float* __restrict__ Lbar0, float* __restrict__ gapbar, float* __restrict__ rad_bar) {
+                            int ldy, float* __restrict__ Lbar0, float* __restrict__ gapbar, float* __restrict__ rad_bar,
+                            const float* __restrict__ mu = nullptr, float* __restrict__ mu_bar = nullptr) {
     // grid (tiles, ceil(rows_kind / 32)): a block takes 32 bound indices k of one tile; thread j owns input column j
     const int t = blockIdx.x, k0 = blockIdx.y * 32, k1 = min(k0 + 32, rows_kind);
     const float* base = Lam0 + (size_t)t * rows_pad * wp0;
@@ -438,20 +471,23 @@ __global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, co
         for (int r = 2 * rows_kind + threadIdx.x; r < rows_pad; r += blockDim.x) gapbar[(size_t)t * rows_pad + r] = 0.f;
     for (int j = threadIdx.x; j < wp0; j += blockDim.x) {
         const float s = sigma[(size_t)t * wp0 + j];
-        float sb = 0.f;
+        const float m = mu ? mu[(size_t)t * wp0 + j] : 0.f;      // non-centred boxes: y = Lam mu +- |Lam| sigma + gap
+        float sb = 0.f, mb = 0.f;
 #pragma unroll 4
         for (int k = k0; k < k1; ++k) {
             const float yu = ybar_up[(size_t)t * ldy + k], yl = ybar_lo[(size_t)t * ldy + k];
             float a = base[(size_t)k * wp0 + j], b = base[(size_t)(rows_kind + k) * wp0 + j];
             if (is_out) { float jv = base[(size_t)(2 * rows_kind + k) * wp0 + j]; a -= jv; b -= jv; }
             const float sa = (a > 0.f) - (a < 0.f), sbn = (b > 0.f) - (b < 0.f);
-            const float lu = yu * sa * s, ll = -yl * sbn * s;
+            const float lu = yu * (sa * s + m), ll = yl * (m - sbn * s);
             obase[(size_t)k * wp0 + j] = lu;
             obase[(size_t)(rows_kind + k) * wp0 + j] = ll;
             if (is_out) obase[(size_t)(2 * rows_kind + k) * wp0 + j] = -(lu + ll);
             sb += yu * fabsf(a) - yl * fabsf(b);
+            mb += yu * a + yl * b;
         }
         atomicAdd(&rad_bar[(size_t)t * wp0 + j], sb);
+        if (mu_bar) atomicAdd(&mu_bar[(size_t)t * wp0 + j], mb);
     }
 }
 
@@ -557,13 +593,20 @@ __global__ void diff_kernel(const float* __restrict__ ubar, const float* __restr
         out[q] = ubar[q] - lbar[q];
 }
 
+__global__ void sum_kernel(const float* __restrict__ a, const float* __restrict__ b, float* __restrict__ out, size_t count) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x)
+        out[q] = a[q] + b[q];
+}
+
 __global__ void write_grads_kernel(int tiles, int N, int wp0, int ld_in, const float* __restrict__ nom_bar,
-                                   const float* __restrict__ rad_bar, float* __restrict__ grad_nom, float* __restrict__ grad_rad) {
+                                   const float* __restrict__ rad_bar, float* __restrict__ grad_nom, float* __restrict__ grad_rad,
+                                   const float* __restrict__ mu_bar = nullptr, float* __restrict__ grad_mu = nullptr) {
     size_t total = (size_t)tiles * N;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int t = (int)(q / N), c = (int)(q - (size_t)t * N);
         grad_nom[(size_t)t * ld_in + c] = nom_bar[(size_t)t * wp0 + c];
         grad_rad[(size_t)t * ld_in + c] = rad_bar[(size_t)t * wp0 + c];
+        if (grad_mu) grad_mu[(size_t)t * ld_in + c] = mu_bar[(size_t)t * wp0 + c];
     }
 }
 
@@ -633,7 +676,7 @@ void ws_free(NnState* S) {
 }
 
 size_t bytes_per_tile(const NnState* S, bool vjp) {
-    size_t f = 3 * (size_t)S->wp[0];
+    size_t f = 5 * (size_t)S->wp[0] + (size_t)S->wp[1];
     for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 23 : 15);
     size_t maxLam = 0;
     for (int s = 2; s <= S->L; ++s) {
@@ -676,6 +719,9 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
     S->nomp = F((size_t)C * S->wp[0]);
     S->radp = F((size_t)C * S->wp[0]);
     S->rad1 = F((size_t)C * S->wp[1]);
+    S->mup = F((size_t)C * S->wp[0]);
+    S->mu1 = F((size_t)C * S->wp[1]);
+    S->mu_bar = F((size_t)C * S->wp[0]);
     for (int l = 1; l < L; ++l) {
         size_t c = (size_t)C * S->wp[l];
         S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
@@ -755,8 +801,13 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
     } else {
         GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
         launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g, st, launches);
+        if (S->mu_cur) {      // non-centred boxes: the centre of z_1 - zhat_1 is W_1 mu
+            GemmArgs gm = plain_args(C, S->wp[1], S->wp[0], S->mu_cur, S->wp[0], S->Wt[1], S->wp[1], S->mu1, S->wp[1]);
+            launch_gemm<AMODE_PLAIN, EPI_STORE>(S, gm, st, launches);
+        }
         relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->rad1, S->lb[1],
-                                                                      S->ub[1], S->kU[1], S->kL[1], S->gU[1], S->gL[1]);
+                                                                      S->ub[1], S->kU[1], S->kL[1], S->gU[1], S->gL[1],
+                                                                      S->mu_cur ? S->mu1 : nullptr);
         ++*launches;
     }
     // ---- N3 / N4: targets s = 2 .. L
@@ -814,7 +865,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
             size_t warps = (size_t)C * rk;
             concretise_hidden_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(
                 C, rp, rk, S->wp[0], S->Lam[s][0], S->radp, S->gap[s], S->zhat[s], S->lb[s], S->ub[s], cert ? S->ce[s] : nullptr,
-                kap_sum, kap_gap);
+                kap_sum, kap_gap, S->mu_cur);
             ++*launches;
             if (cert) {
                 relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(
@@ -964,8 +1015,8 @@ leb_status leb_nn_set_mlp(NnState* S, const leb_mlp* m, cudaStream_t st, long lo
 // ------------------------------------------------------------------------------------------
 // forward
 // ------------------------------------------------------------------------------------------
-leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* rad, const float* J, int ld_in, float* r_lo,
-                          float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
+leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* rad, const float* mu, const float* J, int ld_in,
+                          float* r_lo, float* r_hi, float* margin, int ld_out, unsigned flags, int* domain_flag, cudaStream_t st,
                           long long* launches, LebProf* prof) {
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
@@ -973,6 +1024,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
     if (ibp && cert) return LEB_ERR_UNSUPPORTED;                       // the rounding bookkeeping covers the back-substituted hidden bounds only
+    if (mu && cert) return LEB_ERR_UNSUPPORTED;                        // ... and centred boxes only
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
     if (tiles == 0) return LEB_OK;
@@ -982,8 +1034,10 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
         pad_inputs_kernel<<<gs_grid((size_t)C * S->wp[0]), 256, 0, st>>>(C, N, ld_in, S->wp[0], nom + (size_t)t0 * ld_in,
-                                                                       rad + (size_t)t0 * ld_in, S->nomp, S->radp);
+                                                                       rad + (size_t)t0 * ld_in, S->nomp, S->radp,
+                                                                       mu ? mu + (size_t)t0 * ld_in : nullptr, mu ? S->mup : nullptr);
         ++*launches;
+        S->mu_cur = mu ? S->mup : nullptr;
         forward_chunk(S, C, J, J == nullptr, cert, cert && margin != nullptr, st, launches, ibp);
         size_t warps = (size_t)C * n;
         const int ks = [&] { int k = 0; for (int l = 1; l < L; ++l) k += S->wp[l]; return k; }();
@@ -991,12 +1045,13 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
             C, S->rows_pad[L], n, N, S->wp[0], S->Lam[L][0], S->radp, S->gap[L], J ? J + (size_t)t0 * n * N : nullptr,
             r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out, ld_out, domain_flag, cert ? 1 : 0, S->marg, S->eta, S->wp[L],
             1.f + (float)(S->wp[0] + 8) * 1.1920929e-07f, 1.f + (float)(ks + 64) * 1.1920929e-07f,
-            margin ? margin + (size_t)t0 * ld_out : nullptr);     // value mode: no margin is added, 0 is reported
+            margin ? margin + (size_t)t0 * ld_out : nullptr, S->mu_cur);     // value mode: no margin is added, 0 is reported
         ++*launches;
         S->last_tiles = (tiles <= S->chunk) ? C : 0;
         S->last_with_jac = (J == nullptr);
         S->last_cert = cert;
         S->last_ibp = ibp;
+        S->last_mu = (mu != nullptr);
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
@@ -1028,9 +1083,9 @@ leb_status leb_nn_get_coeffs(NnState* S, int target, float* out, cudaStream_t st
 // ------------------------------------------------------------------------------------------
 // VJP: forward of the chunk (all coefficient blocks kept), then the reverse sweep
 // ------------------------------------------------------------------------------------------
-leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad, const float* g_lo, const float* g_hi,
-                      int ld_in, int ld_out, float* grad_nom, float* grad_rad, unsigned flags, int* domain_flag,
-                      cudaStream_t st, long long* launches, LebProf* prof) {
+leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo,
+                      const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags,
+                      int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
     (void)domain_flag;
     S->prof = prof;
     S->use_tc = !(flags & LEB_FLAG_FFMA_ONLY);
@@ -1043,15 +1098,17 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
     // and was computed in the mode this call names (LEB_FLAG_NO_MARGIN: a value-mode state; otherwise a certified one).
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
-    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp;
+    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp && !mu;
     const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
-                       S->last_cert == want_cert && S->last_ibp == ibp;
+                       S->last_cert == want_cert && S->last_ibp == ibp && S->last_mu == (mu != nullptr);
     S->last_vjp_reused = reuse;
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
         if (!reuse)
             pad_inputs_kernel<<<gs_grid((size_t)C * wp0), 256, 0, st>>>(C, N, ld_in, wp0, nom + (size_t)t0 * ld_in,
-                                                                      rad + (size_t)t0 * ld_in, S->nomp, S->radp);
+                                                                      rad + (size_t)t0 * ld_in, S->nomp, S->radp,
+                                                                      mu ? mu + (size_t)t0 * ld_in : nullptr, mu ? S->mup : nullptr);
+        S->mu_cur = mu ? S->mup : nullptr;
         pad_cotangent_kernel<<<gs_grid((size_t)C * n), 256, 0, st>>>(C, n, ld_out, g_lo + (size_t)t0 * ld_out,
                                                                    g_hi + (size_t)t0 * ld_out, S->glo_p, S->ghi_p);
         *launches += 2;
@@ -1066,6 +1123,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         }
         cudaMemsetAsync(S->nom_bar, 0, (size_t)C * wp0 * 4, st);
         cudaMemsetAsync(S->rad_bar, 0, (size_t)C * wp0 * 4, st);
+        if (mu) cudaMemsetAsync(S->mu_bar, 0, (size_t)C * wp0 * 4, st);
         // ---- targets s = L .. 2
         for (int s = L; s >= 2; --s) {
             const bool is_out = (s == L);
@@ -1093,7 +1151,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
             const float* yu = is_out ? S->ghi_p : S->ubar[s];
             const float* yl = is_out ? S->glo_p : S->lbar[s];
             seed_kernel<<<dim3(C, (rk + 31) / 32), 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
-                                           S->Lbar[0], S->gapbar, S->rad_bar);
+                                           S->Lbar[0], S->gapbar, S->rad_bar, S->mu_cur, mu ? S->mu_bar : nullptr);
             ++*launches;
             int cur = 0;
             for (int l = 1; l <= s - 1; ++l) {
@@ -1135,6 +1193,12 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         }
         diff_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->ubar[1], S->lbar[1], S->rad1, (size_t)C * S->wp[1]);
         *launches += 2;
+        if (mu) {     // l_1, u_1 = zhat_1 + W_1 mu -+ |W_1| sigma: mu_bar += W_1^T (l_bar_1 + u_bar_1)
+            sum_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->ubar[1], S->lbar[1], S->mu1, (size_t)C * S->wp[1]);
+            ++*launches;
+            GemmArgs g = plain_args(C, wp0, S->wp[1], S->mu1, S->wp[1], S->W[1], wp0, S->mu_bar, wp0);
+            launch_gemm<AMODE_PLAIN, EPI_ACC>(S, g, st, launches);
+        }
         {
             GemmArgs g = plain_args(C, wp0, S->wp[1], S->rad1, S->wp[1], S->Wabs1, wp0, S->rad_bar, wp0);
             launch_gemm<AMODE_PLAIN, EPI_ACC>(S, g, st, launches);
@@ -1151,9 +1215,10 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
             }
         }
         write_grads_kernel<<<gs_grid((size_t)C * N), 256, 0, st>>>(C, N, wp0, ld_in, S->nom_bar, S->rad_bar,
-                                                                 grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in);
+                                                                 grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in,
+                                                                 mu ? S->mu_bar : nullptr, (mu && grad_mu) ? grad_mu + (size_t)t0 * ld_in : nullptr);
         ++*launches;
-        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; }   // a value-mode forward state
+        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; S->last_mu = (mu != nullptr); }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;

@@ -203,16 +203,16 @@ class Context:
                                        _ptr(nom), _ptr(w0), _ptr(w), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_pgd")
         return nom, w0, w
 
-    def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = 0):
+    def leb_nn_fwd(self, nom, rad, J=None, r_lo=None, r_hi=None, margin=None, flags: int = 0, mu=None):
         """flags = 0 is the C ABI's default: CERTIFIED mode (rounding errors bounded and added outward).
         FLAG_NO_MARGIN selects value mode, the plain FP32 result the parity tests compare with the oracle."""
-        _check_f32(nom, rad, J, r_lo, r_hi, margin)
+        _check_f32(nom, rad, J, r_lo, r_hi, margin, mu)
         B, T, ld_in = self._bt(nom)
         host = bool(flags & FLAG_HOST_IO)
         if r_lo is None:
             r_lo = self._out(nom, (B, T, self.nn_n), host)
             r_hi = self._out(nom, (B, T, self.nn_n), host)
-        _chk(self.lib.leb_nn_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), None, _ptr(J), ld_in, _ptr(r_lo), _ptr(r_hi),
+        _chk(self.lib.leb_nn_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), _ptr(J), ld_in, _ptr(r_lo), _ptr(r_hi),
                                  _ptr(margin), int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_nn_fwd")
         return r_lo, r_hi
 

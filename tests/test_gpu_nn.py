@@ -405,3 +405,91 @@ def test_crown_ibp_configs_sampled_tiles(mods, cfg, tiles):
     print(f"config {cfg}: CROWN-IBP enclosure width / full CROWN = {wide:.3f}")
     assert wide >= 1.0 - 1e-6
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- non-centred boxes (25a) L272
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_mu_small_nets_match_oracle(mods, dims, act, path):
+    """mu != NULL on the NN path: forward, hidden bounds and the VJP with respect to (a~, sigma, mu) against the oracle;
+    some |mu_j| > sigma_j (the nominal point outside the box).  Full CROWN and CROWN-IBP hidden bounds."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    mu = wl.make_mu(w, 1.5)
+    assert (np.abs(mu) > w.rad).any()
+    ctx = leb.context_for_workload(w)
+    nom, rad, g_lo, g_hi = _flat(w)
+    mu_f = mu.reshape(-1, w.N)
+    for hidden, extra in (("crown", 0), ("ibp", IBP)):
+        flags = PATHS[path] | extra
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=flags, mu=_dev(mu))
+        assert ctx.leb_domain_flag() == 0
+        olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, hidden=hidden, mu=mu_f)
+        assert_bounds_close(to_np(lo).reshape(-1, w.n), olo, f"mu {hidden} {dims} r_lo")
+        assert_bounds_close(to_np(hi).reshape(-1, w.n), ohi, f"mu {hidden} {dims} r_hi")
+        gn, gr, gm = ctx.leb_vjp_mu(1, _dev(w.nom), _dev(w.rad), _dev(mu), _dev(w.g_lo), _dev(w.g_hi), flags=flags)
+        ogn, ogr, ogm = O.leb_nn_vjp(w.mlp.W, w.mlp.b, act, nom, rad, g_lo, g_hi, hidden=hidden, mu=mu_f)
+        S = np.maximum(np.maximum(np.abs(ogn).max(1), np.abs(ogr).max(1)), np.abs(ogm).max(1))
+        from parity_util import assert_grad_dirs_close, GRAD_NORMWISE, report
+        for name, got, ref in (("grad_nom", gn, ogn), ("grad_rad", gr, ogr), ("grad_mu", gm, ogm)):
+            err = np.abs(to_np(got).reshape(ref.shape) - ref)
+            tol = 1e-4 * np.abs(ref) + GRAD_NORMWISE * S[:, None] + 1e-12
+            report(f"mu {hidden} {dims} {name}", (err / tol).max())
+            assert (err <= tol).all(), (name, float((err / tol).max()))
+        # from the resident forward state
+        ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=flags, mu=_dev(mu))
+        g2 = ctx.leb_vjp_mu(1, _dev(w.nom), _dev(w.rad), _dev(mu), _dev(w.g_lo), _dev(w.g_hi), flags=flags | leb.FLAG_REUSE_FWD)
+        assert ctx.leb_nn_state()[2] is True
+        for a, b in zip(g2, (gn, gr, gm)):
+            assert float((a - b).abs().max()) <= 1e-5 * float(b.abs().max())
+    # mu = 0 is the centred bound (bit for bit: the extra terms are exact zeros); the certified mode refuses mu
+    z = torch.zeros_like(_dev(mu))
+    lo0, hi0 = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path], mu=z)
+    lo1, hi1 = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+    assert torch.equal(lo0, lo1) and torch.equal(hi0, hi1)
+    with pytest.raises(leb.LebError) as e:
+        ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path] & ~1, mu=_dev(mu))
+    assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+    ctx.close()
+
+
+def test_mu_config5_sampled_tiles_and_soundness(mods):
+    leb, wl, O = mods
+    w = wl.make_config(5)
+    mu = wl.make_mu(w, 1.5)
+    ctx = leb.context_for_workload(w)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=VAL, mu=_dev(mu))
+    gn, gr, gm = ctx.leb_vjp_mu(1, _dev(w.nom), _dev(w.rad), _dev(mu), _dev(w.g_lo), _dev(w.g_hi), flags=VAL | leb.FLAG_REUSE_FWD)
+    nom, rad, g_lo, g_hi = _flat(w)
+    mu_f = mu.reshape(-1, w.N)
+    idx = np.array([0, 1500, 3777, w.B * w.T - 1])
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx], rad[idx], mu=mu_f[idx])
+    assert_bounds_close(to_np(lo).reshape(-1, w.n)[idx], olo, "cfg5 mu r_lo")
+    assert_bounds_close(to_np(hi).reshape(-1, w.n)[idx], ohi, "cfg5 mu r_hi")
+    ogn, ogr, ogm = O.leb_nn_vjp(w.mlp.W, w.mlp.b, w.mlp.act, nom[idx[:2]], rad[idx[:2]], g_lo[idx[:2]], g_hi[idx[:2]], mu=mu_f[idx[:2]])
+    from parity_util import GRAD_NORMWISE
+    S = np.maximum(np.maximum(np.abs(ogn).max(1), np.abs(ogr).max(1)), np.abs(ogm).max(1))[:, None]
+    for got, ref in ((gn, ogn), (gr, ogr), (gm, ogm)):
+        err = np.abs(to_np(got).reshape(-1, w.N)[idx[:2]] - ref)
+        assert (err <= 1e-4 * np.abs(ref) + GRAD_NORMWISE * S + 1e-12).mean() > 0.999      # kinks of |W - J| (R20): a handful of entries
+    ctx.close()
+    # soundness where it is sharp: a small tanh net, samples of the offset box and all its vertices
+    ws = wl.make_small_mlp([4, 8, 8, 2], 2, 2, 2, seed=3, rad_lo=0.05, rad_hi=0.4)
+    mus = wl.make_mu(ws, 2.0)
+    c2 = leb.context_for_workload(ws)
+    lo, hi = c2.leb_nn_fwd(_dev(ws.nom), _dev(ws.rad), flags=VAL, mu=_dev(mus))
+    glo, ghi = to_np(lo).reshape(-1, ws.n), to_np(hi).reshape(-1, ws.n)
+    Ws = [np.asarray(x, np.float64) for x in ws.mlp.W]; bs = [np.asarray(x, np.float64) for x in ws.mlp.b]
+    rng = np.random.default_rng(3)
+    verts = np.array(list(itertools.product((-1.0, 1.0), repeat=4)))
+    for t in range(4):
+        a0 = ws.nom.reshape(-1, 4)[t].astype(np.float64); sg = ws.rad.reshape(-1, 4)[t].astype(np.float64)
+        m = mus.reshape(-1, 4)[t].astype(np.float64)
+        X = a0[None] + m[None] + np.concatenate([rng.uniform(-1, 1, (100000, 4)), verts]) * sg[None]
+        zs, p, J = O.nominal(Ws, bs, 2, a0)
+        A = X.T
+        for l in range(len(Ws) - 1):
+            A = O.phi(2, Ws[l] @ A + bs[l][:, None])
+        r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ J.T
+        assert np.all(r.max(0) <= ghi[t] + 1e-5 * np.abs(ghi[t]) + 1e-7) and np.all(r.min(0) >= glo[t] - 1e-5 * np.abs(glo[t]) - 1e-7)
+    c2.close()
