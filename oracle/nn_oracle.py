@@ -157,14 +157,20 @@ def relax_tanh_scalar(l, u):
     return kU, bU, kL, bL, ("mixed", dU, dL)
 
 
-def relax(act, l, u):
-    """Vector version: arrays kU, bU, kL, bL and the per-neuron aux list."""
+def relax(act, l, u, alpha=None):
+    """Vector version: arrays kU, bU, kL, bL and the per-neuron aux list.
+    alpha (ReLU only): lower slopes of the unstable neurons (l < 0 < u), any value in [0, 1] is a valid lower bound
+    alpha z <= relu(z); None = the adaptive choice of reading R8.  Stable neurons ignore it."""
     f = relax_relu_scalar if act == ACT_RELU else relax_tanh_scalar
     out = [f(float(a), float(b)) for a, b in zip(l, u)]
     kU = np.array([o[0] for o in out])
     bU = np.array([o[1] for o in out])
     kL = np.array([o[2] for o in out])
     bL = np.array([o[3] for o in out])
+    if alpha is not None:
+        assert act == ACT_RELU
+        unstable = np.array([o[4][0] == "unstable" for o in out])
+        kL = np.where(unstable, alpha, kL)
     return kU, bU, kL, bL, [o[4] for o in out]
 
 
@@ -249,7 +255,7 @@ def ibp_layer(W, b, act, l_prev, u_prev):
     return Wp @ a_lo + Wn @ a_hi + b, Wp @ a_hi + Wn @ a_lo + b
 
 
-def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown", mu=None):
+def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown", mu=None, alphas=None):
     """CROWN + Thm 3 for one tile.  Returns dict with r_lo, r_hi, the hidden
     bounds (ls, us), the output affine bounds (W_up, b_up, W_lo, b_lo), J and p.
 
@@ -260,7 +266,11 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"
 
     mu: non-centred box (25a) PAPER.md:L272: the CROWN bounds are taken on the box c + [-sig, sig], c = a0 + mu, while
     p(a~) and J(a~) of the remainder (10) stay at the nominal point a0; Thm 3's maximisation (21) of the affine r_up(a)
-    = (W_up - J) a + J a~ - p(a~) + b_up (20) then runs over that box.  (Thm 2 / Thm 3 need no a~ in the box.)"""
+    = (W_up - J) a + J a~ - p(a~) + b_up (20) then runs over that box.  (Thm 2 / Thm 3 need no a~ in the box.)
+
+    alphas (ReLU): per hidden layer, the lower slopes of the unstable neurons (see relax); the optimisable-slope variant
+    of CROWN ("alpha-CROWN"): one slope set per tile, shared by every bound of the tile."""
+    al = (lambda k: None) if alphas is None else (lambda k: alphas[k])
     L = len(Ws)
     zs, p, J = nominal(Ws, bs, act, a0)
     if J_given is not None:
@@ -273,20 +283,20 @@ def crown_forward(Ws, bs, act, a0, sig, J_given=None, keep=False, hidden="crown"
     z1c = zs[0] if mu is None else Ws[0] @ c + bs[0]
     ls.append(z1c - A1)
     us.append(z1c + A1)
-    relaxs.append(relax(act, ls[0], us[0]))
+    relaxs.append(relax(act, ls[0], us[0], al(0)))
     # hidden layers s = 2..L-1: full CROWN back-substitution to the input
     for s in range(2, L):
         if hidden == "ibp":
             lo_s, hi_s = ibp_layer(Ws[s - 1], bs[s - 1], act, ls[-1], us[-1])
             ls.append(lo_s)
             us.append(hi_s)
-            relaxs.append(relax(act, ls[-1], us[-1]))
+            relaxs.append(relax(act, ls[-1], us[-1], al(len(ls) - 1)))
             continue
         res = backsub(Ws, bs, relaxs, s, keep=keep)
         Lu, cu, Ll, cl = res[:4]
         us.append(Lu @ c + np.abs(Lu) @ sig + cu)
         ls.append(Ll @ c - np.abs(Ll) @ sig + cl)
-        relaxs.append(relax(act, ls[-1], us[-1]))
+        relaxs.append(relax(act, ls[-1], us[-1], al(len(ls) - 1)))
         if keep:
             kept[s] = res[4:]
     res = backsub(Ws, bs, relaxs, L, keep=keep)
@@ -458,14 +468,14 @@ def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
     return ties
 
 
-def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown", mu=None):
+def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown", mu=None, alphas=None, slope_grads=None):
     """Returns (grad_nom, grad_rad) -- with mu: (grad_nom, grad_rad, grad_mu) -- for one tile; J is the network's own
     Jacobian at a~ (the product's leb_vjp takes no J argument).  `flips`: entries (chain, i, j) from
     output_sign_ties() whose sign(W - J) is negated (the other one-sided gradient at that kink).
     Every bound depends on the box centre c = a~ + mu (adjoint a_bar below, shared by a~ and mu); p(a~), J(a~) and the
     explicit terms J a~ - J c = -J mu depend on a~ and mu separately."""
     L = len(Ws)
-    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True, hidden=hidden, mu=mu)
+    fw = crown_forward(Ws, bs, act, a0, sig, None, keep=True, hidden=hidden, mu=mu, alphas=alphas)
     relaxs, ls, us, zs, J = fw["relaxs"], fw["ls"], fw["us"], fw["zs"], fw["J"]
     a0 = a0 if mu is None else a0 + mu          # the box centre c: what the bounds below see
     a_bar = np.zeros_like(a0)
@@ -539,6 +549,10 @@ def crown_vjp(Ws, bs, act, a0, sig, g_lo, g_hi, flips=(), hidden="crown", mu=Non
     ub = ub + ibp_u[0]
     a_bar += Ws[0].T @ (lb + ub)
     s_bar += np.abs(Ws[0]).T @ (ub - lb)
+    if slope_grads is not None:
+        # adjoints of the lower slopes k^L of every hidden layer (complete now: every target has been reversed); for an
+        # unstable ReLU neuron k^L = alpha is a free parameter, so this is d(objective)/d(alpha)
+        slope_grads.extend(padj[l][2].copy() for l in range(L - 1))
     if mu is None:
         return a_bar + nominal_bar, s_bar
     return a_bar + nominal_bar, s_bar, a_bar - J.T @ (g_hi + g_lo)
@@ -563,3 +577,36 @@ def leb_nn_vjp(Ws, bs, act, nom, rad, g_lo, g_hi, hidden="crown", mu=None):
     for i in range(nom.shape[0]):
         gn[i], gr[i] = crown_vjp(Ws, bs, act, nom[i], rad[i], g_lo[i], g_hi[i], hidden=hidden)
     return gn, gr
+
+
+# --------------------------------------------------------------------------
+# optimisable lower slopes (alpha-CROWN style): projected gradient descent on the lower slopes of the
+# unstable ReLU neurons, one slope set per tile, objective = total width sum_i (r_hi_i - r_lo_i); every iterate is a
+# sound enclosure (any alpha in [0, 1] is), the best one is kept.  The paper gives no such procedure (L194-196 only
+# names CROWN): plain gradient steps with a caller-chosen step size.
+# --------------------------------------------------------------------------
+def default_alphas(Ws, bs, a0, sig):
+    """the adaptive slopes of reading R8 at the bounds they produce (the starting point of the descent)"""
+    fw = crown_forward(Ws, bs, ACT_RELU, a0, sig)
+    return [r[2].copy() for r in fw["relaxs"]]
+
+
+def alpha_refine(Ws, bs, a0, sig, steps, lr):
+    """Returns (r_lo, r_hi, width0, width) of the best iterate."""
+    alphas = default_alphas(Ws, bs, a0, sig)
+    n = Ws[-1].shape[0]
+    best = None
+    w0 = None
+    for it in range(steps + 1):
+        fw = crown_forward(Ws, bs, ACT_RELU, a0, sig, alphas=alphas)
+        w = float((fw["r_hi"] - fw["r_lo"]).sum())
+        if it == 0:
+            w0 = w
+        if best is None or w < best[2]:
+            best = (fw["r_lo"].copy(), fw["r_hi"].copy(), w)
+        if it == steps:
+            break
+        grads = []
+        crown_vjp(Ws, bs, ACT_RELU, a0, sig, -np.ones(n), np.ones(n), alphas=alphas, slope_grads=grads)
+        alphas = [np.clip(a - lr * g, 0.0, 1.0) for a, g in zip(alphas, grads)]
+    return best[0], best[1], w0, best[2]

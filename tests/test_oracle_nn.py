@@ -470,3 +470,63 @@ def test_mu_vjp_matches_central_differences(act, dims, seed, hidden):
         assert abs((fp - fm) / (2 * h) - g[i]) <= 1e-6 * scale + 1e-5 * abs(g[i]), i
         ok += 1
     assert ok >= 2 * N
+
+
+# ---------------------------------------------------------------- optimisable lower slopes (alpha-CROWN)
+def test_alpha_any_slope_is_sound_and_default_reproduces_crown():
+    rng = np.random.default_rng(800)
+    dims = [4, 10, 10, 10, 3]
+    Ws, bs = _net(rng, dims, scale=2.0)
+    a0 = rng.standard_normal(4) * 0.3
+    sig = rng.uniform(0.2, 0.5, 4)
+    base = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig)
+    assert sum((np.array([a[0] for a in r[4]]) == "unstable").sum() for r in base["relaxs"]) >= 6
+    d = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig, alphas=O.default_alphas(Ws, bs, a0, sig))
+    assert np.array_equal(d["r_lo"], base["r_lo"]) and np.array_equal(d["r_hi"], base["r_hi"])
+    X = np.concatenate([a0 + sig * rng.uniform(-1, 1, (20000, 4)), _vertices(a0, sig)])
+    R = _true_r(Ws, bs, O.ACT_RELU, a0, X)
+    for trial in range(5):
+        alphas = [rng.uniform(0, 1, W.shape[0]) for W in Ws[:-1]]
+        out = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig, alphas=alphas)
+        assert np.all(R.min(0) >= out["r_lo"] - 1e-12) and np.all(R.max(0) <= out["r_hi"] + 1e-12)
+        for x in X[::211]:
+            for z, l, u in zip(O.mlp_hidden(Ws, bs, O.ACT_RELU, x), out["ls"], out["us"]):
+                assert np.all(z >= l - 1e-12) and np.all(z <= u + 1e-12)
+
+
+def test_alpha_gradient_and_refinement():
+    rng = np.random.default_rng(801)
+    dims = [4, 10, 10, 10, 3]
+    Ws, bs = _net(rng, dims, scale=2.0)
+    a0 = rng.standard_normal(4) * 0.3
+    sig = rng.uniform(0.2, 0.5, 4)
+    n = 3
+    alphas = [rng.uniform(0.2, 0.8, W.shape[0]) for W in Ws[:-1]]
+    grads = []
+    O.crown_vjp(Ws, bs, O.ACT_RELU, a0, sig, -np.ones(n), np.ones(n), alphas=alphas, slope_grads=grads)
+
+    def Wd(al):
+        f = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig, alphas=al)
+        return (f["r_hi"] - f["r_lo"]).sum(), f
+    _, f0 = Wd(alphas)
+    h, ok = 1e-6, 0
+    for l in range(len(alphas)):
+        unstable = [a[0] == "unstable" for a in f0["relaxs"][l][4]]
+        for k in range(len(unstable)):
+            ap = [a.copy() for a in alphas]; am = [a.copy() for a in alphas]
+            ap[l][k] += h; am[l][k] -= h
+            fp, fm, fc = Wd(ap)[0], Wd(am)[0], Wd(alphas)[0]
+            if not unstable[k]:
+                assert fp == fm                                    # stable neurons ignore alpha
+                continue
+            if abs((fp - fc) - (fc - fm)) > 1e-3 * abs(fp - fm) + 1e-12:
+                continue
+            assert abs((fp - fm) / (2 * h) - grads[l][k]) <= 1e-5 * abs(grads[l][k]) + 1e-7, (l, k)
+            ok += 1
+    assert ok >= 5
+    lo, hi, w0, w = O.alpha_refine(Ws, bs, a0, sig, steps=10, lr=0.05)
+    base = O.crown_forward(Ws, bs, O.ACT_RELU, a0, sig)
+    assert np.isclose(w0, (base["r_hi"] - base["r_lo"]).sum()) and w < 0.98 * w0
+    X = np.concatenate([a0 + sig * rng.uniform(-1, 1, (20000, 4)), _vertices(a0, sig)])
+    R = _true_r(Ws, bs, O.ACT_RELU, a0, X)
+    assert np.all(R.min(0) >= lo - 1e-12) and np.all(R.max(0) <= hi + 1e-12)
