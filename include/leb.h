@@ -181,6 +181,16 @@ leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float*
                       const float* mu, const float* J, int ld_in, float* r_lo, float* r_hi,
                       float* margin, int ld_out, unsigned flags, void* stream);
 
+/* CROWN with optimisable lower slopes (alpha-CROWN style; the paper names CROWN only, L194-196).  ReLU
+ * networks: the lower line of an unstable neuron (l < 0 < u) is alpha z with ANY alpha in [0, 1].  Starting from the adaptive
+ * choice of leb_nn_fwd, `steps` projected gradient steps alpha <- clip(alpha - lr dW/dalpha, 0, 1) on the total width
+ * W = sum_i (r_hi_i - r_lo_i) of each tile's enclosure (one slope set per tile; dW/dalpha comes from the ordinary reverse
+ * sweep), all on the device; every iterate is a sound enclosure and the tightest one per tile is returned.
+ * Value mode only (flags must contain LEB_FLAG_NO_MARGIN), tanh networks: LEB_ERR_UNSUPPORTED.
+ *   width0, width : [B, T] total width of the adaptive-slope enclosure / of the returned one.  Other arguments as leb_nn_fwd. */
+leb_status leb_nn_alpha_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad, int ld_in, int steps, float lr,
+                            float* r_lo, float* r_hi, int ld_out, float* width0, float* width, unsigned flags, void* stream);
+
 /* VJP of the bounds: grad = d/d(a~, sigma) sum_i g_hi[i] r_hi[i] + g_lo[i] r_lo[i], per tile
  * (block-diagonal over tiles).  Stateless by default: the forward pass is recomputed internally, and for kind 1 it
  * is recomputed in value mode whatever the flags say -- the certified margin is a rounding-level pad and is treated

@@ -251,6 +251,37 @@ leb_status leb_nn_fwd(leb_ctx* c, int B, int T, const float* nom, const float* r
     return ok ? LEB_OK : LEB_ERR_CUDA;
 }
 
+leb_status leb_nn_alpha_fwd(leb_ctx* c, int B, int T, const float* nom, const float* rad, int ld_in, int steps, float lr, float* r_lo,
+                            float* r_hi, int ld_out, float* width0, float* width, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || steps < 0 || !(lr >= 0.f)) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!nom || !rad || !r_lo || !r_hi || !width0 || !width) return LEB_ERR_ARG;
+    const int n = leb_nn_n(c->nn), N = leb_nn_N(c->nn);
+    leb_status s = check_traj(B, T, N, n, ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(r_lo) || !al4(r_hi) || !al4(width0) || !al4(width)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    float* d_lo = out_ptr(c, 2, r_lo, tiles * ld_out, host, &ok);
+    float* d_hi = out_ptr(c, 3, r_hi, tiles * ld_out, host, &ok);
+    float* d_w0 = out_ptr(c, 6, width0, tiles, host, &ok);
+    float* d_w = out_ptr(c, 7, width, tiles, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    s = leb_nn_alpha(c->nn, (int)tiles, d_nom, d_rad, ld_in, steps, lr, d_lo, d_hi, ld_out, d_w0, d_w, flags, c->domain_flag, st, &c->launches, &c->prof);
+    if (s != LEB_OK) return s;
+    out_copy(r_lo, d_lo, tiles * ld_out, host, st, &ok);
+    out_copy(r_hi, d_hi, tiles * ld_out, host, st, &ok);
+    out_copy(width0, d_w0, tiles, host, st, &ok);
+    out_copy(width, d_w, tiles, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
 leb_status leb_vjp_mu(leb_ctx* c, int kind, int B, int T, const float* nom, const float* rad, const float* mu, const float* g_lo,
                       const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags,
                       void* stream) {

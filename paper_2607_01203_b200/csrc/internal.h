@@ -107,6 +107,9 @@ leb_status leb_nn_forward(NnState*, int tiles, const float* nom, const float* ra
 leb_status leb_nn_vjp(NnState*, int tiles, const float* nom, const float* rad, const float* mu, const float* g_lo,
                       const float* g_hi, int ld_in, int ld_out, float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags,
                       int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
+leb_status leb_nn_alpha(NnState*, int tiles, const float* nom, const float* rad, int ld_in, int steps, float lr, float* r_lo,
+                        float* r_hi, int ld_out, float* w0, float* wbest, unsigned flags, int* domain_flag, cudaStream_t st,
+                        long long* launches, LebProf* prof);
 void leb_nn_query(const NnState*, int* tiles, int* certified, int* vjp_reused);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);
 leb_status leb_nn_get_coeffs(NnState*, int target, float* out, cudaStream_t st, long long* launches);

@@ -55,6 +55,9 @@ struct NnState {
     std::vector<void*> allocs;
     float *nomp = nullptr, *radp = nullptr, *rad1 = nullptr;
     float *mup = nullptr, *mu1 = nullptr, *mu_bar = nullptr;   // non-centred boxes: padded mu, W_1 mu, and its adjoint
+    float* alpha[kMaxLayers] = {nullptr};                      // optimisable lower ReLU slopes (leb_nn_alpha_fwd), [chunk x wp[l]]
+    int alpha_mode = 0;                                        // 0 off, 1 forward writes the adaptive default, 2 forward reads alpha
+    std::vector<void*> alpha_scratch; size_t alpha_scratch_tiles = 0;
     const float* mu_cur = nullptr;                             // = mup while the chunk in flight has box offsets, else NULL
     float *zhat[kMaxLayers] = {nullptr}, *ahat[kMaxLayers] = {nullptr}, *dphi[kMaxLayers] = {nullptr};
     float *lb[kMaxLayers] = {nullptr}, *ub[kMaxLayers] = {nullptr};
@@ -151,7 +154,7 @@ __global__ void split_tf32_kernel(const float* __restrict__ src, float* __restri
 __global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ zhat,
                                  const float* __restrict__ rad1, float* __restrict__ lb, float* __restrict__ ub,
                                  float* __restrict__ kU, float* __restrict__ kL, float* __restrict__ gU, float* __restrict__ gL,
-                                 const float* __restrict__ mu1 = nullptr) {
+                                 const float* __restrict__ mu1 = nullptr, float* __restrict__ alpha = nullptr, int alpha_mode = 0) {
     size_t total = (size_t)tiles * wp;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int c = (int)(q % wp);
@@ -166,6 +169,10 @@ __global__ void relax_fwd_kernel(int act, int tiles, int w_valid, int wp, const 
         }
         else { l = lb[q]; u = ub[q]; }
         Relax r = relax_any(act, (double)l, (double)u);
+        if (alpha_mode) {     // optimisable lower slope of an unstable ReLU neuron: any value in [0, 1] is a valid lower line
+            if (alpha_mode == 1) alpha[q] = (float)r.kL;
+            else if (r.cL == LINE_RELU_LOW) r.kL = (double)alpha[q];
+        }
         double f = act_f(act, (double)z);
         kU[q] = (float)r.kU;
         kL[q] = (float)r.kL;
@@ -496,13 +503,14 @@ __global__ void relax_vjp_kernel(int act, int tiles, int w_valid, int wp, const 
                                  const float* __restrict__ lb, const float* __restrict__ ub, const float* __restrict__ kUb,
                                  const float* __restrict__ kLb, const float* __restrict__ gUb, const float* __restrict__ gLb,
                                  const float* __restrict__ dpb, float* __restrict__ lbar, float* __restrict__ ubar,
-                                 float* __restrict__ zbar, int is_layer1) {
+                                 float* __restrict__ zbar, int is_layer1, const float* __restrict__ alpha = nullptr) {
     size_t total = (size_t)tiles * wp;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int c = (int)(q % wp);
         if (c >= w_valid) { lbar[q] = 0.f; ubar[q] = 0.f; continue; }
         double z = zhat[q], l = lb[q], u = ub[q];
         Relax r = relax_any(act, l, u);
+        if (alpha && r.cL == LINE_RELU_LOW) r.kL = (double)alpha[q];
         double gu = gUb[q], gl = gLb[q];
         // g = k zhat + b - phi(zhat):  k_bar_eff = k_bar + zhat g_bar,  b_bar = g_bar
         double kbu = (double)kUb[q] + z * gu, kbl = (double)kLb[q] + z * gl;
@@ -593,6 +601,44 @@ __global__ void diff_kernel(const float* __restrict__ ubar, const float* __restr
         out[q] = ubar[q] - lbar[q];
 }
 
+// alpha-CROWN style refinement: one projected gradient step on the lower slopes of the unstable ReLU neurons;
+// d(objective)/d(alpha) = k_bar^L + zhat gap_bar^L (gap^L = alpha zhat - relu(zhat))
+__global__ void alpha_update_kernel(int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ lb,
+                                    const float* __restrict__ ub, const float* __restrict__ kLb, const float* __restrict__ gLb,
+                                    float* __restrict__ alpha, float lr) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid || !(lb[q] < 0.f && ub[q] > 0.f)) continue;
+        const float g = kLb[q] + zhat[q] * gLb[q];
+        const float a = alpha[q] - lr * g;
+        if (a == a) alpha[q] = fminf(fmaxf(a, 0.f), 1.f);
+    }
+}
+
+// keep the tightest iterate of every tile: one block per tile
+__global__ void alpha_best_kernel(int n, int ld_out, int first, const float* __restrict__ cur_lo, const float* __restrict__ cur_hi,
+                                  float* __restrict__ r_lo, float* __restrict__ r_hi, float* __restrict__ w0, float* __restrict__ wbest) {
+    __shared__ float red[8];
+    __shared__ int take;
+    const size_t t = blockIdx.x;
+    float w = 0.f;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) w += cur_hi[t * n + i] - cur_lo[t * n + i];
+    for (int off = 16; off; off >>= 1) w += __shfl_xor_sync(0xffffffffu, w, off);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = w;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float tot = 0.f;
+        for (int q = 0; q < (int)(blockDim.x >> 5); ++q) tot += red[q];
+        if (first) { w0[t] = tot; wbest[t] = tot; take = 1; }
+        else if (tot < wbest[t]) { wbest[t] = tot; take = 1; }
+        else take = 0;
+    }
+    __syncthreads();
+    if (take)
+        for (int i = threadIdx.x; i < n; i += blockDim.x) { r_lo[t * ld_out + i] = cur_lo[t * n + i]; r_hi[t * ld_out + i] = cur_hi[t * n + i]; }
+}
+
 __global__ void sum_kernel(const float* __restrict__ a, const float* __restrict__ b, float* __restrict__ out, size_t count) {
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x)
         out[q] = a[q] + b[q];
@@ -677,7 +723,7 @@ void ws_free(NnState* S) {
 
 size_t bytes_per_tile(const NnState* S, bool vjp) {
     size_t f = 5 * (size_t)S->wp[0] + (size_t)S->wp[1];
-    for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 23 : 15);
+    for (int l = 1; l < S->L; ++l) f += (size_t)S->wp[l] * (vjp ? 24 : 16);
     size_t maxLam = 0;
     for (int s = 2; s <= S->L; ++s) {
         for (int l = 0; l <= s - 2; ++l) f += (size_t)S->rows_pad[s] * S->wp[l];
@@ -727,6 +773,7 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
         S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
         S->kU[l] = F(c); S->kL[l] = F(c); S->gU[l] = F(c); S->gL[l] = F(c);
         S->ce[l] = F(c); S->ct[l] = F(c); S->cv[l] = F(c); S->adev[l] = F(c); S->mU[l] = F(c); S->mL[l] = F(c);
+        S->alpha[l] = F(c);
         if (vjp) {
             S->kUb[l] = F(c); S->kLb[l] = F(c); S->gUb[l] = F(c); S->gLb[l] = F(c); S->dpb[l] = F(c);
             S->zbar[l] = F(c); S->lbar[l] = F(c); S->ubar[l] = F(c);
@@ -807,7 +854,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
         }
         relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->rad1, S->lb[1],
                                                                       S->ub[1], S->kU[1], S->kL[1], S->gU[1], S->gL[1],
-                                                                      S->mu_cur ? S->mu1 : nullptr);
+                                                                      S->mu_cur ? S->mu1 : nullptr, S->alpha[1], S->alpha_mode);
         ++*launches;
     }
     // ---- N3 / N4: targets s = 2 .. L
@@ -827,7 +874,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
             launch_gemm<AMODE_PLAIN, EPI_STORE>(S, g2, st, launches);
             ibp_bounds_kernel<<<gs_grid(cs), 256, 0, st>>>(C, S->w[s], S->wp[s], S->zhat[s], S->cv[s], S->adev[s], S->lb[s], S->ub[s]);
             relax_fwd_kernel<<<gs_grid(cs), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s], S->ub[s], S->kU[s],
-                                                         S->kL[s], S->gU[s], S->gL[s]);
+                                                         S->kL[s], S->gU[s], S->gL[s], nullptr, S->alpha[s], S->alpha_mode);
             *launches += 2;
             continue;
         }
@@ -873,7 +920,8 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
                     S->kU[s], S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s]);
             } else {
                 relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s],
-                                                                              S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s]);
+                                                                              S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s], nullptr,
+                                                                              S->alpha[s], S->alpha_mode);
             }
             ++*launches;
         }
@@ -908,6 +956,7 @@ void leb_nn_destroy(NnState* S) {
     cudaDeviceSynchronize();
     ws_free(S);
     free_weights(S);
+    for (void* p : S->alpha_scratch) cudaFree(p);
     delete S;
 }
 
@@ -1131,7 +1180,8 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
             if (!is_out) {
                 relax_vjp_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], S->lb[s],
                                                                               S->ub[s], S->kUb[s], S->kLb[s], S->gUb[s], S->gLb[s],
-                                                                              S->dpb[s], S->lbar[s], S->ubar[s], S->zbar[s], 0);
+                                                                              S->dpb[s], S->lbar[s], S->ubar[s], S->zbar[s], 0,
+                                                                              S->alpha_mode ? S->alpha[s] : nullptr);
                 ++*launches;
             }
             if (ibp && !is_out) {
@@ -1185,7 +1235,8 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         // ---- layer 1: l_1, u_1 = zhat_1 -+ |W_1| sigma
         relax_vjp_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(S->act, C, S->w[1], S->wp[1], S->zhat[1], S->lb[1], S->ub[1],
                                                                       S->kUb[1], S->kLb[1], S->gUb[1], S->gLb[1], S->dpb[1],
-                                                                      S->lbar[1], S->ubar[1], S->zbar[1], 1);
+                                                                      S->lbar[1], S->ubar[1], S->zbar[1], 1,
+                                                                      S->alpha_mode ? S->alpha[1] : nullptr);
         if (ibp && L > 2) {
             const size_t c1 = (size_t)C * S->wp[1];
             ibp_add_kernel<<<gs_grid(c1), 256, 0, st>>>(c1, S->lbar[1], S->ubar[1], S->zbar[1], S->mU[1], S->mL[1]);
@@ -1221,5 +1272,68 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
         if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; S->last_mu = (mu != nullptr); }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------
+// optimisable lower slopes (alpha-CROWN style): projected gradient descent on the lower slopes of the
+// unstable ReLU neurons, one slope set per tile, objective = total width of the tile's enclosure; every iterate is sound,
+// the tightest one is returned.  Forward and reverse sweep are the ordinary ones (the slope adjoints k_bar^L, gap_bar^L are
+// what the reverse sweep accumulates anyway).
+// ------------------------------------------------------------------------------------------
+leb_status leb_nn_alpha(NnState* S, int tiles, const float* nom, const float* rad, int ld_in, int steps, float lr, float* r_lo,
+                        float* r_hi, int ld_out, float* w0, float* wbest, unsigned flags, int* domain_flag, cudaStream_t st,
+                        long long* launches, LebProf* prof) {
+    if (S->act != ACT_RELU) return LEB_ERR_UNSUPPORTED;
+    if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;       // value mode only
+    if (tiles == 0) return LEB_OK;
+    leb_status ws = ensure_workspace(S, tiles, true);
+    if (ws != LEB_OK) return ws;
+    const int L = S->L, n = S->w[L];
+    const size_t Cmax = (size_t)std::min(S->chunk, tiles);
+    if (S->alpha_scratch_tiles < Cmax) {
+        cudaDeviceSynchronize();
+        for (void* p : S->alpha_scratch) cudaFree(p);
+        S->alpha_scratch.clear();
+        const size_t sizes[6] = {Cmax * n, Cmax * n, Cmax * n, Cmax * n, Cmax * (size_t)ld_in, Cmax * (size_t)ld_in};
+        for (size_t sz : sizes) {
+            void* p = nullptr;
+            if (cudaMalloc(&p, std::max<size_t>(sz, 4) * sizeof(float)) != cudaSuccess) { S->alpha_scratch_tiles = 0; return LEB_ERR_NOMEM; }
+            S->alpha_scratch.push_back(p);
+        }
+        S->alpha_scratch_tiles = Cmax;
+    }
+    float *cur_lo = (float*)S->alpha_scratch[0], *cur_hi = (float*)S->alpha_scratch[1], *gm1 = (float*)S->alpha_scratch[2],
+          *gp1 = (float*)S->alpha_scratch[3], *gsn = (float*)S->alpha_scratch[4], *gsr = (float*)S->alpha_scratch[5];
+    fill_kernel<<<gs_grid(Cmax * n), 256, 0, st>>>(gm1, Cmax * n, -1.f);
+    fill_kernel<<<gs_grid(Cmax * n), 256, 0, st>>>(gp1, Cmax * n, 1.f);
+    *launches += 2;
+    const unsigned f = flags | LEB_FLAG_NO_MARGIN;
+    leb_status rc = LEB_OK;
+    for (int t0 = 0; t0 < tiles && rc == LEB_OK; t0 += S->chunk) {
+        const int C = std::min(S->chunk, tiles - t0);
+        const float* a = nom + (size_t)t0 * ld_in;
+        const float* r = rad + (size_t)t0 * ld_in;
+        for (int it = 0; it <= steps && rc == LEB_OK; ++it) {
+            S->alpha_mode = (it == 0) ? 1 : 2;
+            rc = leb_nn_forward(S, C, a, r, nullptr, nullptr, ld_in, cur_lo, cur_hi, nullptr, n, f, domain_flag, st, launches, prof);
+            if (rc != LEB_OK) break;
+            alpha_best_kernel<<<C, 128, 0, st>>>(n, ld_out, it == 0, cur_lo, cur_hi, r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out,
+                                                 w0 + t0, wbest + t0);
+            ++*launches;
+            if (it == steps) break;
+            S->alpha_mode = 2;
+            rc = leb_nn_vjp(S, C, a, r, nullptr, gm1, gp1, ld_in, n, gsn, gsr, nullptr, f | LEB_FLAG_REUSE_FWD, domain_flag, st, launches, prof);
+            if (rc != LEB_OK) break;
+            for (int l = 1; l < L; ++l) {
+                alpha_update_kernel<<<gs_grid((size_t)C * S->wp[l]), 256, 0, st>>>(C, S->w[l], S->wp[l], S->zhat[l], S->lb[l], S->ub[l],
+                                                                                S->kLb[l], S->gLb[l], S->alpha[l], lr);
+                ++*launches;
+            }
+        }
+    }
+    S->alpha_mode = 0;
+    S->last_tiles = 0;      // the resident state belongs to a refined slope set: not a state leb_vjp may reuse
+    if (rc != LEB_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }

@@ -27,7 +27,7 @@ FLAG_IBP_HIDDEN = 32
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
-    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_pgd", "leb_nn_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
+    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
     "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
@@ -215,6 +215,20 @@ class Context:
         _chk(self.lib.leb_nn_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), _ptr(J), ld_in, _ptr(r_lo), _ptr(r_hi),
                                  _ptr(margin), int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_nn_fwd")
         return r_lo, r_hi
+
+    def leb_nn_alpha_fwd(self, nom, rad, steps: int, lr: float, flags: int = FLAG_NO_MARGIN):
+        """CROWN with optimisable lower ReLU slopes; returns (r_lo, r_hi, width0, width)."""
+        _check_f32(nom, rad)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        r_lo = self._out(nom, (B, T, self.nn_n), host)
+        r_hi = self._out(nom, (B, T, self.nn_n), host)
+        w0 = self._out(nom, (B, T), host)
+        w = self._out(nom, (B, T), host)
+        _chk(self.lib.leb_nn_alpha_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), ld_in, int(steps), ctypes.c_float(lr), _ptr(r_lo),
+                                       _ptr(r_hi), self.nn_n, _ptr(w0), _ptr(w), ctypes.c_uint(flags), _stream_ptr(self.device)),
+             "leb_nn_alpha_fwd")
+        return r_lo, r_hi, w0, w
 
     def leb_vjp(self, kind: int, nom, rad, g_lo, g_hi, grad_nom=None, grad_rad=None, flags: int = 0):
         _check_f32(nom, rad, g_lo, g_hi, grad_nom, grad_rad)

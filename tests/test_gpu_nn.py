@@ -493,3 +493,75 @@ def test_mu_config5_sampled_tiles_and_soundness(mods):
         r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ J.T
         assert np.all(r.max(0) <= ghi[t] + 1e-5 * np.abs(ghi[t]) + 1e-7) and np.all(r.min(0) >= glo[t] - 1e-5 * np.abs(glo[t]) - 1e-7)
     c2.close()
+
+
+# ---------------------------------------------------------------------------------- optimisable lower slopes (alpha-CROWN)
+@pytest.mark.parametrize("path", ["tc", "ffma"])
+def test_alpha_refinement_matches_oracle(mods, path):
+    leb, wl, O = mods
+    for dims, seed in (([4, 10, 10, 10, 3], 5), ([6, 33, 20, 11, 5], 6), ([24, 130, 70, 20], 7)):
+        w = wl.make_small_mlp(dims, 1, 2, 3, seed=seed, rad_lo=0.1, rad_hi=0.4)
+        ctx = leb.context_for_workload(w)
+        nom, rad, _, _ = _flat(w)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        # zero steps = the adaptive slopes of leb_nn_fwd, bit for bit
+        lo0, hi0, w0, wb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 0, 0.05, flags=PATHS[path])
+        plo, phi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+        assert torch.equal(lo0, plo) and torch.equal(hi0, phi) and torch.equal(w0, wb)
+        steps, lr = 8, 0.05
+        lo, hi, w0, wb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), steps, lr, flags=PATHS[path])
+        glo, ghi = to_np(lo).reshape(-1, w.n), to_np(hi).reshape(-1, w.n)
+        gw0, gwb = to_np(w0).reshape(-1), to_np(wb).reshape(-1)
+        assert np.all(gwb <= gw0)
+        improved = 0
+        for t in range(w.B * w.T):
+            olo, ohi, ow0, owb = O.alpha_refine(Ws, bs, nom[t].astype(np.float64), rad[t].astype(np.float64), steps, lr)
+            assert abs(gw0[t] - ow0) <= 1e-5 * ow0
+            assert abs(gwb[t] - owb) <= 2e-3 * owb, (dims, t, gwb[t], owb)         # an iteration amplifies rounding differences
+            improved += owb < 0.999 * ow0
+            # the returned enclosure is sound: >= 2e4 samples + vertices (N <= 6) of the box
+            N = dims[0]
+            rng = np.random.default_rng(t)
+            a0 = nom[t].astype(np.float64); sg = rad[t].astype(np.float64)
+            U = rng.uniform(-1, 1, (20000, N))
+            if N <= 6:
+                U = np.concatenate([U, np.array(list(itertools.product((-1.0, 1.0), repeat=N)))])
+            X = a0[None] + U * sg[None]
+            zs, p, J = O.nominal(Ws, bs, 1, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(1, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ J.T
+            assert np.all(r.max(0) <= ghi[t] + 1e-5 * np.abs(ghi[t]) + 1e-7) and np.all(r.min(0) >= glo[t] - 1e-5 * np.abs(glo[t]) - 1e-7)
+        assert improved >= 1
+        # tanh networks and the certified mode are refused
+        with pytest.raises(leb.LebError) as e:
+            ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 2, 0.05, flags=PATHS[path] & ~1)
+        assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+        ctx.close()
+    wt = wl.make_small_mlp([5, 9, 3], 2, 1, 1)
+    ct = leb.context_for_workload(wt)
+    with pytest.raises(leb.LebError) as e:
+        ct.leb_nn_alpha_fwd(_dev(wt.nom), _dev(wt.rad), 2, 0.05)
+    assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+    ct.close()
+
+
+def test_alpha_refinement_config3(mods):
+    """Config 3 (ReLU, 1 280 tiles, chunked workspace): tighter than the adaptive slopes on most tiles, never looser."""
+    leb, wl, O = mods
+    w = wl.make_config(3)
+    ctx = leb.context_for_workload(w)
+    lo, hi, w0, wb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 6, 10.0)      # dW/dalpha ~ 0.05 here: steps of ~0.5
+    plo, phi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=VAL)
+    assert bool((wb <= w0).all())
+    assert torch.allclose(w0.reshape(-1), (phi - plo).sum(-1).reshape(-1), rtol=1e-5)
+    gain = float((wb.sum() / w0.sum()))
+    print(f"config 3: alpha-refined total width / adaptive-slope width = {gain:.4f}")
+    assert gain < 0.995
+    nom, rad, _, _ = _flat(w)
+    t = 17
+    olo, ohi, ow0, owb = O.alpha_refine([np.asarray(x, np.float64) for x in w.mlp.W], [np.asarray(x, np.float64) for x in w.mlp.b],
+                                        nom[t].astype(np.float64), rad[t].astype(np.float64), 6, 10.0)
+    assert abs(float(wb.reshape(-1)[t]) - owb) <= 2e-3 * owb
+    ctx.close()
