@@ -51,7 +51,7 @@ typedef enum {
     LEB_ERR_SHAPE = 2,       /* ld too small, model/shape mismatch */
     LEB_ERR_ALIGN = 3,       /* pointer not 4-byte aligned */
     LEB_ERR_DOMAIN = 4,      /* reported by leb_domain_flag(): some tile hit a domain error */
-    LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048, with mu != NULL or with CROWN-IBP */
+    LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048 or with CROWN-IBP */
     LEB_ERR_CUDA = 6,
     LEB_ERR_NOMEM = 7,
     LEB_ERR_STATE = 8        /* model not set before the call that needs it */
@@ -168,8 +168,10 @@ leb_status leb_analytic_pgd(leb_ctx* ctx, int B, int T, const float* centre, con
 /* CROWN + Thm 3 bound, eq. (18)-(21) L196-220, for every tile.
  *   mu     : NULL (centred box) or [B, T, ld_in]: the box is a~ + mu + [-sigma, sigma] (25a) L272; the CROWN bounds are
  *            taken on that box, p(a~) and J(a~) stay at the nominal point, and (21) maximises the affine bound (20) over
- *            the box (in the kernels' deviation form: a - a~ in mu -+ sigma).  Value mode only: with mu != NULL and
- *            without LEB_FLAG_NO_MARGIN the call returns LEB_ERR_UNSUPPORTED.
+ *            the box (in the kernels' deviation form: a - a~ in mu -+ sigma).  Certified mode keeps its guarantee: the
+ *            layer-1 shift W_1 mu and the Lam_0 mu sums are padded outward like every other sum; the relaxation
+ *            gaps stay at zhat(a~), clamped to gU >= 0 >= gL, which is sound and up to a few % wider than value
+ *            mode when |W_1 mu| exceeds a neuron's radius.
  *   J      : NULL => the network's own Jacobian at a~ (eq. (7)); otherwise [B, T, n, N]
  *            dense, and the bound is with respect to that matrix (Thm 3 holds for any J).
  *   margin : NULL or [B, T, ld_out].  Certified mode: the outward pad contained in r_lo / r_hi of the entry (the

@@ -451,13 +451,13 @@ def output_sign_ties(Ws, bs, act, a0, sig, rel=1e-6):
     return ties
 
 
-def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5):
+def relax_case_ties(Ws, bs, act, a0, sig, rel=2e-5, mu=None):
     """Hidden neurons (layer, k) whose pre-activation bound sits on a case switch of the relaxation
     table (readings R8/R9/R21): an endpoint l or u within rel * (|l| + |u|) of 0, or (ReLU)
     |u + l| that close to the u > -l switch.  The relaxation -- and with it the bound -- is
     discontinuous there, so an FP32 evaluation may legitimately take the other case.  Test
     plumbing only: calls crown_forward, changes no arithmetic."""
-    fw = crown_forward(Ws, bs, act, a0, sig)
+    fw = crown_forward(Ws, bs, act, a0, sig, mu=mu)
     ties = []
     for layer, (l, u) in enumerate(zip(fw["ls"], fw["us"]), start=1):
         scale = rel * (np.abs(l) + np.abs(u))

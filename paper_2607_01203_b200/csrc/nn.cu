@@ -211,7 +211,8 @@ __global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, i
                                       const float* __restrict__ ahat, const float* __restrict__ v, const float* __restrict__ e,
                                       float* __restrict__ lb, float* __restrict__ ub, float* __restrict__ kU, float* __restrict__ kL,
                                       float* __restrict__ gU, float* __restrict__ gL, float* __restrict__ adev,
-                                      float* __restrict__ mU, float* __restrict__ mL) {
+                                      float* __restrict__ mU, float* __restrict__ mL, const float* __restrict__ m1 = nullptr,
+                                      const float* __restrict__ vmu = nullptr, float gam_mu = 0.f) {
     size_t total = (size_t)tiles * wp;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int c = (int)(q % wp);
@@ -220,9 +221,19 @@ __global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, i
             continue;
         }
         float z = zhat[q], l, u;
+        float vq = v[q];          // radius of z - zhat over the box (what the rounding pads below scale with)
         if (layer1) {
-            float r = __fadd_ru(v[q], e[q]);
-            l = __fadd_rd(z, -r); u = __fadd_ru(z, r);
+            float r = __fadd_ru(vq, e[q]);
+            if (m1) {
+                // non-centred box: z_1 - zhat_1 in W_1 mu -+ |W_1| sigma -+ e_1.  m1 is the FP32 product W_1 mu, wrong by at
+                // most gam_mu |W_1||mu| (vmu, rounded up); the radius seen by the pads is |W_1| (sigma + |mu|)
+                const float mq = m1[q];
+                r = __fadd_ru(r, __fmul_ru(gam_mu, vmu[q]));
+                l = __fadd_rd(z, __fadd_rd(mq, -r)); u = __fadd_ru(z, __fadd_ru(mq, r));
+                vq = __fadd_ru(vq, vmu[q]);
+            } else {
+                l = __fadd_rd(z, -r); u = __fadd_ru(z, r);
+            }
             lb[q] = l; ub[q] = u;
         } else { l = lb[q]; u = ub[q]; }
         const double zd = (double)z, ld = (double)l, ud = (double)u, a = (double)ahat[q];
@@ -232,7 +243,7 @@ __global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, i
         const double d64 = 5.7e-14 * (1.0 + fabs(zd) + fabs(ld) + fabs(ud));          // 2^-44 (1 + |c| + |l| + |u|)
         const double gu = (r.kU * zd + r.bU - a) + fabs((double)kU32 - r.kU) * zdev + d64;
         const double gl = (r.kL * zd + r.bL - a) - fabs((double)kL32 - r.kL) * zdev - d64;
-        const float x = __fmaf_ru(gamma_of(tensor, wp, c), v[q], e[q]);
+        const float x = __fmaf_ru(gamma_of(tensor, wp, c), vq, e[q]);
         const float pu = __fmul_ru(fabsf(kU32), x), pl = __fmul_ru(fabsf(kL32), x);
         kU[q] = kU32;
         kL[q] = kL32;
@@ -354,6 +365,7 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
     const float* lo = Lam0 + ((size_t)t * rows_pad + rows_kind + k) * wp0;
     const float* sg = sigma + (size_t)t * wp0;
     float su = 0.f, sl = 0.f, du = 0.f, dl = 0.f;        // du, dl: Lam_0 mu (non-centred boxes: a - a~ in mu -+ sigma)
+    float au = 0.f, al = 0.f;                            // |Lam_0| |mu|: what the rounding of du, dl scales with (certified mode)
     for (int j = lane * 4; j < wp0; j += 128) {
         float4 a = *reinterpret_cast<const float4*>(up + j), b = *reinterpret_cast<const float4*>(lo + j);
         float4 s = *reinterpret_cast<const float4*>(sg + j);
@@ -363,20 +375,25 @@ __global__ void concretise_hidden_kernel(int tiles, int rows_pad, int rows_kind,
             float4 m = *reinterpret_cast<const float4*>(mu + (size_t)t * wp0 + j);
             du += a.x * m.x + a.y * m.y + a.z * m.z + a.w * m.w;
             dl += b.x * m.x + b.y * m.y + b.z * m.z + b.w * m.w;
+            au += fabsf(a.x * m.x) + fabsf(a.y * m.y) + fabsf(a.z * m.z) + fabsf(a.w * m.w);
+            al += fabsf(b.x * m.x) + fabsf(b.y * m.y) + fabsf(b.z * m.z) + fabsf(b.w * m.w);
         }
     }
 #pragma unroll
     for (int off = 16; off; off >>= 1) {
         su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off);
         du += __shfl_xor_sync(0xffffffffu, du, off); dl += __shfl_xor_sync(0xffffffffu, dl, off);
+        au += __shfl_xor_sync(0xffffffffu, au, off); al += __shfl_xor_sync(0xffffffffu, al, off);
     }
     if (lane == 0) {
         float z = zhat[(size_t)t * rows_kind + k];
         const float gu = gap[(size_t)t * rows_pad + k], gl = gap[(size_t)t * rows_pad + rows_kind + k];
         if (e_s) {
             const float e = e_s[(size_t)t * rows_kind + k];
-            const float pu = __fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), e);
-            const float pl = __fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), e);
+            // the signed sums du, dl (non-centred boxes) are wrong by at most (wp0 + 8) 2^-24 of the sums of magnitudes
+            const float km = __fmul_ru(__fadd_ru(kap_sum, -1.f), 1.0001f);      // (au, al are FP32 sums themselves)
+            const float pu = __fadd_ru(__fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), e), __fadd_ru(du, __fmul_ru(au, km)));
+            const float pl = __fadd_ru(__fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), e), __fadd_ru(-dl, __fmul_ru(al, km)));
             ub[(size_t)t * rows_kind + k] = __fadd_ru(z, pu);
             lb[(size_t)t * rows_kind + k] = __fadd_rd(z, -pl);
         } else {
@@ -401,6 +418,7 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
     const float* lo = Lam0 + ((size_t)t * rows_pad + n + i) * wp0;
     const float* sg = sigma + (size_t)t * wp0;
     float su = 0.f, sl = 0.f, du = 0.f, dl = 0.f;        // du, dl: (Lam_0 - J) mu   (non-centred boxes)
+    float au = 0.f, al = 0.f;                            // sums of |(Lam_0 - J) mu|: what the rounding of du, dl scales with
     const float* mt = mu ? mu + (size_t)t * wp0 : nullptr;
     if (Jgiven) {
         const float* Jr = Jgiven + ((size_t)t * n + i) * N;
@@ -408,7 +426,10 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
             float jv = Jr[j], s = sg[j];
             su += fabsf(up[j] - jv) * s;
             sl += fabsf(lo[j] - jv) * s;
-            if (mt) { du += (up[j] - jv) * mt[j]; dl += (lo[j] - jv) * mt[j]; }
+            if (mt) {
+                const float pa = (up[j] - jv) * mt[j], pb = (lo[j] - jv) * mt[j];
+                du += pa; dl += pb; au += fabsf(pa); al += fabsf(pb);
+            }
         }
     } else {
         const float* Jr = Lam0 + ((size_t)t * rows_pad + 2 * n + i) * wp0;
@@ -419,8 +440,10 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
             sl += fabsf(b.x - c.x) * s.x + fabsf(b.y - c.y) * s.y + fabsf(b.z - c.z) * s.z + fabsf(b.w - c.w) * s.w;
             if (mt) {
                 float4 m = *reinterpret_cast<const float4*>(mt + j);
-                du += (a.x - c.x) * m.x + (a.y - c.y) * m.y + (a.z - c.z) * m.z + (a.w - c.w) * m.w;
-                dl += (b.x - c.x) * m.x + (b.y - c.y) * m.y + (b.z - c.z) * m.z + (b.w - c.w) * m.w;
+                const float pa[4] = {(a.x - c.x) * m.x, (a.y - c.y) * m.y, (a.z - c.z) * m.z, (a.w - c.w) * m.w};
+                const float pb[4] = {(b.x - c.x) * m.x, (b.y - c.y) * m.y, (b.z - c.z) * m.z, (b.w - c.w) * m.w};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) { du += pa[q]; dl += pb[q]; au += fabsf(pa[q]); al += fabsf(pb[q]); }
             }
         }
     }
@@ -428,6 +451,7 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
     for (int off = 16; off; off >>= 1) {
         su += __shfl_xor_sync(0xffffffffu, su, off); sl += __shfl_xor_sync(0xffffffffu, sl, off);
         du += __shfl_xor_sync(0xffffffffu, du, off); dl += __shfl_xor_sync(0xffffffffu, dl, off);
+        au += __shfl_xor_sync(0xffffffffu, au, off); al += __shfl_xor_sync(0xffffffffu, al, off);
     }
     if (lane == 0) {
         float hi = (su + du) + gap[(size_t)t * rows_pad + i];
@@ -438,8 +462,9 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
             // output against the centre the chain was developed around); margin_out = eta, the rounding of these sums and
             // the chain pads inside the gap sum (marg, gathered by row_margin_kernel when a margin report is asked for)
             const float gu = gap[(size_t)t * rows_pad + i], gl = gap[(size_t)t * rows_pad + n + i], et = eta[(size_t)t * ld_eta + i];
-            const float pu = __fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), et);
-            const float pl = __fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), et);
+            const float km = __fmul_ru(__fadd_ru(kap_sum, -1.f), 1.0001f);       // relative rounding of the signed sums du, dl against au, al
+            const float pu = __fadd_ru(__fadd_ru(__fadd_ru(__fmul_ru(su, kap_sum), __fmul_ru(gu, kap_gap)), et), __fadd_ru(du, __fmul_ru(au, km)));
+            const float pl = __fadd_ru(__fadd_ru(__fadd_ru(__fmul_ru(sl, kap_sum), __fmul_ru(-gl, kap_gap)), et), __fadd_ru(-dl, __fmul_ru(al, km)));
             mg = fmaxf(__fadd_ru(pu, -hi), __fadd_ru(pl, lo_v));
             if (margin_out) mg = __fadd_ru(mg, fmaxf(marg[(size_t)t * rows_pad + i], marg[(size_t)t * rows_pad + n + i]));
             hi = pu; lo_v = -pl;
@@ -637,6 +662,10 @@ __global__ void alpha_best_kernel(int n, int ld_out, int first, const float* __r
     __syncthreads();
     if (take)
         for (int i = threadIdx.x; i < n; i += blockDim.x) { r_lo[t * ld_out + i] = cur_lo[t * n + i]; r_hi[t * ld_out + i] = cur_hi[t * n + i]; }
+}
+
+__global__ void abs_kernel(const float* __restrict__ a, float* __restrict__ out, size_t count) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < count; q += (size_t)gridDim.x * blockDim.x) out[q] = fabsf(a[q]);
 }
 
 __global__ void sum_kernel(const float* __restrict__ a, const float* __restrict__ b, float* __restrict__ out, size_t count) {
@@ -841,9 +870,23 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
     if (cert) {
         // certified: the radius is the rounded-up product v_1 = |W_1| sigma, widened by the centre residual e_1
         launch_cert_layer(S, C, 1, false, st, launches);
+        const float* m1 = nullptr;
+        const float* vmu = nullptr;
+        if (S->mu_cur) {
+            // non-centred boxes: mu1 = W_1 mu (FP32 product, nearest) and its rounding scale rad1 = |W_1||mu| (rounded up; the
+            // value-mode radius array is free in certified mode; the cert kernel's e / t outputs of this call go to scratch)
+            GemmArgs gm = plain_args(C, S->wp[1], S->wp[0], S->mu_cur, S->wp[0], S->Wt[1], S->wp[1], S->mu1, S->wp[1]);
+            launch_gemm<AMODE_PLAIN, EPI_STORE>(S, gm, st, launches);
+            abs_kernel<<<gs_grid((size_t)C * S->wp[0]), 256, 0, st>>>(S->mu_cur, S->mu_bar, (size_t)C * S->wp[0]);
+            dim3 grid((S->wp[1] + CJ - 1) / CJ, (C + CM - 1) / CM);
+            cert_layer_kernel<<<grid, 256, 0, st>>>(C, S->wp[1], S->wp[0], S->Wt[1], S->rowsW[1], S->bias[1], S->nomp, nullptr, S->mu_bar, S->wp[0],
+                                                   S->zhat[1], S->ahat[1], S->act, 0, S->mU[1], S->mL[1], S->rad1, S->wp[1]);
+            *launches += 2;
+            m1 = S->mu1; vmu = S->rad1;
+        }
         relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(
             S->act, C, S->w[1], S->wp[1], 1, S->use_tc ? 1 : 0, S->zhat[1], S->ahat[1], S->cv[1], S->ce[1], S->lb[1], S->ub[1], S->kU[1],
-            S->kL[1], S->gU[1], S->gL[1], S->adev[1], S->mU[1], S->mL[1]);
+            S->kL[1], S->gU[1], S->gL[1], S->adev[1], S->mU[1], S->mL[1], m1, vmu, (float)(S->wp[0] + 4) * 5.9604652e-08f * 1.000001f);
         ++*launches;
     } else {
         GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
@@ -1073,7 +1116,6 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
     if (ibp && cert) return LEB_ERR_UNSUPPORTED;                       // the rounding bookkeeping covers the back-substituted hidden bounds only
-    if (mu && cert) return LEB_ERR_UNSUPPORTED;                        // ... and centred boxes only
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
     if (tiles == 0) return LEB_OK;
@@ -1147,7 +1189,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
     // and was computed in the mode this call names (LEB_FLAG_NO_MARGIN: a value-mode state; otherwise a certified one).
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
-    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp && !mu;
+    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp;
     const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
                        S->last_cert == want_cert && S->last_ibp == ibp && S->last_mu == (mu != nullptr);
     S->last_vjp_reused = reuse;

@@ -252,3 +252,72 @@ def test_contraction_error_model(mods, path, K):
     print(f"{path} K={K}: worst observed contraction error = {worst:.3f} of the model bound")
     from parity_util import report
     report(f"contraction error model {path} K={K} (observed error / model bound)", worst)
+
+
+# ---------------------------------------------------------------------------------- certified mode on non-centred boxes
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_certified_mu_sound_and_not_much_wider(mods, dims, act, path):
+    """mu != NULL in certified mode.  The relaxation gaps are taken at the nominal pre-activation zhat(a~), which lies
+    outside a neuron's interval when |W_1 mu| exceeds its radius; the certificate clamps them (gU >= 0 >= gL keeps the gap
+    sums same-signed, which its rounding factors need), so the hidden bounds are up to ~1e-2 wider than the oracle's and
+    the later relaxations differ from the oracle's -- containment of the ORACLE's enclosure is therefore not the test here.
+    What is: strict soundness (no tolerance) of the output enclosure and of every hidden bound on 2e4 samples + sampled
+    vertices of the offset box, with J passed in FP32, and a bounded looseness against the oracle."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    mu = wl.make_mu(w, 1.5)
+    ctx = leb.context_for_workload(w)
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    N = dims[0]
+    nom, rad, mu_f = w.nom.reshape(-1, N), w.rad.reshape(-1, N), mu.reshape(-1, N)
+    J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in nom]).astype(np.float32)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path], mu=_dev(mu))
+    assert ctx.leb_domain_flag() == 0
+    clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+    hidden = [tuple(to_np(x).astype(np.float64) for x in ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])) for layer in range(1, len(dims) - 1)]
+    rng = np.random.default_rng(5)
+    for t in range(w.B * w.T):
+        a0, sg, m = nom[t].astype(np.float64), rad[t].astype(np.float64), mu_f[t].astype(np.float64)
+        X = a0[None] + m[None] + np.concatenate([rng.uniform(-1, 1, (20000, N)), rng.choice([-1.0, 1.0], (4096, N))]) * sg[None]
+        _, p, _ = O.nominal(Ws, bs, act, a0)
+        A = X.T
+        for l in range(len(Ws) - 1):
+            Z = Ws[l] @ A + bs[l][:, None]
+            assert np.all(Z.min(1) >= hidden[l][0][t]) and np.all(Z.max(1) <= hidden[l][1][t]), (dims, t, l)
+            A = O.phi(act, Z)
+        r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
+        assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, J=J32, mu=mu_f)
+    per_tile = np.array([_looseness(clo[t:t + 1], chi[t:t + 1], olo[t:t + 1], ohi[t:t + 1]) for t in range(clo.shape[0])])
+    print(f"certified mu {dims} {path}: looseness over the oracle enclosure median {np.median(per_tile):.3e} max {per_tile.max():.3e}")
+    assert np.median(per_tile) < 5e-2 and per_tile.max() < 0.25, per_tile
+    ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
+def test_certified_mu_never_below_sampled_maximum_strict(mods, path):
+    """Tiny nets, offset boxes (|mu| up to 2 sigma), >= 1e5 samples + all vertices per tile, no tolerance; J passed in FP32."""
+    leb, wl, O = mods
+    for dims, act, seed in (([3, 12, 2], 1, 1), ([4, 8, 8, 2], 2, 3), ([2, 16, 16, 2], 1, 4)):
+        w = wl.make_small_mlp(dims, act, 2, 2, seed=seed, rad_lo=0.05, rad_hi=0.4)
+        mu = wl.make_mu(w, 2.0)
+        ctx = leb.context_for_workload(w)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        N = dims[0]
+        J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in w.nom.reshape(-1, N)]).astype(np.float32)
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path], mu=_dev(mu))
+        clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+        rng = np.random.default_rng(seed)
+        verts = np.array(list(itertools.product((-1.0, 1.0), repeat=N)))
+        for t in range(w.B * w.T):
+            a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+            m = mu.reshape(-1, N)[t].astype(np.float64)
+            X = a0[None] + m[None] + np.concatenate([rng.uniform(-1, 1, (100000, N)), verts]) * sg[None]
+            _, p, _ = O.nominal(Ws, bs, act, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(act, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
+            assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
+        ctx.close()
