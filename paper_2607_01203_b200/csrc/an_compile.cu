@@ -194,11 +194,16 @@ public:
     SJet jmul(const SJet& a, const SJet& b) {
         SJet r;
         r.w = M([&] { return mul(a.w, b.w); });
-        r.wj = M([&] { return add(mul(a.wj, b.w), mul(a.w, b.wj)); });
+        // sums are emitted as running sums (t; m; t + m) so that the peephole can fuse each product into its addition
+        r.wj = M([&] { Sym t = mul(a.wj, b.w); return add(t, mul(a.w, b.wj)); });
         if (kphase) {
-            r.wk = diag ? r.wj : add(mul(a.wk, b.w), mul(a.w, b.wk));
-            Sym cross = diag ? scale(2.f, mul(a.wj, b.wj)) : add(mul(a.wj, b.wk), mul(a.wk, b.wj));
-            r.wjk = add(add(mul(a.wjk, b.w), cross), mul(a.w, b.wjk));
+            if (diag) r.wk = r.wj;
+            else { Sym t = mul(a.wk, b.w); r.wk = add(t, mul(a.w, b.wk)); }
+            Sym t;
+            if (diag) t = scale(2.f, mul(a.wj, b.wj));
+            else { t = mul(a.wj, b.wk); t = add(t, mul(a.wk, b.wj)); }
+            t = add(t, mul(a.wjk, b.w));
+            r.wjk = add(t, mul(a.w, b.wjk));
         }
         return r;
     }
@@ -210,7 +215,8 @@ public:
         if (kphase) {
             r.wk = diag ? r.wj : mul(f1, a.wk);
             Sym jk = diag ? sqr(a.wj) : mul(a.wj, a.wk);
-            r.wjk = add(mul(f2, jk), mul(f1, a.wjk));
+            Sym t = mul(f2, jk);
+            r.wjk = add(t, mul(f1, a.wjk));
         }
         return r;
     }
@@ -384,7 +390,55 @@ void model_f(Builder& B, const Model& M, JV& f) {
 struct RawSeg { std::vector<Ins> ins; std::vector<uint32_t> b; };      // ins: w0 = op, w1 = a (tagged)
 
 inline bool op_has_a(uint32_t op) { return op >= OP_ADD && op != OP_COUNT; }      // a is a slot
-inline bool op_has_b(uint32_t op) { return op == OP_ADD || op == OP_SUB || op == OP_MUL; }   // b is a slot
+inline bool op_has_b(uint32_t op) { return op == OP_ADD || op == OP_SUB || op == OP_MUL || op == OP_MULACC; }   // b is a slot
+
+// Peephole: [q; p = a * b (or c * a); s = q + p] with p used by s only and q, p, s consecutive  ->  [q; s = MULACC / SCALEACC].
+// ins: w0 = op, w1 = a; operands that are results of this list carry `tag` (tag | index).  ext[i] != 0: result i is also
+// read from outside the list (a WJ slot read by a K segment).  Both interval operations are executed unchanged inside the
+// fused instruction, so the enclosure is bit-identical; what goes is one dispatch, one slot and one ring round trip.
+void fuse_mul_add(std::vector<Ins>& ins, std::vector<uint32_t>& b, uint32_t tag, const std::vector<uint8_t>* ext,
+                  std::vector<uint32_t>* remap_out) {
+    const size_t nI = ins.size();
+    auto local = [&](uint32_t s) { return tag ? (s & tag) != 0 : true; };
+    auto idx = [&](uint32_t s) { return tag ? (s & ~tag) : s; };
+    std::vector<uint32_t> uses(nI, 0);
+    for (size_t i = 0; i < nI; ++i) {
+        const uint32_t op = ins[i].w0;
+        if (op_has_a(op) && local(ins[i].w1)) ++uses[idx(ins[i].w1)];
+        if (op_has_b(op) && local(b[i])) ++uses[idx(b[i])];
+    }
+    std::vector<Ins> o;
+    std::vector<uint32_t> ob, map(nI, 0), src;          // src: old index of each kept instruction
+    o.reserve(nI); ob.reserve(nI); src.reserve(nI);
+    auto ref = [&](uint32_t s) { return local(s) ? (tag | map[idx(s)]) : s; };
+    for (size_t i = 0; i < nI; ++i) {
+        const uint32_t op = ins[i].w0;
+        uint32_t a = ins[i].w1, bb = b[i];
+        if (op_has_a(op)) a = ref(a);
+        if (op_has_b(op)) bb = ref(bb);
+        if (op == OP_ADD && o.size() >= 2 && local(a) && local(bb)) {
+            const uint32_t last = (uint32_t)o.size() - 1;
+            uint32_t ia = idx(a), ib = idx(bb);
+            if (ib == last - 1 && ia == last) std::swap(ia, ib);             // interval addition is symmetric
+            const uint32_t pop = o[last].w0, qop = o[last - 1].w0;
+            const bool p_private = uses[src[last]] == 1 && !(ext && (*ext)[src[last]]);
+            if (ia == last - 1 && ib == last && (pop == OP_MUL || pop == OP_SCALE) && qop != OP_OUT && p_private) {
+                o[last].w0 = pop == OP_MUL ? OP_MULACC : OP_SCALEACC;
+                map[i] = last;
+                // the fused instruction now stands for s: it inherits s's uses
+                src[last] = (uint32_t)i;
+                continue;
+            }
+        }
+        map[i] = (uint32_t)o.size();
+        o.push_back(Ins{op, a});
+        ob.push_back(bb);
+        src.push_back((uint32_t)i);
+    }
+    ins.swap(o);
+    b.swap(ob);
+    if (remap_out) remap_out->swap(map);
+}
 
 }  // namespace
 
@@ -424,7 +478,7 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
         (void)wj_len0;
 
         std::vector<RawSeg> ksegs;
-        std::vector<uint8_t> wj_live(B.wj_ins.size() + 64, 0);
+        std::vector<uint8_t> wj_live(B.wj_ins.size() + 64, 0), wj_kuse(B.wj_ins.size() + 64, 0);
         std::vector<int> acc_of(n, -1);
         int n_acc = 0;
         for (int k = j; k < N; ++k) {
@@ -456,8 +510,7 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
             // ---- dead code: keep what the OUT instructions read
             const size_t nk = B.k_ins.size();
             std::vector<uint8_t> live(nk, 0);
-            if (wj_live.size() < B.wj_ins.size()) wj_live.resize(B.wj_ins.size() + 64, 0);   // constants may be added to WJ? (no: kphase emits to K)
-            auto touch = [&](uint32_t s) { if (s & KTAG) live[s & ~KTAG] = 1; else wj_live[s] = 1; };
+            auto touch = [&](uint32_t s) { if (s & KTAG) live[s & ~KTAG] = 1; else { wj_live[s] = 1; wj_kuse[s] = 1; } };
             for (size_t i = nk; i-- > 0;) {
                 const uint32_t op = B.k_ins[i].w0;
                 if (op == OP_OUT) live[i] = 1;
@@ -478,6 +531,7 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
                 if (op_has_a(op) && (seg.ins[i].w1 & KTAG)) seg.ins[i].w1 = KTAG | remap[seg.ins[i].w1 & ~KTAG];
                 if (op_has_b(op) && (seg.b[i] & KTAG)) seg.b[i] = KTAG | remap[seg.b[i] & ~KTAG];
             }
+            fuse_mul_add(seg.ins, seg.b, KTAG, nullptr, nullptr);
             ksegs.push_back(std::move(seg));
         }
         if (ksegs.empty()) continue;
@@ -490,12 +544,33 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
             if (op_has_a(op)) wj_live[B.wj_ins[i].w1] = 1;
             if (op_has_b(op)) wj_live[B.wj_b[i]] = 1;
         }
+        // compact the live WJ instructions, fuse, and keep the composed renumbering for the K segments
         std::vector<uint32_t> wremap(nw, 0);
         Task task{};
         task.j = (uint32_t)j;
         task.wj_begin = (uint32_t)T->ins.size();
         uint32_t nwj = 0;
         for (size_t i = 0; i < nw; ++i) if (wj_live[i]) wremap[i] = nwj++;
+        std::vector<Ins> wins;
+        std::vector<uint32_t> wb;
+        std::vector<uint8_t> wext;
+        wins.reserve(nwj); wb.reserve(nwj); wext.reserve(nwj);
+        for (size_t i = 0; i < nw; ++i) {
+            if (!wj_live[i]) continue;
+            const uint32_t op = B.wj_ins[i].w0;
+            uint32_t a = B.wj_ins[i].w1, b = B.wj_b[i];
+            if (op_has_a(op)) a = wremap[a];
+            if (op_has_b(op)) b = wremap[b];
+            wins.push_back(Ins{op, a});
+            wb.push_back(b);
+            wext.push_back(wj_kuse[i]);
+        }
+        {
+            std::vector<uint32_t> remap2;
+            fuse_mul_add(wins, wb, 0u, &wext, &remap2);
+            for (size_t i = 0; i < nw; ++i) if (wj_live[i]) wremap[i] = remap2[wremap[i]];
+            nwj = (uint32_t)wins.size();
+        }
         task.wj_count = nwj;
         // gradient rows: one per input coordinate this task reads
         std::vector<int> grow(N, -1);
@@ -504,12 +579,9 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
         auto is_input = [](uint32_t op) { return op == OP_BOX || op == OP_PT || op == OP_DELTA || op == OP_BOXMU || op == OP_DELTAMU; };
         uint64_t cost = 0;
         double flops = 0.0;
-        for (size_t i = 0; i < nw; ++i) {
-            if (!wj_live[i]) continue;
-            const uint32_t op = B.wj_ins[i].w0;
-            uint32_t a = B.wj_ins[i].w1, b = B.wj_b[i];
-            if (op_has_a(op)) a = wremap[a];
-            if (op_has_b(op)) b = wremap[b];
+        for (size_t i = 0; i < wins.size(); ++i) {
+            const uint32_t op = wins[i].w0;
+            uint32_t a = wins[i].w1, b = wb[i];
             if (is_input(op)) b = grad_row(a);
             T->ins.push_back(Ins{op | (a << 8), b});
             ++cost; flops += op_flops(op);

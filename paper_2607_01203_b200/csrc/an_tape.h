@@ -45,6 +45,8 @@ enum Op : uint32_t {
     OP_SIN,      // range-exact
     OP_COS,
     OP_OUT,      // acc[b & 0xffff] += a     (RD / RU);  b >> 16 = output index l (the VJP's cotangent)
+    OP_MULACC,   // d = p + a * b   p = the result of the instruction just before (slot d - 1): the product and the sum are the
+    OP_SCALEACC, // d = p + c * a   same two interval operations, fused by the compiler when the product has no other use
     OP_COUNT
 };
 
@@ -82,6 +84,8 @@ inline int op_flops(uint32_t op) {
         case OP_BOX: case OP_ADD: case OP_SUB: case OP_SCALE: case OP_ADDC: case OP_OUT: case OP_DELTAMU: return 2;
         case OP_BOXMU: return 4;
         case OP_MUL: return 14;
+        case OP_MULACC: return 16;
+        case OP_SCALEACC: return 4;
         case OP_SQR: return 5;
         case OP_CUBE: return 4;
         case OP_RECIP: return 2;

@@ -139,7 +139,7 @@ __device__ __forceinline__ void run_fwd(const uint2* __restrict__ ins, uint32_t 
             nxt = __ldg(ins + begin + base + 32 + lane);
             const uint32_t op = nxt.x & OP_MASK;
             if (op >= OP_ADD && ((nxt.x >> SRC_SHIFT) & 3u) == SRC_GLOBAL) prefetch_row(row0 + (size_t)(nxt.x >> 8) * 32);
-            if ((op == OP_ADD || op == OP_SUB || op == OP_MUL) && (nxt.y >> B_SRC_SHIFT) == SRC_GLOBAL) prefetch_row(row0 + (size_t)(nxt.y & B_MASK) * 32);
+            if ((op == OP_ADD || op == OP_SUB || op == OP_MUL || op == OP_MULACC) && (nxt.y >> B_SRC_SHIFT) == SRC_GLOBAL) prefetch_row(row0 + (size_t)(nxt.y & B_MASK) * 32);
         }
         const int m = min(32u, count - base);
         for (int i = 0; i < m; ++i, ++dst) {
@@ -149,10 +149,15 @@ __device__ __forceinline__ void run_fwd(const uint2* __restrict__ ins, uint32_t 
             if (op == OP_MUL) {
                 const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S), y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
                 r = iv_mul(x, y);
-            } else if (op == OP_SCALE) {
+            } else if (op == OP_MULACC) {
+                const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S), y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
+                const float2 p = iv_mul(x, y);
+                r = make_float2(__fadd_rd(prev.x, p.x), __fadd_ru(prev.y, p.y));
+            } else if (op == OP_SCALE || op == OP_SCALEACC) {
                 const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S);
                 const float c = as_f(w1);
                 r = c >= 0.f ? make_float2(__fmul_rd(c, x.x), __fmul_ru(c, x.y)) : make_float2(__fmul_rd(c, x.y), __fmul_ru(c, x.x));
+                if (op == OP_SCALEACC) r = make_float2(__fadd_rd(prev.x, r.x), __fadd_ru(prev.y, r.y));
             } else if (op == OP_ADD) {
                 const float2 x = fetch((w0 >> SRC_SHIFT) & 3u, a, prev, rb, S), y = fetch(w1 >> B_SRC_SHIFT, w1 & B_MASK, prev, rb, S);
                 r = make_float2(__fadd_rd(x.x, y.x), __fadd_ru(x.y, y.y));
@@ -239,8 +244,8 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
         // this chunk's primal operands towards L1 (they were written by the forward sweep, long ago)
         if ((uint32_t)base + lane < count) {
             const uint32_t op = mine.x & OP_MASK;
-            if (op == OP_MUL || op == OP_SQR || op == OP_CUBE || op == OP_SIN || op == OP_COS) prefetch_row(row0 + (size_t)(mine.x >> 8) * 32);
-            if (op == OP_MUL) prefetch_row(row0 + (size_t)(mine.y & B_MASK) * 32);
+            if (op == OP_MUL || op == OP_MULACC || op == OP_SQR || op == OP_CUBE || op == OP_SIN || op == OP_COS) prefetch_row(row0 + (size_t)(mine.x >> 8) * 32);
+            if (op == OP_MUL || op == OP_MULACC) prefetch_row(row0 + (size_t)(mine.y & B_MASK) * 32);
             if (op == OP_RECIP) prefetch_row(row0 + (size_t)(dst0 + base + lane) * 32);
         }
         nxt = make_uint2(0u, 0u);
@@ -261,7 +266,8 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
             if (w0 & OP_FAR) { const float2 g = __ldcg(ADJ + (size_t)dst * 32); d.x += g.x; d.y += g.y; }
             const float dl = d.x, dh = d.y;
             if (dl == 0.f && dh == 0.f) continue;
-            if (op == OP_MUL) {
+            if (op == OP_MUL || op == OP_MULACC) {
+                if (op == OP_MULACC) send(SRC_RING, dst - 1, dl, dh, rb, ADJ);       // the running sum passes the adjoint on
                 const uint32_t b = w1 & B_MASK, sb = w1 >> B_SRC_SHIFT;
                 const float2 x = S[(size_t)a * 32], y = S[(size_t)b * 32];
                 // lower endpoint: first minimum of (xl yl, xl yh, xh yl, xh yh), products rounded down as in the forward
@@ -284,7 +290,8 @@ __device__ __forceinline__ void run_bwd(const uint2* __restrict__ ins, uint32_t 
                 send(sb, b, ay.x, ay.y, rb, ADJ);
                 continue;
             }
-            if (op == OP_SCALE) {
+            if (op == OP_SCALE || op == OP_SCALEACC) {
+                if (op == OP_SCALEACC) send(SRC_RING, dst - 1, dl, dh, rb, ADJ);
                 const float c = as_f(w1);
                 if (c >= 0.f) send(sa, a, c * dl, c * dh, rb, ADJ);
                 else send(sa, a, c * dh, c * dl, rb, ADJ);
@@ -646,11 +653,13 @@ static leb_status ensure_tape(AnState* S, int v) {
     return LEB_OK;
 }
 
-// the task set whose longest task has about `target` instructions (targets are rounded down to powers of two, at least
-// 1024, so that only a handful of sets ever exist)
+// the task set whose longest task has about `target` instructions (targets are rounded down to (4 + m) 2^e, m < 4, at least
+// 256 -- a quarter of an octave -- so that only a handful of sets ever exist and the cut does not jump by a factor of two)
 static const DevSet* ensure_set(AnState* S, int v, uint64_t target64) {
-    uint32_t target = 1024;
+    uint32_t target = 256;
     while ((uint64_t)target * 2 <= target64 && target < 0x40000000u) target <<= 1;
+    for (uint32_t m = 3; m >= 1; --m)
+        if ((uint64_t)target + (uint64_t)m * (target / 4) <= target64) { target += m * (target / 4); break; }
     for (const DevSet& d : S->sets[v]) if (d.target == target) return &d;
     const Tape& T = S->tape[v];
     TaskSet set;
