@@ -273,6 +273,13 @@ leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, voi
  * against the model behind the certified margin. */
 leb_status leb_nn_chain_coeffs(leb_ctx* ctx, int target, float* out, void* stream);
 
+/* The Jacobian J~ the LAST leb_nn_fwd call with J == NULL subtracted in (20) PAPER.md:L209 -- the network's Jacobian at a~
+ * (eq. (7)) as the library's own chain computed it, rounding included.  The certified enclosure is an enclosure of
+ * p(a) - p(a~) - J~ (a - a~) for exactly this matrix, so a caller that linearises with it inherits the guarantee.
+ * out: device [B*T, n, N] contiguous.  LEB_ERR_STATE if no such forward is resident (B*T larger than one chunk, or the
+ * last forward was given the caller's J). */
+leb_status leb_nn_jacobian(leb_ctx* ctx, float* out, void* stream);
+
 /* State of the NN workspace (host-side query, no synchronisation): *tiles = number of tiles whose complete forward
  * state the last leb_nn_fwd / leb_vjp left resident (0: none, e.g. the batch was processed in chunks); *certified =
  * 1 if that state is a certified-mode one; *vjp_reused = 1 if the last leb_vjp(kind 1) call started from the

@@ -482,6 +482,13 @@ leb_status leb_nn_chain_coeffs(leb_ctx* c, int target, float* out, void* stream)
     return leb_nn_get_coeffs(c->nn, target, out, (cudaStream_t)stream, &c->launches);
 }
 
+leb_status leb_nn_jacobian(leb_ctx* c, float* out, void* stream) {
+    if (!c || !out) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    DeviceGuard guard(c->device);
+    return leb_nn_get_jacobian(c->nn, out, (cudaStream_t)stream, &c->launches);
+}
+
 leb_status leb_nn_state(leb_ctx* c, int* tiles, int* certified, int* vjp_reused) {
     if (!c || !tiles || !certified || !vjp_reused) return LEB_ERR_ARG;
     if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;

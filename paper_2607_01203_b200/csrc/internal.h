@@ -113,3 +113,4 @@ leb_status leb_nn_alpha(NnState*, int tiles, const float* nom, const float* rad,
 void leb_nn_query(const NnState*, int* tiles, int* certified, int* vjp_reused);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);
 leb_status leb_nn_get_coeffs(NnState*, int target, float* out, cudaStream_t st, long long* launches);
+leb_status leb_nn_get_jacobian(NnState*, float* out, cudaStream_t st, long long* launches);

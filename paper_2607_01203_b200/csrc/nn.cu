@@ -1171,6 +1171,26 @@ leb_status leb_nn_get_coeffs(NnState* S, int target, float* out, cudaStream_t st
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
 
+// the Jacobian chain rows J~ of the output target (rows [2 n, 3 n) of its Lambda_0 block): [tiles, n, N]
+__global__ void copy_jac_kernel(int tiles, int n, int rows_pad, int N, int wp0, const float* __restrict__ Lam0, float* __restrict__ out) {
+    size_t total = (size_t)tiles * n * N;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % N);
+        size_t r = q / N;
+        int i = (int)(r % n), t = (int)(r / n);
+        out[q] = Lam0[((size_t)t * rows_pad + 2 * (size_t)n + i) * wp0 + c];
+    }
+}
+
+leb_status leb_nn_get_jacobian(NnState* S, float* out, cudaStream_t st, long long* launches) {
+    if (S->last_tiles <= 0 || S->chunk <= 0 || !S->last_with_jac) return LEB_ERR_STATE;
+    const int n = S->w[S->L];
+    copy_jac_kernel<<<gs_grid((size_t)S->last_tiles * n * S->w[0]), 256, 0, st>>>(S->last_tiles, n, S->rows_pad[S->L], S->w[0], S->wp[0],
+                                                                               S->Lam[S->L][0], out);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
 // ------------------------------------------------------------------------------------------
 // VJP: forward of the chunk (all coefficient blocks kept), then the reverse sweep
 // ------------------------------------------------------------------------------------------

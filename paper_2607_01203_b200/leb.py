@@ -28,7 +28,7 @@ FLAG_IBP_HIDDEN = 32
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_jacobian", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
 
@@ -328,6 +328,12 @@ class Context:
     def leb_nn_chain_coeffs(self, target: int, tiles: int, rows: int, N: int):
         out = torch.empty((tiles, 2, rows, N), dtype=torch.float32, device=torch.device("cuda", self.device))
         _chk(self.lib.leb_nn_chain_coeffs(self._ctx, int(target), _ptr(out), _stream_ptr(self.device)), "leb_nn_chain_coeffs")
+        return out
+
+    def leb_nn_jacobian(self, tiles: int, n: int, N: int):
+        """J~ of the last leb_nn_fwd(J=None): [tiles, n, N]"""
+        out = torch.empty((tiles, n, N), dtype=torch.float32, device=torch.device("cuda", self.device))
+        _chk(self.lib.leb_nn_jacobian(self._ctx, _ptr(out), _stream_ptr(self.device)), "leb_nn_jacobian")
         return out
 
     def leb_nn_state(self):

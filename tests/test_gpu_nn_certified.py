@@ -98,6 +98,42 @@ def test_certified_never_below_sampled_maximum_strict(mods, path):
 
 
 @pytest.mark.parametrize("path", list(PATHS))
+def test_certified_is_relative_to_the_readable_jacobian_strict(mods, path):
+    """J = NULL: the enclosure is of p(a) - p(a~) - J~ (a - a~) with J~ the library's own chain rows, rounding included.
+    leb_nn_jacobian returns that matrix; it matches the FP64 Jacobian to FP32 rounding, and the sampled remainder taken
+    with exactly J~ lies inside the certified enclosure with no tolerance (>= 1e5 samples + all vertices per tile)."""
+    leb, wl, O = mods
+    for dims, act, seed in (([3, 12, 2], 1, 11), ([4, 10, 3], 2, 12), ([4, 8, 8, 2], 2, 13), ([2, 16, 16, 2], 1, 14)):
+        w = wl.make_small_mlp(dims, act, 2, 2, seed=seed, rad_lo=0.05, rad_hi=0.4)
+        ctx = leb.context_for_workload(w)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        N = dims[0]
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+        Jt = to_np(ctx.leb_nn_jacobian(w.B * w.T, w.n, N)).astype(np.float64)
+        clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+        rng = np.random.default_rng(seed)
+        verts = np.array(list(itertools.product((-1.0, 1.0), repeat=N)))
+        for t in range(w.B * w.T):
+            a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+            _, p, J64 = O.nominal(Ws, bs, act, a0)
+            assert np.abs(Jt[t] - J64).max() <= 1e-5 * np.abs(J64).max() + 1e-7, (dims, t)
+            U = np.concatenate([rng.uniform(-1, 1, (100000, N)), verts])
+            X = a0[None, :] + U * sg[None, :]
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(act, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ Jt[t].T
+            assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
+        # a forward that was given the caller's J leaves no J~ to read
+        J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in w.nom.reshape(-1, N)]).astype(np.float32)
+        ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path])
+        with pytest.raises(leb.LebError) as e:
+            ctx.leb_nn_jacobian(w.B * w.T, w.n, N)
+        assert e.value.status == leb.LEB_ERR_STATE
+        ctx.close()
+
+
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("cfg", [3, 5])
 def test_certified_config_sampled_tiles(mods, cfg, path):
     """Configs 3 and 5 at BASELINE size in the launch configuration bench.py uses; oracle on sampled tiles."""
