@@ -22,18 +22,21 @@ import numpy as np
 from oracle import pbh_oracle as P
 
 
+def sub_box_offsets(splits):
+    """c_p = -1 + (2 q_p + 1) / splits: centre of part q of [-1, 1] cut into `splits` equal parts, per coordinate; [P, N],
+    sub-box order = row-major over the coordinates, first coordinate slowest."""
+    splits = np.asarray(splits, dtype=np.int64)
+    return np.array([-1.0 + (2.0 * np.array(q, dtype=np.float64) + 1.0) / splits
+                     for q in itertools.product(*[range(int(s)) for s in splits])])
+
+
 def sub_boxes(rad, mu, splits):
-    """Offsets and radii of the grid of sub-boxes of one tile: arrays [P, N]; sub-box order = row-major over the
-    coordinates with splits > 1, first such coordinate slowest."""
+    """Offsets and radii of the grid of sub-boxes of one tile: arrays [P, N]."""
     rad = np.asarray(rad, dtype=np.float64)
     mu = np.zeros_like(rad) if mu is None else np.asarray(mu, dtype=np.float64)
     splits = np.asarray(splits, dtype=np.int64)
-    mus, rads = [], []
-    for q in itertools.product(*[range(int(s)) for s in splits]):
-        q = np.array(q, dtype=np.float64)
-        rads.append(rad / splits)
-        mus.append(mu + rad * (-1.0 + (2.0 * q + 1.0) / splits))
-    return np.array(mus), np.array(rads)
+    c = sub_box_offsets(splits)
+    return mu[None] + rad[None] * c, np.repeat((rad / splits)[None], c.shape[0], 0)
 
 
 def partition(spec, nom, rad, splits, mu=None):
@@ -50,6 +53,38 @@ def partition(spec, nom, rad, splits, mu=None):
         status |= st
         lo[t], hi[t] = l.min(0), h.max(0)
     return lo, hi, status
+
+
+def partition_vjp(spec, nom, rad, splits, g_lo, g_hi, mu=None):
+    """VJP of partition(): the hull takes, per output, the lower bound of ONE sub-box (the first minimum in sub-box order)
+    and the upper bound of one (the first maximum), so the cotangent of r_lo_i goes to that sub-box's lower bound only
+    (reading R20: derivative of the selected branch).  The sub-box inputs are nom (shared), rad_p = rad / splits and
+    mu_p = mu + rad * c_p, c_p = -1 + (2 q_p + 1) / splits, so
+        d/dnom = sum_p gnom_p,   d/drad = sum_p (grad_p / splits + gmu_p * c_p),   d/dmu = sum_p gmu_p.
+    Returns grad [tiles, 3N] (nom | rad | mu)."""
+    nom = np.asarray(nom, dtype=np.float64).reshape(-1, spec.N)
+    rad = np.asarray(rad, dtype=np.float64).reshape(-1, spec.N)
+    mu = None if mu is None else np.asarray(mu, dtype=np.float64).reshape(-1, spec.N)
+    g_lo = np.asarray(g_lo, dtype=np.float64).reshape(-1, spec.n)
+    g_hi = np.asarray(g_hi, dtype=np.float64).reshape(-1, spec.n)
+    splits = np.asarray(splits, dtype=np.int64)
+    N = spec.N
+    out = np.zeros((nom.shape[0], 3 * N))
+    for t in range(nom.shape[0]):
+        mus, rads = sub_boxes(rad[t], None if mu is None else mu[t], splits)
+        P_ = mus.shape[0]
+        noms = np.repeat(nom[t][None], P_, 0)
+        l, h, _ = P.pbh(spec, noms, rads, mu=mus)
+        sel_lo, sel_hi = l.argmin(0), h.argmax(0)            # first extremum in sub-box order
+        gl, gh = np.zeros((P_, spec.n)), np.zeros((P_, spec.n))
+        gl[sel_lo, np.arange(spec.n)] = g_lo[t]
+        gh[sel_hi, np.arange(spec.n)] = g_hi[t]
+        g, _ = P.pbh_vjp(spec, noms, rads, gl, gh, mu=mus)
+        c = sub_box_offsets(splits)
+        out[t, :N] = g[:, :N].sum(0)
+        out[t, N:2 * N] = (g[:, N:2 * N] / splits[None] + g[:, 2 * N:] * c).sum(0)
+        out[t, 2 * N:] = g[:, 2 * N:].sum(0)
+    return out
 
 
 def width_and_grad(spec, nom, centre, rad):

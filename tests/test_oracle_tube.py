@@ -171,3 +171,40 @@ def test_pgd_never_worse_and_flat_for_constant_hessian():
     w_c = R.width_and_grad(sspec, c2, c2, r2)[0]
     w_off = R.width_and_grad(sspec, c2 + 0.3 * r2, c2, r2)[0]
     assert np.all(w_off > w_c)
+
+
+def test_partition_vjp_matches_central_differences():
+    """partition_vjp against central differences of partition() itself in every input direction (nom, rad, mu) with random
+    cotangents; directions on which the selected sub-box changes within the step (a kink of the hull) are skipped, and
+    most must remain.  One part reduces to the plain VJP."""
+    w = wl.make_config(2, B=1, T=2)
+    spec = P.spec_from_workload(w)
+    N, n = w.N, w.n
+    rng = np.random.default_rng(9)
+    nom, rad = w.nom.reshape(-1, N).astype(float), 4.0 * w.rad.reshape(-1, N).astype(float)
+    mu = rad * rng.uniform(-0.8, 0.8, rad.shape)
+    g_lo, g_hi = rng.normal(size=(2, n)), rng.normal(size=(2, n))
+    g1 = R.partition_vjp(spec, nom, rad, np.ones(N, dtype=int), g_lo, g_hi, mu=mu)
+    g0, _ = P.pbh_vjp(spec, nom, rad, g_lo, g_hi, mu=mu)
+    assert np.allclose(g1, g0, rtol=1e-13, atol=1e-15)
+    splits = np.ones(N, dtype=int)
+    splits[[3, 4, 12]] = (2, 3, 2)
+    g = R.partition_vjp(spec, nom, rad, splits, g_lo, g_hi, mu=mu)
+
+    def val(a, r, m):
+        lo, hi, _ = R.partition(spec, a, r, splits, mu=m)
+        return (g_lo * lo + g_hi * hi).sum(1)
+
+    h, ok = 1e-6, 0
+    for d in range(3 * N):
+        e = np.zeros((2, 3 * N))
+        e[:, d] = h
+        args_p = (nom + e[:, :N], rad + e[:, N:2 * N], mu + e[:, 2 * N:])
+        args_m = (nom - e[:, :N], rad - e[:, N:2 * N], mu - e[:, 2 * N:])
+        fp, fm, f0 = val(*args_p), val(*args_m), val(nom, rad, mu)
+        for t in range(2):
+            if abs((fp[t] - f0[t]) - (f0[t] - fm[t])) > 1e-3 * abs(fp[t] - fm[t]) + 1e-13:
+                continue                                     # a kink inside the step
+            assert abs((fp[t] - fm[t]) / (2 * h) - g[t, d]) <= 1e-5 * abs(g[t, d]) + 1e-6 * np.abs(g[t]).max(), (t, d)
+            ok += 1
+    assert ok >= 5 * N
