@@ -149,10 +149,18 @@ leb_status leb_analytic_fwd(leb_ctx* ctx, int B, int T, const float* nom, const 
  * parts along coordinate g (HOST array of N ints; at most 65536 sub-boxes per tile); every sub-box is bounded as a
  * non-centred box about the same nominal point and the hull of the sub-box enclosures is returned.  Sound (every point of
  * the box lies in a sub-box; FP32 sub-boxes are padded to overlap) and never wider than leb_analytic_fwd's enclosure
- * (inclusion isotonicity).  Forward only.  Other arguments as leb_analytic_fwd. */
+ * (inclusion isotonicity).  Other arguments as leb_analytic_fwd. */
 leb_status leb_analytic_partition_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad, const float* mu,
                                       int ld_in, const int* splits, float* r_lo, float* r_hi, int ld_out,
                                       unsigned flags, void* stream);
+
+/* VJP of leb_analytic_partition_fwd: the hull takes each bound from one sub-box (the first minimum / maximum in sub-box
+ * order, reading R20), so the cotangent of an output goes to that sub-box's bound, through the ordinary reverse sweep, and
+ * back through the sub-box construction (radius sigma / splits, offset mu + sigma c_p) to nom, rad and mu.  Recomputes the
+ * sub-box forward (stateless).  g_lo, g_hi: [B, T, ld_out]; grad_nom, grad_rad (, grad_mu when mu != NULL): [B, T, ld_in]. */
+leb_status leb_analytic_partition_vjp(leb_ctx* ctx, int B, int T, const float* nom, const float* rad, const float* mu,
+                                      int ld_in, const int* splits, const float* g_lo, const float* g_hi, int ld_out,
+                                      float* grad_nom, float* grad_rad, float* grad_mu, unsigned flags, void* stream);
 
 /* Nominal-point refinement by projected gradient descent (Sec. IV-D, Table II).  The box of every tile is
  * FIXED (centre, rad); the nominal point a~ moves inside |a~ - centre| <= eps (componentwise) so as to shrink the total

@@ -462,6 +462,57 @@ __global__ void hull_kernel(size_t tiles, int P, int n, int ld_out, const float*
 }
 
 // PGD: mu = centre - nom
+// VJP of the hull: the cotangent of r_lo[l] goes to the sub-box with the first minimum, that of r_hi[l] to the first maximum
+__global__ void hull_select_kernel(size_t tiles, int P, int n, int ld_out, const float* __restrict__ lo_x, const float* __restrict__ hi_x,
+                                   const float* __restrict__ g_lo, const float* __restrict__ g_hi, float* __restrict__ glo_x,
+                                   float* __restrict__ ghi_x) {
+    const size_t total = tiles * (size_t)n;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t t = idx / n;
+        const int l = (int)(idx - t * n);
+        float lo = INFINITY, hi = -INFINITY;
+        int pl = 0, ph = 0;
+        for (int p = 0; p < P; ++p) {
+            const size_t o = (t * P + p) * (size_t)n + l;
+            if (lo_x[o] < lo) { lo = lo_x[o]; pl = p; }
+            if (hi_x[o] > hi) { hi = hi_x[o]; ph = p; }
+        }
+        const float gl = g_lo[t * ld_out + l], gh = g_hi[t * ld_out + l];
+        for (int p = 0; p < P; ++p) {
+            const size_t o = (t * P + p) * (size_t)n + l;
+            glo_x[o] = p == pl ? gl : 0.f;
+            ghi_x[o] = p == ph ? gh : 0.f;
+        }
+    }
+}
+// chain the sub-box gradients back through subbox_kernel's formulas, sub-boxes added in ascending order (reproducible)
+__global__ void subbox_vjp_kernel(size_t tiles, int P, int N, int ld_in, const int* __restrict__ splits, const int* __restrict__ strides,
+                                  const float* __restrict__ mu, const float* __restrict__ gn_x, const float* __restrict__ gr_x,
+                                  const float* __restrict__ gm_x, float* __restrict__ grad_nom, float* __restrict__ grad_rad,
+                                  float* __restrict__ grad_mu) {
+    const size_t total = tiles * (size_t)N;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const size_t t = idx / N;
+        const int g = (int)(idx - t * N);
+        const int s = splits[g], stride = strides[g];
+        const float inv = 1.f / (float)s, eps4 = 4.f * 1.1920929e-07f;
+        const float m = mu ? mu[t * ld_in + g] : 0.f, sg = (m > 0.f) - (m < 0.f);
+        float an = 0.f, ar = 0.f, am = 0.f;
+        for (int p = 0; p < P; ++p) {
+            const size_t o = (t * P + p) * (size_t)N + g;
+            const float gn = gn_x[o], gr = gr_x[o], gm = gm_x[o];
+            an += gn;
+            if (s == 1) { ar += gr; am += gm; continue; }
+            const int q = (p / stride) % s;
+            ar += gr * (inv + eps4) + gm * fmaf((float)(2 * q + 1), inv, -1.f);
+            am += gm + gr * eps4 * sg;
+        }
+        grad_nom[t * ld_in + g] = an;
+        grad_rad[t * ld_in + g] = ar;
+        if (grad_mu) grad_mu[t * ld_in + g] = am;
+    }
+}
+
 __global__ void pgd_mu_kernel(size_t count, const float* __restrict__ centre, const float* __restrict__ nom, float* __restrict__ mu) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (size_t)gridDim.x * blockDim.x) mu[i] = centre[i] - nom[i];
 }
@@ -772,11 +823,9 @@ static unsigned gs_blocks(size_t work) { return (unsigned)std::min<size_t>((work
 
 // input-domain partitioning: hull of the bounds of the grid of sub-boxes, every sub-box a non-centred box
 // about the same nominal point
-leb_status leb_an_partition(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
-                            const int* splits_host, float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
-                            long long* launches, LebProf* prof) {
-    if (tiles == 0) return LEB_OK;
-    const int N = S->model.N, n = S->model.n;
+// the (splits | strides) table of a partition on the device; *P_out = sub-boxes per tile
+static leb_status upload_splits(AnState* S, int tiles, const int* splits_host, long long* P_out, cudaStream_t st) {
+    const int N = S->model.N;
     std::vector<int> tab(2 * (size_t)N);
     long long P = 1;
     for (int g = N - 1; g >= 0; --g) {
@@ -794,6 +843,18 @@ leb_status leb_an_partition(AnState* S, int tiles, const float* nom, const float
     }
     cudaStreamSynchronize(st);        // the table of a previous call may still be in use
     if (cudaMemcpy(S->d_splits, tab.data(), 2 * (size_t)N * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) return LEB_ERR_CUDA;
+    *P_out = P;
+    return LEB_OK;
+}
+
+leb_status leb_an_partition(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                            const int* splits_host, float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
+                            long long* launches, LebProf* prof) {
+    if (tiles == 0) return LEB_OK;
+    const int N = S->model.N, n = S->model.n;
+    long long P = 1;
+    leb_status us = upload_splits(S, tiles, splits_host, &P, st);
+    if (us != LEB_OK) return us;
     const size_t xt = (size_t)tiles * (size_t)P;
     float *nx = scratch(S, 0, xt * N), *rx = scratch(S, 1, xt * N), *mx = scratch(S, 2, xt * N), *lx = scratch(S, 3, xt * n), *hx = scratch(S, 4, xt * n);
     if (!nx || !rx || !mx || !lx || !hx) return LEB_ERR_NOMEM;
@@ -802,6 +863,34 @@ leb_status leb_an_partition(AnState* S, int tiles, const float* nom, const float
     leb_status es = an_run(S, false, (int)xt, nx, rx, mx, N, lx, hx, nullptr, nullptr, n, nullptr, nullptr, nullptr, domain_flag, st, launches, prof);
     if (es != LEB_OK) return es;
     hull_kernel<<<gs_blocks((size_t)tiles * n), 256, 0, st>>>((size_t)tiles, (int)P, n, ld_out, lx, hx, r_lo, r_hi);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+// VJP of the partitioned bound: sub-boxes forward, the hull's selection, the ordinary VJP on the sub-boxes with the selected
+// cotangents, and the chain rule of the sub-box construction
+leb_status leb_an_partition_vjp(AnState* S, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                                const int* splits_host, const float* g_lo, const float* g_hi, int ld_out, float* grad_nom,
+                                float* grad_rad, float* grad_mu, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof) {
+    if (tiles == 0) return LEB_OK;
+    const int N = S->model.N, n = S->model.n;
+    long long P = 1;
+    leb_status us = upload_splits(S, tiles, splits_host, &P, st);
+    if (us != LEB_OK) return us;
+    const size_t xt = (size_t)tiles * (size_t)P;
+    float *nx = scratch(S, 0, xt * N), *rx = scratch(S, 1, xt * N), *mx = scratch(S, 2, xt * N), *lx = scratch(S, 3, xt * n), *hx = scratch(S, 4, xt * n);
+    float *gnx = scratch(S, 5, xt * N), *grx = scratch(S, 6, xt * N), *glx = scratch(S, 7, xt * n), *ghx = scratch(S, 8, xt * n), *gmx = scratch(S, 9, xt * N);
+    if (!nx || !rx || !mx || !lx || !hx || !gnx || !grx || !glx || !ghx || !gmx) return LEB_ERR_NOMEM;
+    subbox_kernel<<<gs_blocks(xt * N), 256, 0, st>>>((size_t)tiles, (int)P, N, ld_in, S->d_splits, S->d_splits + N, nom, rad, mu, nx, rx, mx);
+    ++*launches;
+    leb_status es = an_run(S, false, (int)xt, nx, rx, mx, N, lx, hx, nullptr, nullptr, n, nullptr, nullptr, nullptr, domain_flag, st, launches, prof);
+    if (es != LEB_OK) return es;
+    hull_select_kernel<<<gs_blocks((size_t)tiles * n), 256, 0, st>>>((size_t)tiles, (int)P, n, ld_out, lx, hx, g_lo, g_hi, glx, ghx);
+    ++*launches;
+    es = an_run(S, true, (int)xt, nx, rx, mx, N, nullptr, nullptr, glx, ghx, n, gnx, grx, gmx, domain_flag, st, launches, prof);
+    if (es != LEB_OK) return es;
+    subbox_vjp_kernel<<<gs_blocks((size_t)tiles * N), 256, 0, st>>>((size_t)tiles, (int)P, N, ld_in, S->d_splits, S->d_splits + N, mu, gnx, grx, gmx,
+                                                                  grad_nom, grad_rad, grad_mu);
     ++*launches;
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }

@@ -192,6 +192,39 @@ leb_status leb_analytic_partition_fwd(leb_ctx* c, int B, int T, const float* nom
     return ok ? LEB_OK : LEB_ERR_CUDA;
 }
 
+leb_status leb_analytic_partition_vjp(leb_ctx* c, int B, int T, const float* nom, const float* rad, const float* mu, int ld_in,
+                                      const int* splits, const float* g_lo, const float* g_hi, int ld_out, float* grad_nom,
+                                      float* grad_rad, float* grad_mu, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || !splits) return LEB_ERR_ARG;
+    if (!leb_an_ready(c->an)) return LEB_ERR_STATE;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!nom || !rad || !g_lo || !g_hi || !grad_nom || !grad_rad || (mu && !grad_mu)) return LEB_ERR_ARG;
+    leb_status s = check_traj(B, T, leb_an_N(c->an), leb_an_n(c->an), ld_in, ld_out);
+    if (s != LEB_OK) return s;
+    if (!al4(nom) || !al4(rad) || !al4(mu) || !al4(g_lo) || !al4(g_hi) || !al4(grad_nom) || !al4(grad_rad) || !al4(grad_mu)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool host = flags & LEB_FLAG_HOST_IO;
+    const size_t tiles = (size_t)B * T;
+    bool ok = true;
+    const float* d_nom = in_ptr(c, 0, nom, tiles * ld_in, host, st, &ok);
+    const float* d_rad = in_ptr(c, 1, rad, tiles * ld_in, host, st, &ok);
+    const float* d_glo = in_ptr(c, 2, g_lo, tiles * ld_out, host, st, &ok);
+    const float* d_ghi = in_ptr(c, 3, g_hi, tiles * ld_out, host, st, &ok);
+    const float* d_mu = in_ptr(c, 4, mu, tiles * ld_in, host, st, &ok);
+    float* d_gn = out_ptr(c, 6, grad_nom, tiles * ld_in, host, &ok);
+    float* d_gr = out_ptr(c, 7, grad_rad, tiles * ld_in, host, &ok);
+    float* d_gm = out_ptr(c, 5, (mu ? grad_mu : nullptr), tiles * ld_in, host, &ok);
+    if (!ok) return LEB_ERR_NOMEM;
+    s = leb_an_partition_vjp(c->an, (int)tiles, d_nom, d_rad, d_mu, ld_in, splits, d_glo, d_ghi, ld_out, d_gn, d_gr, d_gm, c->domain_flag, st,
+                             &c->launches, &c->prof);
+    if (s != LEB_OK) return s;
+    out_copy(grad_nom, d_gn, tiles * ld_in, host, st, &ok);
+    out_copy(grad_rad, d_gr, tiles * ld_in, host, st, &ok);
+    if (mu) out_copy(grad_mu, d_gm, tiles * ld_in, host, st, &ok);
+    return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
 leb_status leb_analytic_pgd(leb_ctx* c, int B, int T, const float* centre, const float* rad, const float* eps, int ld_in, int steps,
                             float lr, float* nom, float* width0, float* width, unsigned flags, void* stream) {
     if (!c || B < 0 || T < 0 || steps < 0 || !(lr >= 0.f)) return LEB_ERR_ARG;

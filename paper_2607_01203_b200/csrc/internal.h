@@ -72,6 +72,9 @@ leb_status leb_an_vjp(AnState*, int tiles, const float* nom, const float* rad, c
 leb_status leb_an_partition(AnState*, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
                             const int* splits_host, float* r_lo, float* r_hi, int ld_out, int* domain_flag, cudaStream_t st,
                             long long* launches, LebProf* prof);
+leb_status leb_an_partition_vjp(AnState*, int tiles, const float* nom, const float* rad, const float* mu, int ld_in,
+                                const int* splits_host, const float* g_lo, const float* g_hi, int ld_out, float* grad_nom,
+                                float* grad_rad, float* grad_mu, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
 leb_status leb_an_pgd(AnState*, int tiles, const float* centre, const float* rad, const float* eps, int ld_in, int steps, float lr,
                       float* nom, float* w0, float* wbest, int* domain_flag, cudaStream_t st, long long* launches, LebProf* prof);
 void leb_an_stats(const AnState*, double* flops_fwd, long long* ins_fwd, long long* tape_ins, int* ntasks, int* max_slots);

@@ -27,7 +27,7 @@ FLAG_IBP_HIDDEN = 32
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
-    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
+    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_partition_vjp", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
     "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_jacobian", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
@@ -188,6 +188,20 @@ class Context:
         _chk(self.lib.leb_analytic_partition_fwd(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), ld_in, sp, _ptr(r_lo), _ptr(r_hi),
                                                  self.n, ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_partition_fwd")
         return r_lo, r_hi
+
+    def leb_analytic_partition_vjp(self, nom, rad, splits, g_lo, g_hi, mu=None, flags: int = 0):
+        """VJP of leb_analytic_partition_fwd; returns (grad_nom, grad_rad, grad_mu or None)."""
+        _check_f32(nom, rad, mu, g_lo, g_hi)
+        B, T, ld_in = self._bt(nom)
+        host = bool(flags & FLAG_HOST_IO)
+        grad_nom = self._out(nom, (B, T, ld_in), host)
+        grad_rad = self._out(nom, (B, T, ld_in), host)
+        grad_mu = self._out(nom, (B, T, ld_in), host) if mu is not None else None
+        sp = (ctypes.c_int * self.N)(*[int(x) for x in splits])
+        _chk(self.lib.leb_analytic_partition_vjp(self._ctx, B, T, _ptr(nom), _ptr(rad), _ptr(mu), ld_in, sp, _ptr(g_lo), _ptr(g_hi),
+                                                 int(g_lo.shape[2]), _ptr(grad_nom), _ptr(grad_rad), _ptr(grad_mu),
+                                                 ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_analytic_partition_vjp")
+        return grad_nom, grad_rad, grad_mu
 
     def leb_analytic_pgd(self, centre, rad, eps, nom0, steps: int, lr: float, flags: int = 0):
         """PGD refinement of the nominal point; returns (best nominal points, initial widths, best widths)."""

@@ -198,3 +198,54 @@ def test_pgd_matches_oracle(mods):
     lo, hi = ctx.leb_analytic_fwd(best, _dev(rad), mu=mu)
     assert np.allclose(to_np((hi - lo).sum(-1)).reshape(-1), gwb, rtol=1e-5)
     ctx.close()
+
+
+@pytest.mark.gpu
+def test_partition_vjp_matches_oracle(mods):
+    """leb_analytic_partition_vjp against the oracle's partition_vjp, centred and offset boxes.  Where two sub-boxes give the
+    same extremal bound to within 1e-5 the hull's selection is not unique in FP32 (reading R20: several results are correct):
+    those outputs get a zero cotangent on both sides.  One part per coordinate = the ordinary VJP, bit for bit."""
+    from parity_util import assert_grad_dirs_close
+    leb, wl, P, R, _ = mods
+    w = wl.make_config(2, B=2, T=3)
+    spec = P.spec_from_workload(w)
+    N, n = w.N, w.n
+    rad = (4.0 * w.rad).astype(np.float32)
+    splits = np.ones(N, dtype=int)
+    splits[[3, 4, 12]] = (2, 3, 2)
+    ctx = leb.context_for_workload(w)
+    rng = np.random.default_rng(21)
+    for mu in (None, wl.make_mu(w, 0.8)):
+        g_lo = rng.normal(size=(w.B, w.T, n)).astype(np.float32)
+        g_hi = rng.normal(size=(w.B, w.T, n)).astype(np.float32)
+        nom64, rad64 = w.nom.reshape(-1, N).astype(np.float64), rad.reshape(-1, N).astype(np.float64)
+        mu64 = None if mu is None else mu.reshape(-1, N).astype(np.float64)
+        skipped = 0
+        for t in range(w.B * w.T):
+            mus, rads = R.sub_boxes(rad64[t], None if mu64 is None else mu64[t], splits)
+            l, h, _ = P.pbh(spec, np.repeat(nom64[t][None], mus.shape[0], 0), rads, mu=mus)
+            # near-tie: some sub-box bound differs from the extremum, but by no more than the parity tolerance (exactly equal
+            # bounds -- an output that does not depend on the split coordinates -- select the first sub-box on both sides)
+            dl, dh = l - l.min(0)[None], h.max(0)[None] - h
+            tie_lo = ((dl > 0) & (dl <= 1e-5 * np.abs(l.min(0))[None] + 1e-9)).any(0)
+            tie_hi = ((dh > 0) & (dh <= 1e-5 * np.abs(h.max(0))[None] + 1e-9)).any(0)
+            g_lo.reshape(-1, n)[t][tie_lo] = 0.0
+            g_hi.reshape(-1, n)[t][tie_hi] = 0.0
+            skipped += int(tie_lo.sum() + tie_hi.sum())
+        assert skipped < 0.3 * 2 * n * w.B * w.T
+        gn, gr, gm = ctx.leb_analytic_partition_vjp(_dev(w.nom), _dev(rad), splits, _dev(g_lo), _dev(g_hi), None if mu is None else _dev(mu))
+        ref = R.partition_vjp(spec, nom64, rad64, splits, g_lo.reshape(-1, n), g_hi.reshape(-1, n), mu=mu64)
+        got = np.concatenate([to_np(gn).reshape(-1, N), to_np(gr).reshape(-1, N),
+                              to_np(gm).reshape(-1, N) if gm is not None else np.zeros((w.B * w.T, N))], 1)
+        if mu is None:
+            ref = ref.copy()
+            ref[:, 2 * N:] = 0.0                             # no grad_mu is returned for a centred box
+        assert_grad_dirs_close(got, ref, np.abs(ref).max(1), f"partition VJP mu={'yes' if mu is not None else 'no'}")
+    ones = np.ones(N, dtype=int)
+    g_lo, g_hi = _dev(rng.normal(size=(w.B, w.T, n)).astype(np.float32)), _dev(rng.normal(size=(w.B, w.T, n)).astype(np.float32))
+    mu = _dev(wl.make_mu(w, 0.8))
+    a = ctx.leb_analytic_partition_vjp(_dev(w.nom), _dev(rad), ones, g_lo, g_hi, mu)
+    b = ctx.leb_vjp_mu(0, _dev(w.nom), _dev(rad), mu, g_lo, g_hi)
+    for x, y in zip(a, b):
+        assert torch.equal(x, y)
+    ctx.close()
