@@ -51,7 +51,7 @@ typedef enum {
     LEB_ERR_SHAPE = 2,       /* ld too small, model/shape mismatch */
     LEB_ERR_ALIGN = 3,       /* pointer not 4-byte aligned */
     LEB_ERR_DOMAIN = 4,      /* reported by leb_domain_flag(): some tile hit a domain error */
-    LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048 or with CROWN-IBP */
+    LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048 */
     LEB_ERR_CUDA = 6,
     LEB_ERR_NOMEM = 7,
     LEB_ERR_STATE = 8        /* model not set before the call that needs it */
@@ -105,8 +105,9 @@ enum {
                                   (tcgen05.mma.cta_group::2, nn_gemm_tc2.cuh, the default); same results bit for bit */
     LEB_FLAG_IBP_HIDDEN = 32u, /* NN: CROWN-IBP -- the bounds of hidden layers 2..L-1 by interval propagation of the previous
                                   layer's bounds instead of back-substitution (about 4x fewer flops at config 5, looser
-                                  bounds); the output is back-substituted as always.  Value mode only: without
-                                  LEB_FLAG_NO_MARGIN the call returns LEB_ERR_UNSUPPORTED.  leb_vjp takes the same flag. */
+                                  bounds); the output is back-substituted as always.  Certified mode: the interval
+                                  propagation is the non-centred layer-1 formula applied to the activation deviations,
+                                  every |W| product rounded up.  leb_vjp takes the same flag. */
     LEB_FLAG_REUSE_FWD = 8u  /* leb_vjp(kind 1) becomes STATEFUL: the caller states that (nom, rad) are those of the previous
                                 leb_nn_fwd call on this context (J == NULL).  If the workspace still holds that call's complete
                                 forward state (the batch fitted one chunk) AND that state was computed in the mode this

@@ -55,6 +55,7 @@ struct NnState {
     std::vector<void*> allocs;
     float *nomp = nullptr, *radp = nullptr, *rad1 = nullptr;
     float *mup = nullptr, *mu1 = nullptr, *mu_bar = nullptr;   // non-centred boxes: padded mu, W_1 mu, and its adjoint
+    float *ibp_c = nullptr, *ibp_r = nullptr, *ibp_a = nullptr, *ibp_m = nullptr, *ibp_vm = nullptr;   // certified CROWN-IBP scratch
     float* alpha[kMaxLayers] = {nullptr};                      // optimisable lower ReLU slopes (leb_nn_alpha_fwd), [chunk x wp[l]]
     int alpha_mode = 0;                                        // 0 off, 1 forward writes the adaptive default, 2 forward reads alpha
     std::vector<void*> alpha_scratch; size_t alpha_scratch_tiles = 0;
@@ -572,6 +573,22 @@ __global__ void ibp_dev_kernel(int act, int tiles, int w_valid, int wp, const fl
     }
 }
 
+// certified CROWN-IBP: rigorous centre / radius of the activation deviation phi(z) - ahat on [l, u] (phi monotone):
+// [phi(l) - ahat, phi(u) - ahat] is contained in dc -+ dr with dc, dr as stored (dr rounded up; libm within 1e-15)
+__global__ void ibp_dev_cert_kernel(int act, int tiles, int w_valid, int wp, const float* __restrict__ ahat, const float* __restrict__ lb,
+                                    const float* __restrict__ ub, float* __restrict__ dc, float* __restrict__ dr, float* __restrict__ da) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(q % wp);
+        if (c >= w_valid) { dc[q] = 0.f; dr[q] = 0.f; da[q] = 0.f; continue; }
+        const double a = (double)ahat[q];
+        const double lo = act_f(act, (double)lb[q]) - a - 1e-15, hi = act_f(act, (double)ub[q]) - a + 1e-15;
+        const float m = (float)(0.5 * (lo + hi));
+        dc[q] = m;
+        dr[q] = __double2float_ru(fmax(hi - (double)m, (double)m - lo));
+        da[q] = fabsf(m);
+    }
+}
 __global__ void ibp_bounds_kernel(int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ zc,
                                   const float* __restrict__ zr, float* __restrict__ lb, float* __restrict__ ub) {
     size_t total = (size_t)tiles * wp;
@@ -797,6 +814,11 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
     S->mup = F((size_t)C * S->wp[0]);
     S->mu1 = F((size_t)C * S->wp[1]);
     S->mu_bar = F((size_t)C * S->wp[0]);
+    {
+        int mw = 0;
+        for (int l = 1; l < L; ++l) mw = std::max(mw, S->wp[l]);
+        for (float** p : {&S->ibp_c, &S->ibp_r, &S->ibp_a, &S->ibp_m, &S->ibp_vm}) *p = F((size_t)C * mw);
+    }
     for (int l = 1; l < L; ++l) {
         size_t c = (size_t)C * S->wp[l];
         S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
@@ -905,6 +927,28 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
         const bool is_out = (s == L);
         const int nk = is_out ? (with_jac ? 3 : 2) : 2;
         const int rp = S->rows_pad[s], rk = S->rows_kind[s];
+        if (ibp && !is_out && cert) {
+            // certified CROWN-IBP: z_s - c_s = W_s (a_{s-1} - ahat_{s-1}) + (centre residual), a_{s-1} - ahat_{s-1} in dc -+ dr, so
+            // z_s - c_s in m -+ (|W_s| dr + gam |W_s||dc| + e_s), m = the FP32 product W_s dc (wrong by at most gam |W_s||dc|): the
+            // layer-1 formula of a non-centred box with (mu, sigma) -> (dc, dr), every |W| product rounded up (cert_layer_kernel)
+            const size_t cp = (size_t)C * S->wp[s - 1], cs = (size_t)C * S->wp[s];
+            launch_cert_layer(S, C, s, false, st, launches);                    // e_s, t_s
+            ibp_dev_cert_kernel<<<gs_grid(cp), 256, 0, st>>>(S->act, C, S->w[s - 1], S->wp[s - 1], S->ahat[s - 1], S->lb[s - 1], S->ub[s - 1],
+                                                            S->ibp_c, S->ibp_r, S->ibp_a);
+            GemmArgs gm = plain_args(C, S->wp[s], S->wp[s - 1], S->ibp_c, S->wp[s - 1], S->Wt[s], S->wp[s], S->ibp_m, S->wp[s]);
+            launch_gemm<AMODE_PLAIN, EPI_STORE>(S, gm, st, launches);
+            dim3 grid((S->wp[s] + CJ - 1) / CJ, (C + CM - 1) / CM);
+            cert_layer_kernel<<<grid, 256, 0, st>>>(C, S->wp[s], S->wp[s - 1], S->Wt[s], S->rowsW[s], S->bias[s], S->ahat[s - 1], nullptr, S->ibp_r,
+                                                   S->wp[s - 1], S->zhat[s], S->ahat[s], S->act, 0, S->mU[s], S->mL[s], S->cv[s], S->wp[s]);
+            cert_layer_kernel<<<grid, 256, 0, st>>>(C, S->wp[s], S->wp[s - 1], S->Wt[s], S->rowsW[s], S->bias[s], S->ahat[s - 1], nullptr, S->ibp_a,
+                                                   S->wp[s - 1], S->zhat[s], S->ahat[s], S->act, 0, S->mU[s], S->mL[s], S->ibp_vm, S->wp[s]);
+            relax_fwd_cert_kernel<<<gs_grid(cs), 256, 0, st>>>(
+                S->act, C, S->w[s], S->wp[s], 1, S->use_tc ? 1 : 0, S->zhat[s], S->ahat[s], S->cv[s], S->ce[s], S->lb[s], S->ub[s], S->kU[s],
+                S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s], S->ibp_m, S->ibp_vm,
+                (float)(S->wp[s - 1] + 4) * 5.9604652e-08f * 1.000001f);
+            *launches += 4;
+            continue;
+        }
         if (ibp && !is_out) {
             // CROWN-IBP: l_s, u_s = zhat_s + W_s dc -+ |W_s| dr (the cert-mode arrays serve as scratch: value mode only)
             const size_t cp = (size_t)C * S->wp[s - 1], cs = (size_t)C * S->wp[s];
@@ -1115,7 +1159,6 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
     S->use_pairs = S->use_tc && !(flags & LEB_FLAG_SINGLE_CTA);
     const bool cert = !(flags & LEB_FLAG_NO_MARGIN);                  // certified mode (N6): DESIGN.md §6 "Certified margin"
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
-    if (ibp && cert) return LEB_ERR_UNSUPPORTED;                       // the rounding bookkeeping covers the back-substituted hidden bounds only
     if (cert)
         for (int l = 0; l < S->L; ++l) if (S->wp[l] > 2048) return LEB_ERR_UNSUPPORTED;   // the 1.0001 norm factor covers K <= 2048
     if (tiles == 0) return LEB_OK;
@@ -1209,7 +1252,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     // workspace still holds that call's complete forward state (one chunk, own Jacobian), the reverse sweep starts from it
     // and was computed in the mode this call names (LEB_FLAG_NO_MARGIN: a value-mode state; otherwise a certified one).
     const bool ibp = (flags & LEB_FLAG_IBP_HIDDEN) != 0;
-    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN) && !ibp;
+    const bool want_cert = !(flags & LEB_FLAG_NO_MARGIN);
     const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
                        S->last_cert == want_cert && S->last_ibp == ibp && S->last_mu == (mu != nullptr);
     S->last_vjp_reused = reuse;

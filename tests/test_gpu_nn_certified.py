@@ -291,9 +291,10 @@ def test_contraction_error_model(mods, path, K):
 
 
 # ---------------------------------------------------------------------------------- certified mode on non-centred boxes
+@pytest.mark.parametrize("hidden", ["crown", "ibp"])
 @pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("dims,act", SMALL)
-def test_certified_mu_sound_and_not_much_wider(mods, dims, act, path):
+def test_certified_mu_sound_and_not_much_wider(mods, dims, act, path, hidden):
     """mu != NULL in certified mode.  The relaxation gaps are taken at the nominal pre-activation zhat(a~), which lies
     outside a neuron's interval when |W_1 mu| exceeds its radius; the certificate clamps them (gU >= 0 >= gL keeps the gap
     sums same-signed, which its rounding factors need), so the hidden bounds are up to ~1e-2 wider than the oracle's and
@@ -308,10 +309,11 @@ def test_certified_mu_sound_and_not_much_wider(mods, dims, act, path):
     N = dims[0]
     nom, rad, mu_f = w.nom.reshape(-1, N), w.rad.reshape(-1, N), mu.reshape(-1, N)
     J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in nom]).astype(np.float32)
-    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=PATHS[path], mu=_dev(mu))
+    flags = PATHS[path] | (leb.FLAG_IBP_HIDDEN if hidden == "ibp" else 0)
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=_dev(J32.reshape(w.B, w.T, w.n, N)), flags=flags, mu=_dev(mu))
     assert ctx.leb_domain_flag() == 0
     clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
-    hidden = [tuple(to_np(x).astype(np.float64) for x in ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])) for layer in range(1, len(dims) - 1)]
+    hbounds = [tuple(to_np(x).astype(np.float64) for x in ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])) for layer in range(1, len(dims) - 1)]
     rng = np.random.default_rng(5)
     for t in range(w.B * w.T):
         a0, sg, m = nom[t].astype(np.float64), rad[t].astype(np.float64), mu_f[t].astype(np.float64)
@@ -320,13 +322,13 @@ def test_certified_mu_sound_and_not_much_wider(mods, dims, act, path):
         A = X.T
         for l in range(len(Ws) - 1):
             Z = Ws[l] @ A + bs[l][:, None]
-            assert np.all(Z.min(1) >= hidden[l][0][t]) and np.all(Z.max(1) <= hidden[l][1][t]), (dims, t, l)
+            assert np.all(Z.min(1) >= hbounds[l][0][t]) and np.all(Z.max(1) <= hbounds[l][1][t]), (dims, t, l)
             A = O.phi(act, Z)
         r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
         assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
-    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, J=J32, mu=mu_f)
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, J=J32, mu=mu_f, hidden=hidden)
     per_tile = np.array([_looseness(clo[t:t + 1], chi[t:t + 1], olo[t:t + 1], ohi[t:t + 1]) for t in range(clo.shape[0])])
-    print(f"certified mu {dims} {path}: looseness over the oracle enclosure median {np.median(per_tile):.3e} max {per_tile.max():.3e}")
+    print(f"certified mu {hidden} {dims} {path}: looseness over the oracle enclosure median {np.median(per_tile):.3e} max {per_tile.max():.3e}")
     assert np.median(per_tile) < 5e-2 and per_tile.max() < 0.25, per_tile
     ctx.close()
 
@@ -357,3 +359,72 @@ def test_certified_mu_never_below_sampled_maximum_strict(mods, path):
             r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
             assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
         ctx.close()
+
+
+# ---------------------------------------------------------------------------------- certified CROWN-IBP
+@pytest.mark.parametrize("path", list(PATHS))
+@pytest.mark.parametrize("dims,act", SMALL)
+def test_certified_crown_ibp(mods, dims, act, path):
+    """LEB_FLAG_IBP_HIDDEN without LEB_FLAG_NO_MARGIN.  Interval propagation is monotone in its input bounds, so every
+    certified hidden bound contains the oracle's; the output enclosure contains the oracle's CROWN-IBP enclosure except
+    where a relaxation case switches (reported as a tie by the oracle, R21), is not much wider, and holds with no tolerance
+    on samples and sampled vertices of the box (J passed in FP32: the remainder is defined with exactly that matrix)."""
+    leb, wl, O = mods
+    IBP = leb.FLAG_IBP_HIDDEN
+    w = wl.make_small_mlp(dims, act, 3, 4, rad_lo=0.02, rad_hi=0.2)
+    ctx = leb.context_for_workload(w)
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    N = dims[0]
+    nom, rad = w.nom.reshape(-1, N), w.rad.reshape(-1, N)
+    J32 = np.stack([O.nominal(Ws, bs, act, a0.astype(np.float64))[2] for a0 in nom]).astype(np.float32)
+    Jd = _dev(J32.reshape(w.B, w.T, w.n, N))
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), J=Jd, flags=PATHS[path] | IBP)
+    assert ctx.leb_domain_flag() == 0
+    clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+    hidden = [tuple(to_np(x).astype(np.float64) for x in ctx.leb_nn_hidden_bounds(layer, w.B * w.T, dims[layer])) for layer in range(1, len(dims) - 1)]
+    olo, ohi = O.leb_nn(w.mlp.W, w.mlp.b, act, nom, rad, J=J32, hidden="ibp")
+    rng = np.random.default_rng(8)
+    for t in range(w.B * w.T):
+        a0, sg = nom[t].astype(np.float64), rad[t].astype(np.float64)
+        fw = O.crown_forward(Ws, bs, act, a0, sg, hidden="ibp")
+        for layer, (l, u) in enumerate(hidden, start=1):
+            assert np.all(l[t] <= fw["ls"][layer - 1]) and np.all(u[t] >= fw["us"][layer - 1]), (dims, t, layer)
+        X = a0[None] + np.concatenate([rng.uniform(-1, 1, (20000, N)), rng.choice([-1.0, 1.0], (4096, N))]) * sg[None]
+        _, p, _ = O.nominal(Ws, bs, act, a0)
+        A = X.T
+        for l in range(len(Ws) - 1):
+            Z = Ws[l] @ A + bs[l][:, None]
+            assert np.all(Z.min(1) >= hidden[l][0][t]) and np.all(Z.max(1) <= hidden[l][1][t]), (dims, t, l)
+            A = O.phi(act, Z)
+        r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ J32[t].astype(np.float64).T
+        assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (dims, t)
+        if not (np.all(chi[t] >= ohi[t]) and np.all(clo[t] <= olo[t])):
+            assert O.relax_case_ties(Ws, bs, act, a0, sg, rel=2e-4), (dims, t, float((ohi[t] - chi[t]).max()), float((clo[t] - olo[t]).max()))
+    per_tile = np.array([_looseness(clo[t:t + 1], chi[t:t + 1], olo[t:t + 1], ohi[t:t + 1]) for t in range(clo.shape[0])])
+    print(f"certified crown-ibp {dims} {path}: looseness over the oracle enclosure median {np.median(per_tile):.3e} max {per_tile.max():.3e}")
+    assert np.median(per_tile) < 2e-2 and per_tile.max() < 0.1, per_tile
+    # a certified CROWN-IBP state (of a forward with the library's own Jacobian) is reused by a certified CROWN-IBP VJP
+    ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path] | IBP)
+    g = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path] | IBP | leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state() == (w.B * w.T, True, True)
+    gv = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path] | IBP | leb.FLAG_NO_MARGIN)
+    for a, b in zip(g, gv):
+        assert float((a - b).abs().max()) <= 2e-2 * float(b.abs().max()) + 1e-7
+    ctx.close()
+
+
+def test_certified_crown_ibp_config5_sampled(mods):
+    """Config 5 at full width, 8 tiles: certified CROWN-IBP contains the value-mode CROWN-IBP enclosure and is sound on samples."""
+    leb, wl, O = mods
+    w = wl.make_config(5, B=1, T=8)
+    ctx = leb.context_for_workload(w)
+    IBP = leb.FLAG_IBP_HIDDEN
+    lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=IBP)
+    vlo, vhi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=IBP | leb.FLAG_NO_MARGIN)
+    assert ctx.leb_domain_flag() == 0
+    assert bool((hi >= vhi).all()) and bool((lo <= vlo).all())
+    width = (vhi - vlo).amax(dim=2, keepdim=True)
+    excess = torch.maximum(hi - vhi, vlo - lo) / width
+    print(f"certified crown-ibp config 5: excess over value mode median {float(excess.median()):.3e} max {float(excess.max()):.3e}")
+    assert float(excess.max()) < 0.2
+    ctx.close()
