@@ -197,8 +197,13 @@ leb_status leb_nn_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float*
  * choice of leb_nn_fwd, `steps` projected gradient steps alpha <- clip(alpha - lr dW/dalpha, 0, 1) on the total width
  * W = sum_i (r_hi_i - r_lo_i) of each tile's enclosure (one slope set per tile; dW/dalpha comes from the ordinary reverse
  * sweep), all on the device; every iterate is a sound enclosure and the tightest one per tile is returned.
- * Value mode only (flags must contain LEB_FLAG_NO_MARGIN), tanh networks: LEB_ERR_UNSUPPORTED.
- *   width0, width : [B, T] total width of the adaptive-slope enclosure / of the returned one.  Other arguments as leb_nn_fwd. */
+ * The descent runs on the plain FP32 bound; the kept slopes are then evaluated once more in the mode `flags` names --
+ * certified by default (the certificate of leb_nn_fwd holds for any lower slope in [0, 1]) -- and that is what is returned.
+ * The forward state of this last evaluation stays resident: leb_vjp(kind 1, LEB_FLAG_REUSE_FWD, same mode flags) then
+ * returns the gradient of the REFINED bound with the kept slopes held constant (a stateless leb_vjp differentiates the
+ * adaptive-slope bound of leb_nn_fwd).  tanh networks, LEB_FLAG_IBP_HIDDEN: LEB_ERR_UNSUPPORTED.
+ *   width0, width : [B, T] total width of the adaptive-slope enclosure (plain FP32 bound, what the descent starts from) /
+ *                   of the returned one (in the mode `flags` names).  Other arguments as leb_nn_fwd. */
 leb_status leb_nn_alpha_fwd(leb_ctx* ctx, int B, int T, const float* nom, const float* rad, int ld_in, int steps, float lr,
                             float* r_lo, float* r_hi, int ld_out, float* width0, float* width, unsigned flags, void* stream);
 
@@ -281,6 +286,11 @@ leb_status leb_nn_hidden_bounds(leb_ctx* ctx, int layer, float* l, float* u, voi
  * dims[target]; index 0 = upper chain, 1 = lower chain.  Used to measure the contraction's rounding error
  * against the model behind the certified margin. */
 leb_status leb_nn_chain_coeffs(leb_ctx* ctx, int target, float* out, void* stream);
+
+/* Inspection: the relaxation slopes (k^U, k^L of (18) PAPER.md:L196-200) of hidden layer `layer` (1-based) in the forward
+ * state the LAST leb_nn_fwd / leb_nn_alpha_fwd call left (B*T fitted one chunk).  After leb_nn_alpha_fwd the lower slopes of
+ * the unstable neurons are the refined ones.  kU, kL: device [B*T, dims[layer]] contiguous. */
+leb_status leb_nn_slopes(leb_ctx* ctx, int layer, float* kU, float* kL, void* stream);
 
 /* The Jacobian J~ the LAST leb_nn_fwd call with J == NULL subtracted in (20) PAPER.md:L209 -- the network's Jacobian at a~
  * (eq. (7)) as the library's own chain computed it, rounding included.  The certified enclosure is an enclosure of

@@ -515,6 +515,13 @@ leb_status leb_nn_chain_coeffs(leb_ctx* c, int target, float* out, void* stream)
     return leb_nn_get_coeffs(c->nn, target, out, (cudaStream_t)stream, &c->launches);
 }
 
+leb_status leb_nn_slopes(leb_ctx* c, int layer, float* kU, float* kL, void* stream) {
+    if (!c || !kU || !kL) return LEB_ERR_ARG;
+    if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;
+    DeviceGuard guard(c->device);
+    return leb_nn_get_slopes(c->nn, layer, kU, kL, (cudaStream_t)stream, &c->launches);
+}
+
 leb_status leb_nn_jacobian(leb_ctx* c, float* out, void* stream) {
     if (!c || !out) return LEB_ERR_ARG;
     if (!leb_nn_ready(c->nn)) return LEB_ERR_STATE;

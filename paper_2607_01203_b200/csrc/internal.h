@@ -117,3 +117,4 @@ void leb_nn_query(const NnState*, int* tiles, int* certified, int* vjp_reused);
 leb_status leb_nn_get_hidden(NnState*, int layer, float* l, float* u, cudaStream_t st, long long* launches);
 leb_status leb_nn_get_coeffs(NnState*, int target, float* out, cudaStream_t st, long long* launches);
 leb_status leb_nn_get_jacobian(NnState*, float* out, cudaStream_t st, long long* launches);
+leb_status leb_nn_get_slopes(NnState*, int layer, float* kU, float* kL, cudaStream_t st, long long* launches);

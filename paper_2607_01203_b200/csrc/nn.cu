@@ -57,6 +57,9 @@ struct NnState {
     float *mup = nullptr, *mu1 = nullptr, *mu_bar = nullptr;   // non-centred boxes: padded mu, W_1 mu, and its adjoint
     float *ibp_c = nullptr, *ibp_r = nullptr, *ibp_a = nullptr, *ibp_m = nullptr, *ibp_vm = nullptr;   // certified CROWN-IBP scratch
     float* alpha[kMaxLayers] = {nullptr};                      // optimisable lower ReLU slopes (leb_nn_alpha_fwd), [chunk x wp[l]]
+    float* alpha_best[kMaxLayers] = {nullptr};                 // ... of the tightest iterate so far
+    int* alpha_take = nullptr;                                 // [chunk]: did the last iterate improve the tile?
+    bool last_alpha = false;                                   // the resident forward state was computed with refined slopes
     int alpha_mode = 0;                                        // 0 off, 1 forward writes the adaptive default, 2 forward reads alpha
     std::vector<void*> alpha_scratch; size_t alpha_scratch_tiles = 0;
     const float* mu_cur = nullptr;                             // = mup while the chunk in flight has box offsets, else NULL
@@ -213,7 +216,8 @@ __global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, i
                                       float* __restrict__ lb, float* __restrict__ ub, float* __restrict__ kU, float* __restrict__ kL,
                                       float* __restrict__ gU, float* __restrict__ gL, float* __restrict__ adev,
                                       float* __restrict__ mU, float* __restrict__ mL, const float* __restrict__ m1 = nullptr,
-                                      const float* __restrict__ vmu = nullptr, float gam_mu = 0.f) {
+                                      const float* __restrict__ vmu = nullptr, float gam_mu = 0.f,
+                                      const float* __restrict__ alpha = nullptr) {
     size_t total = (size_t)tiles * wp;
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x) {
         int c = (int)(q % wp);
@@ -239,6 +243,7 @@ __global__ void relax_fwd_cert_kernel(int act, int tiles, int w_valid, int wp, i
         } else { l = lb[q]; u = ub[q]; }
         const double zd = (double)z, ld = (double)l, ud = (double)u, a = (double)ahat[q];
         Relax r = relax_any(act, ld, ud);
+        if (alpha && r.cL == LINE_RELU_LOW) r.kL = (double)alpha[q];      // a given lower slope in [0, 1]: as sound as the rule's
         const float kU32 = (float)r.kU, kL32 = (float)r.kL;
         const double zdev = fmax(ud - zd, zd - ld);
         const double d64 = 5.7e-14 * (1.0 + fabs(zd) + fabs(ld) + fabs(ud));          // 2^-44 (1 + |c| + |l| + |u|)
@@ -645,6 +650,12 @@ __global__ void diff_kernel(const float* __restrict__ ubar, const float* __restr
 
 // alpha-CROWN style refinement: one projected gradient step on the lower slopes of the unstable ReLU neurons;
 // d(objective)/d(alpha) = k_bar^L + zhat gap_bar^L (gap^L = alpha zhat - relu(zhat))
+// keep the slopes of the tiles whose last iterate was the tightest so far
+__global__ void alpha_keep_kernel(int tiles, int wp, const int* __restrict__ take, const float* __restrict__ alpha, float* __restrict__ best) {
+    size_t total = (size_t)tiles * wp;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (size_t)gridDim.x * blockDim.x)
+        if (take[q / wp]) best[q] = alpha[q];
+}
 __global__ void alpha_update_kernel(int tiles, int w_valid, int wp, const float* __restrict__ zhat, const float* __restrict__ lb,
                                     const float* __restrict__ ub, const float* __restrict__ kLb, const float* __restrict__ gLb,
                                     float* __restrict__ alpha, float lr) {
@@ -659,8 +670,11 @@ __global__ void alpha_update_kernel(int tiles, int w_valid, int wp, const float*
 }
 
 // keep the tightest iterate of every tile: one block per tile
+// first: 1 = the adaptive-slope iterate (sets width0), 0 = a later iterate (taken if tighter), 2 = the final evaluation at the kept
+// slopes (always taken; width0 untouched)
 __global__ void alpha_best_kernel(int n, int ld_out, int first, const float* __restrict__ cur_lo, const float* __restrict__ cur_hi,
-                                  float* __restrict__ r_lo, float* __restrict__ r_hi, float* __restrict__ w0, float* __restrict__ wbest) {
+                                  float* __restrict__ r_lo, float* __restrict__ r_hi, float* __restrict__ w0, float* __restrict__ wbest,
+                                  int* __restrict__ take_out) {
     __shared__ float red[8];
     __shared__ int take;
     const size_t t = blockIdx.x;
@@ -672,9 +686,10 @@ __global__ void alpha_best_kernel(int n, int ld_out, int first, const float* __r
     if (threadIdx.x == 0) {
         float tot = 0.f;
         for (int q = 0; q < (int)(blockDim.x >> 5); ++q) tot += red[q];
-        if (first) { w0[t] = tot; wbest[t] = tot; take = 1; }
-        else if (tot < wbest[t]) { wbest[t] = tot; take = 1; }
+        if (first == 1) { w0[t] = tot; wbest[t] = tot; take = 1; }
+        else if (first == 2 || tot < wbest[t]) { wbest[t] = tot; take = 1; }
         else take = 0;
+        take_out[t] = take;
     }
     __syncthreads();
     if (take)
@@ -814,6 +829,7 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
     S->mup = F((size_t)C * S->wp[0]);
     S->mu1 = F((size_t)C * S->wp[1]);
     S->mu_bar = F((size_t)C * S->wp[0]);
+    S->alpha_take = (int*)F((size_t)C);
     {
         int mw = 0;
         for (int l = 1; l < L; ++l) mw = std::max(mw, S->wp[l]);
@@ -824,7 +840,7 @@ leb_status ensure_workspace(NnState* S, int tiles, bool vjp) {
         S->zhat[l] = F(c); S->ahat[l] = F(c); S->dphi[l] = F(c); S->lb[l] = F(c); S->ub[l] = F(c);
         S->kU[l] = F(c); S->kL[l] = F(c); S->gU[l] = F(c); S->gL[l] = F(c);
         S->ce[l] = F(c); S->ct[l] = F(c); S->cv[l] = F(c); S->adev[l] = F(c); S->mU[l] = F(c); S->mL[l] = F(c);
-        S->alpha[l] = F(c);
+        S->alpha[l] = F(c); S->alpha_best[l] = F(c);
         if (vjp) {
             S->kUb[l] = F(c); S->kLb[l] = F(c); S->gUb[l] = F(c); S->gLb[l] = F(c); S->dpb[l] = F(c);
             S->zbar[l] = F(c); S->lbar[l] = F(c); S->ubar[l] = F(c);
@@ -908,7 +924,8 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
         }
         relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[1]), 256, 0, st>>>(
             S->act, C, S->w[1], S->wp[1], 1, S->use_tc ? 1 : 0, S->zhat[1], S->ahat[1], S->cv[1], S->ce[1], S->lb[1], S->ub[1], S->kU[1],
-            S->kL[1], S->gU[1], S->gL[1], S->adev[1], S->mU[1], S->mL[1], m1, vmu, (float)(S->wp[0] + 4) * 5.9604652e-08f * 1.000001f);
+            S->kL[1], S->gU[1], S->gL[1], S->adev[1], S->mU[1], S->mL[1], m1, vmu, (float)(S->wp[0] + 4) * 5.9604652e-08f * 1.000001f,
+            S->alpha_mode == 2 ? S->alpha[1] : nullptr);
         ++*launches;
     } else {
         GemmArgs g = plain_args(C, S->wp[1], S->wp[0], S->radp, S->wp[0], S->Wabs1t, S->wp[1], S->rad1, S->wp[1]);
@@ -945,7 +962,7 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
             relax_fwd_cert_kernel<<<gs_grid(cs), 256, 0, st>>>(
                 S->act, C, S->w[s], S->wp[s], 1, S->use_tc ? 1 : 0, S->zhat[s], S->ahat[s], S->cv[s], S->ce[s], S->lb[s], S->ub[s], S->kU[s],
                 S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s], S->ibp_m, S->ibp_vm,
-                (float)(S->wp[s - 1] + 4) * 5.9604652e-08f * 1.000001f);
+                (float)(S->wp[s - 1] + 4) * 5.9604652e-08f * 1.000001f, S->alpha_mode == 2 ? S->alpha[s] : nullptr);
             *launches += 4;
             continue;
         }
@@ -1004,7 +1021,8 @@ void forward_chunk(NnState* S, int C, const float* Jgiven, bool with_jac, bool c
             if (cert) {
                 relax_fwd_cert_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(
                     S->act, C, S->w[s], S->wp[s], 0, S->use_tc ? 1 : 0, S->zhat[s], S->ahat[s], S->cv[s], S->ce[s], S->lb[s], S->ub[s],
-                    S->kU[s], S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s]);
+                    S->kU[s], S->kL[s], S->gU[s], S->gL[s], S->adev[s], S->mU[s], S->mL[s], nullptr, nullptr, 0.f,
+                    S->alpha_mode == 2 ? S->alpha[s] : nullptr);
             } else {
                 relax_fwd_kernel<<<gs_grid((size_t)C * S->wp[s]), 256, 0, st>>>(S->act, C, S->w[s], S->wp[s], S->zhat[s], nullptr, S->lb[s],
                                                                               S->ub[s], S->kU[s], S->kL[s], S->gU[s], S->gL[s], nullptr,
@@ -1186,6 +1204,7 @@ leb_status leb_nn_forward(NnState* S, int tiles, const float* nom, const float* 
         S->last_cert = cert;
         S->last_ibp = ibp;
         S->last_mu = (mu != nullptr);
+        S->last_alpha = (S->alpha_mode == 2);
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
@@ -1201,6 +1220,15 @@ leb_status leb_nn_get_hidden(NnState* S, int layer, float* l, float* u, cudaStre
     if (layer < 1 || layer >= S->L || S->last_tiles <= 0 || S->chunk <= 0) return LEB_ERR_STATE;
     copy_hidden_kernel<<<gs_grid((size_t)S->last_tiles * S->w[layer]), 256, 0, st>>>(S->last_tiles, S->w[layer], S->wp[layer],
                                                                                     S->lb[layer], S->ub[layer], l, u);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
+}
+
+// relaxation slopes (k_U, k_L) of hidden layer `layer` in the resident forward state: [tiles, dims[layer]] each
+leb_status leb_nn_get_slopes(NnState* S, int layer, float* kU, float* kL, cudaStream_t st, long long* launches) {
+    if (layer < 1 || layer >= S->L || S->last_tiles <= 0 || S->chunk <= 0) return LEB_ERR_STATE;
+    copy_hidden_kernel<<<gs_grid((size_t)S->last_tiles * S->w[layer]), 256, 0, st>>>(S->last_tiles, S->w[layer], S->wp[layer],
+                                                                                    S->kU[layer], S->kL[layer], kU, kL);
     ++*launches;
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
@@ -1256,6 +1284,9 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
     const bool reuse = (flags & LEB_FLAG_REUSE_FWD) && S->last_tiles == tiles && S->last_with_jac && tiles <= S->chunk &&
                        S->last_cert == want_cert && S->last_ibp == ibp && S->last_mu == (mu != nullptr);
     S->last_vjp_reused = reuse;
+    // a state left by leb_nn_alpha_fwd: the reverse sweep of the refined bound holds the kept slopes constant
+    struct AlphaGuard { NnState* S; bool on; ~AlphaGuard() { if (on) S->alpha_mode = 0; } } alpha_guard{S, reuse && S->last_alpha && S->alpha_mode == 0};
+    if (alpha_guard.on) S->alpha_mode = 2;
     for (int t0 = 0; t0 < tiles; t0 += S->chunk) {
         const int C = std::min(S->chunk, tiles - t0);
         if (!reuse)
@@ -1374,7 +1405,7 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
                                                                  grad_nom + (size_t)t0 * ld_in, grad_rad + (size_t)t0 * ld_in,
                                                                  mu ? S->mu_bar : nullptr, (mu && grad_mu) ? grad_mu + (size_t)t0 * ld_in : nullptr);
         ++*launches;
-        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; S->last_mu = (mu != nullptr); }   // a value-mode forward state
+        if (!reuse) { S->last_tiles = (tiles <= S->chunk) ? C : 0; S->last_with_jac = true; S->last_cert = false; S->last_ibp = ibp; S->last_mu = (mu != nullptr); S->last_alpha = (S->alpha_mode == 2); }   // a value-mode forward state
     }
     if (S->launch_failed) { S->launch_failed = false; return LEB_ERR_CUDA; }
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
@@ -1390,7 +1421,7 @@ leb_status leb_nn_alpha(NnState* S, int tiles, const float* nom, const float* ra
                         float* r_hi, int ld_out, float* w0, float* wbest, unsigned flags, int* domain_flag, cudaStream_t st,
                         long long* launches, LebProf* prof) {
     if (S->act != ACT_RELU) return LEB_ERR_UNSUPPORTED;
-    if (!(flags & LEB_FLAG_NO_MARGIN)) return LEB_ERR_UNSUPPORTED;       // value mode only
+    if (flags & LEB_FLAG_IBP_HIDDEN) return LEB_ERR_UNSUPPORTED;
     if (tiles == 0) return LEB_OK;
     leb_status ws = ensure_workspace(S, tiles, true);
     if (ws != LEB_OK) return ws;
@@ -1413,6 +1444,8 @@ leb_status leb_nn_alpha(NnState* S, int tiles, const float* nom, const float* ra
     fill_kernel<<<gs_grid(Cmax * n), 256, 0, st>>>(gm1, Cmax * n, -1.f);
     fill_kernel<<<gs_grid(Cmax * n), 256, 0, st>>>(gp1, Cmax * n, 1.f);
     *launches += 2;
+    // the descent runs on the plain (value-mode) bound; the kept slopes are then evaluated once more in the mode the caller
+    // asked for -- certified by default: any slope in [0, 1] is a valid lower line, so the certificate of leb_nn_fwd carries over
     const unsigned f = flags | LEB_FLAG_NO_MARGIN;
     leb_status rc = LEB_OK;
     for (int t0 = 0; t0 < tiles && rc == LEB_OK; t0 += S->chunk) {
@@ -1423,9 +1456,13 @@ leb_status leb_nn_alpha(NnState* S, int tiles, const float* nom, const float* ra
             S->alpha_mode = (it == 0) ? 1 : 2;
             rc = leb_nn_forward(S, C, a, r, nullptr, nullptr, ld_in, cur_lo, cur_hi, nullptr, n, f, domain_flag, st, launches, prof);
             if (rc != LEB_OK) break;
-            alpha_best_kernel<<<C, 128, 0, st>>>(n, ld_out, it == 0, cur_lo, cur_hi, r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out,
-                                                 w0 + t0, wbest + t0);
+            alpha_best_kernel<<<C, 128, 0, st>>>(n, ld_out, it == 0 ? 1 : 0, cur_lo, cur_hi, r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out,
+                                                 w0 + t0, wbest + t0, S->alpha_take);
             ++*launches;
+            for (int l = 1; l < L; ++l) {
+                alpha_keep_kernel<<<gs_grid((size_t)C * S->wp[l]), 256, 0, st>>>(C, S->wp[l], S->alpha_take, S->alpha[l], S->alpha_best[l]);
+                ++*launches;
+            }
             if (it == steps) break;
             S->alpha_mode = 2;
             rc = leb_nn_vjp(S, C, a, r, nullptr, gm1, gp1, ld_in, n, gsn, gsr, nullptr, f | LEB_FLAG_REUSE_FWD, domain_flag, st, launches, prof);
@@ -1436,9 +1473,20 @@ leb_status leb_nn_alpha(NnState* S, int tiles, const float* nom, const float* ra
                 ++*launches;
             }
         }
+        if (rc != LEB_OK) break;
+        // the kept slopes, in the caller's mode; the state stays resident for leb_vjp(LEB_FLAG_REUSE_FWD)
+        for (int l = 1; l < L; ++l)
+            cudaMemcpyAsync(S->alpha[l], S->alpha_best[l], (size_t)C * S->wp[l] * sizeof(float), cudaMemcpyDeviceToDevice, st);
+        S->alpha_mode = 2;
+        rc = leb_nn_forward(S, C, a, r, nullptr, nullptr, ld_in, cur_lo, cur_hi, nullptr, n, flags, domain_flag, st, launches, prof);
+        if (rc != LEB_OK) break;
+        alpha_best_kernel<<<C, 128, 0, st>>>(n, ld_out, 2, cur_lo, cur_hi, r_lo + (size_t)t0 * ld_out, r_hi + (size_t)t0 * ld_out, w0 + t0,
+                                             wbest + t0, S->alpha_take);
+        ++*launches;
     }
     S->alpha_mode = 0;
-    S->last_tiles = 0;      // the resident state belongs to a refined slope set: not a state leb_vjp may reuse
+    if (tiles > S->chunk || rc != LEB_OK) S->last_tiles = 0;      // several chunks: no complete state is resident
+    else S->last_tiles = tiles;
     if (rc != LEB_OK) return rc;
     return cudaGetLastError() == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }

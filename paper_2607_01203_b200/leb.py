@@ -28,7 +28,7 @@ FLAG_IBP_HIDDEN = 32
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
     "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_partition_vjp", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
-    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_jacobian", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
+    "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_jacobian", "leb_nn_slopes", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
 
@@ -230,7 +230,7 @@ class Context:
                                  _ptr(margin), int(r_lo.shape[2]), ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_nn_fwd")
         return r_lo, r_hi
 
-    def leb_nn_alpha_fwd(self, nom, rad, steps: int, lr: float, flags: int = FLAG_NO_MARGIN):
+    def leb_nn_alpha_fwd(self, nom, rad, steps: int, lr: float, flags: int = 0):
         """CROWN with optimisable lower ReLU slopes; returns (r_lo, r_hi, width0, width)."""
         _check_f32(nom, rad)
         B, T, ld_in = self._bt(nom)
@@ -343,6 +343,14 @@ class Context:
         out = torch.empty((tiles, 2, rows, N), dtype=torch.float32, device=torch.device("cuda", self.device))
         _chk(self.lib.leb_nn_chain_coeffs(self._ctx, int(target), _ptr(out), _stream_ptr(self.device)), "leb_nn_chain_coeffs")
         return out
+
+    def leb_nn_slopes(self, layer: int, tiles: int, width: int):
+        """(k_U, k_L) of hidden layer `layer` in the resident forward state: [tiles, width] each"""
+        dev = torch.device("cuda", self.device)
+        kU = torch.empty((tiles, width), dtype=torch.float32, device=dev)
+        kL = torch.empty((tiles, width), dtype=torch.float32, device=dev)
+        _chk(self.lib.leb_nn_slopes(self._ctx, int(layer), _ptr(kU), _ptr(kL), _stream_ptr(self.device)), "leb_nn_slopes")
+        return kU, kL
 
     def leb_nn_jacobian(self, tiles: int, n: int, N: int):
         """J~ of the last leb_nn_fwd(J=None): [tiles, n, N]"""

@@ -528,10 +528,28 @@ def test_alpha_refinement_matches_oracle(mods, path):
             r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ J.T
             assert np.all(r.max(0) <= ghi[t] + 1e-5 * np.abs(ghi[t]) + 1e-7) and np.all(r.min(0) >= glo[t] - 1e-5 * np.abs(glo[t]) - 1e-7)
         assert improved >= 1
-        # tanh networks and the certified mode are refused
-        with pytest.raises(leb.LebError) as e:
-            ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 2, 0.05, flags=PATHS[path] & ~1)
-        assert e.value.status == leb.LEB_ERR_UNSUPPORTED
+        # the kept slopes can be read back; with exactly those slopes the oracle gives the returned enclosure, and
+        # leb_vjp(REUSE_FWD) on the state the refinement left is the gradient of the REFINED bound, slopes held constant
+        tiles = w.B * w.T
+        assert ctx.leb_nn_state()[0] == tiles
+        kLs = [to_np(ctx.leb_nn_slopes(layer, tiles, dims[layer])[1]).astype(np.float64) for layer in range(1, len(dims) - 1)]
+        g_lo, g_hi = w.g_lo.reshape(-1, w.n), w.g_hi.reshape(-1, w.n)
+        gn, gr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path] | leb.FLAG_REUSE_FWD)
+        assert ctx.leb_nn_state()[2] is True
+        olo, ohi = np.empty_like(glo, dtype=np.float64), np.empty_like(ghi, dtype=np.float64)
+        ogn, ogr = np.empty((tiles, dims[0])), np.empty((tiles, dims[0]))
+        for t in range(tiles):
+            al = [k[t] for k in kLs]
+            fw = O.crown_forward(Ws, bs, 1, nom[t].astype(np.float64), rad[t].astype(np.float64), alphas=al)
+            olo[t], ohi[t] = fw["r_lo"], fw["r_hi"]
+            ogn[t], ogr[t] = O.crown_vjp(Ws, bs, 1, nom[t].astype(np.float64), rad[t].astype(np.float64), g_lo[t].astype(np.float64),
+                                         g_hi[t].astype(np.float64), alphas=al)
+        assert_bounds_close(glo, olo, f"alpha {dims} r_lo at the kept slopes")
+        assert_bounds_close(ghi, ohi, f"alpha {dims} r_hi at the kept slopes")
+        assert_grads_close(to_np(gn), to_np(gr), ogn, ogr, f"alpha {dims} refined-bound")
+        # a stateless leb_vjp differentiates the adaptive-slope bound instead
+        pn, pr = ctx.leb_vjp(1, _dev(w.nom), _dev(w.rad), _dev(w.g_lo), _dev(w.g_hi), flags=PATHS[path])
+        assert not torch.equal(pn, gn)
         ctx.close()
     wt = wl.make_small_mlp([5, 9, 3], 2, 1, 1)
     ct = leb.context_for_workload(wt)
@@ -546,7 +564,7 @@ def test_alpha_refinement_config3(mods):
     leb, wl, O = mods
     w = wl.make_config(3)
     ctx = leb.context_for_workload(w)
-    lo, hi, w0, wb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 6, 10.0)      # dW/dalpha ~ 0.05 here: steps of ~0.5
+    lo, hi, w0, wb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), 6, 10.0, flags=VAL)      # dW/dalpha ~ 0.05 here: steps of ~0.5
     plo, phi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=VAL)
     assert bool((wb <= w0).all())
     assert torch.allclose(w0.reshape(-1), (phi - plo).sum(-1).reshape(-1), rtol=1e-5)

@@ -428,3 +428,42 @@ def test_certified_crown_ibp_config5_sampled(mods):
     print(f"certified crown-ibp config 5: excess over value mode median {float(excess.median()):.3e} max {float(excess.max()):.3e}")
     assert float(excess.max()) < 0.2
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------- certified optimised slopes
+@pytest.mark.parametrize("path", list(PATHS))
+def test_certified_alpha_refinement(mods, path):
+    """leb_nn_alpha_fwd without LEB_FLAG_NO_MARGIN: the kept slopes evaluated in certified mode.  The result contains the
+    value-mode refined enclosure, is at most a little wider, is tighter than the certified adaptive-slope enclosure where
+    the refinement helped, and holds with no tolerance on samples and vertices (J~ read back: the matrix it is relative to)."""
+    leb, wl, O = mods
+    for dims, seed in (([4, 10, 10, 10, 3], 5), ([6, 33, 20, 11, 5], 6)):
+        w = wl.make_small_mlp(dims, 1, 2, 3, seed=seed, rad_lo=0.1, rad_hi=0.4)
+        ctx = leb.context_for_workload(w)
+        Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+        N, tiles = dims[0], w.B * w.T
+        steps, lr = 8, 0.05
+        vlo, vhi, vw0, vwb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), steps, lr, flags=PATHS[path] | leb.FLAG_NO_MARGIN)
+        clo, chi, cw0, cwb = ctx.leb_nn_alpha_fwd(_dev(w.nom), _dev(w.rad), steps, lr, flags=PATHS[path])
+        assert ctx.leb_nn_state()[:2] == (tiles, True)
+        Jt = to_np(ctx.leb_nn_jacobian(tiles, w.n, N)).astype(np.float64)
+        assert bool((chi >= vhi).all()) and bool((clo <= vlo).all())
+        assert bool((cwb <= vwb * (1 + 2e-2) + 1e-6).all())
+        plo, phi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), flags=PATHS[path])
+        pw = (phi - plo).sum(dim=2)
+        assert bool((cwb <= pw * (1 + 1e-6)).all()) and bool((cwb < 0.999 * pw).any())
+        lo64, hi64 = to_np(clo).reshape(-1, w.n).astype(np.float64), to_np(chi).reshape(-1, w.n).astype(np.float64)
+        rng = np.random.default_rng(seed)
+        for t in range(tiles):
+            a0 = w.nom.reshape(-1, N)[t].astype(np.float64); sg = w.rad.reshape(-1, N)[t].astype(np.float64)
+            U = rng.uniform(-1, 1, (50000, N))
+            if N <= 6:
+                U = np.concatenate([U, np.array(list(itertools.product((-1.0, 1.0), repeat=N)))])
+            X = a0[None] + U * sg[None]
+            _, p, _ = O.nominal(Ws, bs, 1, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(1, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ Jt[t].T
+            assert np.all(r.max(0) <= hi64[t]) and np.all(r.min(0) >= lo64[t]), (dims, t)
+        ctx.close()
