@@ -330,6 +330,7 @@ def run_ours(args):
         if world == 1 and not args.no_configs:
             line["configs"] = {f"config{c}": _config_record(c, 3, 2, peaks) for c in (1, 2, 3, 4)}
             line["configs"]["tube"] = _tube_record(peaks)
+            line["configs"]["next_rows"] = _next_rows_record(max(args.steps, 3), 2)
         print(json.dumps(line))
     if ctx is not None:
         ctx.close()
@@ -432,6 +433,71 @@ def _tube_record(peaks, B=16, T=100, n=168, m=56):
         ach = (k_bytes / 1e9) / (k_ms * 1e-3) if k_ms > 0 else 0.0
         rec[name] = {"bound": "hbm", "avg_launch_ms": k_ms / max(k_n, 1), "achieved": ach, "peak": hbm, "unit": "GB/s",
                      "frac": ach / hbm, "algorithmic_gb_per_launch": k_bytes / max(k_n, 1) / 1e9}
+    ctx.close()
+    return rec
+
+
+def _next_rows_record(steps, warmup):
+    """Timings of the SURVEY 8(f) variants (device-resident inputs, CUDA events): non-centred boxes on configs 4 and 5, input-
+    domain partitioning with its VJP and PGD refinement on config 2, optimised slopes on config 3.  Parity-test cases, timing only."""
+    import numpy as np
+    import torch
+    from paper_2607_01203_b200 import leb, workloads as wl
+    dev = torch.device("cuda", 0)
+
+    def timed(f, n):
+        for _ in range(warmup):
+            f()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / max(n, 1)
+
+    def dv(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+    rec = {}
+    # non-centred boxes, analytic (config 4) and NN (config 5, certified, 16 trajectories)
+    for cfg, kw in ((4, {}), (5, {"B": 16})):
+        w = wl.make_config(cfg, **kw)
+        ctx = leb.context_for_workload(w, 0)
+        nom, rad, mu = dv(w.nom), dv(w.rad), dv(wl.make_mu(w, 1.0))
+        g_lo, g_hi = dv(w.g_lo), dv(w.g_hi)
+        kind = 0 if w.kind == "analytic" else 1
+        fwd = (lambda: ctx.leb_analytic_fwd(nom, rad, mu=mu)) if kind == 0 else (lambda: ctx.leb_nn_fwd(nom, rad, mu=mu))
+
+        def step():
+            fwd()
+            ctx.leb_vjp_mu(kind, nom, rad, mu, g_lo, g_hi, flags=leb.FLAG_REUSE_FWD if kind else 0)
+        ms_f, ms_s = timed(fwd, steps), timed(step, steps)
+        rec[f"mu_config{cfg}"] = {"workload": f"{w.name}, B={w.B} x T={w.T} tiles, |mu| <= sigma", "ms_forward": ms_f, "ms_forward_plus_vjp": ms_s,
+                                  "entries_per_s": w.entries / (ms_s * 1e-3)}
+        ctx.close()
+    # partitioning (12 sub-boxes per tile) with its VJP, and 8 PGD steps, config 2
+    w = wl.make_config(2)
+    ctx = leb.context_for_workload(w, 0)
+    nom, rad, g_lo, g_hi = dv(w.nom), dv(w.rad), dv(w.g_lo), dv(w.g_hi)
+    splits = np.ones(w.N, dtype=int)
+    splits[[3, 4, 12]] = (2, 3, 2)
+    rec["partition_config2"] = {"workload": f"{w.name}, {w.B * w.T} tiles x 12 sub-boxes",
+                                "ms_forward": timed(lambda: ctx.leb_analytic_partition_fwd(nom, rad, splits), steps),
+                                "ms_vjp": timed(lambda: ctx.leb_analytic_partition_vjp(nom, rad, splits, g_lo, g_hi), steps)}
+    eps = 0.5 * rad
+    rec["pgd_config2"] = {"workload": f"{w.name}, {w.B * w.T} tiles, 8 projected gradient steps on the nominal point",
+                          "ms": timed(lambda: ctx.leb_analytic_pgd(nom, rad, eps, nom + 0.4 * rad, 8, 0.03), steps)}
+    ctx.close()
+    # optimised lower slopes, config 3 (certified result)
+    w = wl.make_config(3)
+    ctx = leb.context_for_workload(w, 0)
+    nom, rad = dv(w.nom), dv(w.rad)
+    ms = timed(lambda: ctx.leb_nn_alpha_fwd(nom, rad, 6, 10.0), steps)
+    lo, hi, w0, wb = ctx.leb_nn_alpha_fwd(nom, rad, 6, 10.0, flags=leb.FLAG_NO_MARGIN)
+    rec["alpha_config3"] = {"workload": f"{w.name}, {w.B * w.T} tiles, 6 slope steps + certified evaluation", "ms": ms,
+                            "width_over_adaptive_slopes_median": float((wb / w0).median())}
     ctx.close()
     return rec
 
