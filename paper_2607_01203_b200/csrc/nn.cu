@@ -493,11 +493,14 @@ __global__ void concretise_out_kernel(int tiles, int rows_pad, int n, int N, int
 //   output: with S = sign(Lam_0 - J): Lbar0[up i] = g_hi_i S_up sigma, Lbar0[lo i] = -g_lo_i S_lo sigma,
 //           Lbar0[jac i] = -(Lbar0[up i] + Lbar0[lo i])
 //   rad_bar_j += sum_rows |.| weights;  gapbar[up] = ybar_up, gapbar[lo] = ybar_lo
-__global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
+template <bool MU>
+__global__ void __launch_bounds__(256) seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, const float* __restrict__ Lam0,
                             const float* __restrict__ sigma, const float* __restrict__ ybar_up, const float* __restrict__ ybar_lo,
                             int ldy, float* __restrict__ Lbar0, float* __restrict__ gapbar, float* __restrict__ rad_bar,
                             const float* __restrict__ mu = nullptr, float* __restrict__ mu_bar = nullptr) {
-    // grid (tiles, ceil(rows_kind / 32)): a block takes 32 bound indices k of one tile; thread j owns input column j
+    // grid (tiles, ceil(rows_kind / 32)): a block takes 32 bound indices k of one tile.  64 lanes x float4 cover 256 input
+    // columns, the four 64-lane groups take every fourth k; the column sums are joined in shared memory in a fixed order.
+    __shared__ float4 red_s[3][64], red_m[3][64];
     const int t = blockIdx.x, k0 = blockIdx.y * 32, k1 = min(k0 + 32, rows_kind);
     const float* base = Lam0 + (size_t)t * rows_pad * wp0;
     float* obase = Lbar0 + (size_t)t * rows_pad * wp0;
@@ -507,25 +510,58 @@ __global__ void seed_kernel(int is_out, int rows_pad, int rows_kind, int wp0, co
     }
     if (blockIdx.y == 0)
         for (int r = 2 * rows_kind + threadIdx.x; r < rows_pad; r += blockDim.x) gapbar[(size_t)t * rows_pad + r] = 0.f;
-    for (int j = threadIdx.x; j < wp0; j += blockDim.x) {
-        const float s = sigma[(size_t)t * wp0 + j];
-        const float m = mu ? mu[(size_t)t * wp0 + j] : 0.f;      // non-centred boxes: y = Lam mu +- |Lam| sigma + gap
-        float sb = 0.f, mb = 0.f;
+    const int rq = threadIdx.x >> 6, lane64 = threadIdx.x & 63;
+    auto sgn = [](float v) { return (float)((v > 0.f) - (v < 0.f)); };
+    for (int j0 = 0; j0 < wp0; j0 += 256) {
+        const int j = j0 + lane64 * 4;
+        const bool on = j < wp0;
+        float4 s = make_float4(0.f, 0.f, 0.f, 0.f), m = s, sb = s, mb = s;
+        if (on) {
+            s = *reinterpret_cast<const float4*>(sigma + (size_t)t * wp0 + j);
+            if (MU) m = *reinterpret_cast<const float4*>(mu + (size_t)t * wp0 + j);   // non-centred boxes: y = Lam mu +- |Lam| sigma + gap
 #pragma unroll 4
-        for (int k = k0; k < k1; ++k) {
-            const float yu = ybar_up[(size_t)t * ldy + k], yl = ybar_lo[(size_t)t * ldy + k];
-            float a = base[(size_t)k * wp0 + j], b = base[(size_t)(rows_kind + k) * wp0 + j];
-            if (is_out) { float jv = base[(size_t)(2 * rows_kind + k) * wp0 + j]; a -= jv; b -= jv; }
-            const float sa = (a > 0.f) - (a < 0.f), sbn = (b > 0.f) - (b < 0.f);
-            const float lu = yu * (sa * s + m), ll = yl * (m - sbn * s);
-            obase[(size_t)k * wp0 + j] = lu;
-            obase[(size_t)(rows_kind + k) * wp0 + j] = ll;
-            if (is_out) obase[(size_t)(2 * rows_kind + k) * wp0 + j] = -(lu + ll);
-            sb += yu * fabsf(a) - yl * fabsf(b);
-            mb += yu * a + yl * b;
+            for (int k = k0 + rq; k < k1; k += 4) {
+                const float yu = ybar_up[(size_t)t * ldy + k], yl = ybar_lo[(size_t)t * ldy + k];
+                float4 a = *reinterpret_cast<const float4*>(base + (size_t)k * wp0 + j);
+                float4 b = *reinterpret_cast<const float4*>(base + (size_t)(rows_kind + k) * wp0 + j);
+                if (is_out) {
+                    const float4 jv = *reinterpret_cast<const float4*>(base + (size_t)(2 * rows_kind + k) * wp0 + j);
+                    a.x -= jv.x; a.y -= jv.y; a.z -= jv.z; a.w -= jv.w;
+                    b.x -= jv.x; b.y -= jv.y; b.z -= jv.z; b.w -= jv.w;
+                }
+                const float4 lu = make_float4(yu * (sgn(a.x) * s.x + m.x), yu * (sgn(a.y) * s.y + m.y), yu * (sgn(a.z) * s.z + m.z),
+                                              yu * (sgn(a.w) * s.w + m.w));
+                const float4 ll = make_float4(yl * (m.x - sgn(b.x) * s.x), yl * (m.y - sgn(b.y) * s.y), yl * (m.z - sgn(b.z) * s.z),
+                                              yl * (m.w - sgn(b.w) * s.w));
+                *reinterpret_cast<float4*>(obase + (size_t)k * wp0 + j) = lu;
+                *reinterpret_cast<float4*>(obase + (size_t)(rows_kind + k) * wp0 + j) = ll;
+                if (is_out)
+                    *reinterpret_cast<float4*>(obase + (size_t)(2 * rows_kind + k) * wp0 + j) =
+                        make_float4(-(lu.x + ll.x), -(lu.y + ll.y), -(lu.z + ll.z), -(lu.w + ll.w));
+                sb.x += yu * fabsf(a.x) - yl * fabsf(b.x); sb.y += yu * fabsf(a.y) - yl * fabsf(b.y);
+                sb.z += yu * fabsf(a.z) - yl * fabsf(b.z); sb.w += yu * fabsf(a.w) - yl * fabsf(b.w);
+                if (MU) {
+                    mb.x += yu * a.x + yl * b.x; mb.y += yu * a.y + yl * b.y;
+                    mb.z += yu * a.z + yl * b.z; mb.w += yu * a.w + yl * b.w;
+                }
+            }
         }
-        atomicAdd(&rad_bar[(size_t)t * wp0 + j], sb);
-        if (mu_bar) atomicAdd(&mu_bar[(size_t)t * wp0 + j], mb);
+        __syncthreads();
+        if (rq > 0) { red_s[rq - 1][lane64] = sb; if (MU) red_m[rq - 1][lane64] = mb; }
+        __syncthreads();
+        if (rq == 0 && on) {
+            for (int q = 0; q < 3; ++q) {
+                const float4 v = red_s[q][lane64];
+                sb.x += v.x; sb.y += v.y; sb.z += v.z; sb.w += v.w;
+                if (MU) { const float4 u = red_m[q][lane64]; mb.x += u.x; mb.y += u.y; mb.z += u.z; mb.w += u.w; }
+            }
+            float* rb = rad_bar + (size_t)t * wp0 + j;
+            atomicAdd(rb, sb.x); atomicAdd(rb + 1, sb.y); atomicAdd(rb + 2, sb.z); atomicAdd(rb + 3, sb.w);
+            if (MU && mu_bar) {
+                float* mp = mu_bar + (size_t)t * wp0 + j;
+                atomicAdd(mp, mb.x); atomicAdd(mp + 1, mb.y); atomicAdd(mp + 2, mb.z); atomicAdd(mp + 3, mb.w);
+            }
+        }
     }
 }
 
@@ -1336,8 +1372,12 @@ leb_status leb_nn_vjp(NnState* S, int tiles, const float* nom, const float* rad,
             }
             const float* yu = is_out ? S->ghi_p : S->ubar[s];
             const float* yl = is_out ? S->glo_p : S->lbar[s];
-            seed_kernel<<<dim3(C, (rk + 31) / 32), 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
-                                           S->Lbar[0], S->gapbar, S->rad_bar, S->mu_cur, mu ? S->mu_bar : nullptr);
+            if (S->mu_cur)
+                seed_kernel<true><<<dim3(C, (rk + 31) / 32), 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
+                                                                       S->Lbar[0], S->gapbar, S->rad_bar, S->mu_cur, mu ? S->mu_bar : nullptr);
+            else
+                seed_kernel<false><<<dim3(C, (rk + 31) / 32), 256, 0, st>>>(is_out ? 1 : 0, rp, rk, wp0, S->Lam[s][0], S->radp, yu, yl, is_out ? n : S->wp[s],
+                                                                        S->Lbar[0], S->gapbar, S->rad_bar, nullptr, nullptr);
             ++*launches;
             int cur = 0;
             for (int l = 1; l <= s - 1; ++l) {
