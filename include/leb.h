@@ -54,7 +54,8 @@ typedef enum {
     LEB_ERR_UNSUPPORTED = 5, /* unknown model; certified mode with layers wider than 2048 */
     LEB_ERR_CUDA = 6,
     LEB_ERR_NOMEM = 7,
-    LEB_ERR_STATE = 8        /* model not set before the call that needs it */
+    LEB_ERR_STATE = 8,       /* model not set before the call that needs it */
+    LEB_ERR_CAPACITY = 9     /* problem larger than a fixed-capacity entry point holds (leb_jerr_static: B * T > LEB_JERR_STATIC_MAX) */
 } leb_status;
 
 typedef enum { LEB_MODEL_UNICYCLE = 1, LEB_MODEL_QUAD12 = 2, LEB_MODEL_QUADCHAIN = 3, LEB_MODEL_PLANAR_QUAD = 4,
@@ -270,6 +271,20 @@ leb_status leb_tube_propagate(leb_ctx* ctx, int B, int T, int n, int m, const fl
  *   J_err : [B].   n > 1024: LEB_ERR_UNSUPPORTED. */
 leb_status leb_jerr(leb_ctx* ctx, int B, int T, int n, int m, const float* Phi, const float* R_diag,
                     const float* E_diag, float* J_err, float* grad_R, unsigned flags, void* stream);
+
+/* leb_jerr for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same operation, same kernels, same results, but the per-(b, j) partial sums go to a static device array
+ * of LEB_JERR_STATIC_MAX floats (256 KB, held by every GPU that loads the library until the process exits) instead of a
+ * buffer from cudaMalloc.  The call makes no cudaMalloc / cudaFree / allocating library call and records no event.
+ *   - device pointers only: LEB_FLAG_HOST_IO => LEB_ERR_ARG (host staging would have to allocate);
+ *   - B * T > LEB_JERR_STATIC_MAX => LEB_ERR_CAPACITY, nothing is launched;
+ *   - the array is shared by every call on the device and keeps the last call's contents (nothing in it has to start at
+ *     zero: each call writes every entry it reads); calls that overlap on the GPU -- two streams, two contexts on one
+ *     device -- RACE on it: serialise them (one stream, or an event between them).
+ * Other arguments and errors as leb_jerr. */
+#define LEB_JERR_STATIC_MAX 65536
+leb_status leb_jerr_static(leb_ctx* ctx, int B, int T, int n, int m, const float* Phi, const float* R_diag,
+                           const float* E_diag, float* J_err, float* grad_R, unsigned flags, void* stream);
 
 /* *flag = 1 if any tile of any call since the last leb_domain_flag() hit a domain error
  * (synchronises `stream`, then clears the flag). */

@@ -78,6 +78,7 @@ const char* leb_status_str(leb_status s) {
         case LEB_ERR_CUDA: return "CUDA error";
         case LEB_ERR_NOMEM: return "out of device memory";
         case LEB_ERR_STATE: return "model not set";
+        case LEB_ERR_CAPACITY: return "problem larger than the fixed capacity of this entry point";
     }
     return "unknown";
 }
@@ -95,6 +96,7 @@ leb_status leb_create(leb_ctx** out, int device) {
     cudaMemset(c->domain_flag, 0, sizeof(int));
     c->nn = leb_nn_create();
     c->an = leb_an_create();
+    (void)leb_jerr_static_setup(device);      // static scratch of leb_jerr_static; a failure is reported by that entry point
     if (!c->nn || !c->an) { leb_nn_destroy(c->nn); leb_an_destroy(c->an); cudaFree(c->domain_flag); delete c; return LEB_ERR_NOMEM; }
     *out = c;
     return LEB_OK;
@@ -487,6 +489,21 @@ leb_status leb_jerr(leb_ctx* c, int B, int T, int n, int m, const float* Phi, co
     out_copy(J_err, d_J, (size_t)B, host, st, &ok);
     out_copy(grad_R, d_g, nv, host, st, &ok);
     return ok ? LEB_OK : LEB_ERR_CUDA;
+}
+
+leb_status leb_jerr_static(leb_ctx* c, int B, int T, int n, int m, const float* Phi, const float* R_diag, const float* E_diag,
+                           float* J_err, float* grad_R, unsigned flags, void* stream) {
+    if (!c || B < 0 || T < 0 || n < 1 || m < 0) return LEB_ERR_ARG;
+    if (flags & LEB_FLAG_HOST_IO) return LEB_ERR_ARG;                 // staging host buffers would allocate
+    if (n > 1024) return LEB_ERR_UNSUPPORTED;
+    if (T > 65535 || B > 65535) return LEB_ERR_SHAPE;
+    if ((long long)B * T > (long long)LEB_JERR_STATIC_MAX) return LEB_ERR_CAPACITY;
+    if (B == 0 || T == 0) return LEB_OK;
+    if (!Phi || !R_diag || !J_err) return LEB_ERR_ARG;
+    if (!al4(Phi) || !al4(R_diag) || !al4(E_diag) || !al4(J_err) || !al4(grad_R)) return LEB_ERR_ALIGN;
+    DeviceGuard guard(c->device);
+    const cudaError_t e = leb_launch_jerr_static(c->device, B, T, n, n + m, Phi, R_diag, E_diag, J_err, grad_R, (cudaStream_t)stream, &c->launches);
+    return e == cudaSuccess ? LEB_OK : LEB_ERR_CUDA;
 }
 
 leb_status leb_domain_flag(leb_ctx* c, int* flag, void* stream) {

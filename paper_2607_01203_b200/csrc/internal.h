@@ -94,6 +94,9 @@ cudaError_t leb_launch_tube(int B, int T, int n, int N, const float* Phi, const 
                             LebProf* prof);
 cudaError_t leb_launch_jerr(int B, int T, int n, int N, const float* Phi, const float* R_diag, const float* E_diag,
                             float* partial, float* J, float* grad_R, cudaStream_t st, long long* launches, LebProf* prof);
+cudaError_t leb_jerr_static_setup(int device);      // tube.cu: resolves the static scratch on the current device
+cudaError_t leb_launch_jerr_static(int device, int B, int T, int n, int N, const float* Phi, const float* R_diag, const float* E_diag,
+                                   float* J, float* grad_R, cudaStream_t st, long long* launches);
 
 // ---- NN path (nn.cu)
 struct NnState;   // packed weights + workspace, owned by the context

@@ -9,6 +9,7 @@
 // one config-5 batch are 48 GB).  Phi is stored packed, block p(k, j) = (k-1) k / 2 + j of [T (T+1) / 2, N, n] per
 // trajectory, 0 <= j < k <= T.  Widths are accumulated with every operation rounded up (they are bounds).
 #include <algorithm>
+#include <mutex>
 #include "internal.h"
 
 namespace {
@@ -237,6 +238,50 @@ cudaError_t leb_launch_jerr(int B, int T, int n, int N, const float* Phi, const 
     if (vec) jerr_kernel<true><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
     else jerr_kernel<false><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
     prof->end(LEB_KC_TUBE, st, 4.0 * ((double)B * T * (T + 1) / 2 * N * n + 2.0 * B * T * n));
+    jerr_finish_kernel<<<(B + 7) / 8, 256, 0, st>>>(B, T, partial, J);
+    *launches += 2;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------- leb_jerr_static: (35) with no allocation anywhere
+// The per-(b, j) partial sums of jerr_kernel -- the one scratch buffer leb_jerr takes from cudaMalloc -- live in a
+// file-scope device array instead: LEB_JERR_STATIC_MAX floats (256 KB), held by every GPU that loads the library until the
+// process exits.  In host code the name g_jerr_partial is only a stand-in for the symbol, not a device address: the
+// address is resolved once per device, at set-up (leb_create), with that device current, and that pointer is what the
+// kernels are given.  Nothing in the array has to start at zero -- jerr_kernel writes every entry (b, j) that
+// jerr_finish_kernel reads, in the same call -- and it keeps the last call's contents; all calls on a device share it, so
+// two calls that overlap on the GPU (different streams) race.
+static __device__ __align__(256) float g_jerr_partial[LEB_JERR_STATIC_MAX];
+
+namespace {
+constexpr int kMaxDevices = 64;
+float* g_jerr_partial_ptr[kMaxDevices] = {nullptr};
+std::mutex g_jerr_setup_mutex;
+}  // namespace
+
+// set-up: called by leb_create with `device` current
+cudaError_t leb_jerr_static_setup(int device) {
+    if (device < 0 || device >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_jerr_setup_mutex);
+    if (g_jerr_partial_ptr[device]) return cudaSuccess;
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_jerr_partial);
+    if (e != cudaSuccess) return e;
+    g_jerr_partial_ptr[device] = static_cast<float*>(p);
+    return cudaSuccess;
+}
+
+// the two launches of leb_launch_jerr on the static scratch: no allocation, no event, no profiling hook
+cudaError_t leb_launch_jerr_static(int device, int B, int T, int n, int N, const float* Phi, const float* R_diag, const float* E_diag,
+                                   float* J, float* grad_R, cudaStream_t st, long long* launches) {
+    if (B == 0 || T == 0) return cudaSuccess;
+    if (device < 0 || device >= kMaxDevices || !g_jerr_partial_ptr[device]) return cudaErrorNotReady;   // set-up did not run or failed
+    if ((long long)B * T > (long long)LEB_JERR_STATIC_MAX) return cudaErrorInvalidValue;
+    float* partial = g_jerr_partial_ptr[device];
+    const size_t smem = std::max<size_t>((size_t)kJerrWarps * 4 * ((n + 3) / 4), 32) * sizeof(float);
+    const bool vec = (n & 3) == 0 && ((size_t)Phi & 15) == 0;
+    if (vec) jerr_kernel<true><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
+    else jerr_kernel<false><<<dim3(T, B), kJerrWarps * 32, smem, st>>>(T, n, N, Phi, R_diag, E_diag, partial, grad_R);
     jerr_finish_kernel<<<(B + 7) / 8, 256, 0, st>>>(B, T, partial, J);
     *launches += 2;
     return cudaGetLastError();

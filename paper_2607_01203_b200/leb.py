@@ -16,8 +16,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libleb.so")
 
 LEB_OK = 0
+LEB_ERR_ARG = 1
 LEB_ERR_UNSUPPORTED = 5
 LEB_ERR_STATE = 8
+LEB_ERR_CAPACITY = 9
+JERR_STATIC_MAX = 65536
 FLAG_NO_MARGIN = 1
 FLAG_FFMA_ONLY = 2
 FLAG_HOST_IO = 4
@@ -27,7 +30,7 @@ FLAG_IBP_HIDDEN = 32
 
 EXPORTS = [
     "leb_create", "leb_destroy", "leb_status_str", "leb_set_analytic", "leb_set_mlp", "leb_set_nn_chunk",
-    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_partition_vjp", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr",
+    "leb_analytic_fwd", "leb_analytic_partition_fwd", "leb_analytic_partition_vjp", "leb_analytic_pgd", "leb_nn_fwd", "leb_nn_alpha_fwd", "leb_vjp", "leb_vjp_mu", "leb_zonotope_inflate", "leb_zonotope_inflate_vjp", "leb_dist_add", "leb_tube_propagate", "leb_jerr", "leb_jerr_static",
     "leb_domain_flag", "leb_nn_hidden_bounds", "leb_nn_chain_coeffs", "leb_nn_jacobian", "leb_nn_slopes", "leb_nn_state", "leb_analytic_tape_stats", "leb_launch_count", "leb_profile", "leb_profile_read",
     "leb_profile_reset",
 ]
@@ -325,6 +328,15 @@ class Context:
         _chk(self.lib.leb_jerr(self._ctx, B, T, n, int(m), _ptr(Phi), _ptr(R_diag), _ptr(E_diag), _ptr(J), _ptr(g),
                                ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_jerr")
         return J, g
+
+    def leb_jerr_static(self, Phi, R_diag, m: int, J, grad_R=None, E_diag=None, flags: int = 0):
+        """leb_jerr without any allocation (leb.h): the caller passes the outputs J [B] and grad_R [B, T, n] (or None) as
+        device tensors; B * T <= JERR_STATIC_MAX; calls that overlap on the GPU race on the library's static scratch."""
+        _check_f32(Phi, R_diag, E_diag, J, grad_R)
+        B, T, n = self._bt(R_diag)
+        _chk(self.lib.leb_jerr_static(self._ctx, B, T, n, int(m), _ptr(Phi), _ptr(R_diag), _ptr(E_diag), _ptr(J), _ptr(grad_R),
+                                      ctypes.c_uint(flags), _stream_ptr(self.device)), "leb_jerr_static")
+        return J, grad_R
 
     def leb_domain_flag(self) -> int:
         flag = ctypes.c_int(0)
