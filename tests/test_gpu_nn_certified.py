@@ -467,3 +467,35 @@ def test_certified_alpha_refinement(mods, path):
             r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None] - (X - a0[None]) @ Jt[t].T
             assert np.all(r.max(0) <= hi64[t]) and np.all(r.min(0) >= lo64[t]), (dims, t)
         ctx.close()
+
+
+def test_chunking_does_not_change_the_newer_variants(mods):
+    """A batch processed in chunks of 5 tiles (12 tiles: a ragged last chunk) gives the results of the one-chunk run, bit for
+    bit, for non-centred boxes (certified), certified CROWN-IBP with mu, and the slope refinement (certified)."""
+    leb, wl, O = mods
+    w = wl.make_small_mlp([6, 33, 20, 11, 5], 1, 3, 4, seed=3, rad_lo=0.05, rad_hi=0.3)
+    mu = _dev(wl.make_mu(w, 1.0))
+    nom, rad = _dev(w.nom), _dev(w.rad)
+    ctx = leb.context_for_workload(w)
+    IBP = leb.FLAG_IBP_HIDDEN
+
+    def run():
+        a = ctx.leb_nn_fwd(nom, rad, mu=mu)
+        b = ctx.leb_nn_fwd(nom, rad, mu=mu, flags=IBP)
+        c = ctx.leb_nn_alpha_fwd(nom, rad, 4, 0.05)
+        d = ctx.leb_vjp_mu(1, nom, rad, mu, _dev(w.g_lo), _dev(w.g_hi), flags=IBP)
+        return [x.clone() for x in (*a, *b, *c)], [x.clone() for x in d]
+
+    full, gfull = run()
+    ctx.leb_set_nn_chunk(5)
+    part, gpart = run()
+    # several chunks: no complete state is resident, so nothing can be reused
+    ctx.leb_nn_alpha_fwd(nom, rad, 2, 0.05)
+    ctx.leb_vjp(1, nom, rad, _dev(w.g_lo), _dev(w.g_hi), flags=leb.FLAG_REUSE_FWD)
+    assert ctx.leb_nn_state()[2] is False
+    ctx.leb_set_nn_chunk(0)
+    for x, y in zip(full, part):
+        assert torch.equal(x, y)
+    for x, y in zip(gfull, gpart):                       # column sums are atomic adds: equal to rounding
+        assert float((x - y).abs().max()) <= 1e-5 * float(y.abs().max())
+    ctx.close()
