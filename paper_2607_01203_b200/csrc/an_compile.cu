@@ -445,7 +445,6 @@ void fuse_mul_add(std::vector<Ins>& ins, std::vector<uint32_t>& b, uint32_t tag,
 // Compile the model into a tape.  with_mu: non-centred boxes (25a) L272 (reading R4: prefix hull sets).
 void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
     const int n = M.n, N = M.N;
-    T->n = n; T->N = N; T->uses_mu = with_mu;
     *T = Tape();
     T->n = n; T->N = N; T->uses_mu = with_mu;
     auto& task_out = T->task_out;
@@ -464,8 +463,6 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
         }
     }
 
-    std::vector<std::vector<uint32_t>> out_rows(n), var_rows(N);
-    uint32_t acc_rows = 0, grad_rows = 0;
 
     for (int j = 0; j < N; ++j) {
         Builder B;
@@ -474,8 +471,6 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
         JV f(n);
         model_f(B, M, f);                       // pass WJ: memo filled
         Sym Dj = S(B.emit(with_mu ? OP_DELTAMU : OP_DELTA, (uint32_t)j, 0));
-        const size_t wj_len0 = B.wj_ins.size();
-        (void)wj_len0;
 
         std::vector<RawSeg> ksegs;
         std::vector<uint8_t> wj_live(B.wj_ins.size() + 64, 0), wj_kuse(B.wj_ins.size() + 64, 0);
@@ -625,8 +620,8 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
             for (uint32_t q = 0; q < task.seg_count; ++q) scan(T->segs[task.seg_begin + q].begin, T->segs[task.seg_begin + q].count, nwj);
         }
         task.n_slots = nwj + max_k;
-        task.acc_base = acc_rows; task.n_acc = (uint32_t)n_acc;
-        task.grad_base = grad_rows; task.n_grad = (uint32_t)n_grad;
+        task.acc_base = 0; task.n_acc = (uint32_t)n_acc;          // row bases are assigned per task set (leb_build_taskset)
+        task.grad_base = 0; task.n_grad = (uint32_t)n_grad;
         task.cost = (uint32_t)std::min<uint64_t>(cost, 0xffffffffu);
         {   // which output / input each of this task's rows belongs to (for the reduction tables)
             std::vector<uint32_t> to(n_acc), tv(n_grad);
@@ -642,7 +637,6 @@ void leb_compile_tape(const Model& M, bool with_mu, Tape* T) {
         T->base.push_back(task);
         T->ins_fwd += cost;
     }
-    (void)acc_rows; (void)grad_rows; (void)out_rows; (void)var_rows;
 }
 
 void leb_build_taskset(const Tape& T, uint32_t target, TaskSet* set) {
