@@ -45,24 +45,51 @@ __device__ inline Relax relax_relu(double l, double u) {
 // tangent point of the upper line through (l, tanh l), l < 0 < u: root of
 // h(d) = t'(d)(d - l) - (t(d) - t(l)) on (0, u); h > 0 left of the root.  Returns the bracket end
 // d >= d*, the side on which the tangent stays above tanh on [l, u] (sound side).
+// The bracket [a, b] keeps h(a) > 0 >= h(b) as in a bisection -- whatever is returned was evaluated with h <= 0 -- but the
+// points are chosen better: the first is -l / 2 (the exact tangent point for the cubic z - z^3 / 3, which tanh is near 0:
+// without it the iteration from u only converges linearly while |l| << d), then Newton steps from b
+// (h'(d) = t''(d)(d - l)), shortened by 2^-20 so that near the root they stay on that side; a step that leaves the bracket
+// is replaced by the secant point, then by the midpoint.  Ends when b no longer moves by 2^-48 of itself: 7 evaluations of
+// tanh on average and 12 at the 99th percentile instead of 52 -- every lane of a warp waits for the slowest, and at
+// config 5 nearly every warp holds a mixed-sign neuron.  kBisect bounds the loop.
+__device__ __forceinline__ void tangent_h(double m, double l, double tl, double& h, double& dh) {
+    const double t = tanh(m), s = 1.0 - t * t;
+    h = s * (m - l) - (t - tl);
+    dh = -2.0 * t * s * (m - l);
+}
 __device__ inline double tangent_upper(double l, double u) {
-    double tl = th(l), a = 0.0, b = u;
+    constexpr double kShort = 0.99999904632568359375, kTol = 3.5527136788005009e-15;      // 1 - 2^-20, 2^-48
+    const double tl = th(l);
+    double a = 0.0, ha = tl - l;                 // h(0) = tanh(l) - l > 0
+    double b = u, hb, db;
+    tangent_h(b, l, tl, hb, db);
+    const double g = -0.5 * l;
+    if (g < b) {
+        double hg, dg;
+        tangent_h(g, l, tl, hg, dg);
+        if (hg > 0.0) { a = g; ha = hg; } else { b = g; hb = hg; db = dg; }
+    }
     for (int it = 0; it < kBisect; ++it) {
-        double m = 0.5 * (a + b), t = tanh(m);
-        if ((1.0 - t * t) * (m - l) - (t - tl) > 0.0) a = m; else b = m;
+        if (!(b - a > kTol * b)) break;
+        const double step = (hb / db) * kShort;
+        if (!(step > kTol * b)) break;
+        double m = b - step;
+        if (!(m > a)) {
+            m = a + (b - a) * (ha / (ha - hb));
+            if (!(m > a && m < b)) {
+                m = 0.5 * (a + b);
+                if (!(m > a && m < b)) break;
+            }
+        }
+        double hm, dm;
+        tangent_h(m, l, tl, hm, dm);
+        if (hm > 0.0) { a = m; ha = hm; } else { b = m; hb = hm; db = dm; }
     }
     return b;
 }
-// tangent point of the lower line through (u, tanh u): root of h(d) = t'(d)(u - d) - (t(u) - t(d))
-// on (l, 0); h > 0 right of the root.  Returns the end d <= d* (sound side).
-__device__ inline double tangent_lower(double l, double u) {
-    double tu = th(u), a = l, b = 0.0;
-    for (int it = 0; it < kBisect; ++it) {
-        double m = 0.5 * (a + b), t = tanh(m);
-        if ((1.0 - t * t) * (u - m) - (tu - t) > 0.0) b = m; else a = m;
-    }
-    return a;
-}
+// tangent point of the lower line through (u, tanh u), in (l, 0): the mirror image (tanh is odd).  Returns the end
+// d <= d* (sound side).
+__device__ inline double tangent_lower(double l, double u) { return -tangent_upper(-u, -l); }
 
 __device__ inline Relax relax_tanh(double l, double u) {
     Relax r{};
