@@ -499,3 +499,34 @@ def test_chunking_does_not_change_the_newer_variants(mods):
     for x, y in zip(gfull, gpart):                       # column sums are atomic adds: equal to rounding
         assert float((x - y).abs().max()) <= 1e-5 * float(y.abs().max())
     ctx.close()
+
+
+def test_certified_mu_config5_width_sampled_soundness(mods):
+    """Config 5 at full width (224 -> 512 x 4 -> 168, tanh), 4 tiles, offset boxes (|mu| <= 1.5 sigma), certified mode, both
+    hidden-bound variants: the sampled remainder (2e4 samples + 4 096 sampled vertices of the offset box, J~ read back)
+    inside the enclosure with no tolerance, and the enclosure contains the value-mode one."""
+    leb, wl, O = mods
+    w = wl.make_config(5, B=1, T=4)
+    mu = wl.make_mu(w, 1.5)
+    ctx = leb.context_for_workload(w)
+    Ws = [np.asarray(x, np.float64) for x in w.mlp.W]; bs = [np.asarray(x, np.float64) for x in w.mlp.b]
+    N = w.N
+    nom, rad, mu_f = w.nom.reshape(-1, N), w.rad.reshape(-1, N), mu.reshape(-1, N)
+    rng = np.random.default_rng(17)
+    for flags in (0, leb.FLAG_IBP_HIDDEN):
+        lo, hi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), mu=_dev(mu), flags=flags)
+        Jt = to_np(ctx.leb_nn_jacobian(w.B * w.T, w.n, N)).astype(np.float64)
+        vlo, vhi = ctx.leb_nn_fwd(_dev(w.nom), _dev(w.rad), mu=_dev(mu), flags=flags | leb.FLAG_NO_MARGIN)
+        assert ctx.leb_domain_flag() == 0
+        assert bool((hi >= vhi).all()) and bool((lo <= vlo).all())
+        clo, chi = to_np(lo).reshape(-1, w.n).astype(np.float64), to_np(hi).reshape(-1, w.n).astype(np.float64)
+        for t in range(w.B * w.T):
+            a0, sg, m = nom[t].astype(np.float64), rad[t].astype(np.float64), mu_f[t].astype(np.float64)
+            X = a0[None] + m[None] + np.concatenate([rng.uniform(-1, 1, (20000, N)), rng.choice([-1.0, 1.0], (4096, N))]) * sg[None]
+            _, p, _ = O.nominal(Ws, bs, w.mlp.act, a0)
+            A = X.T
+            for l in range(len(Ws) - 1):
+                A = O.phi(w.mlp.act, Ws[l] @ A + bs[l][:, None])
+            r = (Ws[-1] @ A + bs[-1][:, None]).T - p[None, :] - (X - a0[None, :]) @ Jt[t].T
+            assert np.all(r.max(0) <= chi[t]) and np.all(r.min(0) >= clo[t]), (flags, t)
+    ctx.close()

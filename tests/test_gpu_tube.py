@@ -249,3 +249,46 @@ def test_partition_vjp_matches_oracle(mods):
     for x, y in zip(a, b):
         assert torch.equal(x, y)
     ctx.close()
+
+
+@pytest.mark.gpu
+def test_tube_and_jerr_full_horizon_sampled(mods):
+    """The bench's shape (T = 100, n = 168, m = 56; one trajectory, 760 MB of responses drawn on the device as bench.py does):
+    sampled rows of h_mu / h_sigma and sampled (b, j) terms of J_err and its gradient against the definitions written out
+    in FP64 on the same responses (the oracle's loops on full blocks would take minutes; a row is one pass over its blocks)."""
+    leb, _, _, _, TU = mods
+    B, T, n, m = 1, 100, 168, 56
+    N = n + m
+    g = torch.Generator(device="cuda")
+    g.manual_seed(7)
+    nb = T * (T + 1) // 2
+    Phi = torch.randn((B, nb, N, n), device="cuda", generator=g) / n ** 0.5
+    for j in range(T):
+        Phi[:, (j + 1) * j // 2 + j, :n] = torch.eye(n, device="cuda")
+    c = torch.randn((B, T, n), device="cuda", generator=g) * 0.05
+    Rd = torch.rand((B, T, n), device="cuda", generator=g) * 0.1 + 1e-3
+    E = torch.rand((n,), device="cuda", generator=g) * 0.05
+    ctx = leb.Context(0)
+    h_mu, h_sg = ctx.leb_tube_propagate(Phi, c, Rd, m, E)
+    J, gR = ctx.leb_jerr(Phi, Rd, m, E)
+    P64 = Phi[0].double().cpu().numpy()
+    c64, R64, E64 = c[0].double().cpu().numpy(), Rd[0].double().cpu().numpy(), E.double().cpu().numpy()
+    for k in (1, 2, 37, 100):                               # time k: blocks (k, j), j < k
+        blocks = np.stack([P64[TU.block(k, j)] for j in range(k)])              # [k, N, n]
+        omu = np.einsum("jin,jn->i", blocks, c64[:k])
+        osg = np.einsum("jin,jn->i", np.abs(blocks), np.abs(E64)[None] + R64[:k])
+        gmu, gsg = to_np(h_mu)[0, k - 1], to_np(h_sg)[0, k - 1]
+        assert np.all(np.abs(gmu - omu) <= 1e-5 * np.abs(omu) + 2e-6 * np.abs(omu).max())
+        assert_bounds_close(gsg, osg, f"h_sigma full horizon k={k}")
+        assert np.all(gsg >= osg * (1 - 1e-12))
+    tot = 0.0
+    og = np.zeros((T, n))
+    for j in range(T):
+        S = np.zeros(n)
+        for k in range(j + 1, T + 1):
+            S += (P64[TU.block(k, j)] ** 2).sum(0)
+        tot += ((E64 ** 2 + R64[j] ** 2) * S).sum()
+        og[j] = 2.0 * R64[j] * S
+    assert abs(float(J[0]) - tot) <= 1e-5 * tot
+    assert np.all(np.abs(to_np(gR)[0] - og) <= 1e-5 * np.abs(og) + 1e-7 * np.abs(og).max())
+    ctx.close()
