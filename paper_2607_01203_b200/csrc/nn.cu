@@ -582,8 +582,8 @@ __global__ void relax_vjp_kernel(int act, int tiles, int w_valid, int wp, const 
         // g = k zhat + b - phi(zhat):  k_bar_eff = k_bar + zhat g_bar,  b_bar = g_bar
         double kbu = (double)kUb[q] + z * gu, kbl = (double)kLb[q] + z * gl;
         double lo = 0.0, up = 0.0;
-        line_vjp(act, r.cU, true, l, u, r.dU, kbu, gu, lo, up);
-        line_vjp(act, r.cL, false, l, u, r.dL, kbl, gl, lo, up);
+        line_vjp(act, r.cU, true, l, u, r.dU, kbu, gu, lo, up, r.tl, r.tu);
+        line_vjp(act, r.cL, false, l, u, r.dL, kbl, gl, lo, up, r.tl, r.tu);
         double d1 = act_d1(act, z);
         double zb = (r.kU - d1) * gu + (r.kL - d1) * gl + act_d2(act, z) * (double)dpb[q];
         // l_s = zhat_s - ..., u_s = zhat_s + ...: both pass their adjoint straight to zhat_s

@@ -22,6 +22,7 @@ struct Relax {
     double kU, bU, kL, bL;
     int cU, cL;        // LINE_* of the upper / lower line
     double dU, dL;     // tangent points where applicable
+    double tl, tu;     // tanh(l), tanh(u) (tanh only; the VJP reuses them instead of evaluating tanh again)
 };
 
 __device__ __forceinline__ double th(double x) { return tanh(x); }
@@ -57,9 +58,8 @@ __device__ __forceinline__ void tangent_h(double m, double l, double tl, double&
     h = s * (m - l) - (t - tl);
     dh = -2.0 * t * s * (m - l);
 }
-__device__ inline double tangent_upper(double l, double u) {
+__device__ inline double tangent_upper(double l, double u, double tl) {
     constexpr double kShort = 0.99999904632568359375, kTol = 3.5527136788005009e-15;      // 1 - 2^-20, 2^-48
-    const double tl = th(l);
     double a = 0.0, ha = tl - l;                 // h(0) = tanh(l) - l > 0
     double b = u, hb, db;
     tangent_h(b, l, tl, hb, db);
@@ -89,7 +89,7 @@ __device__ inline double tangent_upper(double l, double u) {
 }
 // tangent point of the lower line through (u, tanh u), in (l, 0): the mirror image (tanh is odd).  Returns the end
 // d <= d* (sound side).
-__device__ inline double tangent_lower(double l, double u) { return -tangent_upper(-u, -l); }
+__device__ inline double tangent_lower(double l, double u, double tu) { return -tangent_upper(-u, -l, -tu); }
 
 __device__ inline Relax relax_tanh(double l, double u) {
     Relax r{};
@@ -100,6 +100,7 @@ __device__ inline Relax relax_tanh(double l, double u) {
         return r;
     }
     double tl = th(l), tu = th(u);
+    r.tl = tl; r.tu = tu;
     double kc = (tu - tl) / w, bc = tl - kc * l;
     if (l >= 0.0) {                  // concave part: tangent above, chord below
         double d = 0.5 * (l + u), k = th1(d);
@@ -114,9 +115,9 @@ __device__ inline Relax relax_tanh(double l, double u) {
         return r;
     }
     if (kc <= 1.0 - tu * tu) { r.kU = kc; r.bU = bc; r.cU = LINE_CHORD; }
-    else { double d = tangent_upper(l, u), k = th1(d); r.kU = k; r.bU = th(d) - k * d; r.cU = LINE_TAN_IMPL; r.dU = d; }
+    else { double d = tangent_upper(l, u, tl), k = th1(d); r.kU = k; r.bU = th(d) - k * d; r.cU = LINE_TAN_IMPL; r.dU = d; }
     if (kc <= 1.0 - tl * tl) { r.kL = kc; r.bL = bc; r.cL = LINE_CHORD; }
-    else { double d = tangent_lower(l, u), k = th1(d); r.kL = k; r.bL = th(d) - k * d; r.cL = LINE_TAN_IMPL; r.dL = d; }
+    else { double d = tangent_lower(l, u, tu), k = th1(d); r.kL = k; r.bL = th(d) - k * d; r.cL = LINE_TAN_IMPL; r.dL = d; }
     return r;
 }
 
@@ -127,8 +128,9 @@ __device__ __forceinline__ double act_d1(int act, double z) { return act == ACT_
 __device__ __forceinline__ double act_d2(int act, double z) { return act == ACT_RELU ? 0.0 : th2(z); }
 
 // Adjoint of one line's (k, b) with respect to (l, u):  (lb, ub) += d(k,b)/d(l,u)^T (kb, bb).
+// tl, tu = tanh(l), tanh(u) as relax_tanh computed them (Relax::tl, tu).
 __device__ inline void line_vjp(int act, int how, bool upper, double l, double u, double d, double kb, double bb,
-                                double& lb, double& ub) {
+                                double& lb, double& ub, double tl, double tu) {
     switch (how) {
         case LINE_CHORD: {
             double w = u - l;
@@ -137,9 +139,10 @@ __device__ inline void line_vjp(int act, int how, bool upper, double l, double u
                 lb += kb * (u / w2) + bb * (-u * u / w2);
                 ub += kb * (-l / w2) + bb * (l * l / w2);
             } else {                    // k = (t(u)-t(l))/(u-l), b = t(l) - k l
-                double k = (th(u) - th(l)) / w;
-                double dk_du = (th1(u) - k) / w, dk_dl = (k - th1(l)) / w;
-                double db_dl = th1(l) - k - l * dk_dl, db_du = -l * dk_du;
+                double k = (tu - tl) / w;
+                double t1l = 1.0 - tl * tl, t1u = 1.0 - tu * tu;
+                double dk_du = (t1u - k) / w, dk_dl = (k - t1l) / w;
+                double db_dl = t1l - k - l * dk_dl, db_du = -l * dk_du;
                 lb += kb * dk_dl + bb * db_dl;
                 ub += kb * dk_du + bb * db_du;
             }
@@ -152,9 +155,10 @@ __device__ inline void line_vjp(int act, int how, bool upper, double l, double u
             break;
         }
         case LINE_TAN_IMPL: {           // tangent point defined implicitly by l (upper) or by u (lower)
-            double ad = th2(d) * (kb - d * bb);
-            if (upper) lb += ad * (th1(d) - th1(l)) / (th2(d) * (d - l));
-            else ub += ad * (th1(u) - th1(d)) / (th2(d) * (u - d));
+            const double td = tanh(d), t1d = 1.0 - td * td, t2d = -2.0 * td * t1d;
+            double ad = t2d * (kb - d * bb);
+            if (upper) lb += ad * (t1d - (1.0 - tl * tl)) / (t2d * (d - l));
+            else ub += ad * ((1.0 - tu * tu) - t1d) / (t2d * (u - d));
             break;
         }
         case LINE_DEGEN: {              // b = t(d) - k d +- c (u-l)^2, c = kTanhD2Max/2
