@@ -49,7 +49,7 @@ def test_jerr_static_matches_jerr_two_calls_in_a_row(leb):
         J.fill_(-7.0); g.fill_(-7.0)
         ctx.leb_jerr_static(Phi, R, m, J, g, E_diag=E)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free0                               # the device's free memory did not move
+    assert free0 - torch.cuda.mem_get_info()[0] < (2 << 20)                    # the device's free memory did not drop (2 MiB: the driver's granularity)
     for (J, g), (Jr, gr) in zip(outs, ref):
         assert _close(J, Jr) and _close(g, gr)
         assert torch.equal(J, Jr) and torch.equal(g, gr)                        # same kernels, same order: bit for bit
