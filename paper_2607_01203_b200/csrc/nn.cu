@@ -275,8 +275,11 @@ __global__ void __launch_bounds__(256) cert_layer_kernel(int C, int J, int K, co
                                                          const float* __restrict__ zhat, const float* __restrict__ ahat, int act,
                                                          int out_only, float* __restrict__ e, float* __restrict__ t,
                                                          float* __restrict__ v, int ldo) {
+    // weights and centres are converted to FP64 once per block load (a conversion per use made the kernel conversion-bound)
     __shared__ __align__(16) float Ws[CK][CJ];
-    __shared__ float Xs[CM][CK], Ts[CM][CK], As[CM][CK];
+    __shared__ __align__(16) double Wd[CK][CJ];
+    __shared__ float Ts[CM][CK], As[CM][CK];
+    __shared__ double Xd[CM][CK];
     const int tid = threadIdx.x, tj = tid & 15, tm = tid >> 4;
     const int m0 = blockIdx.y * CM, j0 = blockIdx.x * CJ;
     double s[4] = {0.0, 0.0, 0.0, 0.0}, sa[4] = {0.0, 0.0, 0.0, 0.0};
@@ -285,32 +288,36 @@ __global__ void __launch_bounds__(256) cert_layer_kernel(int C, int J, int K, co
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const int idx = tid + i * 256, kk = idx >> 6, jj = idx & 63;
-            Ws[kk][jj] = (k0 + kk < K && j0 + jj < J) ? Wt[(size_t)(k0 + kk) * ldw + j0 + jj] : 0.f;
+            const float wv = (k0 + kk < K && j0 + jj < J) ? Wt[(size_t)(k0 + kk) * ldw + j0 + jj] : 0.f;
+            Ws[kk][jj] = fabsf(wv);
+            Wd[kk][jj] = (double)wv;
         }
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int idx = tid + i * 256, mm = idx >> 5, kk = idx & 31;
             const bool ok = (m0 + mm < C) && (k0 + kk < K);
             const size_t o = (size_t)(m0 + mm) * ldx + k0 + kk;
-            Xs[mm][kk] = (ok && X) ? X[o] : 0.f;
+            Xd[mm][kk] = (ok && X) ? (double)X[o] : 0.0;
             Ts[mm][kk] = (ok && T) ? T[o] : 0.f;
             As[mm][kk] = (ok && A) ? A[o] : 0.f;
         }
         __syncthreads();
 #pragma unroll 4
         for (int kk = 0; kk < CK; ++kk) {
-            const float4 w4 = *reinterpret_cast<const float4*>(&Ws[kk][tj * 4]);
-            const float w[4] = {w4.x, w4.y, w4.z, w4.w};
-            const float x = Xs[tm][kk], tt = Ts[tm][kk], a = As[tm][kk];
+            const float4 w4 = *reinterpret_cast<const float4*>(&Ws[kk][tj * 4]);                 // |W|
+            const float wabs[4] = {w4.x, w4.y, w4.z, w4.w};
+            const double2 d01 = *reinterpret_cast<const double2*>(&Wd[kk][tj * 4]), d23 = *reinterpret_cast<const double2*>(&Wd[kk][tj * 4 + 2]);
+            const double wd[4] = {d01.x, d01.y, d23.x, d23.y};
+            const double x = Xd[tm][kk], xa = fabs(x);
+            const float tt = Ts[tm][kk], a = As[tm][kk];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const float wa = fabsf(w[c]);
                 if (!out_only) {
-                    s[c] = fma((double)w[c], (double)x, s[c]);
-                    sa[c] = fma((double)wa, fabs((double)x), sa[c]);
-                    vv[c] = __fmaf_ru(wa, a, vv[c]);
+                    s[c] = fma(wd[c], x, s[c]);
+                    sa[c] = fma(fabs(wd[c]), xa, sa[c]);
+                    vv[c] = __fmaf_ru(wabs[c], a, vv[c]);
                 }
-                zt[c] = __fmaf_ru(wa, tt, zt[c]);
+                zt[c] = __fmaf_ru(wabs[c], tt, zt[c]);
             }
         }
         __syncthreads();
